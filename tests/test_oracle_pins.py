@@ -1,0 +1,302 @@
+"""Pins for the CPU oracle (oracle/): checks against what the paper and the mathematics fix, never against itself.
+
+Each test names the plausible mistake it would catch.  All CPU-only.
+"""
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_30728_b200 import datagen, workloads
+
+GOLDEN = Path(__file__).parent / "golden"
+
+
+def _fixture(name):
+    out = {}
+    for line in (GOLDEN / name).read_text().splitlines():
+        if line.startswith("#") or "=" not in line:
+            continue
+        k, v = line.split("=", 1)
+        out[k.strip()] = v.split()
+    return out
+
+
+def _hex(tokens):
+    return [np.frombuffer(bytes.fromhex(t), dtype=np.uint8) for t in tokens]
+
+
+def _bits(a):
+    return np.unpackbits(np.ascontiguousarray(a, np.uint8), axis=-1, bitorder="little")
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# hand-worked fixtures
+# ---------------------------------------------------------------------------------------------------------------------
+def test_golden_strict_worked_example():
+    """PAPER.md:229-231 with T=N; a swapped Mask/Bitval, a wrong bit order or MSB-first packing fails here."""
+    fx = _fixture("worked_example_strict.txt")
+    rows = np.stack(_hex(fx["rows"]))
+    mask, bitval, k, counters = oracle.group_masks(rows, return_counters=True)
+    assert counters.tolist() == [int(c) for c in fx["counters"]]
+    assert mask.tobytes().hex().upper() == fx["mask"][0]
+    assert bitval.tobytes().hex().upper() == fx["bitval"][0]
+    assert k == int(fx["k_bits"][0])
+    for r, want in zip(rows, fx["packed"]):
+        p, kk = oracle.pack_row(r, mask)
+        assert kk == k and p.tobytes().hex().upper() == want
+        assert np.array_equal(oracle.unpack_row(p, mask, bitval), r)
+
+
+def test_golden_thresholded_worked_example():
+    """PAPER.md:231 (>=T / <=N-T, reading R2), :237, :262-271; catches strict '>' comparisons, a missing
+    participation-bit charge and a wrong raw fallback."""
+    fx = _fixture("worked_example_thresholded.txt")
+    rows = np.stack(_hex(fx["rows"]))
+    T, cs = int(fx["threshold"][0]), int(fx["chunk_bytes"][0])
+    mask, bitval, _ = oracle.group_masks(rows, T=T)
+    assert mask.tobytes().hex().upper() == fx["mask"][0]
+    assert bitval.tobytes().hex().upper() == fx["bitval"][0]
+    for r, flag, want in zip(rows, fx["compressed"], fx["stored"]):
+        data, comp = oracle.compress_row_T(r, mask, bitval, cs)
+        assert comp == bool(int(flag))
+        assert data.tobytes().hex().upper() == want
+        assert np.array_equal(oracle.decompress_row_T(data, comp, mask, bitval, cs), r)
+
+
+def test_golden_thresholded_mixed_chunks():
+    """A compressed tensor holding a non-participating chunk: payload order and widths."""
+    fx = _fixture("worked_example_mixed_chunks.txt")
+    mask, bitval, row = _hex(fx["mask"])[0], _hex(fx["bitval"])[0], _hex(fx["row"])[0]
+    data, comp = oracle.compress_row_T(row, mask, bitval, int(fx["chunk_bytes"][0]))
+    assert comp and data.tobytes().hex().upper() == fx["stored"][0]
+    assert np.array_equal(oracle.decompress_row_T(data, comp, mask, bitval, 1), row)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Mask / Bitval
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,rb,seed", [(1, 4, 1), (2, 8, 2), (5, 12, 3), (17, 16, 4), (64, 32, 5)])
+def test_masks_brute_force_tiny_groups(n, rb, seed):
+    """Brute force over all rows, bit by bit, in Python (BASELINE.json north_star): a bit is invariant iff the set of
+    values it takes over the group has one element."""
+    rng = np.random.default_rng(seed)
+    # low-entropy rows so that some bits really are invariant
+    rows = (rng.integers(0, 256, (n, rb), dtype=np.uint8) & rng.integers(0, 256, (1, rb), dtype=np.uint8)) | \
+        rng.integers(0, 256, (1, rb), dtype=np.uint8) & np.uint8(0x11)
+    mask, bitval, k = oracle.group_masks(rows)
+    B = _bits(rows)
+    want_mask = np.zeros(8 * rb, np.uint8)
+    want_val = np.zeros(8 * rb, np.uint8)
+    for p in range(8 * rb):
+        seen = set(int(B[r, p]) for r in range(n))
+        if len(seen) == 1:
+            want_mask[p] = 1
+            want_val[p] = seen.pop()
+    assert np.array_equal(_bits(mask), want_mask)
+    assert np.array_equal(_bits(bitval), want_val)
+    assert k == 8 * rb - int(want_mask.sum())
+
+
+@pytest.mark.parametrize("name", ["tiny", "gnn_dense", "gnn_sparse", "dlrm", "kv", "weights"])
+def test_masks_closed_form_and_invariants(name):
+    """Independent closed form: Bitval = AND of rows, Mask = NOT(OR xor AND) (SURVEY 8(c) pins); and the paper's own
+    invariants: Chunk AND Mask == Bitval for every row, Bitval is 0 wherever Mask is 0."""
+    rows = _sample_group(name)
+    R = rows.view(np.uint8).reshape(rows.shape[0], -1)
+    mask, bitval, k = oracle.group_masks(R)
+    a = np.bitwise_and.reduce(R, axis=0)
+    o = np.bitwise_or.reduce(R, axis=0)
+    assert np.array_equal(bitval, a & ~(o ^ a))
+    assert np.array_equal(mask, ~(o ^ a))
+    assert np.all((R & mask) == bitval)
+    assert not np.any(bitval & ~mask)
+    assert k == 8 * R.shape[1] - int(_bits(mask).sum())
+
+
+def _sample_group(name):
+    if name == "tiny":
+        return workloads.Tiny().rows(128, 64)
+    if name == "gnn_dense":
+        return workloads.GNN(n_rows=10_000).rows(512, 256)
+    if name == "gnn_sparse":
+        return workloads.GNN(n_rows=10_000).rows(7168, 256)
+    if name == "dlrm":
+        return workloads.DLRM(rows_per_table=4096, n_tables=2).rows(4096 + 256, 128)
+    if name == "kv":
+        return workloads.KV(layers=1, pages=4).rows(16 * 5, 16)
+    if name == "weights":
+        w = workloads.WeightMatrix(256, 512)
+        return w.table()[3::4]                      # column tile 3 over all matrix rows
+    raise KeyError(name)
+
+
+def test_special_groups():
+    """Degenerate groups (readings R12, R13): one row / identical rows -> Mask all ones, k=0; a row and its complement
+    -> Mask all zeros, Bitval all zeros, k = all bits."""
+    rb = 24
+    r = datagen.random_bytes(rb, 11)
+    for rows in (r[None, :], np.repeat(r[None, :], 7, axis=0)):
+        mask, bitval, k = oracle.group_masks(rows)
+        assert k == 0 and np.all(mask == 0xFF) and np.array_equal(bitval, r)
+        p, kk = oracle.pack_row(r, mask)
+        assert kk == 0 and p.size == 0
+        assert np.array_equal(oracle.unpack_row(p, mask, bitval), r)       # decode == broadcast of Bitval
+    mask, bitval, k = oracle.group_masks(np.stack([r, ~r]))
+    assert k == 8 * rb and not mask.any() and not bitval.any()
+    p, _ = oracle.pack_row(r, mask)
+    assert np.array_equal(p, r)                                              # all-variant group: pack == memcpy
+    assert np.array_equal(oracle.unpack_row(p, mask, bitval), r)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# pack / unpack
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k,positions_seed", [(1, 0), (3, 1), (5, 2), (9, 3), (11, 4)])
+def test_canonical_bit_order(k, positions_seed):
+    """The 2^k rows that take every value on k chosen bit positions (constant elsewhere): Mask = NOT(those positions),
+    k_g = k, and row number j packs to the integer j, LSB-first (reading R4).  Catches descending walks, MSB-first
+    streams and byte-swapped output."""
+    rb = 8
+    rng = np.random.default_rng(positions_seed)
+    pos = np.sort(rng.choice(8 * rb, size=k, replace=False))
+    const = _bits(datagen.random_bytes(rb, 5 + positions_seed))
+    B = np.repeat(const[None, :], 1 << k, axis=0)
+    for j in range(1 << k):
+        for t, p in enumerate(pos):
+            B[j, p] = (j >> t) & 1
+    rows = np.packbits(B, axis=1, bitorder="little")
+    mask, bitval, kk = oracle.group_masks(rows)
+    assert kk == k
+    want_mask = np.ones(8 * rb, np.uint8)
+    want_mask[pos] = 0
+    assert np.array_equal(_bits(mask), want_mask)
+    for j in range(1 << k):
+        p, _ = oracle.pack_row(rows[j], mask)
+        assert p.size == (k + 7) // 8
+        assert int.from_bytes(p.tobytes(), "little") == j
+
+
+@pytest.mark.parametrize("rb", [4, 12, 64, 256, 512])
+def test_round_trip_random_masks_every_popcount(rb):
+    """unpack(pack(x)) == x on uniformly random bit patterns, for random masks of every popcount 0..8*rb (sampled above
+    64 bytes) (BASELINE.json north_star; losslessness P:11).  The rows satisfy row AND Mask == Bitval."""
+    nbits = 8 * rb
+    pops = range(nbits + 1) if rb <= 12 else sorted(set(np.linspace(0, nbits, 41).astype(int).tolist() + [1, nbits - 1]))
+    rng = np.random.default_rng(rb)
+    for pc in pops:
+        mbits = np.zeros(nbits, np.uint8)
+        mbits[rng.choice(nbits, size=pc, replace=False)] = 1
+        mask = np.packbits(mbits, bitorder="little")
+        bitval = datagen.random_bytes(rb, 1000 + pc) & mask
+        row = (datagen.random_bytes(rb, 2000 + pc) & ~mask) | bitval
+        p, k = oracle.pack_row(row, mask)
+        assert k == nbits - pc and p.size == (k + 7) // 8                  # packed size == variant-bit count
+        if k % 8:
+            assert p[-1] >> (k % 8) == 0                                   # zero padding of the last byte
+        assert np.array_equal(oracle.unpack_row(p, mask, bitval), row)
+        # the packed stream is the variant bits in ascending order (a plain numpy compress of the bit vector)
+        assert np.array_equal(_bits(p)[:k], _bits(row)[mbits == 0])
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# dataset level
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,param,n_rows,rb", [(0, 64, 1000, 64), (0, 7, 50, 12), (1, 5, 203, 32), (1, 8, 64, 16), (0, 1000, 10, 8)])
+def test_dataset_equals_plain_gather(kind, param, n_rows, rb):
+    """(c2) against (c1): gather-decompress == out[i] = X[ids[i]] byte for byte, with a ragged last group; sizes:
+    packed = sum ceil(k_g/8) over rows, <= raw; metadata = 2*row_bytes per group."""
+    X = (datagen.random_bytes(n_rows * rb, 77).reshape(n_rows, rb) & 0x3C) | 0x41
+    ds = oracle.Dataset(X, kind, param)
+    ids = (datagen.u64(500, 3) % np.uint64(n_rows)).astype(np.int64)
+    assert np.array_equal(ds.gather_decompress(ids), oracle.gather_plain(X, ids))
+    want_groups = -(-n_rows // param) if kind == 0 else min(param, n_rows)
+    assert ds.n_groups == want_groups
+    assert ds.metadata_bytes == 2 * rb * want_groups
+    total = 0
+    for r in range(n_rows):
+        g = r // param if kind == 0 else r % param
+        pr = ds.packed_row(r)
+        assert pr.size == (ds.k_bits(g) + 7) // 8                          # equal for every row of a group
+        total += pr.size
+    assert total == ds.packed_bytes <= X.nbytes
+    with pytest.raises(IndexError):
+        ds.gather_decompress(np.array([n_rows], np.int64))
+
+
+def test_dataset_index_span():
+    X = workloads.KV(layers=1, pages=4, heads=2).table()
+    ds = oracle.Dataset(X, 0, 16)
+    ids = np.array([3, 0, 7, 3], np.int64)
+    out = ds.gather_decompress(ids, index_span=32)
+    assert np.array_equal(out, oracle.gather_plain(X, ids, 32))
+    assert np.array_equal(out[:32], X.view(np.uint8).reshape(X.shape[0], -1)[96:128])
+
+
+def test_tiny_analytic_lower_bound():
+    """Tiny (multiples of 2^-6, |x| <= 8): the low 15 mantissa bits of every fp32 element are zero, so every group has
+    popcount(Mask) >= 15*128 (SURVEY 8(c) analytic bounds); DLRM: low 16 bits zero and exponent MSB zero -> >= 17*64;
+    bf16 N(0,0.02) weights: exponent top bits are 011 -> >= 3*128."""
+    X = workloads.Tiny().table()
+    ds = oracle.Dataset(X, 0, 64)
+    for g in range(ds.n_groups):
+        m = ds.mask(g).view(np.uint32)
+        assert np.all(m & 0x7FFF == 0x7FFF)
+        assert 8 * 512 - ds.k_bits(g) >= 15 * 128
+    d = workloads.DLRM(rows_per_table=1024, n_tables=1)
+    ds = oracle.Dataset(d.table(), 0, 128)
+    for g in range(ds.n_groups):
+        assert np.all(ds.mask(g).view(np.uint32) & 0x4000FFFF == 0x4000FFFF)
+        assert np.all(ds.bitval(g).view(np.uint32) & 0x4000FFFF == 0)
+    w = workloads.WeightMatrix(512, 256)
+    ds = oracle.Dataset(w.table(), 1, 2)
+    for g in range(ds.n_groups):
+        assert np.all(ds.mask(g).view(np.uint16) & 0x7000 == 0x7000)
+        assert np.all(ds.bitval(g).view(np.uint16) & 0x7000 == 0x3000)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# thresholded mode (specified in 8(c))
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cs,want_pct", [(1, 12.5), (8, 1.5625)])
+def test_participation_overhead_closed_form(cs, want_pct):
+    """one participation bit per chunk = 12.5 % at 1-byte chunks, '1.6 %' (1.5625 %) at 8-byte chunks.
+    With every bit invariant and matching, stored size == exactly the participation bits."""
+    rb = 512
+    mask = np.full(rb, 0xFF, np.uint8)
+    bitval = datagen.random_bytes(rb, 9)
+    data, comp = oracle.compress_row_T(bitval, mask, bitval, cs)
+    assert comp and data.size == rb // cs // 8
+    assert 100.0 * data.size / rb == want_pct
+
+
+def test_bitmask_size_closed_form():
+    """bitmask = dataset / (tensor * 8): 512 GB of 1 KB tensors -> 64 MB (one flag bit per tensor)."""
+    assert (512 * 2 ** 30) // (1024 * 8) == 64 * 2 ** 20
+
+
+@pytest.mark.parametrize("cs", [1, 2, 4, 8])
+def test_thresholded_round_trip_and_bounds(cs):
+    """Round trip; compressed <= raw for every row; at T=N every chunk participates and the payload after the
+    participation bits equals the strict payload."""
+    w = workloads.GNN(n_rows=4096)
+    rows = np.concatenate([w.rows(0, 200), w.rows(3000, 56)])
+    R = rows.view(np.uint8).reshape(rows.shape[0], -1)
+    rb = R.shape[1]
+    for T in (int(0.8 * len(R)), len(R)):
+        mask, bitval, _ = oracle.group_masks(R, T=T)
+        n_comp = 0
+        for r in R[::5]:
+            data, comp = oracle.compress_row_T(r, mask, bitval, cs)
+            assert data.size <= rb
+            assert comp or data.size == rb
+            n_comp += comp
+            assert np.array_equal(oracle.decompress_row_T(data, comp, mask, bitval, cs), r)
+            if T == len(R) and comp:
+                nch = rb // cs
+                bits = _bits(data)
+                assert np.all(bits[:nch] == 1)
+                strict, k = oracle.pack_row(r, mask)
+                assert np.array_equal(bits[nch:nch + k], _bits(strict)[:k])
+        assert n_comp > 0
