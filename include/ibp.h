@@ -1,0 +1,198 @@
+/*
+ * ibp.h -- C ABI of the B200-native Invariant Bit Packing library (libibp.so).
+ *
+ * What it is: the data-parallel hot path of IBP ("Reducing the GPU Memory Bottleneck with Lossless Compression for
+ * ML", arxiv/paper_2605_30728; cited below as P:<line> of PAPER.md): a fused gather-and-decompress of indexed
+ * compressed rows.  Rows ("tensors" in the paper) are compressed once on the host by removing the bits that are
+ * identical across each group of rows, and kept in pinned, GPU-mapped host memory.  A CUDA kernel then
+ * reads requested rows zero-copy over PCIe, re-inserts the invariant bits from per-group Mask/Bitval
+ * metadata held in GPU memory, and writes the original rows into an HBM tensor.
+ *
+ * Mode: "group-strict" IBP = the paper's clustered compression with clusters that are fixed runs of rows
+ * and threshold T = N_group: a bit is invariant iff every row of the group agrees, so every row of a group
+ * has the same packed length and there are no participation bits and no per-row raw flag.
+ *
+ * Conventions
+ *   - Bit p of a row is bit (p mod 8) of byte (p div 8).  Mask bit 1 = invariant; Bitval holds the invariant values
+ *     and is 0 where Mask is 0.
+ *   - A packed row is the row's bits at the Mask=0 positions, ascending p, LSB-first, zero padded to ceil(k/8)
+ *     bytes and then to `align_bytes` (the alignment unit A).  This is the oracle's canonical order.
+ *   - Store layout.  Blocked groups: groups in order, each group's base aligned to max(A,16); rows of a group at
+ *     base + j*stride_g.  Strided groups: matrix row r (= id div S) at r*rowstride, tile t at prefix_t inside it.
+ *   - Pointers are named *_host (CPU addressable), *_dev (GPU addressable on the handle's device).
+ *   - Streams are passed as void* (a cudaStream_t); NULL = the legacy default stream.
+ *   - Every function returns ibp_status; 0 = success.  No C++ exception crosses this boundary.  ibp_last_error()
+ *     returns a thread-local message for the last failing call.
+ *   - There is no CPU fallback: ibp_build is host code by design (the compressor); every other step
+ *     needs a CUDA device of compute capability 10.0 and fails with IBP_ERR_CUDA without one.
+ *
+ * Ownership: the caller owns rows_host, row_ids_dev, out_dev, packed_dev and the stream.  The handle owns all it
+ * allocates (packed store, metadata copies on host and device) until ibp_destroy, which the caller may only call
+ * after synchronising every stream that used the handle.
+ * Thread safety: concurrent gather/decompress calls on one handle are allowed; build/upload/configure/destroy are not.
+ */
+#ifndef IBP_H
+#define IBP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ibp_handle ibp_handle;
+
+typedef enum {
+    IBP_OK = 0,
+    IBP_ERR_INVALID_ARG = 1,
+    IBP_ERR_OUT_OF_MEMORY = 2,
+    IBP_ERR_CUDA = 3,
+    IBP_ERR_BAD_STATE = 4,   /* e.g. gather before ibp_upload_metadata */
+    IBP_ERR_UNSUPPORTED = 5  /* e.g. threshold < 1 (the paper's thresholded mode is not on this path) */
+} ibp_status;
+
+typedef enum {
+    IBP_GROUP_BLOCKED = 0, /* group(id) = id div group_param : runs of consecutive rows                    */
+    IBP_GROUP_STRIDED = 1  /* group(id) = id mod group_param : column tiles of a row-major matrix (S tiles) */
+} ibp_group_kind;
+
+enum {
+    IBP_FLAG_PAGEABLE_STORE = 1u,  /* keep the packed store in ordinary memory: no zero-copy gather (CPU-only tests)  */
+    IBP_FLAG_HOSTALLOC_STORE = 2u  /* use cudaHostAlloc pinned memory instead of the default managed-host allocation  */
+};
+
+typedef enum {
+    IBP_STORE_PAGEABLE = 0,     /* ordinary host memory; the GPU cannot read it in place                              */
+    IBP_STORE_PINNED = 1,       /* cudaHostAlloc(mapped|portable): page-locked, 4 KB GPU pages                        */
+    IBP_STORE_MANAGED_HOST = 2  /* cudaMallocManaged, preferred location CPU, accessed-by GPU: host-resident, read in
+                                   place over PCIe, mapped by the GPU with large pages        */
+} ibp_store_kind;
+
+typedef struct {
+    uint32_t struct_size;   /* = sizeof(ibp_build_params), for ABI growth                                        */
+    uint32_t row_bytes;     /* bytes per row; multiple of 4 (the paper's 4-byte chunk), 4 .. 65536        */
+    uint64_t n_rows;
+    uint32_t group_kind;    /* ibp_group_kind                                                                    */
+    uint32_t group_param;   /* G (blocked) or S (strided); >= 1                                                  */
+    uint32_t threshold_num; /* T/N; only 1/1 (strict) is supported here, 0/0 means 1/1                           */
+    uint32_t threshold_den;
+    uint32_t align_bytes;   /* packed-row alignment unit A: power of two in 1..128; 0 = default (32)             */
+    uint32_t index_span;    /* consecutive rows selected by one id in ibp_gather_decompress; 0 = 1               */
+    uint32_t flags;         /* IBP_FLAG_*                                                                        */
+    uint32_t n_threads;     /* host threads for the build; 0 = all                                               */
+} ibp_build_params;
+
+typedef struct {
+    uint64_t n_rows, n_groups;
+    uint64_t packed_bytes_stored;      /* size of the packed store incl. alignment padding                       */
+    uint64_t packed_bytes_rows;        /* sum over rows of the row stride roundup(ceil(k_g/8), A)                */
+    uint64_t packed_bytes_bytealigned; /* sum over rows of ceil(k_g/8): the oracle's canonical size      */
+    uint64_t metadata_bytes;           /* 2*row_bytes per group: Mask + Bitval                    */
+    uint64_t aux_bytes;                /* per-group table (base offset, stride, k): 16 B per group               */
+    uint32_t row_bytes, align_bytes, index_span, group_kind, group_param;
+    uint32_t max_row_stride;           /* largest packed-row stride in bytes                                     */
+    int32_t  device;                   /* device holding the metadata, -1 before ibp_upload_metadata             */
+    uint32_t store_kind;               /* ibp_store_kind                                                         */
+} ibp_info;
+
+/* -- S0, S0': host-side compressor (P:229-231 masks with T=N per group; P:237-241, P:275-298 packing). ---------------
+ * rows_host: n_rows x row_bytes, row-major, borrowed for the duration of the call.  Synchronous, multi-threaded,
+ * CPU only.  The handle allocates its own packed store in host memory the GPU reads in place (ibp_store_kind:
+ * managed-host by default, cudaHostAlloc with IBP_FLAG_HOSTALLOC_STORE) when a CUDA device is present and
+ * IBP_FLAG_PAGEABLE_STORE is not set, else ordinary memory (then only ibp_decompress_resident and the host
+ * accessors work).  Errors: INVALID_ARG (null pointers, row_bytes not a multiple of 4, bad A, span not
+ * compatible with the groups), UNSUPPORTED (threshold != 1), OUT_OF_MEMORY.                                        */
+ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle);
+
+/* -- S0'': copy Mask/Bitval and the group table to HBM on `device` ("stored in GPU memory").  Idempotent for the
+ * same device; INVALID_ARG for a second device.  Synchronises the stream before returning.                         */
+ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream);
+
+/* -- S1-S6: the hot path.  For i in [0,n), j in [0,index_span):
+ *      out_dev[(i*index_span + j)*row_bytes ...] = original row  row_ids_dev[i]*index_span + j.
+ * row_ids_dev: n int64 on the device.  out_dev: n*index_span*row_bytes bytes on the device, 16-byte aligned.
+ * Asynchronous on the stream.  Duplicate ids allowed.  n == 0 is a no-op.  Ids are not validated (out of range =
+ * undefined behaviour), see ibp_validate_ids.  BAD_STATE before upload or with a pageable store.                   */
+ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);
+
+/* Same result with HOST buffers: row_ids_host (n int64) is copied to the device, the gather runs, and the rows are
+ * copied back into out_host, all on the stream, which is synchronised before returning.  The end-to-end entry point
+ * bench.py times.  The buffers should be pinned for full copy speed; pageable memory works.                        */
+ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host, int64_t n, void* out_host, void* cuda_stream);
+
+/* -- S8: decode rows [first_row, first_row+n_rows) whose packed bytes the caller already staged in device memory
+ * exactly as they lie in the host store (ibp_packed_range gives the source range; e.g. cudaMemcpyAsync, or a
+ * compressed GPU cache slab).  first_row must start a layout unit: a multiple of G (blocked) or of S
+ * (strided).  packed_dev must be 16-byte aligned.  Asynchronous on the stream.                                     */
+ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_t first_row, int64_t n_rows,
+                                   void* out_dev, void* cuda_stream);
+
+/* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
+ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
+
+/* Location of one packed row inside the store (host pointer, stride bytes, variant bits k).  For cross-checks.    */
+ibp_status ibp_packed_row(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stride_bytes, uint32_t* k_bits);
+
+/* Host copies of one group's metadata: Mask and Bitval (row_bytes each) and k_g.  For oracle cross-checks.        */
+ibp_status ibp_get_metadata_host(const ibp_handle* h, int64_t group, const void** mask, const void** bitval, uint32_t* k_bits);
+
+ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out);
+
+/* Launch shape of the decode kernels: max_ctas limits the grid (0 = library default), so that a consumer kernel can
+ * share the GPU ("We reserved only 64 SMs for decompression"); warps_per_cta 0 = default.                    */
+ibp_status ibp_configure(ibp_handle* h, uint32_t max_ctas, uint32_t warps_per_cta);
+
+/* Debug pre-pass: *n_bad_host = number of ids outside [0, n_rows/index_span).  Synchronises the stream.           */
+ibp_status ibp_validate_ids(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, int64_t* n_bad_host, void* cuda_stream);
+
+/* Sum over the DISTINCT ids of a batch of the packed bytes one id moves over PCIe (index_span rows each): the
+ * algorithmic link traffic of one ibp_gather_decompress call.  stored = with alignment padding, bytealigned =
+ * ceil(k/8) per row.  Host-side helper for roofline accounting; ids on the host.                                   */
+ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* row_ids_host, int64_t n, uint64_t* n_unique,
+                                uint64_t* stored, uint64_t* bytealigned);
+
+void ibp_destroy(ibp_handle* h);
+const char* ibp_last_error(void);
+const char* ibp_version(void);
+
+/* -- Baseline in the same library so both are timed the same way ("GPU (Aligned)" zero-copy gather):
+ *      out_dev[i*row_bytes ...] = rows_host_mapped[row_ids_dev[i]*row_bytes ...], uncompressed.
+ * rows_host_mapped must be pinned+mapped host memory (device-visible address) or device memory; row_bytes % 16 == 0. */
+ibp_status ibp_gather_uncompressed(const void* rows_mapped, uint32_t row_bytes, const int64_t* row_ids_dev, int64_t n,
+                                   void* out_dev, void* cuda_stream);
+
+/* Same gather with the locality-ordered pre-pass of ibp_gather_decompress when locality_order
+ * != 0; n_rows = number of rows of the table (needed to size the buckets).                                         */
+ibp_status ibp_gather_uncompressed_ex(const void* rows_mapped, uint32_t row_bytes, uint64_t n_rows, const int64_t* row_ids_dev,
+                                      int64_t n, void* out_dev, int locality_order, void* cuda_stream);
+
+/* Tuning/test hook: locality-ordered processing of random gathers: 1 = always, 0 = never, -1 = automatic (default:
+ * on for IBP_STORE_PINNED stores above 64 MiB and batches of >= 4096 ids).  Results are identical either way.        */
+ibp_status ibp_set_order_mode(ibp_handle* h, int mode);
+
+/* Tuning/test hook: engine that moves packed rows into shared memory: 1 = cp.async.bulk + mbarrier (TMA, default),
+ * 0 = 16-byte cp.async through the load/store unit.  Results are identical either way.                              */
+ibp_status ibp_set_fetch_mode(ibp_handle* h, int mode);
+
+/* Tuning/test hook: rows each warp keeps in flight in random gathers (ring depth): 1, 2 or 4.                       */
+ibp_status ibp_set_rows_in_flight(ibp_handle* h, int n);
+
+/* -- Pinned, GPU-mapped host memory for callers that are not CUDA programs (the baseline table, pinned id buffers).  */
+ibp_status ibp_host_alloc(size_t nbytes, void** host_ptr, void** dev_ptr);
+ibp_status ibp_host_free(void* host_ptr);
+/* Host-resident managed memory with a direct mapping on `device` (the store kind IBP_STORE_MANAGED_HOST); one pointer
+ * serves host and device.                                                                                           */
+ibp_status ibp_host_alloc_managed(size_t nbytes, int device, void** ptr);
+ibp_status ibp_host_free_managed(void* ptr);
+
+/* -- Link ceilings measured on this machine, for the roofline (BASELINE.json: "measured cudaMemcpy H2D ceiling").
+ * ibp_measure_h2d: best of `reps` cudaMemcpyAsync H2D copies of nbytes from pinned memory, in GB/s.
+ * ibp_measure_zero_copy_read: best of `reps` SM-issued contiguous 16-byte zero-copy reads of nbytes, in GB/s.       */
+ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, double* gbps);
+ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IBP_H */

@@ -114,8 +114,8 @@ def unpack_row(packed, mask, bitval):
     mask = np.ascontiguousarray(mask, np.uint8)
     bitval = np.ascontiguousarray(bitval, np.uint8)
     rb = mask.size
-    buf = np.zeros(rb + 8, np.uint8)
     p = np.ascontiguousarray(packed, np.uint8)
+    buf = np.zeros(max(rb, p.size) + 8, np.uint8)      # input may carry alignment padding; only ceil(k/8) bytes are read
     buf[: p.size] = p
     out = np.zeros(rb, np.uint8)
     lib().ibp_oracle_unpack_row(buf.ctypes.data, mask.ctypes.data, bitval.ctypes.data, rb, out.ctypes.data)

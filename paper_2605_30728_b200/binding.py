@@ -1,0 +1,255 @@
+"""Thin ctypes binding of libibp.so (include/ibp.h): same names, argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; this module never computes anything and there is
+no CPU fallback: if libibp.so cannot be built/loaded, or a call fails, an exception is raised.
+PyTorch (optional here) supplies device memory and streams: pass `tensor.data_ptr()` and
+`torch.cuda.current_stream().cuda_stream`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from ._build import build_library
+
+IBP_OK = 0
+STATUS = {0: "IBP_OK", 1: "IBP_ERR_INVALID_ARG", 2: "IBP_ERR_OUT_OF_MEMORY", 3: "IBP_ERR_CUDA", 4: "IBP_ERR_BAD_STATE",
+          5: "IBP_ERR_UNSUPPORTED"}
+IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED = 0, 1
+IBP_FLAG_PAGEABLE_STORE = 1
+IBP_FLAG_HOSTALLOC_STORE = 2
+IBP_STORE_PAGEABLE, IBP_STORE_PINNED, IBP_STORE_MANAGED_HOST = 0, 1, 2
+
+
+class IbpError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class ibp_build_params(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("row_bytes", C.c_uint32), ("n_rows", C.c_uint64),
+                ("group_kind", C.c_uint32), ("group_param", C.c_uint32), ("threshold_num", C.c_uint32),
+                ("threshold_den", C.c_uint32), ("align_bytes", C.c_uint32), ("index_span", C.c_uint32),
+                ("flags", C.c_uint32), ("n_threads", C.c_uint32)]
+
+
+class ibp_info(C.Structure):
+    _fields_ = [("n_rows", C.c_uint64), ("n_groups", C.c_uint64), ("packed_bytes_stored", C.c_uint64),
+                ("packed_bytes_rows", C.c_uint64), ("packed_bytes_bytealigned", C.c_uint64),
+                ("metadata_bytes", C.c_uint64), ("aux_bytes", C.c_uint64), ("row_bytes", C.c_uint32),
+                ("align_bytes", C.c_uint32), ("index_span", C.c_uint32), ("group_kind", C.c_uint32),
+                ("group_param", C.c_uint32), ("max_row_stride", C.c_uint32), ("device", C.c_int32),
+                ("store_kind", C.c_uint32)]
+
+
+# name -> (restype, argtypes); every symbol include/ibp.h declares (tests/test_abi.py checks the two lists agree)
+_vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int
+SIGNATURES = {
+    "ibp_build": (_int, [_vp, C.POINTER(ibp_build_params), C.POINTER(_vp)]),
+    "ibp_upload_metadata": (_int, [_vp, _int, _vp]),
+    "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
+    "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
+    "ibp_decompress_resident": (_int, [_vp, _vp, _i64, _i64, _vp, _vp]),
+    "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
+    "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
+    "ibp_get_metadata_host": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_u32)]),
+    "ibp_get_info": (_int, [_vp, C.POINTER(ibp_info)]),
+    "ibp_configure": (_int, [_vp, _u32, _u32]),
+    "ibp_validate_ids": (_int, [_vp, _vp, _i64, C.POINTER(_i64), _vp]),
+    "ibp_batch_link_bytes": (_int, [_vp, _vp, _i64, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]),
+    "ibp_destroy": (None, [_vp]),
+    "ibp_last_error": (C.c_char_p, []),
+    "ibp_version": (C.c_char_p, []),
+    "ibp_gather_uncompressed": (_int, [_vp, _u32, _vp, _i64, _vp, _vp]),
+    "ibp_gather_uncompressed_ex": (_int, [_vp, _u32, _u64, _vp, _i64, _vp, _int, _vp]),
+    "ibp_set_order_mode": (_int, [_vp, _int]),
+    "ibp_set_fetch_mode": (_int, [_vp, _int]),
+    "ibp_set_rows_in_flight": (_int, [_vp, _int]),
+    "ibp_host_alloc": (_int, [C.c_size_t, C.POINTER(_vp), C.POINTER(_vp)]),
+    "ibp_host_free": (_int, [_vp]),
+    "ibp_host_alloc_managed": (_int, [C.c_size_t, _int, C.POINTER(_vp)]),
+    "ibp_host_free_managed": (_int, [_vp]),
+    "ibp_measure_h2d": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
+    "ibp_measure_zero_copy_read": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
+}
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) the CUDA library.  Raises if nvcc or the sources are missing: no fallback."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(str(build_library()))
+        for name, (res, args) in SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(status):
+    if status != IBP_OK:
+        raise IbpError(status, lib().ibp_last_error().decode())
+
+
+def _ptr(x):
+    """numpy array -> address; int -> itself (device pointer); None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return int(x)
+
+
+class Handle:
+    """Owns an ibp_handle*.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, ptr):
+        self._h = ptr
+
+    def upload_metadata(self, device=0, stream=None):
+        _check(lib().ibp_upload_metadata(self._h, device, stream))
+        return self
+
+    def gather_decompress(self, row_ids_dev, n, out_dev, stream=None):
+        _check(lib().ibp_gather_decompress(self._h, _ptr(row_ids_dev), n, _ptr(out_dev), stream))
+
+    def gather_decompress_host(self, row_ids_host, n, out_host, stream=None):
+        _check(lib().ibp_gather_decompress_host(self._h, _ptr(row_ids_host), n, _ptr(out_host), stream))
+
+    def decompress_resident(self, packed_dev, first_row, n_rows, out_dev, stream=None):
+        _check(lib().ibp_decompress_resident(self._h, _ptr(packed_dev), first_row, n_rows, _ptr(out_dev), stream))
+
+    def packed_range(self, first_row, n_rows):
+        p, nb = _vp(), _u64()
+        _check(lib().ibp_packed_range(self._h, first_row, n_rows, C.byref(p), C.byref(nb)))
+        return p.value, nb.value
+
+    def packed_row(self, row):
+        """(bytes of the stored packed row incl. alignment padding, k_bits)"""
+        p, st, k = _vp(), _u32(), _u32()
+        _check(lib().ibp_packed_row(self._h, row, C.byref(p), C.byref(st), C.byref(k)))
+        data = np.ctypeslib.as_array(C.cast(p.value, C.POINTER(C.c_uint8)), (st.value,)).copy() if st.value else np.zeros(0, np.uint8)
+        return data, k.value
+
+    def packed_view(self, host_ptr, nbytes):
+        return np.ctypeslib.as_array(C.cast(host_ptr, C.POINTER(C.c_uint8)), (nbytes,))
+
+    def metadata_host(self, group):
+        m, b, k = _vp(), _vp(), _u32()
+        _check(lib().ibp_get_metadata_host(self._h, group, C.byref(m), C.byref(b), C.byref(k)))
+        rb = self.info().row_bytes
+        mask = np.ctypeslib.as_array(C.cast(m.value, C.POINTER(C.c_uint8)), (rb,)).copy()
+        bitval = np.ctypeslib.as_array(C.cast(b.value, C.POINTER(C.c_uint8)), (rb,)).copy()
+        return mask, bitval, k.value
+
+    def info(self):
+        out = ibp_info()
+        _check(lib().ibp_get_info(self._h, C.byref(out)))
+        return out
+
+    def configure(self, max_ctas=0, warps_per_cta=0):
+        _check(lib().ibp_configure(self._h, max_ctas, warps_per_cta))
+        return self
+
+    def set_order_mode(self, mode):
+        _check(lib().ibp_set_order_mode(self._h, mode))
+        return self
+
+    def set_fetch_mode(self, mode):
+        _check(lib().ibp_set_fetch_mode(self._h, mode))
+        return self
+
+    def set_rows_in_flight(self, n):
+        _check(lib().ibp_set_rows_in_flight(self._h, n))
+        return self
+
+    def validate_ids(self, row_ids_dev, n, stream=None):
+        bad = _i64()
+        _check(lib().ibp_validate_ids(self._h, _ptr(row_ids_dev), n, C.byref(bad), stream))
+        return bad.value
+
+    def batch_link_bytes(self, row_ids_host):
+        ids = np.ascontiguousarray(row_ids_host, dtype=np.int64)
+        nu, st, ba = _u64(), _u64(), _u64()
+        _check(lib().ibp_batch_link_bytes(self._h, ids.ctypes.data, ids.size, C.byref(nu), C.byref(st), C.byref(ba)))
+        return nu.value, st.value, ba.value
+
+    def destroy(self):
+        if self._h:
+            lib().ibp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def ibp_build(rows_host: np.ndarray, row_bytes: int, group_kind: int, group_param: int, align_bytes: int = 0,
+              index_span: int = 1, flags: int = 0, n_threads: int = 0, threshold=(1, 1)) -> Handle:
+    rows = np.ascontiguousarray(rows_host)
+    assert rows.nbytes % row_bytes == 0
+    p = ibp_build_params(C.sizeof(ibp_build_params), row_bytes, rows.nbytes // row_bytes, group_kind, group_param,
+                         threshold[0], threshold[1], align_bytes, index_span, flags, n_threads)
+    h = _vp()
+    _check(lib().ibp_build(rows.ctypes.data, C.byref(p), C.byref(h)))
+    return Handle(h)
+
+
+def ibp_gather_uncompressed(rows_mapped, row_bytes, row_ids_dev, n, out_dev, stream=None, n_rows=0, locality_order=False):
+    if locality_order:
+        _check(lib().ibp_gather_uncompressed_ex(_ptr(rows_mapped), row_bytes, n_rows, _ptr(row_ids_dev), n, _ptr(out_dev), 1, stream))
+    else:
+        _check(lib().ibp_gather_uncompressed(_ptr(rows_mapped), row_bytes, _ptr(row_ids_dev), n, _ptr(out_dev), stream))
+
+
+class PinnedBuffer:
+    """GPU-visible host memory viewed as a numpy array: pinned (ibp_host_alloc) or managed-host (ibp_host_alloc_managed)."""
+
+    def __init__(self, nbytes, managed=False, device=0):
+        hp, dp = _vp(), _vp()
+        self.managed = managed
+        if managed:
+            _check(lib().ibp_host_alloc_managed(nbytes, device, C.byref(hp)))
+            dp = hp
+        else:
+            _check(lib().ibp_host_alloc(nbytes, C.byref(hp), C.byref(dp)))
+        self.host_ptr, self.dev_ptr, self.nbytes = hp.value, dp.value, nbytes
+        self.array = np.ctypeslib.as_array(C.cast(hp.value, C.POINTER(C.c_uint8)), (nbytes,))
+
+    def view(self, dtype, shape=None):
+        a = self.array.view(dtype)
+        return a.reshape(shape) if shape is not None else a
+
+    def free(self):
+        if self.host_ptr:
+            self.array = None
+            _check(lib().ibp_host_free_managed(self.host_ptr) if self.managed else lib().ibp_host_free(self.host_ptr))
+            self.host_ptr = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def ibp_measure_h2d(device=0, nbytes=1 << 30, reps=10) -> float:
+    g = C.c_double()
+    _check(lib().ibp_measure_h2d(device, nbytes, reps, C.byref(g)))
+    return g.value
+
+
+def ibp_measure_zero_copy_read(device=0, nbytes=1 << 30, reps=5) -> float:
+    g = C.c_double()
+    _check(lib().ibp_measure_zero_copy_read(device, nbytes, reps, C.byref(g)))
+    return g.value
+
+
+def ibp_version() -> str:
+    return lib().ibp_version().decode()

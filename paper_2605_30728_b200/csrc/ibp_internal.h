@@ -1,0 +1,58 @@
+// ibp_internal.h -- private state of libibp.so (not part of the C ABI; shares nothing with oracle/).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "ibp.h"
+
+// One entry per group, 16 bytes, mirrored in HBM.
+//   blocked: packed row j of the group lies at store + base + j*stride
+//   strided: tile t of matrix row r lies at store + r*row_stride_strided + base   (base = prefix_t)
+struct IbpGroupEntry {
+    uint64_t base;
+    uint32_t stride;   // roundup(ceil(k/8), A); 0 when k == 0
+    uint32_t k_bits;   // variant bits per row of this group
+};
+
+struct ibp_handle {
+    ibp_build_params p{};
+    uint64_t n_groups = 0;
+    uint32_t n_words = 0;                  // row_bytes / 4
+    uint64_t row_stride_strided = 0;       // bytes of one packed matrix row (strided groups)
+    uint32_t max_stride = 0;
+
+    // host copies
+    std::vector<uint32_t> meta;            // per group: Mask words then Bitval words (2*n_words)
+    std::vector<IbpGroupEntry> gtab;
+    uint8_t* store = nullptr;              // packed store (pinned+mapped, or malloc)
+    uint8_t* store_dev = nullptr;          // device-visible address of the store (nullptr if pageable)
+    uint64_t store_bytes = 0;              // incl. slack
+    uint64_t store_used = 0;
+    int store_kind = IBP_STORE_PAGEABLE;   // ibp_store_kind
+    uint64_t packed_bytes_rows = 0, packed_bytes_bytealigned = 0;
+
+    // device copies
+    int device = -1;
+    uint32_t* meta_dev = nullptr;
+    IbpGroupEntry* gtab_dev = nullptr;
+
+    // launch configuration
+    uint32_t max_ctas = 0, warps_per_cta = 0;
+    int sm_count = 0;
+    int order_mode = -1;                   // -1 auto, 0 off, 1 on (locality-ordered gather)
+    int rows_in_flight = 2;                // random gathers: rows each warp keeps in flight (1, 2 or 4)
+    int fetch_mode = 1;                    // 0 = cp.async (LSU), 1 = cp.async.bulk (TMA)
+};
+
+// error plumbing (thread local)
+void ibp_set_error(const char* fmt, ...);
+
+// byte offset of packed row `id` inside the store
+static inline uint64_t ibp_row_offset(const ibp_handle* h, uint64_t id) {
+    if (h->p.group_kind == IBP_GROUP_BLOCKED) {
+        const uint64_t g = id / h->p.group_param;
+        return h->gtab[g].base + (id - g * h->p.group_param) * (uint64_t)h->gtab[g].stride;
+    }
+    return (id / h->p.group_param) * h->row_stride_strided + h->gtab[id % h->p.group_param].base;
+}

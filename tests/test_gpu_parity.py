@@ -1,0 +1,239 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element as raw bytes.
+
+Bar: bit-exact (integer/byte work; floats are compared as bit patterns so NaN payloads, -0.0 and denormals count).
+Sizes span several tiles (warps, CTAs, grid-stride rounds) and ragged tails; edge cases: empty batch, duplicates,
+groups with no variant bit, groups with no invariant bit, multi-pass rows, every alignment unit.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_30728_b200 import binding as ibp
+from paper_2605_30728_b200 import datagen, workloads
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _gather(h, ids, span=1, rb=None):
+    rb = rb or h.info().row_bytes
+    ids_d = _dev(np.asarray(ids, np.int64))
+    out = torch.full((max(1, len(ids) * span), rb), 0xA5, dtype=torch.uint8, device="cuda")
+    h.gather_decompress(ids_d.data_ptr(), len(ids), out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()[: len(ids) * span]
+
+
+def _resident(h, first, n):
+    ptr, nbytes = h.packed_range(first, n)
+    packed = _dev(h.packed_view(ptr, nbytes).copy()) if nbytes else torch.zeros(16, dtype=torch.uint8, device="cuda")
+    out = torch.full((max(1, n), h.info().row_bytes), 0x5A, dtype=torch.uint8, device="cuda")
+    h.decompress_resident(packed.data_ptr(), first, n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()[:n]
+
+
+def _u8(X):
+    X = np.ascontiguousarray(X)
+    return X.view(np.uint8).reshape(X.shape[0], -1)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("align", [1, 4, 16, 32, 64, 128])
+@pytest.mark.parametrize("order_mode", [0, 1])
+@pytest.mark.parametrize("fetch_mode", [0, 1])
+def test_tiny_config_gather(align, order_mode, fetch_mode):
+    """BASELINE.json configs[0] exactly: 4,096 x 128 fp32, groups of 64, 1,024 uniform ids; both fetch engines
+    (cp.async through the LSU, cp.async.bulk through the TMA unit) and both processing orders."""
+    w = workloads.Tiny()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 64, align_bytes=align).upload_metadata(0).set_order_mode(order_mode).set_fetch_mode(fetch_mode)
+    ds = oracle.Dataset(X, 0, 64)
+    for it in range(3):
+        ids = w.ids(it)
+        got = _gather(h, ids)
+        assert np.array_equal(got, ds.gather_decompress(ids))          # (c2) the oracle codec
+        assert np.array_equal(got, oracle.gather_plain(X, ids))        # (c1) the plain definition
+    h.destroy()
+
+
+@pytest.mark.parametrize("kind,param,n,rb,align", [
+    (0, 7, 50, 12, 1), (0, 7, 50, 12, 16), (0, 64, 3000, 64, 32), (0, 1000, 10, 8, 4), (0, 16, 40, 4, 16),
+    (1, 5, 203, 32, 16), (1, 8, 64, 16, 1), (1, 3, 2, 4, 16), (0, 1, 9, 20, 8), (0, 33, 1000, 100, 32),
+    (0, 128, 700, 256, 32), (0, 256, 1500, 512, 32), (0, 50, 333, 1024, 32), (0, 20, 77, 4096, 64), (1, 6, 600, 2048, 16),
+    (0, 9, 100, 516, 4), (0, 9, 100, 264, 1), (0, 4, 30, 8192, 128),
+])
+def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
+    """Shapes the fast paths do not special-case: odd row sizes (W=1,2,4; 1..16 passes), ragged last groups, strided
+    groups with a partial last matrix row, every alignment unit; gather (both orders) and resident decode."""
+    X = (datagen.random_bytes(n * rb, 5 + rb).reshape(n, rb) & datagen.random_bytes(rb, 9)[None, :]) | 0x01
+    h = ibp.ibp_build(X, rb, kind, param, align_bytes=align).upload_metadata(0)
+    ds = oracle.Dataset(X, kind, param)
+    ids = np.concatenate([(datagen.u64(777, 3) % np.uint64(n)).astype(np.int64), np.arange(n, dtype=np.int64)])
+    want = ds.gather_decompress(ids)
+    assert np.array_equal(want, oracle.gather_plain(X, ids))
+    for fetch in (0, 1):
+        h.set_fetch_mode(fetch)
+        for mode in (0, 1):
+            h.set_order_mode(mode)
+            assert np.array_equal(_gather(h, ids), want)
+        assert np.array_equal(_resident(h, 0, n), X)                    # whole table from HBM
+    if kind == 0 and n > 2 * param:
+        first = param * ((n // param) // 2)
+        assert np.array_equal(_resident(h, first, n - first), X[first:])
+        assert np.array_equal(_resident(h, first, param), X[first:first + param])
+    if kind == 1 and n > 2 * param:
+        first = param * ((n // param) // 2)
+        assert np.array_equal(_resident(h, first, n - first), X[first:])
+    h.destroy()
+
+
+def test_edge_cases():
+    rb = 256
+    r = datagen.random_bytes(rb, 3)
+    # all-identical group (k=0: nothing crosses PCIe), a group with a row and its complement (k = all bits: raw copy),
+    # NaN / -0.0 / denormal patterns survive, duplicates, empty batch
+    special = np.frombuffer(np.array([np.nan, -0.0, 1e-45, np.inf, -np.inf, 0.0, 1.0, -1.0] * 8, np.float32).tobytes(), np.uint8)
+    X = np.stack([r] * 4 + [r, ~r, r, ~r] + [special, special ^ 1, special, special ^ 0x80])
+    h = ibp.ibp_build(X, rb, 0, 4, align_bytes=16).upload_metadata(0)
+    ks = [h.metadata_host(g)[2] for g in range(3)]
+    assert ks[0] == 0 and ks[1] == 8 * rb
+    ids = np.array([0, 3, 3, 3, 4, 5, 11, 8, 9, 10, 0, 7], np.int64)
+    assert np.array_equal(_gather(h, ids), X[ids])
+    assert _gather(h, np.zeros(0, np.int64)).shape[0] == 0               # n == 0 is a no-op
+    assert np.array_equal(_resident(h, 0, 12), X)
+    assert np.array_equal(_resident(h, 4, 4), X[4:8])
+    # id validation pre-pass
+    bad = _dev(np.array([0, 11, 12, -1, 5], np.int64))
+    assert h.validate_ids(bad.data_ptr(), 5, torch.cuda.current_stream().cuda_stream) == 2
+    # argument errors are reported, not ignored
+    out = torch.zeros(16 + rb, dtype=torch.uint8, device="cuda")
+    with pytest.raises(ibp.IbpError):
+        h.gather_decompress(bad.data_ptr(), 1, out.data_ptr() + 1)
+    with pytest.raises(ibp.IbpError):
+        h.decompress_resident(out.data_ptr(), 2, 4, out.data_ptr())
+    h.destroy()
+
+
+@pytest.mark.parametrize("n_ids", [1, 31, 33, 4097, 100_000])
+def test_gnn_shape_batches(n_ids):
+    """configs[1] shape at 200k rows: dense + sparse halves and the mixed group at the boundary; batch sizes around the
+    warp / CTA / grid-stride boundaries; launch configuration of bench.py (defaults)."""
+    w = workloads.GNN(n_rows=200_000, batch=n_ids)
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 256, align_bytes=32).upload_metadata(0)
+    ids = w.ids(0)
+    assert len(np.unique(ids)) == len(ids) == n_ids
+    got = _gather(h, ids)
+    assert np.array_equal(got, oracle.gather_plain(X, ids))
+    # the oracle codec on the groups this batch touches (groups are independent): masks, k, decode
+    Xb = _u8(X)
+    for g in np.unique(ids // 256)[:40]:
+        rows = Xb[g * 256:(g + 1) * 256]
+        mask, bitval, k = oracle.group_masks(rows)
+        m, b, kk = h.metadata_host(int(g))
+        assert k == kk and np.array_equal(m, mask) and np.array_equal(b, bitval)
+    h.destroy()
+
+
+@pytest.mark.parametrize("flags,kind", [(0, ibp.IBP_STORE_MANAGED_HOST), (ibp.IBP_FLAG_HOSTALLOC_STORE, ibp.IBP_STORE_PINNED)])
+def test_dlrm_shape_duplicates(flags, kind):
+    """configs[2] shape, small; both GPU-visible store kinds (managed-host default, cudaHostAlloc by flag)."""
+    w = workloads.DLRM(rows_per_table=50_000, n_tables=26, samples=2048)
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 128, align_bytes=32, flags=flags).upload_metadata(0)
+    assert h.info().store_kind == kind
+    ids = w.ids(0)
+    assert len(np.unique(ids)) < len(ids)                                 # repeats kept (reading R16)
+    for mode in (0, 1):
+        h.set_order_mode(mode)
+        assert np.array_equal(_gather(h, ids), oracle.gather_plain(X, ids))
+    h.destroy()
+
+
+def test_kv_shape_spans():
+    """configs[3] shape, small: one id = one page of one layer of K or V = heads*16 consecutive rows, groups of 16."""
+    w = workloads.KV(layers=2, pages=64, heads=8, pages_per_layer=16)
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 16, align_bytes=16, index_span=w.index_span).upload_metadata(0)
+    ds = oracle.Dataset(X, 0, 16)
+    ids = w.ids(0)
+    got = _gather(h, ids, span=w.index_span)
+    assert np.array_equal(got, ds.gather_decompress(ids, w.index_span))
+    assert np.array_equal(got, oracle.gather_plain(X, ids, w.index_span))
+    h.destroy()
+
+
+def test_weight_shape_stream_and_resident():
+    """configs[4] shape, small: strided column-tile groups; whole matrix gathered in order, and decoded from HBM."""
+    for rows, cols in ((256, 512), (96, 1408)):
+        w = workloads.WeightMatrix(rows, cols)
+        X = w.table()
+        h = ibp.ibp_build(X, 256, 1, w.group_param, align_bytes=16).upload_metadata(0)
+        ds = oracle.Dataset(X, 1, w.group_param)
+        ids = w.ids(0)
+        got = _gather(h, ids)
+        assert np.array_equal(got, ds.gather_decompress(ids))
+        assert np.array_equal(got, _u8(X))
+        assert np.array_equal(_resident(h, 0, w.n_rows), _u8(X))
+        h.destroy()
+
+
+def test_fig7_sweep_shapes():
+    """PAPER.md:399 microbenchmark shape: synthetic masks of chosen popcount; 256 B / 1 KB / 4 KB tensors, one group."""
+    for rb, savings in ((256, 0.1), (256, 0.9), (1024, 0.5), (1024, 0.95), (4096, 0.3), (4096, 0.9)):
+        w = workloads.Sweep(rb, savings, n_rows=3000)
+        X = w.table()
+        h = ibp.ibp_build(X, rb, 0, w.n_rows, align_bytes=32).upload_metadata(0)
+        m, b, k = h.metadata_host(0)
+        assert k <= 8 * rb - w.n_fixed + 0                                   # at least the chosen bits are invariant
+        ids = w.ids(0)
+        assert np.array_equal(_gather(h, ids), _u8(X)[ids])
+        h.destroy()
+
+
+def test_uncompressed_baseline_and_host_api():
+    w = workloads.Tiny()
+    X = w.table()
+    ids = w.ids(1)
+    pin = ibp.PinnedBuffer(X.nbytes)
+    pin.view(np.float32, X.shape)[:] = X
+    ids_d = _dev(ids)
+    out = torch.zeros((len(ids), 512), dtype=torch.uint8, device="cuda")
+    for order in (False, True):
+        out.zero_()
+        ibp.ibp_gather_uncompressed(pin.dev_ptr, 512, ids_d.data_ptr(), len(ids), out.data_ptr(),
+                                    torch.cuda.current_stream().cuda_stream, n_rows=w.n_rows, locality_order=order)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), oracle.gather_plain(X, ids))
+    # end-to-end entry point with host buffers
+    h = ibp.ibp_build(X, 512, 0, 64).upload_metadata(0)
+    out_h = np.zeros((len(ids), 512), np.uint8)
+    h.gather_decompress_host(ids, len(ids), out_h, torch.cuda.current_stream().cuda_stream)
+    assert np.array_equal(out_h, oracle.gather_plain(X, ids))
+    h.destroy()
+    pin.free()
+
+
+def test_configure_limits_grid_and_streams():
+    """SM-limited launch and a non-default stream give the same bytes."""
+    w = workloads.Tiny()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 64).upload_metadata(0)
+    ids = w.ids(2)
+    want = oracle.gather_plain(X, ids)
+    s = torch.cuda.Stream()
+    for ctas, warps in ((1, 1), (3, 2), (64, 8), (0, 16)):
+        h.configure(ctas, warps)
+        ids_d = _dev(ids)
+        out = torch.zeros((len(ids), 512), dtype=torch.uint8, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            h.gather_decompress(ids_d.data_ptr(), len(ids), out.data_ptr(), s.cuda_stream)
+        s.synchronize()
+        assert np.array_equal(out.cpu().numpy(), want)
+    h.destroy()

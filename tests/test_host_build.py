@@ -1,0 +1,140 @@
+"""CPU-only: the library's host compressor (ibp_build, S0/S0') against the independent oracle.
+
+The library keeps the canonical bit order, so Mask, Bitval, k_g AND the packed bytes of every row must equal the
+oracle's, and the oracle's unpacker must decode the library's store back to the original rows.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_30728_b200 import binding as ibp
+from paper_2605_30728_b200 import datagen, workloads
+
+
+def _check_against_oracle(X, kind, param, align, span=1, rows_to_check=None):
+    Xb = np.ascontiguousarray(X).view(np.uint8).reshape(X.shape[0], -1)
+    n, rb = Xb.shape
+    h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, index_span=span, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    ds = oracle.Dataset(Xb, kind, param)
+    info = h.info()
+    assert info.n_groups == ds.n_groups
+    assert info.metadata_bytes == ds.metadata_bytes == 2 * rb * ds.n_groups       # fixed size per group
+    assert info.packed_bytes_bytealigned == ds.packed_bytes                        # sum of ceil(k/8)
+    assert info.packed_bytes_rows >= info.packed_bytes_bytealigned
+    assert info.packed_bytes_stored >= info.packed_bytes_rows
+    for g in range(ds.n_groups):
+        m, b, k = h.metadata_host(g)
+        assert k == ds.k_bits(g)
+        assert np.array_equal(m, ds.mask(g)) and np.array_equal(b, ds.bitval(g))
+    A = info.align_bytes
+    rows = range(n) if rows_to_check is None else rows_to_check
+    for r in rows:
+        g = r // param if kind == 0 else r % param
+        data, k = h.packed_row(r)
+        want = ds.packed_row(r)
+        assert k == ds.k_bits(g)
+        assert data.size == -(-want.size // A) * A                                 # stride = roundup(ceil(k/8), A)
+        assert np.array_equal(data[: want.size], want)                             # canonical packed bytes
+        assert not data[want.size:].any()                                          # zero padding
+        assert np.array_equal(oracle.unpack_row(data, ds.mask(g), ds.bitval(g)), Xb[r])
+    # whole-range accessor: contiguous, starts at row 0, covers every row
+    ptr, nbytes = h.packed_range(0, n)
+    assert nbytes >= info.packed_bytes_rows and nbytes % 16 == 0
+    h.destroy()
+    ds.close()
+
+
+@pytest.mark.parametrize("align", [1, 4, 16, 32, 128])
+def test_tiny_blocked(align):
+    _check_against_oracle(workloads.Tiny(n_rows=512).table(), 0, 64, align)
+
+
+@pytest.mark.parametrize("kind,param,n,rb", [(0, 7, 50, 12), (0, 64, 1000, 64), (0, 1000, 10, 8), (1, 5, 203, 32),
+                                             (1, 8, 64, 16), (1, 3, 2, 4), (0, 1, 9, 20), (0, 16, 40, 4)])
+def test_small_shapes_ragged(kind, param, n, rb):
+    X = (datagen.random_bytes(n * rb, 5).reshape(n, rb) & 0x5A) | 0x21
+    _check_against_oracle(X, kind, param, 16)
+    _check_against_oracle(X, kind, param, 1)
+
+
+def test_workload_shapes():
+    g = workloads.GNN(n_rows=4096)
+    _check_against_oracle(g.table(), 0, 256, 32, rows_to_check=range(0, 4096, 37))
+    d = workloads.DLRM(rows_per_table=1024, n_tables=2)
+    _check_against_oracle(d.table(), 0, 128, 32, rows_to_check=range(0, 2048, 17))
+    kv = workloads.KV(layers=1, pages=4, heads=4)
+    _check_against_oracle(kv.table(), 0, 16, 16, span=64, rows_to_check=range(0, kv.n_rows, 5))
+    w = workloads.WeightMatrix(128, 512)
+    _check_against_oracle(w.table(), 1, 4, 16, rows_to_check=range(0, w.n_rows, 3))
+
+
+def test_degenerate_groups():
+    rb = 64
+    r = datagen.random_bytes(rb, 3)
+    same = np.repeat(r[None, :], 10, axis=0)                     # k = 0: nothing stored
+    h = ibp.ibp_build(same, rb, 0, 10, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    m, b, k = h.metadata_host(0)
+    assert k == 0 and np.all(m == 0xFF) and np.array_equal(b, r)
+    assert h.info().packed_bytes_rows == 0
+    h.destroy()
+    both = np.stack([r, ~r])                                     # no invariant bit: packed == raw (reading R13)
+    h = ibp.ibp_build(both, rb, 0, 2, align_bytes=1, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    m, b, k = h.metadata_host(0)
+    assert k == 8 * rb and not m.any() and not b.any()
+    for i in range(2):
+        data, _ = h.packed_row(i)
+        assert np.array_equal(data, both[i])
+    h.destroy()
+
+
+def test_soft_pext_fallback_matches(monkeypatch):
+    """63/64-bit fill edge cases of the word-wise packer: masks that make the accumulator wrap at every offset."""
+    rb = 64
+    for seed in range(40):
+        rng = np.random.default_rng(seed)
+        keep = rng.integers(0, 256, rb, dtype=np.uint8) | (0xFF if seed % 5 == 0 else 0)
+        base = datagen.random_bytes(rb, 100 + seed) & ~keep
+        rows = (datagen.random_bytes(8 * rb, 200 + seed).reshape(8, rb) & keep) | base
+        rows[0] = base
+        rows[1] = base | keep
+        _check_against_oracle(rows, 0, 8, 1)
+
+
+def test_argument_errors():
+    X = np.zeros((8, 16), np.uint8)
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X.reshape(-1)[:126].reshape(9, 14), 14, 0, 4)
+    assert e.value.status == 1                                   # row_bytes not a multiple of 4 (reading R11)
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X, 16, 0, 4, threshold=(4, 5))
+    assert e.value.status == 5                                   # thresholded mode is not on this path
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X, 16, 0, 4, align_bytes=48)
+    assert e.value.status == 1
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X, 16, 1, 4, index_span=2)
+    assert e.value.status == 1
+    h = ibp.ibp_build(X, 16, 0, 4, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    with pytest.raises(ibp.IbpError) as e:
+        h.packed_range(2, 4)                                     # must start a layout unit
+    assert e.value.status == 1
+    with pytest.raises(ibp.IbpError) as e:
+        h.gather_decompress(0, 1, 0)                             # before upload: BAD_STATE, never a silent fallback
+    assert e.value.status == 4
+    h.destroy()
+
+
+def test_batch_link_bytes():
+    w = workloads.Tiny(n_rows=256)
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 64, align_bytes=32, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    ids = np.array([0, 5, 5, 70, 255, 0], np.int64)
+    nu, stored, ba = h.batch_link_bytes(ids)
+    assert nu == 4
+    want_s = want_b = 0
+    for r in (0, 5, 70, 255):
+        data, k = h.packed_row(r)
+        want_s += data.size
+        want_b += (k + 7) // 8
+    assert (stored, ba) == (want_s, want_b)
+    h.destroy()
