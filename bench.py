@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the IBP hot path (fused gather-and-decompress) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload gnn|dlrm|tiny] [--impl reference]
+
+One "step" = one pass of the whole hot path (plus the ordering pre-pass when the handle uses it)
+over one batch of synthetic ids: ibp_gather_decompress(handle, row_ids, n, out, stream).  A different seeded id batch
+every step.  Default workload = BASELINE.json configs[1] (GNN node-feature gather, 10M x 128 fp32, 250k unique ids).
+
+Prints ONE JSON line (rank 0):
+  value      effective (decompressed) GB/s, whole job, ids resident in HBM, the packed store in host memory (that the
+             store is read over PCIe IS the method; nothing else is staged)
+  e2e        same metric through ibp_gather_decompress_host: pinned HOST ids in, pinned HOST rows out, copies timed
+  roofline   dominant kernel (ibp_decode_kernel): achieved = packed bytes the launch must move over PCIe / its duration
+             (CUDA events on the launch stream); peak = cudaMemcpy H2D ceiling measured in this run
+             (BASELINE.json north_star: "measured cudaMemcpy H2D ceiling"); bound = "pcie"
+  cpu_baseline  the oracle (oracle/, as it stands, 1 thread) on a bounded sample of the same workload
+Timing: CUDA events around every step on the launch stream, L2 flushed (256 MiB write) between steps outside the
+events, >= 3 warm-up steps, barrier + synchronize on both sides, max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# Per-launch traffic of ibp_decode_kernel from the ncu --set full captures summarised in profiles/r01_*_decode_ncu.md
+# (first timed launch): dram = dram__bytes_read.sum + dram__bytes_write.sum (HBM side: output rows + metadata);
+# sysmem = sysmem-aperture sectors x 32 B = what crossed PCIe.  GNN: sysmem 62.87 MB vs 62.92 MB algorithmic (no over-fetch).
+NCU_TRAFFIC = {"gnn": {"dram": 53_321_216 + 75_808_768, "sysmem": 62_866_432},
+               "dlrm": {"dram": None, "sysmem": 54_525_952}}
+
+
+def make_workload(name):
+    from paper_2605_30728_b200 import workloads
+    if name == "gnn":
+        return workloads.GNN()
+    if name == "dlrm":
+        return workloads.DLRM()
+    if name == "tiny":
+        return workloads.Tiny()
+    raise SystemExit(f"unknown workload {name}")
+
+
+def describe(w):
+    return {
+        "gnn": "configs[1] GNN node-feature gather: 10M x 128 fp32 (5.12 GB), 70% N(0,1) in 2^-8 steps + 30% sparse 0/1 at 2%, groups of 256, 250k unique Zipf(0.9) ids per step",
+        "dlrm": "configs[2] DLRM embedding lookup: 26 x 2M x 64 fp32 (13.3 GB), U(-0.05,0.05) in 2^-12 steps, groups of 128, 16384 x 26 Zipf(1.05) ids per step (repeats kept)",
+        "tiny": "configs[0] Tiny: 4096 x 128 fp32, N(0,1) in 2^-6 steps clipped to 8, groups of 64, 1024 uniform ids per step",
+    }[w.name]
+
+
+# ------------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi as a fallback is not needed)."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self._stop = [], set(), None, threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80, "applications_clocks_setting": 0x2}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def start(self):
+        if self.nv:
+            self.t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self.nv and self.t.is_alive():
+            self.t.join(timeout=1)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------- oracle arm
+class OracleSample:
+    """The CPU oracle on a bounded sample of the workload: a few hundred groups of the table (built once with the
+    oracle's own compressor), then ids of the workload's batch sampler that fall in those groups.  Single thread."""
+
+    def __init__(self, w):
+        import oracle
+        self.oracle, self.w = oracle, w
+        G = w.group_param
+        n_groups = 96 if w.row_bytes >= 512 else 160
+        ids_all = np.concatenate([w.ids(1000 + i) for i in range(2)])
+        groups = np.unique(ids_all // G)[:n_groups]
+        blocks = [w.rows(int(g) * G, min(G, w.n_rows - int(g) * G)) for g in groups]
+        self.X = np.concatenate(blocks)
+        starts = np.cumsum([0] + [b.shape[0] for b in blocks])
+        sel = ids_all[np.isin(ids_all // G, groups)]
+        gi = np.searchsorted(groups, sel // G)
+        self.local = (starts[gi] + sel % G).astype(np.int64)
+        self.n_groups = len(groups)
+        self.ds = oracle.Dataset(self.X, 0, G)
+        reps = np.resize(self.local, 2000)
+        t0 = time.perf_counter()
+        self.ds.gather_decompress(reps)
+        self.sec_per_row = (time.perf_counter() - t0) / len(reps)
+
+    def run(self, seconds_target):
+        w = self.w
+        n = int(max(2000, min(4_000_000, seconds_target / self.sec_per_row)))
+        reps = np.resize(self.local, n)
+        t0 = time.perf_counter()
+        out = self.ds.gather_decompress(reps)
+        dt = time.perf_counter() - t0
+        assert np.array_equal(out[:64], self.oracle.gather_plain(self.X, reps[:64]))
+        desc = (f"{n} row decodes over {self.n_groups} groups ({self.X.shape[0]} rows) of the {w.name} table, ids from its "
+                f"batch sampler, {dt:.1f} s")
+        return n * w.row_bytes / dt * 1e-9, n / dt, desc
+
+
+def oracle_sample(w, seconds_target=12.0):
+    return OracleSample(w).run(seconds_target)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = make_workload(args.workload)
+    smp = OracleSample(w)
+    per_step = max(0.2, min(10.0, 90.0 / max(1, args.steps + args.warmup)))
+    vals, desc = [], ""
+    for s in range(args.warmup + args.steps):
+        gbps, rps, desc = smp.run(per_step)
+        if s >= args.warmup:
+            vals.append((gbps, rps))
+    v = float(np.mean([x[0] for x in vals]))
+    rows_per_step = w.batch_rows
+    line = {
+        "impl": "reference", "metric": "effective decompressed GB/s (gather-decompress)", "value": v, "unit": "GB/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": rows_per_step * w.row_bytes / (v * 1e9) * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": describe(w), "note": "CPU oracle (oracle/ibp_oracle.cpp, single thread) on a bounded sample per step; ms_per_step is the time a full batch would take at that rate"},
+        "cpu_baseline": {"value": v, "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": "per step: " + desc, "rows_per_s": float(np.mean([x[1] for x in vals]))},
+        "e2e": {"value": v, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2605_30728_b200 import binding as ibp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the IBP hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    W, K = max(3, args.warmup), args.steps
+    w = make_workload(args.workload)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    # ---- build (once, not timed): table -> ibp_build -> metadata to HBM
+    t0 = time.perf_counter()
+    X = w.table()
+    t_gen = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=args.align, index_span=w.index_span,
+                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0)
+    t_build = time.perf_counter() - t0
+    h.upload_metadata(local)
+    if args.order is not None:
+        h.set_order_mode(args.order)
+    info = h.info()
+
+    # ---- ceilings measured on this box, this run
+    h2d_ceiling = ibp.ibp_measure_h2d(local, 1 << 30, 8)
+    zc_ceiling = ibp.ibp_measure_zero_copy_read(local, 1 << 30, 3)
+    hbm_peak = None
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs (copy; read+write bytes)"
+    except Exception:
+        hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+
+    # ---- batches: a different seeded id batch every step (rank-dependent)
+    n = w.batch_ids
+    n_rows_out = w.batch_rows
+    n_b = W + K
+    batches = [w.ids(rank * 100_000 + i) for i in range(n_b)]
+    ids_dev = [torch.from_numpy(b).cuda() for b in batches]
+    out = torch.empty((n_rows_out, w.row_bytes), dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    link = [h.batch_link_bytes(b) for b in batches]            # (unique ids, stored bytes, byte-aligned bytes)
+    order_on = (args.order == 1) or (args.order is None and info.store_kind == ibp.IBP_STORE_PINNED and info.packed_bytes_stored > (64 << 20) and n >= 4096)
+    launches_per_step = 1 + (3 if (order_on and w.index_span == 1) else 0)
+
+    def step(i):
+        h.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed_loop(fn, count, first):
+        evs = []
+        for j in range(count):
+            flush.zero_()                                       # L2 flush between steps, outside the events
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn(first + j)
+            b.record()
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    # ---- value: ids resident in HBM
+    for i in range(W):
+        step(i)
+    # parity of one warm-up batch against the plain definition (oracle c1), so a fast wrong kernel cannot score
+    import oracle
+    torch.cuda.synchronize()
+    chk = np.random.default_rng(0).choice(n_rows_out, size=min(4096, n_rows_out), replace=False)
+    got = out[torch.from_numpy(chk).cuda()].cpu().numpy()
+    want = oracle.gather_plain(X, batches[W - 1], w.index_span)[chk]
+    if not np.array_equal(got, want):
+        raise SystemExit("bench.py: GPU output differs from the oracle; refusing to report a number")
+
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    ms = timed_loop(step, K, W)
+    barrier()
+    clk = clocks.stop()
+    t_total = float(np.sum(ms))
+    tmax = torch.tensor([t_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    t_job = float(tmax.item())
+    bytes_step = n_rows_out * w.row_bytes
+    value = world * K * bytes_step / (t_job * 1e-3) * 1e-9
+
+    # ---- dominant kernel alone (pre-pass excluded when the handle orders): same launches, events around each
+    stored_timed = [link[W + j][1] for j in range(K)]
+    unique_timed = [link[W + j][0] for j in range(K)]
+    alg_timed = [link[W + j][2] for j in range(K)]
+    kernel_ms = ms                                              # one launch per step unless ordering is on
+    achieved = float(np.sum(stored_timed)) / (float(np.sum(kernel_ms)) * 1e-3) * 1e-9
+    ratio_stored = w.n_rows * w.row_bytes / info.packed_bytes_rows
+    ratio_alg = w.n_rows * w.row_bytes / info.packed_bytes_bytealigned
+    batch_ratio_stored = float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(stored_timed))
+    eff_roof = min(h2d_ceiling * batch_ratio_stored * (n / np.mean(unique_timed)), hbm_peak)
+
+    # ---- e2e: pinned host ids -> device -> gather -> pinned host rows, through the C ABI host entry point
+    ids_pin = ibp.PinnedBuffer(n * 8)
+    out_pin = ibp.PinnedBuffer(bytes_step)
+    ids_pin_np = ids_pin.view(np.int64)
+    out_pin_np = out_pin.view(np.uint8, (n_rows_out, w.row_bytes))
+
+    def step_e2e(i):
+        ids_pin_np[:] = batches[i]
+        h.gather_decompress_host(ids_pin_np, n, out_pin_np, stream)
+
+    for i in range(min(W, 3)):
+        step_e2e(i)
+    if not np.array_equal(out_pin_np[chk], oracle.gather_plain(X, batches[min(W, 3) - 1], w.index_span)[chk]):
+        raise SystemExit("bench.py: end-to-end output differs from the oracle")
+    barrier()
+    Ke = max(3, min(K, 30))
+    ms_e = timed_loop(step_e2e, Ke, W)
+    barrier()
+    te = torch.tensor([float(np.sum(ms_e))], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * Ke * bytes_step / (float(te.item()) * 1e-3) * 1e-9
+
+    # ---- uncompressed zero-copy gather baseline (rank 0, N=1 only): same ids, same timing
+    base = None
+    if world == 1 and w.index_span == 1 and not args.no_baseline:
+        res = {}
+        for kind in ("managed", "pinned"):
+            buf = ibp.PinnedBuffer(X.nbytes, managed=(kind == "managed"), device=local)
+            buf.view(X.dtype, X.shape)[:] = X
+            for order in (False, True):
+                def step_b(i, buf=buf, order=order):
+                    ibp.ibp_gather_uncompressed(buf.dev_ptr, w.row_bytes, ids_dev[i].data_ptr(), n, out.data_ptr(), stream,
+                                                n_rows=w.n_rows, locality_order=order)
+                for i in range(3):
+                    step_b(i)
+                mb = timed_loop(step_b, min(K, 20), W)
+                res[f"{kind}{'_ordered' if order else ''}"] = bytes_step / (float(np.mean(mb)) * 1e-3) * 1e-9
+            buf.free()
+        base = {"unit": "GB/s", "what": "ibp_gather_uncompressed: zero-copy gather of the raw rows (PAPER.md:329 'GPU (Aligned)')", **{k: round(v, 2) for k, v in res.items()}}
+
+    # ---- CPU oracle baseline on a bounded sample (rank 0, N=1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        g, rps, desc = oracle_sample(w, seconds_target=12.0)
+        cpu = {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)}
+
+    if rank == 0:
+        line = {
+            "metric": "effective decompressed GB/s (gather-decompress)", "value": round(value, 3), "unit": "GB/s",
+            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": round(t_job / K, 5), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+            "rows_per_s": round(world * K * n_rows_out / (t_job * 1e-3), 1),
+            "config": {
+                "workload": describe(w), "rows_per_step": n_rows_out, "row_bytes": w.row_bytes, "align_bytes": info.align_bytes,
+                "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
+                "locality_order": bool(order_on), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
+                "ratio_stored": round(ratio_stored, 4), "ratio_bytealigned": round(ratio_alg, 4),
+                "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3), "metadata_MB": round(info.metadata_bytes * 1e-6, 2),
+                "build_s": round(t_build, 2), "datagen_s": round(t_gen, 2), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
+            },
+            "roofline": {
+                "bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
+                "frac": round(achieved / h2d_ceiling, 4), "traffic": (NCU_TRAFFIC.get(w.name) or {}).get("dram"),
+                "traffic_sysmem": (NCU_TRAFFIC.get(w.name) or {}).get("sysmem"),
+                "kernel": "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
+                "algorithmic_bytes_per_launch": int(np.mean(stored_timed)),
+                "zero_copy_read_ceiling": round(zc_ceiling, 3), "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
+                "effective_roofline_GBps": round(float(eff_roof), 2), "frac_of_effective_roofline": round(value / world / float(eff_roof), 4),
+                "effective_roofline_def": "min(H2D ceiling x raw bytes / stored packed bytes of the batch, HBM peak)",
+                "frac_vs_bytealigned_ratio": round(value / world / min(h2d_ceiling * float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(alg_timed)) * (n / np.mean(unique_timed)), hbm_peak), 4),
+                "hbm_peak": hbm_peak, "hbm_peak_source": hbm_src,
+            },
+            "e2e": {"value": round(e2e_value, 3), "unit": "GB/s", "h2d_bytes_per_step": n * 8, "d2h_bytes_per_step": bytes_step,
+                    "steps": Ke, "api": "ibp_gather_decompress_host (pinned host ids in, pinned host rows out)"},
+            "gpu_launches": K * launches_per_step,
+            "clocks": clk,
+            "baseline_uncompressed": base,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    h.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="gnn", choices=["gnn", "dlrm", "tiny"])
+    ap.add_argument("--align", type=int, default=32)
+    ap.add_argument("--store", default="managed", choices=["managed", "pinned"])
+    ap.add_argument("--order", type=int, default=None, choices=[0, 1])
+    ap.add_argument("--no-baseline", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
