@@ -128,6 +128,11 @@ ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host
 ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_t first_row, int64_t n_rows,
                                    void* out_dev, void* cuda_stream);
 
+/* Zero-copy gather of the contiguous rows [first_row, first_row+n_rows) straight from the host store (whole weight
+ * matrices / layers streamed in order): same unit rule as above, no id list.  out_dev[j*row_bytes ...] = row
+ * first_row + j.  Asynchronous on the stream.                                                                      */
+ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream);
+
 /* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
 ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
 

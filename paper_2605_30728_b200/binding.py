@@ -52,6 +52,7 @@ SIGNATURES = {
     "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_decompress_resident": (_int, [_vp, _vp, _i64, _i64, _vp, _vp]),
+    "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
     "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
     "ibp_get_metadata_host": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_u32)]),
@@ -122,6 +123,9 @@ class Handle:
 
     def decompress_resident(self, packed_dev, first_row, n_rows, out_dev, stream=None):
         _check(lib().ibp_decompress_resident(self._h, _ptr(packed_dev), first_row, n_rows, _ptr(out_dev), stream))
+
+    def gather_decompress_range(self, first_row, n_rows, out_dev, stream=None):
+        _check(lib().ibp_gather_decompress_range(self._h, first_row, n_rows, _ptr(out_dev), stream))
 
     def packed_range(self, first_row, n_rows):
         p, nb = _vp(), _u64()

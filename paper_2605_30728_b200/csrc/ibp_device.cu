@@ -530,21 +530,12 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     return launch_decode(h, P, MODE_SPANS, st);
 }
 
-extern "C" ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream) {
-    ibp_status s = check_ready(h, "ibp_decompress_resident");
-    if (s != IBP_OK) return s;
-    if (n_rows == 0) return IBP_OK;
-    if (!packed_dev || !out_dev || first_row < 0 || n_rows < 0 || (uint64_t)(first_row + n_rows) > h->p.n_rows ||
-        ((uintptr_t)out_dev & 15u) || ((uintptr_t)packed_dev & 15u)) {
-        ibp_set_error("ibp_decompress_resident: bad argument (range, null pointer or alignment)");
-        return IBP_ERR_INVALID_ARG;
-    }
-    if ((uint64_t)first_row % h->p.group_param) { ibp_set_error("ibp_decompress_resident: first_row must be a multiple of %u", h->p.group_param); return IBP_ERR_INVALID_ARG; }
-    if (n_rows > 0xFFFFFFFFll) { ibp_set_error("ibp_decompress_resident: range too long"); return IBP_ERR_INVALID_ARG; }
-    cudaStream_t st = (cudaStream_t)cuda_stream;
+// Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
+// byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
+static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st) {
     DecodeParams P;
     fill_common(h, P);
-    P.store = (const uint8_t*)packed_dev;
+    P.store = packed;
     P.bias = ibp_row_offset(h, (uint64_t)first_row);
     P.out = (uint8_t*)out_dev;
     P.n = n_rows;
@@ -561,6 +552,36 @@ extern "C" ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_
     P.rows_per_unit = 16;
     P.n_units = (int64_t)(((n_mrows + P.rows_per_unit - 1) / P.rows_per_unit) * S);
     return launch_decode(h, P, MODE_STRIDED, st);
+}
+
+static ibp_status check_range(const ibp_handle* h, const char* who, int64_t first_row, int64_t n_rows, const void* out_dev) {
+    if (!out_dev || first_row < 0 || n_rows < 0 || (uint64_t)(first_row + n_rows) > h->p.n_rows || ((uintptr_t)out_dev & 15u)) {
+        ibp_set_error("%s: bad argument (range, null pointer or alignment)", who);
+        return IBP_ERR_INVALID_ARG;
+    }
+    if ((uint64_t)first_row % h->p.group_param) { ibp_set_error("%s: first_row must be a multiple of %u", who, h->p.group_param); return IBP_ERR_INVALID_ARG; }
+    if (n_rows > 0xFFFFFFFFll) { ibp_set_error("%s: range too long", who); return IBP_ERR_INVALID_ARG; }
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream) {
+    ibp_status s = check_ready(h, "ibp_decompress_resident");
+    if (s != IBP_OK) return s;
+    if (n_rows == 0) return IBP_OK;
+    if (!packed_dev || ((uintptr_t)packed_dev & 15u)) { ibp_set_error("ibp_decompress_resident: packed_dev must be a 16-byte aligned device pointer"); return IBP_ERR_INVALID_ARG; }
+    s = check_range(h, "ibp_decompress_resident", first_row, n_rows, out_dev);
+    if (s != IBP_OK) return s;
+    return decode_range(h, (const uint8_t*)packed_dev, first_row, n_rows, out_dev, (cudaStream_t)cuda_stream);
+}
+
+extern "C" ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream) {
+    ibp_status s = check_ready(h, "ibp_gather_decompress_range");
+    if (s != IBP_OK) return s;
+    if (n_rows == 0) return IBP_OK;
+    if (!h->store_dev) { ibp_set_error("ibp_gather_decompress_range: the packed store is not GPU-mapped (pageable store)"); return IBP_ERR_BAD_STATE; }
+    s = check_range(h, "ibp_gather_decompress_range", first_row, n_rows, out_dev);
+    if (s != IBP_OK) return s;
+    return decode_range(h, h->store_dev + ibp_row_offset(h, (uint64_t)first_row), first_row, n_rows, out_dev, (cudaStream_t)cuda_stream);
 }
 
 extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host, int64_t n, void* out_host, void* cuda_stream) {

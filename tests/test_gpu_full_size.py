@@ -1,0 +1,116 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs[1..4]), in the launch configuration bench.py times (library defaults).
+
+Every output row of a batch is compared, as raw bytes, with the plain definition out[i] = X[ids[i]] (oracle c1: a numpy
+gather of the original table), and the oracle codec (c2) is run on sampled groups the batch touches: Mask, Bitval, k must
+equal the library's, and the oracle's unpacker must decode the library's packed bytes of sampled rows to the original.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_30728_b200 import binding as ibp
+from paper_2605_30728_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _u8(X):
+    return X.view(np.uint8).reshape(X.shape[0], -1)
+
+
+def _check_codec_on_groups(h, X, group_ids, G, strided_S=None):
+    Xb = _u8(X)
+    for g in group_ids:
+        rows = Xb[g::strided_S] if strided_S else Xb[g * G:(g + 1) * G]
+        mask, bitval, k = oracle.group_masks(rows)
+        m, b, kk = h.metadata_host(int(g))
+        assert kk == k and np.array_equal(m, mask) and np.array_equal(b, bitval)
+        r = int(g) if strided_S else int(g) * G + (int(g) % rows.shape[0])
+        data, _ = h.packed_row(r)
+        want, _ = oracle.pack_row(Xb[r], mask)
+        assert np.array_equal(data[: want.size], want)
+        assert np.array_equal(oracle.unpack_row(data, mask, bitval), Xb[r])
+
+
+def _gather(h, ids, n_out_rows, rb):
+    st = torch.cuda.current_stream().cuda_stream
+    ids_d = torch.from_numpy(ids).cuda()
+    out = torch.empty((n_out_rows, rb), dtype=torch.uint8, device="cuda")
+    h.gather_decompress(ids_d.data_ptr(), len(ids), out.data_ptr(), st)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def test_full_gnn():
+    w = workloads.GNN()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 256, align_bytes=32).upload_metadata(0)
+    info = h.info()
+    assert info.n_groups == 39063 and info.metadata_bytes == 39063 * 1024
+    for it in (0, 1):
+        ids = w.ids(it)
+        assert len(ids) == 250_000 == len(np.unique(ids))
+        got = _gather(h, ids, len(ids), 512)
+        assert np.array_equal(got, oracle.gather_plain(X, ids))
+    touched = np.unique(w.ids(0) // 256)
+    _check_codec_on_groups(h, X, list(touched[:12]) + list(touched[-12:]) + [27343, 39062], 256)   # incl. the mixed and the short group
+    h.destroy()
+
+
+def test_full_dlrm():
+    w = workloads.DLRM()
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 128, align_bytes=32).upload_metadata(0)
+    assert h.info().n_groups == 406_250
+    ids = w.ids(0)
+    assert len(ids) == 16_384 * 26 and len(np.unique(ids)) < len(ids)
+    got = _gather(h, ids, len(ids), 256)
+    assert np.array_equal(got, oracle.gather_plain(X, ids))
+    touched = np.unique(ids // 128)
+    _check_codec_on_groups(h, X, list(touched[:10]) + list(touched[-10:]), 128)
+    h.destroy()
+
+
+def test_full_kv():
+    w = workloads.KV()
+    assert w.n_rows == 67_108_864 and w.index_span == 512 and w.batch_ids == 4096
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 16, align_bytes=16, index_span=512).upload_metadata(0)
+    assert h.info().n_groups == 4_194_304
+    ids = w.ids(0)
+    got = _gather(h, ids, len(ids) * 512, 256)
+    assert np.array_equal(got, oracle.gather_plain(X, ids, 512))
+    first_rows = ids[:6] * 512
+    _check_codec_on_groups(h, X, [int(r // 16) + j for r in first_rows for j in (0, 31)], 16)
+    # a staged page range decoded from HBM
+    st = torch.cuda.current_stream().cuda_stream
+    first, n = int(ids[3]) * 512, 4 * 512
+    ptr, nbytes = h.packed_range(first, n)
+    packed = torch.from_numpy(h.packed_view(ptr, nbytes).copy()).cuda()
+    out = torch.empty((n, 256), dtype=torch.uint8, device="cuda")
+    h.decompress_resident(packed.data_ptr(), first, n, out.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), _u8(X)[first:first + n])
+    h.destroy()
+
+
+@pytest.mark.parametrize("layer", [0, 31])
+def test_full_weight_layer(layer):
+    """One whole 7B-shaped decoder layer (7 matrices, 405 MB) streamed in order, zero-copy and staged+resident."""
+    st = torch.cuda.current_stream().cuda_stream
+    for w in workloads.weight_layer(layer):
+        X = w.table()
+        h = ibp.ibp_build(X, 256, 1, w.group_param, align_bytes=16).upload_metadata(0)
+        out = torch.empty((w.n_rows, 256), dtype=torch.uint8, device="cuda")
+        h.gather_decompress_range(0, w.n_rows, out.data_ptr(), st)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), _u8(X))
+        ptr, nbytes = h.packed_range(0, w.n_rows)
+        packed = torch.from_numpy(h.packed_view(ptr, nbytes).copy()).cuda()
+        out.zero_()
+        h.decompress_resident(packed.data_ptr(), 0, w.n_rows, out.data_ptr(), st)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), _u8(X))
+        _check_codec_on_groups(h, X, [0, w.group_param - 1], None, strided_S=w.group_param)
+        h.destroy()

@@ -37,6 +37,13 @@ def _resident(h, first, n):
     return out.cpu().numpy()[:n]
 
 
+def _range(h, first, n):
+    out = torch.full((max(1, n), h.info().row_bytes), 0x3C, dtype=torch.uint8, device="cuda")
+    h.gather_decompress_range(first, n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()[:n]
+
+
 def _u8(X):
     X = np.ascontiguousarray(X)
     return X.view(np.uint8).reshape(X.shape[0], -1)
@@ -82,6 +89,7 @@ def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
             h.set_order_mode(mode)
             assert np.array_equal(_gather(h, ids), want)
         assert np.array_equal(_resident(h, 0, n), X)                    # whole table from HBM
+        assert np.array_equal(_range(h, 0, n), X)                       # whole table zero-copy, no id list
     if kind == 0 and n > 2 * param:
         first = param * ((n // param) // 2)
         assert np.array_equal(_resident(h, first, n - first), X[first:])
@@ -180,6 +188,9 @@ def test_weight_shape_stream_and_resident():
         assert np.array_equal(got, ds.gather_decompress(ids))
         assert np.array_equal(got, _u8(X))
         assert np.array_equal(_resident(h, 0, w.n_rows), _u8(X))
+        assert np.array_equal(_range(h, 0, w.n_rows), _u8(X))
+        half = (w.mat_rows // 2) * w.group_param
+        assert np.array_equal(_range(h, half, w.n_rows - half), _u8(X)[half:])
         h.destroy()
 
 
