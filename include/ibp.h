@@ -180,6 +180,10 @@ ibp_status ibp_set_order_mode(ibp_handle* h, int mode);
  * 0 = 16-byte cp.async through the load/store unit.  Results are identical either way.                              */
 ibp_status ibp_set_fetch_mode(ibp_handle* h, int mode);
 
+/* Tuning/test hook: contiguous runs (spans, ranges, resident decode): 1 = TMA producer/consumer stream kernel (default),
+ * 0 = per-row fetch kernel.  Results are identical either way.                                                       */
+ibp_status ibp_set_stream_mode(ibp_handle* h, int mode);
+
 /* Tuning/test hook: rows each warp keeps in flight in random gathers (ring depth): 1, 2 or 4.                       */
 ibp_status ibp_set_rows_in_flight(ibp_handle* h, int n);
 

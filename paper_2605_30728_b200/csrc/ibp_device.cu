@@ -137,6 +137,12 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+__device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t group_shift, uint64_t id) {
+    return group_shift != 0xFFFFFFFFu ? (id >> group_shift) : (id / group_param);
+}
+
+#include "ibp_stream.cuh"
+
 template <int W, int NST, int MODE, int FETCH>
 __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -444,6 +450,86 @@ static void fill_common(const ibp_handle* h, DecodeParams& P) {
     if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t s = 0; while ((1u << s) < h->p.group_param) ++s; P.group_shift = s; }
 }
 
+// ------------------------------------------------------------------------------------------------ stream launch
+// Contiguous runs of rows (spans of blocked groups, whole ranges of either kind) through the TMA producer/consumer
+// pipeline of ibp_stream.cuh.  `packed` is the device-visible address of byte `bias` of the packed store.
+template <int W, int NS>
+static ibp_status launch_stream_one(const StreamParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
+    constexpr int NW = 8;
+    auto kern = ibp_stream_kernel<W, NS, NW>;
+    static thread_local size_t attr_smem = 0;
+    if (smem > 48 * 1024 && smem > attr_smem) {
+        IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    int occ = 0;
+    IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
+    int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
+    if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
+    kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(P);
+    IBP_CUDA(cudaGetLastError());
+    return IBP_OK;
+}
+
+static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
+                                int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st) {
+    if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+    const int W = pick_W(h->p.row_bytes);
+    const uint32_t NW = 8;
+    StreamParams P;
+    memset(&P, 0, sizeof P);
+    P.store = packed; P.bias = bias;
+    P.meta = h->meta_dev; P.mvtab = h->mvtab_dev; P.gtab = h->gtab_dev;
+    P.ids = ids_dev; P.out = (uint8_t*)out_dev;
+    P.first_row = first_row; P.span_rows = span_rows;
+    P.row_stride_strided = h->row_stride_strided;
+    P.row_bytes = h->p.row_bytes; P.n_words = h->n_words;
+    P.n_pass = (h->n_words + 32 * W - 1) / (32 * W);
+    P.group_param = h->p.group_param;
+    P.group_shift = 0xFFFFFFFFu;
+    if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t sft = 0; while ((1u << sft) < h->p.group_param) ++sft; P.group_shift = sft; }
+    P.strided = h->p.group_kind == IBP_GROUP_STRIDED;
+    const uint64_t G = h->p.group_param;
+    uint64_t need;                                   // bytes one stage must hold
+    if (!P.strided) {
+        uint32_t U = (uint32_t)std::min<uint64_t>(G, 16);
+        if (G % U) U = 16;
+        const uint64_t stride = std::max<uint32_t>(h->max_stride, 16u);
+        uint64_t rc = std::min<uint64_t>((uint64_t)NW * U, (48ull * 1024) / stride);
+        rc = std::max<uint64_t>(rc, 1);
+        if (rc >= U) rc = rc / U * U; else U = (uint32_t)rc;
+        rc = (uint64_t)std::min<int64_t>((int64_t)rc, span_rows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = U;
+        need = rc * h->max_stride + (rc / G + 2) * 128 + 64;
+        P.chunks_per_span = (uint32_t)((span_rows + (int64_t)rc - 1) / (int64_t)rc);
+    } else {
+        const uint64_t rs = h->row_stride_strided;
+        const uint64_t cap = rs > 8192 ? 64ull * 1024 : 48ull * 1024;
+        uint64_t rc = std::max<uint64_t>(1, (cap - 64) / std::max<uint64_t>(rs, 16));
+        const int64_t n_mrows = (span_rows + (int64_t)G - 1) / (int64_t)G;
+        rc = (uint64_t)std::min<int64_t>((int64_t)rc, n_mrows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = (uint32_t)rc;
+        need = rc * rs + 64;
+        P.chunks_per_span = (uint32_t)((n_mrows + (int64_t)rc - 1) / (int64_t)rc);
+    }
+    P.stage_bytes = (uint32_t)((need + 127) / 128 * 128);
+    P.n_chunks = n_spans * (int64_t)P.chunks_per_span;
+    const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
+    const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
+    if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
+#define IBP_STREAM(W_)                                                                          \
+    return ns == 2 ? launch_stream_one<W_, 2>(P, h->max_ctas, h->sm_count, smem, st)            \
+                   : launch_stream_one<W_, 3>(P, h->max_ctas, h->sm_count, smem, st)
+    switch (W) {
+        case 4: IBP_STREAM(4);
+        case 2: IBP_STREAM(2);
+        default: IBP_STREAM(1);
+    }
+#undef IBP_STREAM
+}
+
 static ibp_status check_ready(const ibp_handle* h, const char* who) {
     if (!h) { ibp_set_error("%s: null handle", who); return IBP_ERR_INVALID_ARG; }
     if (h->device < 0 || !h->meta_dev) { ibp_set_error("%s: call ibp_upload_metadata first", who); return IBP_ERR_BAD_STATE; }
@@ -467,6 +553,13 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
     IBP_CUDA(cudaMalloc((void**)&h->gtab_dev, h->gtab.size() * sizeof(IbpGroupEntry)));
     IBP_CUDA(cudaMemcpyAsync(h->meta_dev, h->meta.data(), h->meta.size() * 4, cudaMemcpyHostToDevice, st));
     IBP_CUDA(cudaMemcpyAsync(h->gtab_dev, h->gtab.data(), h->gtab.size() * sizeof(IbpGroupEntry), cudaMemcpyHostToDevice, st));
+    // expand move masks per (group, word) when the table has few groups (strided column tiles, small tables): 20 B per word
+    if (h->n_groups * (uint64_t)h->n_words * 20ull <= (8ull << 20)) {
+        const uint64_t cells = h->n_groups * (uint64_t)h->n_words;
+        IBP_CUDA(cudaMalloc((void**)&h->mvtab_dev, cells * 20));
+        ibp_build_mvtab<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(h->meta_dev, h->n_words, h->n_groups, h->mvtab_dev);
+        IBP_CUDA(cudaGetLastError());
+    }
     IBP_CUDA(cudaStreamSynchronize(st));
     h->sm_count = prop.multiProcessorCount;
     if (h->store_kind == IBP_STORE_PINNED && !h->store_dev) {
@@ -521,7 +614,9 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
         if (ws) IBP_CUDA(cudaFreeAsync(ws, st));
         return s;
     }
-    // spans of blocked groups: R consecutive rows per warp, never crossing a group needlessly
+    if (h->stream_mode)
+        return launch_stream(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
+    // (fallback) spans of blocked groups: R consecutive rows per warp, never crossing a group needlessly
     const uint32_t G = h->p.group_param;
     P.rows_per_unit = std::min<uint32_t>(std::min<uint32_t>(G, 16u), h->p.index_span);
     if (G % P.rows_per_unit) P.rows_per_unit = std::min<uint32_t>(16u, h->p.index_span);
@@ -533,6 +628,8 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
 // byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
 static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st) {
+    if (h->stream_mode)
+        return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     DecodeParams P;
     fill_common(h, P);
     P.store = packed;
@@ -758,6 +855,13 @@ static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps
 }
 extern "C" ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, false); }
 extern "C" ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, true); }
+
+// Test/tuning hook: 1 = contiguous runs through the TMA producer/consumer stream kernel (default), 0 = per-row fetch.
+extern "C" ibp_status ibp_set_stream_mode(ibp_handle* h, int mode) {
+    if (!h || mode < 0 || mode > 1) { ibp_set_error("ibp_set_stream_mode: bad argument"); return IBP_ERR_INVALID_ARG; }
+    h->stream_mode = mode;
+    return IBP_OK;
+}
 
 // Test/tuning hook: engine for the packed-row fetch: 0 = cp.async through the LSU, 1 = cp.async.bulk (TMA) + mbarrier.
 extern "C" ibp_status ibp_set_rows_in_flight(ibp_handle* h, int nst) {

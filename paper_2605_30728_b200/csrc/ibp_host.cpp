@@ -380,6 +380,7 @@ extern "C" void ibp_destroy(ibp_handle* h) {
     if (!h) return;
     if (h->meta_dev) cudaFree(h->meta_dev);
     if (h->gtab_dev) cudaFree(h->gtab_dev);
+    if (h->mvtab_dev) cudaFree(h->mvtab_dev);
     if (h->store) {
         if (h->store_kind == IBP_STORE_PINNED) cudaFreeHost(h->store);
         else if (h->store_kind == IBP_STORE_MANAGED_HOST) cudaFree(h->store);

@@ -36,12 +36,14 @@ struct ibp_handle {
     int device = -1;
     uint32_t* meta_dev = nullptr;
     IbpGroupEntry* gtab_dev = nullptr;
+    uint32_t* mvtab_dev = nullptr;         // optional expand move masks, 5 per (group, word)
 
     // launch configuration
     uint32_t max_ctas = 0, warps_per_cta = 0;
     int sm_count = 0;
     int order_mode = -1;                   // -1 auto, 0 off, 1 on (locality-ordered gather)
     int rows_in_flight = 2;                // random gathers: rows each warp keeps in flight (1, 2 or 4)
+    int stream_mode = 1;                   // contiguous runs: 1 = TMA pipeline stream kernel, 0 = per-row fetch
     int fetch_mode = 1;                    // 0 = cp.async (LSU), 1 = cp.async.bulk (TMA)
 };
 

@@ -1,0 +1,220 @@
+// ibp_stream.cuh -- decode of CONTIGUOUS runs of rows (KV page spans, whole weight matrices, resident ranges).
+//
+// A warp-specialised TMA pipeline (the Blackwell idiom; PAPER.md:213's shared-memory workspace + asynchronous reads):
+//   producer  one elected lane of the last warp: for every chunk (a run of consecutive rows = one contiguous byte
+//             range of the packed store) waits for the stage to be free (empty mbarrier), arms the full mbarrier with
+//             the byte count and issues large cp.async.bulk copies (<= 16 KB each) of the 16-byte-aligned cover.
+//             Host store: the link sees long contiguous reads instead of one short read per row.  HBM source: same code.
+//   consumers NW warps wait on the full mbarrier, decode "pieces" of the chunk (rows of one group: Mask/Bitval, bit
+//             offsets and the five bit-expand move masks live in registers for the whole piece), then release the stage.
+// Bit re-insertion (S5) is the branch-free 5-stage expand of Hacker's Delight 7-5 (x = (x & ~mv_i) | ((x << 2^i) & mv_i)):
+// 11 integer ops per 32-bit word whatever the mask looks like, with the move masks computed once per piece, or loaded
+// from a per-group table built at upload time when the table has few groups (strided column-tile tables).
+#pragma once
+
+struct StreamParams {
+    const uint8_t* store;          // device-visible packed bytes; row at store + offset(id) - bias
+    uint64_t bias;
+    const uint32_t* meta;          // per group: Mask words, Bitval words
+    const uint32_t* mvtab;         // optional: per group, per word: 5 expand move masks (n_words * 5), else nullptr
+    const IbpGroupEntry* gtab;
+    const int64_t* ids;            // span gather: one id per span; nullptr: a single range
+    uint8_t* out;
+    int64_t first_row;             // range mode: first row id
+    int64_t span_rows;             // rows per span / rows of the range
+    int64_t n_chunks;
+    uint64_t row_stride_strided;
+    uint32_t chunks_per_span, rows_per_chunk, piece_rows;
+    uint32_t row_bytes, n_words, n_pass;
+    uint32_t group_param, group_shift, strided;
+    uint32_t stage_bytes;
+};
+
+// The five move masks of the parallel-suffix expand for deposit positions nv (set bits = positions to fill, lowest first).
+__device__ __forceinline__ void expand_masks(uint32_t nv, uint32_t mv[5]) {
+    uint32_t m = nv, mk = ~nv << 1;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        uint32_t mp = mk ^ (mk << 1);
+        mp ^= mp << 2;
+        mp ^= mp << 4;
+        mp ^= mp << 8;
+        mp ^= mp << 16;
+        const uint32_t v = mp & m;
+        mv[i] = v;
+        m = (m ^ v) | (v >> (1 << i));
+        mk &= ~mp;
+    }
+}
+__device__ __forceinline__ uint32_t expand_bits(uint32_t x, const uint32_t mv[5]) {
+#pragma unroll
+    for (int i = 4; i >= 0; --i) x = (x & ~mv[i]) | ((x << (1 << i)) & mv[i]);
+    return x;
+}
+
+// Fills mvtab for groups [0, n_groups): one thread per (group, word).
+__global__ void ibp_build_mvtab(const uint32_t* __restrict__ meta, uint32_t n_words, uint64_t n_groups, uint32_t* __restrict__ mvtab) {
+    const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+    if (i >= n_groups * n_words) return;
+    const uint64_t g = i / n_words, w = i - g * n_words;
+    uint32_t mv[5];
+    expand_masks(~meta[g * 2ull * n_words + w], mv);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) mvtab[i * 5 + k] = mv[k];
+}
+
+template <int W, int NS, int NW>
+__global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const StreamParams P) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t full_s = smem_s + NS * P.stage_bytes, empty_s = full_s + NS * 8;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) { mbar_init(full_s + s * 8, 1); mbar_init(empty_s + s * 8, NW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint64_t S = P.group_param;
+
+    // chunk c -> first row id, rows (blocked) or matrix rows (strided), first output row, packed byte range
+    auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0, uint64_t& b0, uint64_t& b1) {
+        const int64_t si = c / P.chunks_per_span;
+        const int64_t cc = c - si * P.chunks_per_span;
+        const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
+        if (!P.strided) {
+            const int64_t r = cc * P.rows_per_chunk;
+            row0 = span_first + r;
+            nrows = (uint32_t)min((int64_t)P.rows_per_chunk, P.span_rows - r);
+            out0 = si * P.span_rows + r;
+            const uint64_t g0 = group_of_u(P.group_param, P.group_shift, (uint64_t)row0);
+            const uint64_t last = (uint64_t)row0 + nrows - 1, g1 = group_of_u(P.group_param, P.group_shift, last);
+            const IbpGroupEntry e0 = P.gtab[g0];
+            const IbpGroupEntry e1 = g1 == g0 ? e0 : P.gtab[g1];
+            b0 = e0.base + ((uint64_t)row0 - g0 * S) * e0.stride;
+            b1 = e1.base + (last - g1 * S) * e1.stride + e1.stride;
+        } else {
+            const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
+            const int64_t mr = cc * P.rows_per_chunk;
+            nrows = (uint32_t)min((int64_t)P.rows_per_chunk, n_mrows - mr);
+            row0 = span_first + mr * (int64_t)S;
+            out0 = si * P.span_rows + mr * (int64_t)S;
+            b0 = ((uint64_t)row0 / S) * P.row_stride_strided;
+            b1 = b0 + (uint64_t)nrows * P.row_stride_strided;
+        }
+    };
+
+    if (wib == NW) {
+        // ------------------------------------------------------------------ producer
+        if (lane != 0) return;
+        uint32_t k = 0;
+        for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+            const uint32_t s = k % NS;
+            mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
+            int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;
+            chunk_geom(c, row0, nrows, out0, b0, b1);
+            const uint8_t* src = P.store + (b0 - P.bias);
+            const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
+            const uint32_t bytes = (uint32_t)((head + (b1 - b0) + 15u) & ~15ull);
+            mbar_expect_tx(full_s + s * 8, bytes);
+            const uint32_t dst = smem_s + s * P.stage_bytes;
+            for (uint32_t o = 0; o < bytes; o += 16384u)
+                bulk_g2s(dst + o, src - head + o, min(16384u, bytes - o), full_s + s * 8);
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumers
+    uint32_t m[W], b[W], ex[W], mv[W][5];
+    uint64_t prep_g = ~0ull;
+    uint32_t k = 0;
+    for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+        const uint32_t s = k % NS;
+        int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;
+        chunk_geom(c, row0, nrows, out0, b0, b1);
+        const uint32_t head = (uint32_t)((uintptr_t)(P.store + (b0 - P.bias)) & 15u);
+        const uint32_t* stage = (const uint32_t*)(smem + (size_t)s * P.stage_bytes);
+        bool waited = false;
+
+        // Decode one row whose packed bytes start at byte `roff` of the stage; metadata of group g.
+        auto decode_row = [&](uint64_t g, uint32_t roff, uint8_t* orow) {
+            const uint32_t* gm = P.meta + g * 2ull * P.n_words;
+            uint32_t carry = 0;
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                const bool active = w0 < P.n_words;
+                if (P.n_pass > 1 || g != prep_g) {
+                    // ---- S2 + S4 once per piece: metadata, bit offsets, expand masks
+                    if (active) { VecIO<W>::ld(gm + w0, m); VecIO<W>::ld(gm + P.n_words + w0, b); }
+                    else {
+#pragma unroll
+                        for (int q = 0; q < W; ++q) { m[q] = 0xFFFFFFFFu; b[q] = 0; }
+                    }
+                    uint32_t t = 0;
+#pragma unroll
+                    for (int q = 0; q < W; ++q) { ex[q] = t; t += __popc(~m[q]); }
+                    const uint32_t incl = warp_inclusive_scan(t, lane);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) ex[q] += incl - t + carry;
+                    carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
+                    if (P.mvtab && active) {
+                        const uint32_t* tv = P.mvtab + (g * P.n_words + w0) * 5ull;
+#pragma unroll
+                        for (int q = 0; q < W; ++q)
+#pragma unroll
+                            for (int i = 0; i < 5; ++i) mv[q][i] = __ldg(tv + q * 5 + i);
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < W; ++q) expand_masks(~m[q], mv[q]);
+                    }
+                    prep_g = g;
+                }
+                if (!waited) { mbar_wait(full_s + s * 8, (k / NS) & 1u); waited = true; }
+                // ---- S5: extract k bits at the word's bit offset, expand, OR Bitval
+                const uint32_t rowbits = roff * 8u;
+                uint32_t o[W];
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    const uint32_t bit = rowbits + ex[q];
+                    const uint32_t wq = bit >> 5;
+                    const uint32_t x = __funnelshift_r(stage[wq], stage[wq + 1], bit);
+                    o[q] = (expand_bits(x, mv[q]) & ~m[q]) | b[q];
+                }
+                if (active) VecIO<W>::st(orow + (size_t)w0 * 4, o);   // ---- S6
+            }
+        };
+
+        if (!P.strided) {
+            const uint32_t U = P.piece_rows, n_pieces = (nrows + U - 1) / U;
+            for (uint32_t p = wib; p < n_pieces; p += NW) {
+                const uint32_t j0 = p * U, j1 = min(nrows, j0 + U);
+                uint64_t g = ~0ull; uint32_t roff = 0, stride = 0; uint64_t g_end = 0;
+                for (uint32_t j = j0; j < j1; ++j) {
+                    const uint64_t id = (uint64_t)row0 + j;
+                    if (g == ~0ull || id >= g_end) {
+                        g = group_of_u(P.group_param, P.group_shift, id);
+                        const IbpGroupEntry e = P.gtab[g];
+                        stride = e.stride;
+                        roff = head + (uint32_t)(e.base + (id - g * S) * e.stride - b0);
+                        g_end = (g + 1) * S;
+                    }
+                    decode_row(g, roff, P.out + (uint64_t)(out0 + j) * P.row_bytes);
+                    roff += stride;
+                }
+            }
+        } else {
+            const int64_t id_end = (P.ids ? 0 : P.first_row) + P.span_rows;   // strided tables are decoded as ranges only
+            for (uint32_t t = wib; t < (uint32_t)S; t += NW) {
+                const IbpGroupEntry e = P.gtab[t];
+                for (uint32_t j = 0; j < nrows; ++j) {
+                    const int64_t id = row0 + (int64_t)j * (int64_t)S + t;
+                    if (id >= id_end) break;
+                    decode_row(t, head + (uint32_t)(j * P.row_stride_strided + e.base), P.out + (uint64_t)(out0 + (int64_t)j * (int64_t)S + t) * P.row_bytes);
+                }
+            }
+        }
+        if (!waited) mbar_wait(full_s + s * 8, (k / NS) & 1u);   // a warp without a piece still has to follow the phases
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+    }
+}

@@ -88,8 +88,10 @@ def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
         for mode in (0, 1):
             h.set_order_mode(mode)
             assert np.array_equal(_gather(h, ids), want)
-        assert np.array_equal(_resident(h, 0, n), X)                    # whole table from HBM
-        assert np.array_equal(_range(h, 0, n), X)                       # whole table zero-copy, no id list
+        for sm in (0, 1):                                               # per-row fetch kernel / TMA stream kernel
+            h.set_stream_mode(sm)
+            assert np.array_equal(_resident(h, 0, n), X)                # whole table from HBM
+            assert np.array_equal(_range(h, 0, n), X)                   # whole table zero-copy, no id list
     if kind == 0 and n > 2 * param:
         first = param * ((n // param) // 2)
         assert np.array_equal(_resident(h, first, n - first), X[first:])
@@ -170,9 +172,11 @@ def test_kv_shape_spans():
     h = ibp.ibp_build(X, 256, 0, 16, align_bytes=16, index_span=w.index_span).upload_metadata(0)
     ds = oracle.Dataset(X, 0, 16)
     ids = w.ids(0)
-    got = _gather(h, ids, span=w.index_span)
-    assert np.array_equal(got, ds.gather_decompress(ids, w.index_span))
-    assert np.array_equal(got, oracle.gather_plain(X, ids, w.index_span))
+    for sm in (0, 1):
+        h.set_stream_mode(sm)
+        got = _gather(h, ids, span=w.index_span)
+        assert np.array_equal(got, ds.gather_decompress(ids, w.index_span))
+        assert np.array_equal(got, oracle.gather_plain(X, ids, w.index_span))
     h.destroy()
 
 
