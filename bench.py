@@ -47,6 +47,8 @@ def make_workload(name):
         return workloads.DLRM()
     if name == "tiny":
         return workloads.Tiny()
+    if name == "kv":
+        return workloads.KV()
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -55,6 +57,7 @@ def describe(w):
         "gnn": "configs[1] GNN node-feature gather: 10M x 128 fp32 (5.12 GB), 70% N(0,1) in 2^-8 steps + 30% sparse 0/1 at 2%, groups of 256, 250k unique Zipf(0.9) ids per step",
         "dlrm": "configs[2] DLRM embedding lookup: 26 x 2M x 64 fp32 (13.3 GB), U(-0.05,0.05) in 2^-12 steps, groups of 128, 16384 x 26 Zipf(1.05) ids per step (repeats kept)",
         "tiny": "configs[0] Tiny: 4096 x 128 fp32, N(0,1) in 2^-6 steps clipped to 8, groups of 64, 1024 uniform ids per step",
+        "kv": "configs[3] LLM KV-cache offload: bf16 K/V, 32 layers x 32 heads x head_dim 128, 16-token pages, 8 x 4096 tokens (17.2 GB); K~N(0,1), V~N(0,0.5); group = one page of one head; 64 random pages per layer fetched per step (4096 spans of 512 rows, 512 MiB out)",
     }[w.name]
 
 
@@ -112,6 +115,8 @@ class OracleSample:
         G = w.group_param
         n_groups = 96 if w.row_bytes >= 512 else 160
         ids_all = np.concatenate([w.ids(1000 + i) for i in range(2)])
+        if w.index_span > 1:                                   # span ids -> row ids (first spans only: bounded sample)
+            ids_all = (ids_all[:8, None] * w.index_span + np.arange(w.index_span)[None, :]).reshape(-1)
         groups = np.unique(ids_all // G)[:n_groups]
         blocks = [w.rows(int(g) * G, min(G, w.n_rows - int(g) * G)) for g in groups]
         self.X = np.concatenate(blocks)
@@ -193,12 +198,15 @@ def run_cuda(args):
     X = w.table()
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
-    h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=args.align, index_span=w.index_span,
+    align = args.align if args.align else w.align_bytes
+    h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
                       flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0)
     t_build = time.perf_counter() - t0
     h.upload_metadata(local)
     if args.order is not None:
         h.set_order_mode(args.order)
+    if args.decode_ctas:
+        h.configure(args.decode_ctas, 0)
     info = h.info()
 
     # ---- ceilings measured on this box, this run
@@ -306,15 +314,15 @@ def run_cuda(args):
 
     # ---- uncompressed zero-copy gather baseline (rank 0, N=1 only): same ids, same timing
     base = None
-    if world == 1 and w.index_span == 1 and not args.no_baseline:
+    if world == 1 and not args.no_baseline:
         res = {}
         for kind in ("managed", "pinned"):
             buf = ibp.PinnedBuffer(X.nbytes, managed=(kind == "managed"), device=local)
             buf.view(X.dtype, X.shape)[:] = X
-            for order in (False, True):
+            for order in ((False, True) if w.index_span == 1 else (False,)):
                 def step_b(i, buf=buf, order=order):
-                    ibp.ibp_gather_uncompressed(buf.dev_ptr, w.row_bytes, ids_dev[i].data_ptr(), n, out.data_ptr(), stream,
-                                                n_rows=w.n_rows, locality_order=order)
+                    ibp.ibp_gather_uncompressed(buf.dev_ptr, w.row_bytes * w.index_span, ids_dev[i].data_ptr(), n, out.data_ptr(), stream,
+                                                n_rows=w.n_rows // w.index_span, locality_order=order)
                 for i in range(3):
                     step_b(i)
                 mb = timed_loop(step_b, min(K, 20), W)
@@ -346,7 +354,7 @@ def run_cuda(args):
                 "bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
                 "frac": round(achieved / h2d_ceiling, 4), "traffic": (NCU_TRAFFIC.get(w.name) or {}).get("dram"),
                 "traffic_sysmem": (NCU_TRAFFIC.get(w.name) or {}).get("sysmem"),
-                "kernel": "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
+                "kernel": "ibp_stream_kernel" if w.index_span > 1 else "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
                 "algorithmic_bytes_per_launch": int(np.mean(stored_timed)),
                 "zero_copy_read_ceiling": round(zc_ceiling, 3), "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
                 "effective_roofline_GBps": round(float(eff_roof), 2), "frac_of_effective_roofline": round(value / world / float(eff_roof), 4),
@@ -367,21 +375,172 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------- weight streaming
+def run_weights(args):
+    """BASELINE configs[4]: bf16 matrices of a 7B-shaped decoder (4 x 4096x4096 + 3 x 4096x11008 per layer) held packed in
+    host memory; one step = one whole layer streamed in order (7 x ibp_gather_decompress_range), and, with the overlap
+    harness (S7), layer l+1's fetch against a consumer GEMM ([M,4096] activation x the 7 matrices) on layer l."""
+    import torch
+    from paper_2605_30728_b200 import binding as ibp, workloads
+    from paper_2605_30728_b200.overlap import DoubleBufferedPipeline, summarize
+    import oracle
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --workload weights runs on one GPU")
+    torch.cuda.set_device(0)
+    W, K, L = max(3, args.warmup), args.steps, args.layers
+    t0 = time.perf_counter()
+    layers, raw_bytes, stored, bytealigned = [], 0, 0, 0
+    check = None
+    for l in range(L):
+        mats = []
+        for wm in workloads.weight_layer(l):
+            X = wm.table()
+            h = ibp.ibp_build(X, 256, 1, wm.group_param, align_bytes=args.align if args.align else 16,
+                              flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0).upload_metadata(0)
+            if args.decode_ctas:
+                h.configure(args.decode_ctas, 0)
+            info = h.info()
+            raw_bytes += X.nbytes; stored += info.packed_bytes_rows; bytealigned += info.packed_bytes_bytealigned
+            mats.append((h, wm.n_rows, wm.mat_rows, wm.mat_cols))
+            if l == L - 1 and wm.slot == 6:
+                check = X.view(np.uint8).reshape(wm.n_rows, -1).copy()
+        layers.append(mats)
+    t_build = time.perf_counter() - t0
+    layer_rows = sum(m[1] for m in layers[0])
+    layer_bytes = layer_rows * 256
+    h2d_ceiling = ibp.ibp_measure_h2d(0, 1 << 30, 8)
+    zc_ceiling = ibp.ibp_measure_zero_copy_read(0, 1 << 30, 3)
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_peak = 6650.0
+    bufs = [torch.empty((layer_rows, 256), dtype=torch.uint8, device="cuda") for _ in range(2)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def fetch(i, bi, stream_ptr):
+        off = 0
+        for (h, n_rows, _, _) in layers[i % L]:
+            h.gather_decompress_range(0, n_rows, bufs[bi].data_ptr() + off * 256, stream_ptr)
+            off += n_rows
+
+    stream = torch.cuda.current_stream().cuda_stream
+    for i in range(W):
+        fetch(i, 0, stream)
+    fetch(L - 1, 1, stream)
+    torch.cuda.synchronize()
+    last_rows = layers[L - 1][6][1]
+    if not np.array_equal(bufs[1][layer_rows - last_rows:].cpu().numpy(), check):
+        raise SystemExit("bench.py: streamed layer differs from the original matrix")
+    clocks = ClockSampler(0)
+    clocks.start()
+    ms = []
+    for j in range(K):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fetch(W + j, j % 2, stream); b.record()
+        b.synchronize()
+        ms.append(a.elapsed_time(b))
+    clk = clocks.stop()
+    t_step = float(np.mean(ms))
+    value = layer_bytes / (t_step * 1e-3) * 1e-9
+    stored_layer = stored / L
+    achieved = stored_layer / (t_step * 1e-3) * 1e-9
+
+    # ---- S8: the same layer decoded from HBM (packed bytes staged once, outside the timing)
+    staged = []
+    for (h, n_rows, _, _) in layers[0]:
+        ptr, nb = h.packed_range(0, n_rows)
+        staged.append((h, n_rows, torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda(), nb))
+    def resident():
+        off = 0
+        for (h, n_rows, buf, nb) in staged:
+            h.decompress_resident(buf.data_ptr(), 0, n_rows, bufs[0].data_ptr() + off * 256, stream)
+            off += n_rows
+    for _ in range(3):
+        resident()
+    rs = []
+    for _ in range(10):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); resident(); b.record(); b.synchronize()
+        rs.append(a.elapsed_time(b))
+    t_res = float(np.mean(rs))
+    res_bytes = sum(s[3] for s in staged) + layer_bytes
+
+    # ---- S7: overlap with a consumer GEMM on the previous layer
+    M = args.gemm_m
+    act = torch.randn((M, 4096), dtype=torch.bfloat16, device="cuda")
+    shapes = [(m[2], m[3]) for m in layers[0]]
+    outs = [torch.empty((M, c), dtype=torch.bfloat16, device="cuda") for (_, c) in shapes]
+
+    def consume(i, bi):
+        off = 0
+        for j, (r, c) in enumerate(shapes):
+            wmat = bufs[bi][off:off + r * (c // 128)].view(torch.bfloat16).view(r, c)
+            torch.matmul(act, wmat, out=outs[j])
+            off += r * (c // 128)
+
+    n_pipe = min(max(K, 8), 16)
+    pipe = DoubleBufferedPipeline(fetch, consume, n_pipe)
+    for _ in range(2):
+        pipe.run_overlapped()
+    ov = summarize(pipe.run_fetch_only(), pipe.run_consume_only(), pipe.run_serial(), pipe.run_overlapped())
+    ov.update({"steps": n_pipe, "consumer": f"torch.matmul [M={M},4096] bf16 x the 7 decoded matrices of the previous layer (cuBLAS)",
+               "decode_ctas": args.decode_ctas or "library default (persistent, occupancy x SMs)"})
+
+    smp = OracleSample(workloads.KV(layers=1, pages=8))
+    g, rps, desc = smp.run(8.0) if not args.no_cpu else (None, None, None)
+    line = {
+        "metric": "effective decompressed GB/s (gather-decompress)", "value": round(value, 3), "unit": "GB/s", "n_gpus": 1,
+        "steps": K, "warmup": W, "ms_per_step": round(t_step, 4), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic", "rows_per_s": round(layer_rows / (t_step * 1e-3), 1),
+        "config": {"workload": f"configs[4] LLM weight streaming: bf16 N(0,0.02) matrices of a 7B-shaped decoder, 4 x 4096x4096 + 3 x 4096x11008 per layer, {L} layers in host memory ({raw_bytes * 1e-9:.2f} GB raw; BASELINE: 32 layers, 12.95 GB), groups = 128-column tiles (strided); one step = one whole layer (7 range gathers, {layer_bytes * 1e-6:.1f} MB out)",
+                   "align_bytes": args.align if args.align else 16, "store": args.store, "ratio_stored": round(raw_bytes / stored, 4),
+                   "ratio_bytealigned": round(raw_bytes / bytealigned, 4), "build_s": round(t_build, 1),
+                   "l2": "flushed with a 256 MiB write between steps (outside the events)"},
+        "roofline": {"bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
+                     "frac": round(achieved / h2d_ceiling, 4), "traffic": None, "kernel": "ibp_stream_kernel",
+                     "algorithmic_bytes_per_launch": int(stored_layer / 7), "zero_copy_read_ceiling": round(zc_ceiling, 3),
+                     "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
+                     "effective_roofline_GBps": round(h2d_ceiling * raw_bytes / stored, 2),
+                     "frac_of_effective_roofline": round(value / (h2d_ceiling * raw_bytes / stored), 4)},
+        "resident_decode": {"ms_per_layer": round(t_res, 4), "in_plus_out_GBps": round(res_bytes / (t_res * 1e-3) * 1e-9, 1),
+                            "out_GBps": round(layer_bytes / (t_res * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": hbm_peak,
+                            "frac": round(res_bytes / (t_res * 1e-3) * 1e-9 / hbm_peak, 4), "kernel": "ibp_stream_kernel (ibp_decompress_resident)"},
+        "overlap": ov,
+        "e2e": {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "note": "the consumer of streamed weights is on the GPU; no host round trip exists on this path"},
+        "gpu_launches": K * 7, "clocks": clk,
+        "cpu_baseline": None if g is None else {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)},
+    }
+    print(json.dumps(line), flush=True)
+    for mats in layers:
+        for m in mats:
+            m[0].destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="gnn", choices=["gnn", "dlrm", "tiny"])
-    ap.add_argument("--align", type=int, default=32)
+    ap.add_argument("--workload", default="gnn", choices=["gnn", "dlrm", "tiny", "kv", "weights"])
+    ap.add_argument("--align", type=int, default=0, help="packed-row alignment unit A; 0 = the workload's default")
+    ap.add_argument("--layers", type=int, default=8, help="weights workload: decoder layers held in host memory (32 = BASELINE's 13 GB)")
+    ap.add_argument("--gemm-m", type=int, default=16384, help="weights workload: rows of the consumer GEMM's activation")
+    ap.add_argument("--decode-ctas", type=int, default=0, help="limit the decode grid (SM share of the fetch); 0 = library default")
     ap.add_argument("--store", default="managed", choices=["managed", "pinned"])
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
+        if args.workload == "weights":
+            args.workload = "kv"      # the oracle arm samples row decodes; bf16 256-byte rows either way
         run_reference(args)
+    elif args.workload == "weights":
+        run_weights(args)
     else:
         run_cuda(args)
 

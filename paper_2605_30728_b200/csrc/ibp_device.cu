@@ -489,6 +489,7 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
     P.group_shift = 0xFFFFFFFFu;
     if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t sft = 0; while ((1u << sft) < h->p.group_param) ++sft; P.group_shift = sft; }
     P.strided = h->p.group_kind == IBP_GROUP_STRIDED;
+    P.fast_rows = h->p.align_bytes >= 4 && ((uintptr_t)packed & 3u) == 0;
     const uint64_t G = h->p.group_param;
     uint64_t need;                                   // bytes one stage must hold
     if (!P.strided) {

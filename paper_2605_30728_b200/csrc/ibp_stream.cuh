@@ -28,6 +28,7 @@ struct StreamParams {
     uint32_t row_bytes, n_words, n_pass;
     uint32_t group_param, group_shift, strided;
     uint32_t stage_bytes;
+    uint32_t fast_rows;            // packed rows start on 4-byte boundaries (A >= 4): the hoisted single-pass path applies
 };
 
 // The five move masks of the parallel-suffix expand for deposit positions nv (set bits = positions to fill, lowest first).
@@ -125,8 +126,63 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     }
 
     // ---------------------------------------------------------------------- consumers
+    // Fast path (single-pass rows whose packed bytes start on a 4-byte boundary, i.e. A >= 4): everything that depends
+    // only on the group is hoisted out of the row loop -- Mask/Bitval, the word offset and shift of each of the lane's W
+    // words inside a packed row, the five expand masks -- and the row loop is: 2 ld.shared + 1 funnel shift + 11 logic
+    // ops per word, one vector store, two pointer bumps.
     uint32_t m[W], b[W], ex[W], mv[W][5];
     uint64_t prep_g = ~0ull;
+    const uint32_t w0_fast = lane * W;
+    const bool fast = P.n_pass == 1 && P.fast_rows;
+    const bool active_fast = w0_fast < P.n_words;
+
+    auto prepare = [&](uint64_t g) {   // S2 + S4 for a single-pass row of group g
+        const uint32_t* gm = P.meta + g * 2ull * P.n_words;
+        if (active_fast) { VecIO<W>::ld(gm + w0_fast, m); VecIO<W>::ld(gm + P.n_words + w0_fast, b); }
+        else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) { m[q] = 0xFFFFFFFFu; b[q] = 0; }
+        }
+        uint32_t t = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) { ex[q] = t; t += __popc(~m[q]); }
+        const uint32_t incl = warp_inclusive_scan(t, lane);
+#pragma unroll
+        for (int q = 0; q < W; ++q) ex[q] += incl - t;
+        if (P.mvtab && active_fast) {
+            const uint32_t* tv = P.mvtab + (g * P.n_words + w0_fast) * 5ull;
+#pragma unroll
+            for (int q = 0; q < W; ++q)
+#pragma unroll
+                for (int i = 0; i < 5; ++i) mv[q][i] = __ldg(tv + q * 5 + i);
+        } else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) expand_masks(~m[q], mv[q]);
+        }
+        prep_g = g;
+    };
+
+    // `count` rows of the prepared group: packed row r at shared address saddr + r*sstride, output row at optr + r*ostride
+    auto decode_run = [&](uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
+        uint32_t wa[W], sh[W];
+#pragma unroll
+        for (int q = 0; q < W; ++q) { wa[q] = saddr + (ex[q] >> 5) * 4u; sh[q] = ex[q] & 31u; }
+        optr += (size_t)w0_fast * 4;
+        for (uint32_t r = 0; r < count; ++r) {
+            uint32_t o[W];
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                uint32_t lo, hi;
+                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wa[q]));
+                const uint32_t x = __funnelshift_r(lo, hi, sh[q]);
+                o[q] = (expand_bits(x, mv[q]) & ~m[q]) | b[q];
+                wa[q] += sstride;
+            }
+            if (active_fast) VecIO<W>::st(optr, o);
+            optr += ostride;
+        }
+    };
+
     uint32_t k = 0;
     for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
         const uint32_t s = k % NS;
@@ -134,82 +190,83 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         chunk_geom(c, row0, nrows, out0, b0, b1);
         const uint32_t head = (uint32_t)((uintptr_t)(P.store + (b0 - P.bias)) & 15u);
         const uint32_t* stage = (const uint32_t*)(smem + (size_t)s * P.stage_bytes);
+        const uint32_t stage_s = smem_s + s * P.stage_bytes;
         bool waited = false;
 
-        // Decode one row whose packed bytes start at byte `roff` of the stage; metadata of group g.
-        auto decode_row = [&](uint64_t g, uint32_t roff, uint8_t* orow) {
+        // Generic path: any number of passes, any byte alignment; metadata reloaded per pass, run-wise bit deposit.
+        auto decode_row_generic = [&](uint64_t g, uint32_t roff, uint8_t* orow) {
             const uint32_t* gm = P.meta + g * 2ull * P.n_words;
             uint32_t carry = 0;
+            prep_g = ~0ull;
             for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
                 const uint32_t w0 = (pass * 32u + lane) * W;
                 const bool active = w0 < P.n_words;
-                if (P.n_pass > 1 || g != prep_g) {
-                    // ---- S2 + S4 once per piece: metadata, bit offsets, expand masks
-                    if (active) { VecIO<W>::ld(gm + w0, m); VecIO<W>::ld(gm + P.n_words + w0, b); }
-                    else {
+                uint32_t mm[W], bb[W], kq[W];
+                if (active) { VecIO<W>::ld(gm + w0, mm); VecIO<W>::ld(gm + P.n_words + w0, bb); }
+                else {
 #pragma unroll
-                        for (int q = 0; q < W; ++q) { m[q] = 0xFFFFFFFFu; b[q] = 0; }
-                    }
-                    uint32_t t = 0;
-#pragma unroll
-                    for (int q = 0; q < W; ++q) { ex[q] = t; t += __popc(~m[q]); }
-                    const uint32_t incl = warp_inclusive_scan(t, lane);
-#pragma unroll
-                    for (int q = 0; q < W; ++q) ex[q] += incl - t + carry;
-                    carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
-                    if (P.mvtab && active) {
-                        const uint32_t* tv = P.mvtab + (g * P.n_words + w0) * 5ull;
-#pragma unroll
-                        for (int q = 0; q < W; ++q)
-#pragma unroll
-                            for (int i = 0; i < 5; ++i) mv[q][i] = __ldg(tv + q * 5 + i);
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < W; ++q) expand_masks(~m[q], mv[q]);
-                    }
-                    prep_g = g;
+                    for (int q = 0; q < W; ++q) { mm[q] = 0xFFFFFFFFu; bb[q] = 0; }
                 }
+                uint32_t t = 0;
+#pragma unroll
+                for (int q = 0; q < W; ++q) { kq[q] = __popc(~mm[q]); t += kq[q]; }
+                const uint32_t incl = warp_inclusive_scan(t, lane);
+                uint32_t bit = roff * 8u + carry + incl - t;
+                carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
                 if (!waited) { mbar_wait(full_s + s * 8, (k / NS) & 1u); waited = true; }
-                // ---- S5: extract k bits at the word's bit offset, expand, OR Bitval
-                const uint32_t rowbits = roff * 8u;
                 uint32_t o[W];
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    const uint32_t bit = rowbits + ex[q];
-                    const uint32_t wq = bit >> 5;
-                    const uint32_t x = __funnelshift_r(stage[wq], stage[wq + 1], bit);
-                    o[q] = (expand_bits(x, mv[q]) & ~m[q]) | b[q];
+                    uint32_t word = bb[q];
+                    if (kq[q]) {
+                        const uint32_t wq = bit >> 5;
+                        word |= deposit_runs(__funnelshift_r(stage[wq], stage[wq + 1], bit), ~mm[q]);
+                        bit += kq[q];
+                    }
+                    o[q] = word;
                 }
-                if (active) VecIO<W>::st(orow + (size_t)w0 * 4, o);   // ---- S6
+                if (active) VecIO<W>::st(orow + (size_t)w0 * 4, o);
             }
         };
 
         if (!P.strided) {
             const uint32_t U = P.piece_rows, n_pieces = (nrows + U - 1) / U;
             for (uint32_t p = wib; p < n_pieces; p += NW) {
-                const uint32_t j0 = p * U, j1 = min(nrows, j0 + U);
-                uint64_t g = ~0ull; uint32_t roff = 0, stride = 0; uint64_t g_end = 0;
-                for (uint32_t j = j0; j < j1; ++j) {
+                uint32_t j = p * U;
+                const uint32_t j1 = min(nrows, j + U);
+                while (j < j1) {                                   // runs of rows of one group inside the piece
                     const uint64_t id = (uint64_t)row0 + j;
-                    if (g == ~0ull || id >= g_end) {
-                        g = group_of_u(P.group_param, P.group_shift, id);
-                        const IbpGroupEntry e = P.gtab[g];
-                        stride = e.stride;
-                        roff = head + (uint32_t)(e.base + (id - g * S) * e.stride - b0);
-                        g_end = (g + 1) * S;
+                    const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
+                    const uint32_t run = (uint32_t)min((uint64_t)(j1 - j), (g + 1) * S - id);
+                    const IbpGroupEntry e = P.gtab[g];
+                    const uint32_t roff = head + (uint32_t)(e.base + (id - g * S) * e.stride - b0);
+                    uint8_t* orow = P.out + (uint64_t)(out0 + j) * P.row_bytes;
+                    if (fast) {
+                        if (g != prep_g) prepare(g);
+                        if (!waited) { mbar_wait(full_s + s * 8, (k / NS) & 1u); waited = true; }
+                        decode_run(stage_s + roff, e.stride, orow, P.row_bytes, run);
+                    } else {
+                        for (uint32_t r = 0; r < run; ++r) decode_row_generic(g, roff + r * e.stride, orow + (uint64_t)r * P.row_bytes);
                     }
-                    decode_row(g, roff, P.out + (uint64_t)(out0 + j) * P.row_bytes);
-                    roff += stride;
+                    j += run;
                 }
             }
         } else {
-            const int64_t id_end = (P.ids ? 0 : P.first_row) + P.span_rows;   // strided tables are decoded as ranges only
+            const int64_t id_end = P.first_row + P.span_rows;     // strided tables are decoded as ranges only
             for (uint32_t t = wib; t < (uint32_t)S; t += NW) {
+                const int64_t left = (id_end - (row0 + (int64_t)t) + (int64_t)S - 1) / (int64_t)S;   // rows of tile t in range
+                const uint32_t cnt = left <= 0 ? 0u : (uint32_t)min((int64_t)nrows, left);
+                if (!cnt) continue;
                 const IbpGroupEntry e = P.gtab[t];
-                for (uint32_t j = 0; j < nrows; ++j) {
-                    const int64_t id = row0 + (int64_t)j * (int64_t)S + t;
-                    if (id >= id_end) break;
-                    decode_row(t, head + (uint32_t)(j * P.row_stride_strided + e.base), P.out + (uint64_t)(out0 + (int64_t)j * (int64_t)S + t) * P.row_bytes);
+                const uint32_t roff = head + (uint32_t)e.base;
+                uint8_t* orow = P.out + (uint64_t)(out0 + t) * P.row_bytes;
+                if (fast) {
+                    if ((uint64_t)t != prep_g) prepare(t);
+                    if (!waited) { mbar_wait(full_s + s * 8, (k / NS) & 1u); waited = true; }
+                    decode_run(stage_s + roff, (uint32_t)P.row_stride_strided, orow, S * P.row_bytes, cnt);
+                } else {
+                    for (uint32_t r = 0; r < cnt; ++r)
+                        decode_row_generic(t, roff + r * (uint32_t)P.row_stride_strided, orow + (uint64_t)r * S * P.row_bytes);
                 }
             }
         }
