@@ -207,6 +207,8 @@ def run_cuda(args):
         h.set_order_mode(args.order)
     if args.decode_ctas:
         h.configure(args.decode_ctas, 0)
+    dedup = args.dedup if args.dedup is not None else (0 if w.ids_unique else -1)
+    h.set_dedup_mode(dedup)
     info = h.info()
 
     # ---- ceilings measured on this box, this run
@@ -228,8 +230,9 @@ def run_cuda(args):
     out = torch.empty((n_rows_out, w.row_bytes), dtype=torch.uint8, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     link = [h.batch_link_bytes(b) for b in batches]            # (unique ids, stored bytes, byte-aligned bytes)
-    order_on = (args.order == 1) or (args.order is None and info.store_kind == ibp.IBP_STORE_PINNED and info.packed_bytes_stored > (64 << 20) and n >= 4096)
-    launches_per_step = 1 + (3 if (order_on and w.index_span == 1) else 0)
+    order_on = w.index_span == 1 and ((args.order == 1) or (args.order is None and info.packed_bytes_stored > (64 << 20) and n >= 4096))
+    dedup_on = w.index_span == 1 and (dedup == 1 or (dedup < 0 and n >= 16384))
+    launches_per_step = 1 + (3 if order_on else 0) + (2 if dedup_on else 0)
 
     def step(i):
         h.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
@@ -345,7 +348,7 @@ def run_cuda(args):
             "config": {
                 "workload": describe(w), "rows_per_step": n_rows_out, "row_bytes": w.row_bytes, "align_bytes": info.align_bytes,
                 "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
-                "locality_order": bool(order_on), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
+                "locality_order": bool(order_on), "dedup": bool(dedup_on), "ids_unique_by_construction": bool(w.ids_unique), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
                 "ratio_stored": round(ratio_stored, 4), "ratio_bytealigned": round(ratio_alg, 4),
                 "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3), "metadata_MB": round(info.metadata_bytes * 1e-6, 2),
                 "build_s": round(t_build, 2), "datagen_s": round(t_gen, 2), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
@@ -532,6 +535,7 @@ def main():
     ap.add_argument("--decode-ctas", type=int, default=0, help="limit the decode grid (SM share of the fetch); 0 = library default")
     ap.add_argument("--store", default="managed", choices=["managed", "pinned"])
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
+    ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -173,12 +173,18 @@ ibp_status ibp_gather_uncompressed_ex(const void* rows_mapped, uint32_t row_byte
                                       int64_t n, void* out_dev, int locality_order, void* cuda_stream);
 
 /* Tuning/test hook: locality-ordered processing of random gathers: 1 = always, 0 = never, -1 = automatic (default:
- * on for IBP_STORE_PINNED stores above 64 MiB and batches of >= 4096 ids).  Results are identical either way.        */
+ * on for stores above 64 MiB and batches of >= 4096 ids).  Results are identical either way.                         */
 ibp_status ibp_set_order_mode(ibp_handle* h, int mode);
 
 /* Tuning/test hook: engine that moves packed rows into shared memory: 1 = cp.async.bulk + mbarrier (TMA, default),
  * 0 = 16-byte cp.async through the load/store unit.  Results are identical either way.                              */
 ibp_status ibp_set_fetch_mode(ibp_handle* h, int mode);
+
+/* De-duplication of random gathers (index_span 1): 1 = every distinct id of the batch crosses PCIe once and its decoded row
+ * is replicated HBM -> HBM to the positions of its repeats (skewed batches, e.g. DLRM lookups); 0 = every id is fetched
+ * (for callers that know their ids are distinct, e.g. a de-duplicating GNN sampler); -1 = automatic (default): on for
+ * batches of >= 16384 ids.  Output is identical either way.  Needs n_rows < 2^32 - 1, else it is ignored.          */
+ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode);
 
 /* Tuning/test hook: contiguous runs (spans, ranges, resident decode): 1 = TMA producer/consumer stream kernel (default),
  * 0 = per-row fetch kernel.  Results are identical either way.                                                       */

@@ -68,6 +68,7 @@ SIGNATURES = {
     "ibp_set_order_mode": (_int, [_vp, _int]),
     "ibp_set_fetch_mode": (_int, [_vp, _int]),
     "ibp_set_stream_mode": (_int, [_vp, _int]),
+    "ibp_set_dedup_mode": (_int, [_vp, _int]),
     "ibp_set_rows_in_flight": (_int, [_vp, _int]),
     "ibp_host_alloc": (_int, [C.c_size_t, C.POINTER(_vp), C.POINTER(_vp)]),
     "ibp_host_free": (_int, [_vp]),
@@ -166,6 +167,10 @@ class Handle:
 
     def set_fetch_mode(self, mode):
         _check(lib().ibp_set_fetch_mode(self._h, mode))
+        return self
+
+    def set_dedup_mode(self, mode):
+        _check(lib().ibp_set_dedup_mode(self._h, mode))
         return self
 
     def set_stream_mode(self, mode):

@@ -47,6 +47,7 @@ struct DecodeParams {
     int64_t n;                     // ids (gather) or rows (range)
     int64_t first_row;             // ranges
     int64_t n_units;
+    const uint32_t* n_units_dev;   // MODE_ROWS with de-duplication: number of work-list entries, known only on the device
     uint64_t row_stride_strided;
     uint32_t row_bytes, n_words, n_pass;
     uint32_t group_param, group_shift;   // group_shift >= 0 when group_param is a power of two, else 0xFFFFFFFF
@@ -174,13 +175,14 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
     // of the (locality-ordered) list, so that the NST rows it keeps in flight, together with the other warps', form
     // one contiguous window of the list.  Other modes: units of consecutive rows, grid-stride over units.
     const int64_t gw = (int64_t)blockIdx.x * wpc + wib, NWT = (int64_t)gridDim.x * wpc;
-    const int64_t n_units = MODE == MODE_ROWS ? (gw < P.n_units ? gw + 1 : 0) : P.n_units;
+    const int64_t n_total = (MODE == MODE_ROWS && P.n_units_dev) ? (int64_t)*P.n_units_dev : P.n_units;
+    const int64_t n_units = MODE == MODE_ROWS ? (gw < n_total ? gw + 1 : 0) : n_total;
     for (int64_t u = gw; u < n_units; u += NWT) {
         // ---- unit -> rows
         int64_t id0 = 0, out0 = 0;
         uint32_t nrows, id_step = 0, out_step = 0;
         if (MODE == MODE_ROWS) {
-            nrows = (uint32_t)((P.n_units - gw + NWT - 1) / NWT);
+            nrows = (uint32_t)((n_total - gw + NWT - 1) / NWT);
         } else if (MODE == MODE_SPANS) {
             const int64_t si = u / P.units_per_span;
             const uint32_t c = (uint32_t)(u - si * P.units_per_span);
@@ -316,8 +318,12 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
 // Random gathers over a multi-GB host store are bound by address translation, not by the link, unless the rows in
 // flight are close in the store (measured: DESIGN.md section 6).  A counting sort by coarse store region gives the
 // kernel a processing order with that locality; out[] positions are unchanged.
-__global__ void ibp_bucket_hist(const int64_t* __restrict__ ids, int64_t n, uint32_t shift, uint32_t nb, uint32_t* __restrict__ cnt) {
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+// `list` (optional) restricts the pass to the batch positions list[0..*n_dev) (the representatives after de-duplication).
+__global__ void ibp_bucket_hist(const int64_t* __restrict__ ids, const int32_t* __restrict__ list, const uint32_t* __restrict__ n_dev,
+                                int64_t n, uint32_t shift, uint32_t nb, uint32_t* __restrict__ cnt) {
+    if (n_dev) n = *n_dev;
+    for (int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; j < n; j += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = list ? list[j] : j;
         const uint64_t bk = (uint64_t)ids[i] >> shift;
         atomicAdd(&cnt[bk < nb ? bk : nb - 1], 1u);
     }
@@ -338,8 +344,11 @@ __global__ void ibp_bucket_scan(uint32_t* cnt, uint32_t nb) {   // one CTA, 1024
     uint32_t run = part[threadIdx.x] - s;
     for (uint32_t i = lo; i < hi; ++i) { const uint32_t c = cnt[i]; cnt[i] = run; run += c; }
 }
-__global__ void ibp_bucket_scatter(const int64_t* __restrict__ ids, int64_t n, uint32_t shift, uint32_t nb, uint32_t* __restrict__ cursor, int32_t* __restrict__ order) {
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+__global__ void ibp_bucket_scatter(const int64_t* __restrict__ ids, const int32_t* __restrict__ list, const uint32_t* __restrict__ n_dev,
+                                   int64_t n, uint32_t shift, uint32_t nb, uint32_t* __restrict__ cursor, int32_t* __restrict__ order) {
+    if (n_dev) n = *n_dev;
+    for (int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; j < n; j += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = list ? list[j] : j;
         const uint64_t bk = (uint64_t)ids[i] >> shift;
         const uint32_t pos = atomicAdd(&cursor[bk < nb ? bk : nb - 1], 1u);
         order[pos] = (int32_t)i;
@@ -356,8 +365,8 @@ static void bucket_shape(uint64_t n_rows, uint64_t store_bytes, uint64_t target,
     *nb = (uint32_t)(((n_rows - 1) >> s) + 1);
 }
 
-static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_space, uint64_t store_bytes, cudaStream_t st,
-                             int32_t** order_out, void** ws_out) {
+static ibp_status make_order(const int64_t* ids_dev, const int32_t* list, const uint32_t* n_dev, int64_t n, uint64_t n_ids_space,
+                             uint64_t store_bytes, cudaStream_t st, int32_t** order_out, void** ws_out) {
     uint32_t shift, nb;
     uint64_t target = 256ull << 10;
     if (const char* e = getenv("IBP_BUCKET_BYTES")) target = strtoull(e, nullptr, 10);   // tuning experiments only
@@ -369,13 +378,51 @@ static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_s
     int32_t* order = (int32_t*)(ws + cnt_bytes);
     IBP_CUDA(cudaMemsetAsync(cnt, 0, cnt_bytes, st));
     const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, 148 * 8);
-    ibp_bucket_hist<<<blocks, thr, 0, st>>>(ids_dev, n, shift, nb, cnt);
+    ibp_bucket_hist<<<blocks, thr, 0, st>>>(ids_dev, list, n_dev, n, shift, nb, cnt);
     ibp_bucket_scan<<<1, 1024, 0, st>>>(cnt, nb);
-    ibp_bucket_scatter<<<blocks, thr, 0, st>>>(ids_dev, n, shift, nb, cnt, order);
+    ibp_bucket_scatter<<<blocks, thr, 0, st>>>(ids_dev, list, n_dev, n, shift, nb, cnt, order);
     IBP_CUDA(cudaGetLastError());
     *order_out = order;
     *ws_out = ws;
     return IBP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ de-duplication
+// Skewed batches (DLRM lookups, Zipf) repeat ids; a repeated row need not cross PCIe twice.  Pass 1 claims one
+// representative position per distinct id in an open-addressing table (64-bit entries: id in the high word, the winner's
+// batch position in the low word; one CAS per id, none when the id is already there) and appends the winners to a work
+// list.  The decode kernel then runs over the work list only, and pass 3 copies each representative's decoded row
+// (HBM -> HBM) to the positions of its repeats.  Output is identical to the plain path.
+__global__ void ibp_dedup_insert(const int64_t* __restrict__ ids, int64_t n, unsigned long long* __restrict__ table, uint32_t mask,
+                                 int32_t* __restrict__ rep, int32_t* __restrict__ uniq, uint32_t* __restrict__ n_uniq) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint64_t key = (uint64_t)ids[i];
+        uint32_t slot = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 32) & mask;
+        const unsigned long long mine = (key << 32) | (uint32_t)i;
+        int32_t r;
+        for (;;) {
+            unsigned long long cur = table[slot];
+            if (cur == ~0ull) cur = atomicCAS(&table[slot], ~0ull, mine);
+            if (cur == ~0ull) { r = (int32_t)i; uniq[atomicAdd(n_uniq, 1u)] = (int32_t)i; break; }
+            if ((cur >> 32) == key) { r = (int32_t)(uint32_t)cur; break; }
+            slot = (slot + 1) & mask;
+        }
+        rep[i] = r;
+    }
+}
+__global__ void ibp_dedup_copy(const int32_t* __restrict__ rep, int64_t n, uint32_t row_bytes, uint8_t* __restrict__ out) {
+    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    for (int64_t i = (int64_t)blockIdx.x * wpc + (threadIdx.x >> 5); i < n; i += (int64_t)gridDim.x * wpc) {
+        const int32_t r = rep[i];
+        if (r == (int32_t)i) continue;
+        const uint4* src = (const uint4*)(out + (uint64_t)r * row_bytes);
+        uint4* dst = (uint4*)(out + (uint64_t)i * row_bytes);
+        if (row_bytes % 16 == 0) {
+            for (uint32_t v = lane; v < row_bytes / 16; v += 32) dst[v] = src[v];
+        } else {
+            for (uint32_t v = lane; v < row_bytes / 4; v += 32) ((uint32_t*)dst)[v] = ((const uint32_t*)src)[v];
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ launch
@@ -600,19 +647,47 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     if (h->p.index_span == 1) {
         if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
         P.n_units = n;
-        void* ws = nullptr;
-        // automatic: only the 4 KB-page pinned store needs the locality order (managed-host stores are mapped with
-        // large pages; there the order buys nothing and makes duplicate ids collide in time)
-        const bool order = h->order_mode == 1 ||
-                           (h->order_mode < 0 && h->store_kind == IBP_STORE_PINNED && h->store_used > (64ull << 20) && n >= 4096);
+        void *ws = nullptr, *ws2 = nullptr;
+        const int32_t* list = nullptr;      // work list of batch positions (representatives), or nullptr = all
+        const uint32_t* n_list = nullptr;
+        int32_t* rep = nullptr;
+        const bool dedup = (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
+        if (dedup) {
+            uint32_t cap = 1024;
+            while ((uint64_t)cap < 2ull * (uint64_t)n) cap <<= 1;
+            const size_t tab_bytes = (size_t)cap * 8, idx_bytes = ((size_t)n * 4 + 255) / 256 * 256;
+            uint8_t* w2 = nullptr;
+            IBP_CUDA(cudaMallocAsync((void**)&w2, tab_bytes + 2 * idx_bytes + 256, st));
+            ws2 = w2;
+            unsigned long long* table = (unsigned long long*)w2;
+            rep = (int32_t*)(w2 + tab_bytes);
+            int32_t* uniq = (int32_t*)(w2 + tab_bytes + idx_bytes);
+            uint32_t* n_uniq = (uint32_t*)(w2 + tab_bytes + 2 * idx_bytes);
+            IBP_CUDA(cudaMemsetAsync(table, 0xFF, tab_bytes, st));
+            IBP_CUDA(cudaMemsetAsync(n_uniq, 0, 4, st));
+            ibp_dedup_insert<<<(int)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(row_ids_dev, n, table, cap - 1, rep, uniq, n_uniq);
+            IBP_CUDA(cudaGetLastError());
+            list = uniq; n_list = n_uniq;
+        }
+        // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
+        // Essential for the 4 KB-page pinned store, a few percent for the managed-host store -- unless repeated ids are
+        // fetched one by one (dedup off on a batch with repeats), where neighbours in the order collide on the same lines.
+        const bool order = h->order_mode == 1 || (h->order_mode < 0 && h->store_used > (64ull << 20) && n >= 4096);
         if (order) {
             int32_t* ord = nullptr;
-            s = make_order(row_ids_dev, n, h->p.n_rows, h->store_used, st, &ord, &ws);
+            s = make_order(row_ids_dev, list, n_list, n, h->p.n_rows, h->store_used, st, &ord, &ws);
             if (s != IBP_OK) return s;
-            P.order = ord;
+            list = ord;
         }
+        P.order = list;
+        P.n_units_dev = n_list;
         s = launch_decode(h, P, MODE_ROWS, st);
+        if (s == IBP_OK && dedup) {
+            ibp_dedup_copy<<<(int)std::min<int64_t>((n + 7) / 8, 148 * 8), 256, 0, st>>>(rep, n, h->p.row_bytes, (uint8_t*)out_dev);
+            if (cudaGetLastError() != cudaSuccess) { ibp_set_error("ibp_dedup_copy launch failed"); s = IBP_ERR_CUDA; }
+        }
         if (ws) IBP_CUDA(cudaFreeAsync(ws, st));
+        if (ws2) IBP_CUDA(cudaFreeAsync(ws2, st));
         return s;
     }
     if (h->stream_mode)
@@ -756,7 +831,7 @@ extern "C" ibp_status ibp_gather_uncompressed_ex(const void* rows_mapped, uint32
     int32_t* ord = nullptr;
     void* ws = nullptr;
     if (locality_order && n_rows > 0) {
-        ibp_status s = make_order(row_ids_dev, n, n_rows, n_rows * (uint64_t)row_bytes, st, &ord, &ws);
+        ibp_status s = make_order(row_ids_dev, nullptr, nullptr, n, n_rows, n_rows * (uint64_t)row_bytes, st, &ord, &ws);
         if (s != IBP_OK) return s;
     }
     const int wpc = 8;
@@ -856,6 +931,14 @@ static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps
 }
 extern "C" ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, false); }
 extern "C" ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, true); }
+
+// 1 = de-duplicate the ids of a random gather before fetching; 0 = fetch every id (the caller knows the ids are distinct);
+// -1 = automatic (default): on for batches of >= 16384 ids.
+extern "C" ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode) {
+    if (!h || mode < -1 || mode > 1) { ibp_set_error("ibp_set_dedup_mode: bad argument"); return IBP_ERR_INVALID_ARG; }
+    h->dedup_mode = mode;
+    return IBP_OK;
+}
 
 // Test/tuning hook: 1 = contiguous runs through the TMA producer/consumer stream kernel (default), 0 = per-row fetch.
 extern "C" ibp_status ibp_set_stream_mode(ibp_handle* h, int mode) {

@@ -43,6 +43,7 @@ class Workload:
     index_span: int = 1
     align_bytes: int = 32           # packed-row alignment unit A used by default for this workload
     batch_ids: int = 0              # ids per batch (each id selects index_span rows)
+    ids_unique: bool = False        # the batch sampler guarantees distinct ids (lets the caller switch de-duplication off)
     note: str = ""
     _cache: dict = field(default_factory=dict, repr=False)
 
@@ -107,7 +108,7 @@ class GNN(Workload):
     contiguous by type); groups of 256; 250k UNIQUE ids per batch, Zipf(0.9) through a seeded permutation (R16, R21)."""
 
     def __init__(self, n_rows=10_000_000, batch=250_000):
-        super().__init__("gnn", 1, n_rows, 512, "f32", BLOCKED, 256, 1, 32, batch)
+        super().__init__("gnn", 1, n_rows, 512, "f32", BLOCKED, 256, 1, 32, batch, ids_unique=True)
         self.n_dense = (n_rows * 7) // 10
 
     def fill_rows(self, first, count, out):

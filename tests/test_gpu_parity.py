@@ -87,7 +87,11 @@ def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
         h.set_fetch_mode(fetch)
         for mode in (0, 1):
             h.set_order_mode(mode)
+            h.set_dedup_mode(mode ^ fetch)
             assert np.array_equal(_gather(h, ids), want)
+    h.set_dedup_mode(0)
+    for fetch in (0, 1):
+        h.set_fetch_mode(fetch)
         for sm in (0, 1):                                               # per-row fetch kernel / TMA stream kernel
             h.set_stream_mode(sm)
             assert np.array_equal(_resident(h, 0, n), X)                # whole table from HBM
@@ -159,9 +163,13 @@ def test_dlrm_shape_duplicates(flags, kind):
     assert h.info().store_kind == kind
     ids = w.ids(0)
     assert len(np.unique(ids)) < len(ids)                                 # repeats kept (reading R16)
-    for mode in (0, 1):
-        h.set_order_mode(mode)
-        assert np.array_equal(_gather(h, ids), oracle.gather_plain(X, ids))
+    for dedup in (0, 1):                                                  # fetch every id / fetch distinct ids once
+        h.set_dedup_mode(dedup)
+        for mode in (0, 1):
+            h.set_order_mode(mode)
+            assert np.array_equal(_gather(h, ids), oracle.gather_plain(X, ids))
+    same = np.full(5000, int(ids[7]), np.int64)                           # a batch that is one id repeated
+    assert np.array_equal(_gather(h, same), oracle.gather_plain(X, same))
     h.destroy()
 
 
