@@ -47,9 +47,15 @@ __device__ __forceinline__ void expand_masks(uint32_t nv, uint32_t mv[5]) {
         mk &= ~mp;
     }
 }
+// bit-select in ONE logic op: (c & a) | (~c & b)  (lop3 truth table 0xE4 for inputs a, b, c)
+__device__ __forceinline__ uint32_t bitselect(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
 __device__ __forceinline__ uint32_t expand_bits(uint32_t x, const uint32_t mv[5]) {
 #pragma unroll
-    for (int i = 4; i >= 0; --i) x = (x & ~mv[i]) | ((x << (1 << i)) & mv[i]);
+    for (int i = 4; i >= 0; --i) x = bitselect(x << (1 << i), x, mv[i]);
     return x;
 }
 
@@ -157,7 +163,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 for (int i = 0; i < 5; ++i) mv[q][i] = __ldg(tv + q * 5 + i);
         } else {
 #pragma unroll
-            for (int q = 0; q < W; ++q) expand_masks(~m[q], mv[q]);
+            for (int q = 0; q < W; ++q) {
+                if (q > 0 && m[q] == m[q - 1]) {               // homogeneous float data: neighbouring words share a mask
+#pragma unroll
+                    for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+                } else {
+                    expand_masks(~m[q], mv[q]);
+                }
+            }
         }
         prep_g = g;
     };
@@ -175,7 +188,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 uint32_t lo, hi;
                 asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wa[q]));
                 const uint32_t x = __funnelshift_r(lo, hi, sh[q]);
-                o[q] = (expand_bits(x, mv[q]) & ~m[q]) | b[q];
+                o[q] = bitselect(b[q], expand_bits(x, mv[q]), m[q]);   // Bitval where Mask is 1, expanded bits elsewhere
                 wa[q] += sstride;
             }
             if (active_fast) VecIO<W>::st(optr, o);
@@ -231,6 +244,18 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
 
         if (!P.strided) {
             const uint32_t U = P.piece_rows, n_pieces = (nrows + U - 1) / U;
+            if (fast && c + gridDim.x < P.n_chunks) {
+                // warm L1/L2 with the metadata of this warp's first piece of its NEXT chunk: the loads in prepare() are
+                // otherwise a dependent HBM round trip at the head of every piece
+                int64_t nrow0, nout0; uint32_t nn; uint64_t nb0, nb1;
+                chunk_geom(c + gridDim.x, nrow0, nn, nout0, nb0, nb1);
+                if (wib * U < nn && active_fast) {
+                    const uint64_t ng = group_of_u(P.group_param, P.group_shift, (uint64_t)nrow0 + wib * U);
+                    const uint32_t* ngm = P.meta + ng * 2ull * P.n_words + w0_fast;
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm + P.n_words));
+                }
+            }
             for (uint32_t p = wib; p < n_pieces; p += NW) {
                 uint32_t j = p * U;
                 const uint32_t j1 = min(nrows, j + U);
