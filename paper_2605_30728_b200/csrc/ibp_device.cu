@@ -55,6 +55,7 @@ struct DecodeParams {
     uint32_t rows_per_unit, units_per_span;
     uint32_t slot_bytes;
     uint32_t strided;              // group kind of the handle (MODE_ROWS serves both kinds)
+    uint32_t keep_l2;              // write the rows with the default cache policy (a later pass re-reads them) instead of streaming
 };
 
 // ------------------------------------------------------------------------------------------------ device helpers
@@ -93,14 +94,17 @@ template <int W> struct VecIO;
 template <> struct VecIO<1> {
     static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { v[0] = __ldg(p); }
     static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.b32 [%0], %1;" ::"l"(p), "r"(v[0]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint32_t*)p = v[0]; }
 };
 template <> struct VecIO<2> {
     static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint2 t = __ldg((const uint2*)p); v[0] = t.x; v[1] = t.y; }
     static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v2.b32 [%0], {%1,%2};" ::"l"(p), "r"(v[0]), "r"(v[1]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint2*)p = make_uint2(v[0], v[1]); }
 };
 template <> struct VecIO<4> {
     static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint4 t = __ldg((const uint4*)p); v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w; }
     static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint4*)p = make_uint4(v[0], v[1], v[2], v[3]); }
 };
 
 __device__ __forceinline__ uint64_t group_of(const DecodeParams& P, uint64_t id, bool strided) {
@@ -304,7 +308,10 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
                     o[c] = word;
                 }
                 // ---- S6
-                if (active) VecIO<W>::st(orow + (size_t)w0 * 4, o);
+                if (active) {
+                    if (MODE == MODE_ROWS && P.keep_l2) VecIO<W>::st_keep(orow + (size_t)w0 * 4, o);
+                    else VecIO<W>::st(orow + (size_t)w0 * 4, o);
+                }
                 carry += tot;
             }
             ++seq_d;
@@ -328,21 +335,35 @@ __global__ void ibp_bucket_hist(const int64_t* __restrict__ ids, const int32_t* 
         atomicAdd(&cnt[bk < nb ? bk : nb - 1], 1u);
     }
 }
-__global__ void ibp_bucket_scan(uint32_t* cnt, uint32_t nb) {   // one CTA, 1024 threads; exclusive scan in place
-    __shared__ uint32_t part[1024];
-    const uint32_t per = (nb + 1023) / 1024, lo = threadIdx.x * per, hi = min(nb, lo + per);
+// Exclusive scan in place, one CTA of 1024 threads.  cnt has nb_pad entries (a multiple of 4096, zero beyond nb): warp w owns
+// the contiguous segment [w*nb_pad/32, (w+1)*nb_pad/32), lanes read consecutive uint4 (coalesced), two passes (segment
+// totals, then the scan proper with the next vector prefetched).
+__global__ void __launch_bounds__(1024) ibp_bucket_scan(uint32_t* cnt, uint32_t nb_pad) {
+    __shared__ uint32_t wsum[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const uint32_t per_warp = nb_pad / 32, iters = per_warp / 128;
+    uint4* seg = (uint4*)(cnt + (size_t)wid * per_warp) + lane;
     uint32_t s = 0;
-    for (uint32_t i = lo; i < hi; ++i) s += cnt[i];
-    part[threadIdx.x] = s;
+    for (uint32_t it = 0; it < iters; ++it) { const uint4 v = seg[it * 32]; s += v.x + v.y + v.z + v.w; }
+#pragma unroll
+    for (int d = 16; d; d >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, d);
+    if (lane == 0) wsum[wid] = s;
     __syncthreads();
-    for (uint32_t d = 1; d < 1024; d <<= 1) {
-        uint32_t t = threadIdx.x >= d ? part[threadIdx.x - d] : 0;
-        __syncthreads();
-        part[threadIdx.x] += t;
-        __syncthreads();
+    if (wid == 0) { const uint32_t v = wsum[lane]; wsum[lane] = warp_inclusive_scan(v, lane) - v; }
+    __syncthreads();
+    uint32_t run = wsum[wid];
+    uint4 v = iters ? seg[0] : make_uint4(0, 0, 0, 0);
+    for (uint32_t it = 0; it < iters; ++it) {
+        const uint4 nxt = it + 1 < iters ? seg[(it + 1) * 32] : make_uint4(0, 0, 0, 0);
+        const uint32_t t = v.x + v.y + v.z + v.w;
+        const uint32_t incl = warp_inclusive_scan(t, lane);
+        uint32_t e = run + incl - t;
+        uint4 o;
+        o.x = e; e += v.x; o.y = e; e += v.y; o.z = e; e += v.z; o.w = e;
+        seg[it * 32] = o;
+        run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+        v = nxt;
     }
-    uint32_t run = part[threadIdx.x] - s;
-    for (uint32_t i = lo; i < hi; ++i) { const uint32_t c = cnt[i]; cnt[i] = run; run += c; }
 }
 __global__ void ibp_bucket_scatter(const int64_t* __restrict__ ids, const int32_t* __restrict__ list, const uint32_t* __restrict__ n_dev,
                                    int64_t n, uint32_t shift, uint32_t nb, uint32_t* __restrict__ cursor, int32_t* __restrict__ order) {
@@ -360,31 +381,9 @@ static void bucket_shape(uint64_t n_rows, uint64_t store_bytes, uint64_t target,
     const double bytes_per_row = (double)std::max<uint64_t>(store_bytes, 1) / (double)std::max<uint64_t>(n_rows, 1);
     uint32_t s = 0;
     while (s < 40 && (double)(1ull << s) * bytes_per_row < (double)target) ++s;
-    while (((n_rows - 1) >> s) + 1 > (1u << 20)) ++s;
+    while (((n_rows - 1) >> s) + 1 > (1u << 18)) ++s;
     *shift = s;
     *nb = (uint32_t)(((n_rows - 1) >> s) + 1);
-}
-
-static ibp_status make_order(const int64_t* ids_dev, const int32_t* list, const uint32_t* n_dev, int64_t n, uint64_t n_ids_space,
-                             uint64_t store_bytes, cudaStream_t st, int32_t** order_out, void** ws_out) {
-    uint32_t shift, nb;
-    uint64_t target = 256ull << 10;
-    if (const char* e = getenv("IBP_BUCKET_BYTES")) target = strtoull(e, nullptr, 10);   // tuning experiments only
-    bucket_shape(n_ids_space, store_bytes, target, &shift, &nb);
-    uint8_t* ws = nullptr;
-    const size_t cnt_bytes = ((size_t)nb * 4 + 255) / 256 * 256;
-    IBP_CUDA(cudaMallocAsync((void**)&ws, cnt_bytes + (size_t)n * 4, st));
-    uint32_t* cnt = (uint32_t*)ws;
-    int32_t* order = (int32_t*)(ws + cnt_bytes);
-    IBP_CUDA(cudaMemsetAsync(cnt, 0, cnt_bytes, st));
-    const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, 148 * 8);
-    ibp_bucket_hist<<<blocks, thr, 0, st>>>(ids_dev, list, n_dev, n, shift, nb, cnt);
-    ibp_bucket_scan<<<1, 1024, 0, st>>>(cnt, nb);
-    ibp_bucket_scatter<<<blocks, thr, 0, st>>>(ids_dev, list, n_dev, n, shift, nb, cnt, order);
-    IBP_CUDA(cudaGetLastError());
-    *order_out = order;
-    *ws_out = ws;
-    return IBP_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ de-duplication
@@ -394,35 +393,109 @@ static ibp_status make_order(const int64_t* ids_dev, const int32_t* list, const 
 // list.  The decode kernel then runs over the work list only, and pass 3 copies each representative's decoded row
 // (HBM -> HBM) to the positions of its repeats.  Output is identical to the plain path.
 __global__ void ibp_dedup_insert(const int64_t* __restrict__ ids, int64_t n, unsigned long long* __restrict__ table, uint32_t mask,
-                                 int32_t* __restrict__ rep, int32_t* __restrict__ uniq, uint32_t* __restrict__ n_uniq) {
+                                 int32_t* __restrict__ rep, int32_t* __restrict__ uniq, uint32_t* __restrict__ n_uniq,
+                                 uint32_t* __restrict__ cnt, uint32_t shift, uint32_t nb) {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const uint64_t key = (uint64_t)ids[i];
         uint32_t slot = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 32) & mask;
-        const unsigned long long mine = (key << 32) | (uint32_t)i;
+        const unsigned long long mine = ((key + 1) << 32) | (uint32_t)i;     // 0 = empty slot
         int32_t r;
         for (;;) {
             unsigned long long cur = table[slot];
-            if (cur == ~0ull) cur = atomicCAS(&table[slot], ~0ull, mine);
-            if (cur == ~0ull) { r = (int32_t)i; uniq[atomicAdd(n_uniq, 1u)] = (int32_t)i; break; }
-            if ((cur >> 32) == key) { r = (int32_t)(uint32_t)cur; break; }
+            if (cur == 0ull) cur = atomicCAS(&table[slot], 0ull, mine);
+            if (cur == 0ull) {
+                r = (int32_t)i;
+                uniq[atomicAdd(n_uniq, 1u)] = (int32_t)i;
+                if (cnt) { const uint64_t bk = key >> shift; atomicAdd(&cnt[bk < nb ? bk : nb - 1], 1u); }   // locality histogram
+                break;
+            }
+            if ((cur >> 32) == key + 1) { r = (int32_t)(uint32_t)cur; break; }
             slot = (slot + 1) & mask;
         }
         rep[i] = r;
     }
 }
+// LPR lanes per row (a power of two, 16 bytes per lane and trip): a 256-byte row keeps half a warp busy, so a warp copies two.
+template <int LPR>
 __global__ void ibp_dedup_copy(const int32_t* __restrict__ rep, int64_t n, uint32_t row_bytes, uint8_t* __restrict__ out) {
-    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
-    for (int64_t i = (int64_t)blockIdx.x * wpc + (threadIdx.x >> 5); i < n; i += (int64_t)gridDim.x * wpc) {
+    constexpr int RPW = 32 / LPR;
+    const int lane = threadIdx.x & 31, sub = lane / LPR, sl = lane % LPR, wpc = blockDim.x >> 5;
+    for (int64_t i = ((int64_t)blockIdx.x * wpc + (threadIdx.x >> 5)) * RPW + sub; i < n; i += (int64_t)gridDim.x * wpc * RPW) {
         const int32_t r = rep[i];
         if (r == (int32_t)i) continue;
         const uint4* src = (const uint4*)(out + (uint64_t)r * row_bytes);
         uint4* dst = (uint4*)(out + (uint64_t)i * row_bytes);
         if (row_bytes % 16 == 0) {
-            for (uint32_t v = lane; v < row_bytes / 16; v += 32) dst[v] = src[v];
+            for (uint32_t v = sl; v < row_bytes / 16; v += LPR) {
+                const uint4 t = src[v];
+                asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst + v), "r"(t.x), "r"(t.y), "r"(t.z), "r"(t.w) : "memory");
+            }
         } else {
-            for (uint32_t v = lane; v < row_bytes / 4; v += 32) ((uint32_t*)dst)[v] = ((const uint32_t*)src)[v];
+            for (uint32_t v = sl; v < row_bytes / 4; v += LPR) ((uint32_t*)dst)[v] = ((const uint32_t*)src)[v];
         }
     }
+}
+
+// Pre-passes of a random gather, in one workspace and one memset: de-duplication (optional), then the locality order
+// (optional) of the surviving positions.  Outputs: list/n_list = processing order (device pointers into the workspace; n_list
+// is nullptr when the count is n), rep = representative position of every id (dedup only).  The caller frees ws on the stream.
+struct RowPrepass {
+    void* ws = nullptr;
+    int32_t* rep = nullptr;
+    const int32_t* list = nullptr;
+    const uint32_t* n_list = nullptr;
+};
+
+static ibp_status rows_prepass(const int64_t* ids_dev, int64_t n, bool dedup, bool order, uint64_t n_ids_space, uint64_t store_bytes,
+                               cudaStream_t st, RowPrepass* R) {
+    uint32_t shift = 0, nb = 0, nb_pad = 0, cap = 0;
+    if (order) {
+        uint64_t target = 256ull << 10;
+        if (const char* e = getenv("IBP_BUCKET_BYTES")) target = strtoull(e, nullptr, 10);   // tuning experiments only
+        bucket_shape(n_ids_space, store_bytes, target, &shift, &nb);
+        nb_pad = (nb + 4095u) / 4096u * 4096u;
+    }
+    if (dedup) { cap = 1024; while ((uint64_t)cap < 2ull * (uint64_t)n) cap <<= 1; }
+    const size_t cnt_bytes = (size_t)nb_pad * 4, tab_bytes = (size_t)cap * 8, idx_bytes = ((size_t)n * 4 + 255) / 256 * 256;
+    const size_t zero_bytes = 256 + cnt_bytes + tab_bytes;
+    uint8_t* ws = nullptr;
+    IBP_CUDA(cudaMallocAsync((void**)&ws, zero_bytes + (dedup ? 2 : 0) * idx_bytes + (order ? idx_bytes : 0), st));
+    R->ws = ws;
+    IBP_CUDA(cudaMemsetAsync(ws, 0, zero_bytes, st));
+    uint32_t* n_uniq = (uint32_t*)ws;
+    uint32_t* cnt = order ? (uint32_t*)(ws + 256) : nullptr;
+    unsigned long long* table = (unsigned long long*)(ws + 256 + cnt_bytes);
+    uint8_t* idx = ws + zero_bytes;
+    const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, 148 * 8);
+    const int32_t* list = nullptr;
+    const uint32_t* n_list = nullptr;
+    if (dedup) {
+        R->rep = (int32_t*)idx;
+        int32_t* uniq = (int32_t*)(idx + idx_bytes);
+        idx += 2 * idx_bytes;
+        ibp_dedup_insert<<<blocks, thr, 0, st>>>(ids_dev, n, table, cap - 1, R->rep, uniq, n_uniq, cnt, shift, nb);
+        list = uniq; n_list = n_uniq;
+    }
+    if (order) {
+        int32_t* ord = (int32_t*)idx;
+        if (!dedup) ibp_bucket_hist<<<blocks, thr, 0, st>>>(ids_dev, nullptr, nullptr, n, shift, nb, cnt);
+        ibp_bucket_scan<<<1, 1024, 0, st>>>(cnt, nb_pad);
+        ibp_bucket_scatter<<<blocks, thr, 0, st>>>(ids_dev, list, n_list, n, shift, nb, cnt, ord);
+        list = ord;
+    }
+    IBP_CUDA(cudaGetLastError());
+    R->list = list;
+    R->n_list = n_list;
+    return IBP_OK;
+}
+
+static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_space, uint64_t store_bytes, cudaStream_t st,
+                             int32_t** order_out, void** ws_out) {
+    RowPrepass R;
+    ibp_status s = rows_prepass(ids_dev, n, false, true, n_ids_space, store_bytes, st, &R);
+    *order_out = (int32_t*)R.list;
+    *ws_out = R.ws;
+    return s;
 }
 
 // ------------------------------------------------------------------------------------------------ launch
@@ -438,6 +511,9 @@ static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64
     }
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
+    // random rows: 2 CTAs per SM keep enough reads in flight for the link; more only widens the window of store pages touched
+    // at once (measured: DLRM 0.716 -> 0.685 ms, GNN 1.388 -> 1.375 ms per batch)
+    if (MODE == MODE_ROWS) occ = std::min(occ, 2);
     int64_t blocks = std::min<int64_t>(blocks_needed, (int64_t)std::max(occ, 1) * sm_count);
     if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
     kern<<<(int)blocks, wpc * 32, smem, st>>>(P);
@@ -647,47 +723,33 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     if (h->p.index_span == 1) {
         if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
         P.n_units = n;
-        void *ws = nullptr, *ws2 = nullptr;
-        const int32_t* list = nullptr;      // work list of batch positions (representatives), or nullptr = all
-        const uint32_t* n_list = nullptr;
-        int32_t* rep = nullptr;
         const bool dedup = (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
-        if (dedup) {
-            uint32_t cap = 1024;
-            while ((uint64_t)cap < 2ull * (uint64_t)n) cap <<= 1;
-            const size_t tab_bytes = (size_t)cap * 8, idx_bytes = ((size_t)n * 4 + 255) / 256 * 256;
-            uint8_t* w2 = nullptr;
-            IBP_CUDA(cudaMallocAsync((void**)&w2, tab_bytes + 2 * idx_bytes + 256, st));
-            ws2 = w2;
-            unsigned long long* table = (unsigned long long*)w2;
-            rep = (int32_t*)(w2 + tab_bytes);
-            int32_t* uniq = (int32_t*)(w2 + tab_bytes + idx_bytes);
-            uint32_t* n_uniq = (uint32_t*)(w2 + tab_bytes + 2 * idx_bytes);
-            IBP_CUDA(cudaMemsetAsync(table, 0xFF, tab_bytes, st));
-            IBP_CUDA(cudaMemsetAsync(n_uniq, 0, 4, st));
-            ibp_dedup_insert<<<(int)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(row_ids_dev, n, table, cap - 1, rep, uniq, n_uniq);
-            IBP_CUDA(cudaGetLastError());
-            list = uniq; n_list = n_uniq;
-        }
         // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
         // Essential for the 4 KB-page pinned store, a few percent for the managed-host store -- unless repeated ids are
         // fetched one by one (dedup off on a batch with repeats), where neighbours in the order collide on the same lines.
         const bool order = h->order_mode == 1 || (h->order_mode < 0 && h->store_used > (64ull << 20) && n >= 4096);
-        if (order) {
-            int32_t* ord = nullptr;
-            s = make_order(row_ids_dev, list, n_list, n, h->p.n_rows, h->store_used, st, &ord, &ws);
+        RowPrepass R;
+        if (dedup || order) {
+            s = rows_prepass(row_ids_dev, n, dedup, order, h->p.n_rows, h->store_used, st, &R);
             if (s != IBP_OK) return s;
-            list = ord;
         }
-        P.order = list;
-        P.n_units_dev = n_list;
+        P.order = R.list;
+        P.n_units_dev = R.n_list;
+        P.keep_l2 = dedup;                  // the replication pass re-reads the decoded rows: keep them in L2
         s = launch_decode(h, P, MODE_ROWS, st);
         if (s == IBP_OK && dedup) {
-            ibp_dedup_copy<<<(int)std::min<int64_t>((n + 7) / 8, 148 * 8), 256, 0, st>>>(rep, n, h->p.row_bytes, (uint8_t*)out_dev);
+            const uint32_t rb = h->p.row_bytes;
+            const int lpr = rb >= 512 ? 32 : rb >= 256 ? 16 : rb >= 128 ? 8 : 4, rpw = 32 / lpr;
+            const int blocks = (int)std::min<int64_t>((n + 8 * rpw - 1) / (8 * rpw), 148 * 8);
+            switch (lpr) {
+                case 32: ibp_dedup_copy<32><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+                case 16: ibp_dedup_copy<16><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+                case 8: ibp_dedup_copy<8><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+                default: ibp_dedup_copy<4><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+            }
             if (cudaGetLastError() != cudaSuccess) { ibp_set_error("ibp_dedup_copy launch failed"); s = IBP_ERR_CUDA; }
         }
-        if (ws) IBP_CUDA(cudaFreeAsync(ws, st));
-        if (ws2) IBP_CUDA(cudaFreeAsync(ws2, st));
+        if (R.ws) IBP_CUDA(cudaFreeAsync(R.ws, st));
         return s;
     }
     if (h->stream_mode)
@@ -831,7 +893,7 @@ extern "C" ibp_status ibp_gather_uncompressed_ex(const void* rows_mapped, uint32
     int32_t* ord = nullptr;
     void* ws = nullptr;
     if (locality_order && n_rows > 0) {
-        ibp_status s = make_order(row_ids_dev, nullptr, nullptr, n, n_rows, n_rows * (uint64_t)row_bytes, st, &ord, &ws);
+        ibp_status s = make_order(row_ids_dev, n, n_rows, n_rows * (uint64_t)row_bytes, st, &ord, &ws);
         if (s != IBP_OK) return s;
     }
     const int wpc = 8;
