@@ -69,6 +69,23 @@ def lib():
         L.ibp_oracle_packed_row.restype = vp
         L.ibp_oracle_gather_decompress.argtypes = [vp, vp, i64, u32, vp]
         L.ibp_oracle_gather_decompress.restype = C.c_int
+        L.ibp_oracle_build_T.argtypes = [vp, u64, u32, u32, u32, u32, u32, u32]
+        L.ibp_oracle_build_T.restype = vp
+        L.ibp_oracle_destroy_T.argtypes = [vp]
+        L.ibp_oracle_destroy_T.restype = None
+        for name in ("n_groups", "n_raw", "stored_bytes", "rowflag_bytes"):
+            f = getattr(L, "ibp_oracle_T_" + name)
+            f.argtypes, f.restype = [vp], u64
+        L.ibp_oracle_T_threshold.argtypes = [vp, u64]
+        L.ibp_oracle_T_threshold.restype = u64
+        L.ibp_oracle_T_mask.argtypes = [vp, u64]
+        L.ibp_oracle_T_mask.restype = vp
+        L.ibp_oracle_T_bitval.argtypes = [vp, u64]
+        L.ibp_oracle_T_bitval.restype = vp
+        L.ibp_oracle_T_row.argtypes = [vp, u64, C.POINTER(u64), C.POINTER(C.c_int)]
+        L.ibp_oracle_T_row.restype = vp
+        L.ibp_oracle_gather_decompress_T.argtypes = [vp, vp, i64, u32, vp]
+        L.ibp_oracle_gather_decompress_T.restype = C.c_int
         _lib = L
     return _lib
 
@@ -189,6 +206,57 @@ class Dataset:
     def close(self):
         if self._h:
             lib().ibp_oracle_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class DatasetT:
+    """Thresholded (paper-default) IBP over a whole table: Mask/Bitval per group with T = ceil(tau N_g), participation
+    bits, raw rows and the per-row bitmask (SURVEY 8(c2) thresholded steps 1-7)."""
+
+    def __init__(self, X, group_kind: int, group_param: int, thr_num: int = 4, thr_den: int = 5, chunk_bytes: int = 4):
+        Xb = _u8(X)
+        self.n_rows, self.row_bytes = Xb.shape
+        self._h = lib().ibp_oracle_build_T(Xb.ctypes.data, self.n_rows, self.row_bytes, group_kind, group_param, thr_num, thr_den, chunk_bytes)
+        if not self._h:
+            raise ValueError("ibp_oracle_build_T rejected its arguments")
+        self.n_groups = int(lib().ibp_oracle_T_n_groups(self._h))
+        self.n_raw = int(lib().ibp_oracle_T_n_raw(self._h))
+        self.stored_bytes = int(lib().ibp_oracle_T_stored_bytes(self._h))
+        self.rowflag_bytes = int(lib().ibp_oracle_T_rowflag_bytes(self._h))
+        self.metadata_bytes = 2 * self.row_bytes * self.n_groups
+
+    def threshold(self, g):
+        return int(lib().ibp_oracle_T_threshold(self._h, g))
+
+    def mask(self, g):
+        return np.ctypeslib.as_array(C.cast(lib().ibp_oracle_T_mask(self._h, g), C.POINTER(C.c_uint8)), (self.row_bytes,)).copy()
+
+    def bitval(self, g):
+        return np.ctypeslib.as_array(C.cast(lib().ibp_oracle_T_bitval(self._h, g), C.POINTER(C.c_uint8)), (self.row_bytes,)).copy()
+
+    def row(self, row_id):
+        """(stored bytes of the row, is_compressed)"""
+        n, f = C.c_uint64(0), C.c_int(0)
+        p = lib().ibp_oracle_T_row(self._h, row_id, C.byref(n), C.byref(f))
+        data = np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_uint8)), (n.value,)).copy() if n.value else np.zeros(0, np.uint8)
+        return data, bool(f.value)
+
+    def gather_decompress(self, ids, index_span: int = 1):
+        ids = np.ascontiguousarray(ids, dtype=np.int64)
+        out = np.zeros((ids.size * index_span, self.row_bytes), np.uint8)
+        if lib().ibp_oracle_gather_decompress_T(self._h, ids.ctypes.data, ids.size, index_span, out.ctypes.data):
+            raise IndexError("row id out of range")
+        return out
+
+    def close(self):
+        if self._h:
+            lib().ibp_oracle_destroy_T(self._h)
             self._h = None
 
     def __del__(self):

@@ -18,6 +18,9 @@
 //   ibp_oracle_build/gather  : equals the plain gather out[i] = X[ids[i]] byte for byte (losslessness)
 //   thresholded mode (T<N)   : round trip; compressed <= raw; participation overhead row_bytes/CS bits
 //                              (P:527 prints 12.5% and 1.6%); at T=N payload == strict payload; hand-worked fixture
+//   ibp_oracle_build_T/gather: equals the plain gather byte for byte; bitmask bytes = ceil(n_rows/8); at tau=1
+//                              Mask/Bitval equal the strict dataset's; T = ceil(tau N_g) against Fig. 2's T=4, N=5;
+//                              hand-worked 5-row dataset fixture (sizes, flags, stored bytes)
 //   Ratios on the paper's real datasets (Tables 2, 4, 5): parity unpinned -- the datasets are not available.
 //
 // Build: g++ -O1 -shared -fPIC oracle/ibp_oracle.cpp -o oracle/libibp_oracle.so
@@ -237,4 +240,95 @@ int ibp_oracle_gather_decompress(const ibp_oracle_ds* d, const int64_t* ids, int
     return bad;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Dataset level, thresholded mode (the paper's default codec; S8c thresholded steps 1-7).
+//   Scope: one Mask/Bitval per group (clustered compression); a single group spanning every row is the paper's
+//   global pair ("For the entire dataset, only one Mask and Bitval is constructed").
+//   T = ceil(tau * N_g) with tau = thr_num/thr_den ("T=0.8N"), per group, N_g = rows of that group.
+//   Every row goes through ibp_oracle_compress_row_T: it is either compressed (participation bits + payloads) or kept
+//   raw, and one bit per row records which (the bitmask of P:363; 1 = compressed).
+//   Canonical store: the stored bytes of the rows, in row-id order, densely concatenated.  (The paper keeps each row in
+//   its original slot; only the first `size` bytes of a slot are meaningful, so the dense form holds the same
+//   information.)
+// ---------------------------------------------------------------------------------------------------------------
+struct ibp_oracle_ds_T {
+    uint64_t n_rows = 0, n_groups = 0, n_raw = 0;
+    uint32_t row_bytes = 0, group_kind = 0, group_param = 0, CS = 4;
+    std::vector<uint8_t> mask, bitval;      // n_groups x row_bytes each
+    std::vector<uint64_t> T;                // per group
+    std::vector<uint64_t> row_offset;       // n_rows + 1 byte offsets into stored
+    std::vector<uint8_t> rowflag;           // ceil(n_rows/8) bytes, bit r = 1 iff row r is compressed
+    std::vector<uint8_t> stored;
+};
+
+static uint64_t group_of_T(const ibp_oracle_ds_T* d, uint64_t id) {
+    return d->group_kind == 0 ? id / d->group_param : id % d->group_param;
+}
+
+ibp_oracle_ds_T* ibp_oracle_build_T(const uint8_t* rows, uint64_t n_rows, uint32_t row_bytes, uint32_t group_kind,
+                                    uint32_t group_param, uint32_t thr_num, uint32_t thr_den, uint32_t CS) {
+    if (!rows || n_rows == 0 || row_bytes == 0 || group_param == 0 || group_kind > 1 || CS == 0 || row_bytes % CS) return nullptr;
+    if (thr_den == 0 || thr_num > thr_den || 2ull * thr_num <= thr_den) return nullptr;   // tau in (0.5, 1], R3
+    ibp_oracle_ds_T* d = new ibp_oracle_ds_T();
+    d->n_rows = n_rows; d->row_bytes = row_bytes; d->group_kind = group_kind; d->group_param = group_param; d->CS = CS;
+    d->n_groups = group_kind == 0 ? (n_rows + group_param - 1) / group_param : (n_rows < group_param ? n_rows : group_param);
+    d->mask.assign(d->n_groups * row_bytes, 0);
+    d->bitval.assign(d->n_groups * row_bytes, 0);
+    d->T.assign(d->n_groups, 0);
+    for (uint64_t g = 0; g < d->n_groups; ++g) {
+        uint64_t first, count, stride;
+        if (group_kind == 0) { first = g * group_param; count = n_rows - first < group_param ? n_rows - first : group_param; stride = row_bytes; }
+        else { first = g; count = (n_rows - g + group_param - 1) / group_param; stride = (uint64_t)group_param * row_bytes; }
+        const uint64_t T = (count * thr_num + thr_den - 1) / thr_den;                     // ceil(tau * N_g)
+        d->T[g] = T;
+        ibp_oracle_group_masks_T(rows + first * row_bytes, count, stride, row_bytes, T, &d->mask[g * row_bytes], &d->bitval[g * row_bytes], nullptr);
+    }
+    d->row_offset.assign(n_rows + 1, 0);
+    d->rowflag.assign((n_rows + 7) / 8, 0);
+    std::vector<uint8_t> tmp(row_bytes);
+    for (uint64_t id = 0; id < n_rows; ++id) {
+        const uint64_t g = group_of_T(d, id);
+        int comp = 0;
+        const uint32_t size = ibp_oracle_compress_row_T(rows + id * row_bytes, &d->mask[g * row_bytes], &d->bitval[g * row_bytes], row_bytes, CS, tmp.data(), &comp);
+        put_bit(d->rowflag.data(), id, comp);
+        if (!comp) d->n_raw += 1;
+        d->row_offset[id + 1] = d->row_offset[id] + size;
+        d->stored.insert(d->stored.end(), tmp.begin(), tmp.begin() + size);
+    }
+    return d;
+}
+
+void ibp_oracle_destroy_T(ibp_oracle_ds_T* d) { delete d; }
+uint64_t ibp_oracle_T_n_groups(const ibp_oracle_ds_T* d) { return d->n_groups; }
+uint64_t ibp_oracle_T_n_raw(const ibp_oracle_ds_T* d) { return d->n_raw; }
+uint64_t ibp_oracle_T_stored_bytes(const ibp_oracle_ds_T* d) { return d->row_offset[d->n_rows]; }
+uint64_t ibp_oracle_T_rowflag_bytes(const ibp_oracle_ds_T* d) { return d->rowflag.size(); }
+uint64_t ibp_oracle_T_threshold(const ibp_oracle_ds_T* d, uint64_t g) { return d->T[g]; }
+const uint8_t* ibp_oracle_T_mask(const ibp_oracle_ds_T* d, uint64_t g) { return &d->mask[g * d->row_bytes]; }
+const uint8_t* ibp_oracle_T_bitval(const ibp_oracle_ds_T* d, uint64_t g) { return &d->bitval[g * d->row_bytes]; }
+const uint8_t* ibp_oracle_T_row(const ibp_oracle_ds_T* d, uint64_t id, uint64_t* nbytes, int* is_compressed) {
+    *nbytes = d->row_offset[id + 1] - d->row_offset[id];
+    *is_compressed = get_bit(d->rowflag.data(), id);
+    return d->stored.data() + d->row_offset[id];
+}
+
+// Gather-decompress in thresholded mode (S8c thresholded step 7): check the per-row bit, copy or decode.
+int ibp_oracle_gather_decompress_T(const ibp_oracle_ds_T* d, const int64_t* ids, int64_t n, uint32_t index_span, uint8_t* out) {
+    int bad = 0;
+    std::vector<uint8_t> in(d->row_bytes + 8);
+    for (int64_t i = 0; i < n; ++i)
+        for (uint32_t j = 0; j < index_span; ++j) {
+            const int64_t id = ids[i] * (int64_t)index_span + j;
+            if (id < 0 || (uint64_t)id >= d->n_rows) { bad = 1; continue; }
+            const uint64_t g = group_of_T(d, (uint64_t)id);
+            const uint64_t size = d->row_offset[id + 1] - d->row_offset[id];
+            std::memset(in.data(), 0, in.size());
+            std::memcpy(in.data(), d->stored.data() + d->row_offset[id], size);
+            ibp_oracle_decompress_row_T(in.data(), get_bit(d->rowflag.data(), (uint64_t)id), &d->mask[g * d->row_bytes],
+                                        &d->bitval[g * d->row_bytes], d->row_bytes, d->CS, out + ((uint64_t)i * index_span + j) * d->row_bytes);
+        }
+    return bad;
+}
+
 }  // extern "C"
+

@@ -300,3 +300,83 @@ def test_thresholded_round_trip_and_bounds(cs):
                 strict, k = oracle.pack_row(r, mask)
                 assert np.array_equal(bits[nch:nch + k], _bits(strict)[:k])
         assert n_comp > 0
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# thresholded mode at dataset level (oracle.DatasetT): Mask/Bitval per group with T = ceil(tau N_g), per-row flags, store
+# ---------------------------------------------------------------------------------------------------------------------
+def test_datasetT_golden_worked_example():
+    """The hand-worked five-tensor example (tests/golden/worked_example_thresholded.txt; T=4, N=5 as in the caption of
+    Fig. 2) run as a one-group dataset with tau = 4/5: flags, sizes, stored bytes, the per-row bitmask
+    (PAPER.md:363, 1 = compressed) and the decoded rows.  Catches a wrong T rounding, swapped flag polarity, a store
+    that is not in row order."""
+    fx = _fixture("worked_example_thresholded.txt")
+    rows = np.stack(_hex(fx["rows"]))
+    ds = oracle.DatasetT(rows, oracle.BLOCKED, 5, 4, 5, chunk_bytes=1)
+    assert ds.n_groups == 1 and ds.threshold(0) == 4
+    assert ds.mask(0).tobytes().hex().upper() == fx["mask"][0]
+    assert ds.bitval(0).tobytes().hex().upper() == fx["bitval"][0]
+    flags = [int(f) for f in fx["compressed"]]
+    for r in range(5):
+        data, comp = ds.row(r)
+        assert comp == bool(flags[r]) and data.tobytes().hex().upper() == fx["stored"][r]
+    assert ds.stored_bytes == sum(len(t) // 2 for t in fx["stored"]) == 8
+    assert ds.n_raw == 3 and ds.rowflag_bytes == 1
+    assert np.array_equal(ds.gather_decompress(np.array([4, 0, 2, 1, 3, 0])), rows[[4, 0, 2, 1, 3, 0]])
+
+
+@pytest.mark.parametrize("n,num,den,want", [(5, 4, 5, 4), (256, 4, 5, 205), (128, 4, 5, 103), (64, 7, 10, 45), (100, 1, 1, 100), (3, 4, 5, 3)])
+def test_datasetT_threshold_rounding(n, num, den, want):
+    """T = ceil(tau N): 'at least T/N = 80 %' and Fig. 2's T=4 for N=5; a floor would give 204/102/44/2."""
+    rows = datagen.random_bytes(n * 8, 3).reshape(n, 8)
+    ds = oracle.DatasetT(rows, oracle.BLOCKED, n, num, den)
+    assert ds.threshold(0) == want
+
+
+@pytest.mark.parametrize("kind,param,n_rows,num,den", [(0, 64, 1000, 4, 5), (0, 256, 700, 7, 10), (1, 6, 600, 4, 5), (0, 1 << 30, 500, 9, 10), (0, 16, 333, 1, 1)])
+def test_datasetT_equals_plain_gather_and_invariants(kind, param, n_rows, num, den):
+    """Losslessness at dataset level for blocked, strided and global (one group) scopes; the compressed
+    dataset never exceeds the raw one; one flag bit per row; raw rows are stored verbatim; the stored size
+    of a compressed row is row_bytes - floor((bitsSaved - chunks)/8) recomputed word-wise in numpy (Fig. 3 lines 13-18)."""
+    w = workloads.GNN(n_rows=4096)
+    X = np.concatenate([w.rows(0, n_rows // 2), w.rows(3000, n_rows - n_rows // 2)])
+    Xb = X.view(np.uint8).reshape(n_rows, -1)
+    rb = Xb.shape[1]
+    ds = oracle.DatasetT(X, kind, min(param, n_rows) if kind == 0 else param, num, den)
+    assert ds.n_groups == (-(-n_rows // min(param, n_rows)) if kind == 0 else param)
+    assert ds.rowflag_bytes == -(-n_rows // 8)
+    assert ds.stored_bytes <= Xb.nbytes
+    ids = (datagen.u64(400, 5) % np.uint64(n_rows)).astype(np.int64)
+    assert np.array_equal(ds.gather_decompress(ids), Xb[ids])
+    total, n_raw = 0, 0
+    W = Xb.view("<u4")
+    for r in range(n_rows):
+        g = r // min(param, n_rows) if kind == 0 else r % param
+        M, B = ds.mask(g).view("<u4"), ds.bitval(g).view("<u4")
+        part = (W[r] & M) == B
+        saved = int(sum(bin(int(m)).count("1") for m in M[part])) - rb // 4
+        size = rb - saved // 8 if saved >= 8 else rb
+        data, comp = ds.row(r)
+        assert data.size == size and comp == (size < rb)
+        if not comp:
+            assert np.array_equal(data, Xb[r])
+            n_raw += 1
+        total += size
+    assert total == ds.stored_bytes and n_raw == ds.n_raw
+
+
+def test_datasetT_tau_one_equals_strict_masks():
+    """At tau = 1 the thresholded masks are the strict ones (>= N / <= 0): equal to oracle.Dataset group by group."""
+    w = workloads.Tiny()
+    X = w.rows(0, 512)
+    a, b = oracle.Dataset(X, oracle.BLOCKED, 64), oracle.DatasetT(X, oracle.BLOCKED, 64, 1, 1)
+    for g in range(a.n_groups):
+        assert np.array_equal(a.mask(g), b.mask(g)) and np.array_equal(a.bitval(g), b.bitval(g))
+    assert b.n_raw == 0
+
+
+def test_datasetT_rejects_tau_at_most_half():
+    """R3: T must exceed N/2 or a bit could be invariant-1 and invariant-0 at once (PAPER.md:231-233 sweeps 0.7..1)."""
+    rows = datagen.random_bytes(64, 1).reshape(8, 8)
+    with pytest.raises(ValueError):
+        oracle.DatasetT(rows, oracle.BLOCKED, 8, 1, 2)
