@@ -8,15 +8,27 @@
  * reads requested rows zero-copy over PCIe, re-inserts the invariant bits from per-group Mask/Bitval
  * metadata held in GPU memory, and writes the original rows into an HBM tensor.
  *
- * Mode: "group-strict" IBP = the paper's clustered compression with clusters that are fixed runs of rows
- * and threshold T = N_group: a bit is invariant iff every row of the group agrees, so every row of a group
- * has the same packed length and there are no participation bits and no per-row raw flag.
+ * Two modes, selected by ibp_build_params.threshold_num/den (= tau = T/N):
+ *   strict (tau = 1, the default): the paper's clustered compression with clusters that are fixed runs of
+ *     rows and T = N_group: a bit is invariant iff every row of the group agrees, so every row of a group has the same
+ *     packed length and there are no participation bits and no per-row raw flag.
+ *   thresholded (1/2 < tau < 1; the paper's default codec, tau = 0.8): a bit is invariant when at least T = ceil(tau N_g)
+ *     rows of the group agree; every 4-byte chunk of a row carries a participation bit saying whether it
+ *     matches Bitval under Mask; rows that would not shrink by a whole byte are kept raw and flagged in a
+ *     one-bit-per-row bitmask held in GPU memory.  A single group spanning all rows (blocked, group_param
+ *     >= n_rows) is the paper's one global Mask/Bitval.  Row sizes depend on the data, so the library keeps a
+ *     4-byte offset per row in GPU memory (16-byte units) over a dense store instead of the paper's fixed in-place
+ *     slots: same bytes cross PCIe, less host memory, contiguous spans stay contiguous.
  *
  * Conventions
  *   - Bit p of a row is bit (p mod 8) of byte (p div 8).  Mask bit 1 = invariant; Bitval holds the invariant values
  *     and is 0 where Mask is 0.
  *   - A packed row is the row's bits at the Mask=0 positions, ascending p, LSB-first, zero padded to ceil(k/8)
  *     bytes and then to `align_bytes` (the alignment unit A).  This is the oracle's canonical order.
+ *   - Thresholded mode: a compressed row is [participation bits, one per 4-byte chunk, chunk order][per chunk: its bits
+ *     at the Mask=0 positions if it participates, else all 32 bits], LSB-first, zero padded to
+ *     row_bytes - floor((bitsSaved - chunks)/8) bytes (Fig. 3 = P:243-299) and then to A; a raw row is the row.
+ *     Rows lie in id order, each starting on a multiple of A (A >= 16 in this mode).
  *   - Store layout.  Blocked groups: groups in order, each group's base aligned to max(A,16); rows of a group at
  *     base + j*stride_g.  Strided groups: matrix row r (= id div S) at r*rowstride, tile t at prefix_t inside it.
  *   - Pointers are named *_host (CPU addressable), *_dev (GPU addressable on the handle's device).
@@ -49,7 +61,7 @@ typedef enum {
     IBP_ERR_OUT_OF_MEMORY = 2,
     IBP_ERR_CUDA = 3,
     IBP_ERR_BAD_STATE = 4,   /* e.g. gather before ibp_upload_metadata */
-    IBP_ERR_UNSUPPORTED = 5  /* e.g. threshold < 1 (the paper's thresholded mode is not on this path) */
+    IBP_ERR_UNSUPPORTED = 5  /* e.g. a thresholded store above 64 GiB, a device that is not sm_100 */
 } ibp_status;
 
 typedef enum {
@@ -75,9 +87,9 @@ typedef struct {
     uint64_t n_rows;
     uint32_t group_kind;    /* ibp_group_kind                                                                    */
     uint32_t group_param;   /* G (blocked) or S (strided); >= 1                                                  */
-    uint32_t threshold_num; /* T/N; only 1/1 (strict) is supported here, 0/0 means 1/1                           */
+    uint32_t threshold_num; /* tau = T/N as a fraction: 1/1 (or 0/0) = strict; 1/2 < tau < 1 = thresholded, e.g. 4/5   */
     uint32_t threshold_den;
-    uint32_t align_bytes;   /* packed-row alignment unit A: power of two in 1..128; 0 = default (32)             */
+    uint32_t align_bytes;   /* packed-row alignment unit A: power of two in 1..128 (16..128 thresholded); 0 = 32 */
     uint32_t index_span;    /* consecutive rows selected by one id in ibp_gather_decompress; 0 = 1               */
     uint32_t flags;         /* IBP_FLAG_*                                                                        */
     uint32_t n_threads;     /* host threads for the build; 0 = all                                               */
@@ -94,6 +106,12 @@ typedef struct {
     uint32_t max_row_stride;           /* largest packed-row stride in bytes                                     */
     int32_t  device;                   /* device holding the metadata, -1 before ibp_upload_metadata             */
     uint32_t store_kind;               /* ibp_store_kind                                                         */
+    uint32_t thresholded;              /* 0 = strict, 1 = thresholded mode                                       */
+    uint32_t threshold_num, threshold_den;
+    uint32_t reserved0;
+    uint64_t n_rows_raw;               /* thresholded: rows kept uncompressed                            */
+    uint64_t rowflag_bytes;            /* thresholded: per-row bitmask, 4*ceil(n_rows/32) bytes          */
+    uint64_t rowoffset_bytes;          /* thresholded: per-row offsets, 4*(n_rows+1) bytes                       */
 } ibp_info;
 
 /* -- S0, S0': host-side compressor (P:229-231 masks with T=N per group; P:237-241, P:275-298 packing). ---------------
@@ -101,8 +119,9 @@ typedef struct {
  * CPU only.  The handle allocates its own packed store in host memory the GPU reads in place (ibp_store_kind:
  * managed-host by default, cudaHostAlloc with IBP_FLAG_HOSTALLOC_STORE) when a CUDA device is present and
  * IBP_FLAG_PAGEABLE_STORE is not set, else ordinary memory (then only ibp_decompress_resident and the host
- * accessors work).  Errors: INVALID_ARG (null pointers, row_bytes not a multiple of 4, bad A, span not
- * compatible with the groups), UNSUPPORTED (threshold != 1), OUT_OF_MEMORY.                                        */
+ * accessors work).  Thresholded mode: per-bit counters, T = ceil(tau N_g), participation bits, raw rows.
+ * Errors: INVALID_ARG (null pointers, row_bytes not a multiple of 4, bad A, tau <= 1/2 or > 1, span not compatible
+ * with the groups), UNSUPPORTED (thresholded store above 64 GiB), OUT_OF_MEMORY.                                   */
 ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle);
 
 /* -- S0'': copy Mask/Bitval and the group table to HBM on `device` ("stored in GPU memory").  Idempotent for the
@@ -124,7 +143,8 @@ ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host
 /* -- S8: decode rows [first_row, first_row+n_rows) whose packed bytes the caller already staged in device memory
  * exactly as they lie in the host store (ibp_packed_range gives the source range; e.g. cudaMemcpyAsync, or a
  * compressed GPU cache slab).  first_row must start a layout unit: a multiple of G (blocked) or of S
- * (strided).  packed_dev must be 16-byte aligned.  Asynchronous on the stream.                                     */
+ * (strided); in thresholded mode with blocked groups every row starts a unit.  packed_dev must be 16-byte aligned.
+ * Asynchronous on the stream.                                                                                      */
 ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_t first_row, int64_t n_rows,
                                    void* out_dev, void* cuda_stream);
 
@@ -136,10 +156,18 @@ ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t
 /* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
 ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
 
-/* Location of one packed row inside the store (host pointer, stride bytes, variant bits k).  For cross-checks.    */
+/* Location of one packed row inside the store (host pointer, stride bytes, variant bits k).  For cross-checks.
+ * Thresholded mode: stride = stored bytes incl. padding, k_bits = 8 * the row's byte-aligned size.                 */
 ibp_status ibp_packed_row(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stride_bytes, uint32_t* k_bits);
 
-/* Host copies of one group's metadata: Mask and Bitval (row_bytes each) and k_g.  For oracle cross-checks.        */
+/* Both modes: where a row lies (host pointer), the bytes it occupies incl. alignment padding, its byte-aligned size
+ * (strict: ceil(k_g/8); thresholded: row_bytes - bytesSaved, or row_bytes when raw) and whether it is compressed
+ * (strict: always 1; thresholded: the row's bit of the bitmask).  Any out pointer may be NULL.               */
+ibp_status ibp_row_info(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stored_bytes, uint32_t* size_bytes,
+                        int* is_compressed);
+
+/* Host copies of one group's metadata: Mask and Bitval (row_bytes each) and k_g = 8*row_bytes - popcount(Mask).  For
+ * oracle cross-checks.                                                                                              */
 ibp_status ibp_get_metadata_host(const ibp_handle* h, int64_t group, const void** mask, const void** bitval, uint32_t* k_bits);
 
 ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out);

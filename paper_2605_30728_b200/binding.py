@@ -41,7 +41,9 @@ class ibp_info(C.Structure):
                 ("metadata_bytes", C.c_uint64), ("aux_bytes", C.c_uint64), ("row_bytes", C.c_uint32),
                 ("align_bytes", C.c_uint32), ("index_span", C.c_uint32), ("group_kind", C.c_uint32),
                 ("group_param", C.c_uint32), ("max_row_stride", C.c_uint32), ("device", C.c_int32),
-                ("store_kind", C.c_uint32)]
+                ("store_kind", C.c_uint32), ("thresholded", C.c_uint32), ("threshold_num", C.c_uint32),
+                ("threshold_den", C.c_uint32), ("reserved0", C.c_uint32), ("n_rows_raw", C.c_uint64),
+                ("rowflag_bytes", C.c_uint64), ("rowoffset_bytes", C.c_uint64)]
 
 
 # name -> (restype, argtypes); every symbol include/ibp.h declares (tests/test_abi.py checks the two lists agree)
@@ -55,6 +57,7 @@ SIGNATURES = {
     "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
     "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
+    "ibp_row_info": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32), C.POINTER(_int)]),
     "ibp_get_metadata_host": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_u32)]),
     "ibp_get_info": (_int, [_vp, C.POINTER(ibp_info)]),
     "ibp_configure": (_int, [_vp, _u32, _u32]),
@@ -140,6 +143,13 @@ class Handle:
         _check(lib().ibp_packed_row(self._h, row, C.byref(p), C.byref(st), C.byref(k)))
         data = np.ctypeslib.as_array(C.cast(p.value, C.POINTER(C.c_uint8)), (st.value,)).copy() if st.value else np.zeros(0, np.uint8)
         return data, k.value
+
+    def row_info(self, row):
+        """(the row's byte-aligned stored bytes, bytes occupied incl. padding, is_compressed)"""
+        p, st, sz, fl = _vp(), _u32(), _u32(), _int()
+        _check(lib().ibp_row_info(self._h, row, C.byref(p), C.byref(st), C.byref(sz), C.byref(fl)))
+        data = np.ctypeslib.as_array(C.cast(p.value, C.POINTER(C.c_uint8)), (sz.value,)).copy() if sz.value else np.zeros(0, np.uint8)
+        return data, st.value, bool(fl.value)
 
     def packed_view(self, host_ptr, nbytes):
         return np.ctypeslib.as_array(C.cast(host_ptr, C.POINTER(C.c_uint8)), (nbytes,))

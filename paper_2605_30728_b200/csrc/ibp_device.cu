@@ -55,6 +55,8 @@ struct DecodeParams {
     uint32_t rows_per_unit, units_per_span;
     uint32_t slot_bytes;
     uint32_t strided;              // group kind of the handle (MODE_ROWS serves both kinds)
+    const uint32_t* row_off;       // thresholded mode: per-row offsets (16-byte units), n_rows + 1 entries
+    const uint32_t* row_flag;      // thresholded mode: bit r = 1 iff row r is compressed
     uint32_t keep_l2;              // write the rows with the default cache policy (a later pass re-reads them) instead of streaming
 };
 
@@ -148,7 +150,11 @@ __device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t gr
 
 #include "ibp_stream.cuh"
 
-template <int W, int NST, int MODE, int FETCH>
+// TM = thresholded mode (the paper's default codec): the row's location and length come from the per-row
+// offset table, the per-row bitmask says whether it is stored raw, the first n_words bits of a compressed row are
+// the participation bits (one per 4-byte chunk), and a chunk contributes 32 - popc(Mask_i) bits if it participates, else 32
+// (reading R7) -- so the exclusive scan of step 3 runs per row instead of per group.
+template <int W, int NST, int MODE, int FETCH, bool TM>
 __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
@@ -222,14 +228,22 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
         auto fetch = [&](uint32_t j) {
             uint64_t id; int64_t oi_unused;
             locate(j, id, oi_unused);
-            const uint64_t g = group_of(P, id, STRIDED);
-            if (g != fg) { fg = g; fe = P.gtab[g]; }
-            const uint64_t off = STRIDED ? (id / P.group_param) * P.row_stride_strided + fe.base
-                                         : fe.base + (id - g * P.group_param) * (uint64_t)fe.stride;
-            const uint8_t* src = P.store + (off - P.bias);
-            const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
-            const uint8_t* a0 = src - head;                                   // 16-byte aligned cover
-            const uint32_t nvec = fe.stride ? (head + fe.stride + 15u) >> 4 : 0u;
+            const uint8_t* a0;
+            uint32_t nvec;
+            if (TM) {
+                const uint32_t o0 = __ldg(P.row_off + id), o1 = __ldg(P.row_off + id + 1);
+                a0 = P.store + (16ull * o0 - P.bias);                         // rows start on 16-byte boundaries
+                nvec = o1 - o0;
+            } else {
+                const uint64_t g = group_of(P, id, STRIDED);
+                if (g != fg) { fg = g; fe = P.gtab[g]; }
+                const uint64_t off = STRIDED ? (id / P.group_param) * P.row_stride_strided + fe.base
+                                             : fe.base + (id - g * P.group_param) * (uint64_t)fe.stride;
+                const uint8_t* src = P.store + (off - P.bias);
+                const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
+                a0 = src - head;                                              // 16-byte aligned cover
+                nvec = fe.stride ? (head + fe.stride + 15u) >> 4 : 0u;
+            }
             const uint32_t slot = seq_f % NST;
             const uint32_t dst = ring_s + slot * P.slot_bytes;
             if (FETCH == FETCH_TMA) {
@@ -256,10 +270,17 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
             uint64_t id; int64_t out_idx;
             locate(j, id, out_idx);
             const uint64_t g = group_of(P, id, STRIDED);
-            if (g != dg) { dg = g; de = P.gtab[g]; }
-            const uint64_t off = STRIDED ? (id / P.group_param) * P.row_stride_strided + de.base
-                                         : de.base + (id - g * P.group_param) * (uint64_t)de.stride;
-            const uint32_t head_bits = (uint32_t)(((uintptr_t)(P.store + (off - P.bias))) & 15u) * 8u;
+            uint32_t head_bits = 0;
+            bool compressed = true;
+            if (TM) {
+                compressed = (__ldg(P.row_flag + (id >> 5)) >> (id & 31u)) & 1u;
+                head_bits = P.n_words;                                        // payloads follow the participation bits (R8)
+            } else {
+                if (g != dg) { dg = g; de = P.gtab[g]; }
+                const uint64_t off = STRIDED ? (id / P.group_param) * P.row_stride_strided + de.base
+                                             : de.base + (id - g * P.group_param) * (uint64_t)de.stride;
+                head_bits = (uint32_t)(((uintptr_t)(P.store + (off - P.bias))) & 15u) * 8u;
+            }
             const uint32_t dslot = seq_d % NST;
             const uint32_t* slot = (const uint32_t*)(ring + (size_t)dslot * P.slot_bytes);
             uint8_t* orow = P.out + (uint64_t)out_idx * P.row_bytes;
@@ -278,12 +299,14 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
 #pragma unroll
                         for (int q = 0; q < W; ++q) { m[q] = 0xFFFFFFFFu; b[q] = 0; }
                     }
-                    uint32_t t = 0;
+                    if (!TM) {
+                        uint32_t t = 0;
 #pragma unroll
-                    for (int q = 0; q < W; ++q) { kk[q] = __popc(~m[q]); t += kk[q]; }
-                    const uint32_t incl = warp_inclusive_scan(t, lane);
-                    excl = incl - t;
-                    tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                        for (int q = 0; q < W; ++q) { kk[q] = __popc(~m[q]); t += kk[q]; }
+                        const uint32_t incl = warp_inclusive_scan(t, lane);
+                        excl = incl - t;
+                        tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                    }
                     meta_g = g;
                 } else {
                     tot = 0;   // single pass: carry is not used again
@@ -292,6 +315,27 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
                     if (FETCH == FETCH_TMA) mbar_wait(bars_s + dslot * 8, (seq_d / NST) & 1u);
                     else { cp_async_wait<NST - 1>(); __syncwarp(); }
                     waited = true;
+                }
+                uint32_t part = 0xFFFFFFFFu;   // bit c = chunk c of this lane participates
+                if (TM) {
+                    if (!compressed) {         // the row was kept raw -- copy it through
+                        if (active) {
+                            uint32_t o[W];
+#pragma unroll
+                            for (int c = 0; c < W; ++c) o[c] = slot[w0 + c];
+                            VecIO<W>::st(orow + (size_t)w0 * 4, o);
+                        }
+                        continue;
+                    }
+                    // S4 per row: participation bits of the lane's W chunks (W divides 32: they sit in one word), kept-bit
+                    // counts, exclusive scan
+                    part = active ? slot[w0 >> 5] >> (w0 & 31u) : 0u;
+                    uint32_t t = 0;
+#pragma unroll
+                    for (int q = 0; q < W; ++q) { kk[q] = active ? (((part >> q) & 1u) ? __popc(~m[q]) : 32u) : 0u; t += kk[q]; }
+                    const uint32_t incl = warp_inclusive_scan(t, lane);
+                    excl = incl - t;
+                    tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
                 }
                 // ---- S5: extract + deposit + OR
                 uint32_t q = head_bits + carry + excl;
@@ -302,7 +346,8 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
                     if (kk[c]) {
                         const uint32_t wq = q >> 5;
                         const uint32_t x = __funnelshift_r(slot[wq], slot[wq + 1], q & 31u);
-                        word |= deposit_runs(x, ~m[c]);
+                        if (TM && !((part >> c) & 1u)) word = x;              // non-participating chunk: all 32 bits
+                        else word |= deposit_runs(x, ~m[c]);
                         q += kk[c];
                     }
                     o[c] = word;
@@ -501,9 +546,9 @@ static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_s
 // ------------------------------------------------------------------------------------------------ launch
 // The grid is persistent: at most as many CTAs as are resident at once, so that the units in flight form one contiguous
 // window of the (locality-ordered) unit list; a larger grid with a grid-stride loop would interleave far-apart windows.
-template <int W, int NST, int MODE, int FETCH>
+template <int W, int NST, int MODE, int FETCH, bool TM = false>
 static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64_t max_ctas, int sm_count, int wpc, size_t smem, cudaStream_t st) {
-    auto kern = ibp_decode_kernel<W, NST, MODE, FETCH>;
+    auto kern = ibp_decode_kernel<W, NST, MODE, FETCH, TM>;
     static thread_local size_t attr_smem = 0;
     if (smem > 48 * 1024 && smem > attr_smem) {
         IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -541,6 +586,7 @@ static ibp_status launch_decode(ibp_handle* h, DecodeParams& P, int mode, cudaSt
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory ring", h->max_stride); return IBP_ERR_UNSUPPORTED; }
     const int64_t blocks = (P.n_units + wpc - 1) / wpc;
 #define IBP_LAUNCH(W_, NST_, MODE_)                                                                                   \
+    if (h->thresholded) return launch_one<W_, NST_, MODE_, FETCH_TMA, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
     return fetch == FETCH_TMA ? launch_one<W_, NST_, MODE_, FETCH_TMA>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st) \
                               : launch_one<W_, NST_, MODE_, FETCH_LSU>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st)
 #define IBP_BY_W(NST_, MODE_)                        \
@@ -571,6 +617,8 @@ static void fill_common(const ibp_handle* h, DecodeParams& P) {
     P.strided = h->p.group_kind == IBP_GROUP_STRIDED;
     P.group_shift = 0xFFFFFFFFu;
     if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t s = 0; while ((1u << s) < h->p.group_param) ++s; P.group_shift = s; }
+    P.row_off = h->row_off_dev;
+    P.row_flag = h->row_flag_dev;
 }
 
 // ------------------------------------------------------------------------------------------------ stream launch
@@ -677,8 +725,14 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
     IBP_CUDA(cudaMalloc((void**)&h->gtab_dev, h->gtab.size() * sizeof(IbpGroupEntry)));
     IBP_CUDA(cudaMemcpyAsync(h->meta_dev, h->meta.data(), h->meta.size() * 4, cudaMemcpyHostToDevice, st));
     IBP_CUDA(cudaMemcpyAsync(h->gtab_dev, h->gtab.data(), h->gtab.size() * sizeof(IbpGroupEntry), cudaMemcpyHostToDevice, st));
+    if (h->thresholded) {
+        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, h->row_off.size() * 4));
+        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, h->row_flag.size() * 4));
+        IBP_CUDA(cudaMemcpyAsync(h->row_off_dev, h->row_off.data(), h->row_off.size() * 4, cudaMemcpyHostToDevice, st));
+        IBP_CUDA(cudaMemcpyAsync(h->row_flag_dev, h->row_flag.data(), h->row_flag.size() * 4, cudaMemcpyHostToDevice, st));
+    }
     // expand move masks per (group, word) when the table has few groups (strided column tiles, small tables): 20 B per word
-    if (h->n_groups * (uint64_t)h->n_words * 20ull <= (8ull << 20)) {
+    if (!h->thresholded && h->n_groups * (uint64_t)h->n_words * 20ull <= (8ull << 20)) {
         const uint64_t cells = h->n_groups * (uint64_t)h->n_words;
         IBP_CUDA(cudaMalloc((void**)&h->mvtab_dev, cells * 20));
         ibp_build_mvtab<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(h->meta_dev, h->n_words, h->n_groups, h->mvtab_dev);
@@ -752,7 +806,7 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
         if (R.ws) IBP_CUDA(cudaFreeAsync(R.ws, st));
         return s;
     }
-    if (h->stream_mode)
+    if (h->stream_mode && !h->thresholded)
         return launch_stream(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
     // (fallback) spans of blocked groups: R consecutive rows per warp, never crossing a group needlessly
     const uint32_t G = h->p.group_param;
@@ -766,7 +820,7 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
 // byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
 static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st) {
-    if (h->stream_mode)
+    if (h->stream_mode && !h->thresholded)
         return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     DecodeParams P;
     fill_common(h, P);
@@ -794,7 +848,8 @@ static ibp_status check_range(const ibp_handle* h, const char* who, int64_t firs
         ibp_set_error("%s: bad argument (range, null pointer or alignment)", who);
         return IBP_ERR_INVALID_ARG;
     }
-    if ((uint64_t)first_row % h->p.group_param) { ibp_set_error("%s: first_row must be a multiple of %u", who, h->p.group_param); return IBP_ERR_INVALID_ARG; }
+    const bool any_row = h->thresholded && h->p.group_kind == IBP_GROUP_BLOCKED;   // per-row offsets: every row starts a unit
+    if (!any_row && (uint64_t)first_row % h->p.group_param) { ibp_set_error("%s: first_row must be a multiple of %u", who, h->p.group_param); return IBP_ERR_INVALID_ARG; }
     if (n_rows > 0xFFFFFFFFll) { ibp_set_error("%s: range too long", who); return IBP_ERR_INVALID_ARG; }
     return IBP_OK;
 }

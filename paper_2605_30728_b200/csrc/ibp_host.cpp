@@ -26,7 +26,7 @@ void ibp_set_error(const char* fmt, ...) {
     va_end(ap);
 }
 extern "C" const char* ibp_last_error(void) { return g_err; }
-extern "C" const char* ibp_version(void) { return "ibp-b200 0.1 (sm_100a, group-strict IBP)"; }
+extern "C" const char* ibp_version(void) { return "ibp-b200 0.2 (sm_100a; group-strict and thresholded IBP)"; }
 
 // ------------------------------------------------------------------------------------------------ bit helpers
 static inline uint64_t pext64_soft(uint64_t v, uint64_t m) {
@@ -84,6 +84,70 @@ static void pack_row_words(const uint32_t* row, const uint32_t* mask, uint32_t n
 
 static inline uint64_t round_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
+// ------------------------------------------------------------------------------------------------ packed store
+// Allocates h->store (h->store_bytes bytes, already set) and zero-fills it.
+static ibp_status alloc_store(ibp_handle* h, int nthreads) {
+    // ---- packed store in host memory that the GPU can read in place (P:239 zero-copy).  Two kinds (DESIGN.md 6):
+    //   managed-host: cudaMallocManaged + preferred location CPU; ibp_upload_metadata adds the direct GPU mapping
+    //                 (accessed-by).  The pages stay in host memory, SM loads cross PCIe, and the GPU maps them
+    //                 with large pages, which is what makes random row gathers translation-friendly.  Default.
+    //   pinned:       cudaHostAlloc(mapped | portable), 4 KB GPU pages.  IBP_FLAG_HOSTALLOC_STORE.
+    // Without a CUDA device (or with IBP_FLAG_PAGEABLE_STORE): ordinary memory, host accessors + resident decode only.
+    const ibp_build_params& p = h->p;
+    bool want_gpu_visible = !(p.flags & IBP_FLAG_PAGEABLE_STORE);
+    if (want_gpu_visible) {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { want_gpu_visible = false; (void)cudaGetLastError(); }
+    }
+    if (want_gpu_visible && !(p.flags & IBP_FLAG_HOSTALLOC_STORE)) {
+        int dev = 0, managed = 0, concurrent = 0;
+        (void)cudaGetDevice(&dev);
+        (void)cudaDeviceGetAttribute(&managed, cudaDevAttrManagedMemory, dev);
+        (void)cudaDeviceGetAttribute(&concurrent, cudaDevAttrConcurrentManagedAccess, dev);
+        void* ptr = nullptr;
+        if (managed && concurrent && cudaMallocManaged(&ptr, h->store_bytes, cudaMemAttachGlobal) == cudaSuccess) {
+            if (cudaMemAdvise(ptr, h->store_bytes, cudaMemAdviseSetPreferredLocation, cudaCpuDeviceId) == cudaSuccess) {
+                h->store = (uint8_t*)ptr;
+                h->store_kind = IBP_STORE_MANAGED_HOST;
+            } else {
+                cudaFree(ptr);
+            }
+        }
+        (void)cudaGetLastError();
+    }
+    if (want_gpu_visible && !h->store) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaHostAlloc(&ptr, h->store_bytes, cudaHostAllocMapped | cudaHostAllocPortable);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            ibp_set_error("ibp_build: cudaHostAlloc(%llu) failed: %s", (unsigned long long)h->store_bytes, cudaGetErrorString(e));
+            return IBP_ERR_OUT_OF_MEMORY;
+        }
+        h->store = (uint8_t*)ptr;
+        h->store_kind = IBP_STORE_PINNED;
+        void* dptr = nullptr;
+        if (cudaHostGetDevicePointer(&dptr, ptr, 0) == cudaSuccess) h->store_dev = (uint8_t*)dptr;
+        else (void)cudaGetLastError();
+    }
+    if (!h->store) {
+        void* ptr = nullptr;
+        if (posix_memalign(&ptr, 4096, h->store_bytes) != 0) { ibp_set_error("ibp_build: out of memory (store)"); return IBP_ERR_OUT_OF_MEMORY; }
+        h->store = (uint8_t*)ptr;
+        h->store_kind = IBP_STORE_PAGEABLE;
+    }
+
+    // ---- S0': pack.  Zero first (padding bytes must be 0), then every row writes exactly ceil(k/8) bytes.
+    {
+        const uint64_t chunk = 1ull << 22, nchunks = (h->store_bytes + chunk - 1) / chunk;
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+        for (int64_t c = 0; c < (int64_t)nchunks; ++c)
+            memset(h->store + (uint64_t)c * chunk, 0, std::min<uint64_t>(chunk, h->store_bytes - (uint64_t)c * chunk));
+    }
+    return IBP_OK;
+}
+
+static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nthreads);
+
 // ------------------------------------------------------------------------------------------------ build
 extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle) {
     if (!rows_host || !params || !out_handle) { ibp_set_error("ibp_build: null argument"); return IBP_ERR_INVALID_ARG; }
@@ -93,9 +157,11 @@ extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* p
     if (p.n_rows == 0 || p.group_param == 0 || p.group_kind > 1) { ibp_set_error("ibp_build: n_rows, group_param must be >= 1 and group_kind 0|1"); return IBP_ERR_INVALID_ARG; }
     if (p.threshold_num == 0 && p.threshold_den == 0) p.threshold_num = p.threshold_den = 1;
     if (p.threshold_den == 0 || p.threshold_num > p.threshold_den) { ibp_set_error("ibp_build: bad threshold"); return IBP_ERR_INVALID_ARG; }
-    if (p.threshold_num != p.threshold_den) { ibp_set_error("ibp_build: thresholded mode (T<N) is not on this path"); return IBP_ERR_UNSUPPORTED; }
+    const bool thresholded = p.threshold_num != p.threshold_den;
+    if (thresholded && 2ull * p.threshold_num <= p.threshold_den) { ibp_set_error("ibp_build: threshold must exceed 1/2 (a bit cannot be invariant-1 and invariant-0 at once)"); return IBP_ERR_INVALID_ARG; }
     if (p.align_bytes == 0) p.align_bytes = 32;
     if (p.align_bytes > 128 || (p.align_bytes & (p.align_bytes - 1))) { ibp_set_error("ibp_build: align_bytes %u must be a power of two <= 128", p.align_bytes); return IBP_ERR_INVALID_ARG; }
+    if (thresholded && p.align_bytes < 16) { ibp_set_error("ibp_build: thresholded mode needs align_bytes >= 16 (row offsets are kept in 16-byte units)"); return IBP_ERR_INVALID_ARG; }
     if (p.index_span == 0) p.index_span = 1;
     if (p.n_rows % p.index_span) { ibp_set_error("ibp_build: n_rows must be a multiple of index_span"); return IBP_ERR_INVALID_ARG; }
     if (p.index_span > 1 && p.group_kind != IBP_GROUP_BLOCKED) { ibp_set_error("ibp_build: index_span > 1 needs blocked groups"); return IBP_ERR_INVALID_ARG; }
@@ -114,6 +180,15 @@ extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* p
         h->meta.assign(ng * 2 * nw, 0);
         h->gtab.assign(ng, IbpGroupEntry{0, 0, 0});
     } catch (...) { delete h; ibp_set_error("ibp_build: out of memory (metadata)"); return IBP_ERR_OUT_OF_MEMORY; }
+
+    if (thresholded) {
+        ibp_status st = IBP_OK;
+        try { st = build_thresholded(h, rows, nthreads); }
+        catch (...) { ibp_set_error("ibp_build: out of memory (thresholded build)"); st = IBP_ERR_OUT_OF_MEMORY; }
+        if (st != IBP_OK) { ibp_destroy(h); return st; }
+        *out_handle = h;
+        return IBP_OK;
+    }
 
     // ---- S0: Mask/Bitval per group.  AND and OR over the rows; a bit is invariant iff AND == OR there (T = N).
     if (p.group_kind == IBP_GROUP_BLOCKED) {
@@ -199,61 +274,9 @@ extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* p
     h->store_used = cursor;
     h->store_bytes = round_up(cursor + 64, 4096);   // slack: 16-byte vector reads may run past the last row
 
-    // ---- packed store in host memory that the GPU can read in place (P:239 zero-copy).  Two kinds (DESIGN.md 6):
-    //   managed-host: cudaMallocManaged + preferred location CPU; ibp_upload_metadata adds the direct GPU mapping
-    //                 (accessed-by).  The pages stay in host memory, SM loads cross PCIe, and the GPU maps them
-    //                 with large pages, which is what makes random row gathers translation-friendly.  Default.
-    //   pinned:       cudaHostAlloc(mapped | portable), 4 KB GPU pages.  IBP_FLAG_HOSTALLOC_STORE.
-    // Without a CUDA device (or with IBP_FLAG_PAGEABLE_STORE): ordinary memory, host accessors + resident decode only.
-    bool want_gpu_visible = !(p.flags & IBP_FLAG_PAGEABLE_STORE);
-    if (want_gpu_visible) {
-        int ndev = 0;
-        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { want_gpu_visible = false; (void)cudaGetLastError(); }
-    }
-    if (want_gpu_visible && !(p.flags & IBP_FLAG_HOSTALLOC_STORE)) {
-        int dev = 0, managed = 0, concurrent = 0;
-        (void)cudaGetDevice(&dev);
-        (void)cudaDeviceGetAttribute(&managed, cudaDevAttrManagedMemory, dev);
-        (void)cudaDeviceGetAttribute(&concurrent, cudaDevAttrConcurrentManagedAccess, dev);
-        void* ptr = nullptr;
-        if (managed && concurrent && cudaMallocManaged(&ptr, h->store_bytes, cudaMemAttachGlobal) == cudaSuccess) {
-            if (cudaMemAdvise(ptr, h->store_bytes, cudaMemAdviseSetPreferredLocation, cudaCpuDeviceId) == cudaSuccess) {
-                h->store = (uint8_t*)ptr;
-                h->store_kind = IBP_STORE_MANAGED_HOST;
-            } else {
-                cudaFree(ptr);
-            }
-        }
-        (void)cudaGetLastError();
-    }
-    if (want_gpu_visible && !h->store) {
-        void* ptr = nullptr;
-        cudaError_t e = cudaHostAlloc(&ptr, h->store_bytes, cudaHostAllocMapped | cudaHostAllocPortable);
-        if (e != cudaSuccess) {
-            (void)cudaGetLastError();
-            ibp_set_error("ibp_build: cudaHostAlloc(%llu) failed: %s", (unsigned long long)h->store_bytes, cudaGetErrorString(e));
-            delete h;
-            return IBP_ERR_OUT_OF_MEMORY;
-        }
-        h->store = (uint8_t*)ptr;
-        h->store_kind = IBP_STORE_PINNED;
-        void* dptr = nullptr;
-        if (cudaHostGetDevicePointer(&dptr, ptr, 0) == cudaSuccess) h->store_dev = (uint8_t*)dptr;
-        else (void)cudaGetLastError();
-    }
-    if (!h->store) {
-        void* ptr = nullptr;
-        if (posix_memalign(&ptr, 4096, h->store_bytes) != 0) { delete h; ibp_set_error("ibp_build: out of memory (store)"); return IBP_ERR_OUT_OF_MEMORY; }
-        h->store = (uint8_t*)ptr;
-        h->store_kind = IBP_STORE_PAGEABLE;
-    }
-
-    // ---- S0': pack.  Zero first (padding bytes must be 0), then every row writes exactly ceil(k/8) bytes.
     {
-        const uint64_t chunk = 1ull << 22, nchunks = (h->store_bytes + chunk - 1) / chunk;
-#pragma omp parallel for schedule(static) num_threads(nthreads)
-        for (int64_t c = 0; c < (int64_t)nchunks; ++c)
-            memset(h->store + (uint64_t)c * chunk, 0, std::min<uint64_t>(chunk, h->store_bytes - (uint64_t)c * chunk));
+        const ibp_status st = alloc_store(h, nthreads);
+        if (st != IBP_OK) { delete h; return st; }
     }
     if (p.group_kind == IBP_GROUP_BLOCKED) {
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
@@ -283,6 +306,212 @@ extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* p
     return IBP_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ thresholded build
+// The paper's default codec (Fig. 3 = P:243-299), own implementation (independent of oracle/):
+//   S0  per-bit counters via bit-sliced planes (8 planes = counts up to 255 per flush), Mask/Bitval from
+//       count >= T / count <= N_g - T with T = ceil(tau N_g)            (reading R2)
+//   S0' per row: participation of each 4-byte chunk ((chunk & Mask) == Bitval), size = row_bytes -
+//       floor((bitsSaved - chunks)/8) or raw (Fig. 3 lines 13-18), offsets, then the bit stream
+//       [participation bits][payloads] written 64 bits at a time with pext
+namespace {
+
+struct BitCounter {                        // counts, for every bit position of a row of nw words, the rows that have it set
+    uint32_t nw, pending = 0;
+    std::vector<uint32_t> planes;          // 8 planes x nw words: plane j holds bit j of the 32 running counters of a word
+    std::vector<uint32_t> cnt;             // 32 x nw totals
+    explicit BitCounter(uint32_t nw_) : nw(nw_), planes(8ull * nw_, 0u), cnt(32ull * nw_, 0u) {}
+    void add(const uint32_t* x) {
+        uint32_t* P = planes.data();
+        for (uint32_t w = 0; w < nw; ++w) {
+            uint32_t c = x[w];
+#pragma GCC unroll 8
+            for (int j = 0; j < 8; ++j) { const uint32_t t = P[j * nw + w]; P[j * nw + w] = t ^ c; c &= t; }
+        }
+        if (++pending == 255) flush();
+    }
+    void flush() {
+        for (int j = 0; j < 8; ++j)
+            for (uint32_t w = 0; w < nw; ++w) {
+                uint32_t v = planes[j * nw + w];
+                planes[j * nw + w] = 0;
+                for (; v; v &= v - 1) cnt[w * 32 + __builtin_ctz(v)] += 1u << j;
+            }
+        pending = 0;
+    }
+    void reset() { std::fill(planes.begin(), planes.end(), 0u); std::fill(cnt.begin(), cnt.end(), 0u); pending = 0; }
+    void merge(BitCounter& o) { o.flush(); for (size_t i = 0; i < cnt.size(); ++i) cnt[i] += o.cnt[i]; }
+};
+
+// Mask/Bitval words of one group from its counters (P:231 with >= / <=, reading R2).  Returns popcount(~Mask).
+uint32_t masks_from_counts(const uint32_t* cnt, uint32_t nw, uint64_t N, uint64_t T, uint32_t* mask, uint32_t* bitval) {
+    uint32_t k = 0;
+    for (uint32_t w = 0; w < nw; ++w) {
+        uint32_t m = 0, b = 0;
+        for (int bit = 0; bit < 32; ++bit) {
+            const uint64_t c = cnt[w * 32 + bit];
+            if (c >= T) { m |= 1u << bit; b |= 1u << bit; }
+            else if (c <= N - T) { m |= 1u << bit; }
+        }
+        mask[w] = m; bitval[w] = b;
+        k += (uint32_t)__builtin_popcount(~m);
+    }
+    return k;
+}
+
+struct BitWriter {                         // LSB-first bit stream into dst; never writes past nbytes
+    uint8_t* dst; uint32_t nbytes, out = 0; uint64_t acc = 0; unsigned fill = 0;
+    BitWriter(uint8_t* d, uint32_t n) : dst(d), nbytes(n) {}
+    inline void put(uint64_t x, unsigned k) {          // k <= 32 bits of x (upper bits of x must be 0)
+        acc |= x << fill;
+        if (fill + k >= 64) {
+            memcpy(dst + out, &acc, 8);
+            out += 8;
+            acc = fill ? (x >> (64 - fill)) : 0;
+            fill = fill + k - 64;
+        } else {
+            fill += k;
+        }
+    }
+    void finish() { for (; out < nbytes; ++out, acc >>= 8) dst[out] = (uint8_t)acc; }
+};
+
+// size in bytes of row x under (mask, bitval); *comp = 0 when it is kept raw (Fig. 3 lines 1-19)
+inline uint32_t row_size_T(const uint32_t* x, const uint32_t* mask, const uint32_t* bitval, uint32_t nw, int* comp) {
+    int64_t saved = 0;
+    for (uint32_t w = 0; w < nw; ++w)
+        if ((x[w] & mask[w]) == bitval[w]) saved += __builtin_popcount(mask[w]);
+    const int64_t bytes_saved = (saved - (int64_t)nw) >= 8 ? (saved - (int64_t)nw) / 8 : 0;
+    *comp = bytes_saved > 0;
+    return (uint32_t)(4ll * nw - bytes_saved);
+}
+
+}  // namespace
+
+static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nthreads) {
+    const ibp_build_params& p = h->p;
+    const uint32_t nw = h->n_words;
+    const uint64_t ng = h->n_groups, G = p.group_param, n = p.n_rows;
+    h->thresholded = true;
+    auto thr = [&](uint64_t N) { return (N * p.threshold_num + p.threshold_den - 1) / p.threshold_den; };
+
+    // ---- S0: counters -> Mask/Bitval
+    if (p.group_kind == IBP_GROUP_BLOCKED && ng >= (uint64_t)nthreads * 4) {
+#pragma omp parallel num_threads(nthreads)
+        {
+            BitCounter bc(nw);
+#pragma omp for schedule(dynamic, 16)
+            for (int64_t g = 0; g < (int64_t)ng; ++g) {
+                const uint64_t first = (uint64_t)g * G, count = std::min<uint64_t>(G, n - first);
+                bc.reset();
+                for (uint64_t r = 0; r < count; ++r) bc.add(rows + (first + r) * nw);
+                bc.flush();
+                uint32_t* m = &h->meta[(uint64_t)g * 2 * nw];
+                h->gtab[g].k_bits = masks_from_counts(bc.cnt.data(), nw, count, thr(count), m, m + nw);
+            }
+        }
+    } else if (p.group_kind == IBP_GROUP_BLOCKED) {
+        // few large groups (e.g. one global Mask/Bitval): split the rows of each group over the threads
+        for (uint64_t g = 0; g < ng; ++g) {
+            const uint64_t first = g * G, count = std::min<uint64_t>(G, n - first);
+            BitCounter total(nw);
+#pragma omp parallel num_threads(nthreads)
+            {
+                BitCounter bc(nw);
+#pragma omp for schedule(static)
+                for (int64_t r = 0; r < (int64_t)count; ++r) bc.add(rows + (first + (uint64_t)r) * nw);
+#pragma omp critical
+                total.merge(bc);
+            }
+            uint32_t* m = &h->meta[g * 2 * nw];
+            h->gtab[g].k_bits = masks_from_counts(total.cnt.data(), nw, count, thr(count), m, m + nw);
+        }
+    } else {
+        // strided: group t = rows with id mod S == t; every thread keeps one counter set per tile
+        const uint64_t S = ng, n_mrows = (n + G - 1) / G;
+        std::vector<BitCounter> total(S, BitCounter(nw));
+#pragma omp parallel num_threads(nthreads)
+        {
+            std::vector<BitCounter> bc(S, BitCounter(nw));
+#pragma omp for schedule(static)
+            for (int64_t r = 0; r < (int64_t)n_mrows; ++r) {
+                const uint64_t id0 = (uint64_t)r * G, cnt = std::min<uint64_t>(G, n - id0);
+                for (uint64_t t = 0; t < cnt; ++t) bc[t].add(rows + (id0 + t) * nw);
+            }
+#pragma omp critical
+            for (uint64_t t = 0; t < S; ++t) total[t].merge(bc[t]);
+        }
+        for (uint64_t t = 0; t < S; ++t) {
+            const uint64_t count = (n - t + G - 1) / G;
+            uint32_t* m = &h->meta[t * 2 * nw];
+            h->gtab[t].k_bits = masks_from_counts(total[t].cnt.data(), nw, count, thr(count), m, m + nw);
+        }
+    }
+
+    // ---- S0' pass 1: sizes, flags, offsets
+    const uint64_t A = p.align_bytes;
+    std::vector<uint32_t> size(n);
+    h->row_flag.assign((n + 31) / 32, 0u);
+    uint64_t n_raw = 0, bytes_aligned = 0;
+#pragma omp parallel for schedule(static) num_threads(nthreads) reduction(+ : n_raw, bytes_aligned)
+    for (int64_t wd = 0; wd < (int64_t)h->row_flag.size(); ++wd) {          // 32 rows per flag word: no write sharing
+        uint32_t flags = 0;
+        for (uint64_t r = (uint64_t)wd * 32; r < std::min<uint64_t>(n, (uint64_t)wd * 32 + 32); ++r) {
+            const uint32_t* m = &h->meta[ibp_group_of(h, r) * 2 * nw];
+            int comp = 0;
+            size[r] = row_size_T(rows + r * nw, m, m + nw, nw, &comp);
+            if (comp) flags |= 1u << (r & 31); else ++n_raw;
+            bytes_aligned += size[r];
+        }
+        h->row_flag[wd] = flags;
+    }
+    h->n_rows_raw = n_raw;
+    h->packed_bytes_bytealigned = bytes_aligned;
+    h->row_off.assign(n + 1, 0u);
+    uint64_t cursor = 0;                                                    // in 16-byte units
+    for (uint64_t r = 0; r < n; ++r) {
+        h->row_off[r] = (uint32_t)cursor;
+        cursor += round_up(size[r], A) / 16;
+        if (cursor > 0xFFFFFFFFull) { ibp_set_error("ibp_build: thresholded store exceeds 64 GiB (4-byte row offsets in 16-byte units)"); return IBP_ERR_UNSUPPORTED; }
+    }
+    h->row_off[n] = (uint32_t)cursor;
+    h->packed_bytes_rows = cursor * 16;
+    h->store_used = cursor * 16;
+    h->store_bytes = round_up(h->store_used + 64, 4096);
+    h->max_stride = (uint32_t)round_up(p.row_bytes, A);
+    for (uint64_t g = 0; g < ng; ++g) { h->gtab[g].base = 0; h->gtab[g].stride = 0; }    // unused in this mode
+
+    ibp_status st = alloc_store(h, nthreads);
+    if (st != IBP_OK) return st;
+
+    // ---- S0' pass 2: the bit streams
+#pragma omp parallel for schedule(dynamic, 1024) num_threads(nthreads)
+    for (int64_t r = 0; r < (int64_t)n; ++r) {
+        const uint32_t* x = rows + (uint64_t)r * nw;
+        uint8_t* dst = h->store + 16ull * h->row_off[r];
+        if (!((h->row_flag[r >> 5] >> (r & 31)) & 1u)) { memcpy(dst, x, 4ull * nw); continue; }
+        const uint32_t* m = &h->meta[ibp_group_of(h, (uint64_t)r) * 2 * nw];
+        const uint32_t* b = m + nw;
+        BitWriter bw(dst, size[r]);
+        for (uint32_t w0 = 0; w0 < nw; w0 += 32) {                           // participation bits, chunk order (R8)
+            uint32_t part = 0;
+            const uint32_t cnt = std::min<uint32_t>(32, nw - w0);
+            for (uint32_t j = 0; j < cnt; ++j) part |= (uint32_t)((x[w0 + j] & m[w0 + j]) == b[w0 + j]) << j;
+            bw.put(part, cnt);
+        }
+        for (uint32_t w = 0; w < nw; ++w) {
+            if ((x[w] & m[w]) == b[w]) {
+                const uint32_t nv = ~m[w];
+                const unsigned k = (unsigned)__builtin_popcount(nv);
+                if (k) bw.put(pext64(x[w], nv), k);
+            } else {
+                bw.put(x[w], 32);
+            }
+        }
+        bw.finish();
+    }
+    return IBP_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ accessors
 extern "C" ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out) {
     if (!h || !out) { ibp_set_error("ibp_get_info: null argument"); return IBP_ERR_INVALID_ARG; }
@@ -302,6 +531,13 @@ extern "C" ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out) {
     out->max_row_stride = h->max_stride;
     out->device = h->device;
     out->store_kind = (uint32_t)h->store_kind;
+    out->thresholded = h->thresholded ? 1u : 0u;
+    out->threshold_num = h->p.threshold_num;
+    out->threshold_den = h->p.threshold_den;
+    out->n_rows_raw = h->n_rows_raw;
+    out->rowflag_bytes = h->row_flag.size() * 4ull;
+    out->rowoffset_bytes = h->row_off.size() * 4ull;
+    if (h->thresholded) out->aux_bytes = out->rowflag_bytes + out->rowoffset_bytes;
     return IBP_OK;
 }
 
@@ -314,9 +550,42 @@ extern "C" ibp_status ibp_get_metadata_host(const ibp_handle* h, int64_t group, 
     return IBP_OK;
 }
 
+// byte-aligned size of a thresholded row, recovered from its stored form (participation bits first)
+static uint32_t row_size_from_store(const ibp_handle* h, uint64_t row) {
+    if (!((h->row_flag[row >> 5] >> (row & 31)) & 1u)) return h->p.row_bytes;
+    const uint32_t nw = h->n_words;
+    const uint32_t* m = &h->meta[ibp_group_of(h, row) * 2 * nw];
+    const uint8_t* src = h->store + 16ull * h->row_off[row];
+    uint64_t bits = nw;
+    for (uint32_t w = 0; w < nw; ++w) bits += ((src[w >> 3] >> (w & 7)) & 1u) ? (uint32_t)__builtin_popcount(~m[w]) : 32u;
+    return (uint32_t)((bits + 7) / 8);
+}
+
+extern "C" ibp_status ibp_row_info(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stored_bytes, uint32_t* size_bytes, int* is_compressed) {
+    if (!h || row < 0 || (uint64_t)row >= h->p.n_rows) { ibp_set_error("ibp_row_info: bad row"); return IBP_ERR_INVALID_ARG; }
+    if (host_ptr) *host_ptr = h->store + ibp_row_offset(h, (uint64_t)row);
+    if (h->thresholded) {
+        if (stored_bytes) *stored_bytes = 16u * (h->row_off[row + 1] - h->row_off[row]);
+        if (size_bytes) *size_bytes = row_size_from_store(h, (uint64_t)row);
+        if (is_compressed) *is_compressed = (int)((h->row_flag[row >> 5] >> (row & 31)) & 1u);
+    } else {
+        const IbpGroupEntry& e = h->gtab[ibp_group_of(h, (uint64_t)row)];
+        if (stored_bytes) *stored_bytes = e.stride;
+        if (size_bytes) *size_bytes = (e.k_bits + 7) / 8;
+        if (is_compressed) *is_compressed = 1;
+    }
+    return IBP_OK;
+}
+
 extern "C" ibp_status ibp_packed_row(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stride_bytes, uint32_t* k_bits) {
     if (!h || row < 0 || (uint64_t)row >= h->p.n_rows) { ibp_set_error("ibp_packed_row: bad row"); return IBP_ERR_INVALID_ARG; }
-    const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? (uint64_t)row / h->p.group_param : (uint64_t)row % h->p.group_param;
+    if (h->thresholded) {
+        uint32_t size = 0;
+        const ibp_status s = ibp_row_info(h, row, host_ptr, stride_bytes, &size, nullptr);
+        if (k_bits) *k_bits = 8u * size;
+        return s;
+    }
+    const uint64_t g = ibp_group_of(h, (uint64_t)row);
     if (host_ptr) *host_ptr = h->store + ibp_row_offset(h, (uint64_t)row);
     if (stride_bytes) *stride_bytes = h->gtab[g].stride;
     if (k_bits) *k_bits = h->gtab[g].k_bits;
@@ -328,10 +597,12 @@ extern "C" ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, i
         ibp_set_error("ibp_packed_range: bad range");
         return IBP_ERR_INVALID_ARG;
     }
-    if ((uint64_t)first_row % h->p.group_param) { ibp_set_error("ibp_packed_range: first_row must start a layout unit (multiple of %u)", h->p.group_param); return IBP_ERR_INVALID_ARG; }
+    if (!(h->thresholded && h->p.group_kind == IBP_GROUP_BLOCKED) && (uint64_t)first_row % h->p.group_param) { ibp_set_error("ibp_packed_range: first_row must start a layout unit (multiple of %u)", h->p.group_param); return IBP_ERR_INVALID_ARG; }
     const uint64_t begin = (uint64_t)first_row < h->p.n_rows ? ibp_row_offset(h, (uint64_t)first_row) : h->store_used;
     uint64_t end = begin;
-    if (n_rows > 0) {
+    if (h->thresholded) {
+        end = 16ull * h->row_off[first_row + n_rows];
+    } else if (n_rows > 0) {
         const uint64_t last = (uint64_t)(first_row + n_rows - 1);
         const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? last / h->p.group_param : last % h->p.group_param;
         end = ibp_row_offset(h, last) + h->gtab[g].stride;
@@ -352,6 +623,7 @@ extern "C" ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* i
         if (id < 0 || (uint64_t)id * span >= h->p.n_rows) { ibp_set_error("ibp_batch_link_bytes: id out of range"); return IBP_ERR_INVALID_ARG; }
         for (uint64_t j = 0; j < span; ++j) {
             const uint64_t r = (uint64_t)id * span + j;
+            if (h->thresholded) { s += 16ull * (h->row_off[r + 1] - h->row_off[r]); b += row_size_from_store(h, r); continue; }
             const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? r / h->p.group_param : r % h->p.group_param;
             s += h->gtab[g].stride;
             b += (h->gtab[g].k_bits + 7) / 8;
@@ -381,6 +653,8 @@ extern "C" void ibp_destroy(ibp_handle* h) {
     if (h->meta_dev) cudaFree(h->meta_dev);
     if (h->gtab_dev) cudaFree(h->gtab_dev);
     if (h->mvtab_dev) cudaFree(h->mvtab_dev);
+    if (h->row_off_dev) cudaFree(h->row_off_dev);
+    if (h->row_flag_dev) cudaFree(h->row_flag_dev);
     if (h->store) {
         if (h->store_kind == IBP_STORE_PINNED) cudaFreeHost(h->store);
         else if (h->store_kind == IBP_STORE_MANAGED_HOST) cudaFree(h->store);

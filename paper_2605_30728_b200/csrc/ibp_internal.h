@@ -32,6 +32,14 @@ struct ibp_handle {
     int store_kind = IBP_STORE_PAGEABLE;   // ibp_store_kind
     uint64_t packed_bytes_rows = 0, packed_bytes_bytealigned = 0;
 
+    // thresholded mode (tau < 1): data-dependent row sizes
+    bool thresholded = false;
+    std::vector<uint32_t> row_off;         // n_rows + 1 offsets into the store, in 16-byte units
+    std::vector<uint32_t> row_flag;        // bit r (word r/32, bit r%32) = 1 iff row r is compressed
+    uint64_t n_rows_raw = 0;
+    uint32_t* row_off_dev = nullptr;
+    uint32_t* row_flag_dev = nullptr;
+
     // device copies
     int device = -1;
     uint32_t* meta_dev = nullptr;
@@ -53,9 +61,15 @@ void ibp_set_error(const char* fmt, ...);
 
 // byte offset of packed row `id` inside the store
 static inline uint64_t ibp_row_offset(const ibp_handle* h, uint64_t id) {
+    if (h->thresholded) return 16ull * h->row_off[id];
     if (h->p.group_kind == IBP_GROUP_BLOCKED) {
         const uint64_t g = id / h->p.group_param;
         return h->gtab[g].base + (id - g * h->p.group_param) * (uint64_t)h->gtab[g].stride;
     }
     return (id / h->p.group_param) * h->row_stride_strided + h->gtab[id % h->p.group_param].base;
+}
+
+// group of a row id
+static inline uint64_t ibp_group_of(const ibp_handle* h, uint64_t id) {
+    return h->p.group_kind == IBP_GROUP_BLOCKED ? id / h->p.group_param : id % h->p.group_param;
 }

@@ -260,3 +260,100 @@ def test_configure_limits_grid_and_streams():
         s.synchronize()
         assert np.array_equal(out.cpu().numpy(), want)
     h.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# thresholded mode (tau < 1): the paper's default codec on the CUDA path (participation bits, raw rows, per-row offsets)
+# ---------------------------------------------------------------------------------------------------------------------
+def _perturbed(n, rb, seed):
+    """Rows with a common structure, some with chunks that break the consensus (non-participating chunks)
+    and some fully random (kept raw)."""
+    rng = np.random.default_rng(seed)
+    keep = datagen.random_bytes(rb, 9)
+    X = (datagen.random_bytes(n * rb, 5 + rb).reshape(n, rb) & keep[None, :]) | 0x01
+    for r in rng.choice(n, max(1, n // 5), replace=False):
+        X[r, rng.integers(0, rb)] ^= 0xFF
+    for r in rng.choice(n, n // 20 + 1, replace=False):
+        X[r] = datagen.random_bytes(rb, 1000 + int(r))
+    return X
+
+
+@pytest.mark.parametrize("align", [16, 32, 128])
+@pytest.mark.parametrize("thr", [(4, 5), (7, 10), (99, 100)])
+def test_T_tiny_config_gather(align, thr):
+    """BASELINE.json configs[0] under the paper's thresholded codec (tau = 0.8 default)."""
+    w = workloads.Tiny()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 64, align_bytes=align, threshold=thr).upload_metadata(0)
+    ds = oracle.DatasetT(X, 0, 64, *thr)
+    assert h.info().n_rows_raw == ds.n_raw
+    for it in range(3):
+        ids = w.ids(it)
+        for order_mode, dedup in ((0, 0), (1, 0), (1, 1)):
+            h.set_order_mode(order_mode).set_dedup_mode(dedup)
+            got = _gather(h, ids)
+            assert np.array_equal(got, ds.gather_decompress(ids))          # (c2) the oracle codec
+            assert np.array_equal(got, oracle.gather_plain(X, ids))        # (c1) the plain definition
+    h.destroy()
+
+
+@pytest.mark.parametrize("kind,param,n,rb,align,thr", [
+    (0, 7, 50, 12, 16, (4, 5)), (0, 64, 3000, 64, 32, (4, 5)), (0, 1000, 10, 8, 16, (4, 5)), (0, 16, 40, 4, 16, (3, 4)),
+    (1, 5, 203, 32, 16, (4, 5)), (1, 8, 64, 16, 32, (4, 5)), (0, 33, 1000, 100, 32, (7, 10)), (0, 128, 700, 256, 32, (4, 5)),
+    (0, 256, 1500, 512, 32, (4, 5)), (0, 50, 333, 1024, 64, (4, 5)), (0, 20, 77, 4096, 64, (4, 5)), (1, 6, 600, 2048, 16, (9, 10)),
+    (0, 9, 100, 516, 16, (4, 5)), (0, 1 << 30, 2000, 128, 32, (4, 5)), (0, 4, 30, 8192, 128, (4, 5)),
+])
+def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
+    """W=1,2,4 and 1..16 passes, ragged last groups, strided groups, one global group; rows with non-participating chunks
+    and raw rows; gather (orders, dedup), zero-copy range, resident decode, partial ranges starting at any row."""
+    X = _perturbed(n, rb, rb + n)
+    gp = min(param, n) if kind == 0 else param
+    h = ibp.ibp_build(X, rb, kind, gp, align_bytes=align, threshold=thr).upload_metadata(0)
+    ds = oracle.DatasetT(X, kind, gp, *thr)
+    info = h.info()
+    assert info.n_rows_raw == ds.n_raw and info.packed_bytes_bytealigned == ds.stored_bytes
+    ids = np.concatenate([(datagen.u64(777, 3) % np.uint64(n)).astype(np.int64), np.arange(n, dtype=np.int64)])
+    want = ds.gather_decompress(ids)
+    assert np.array_equal(want, oracle.gather_plain(X, ids))
+    for mode in (0, 1):
+        h.set_order_mode(mode)
+        for dd in (0, 1):
+            h.set_dedup_mode(dd)
+            assert np.array_equal(_gather(h, ids), want)
+    assert np.array_equal(_resident(h, 0, n), X)
+    assert np.array_equal(_range(h, 0, n), X)
+    if n > 2 * gp:
+        first = gp * ((n // gp) // 2)
+        assert np.array_equal(_resident(h, first, n - first), X[first:])
+        assert np.array_equal(_range(h, first, gp), X[first:first + gp])
+    if kind == 0 and n > 5:
+        assert np.array_equal(_resident(h, 3, n - 5), X[3:n - 2])           # per-row offsets: any row starts a unit
+    h.destroy()
+
+
+def test_T_edge_cases_and_spans():
+    rb = 256
+    r = datagen.random_bytes(rb, 3)
+    special = np.frombuffer(np.array([np.nan, -0.0, 1e-45, np.inf, -np.inf, 0.0, 1.0, -1.0] * 8, np.float32).tobytes(), np.uint8)
+    # group 0: identical rows (every chunk participates, nothing but participation bits is stored);
+    # group 1: rows and complements (no bit reaches T: Mask = 0, every row raw); group 2: special float patterns
+    X = np.stack([r] * 4 + [r, ~r, r, ~r] + [special, special ^ 1, special, special ^ 0x80])
+    h = ibp.ibp_build(X, rb, 0, 4, align_bytes=16, threshold=(3, 4)).upload_metadata(0)
+    ds = oracle.DatasetT(X, 0, 4, 3, 4)
+    data, stored, comp = h.row_info(0)
+    assert comp and data.size == rb // 4 // 8 and stored == 16              # 64 participation bits = 8 bytes (P:527)
+    assert all(not h.row_info(i)[2] for i in range(4, 8))                   # kept raw (P:303)
+    ids = np.array([0, 3, 3, 3, 4, 5, 11, 8, 9, 10, 0, 7], np.int64)
+    assert np.array_equal(_gather(h, ids), X[ids])
+    assert np.array_equal(_gather(h, ids), ds.gather_decompress(ids))
+    assert _gather(h, np.zeros(0, np.int64)).shape[0] == 0
+    assert np.array_equal(_resident(h, 0, 12), X)
+    assert np.array_equal(_resident(h, 5, 6), X[5:11])
+    h.destroy()
+    # index_span > 1 (KV-style page spans) in thresholded mode
+    w = workloads.KV(layers=1, pages=8)
+    Xk = w.table()
+    hk = ibp.ibp_build(Xk, w.row_bytes, w.group_kind, w.group_param, align_bytes=16, index_span=w.index_span, threshold=(4, 5)).upload_metadata(0)
+    ids = np.array([3, 0, 5, 5, 1], np.int64)
+    assert np.array_equal(_gather(hk, ids, span=w.index_span), oracle.gather_plain(Xk, ids, w.index_span))
+    hk.destroy()

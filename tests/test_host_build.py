@@ -106,8 +106,11 @@ def test_argument_errors():
         ibp.ibp_build(X.reshape(-1)[:126].reshape(9, 14), 14, 0, 4)
     assert e.value.status == 1                                   # row_bytes not a multiple of 4 (reading R11)
     with pytest.raises(ibp.IbpError) as e:
-        ibp.ibp_build(X, 16, 0, 4, threshold=(4, 5))
-    assert e.value.status == 5                                   # thresholded mode is not on this path
+        ibp.ibp_build(X, 16, 0, 4, threshold=(1, 2))
+    assert e.value.status == 1                                   # tau must exceed 1/2 (reading R3)
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X, 16, 0, 4, threshold=(4, 5), align_bytes=4)
+    assert e.value.status == 1                                   # thresholded rows start on 16-byte units
     with pytest.raises(ibp.IbpError) as e:
         ibp.ibp_build(X, 16, 0, 4, align_bytes=48)
     assert e.value.status == 1
@@ -138,3 +141,74 @@ def test_batch_link_bytes():
         want_b += (k + 7) // 8
     assert (stored, ba) == (want_s, want_b)
     h.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# thresholded mode (tau < 1; the paper's default codec): the library's compressor against oracle.DatasetT
+# ---------------------------------------------------------------------------------------------------------------------
+def _check_T_against_oracle(X, kind, param, thr, align=32, rows_to_check=None):
+    Xb = np.ascontiguousarray(X).view(np.uint8).reshape(X.shape[0], -1)
+    n, rb = Xb.shape
+    h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, flags=ibp.IBP_FLAG_PAGEABLE_STORE, threshold=thr)
+    ds = oracle.DatasetT(Xb, kind, param, thr[0], thr[1])
+    info = h.info()
+    assert info.thresholded == 1 and (info.threshold_num, info.threshold_den) == thr
+    assert info.n_groups == ds.n_groups
+    assert info.metadata_bytes == ds.metadata_bytes
+    assert info.n_rows_raw == ds.n_raw
+    assert info.packed_bytes_bytealigned == ds.stored_bytes                 # sum of the byte-aligned row sizes
+    assert info.rowflag_bytes == 4 * (-(-n // 32))                          # one bit per row, in 32-bit words
+    for g in range(ds.n_groups):
+        m, b, k = h.metadata_host(g)
+        assert np.array_equal(m, ds.mask(g)) and np.array_equal(b, ds.bitval(g))
+        assert k == 8 * rb - int(np.unpackbits(ds.mask(g)).sum())
+    A = info.align_bytes
+    total = 0
+    for r in (range(n) if rows_to_check is None else rows_to_check):
+        data, stored, comp = h.row_info(r)
+        want, want_comp = ds.row(r)
+        assert comp == want_comp
+        assert np.array_equal(data, want)                                   # canonical bytes: participation bits, payloads
+        assert stored == -(-want.size // A) * A
+        total += stored
+    if rows_to_check is None:
+        assert total == info.packed_bytes_rows
+        ptr, nbytes = h.packed_range(0, n)
+        assert nbytes == total
+        nu, st, ba = h.batch_link_bytes(np.arange(n, dtype=np.int64))
+        assert (nu, st, ba) == (n, total, ds.stored_bytes)
+    h.destroy()
+    ds.close()
+
+
+def test_T_golden_worked_example_rows_padded_to_4_bytes():
+    """The hand-worked example of tests/golden/worked_example_thresholded.txt uses 1-byte chunks; the library fixes 4-byte
+    chunks (reading R10), so the same five tensors are checked through the oracle at CS=4 here and the fixture itself
+    in test_oracle_pins.py."""
+    rows = np.array([[0xB4, 0x0F, 0xB4, 0x0F], [0xA6, 0x0F, 0xA6, 0x0F], [0xB5, 0x0F, 0xB5, 0x0F], [0xA4, 0x1F, 0xA4, 0x1F],
+                     [0x36, 0x0E, 0x36, 0x0E]] * 3, np.uint8)
+    _check_T_against_oracle(rows, 0, 5, (4, 5), align=16)
+
+
+@pytest.mark.parametrize("kind,param,n,rb,thr", [(0, 64, 1000, 64, (4, 5)), (0, 7, 50, 12, (4, 5)), (0, 256, 700, 512, (7, 10)),
+                                                 (1, 5, 203, 32, (4, 5)), (1, 6, 600, 256, (9, 10)), (0, 1 << 30, 900, 128, (4, 5)),
+                                                 (0, 300, 1000, 8, (4, 5)), (0, 16, 100, 2048, (3, 4))])
+def test_T_shapes_against_oracle(kind, param, n, rb, thr):
+    rng = np.random.default_rng(rb + n)
+    keep = datagen.random_bytes(rb, 9)
+    X = (datagen.random_bytes(n * rb, 5 + rb).reshape(n, rb) & keep[None, :]) | 0x01
+    # rows that break the consensus in some chunks (non-participating chunks) and some that break all (raw rows)
+    for r in rng.choice(n, n // 5, replace=False):
+        X[r, rng.integers(0, rb)] ^= 0xFF
+    for r in rng.choice(n, n // 20 + 1, replace=False):
+        X[r] = datagen.random_bytes(rb, 1000 + int(r))
+    _check_T_against_oracle(X, kind, min(param, n) if kind == 0 else param, thr)
+
+
+def test_T_workload_shapes():
+    w = workloads.GNN(n_rows=4096)
+    X = np.concatenate([w.rows(0, 1024), w.rows(3000, 1024)])
+    _check_T_against_oracle(X, 0, 256, (4, 5))
+    _check_T_against_oracle(X, 0, 1 << 20, (4, 5), rows_to_check=range(0, 2048, 7))   # one global Mask/Bitval (P:231)
+    t = workloads.Tiny(n_rows=512).table()
+    _check_T_against_oracle(t, 0, 64, (4, 5), align=16)
