@@ -109,7 +109,7 @@ class OracleSample:
     """The CPU oracle on a bounded sample of the workload: a few hundred groups of the table (built once with the
     oracle's own compressor), then ids of the workload's batch sampler that fall in those groups.  Single thread."""
 
-    def __init__(self, w):
+    def __init__(self, w, thr=(1, 1)):
         import oracle
         self.oracle, self.w = oracle, w
         G = w.group_param
@@ -125,7 +125,7 @@ class OracleSample:
         gi = np.searchsorted(groups, sel // G)
         self.local = (starts[gi] + sel % G).astype(np.int64)
         self.n_groups = len(groups)
-        self.ds = oracle.Dataset(self.X, 0, G)
+        self.ds = oracle.Dataset(self.X, 0, G) if thr[0] == thr[1] else oracle.DatasetT(self.X, 0, G, thr[0], thr[1])
         reps = np.resize(self.local, 2000)
         t0 = time.perf_counter()
         self.ds.gather_decompress(reps)
@@ -144,8 +144,13 @@ class OracleSample:
         return n * w.row_bytes / dt * 1e-9, n / dt, desc
 
 
-def oracle_sample(w, seconds_target=12.0):
-    return OracleSample(w).run(seconds_target)
+def oracle_sample(w, seconds_target=12.0, thr=(1, 1)):
+    return OracleSample(w, thr).run(seconds_target)
+
+
+def parse_threshold(text):
+    num, den = (int(t) for t in text.split("/"))
+    return num, den
 
 
 def run_reference(args):
@@ -153,7 +158,7 @@ def run_reference(args):
     if rank != 0:
         return
     w = make_workload(args.workload)
-    smp = OracleSample(w)
+    smp = OracleSample(w, parse_threshold(args.threshold))
     per_step = max(0.2, min(10.0, 90.0 / max(1, args.steps + args.warmup)))
     vals, desc = [], ""
     for s in range(args.warmup + args.steps):
@@ -199,8 +204,9 @@ def run_cuda(args):
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
     align = args.align if args.align else w.align_bytes
+    thr = parse_threshold(args.threshold)
     h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
-                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0)
+                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0, threshold=thr)
     t_build = time.perf_counter() - t0
     h.upload_metadata(local)
     if args.order is not None:
@@ -338,7 +344,7 @@ def run_cuda(args):
         resident = {"rows": nr, "ms": round(t_r, 4), "out_GBps": round(nr * w.row_bytes / (t_r * 1e-3) * 1e-9, 1),
                     "in_plus_out_GBps": round((nb + nr * w.row_bytes) / (t_r * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": hbm_peak,
                     "frac": round((nb + nr * w.row_bytes + meta_bytes) / (t_r * 1e-3) * 1e-9 / hbm_peak, 4),
-                    "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes), "kernel": "ibp_stream_kernel (ibp_decompress_resident)",
+                    "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes), "kernel": ("ibp_decode_kernel" if info.thresholded else "ibp_stream_kernel") + " (ibp_decompress_resident)",
                     "what": "packed bytes of the first rows of the table staged in HBM, decoded to HBM; L2 flushed between launches"}
         del staged, outr
 
@@ -363,7 +369,7 @@ def run_cuda(args):
     # ---- CPU oracle baseline on a bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        g, rps, desc = oracle_sample(w, seconds_target=12.0)
+        g, rps, desc = oracle_sample(w, seconds_target=12.0, thr=thr)
         cpu = {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)}
 
     if rank == 0:
@@ -374,6 +380,7 @@ def run_cuda(args):
             "rows_per_s": round(world * K * n_rows_out / (t_job * 1e-3), 1),
             "config": {
                 "workload": describe(w), "rows_per_step": n_rows_out, "row_bytes": w.row_bytes, "align_bytes": info.align_bytes,
+                "codec": "group-strict (tau = 1)" if not info.thresholded else f"thresholded, tau = {thr[0]}/{thr[1]} per group, 4-byte chunks, participation bits; {info.n_rows_raw} of {info.n_rows} rows kept raw",
                 "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
                 "locality_order": bool(order_on), "dedup": bool(dedup_on), "ids_unique_by_construction": bool(w.ids_unique), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
                 "ratio_stored": round(ratio_stored, 4), "ratio_bytealigned": round(ratio_alg, 4),
@@ -382,9 +389,9 @@ def run_cuda(args):
             },
             "roofline": {
                 "bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
-                "frac": round(achieved / h2d_ceiling, 4), "traffic": (NCU_TRAFFIC.get(w.name) or {}).get("dram"),
-                "traffic_sysmem": (NCU_TRAFFIC.get(w.name) or {}).get("sysmem"),
-                "kernel": "ibp_stream_kernel" if w.index_span > 1 else "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
+                "frac": round(achieved / h2d_ceiling, 4), "traffic": None if info.thresholded else (NCU_TRAFFIC.get(w.name) or {}).get("dram"),
+                "traffic_sysmem": None if info.thresholded else (NCU_TRAFFIC.get(w.name) or {}).get("sysmem"),
+                "kernel": "ibp_stream_kernel" if (w.index_span > 1 and not info.thresholded) else "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
                 "algorithmic_bytes_per_launch": int(np.mean(stored_timed)),
                 "zero_copy_read_ceiling": round(zc_ceiling, 3), "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
                 "effective_roofline_GBps": round(float(eff_roof), 2), "frac_of_effective_roofline": round(value / world / float(eff_roof), 4),
@@ -428,7 +435,8 @@ def run_weights(args):
         for wm in workloads.weight_layer(l):
             X = wm.table()
             h = ibp.ibp_build(X, 256, 1, wm.group_param, align_bytes=args.align if args.align else 16,
-                              flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0).upload_metadata(0)
+                              flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0,
+                              threshold=parse_threshold(args.threshold)).upload_metadata(0)
             if args.decode_ctas:
                 h.configure(args.decode_ctas, 0)
             info = h.info()
@@ -562,6 +570,7 @@ def main():
     ap.add_argument("--gemm-m", type=int, default=16384, help="weights workload: rows of the consumer GEMM's activation")
     ap.add_argument("--decode-ctas", type=int, default=0, help="limit the decode grid (SM share of the fetch); 0 = library default")
     ap.add_argument("--store", default="managed", choices=["managed", "pinned"])
+    ap.add_argument("--threshold", default="1/1", help="tau = T/N as a fraction: 1/1 = group-strict (BASELINE.json), 4/5 = the paper's thresholded codec")
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
     ap.add_argument("--no-baseline", action="store_true")

@@ -149,6 +149,7 @@ __device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t gr
 }
 
 #include "ibp_stream.cuh"
+#include "ibp_stream_t.cuh"
 
 // TM = thresholded mode (the paper's default codec): the row's location and length come from the per-row
 // offset table, the per-row bitmask says whether it is stored raw, the first n_words bits of a compressed row are
@@ -702,6 +703,86 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
 #undef IBP_STREAM
 }
 
+// Thresholded-mode contiguous runs through ibp_stream_t_kernel.  Returns IBP_ERR_UNSUPPORTED (without setting an error
+// the caller would report) when the shape does not fit: the caller then uses the per-row kernel.
+template <int W, int NS>
+static ibp_status launch_stream_t_one(const StreamTParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
+    constexpr int NW = 8;
+    auto kern = ibp_stream_t_kernel<W, NS, NW>;
+    static thread_local size_t attr_smem = 0;
+    if (smem > 48 * 1024 && smem > attr_smem) {
+        IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    int occ = 0;
+    IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
+    int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
+    if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
+    kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(P);
+    IBP_CUDA(cudaGetLastError());
+    return IBP_OK;
+}
+
+static bool stream_t_fits(const ibp_handle* h) {
+    const int W = pick_W(h->p.row_bytes);
+    if ((h->n_words + 32 * W - 1) / (32 * W) != 1) return false;                       // single-pass rows only
+    if (h->p.group_kind == IBP_GROUP_STRIDED && (uint64_t)h->p.group_param * h->max_stride + 64 > 96ull * 1024) return false;
+    return true;
+}
+
+static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
+                                  int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st) {
+    if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+    const int W = pick_W(h->p.row_bytes);
+    const uint32_t NW = 8;
+    StreamTParams P;
+    memset(&P, 0, sizeof P);
+    P.store = packed; P.bias = bias;
+    P.meta = h->meta_dev; P.row_off = h->row_off_dev; P.row_flag = h->row_flag_dev;
+    P.ids = ids_dev; P.out = (uint8_t*)out_dev;
+    P.first_row = first_row; P.span_rows = span_rows;
+    P.row_bytes = h->p.row_bytes; P.n_words = h->n_words;
+    P.group_param = h->p.group_param;
+    P.group_shift = 0xFFFFFFFFu;
+    if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t sft = 0; while ((1u << sft) < h->p.group_param) ++sft; P.group_shift = sft; }
+    P.strided = h->p.group_kind == IBP_GROUP_STRIDED;
+    const uint64_t stride = h->max_stride;                                             // a raw row: the largest stored row
+    uint64_t per;                                                                      // consecutive rows per chunk
+    if (!P.strided) {
+        const uint32_t U = 16;
+        uint64_t rc = std::min<uint64_t>((uint64_t)NW * U, (48ull * 1024) / stride);
+        rc = std::max<uint64_t>(rc, 1);
+        if (rc >= U) rc = rc / U * U;
+        rc = (uint64_t)std::min<int64_t>((int64_t)rc, span_rows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = (uint32_t)std::min<uint64_t>(U, rc);
+        per = rc;
+    } else {
+        const uint64_t S = h->p.group_param, rs = S * stride;
+        uint64_t rc = std::max<uint64_t>(1, std::min<uint64_t>(32, (48ull * 1024) / rs));
+        const int64_t n_mrows = (span_rows + (int64_t)S - 1) / (int64_t)S;
+        rc = (uint64_t)std::min<int64_t>((int64_t)rc, n_mrows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = (uint32_t)rc;
+        per = rc * S;
+    }
+    P.stage_bytes = (uint32_t)((per * stride + 64 + 127) / 128 * 128);
+    P.chunks_per_span = (uint32_t)((span_rows + (int64_t)per - 1) / (int64_t)per);
+    P.n_chunks = n_spans * (int64_t)P.chunks_per_span;
+    const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
+    const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
+    if (smem > 220 * 1024) { ibp_set_error("thresholded rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
+#define IBP_STREAM_T(W_)                                                                          \
+    return ns == 2 ? launch_stream_t_one<W_, 2>(P, h->max_ctas, h->sm_count, smem, st)            \
+                   : launch_stream_t_one<W_, 3>(P, h->max_ctas, h->sm_count, smem, st)
+    switch (W) {
+        case 4: IBP_STREAM_T(4);
+        case 2: IBP_STREAM_T(2);
+        default: IBP_STREAM_T(1);
+    }
+#undef IBP_STREAM_T
+}
+
 static ibp_status check_ready(const ibp_handle* h, const char* who) {
     if (!h) { ibp_set_error("%s: null handle", who); return IBP_ERR_INVALID_ARG; }
     if (h->device < 0 || !h->meta_dev) { ibp_set_error("%s: call ibp_upload_metadata first", who); return IBP_ERR_BAD_STATE; }
@@ -806,6 +887,8 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
         if (R.ws) IBP_CUDA(cudaFreeAsync(R.ws, st));
         return s;
     }
+    if (h->stream_mode && h->thresholded && stream_t_fits(h))
+        return launch_stream_t(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
     if (h->stream_mode && !h->thresholded)
         return launch_stream(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
     // (fallback) spans of blocked groups: R consecutive rows per warp, never crossing a group needlessly
@@ -820,6 +903,8 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
 // byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
 static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st) {
+    if (h->stream_mode && h->thresholded && stream_t_fits(h))
+        return launch_stream_t(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     if (h->stream_mode && !h->thresholded)
         return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     DecodeParams P;

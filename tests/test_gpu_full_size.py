@@ -114,3 +114,49 @@ def test_full_weight_layer(layer):
         assert np.array_equal(out.cpu().numpy(), _u8(X))
         _check_codec_on_groups(h, X, [0, w.group_param - 1], None, strided_S=w.group_param)
         h.destroy()
+
+
+def _check_T_codec_on_groups(h, X, group_ids, G, thr):
+    """Oracle (c2, thresholded) on sampled groups: Mask/Bitval from counters with T = ceil(tau N_g), and the stored form of
+    every row of the group (flag, size, canonical bytes)."""
+    Xb = _u8(X)
+    for g in group_ids:
+        rows = Xb[g * G:(g + 1) * G]
+        T = -(-rows.shape[0] * thr[0] // thr[1])
+        mask, bitval, _ = oracle.group_masks(rows, T=T)
+        m, b, _ = h.metadata_host(int(g))
+        assert np.array_equal(m, mask) and np.array_equal(b, bitval)
+        for j in range(0, rows.shape[0], 37):
+            want, comp = oracle.compress_row_T(rows[j], mask, bitval, 4)
+            data, _, flag = h.row_info(int(g) * G + j)
+            assert flag == comp and np.array_equal(data, want)
+            assert np.array_equal(oracle.decompress_row_T(data, flag, mask, bitval, 4), rows[j])
+
+
+def test_full_gnn_thresholded():
+    """configs[1] at full size under the paper's default codec (tau = 0.8 per group)."""
+    w = workloads.GNN()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 256, align_bytes=32, threshold=(4, 5)).upload_metadata(0)
+    info = h.info()
+    assert info.thresholded == 1 and info.n_groups == 39063 and info.rowflag_bytes == 4 * 312_500
+    assert info.packed_bytes_bytealigned < X.nbytes
+    for it in (0, 1):
+        ids = w.ids(it)
+        got = _gather(h, ids, len(ids), 512)
+        assert np.array_equal(got, oracle.gather_plain(X, ids))
+    touched = np.unique(w.ids(0) // 256)
+    _check_T_codec_on_groups(h, X, list(touched[:6]) + list(touched[-6:]) + [27343, 39062], 256, (4, 5))
+    h.destroy()
+
+
+def test_full_dlrm_thresholded():
+    w = workloads.DLRM()
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 128, align_bytes=32, threshold=(4, 5)).upload_metadata(0)
+    ids = w.ids(0)
+    got = _gather(h, ids, len(ids), 256)
+    assert np.array_equal(got, oracle.gather_plain(X, ids))
+    touched = np.unique(ids // 128)
+    _check_T_codec_on_groups(h, X, list(touched[:5]) + list(touched[-5:]), 128, (4, 5))
+    h.destroy()

@@ -320,14 +320,16 @@ def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
         for dd in (0, 1):
             h.set_dedup_mode(dd)
             assert np.array_equal(_gather(h, ids), want)
-    assert np.array_equal(_resident(h, 0, n), X)
-    assert np.array_equal(_range(h, 0, n), X)
-    if n > 2 * gp:
-        first = gp * ((n // gp) // 2)
-        assert np.array_equal(_resident(h, first, n - first), X[first:])
-        assert np.array_equal(_range(h, first, gp), X[first:first + gp])
-    if kind == 0 and n > 5:
-        assert np.array_equal(_resident(h, 3, n - 5), X[3:n - 2])           # per-row offsets: any row starts a unit
+    for sm in (0, 1):                                                       # per-row fetch kernel / TMA stream kernel
+        h.set_stream_mode(sm)
+        assert np.array_equal(_resident(h, 0, n), X)
+        assert np.array_equal(_range(h, 0, n), X)
+        if n > 2 * gp:
+            first = gp * ((n // gp) // 2)
+            assert np.array_equal(_resident(h, first, n - first), X[first:])
+            assert np.array_equal(_range(h, first, gp), X[first:first + gp])
+        if kind == 0 and n > 5:
+            assert np.array_equal(_resident(h, 3, n - 5), X[3:n - 2])       # per-row offsets: any row starts a unit
     h.destroy()
 
 
@@ -355,5 +357,7 @@ def test_T_edge_cases_and_spans():
     Xk = w.table()
     hk = ibp.ibp_build(Xk, w.row_bytes, w.group_kind, w.group_param, align_bytes=16, index_span=w.index_span, threshold=(4, 5)).upload_metadata(0)
     ids = np.array([3, 0, 5, 5, 1], np.int64)
-    assert np.array_equal(_gather(hk, ids, span=w.index_span), oracle.gather_plain(Xk, ids, w.index_span))
+    for sm in (0, 1):
+        hk.set_stream_mode(sm)
+        assert np.array_equal(_gather(hk, ids, span=w.index_span), oracle.gather_plain(Xk, ids, w.index_span))
     hk.destroy()
