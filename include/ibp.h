@@ -124,6 +124,19 @@ typedef struct {
  * with the groups), UNSUPPORTED (thresholded store above 64 GiB), OUT_OF_MEMORY.                                   */
 ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle);
 
+/* -- GPU-side compressor (P:227-229 preprocessing "performed on the GPU", P:239 tensors partitioned
+ * among warps, Fig. 3 = P:243-299; the way to build masks online, e.g. per-prefill KV masks).
+ * rows_dev: n_rows x row_bytes, row-major, 16-byte aligned, readable by `device`: HBM, or pinned / managed host memory
+ * read zero-copy.  Same parameters, modes and result as ibp_build -- identical Mask/Bitval/k_g and identical
+ * packed bytes -- but S0 (AND/OR reduction or bit-sliced per-bit counters) and S0' (sizes, offsets, bit packing) run in
+ * CUDA kernels, and the packed rows are written in place into the host store over PCIe.  The returned handle is
+ * already attached to `device` (no ibp_upload_metadata needed; calling it is a no-op).  Host work that remains: the
+ * store allocation, the prefix sum over per-group sizes (strict), copies of the metadata for the host accessors.
+ * Synchronises the stream.  Errors as ibp_build, plus INVALID_ARG for IBP_FLAG_PAGEABLE_STORE, CUDA/UNSUPPORTED for a
+ * missing or non-sm_100 device, UNSUPPORTED for groups of more than 2^32-1 rows.                                    */
+ibp_status ibp_build_device(const void* rows_dev, const ibp_build_params* params, int device, void* cuda_stream,
+                            ibp_handle** out_handle);
+
 /* -- S0'': copy Mask/Bitval and the group table to HBM on `device` ("stored in GPU memory").  Idempotent for the
  * same device; INVALID_ARG for a second device.  Synchronises the stream before returning.                         */
 ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream);

@@ -50,6 +50,7 @@ class ibp_info(C.Structure):
 _vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int
 SIGNATURES = {
     "ibp_build": (_int, [_vp, C.POINTER(ibp_build_params), C.POINTER(_vp)]),
+    "ibp_build_device": (_int, [_vp, C.POINTER(ibp_build_params), _int, _vp, C.POINTER(_vp)]),
     "ibp_upload_metadata": (_int, [_vp, _int, _vp]),
     "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
@@ -222,6 +223,16 @@ def ibp_build(rows_host: np.ndarray, row_bytes: int, group_kind: int, group_para
                          threshold[0], threshold[1], align_bytes, index_span, flags, n_threads)
     h = _vp()
     _check(lib().ibp_build(rows.ctypes.data, C.byref(p), C.byref(h)))
+    return Handle(h)
+
+
+def ibp_build_device(rows_dev, n_rows: int, row_bytes: int, group_kind: int, group_param: int, align_bytes: int = 0,
+                     index_span: int = 1, flags: int = 0, threshold=(1, 1), device: int = 0, stream=None) -> Handle:
+    """rows_dev: address of n_rows x row_bytes bytes the device can read (HBM or mapped host memory)."""
+    p = ibp_build_params(C.sizeof(ibp_build_params), row_bytes, n_rows, group_kind, group_param,
+                         threshold[0], threshold[1], align_bytes, index_span, flags, 0)
+    h = _vp()
+    _check(lib().ibp_build_device(_ptr(rows_dev), C.byref(p), device, stream, C.byref(h)))
     return Handle(h)
 
 

@@ -1,0 +1,764 @@
+// ibp_build_device.cu -- the GPU-side compressor of libibp.so (sm_100a): ibp_build_device.
+//
+// The paper's compressor runs on the GPU over zero-copy tensors (PAPER.md:227-229 preprocessing "performed on the GPU", P:239
+// "tensors are partitioned among GPU warps", Fig. 3 = P:243-299 getCompressSize / compress) and writes the
+// compressed rows in place into CPU memory.  Here:
+//   ibp_mask_kernel     S0   per group: AND/OR reduction (strict, T = N) or bit-sliced per-bit counters (thresholded)
+//                            held in registers -- each lane owns W 32-bit words of the row, plane j of a word holds bit j of
+//                            its 32 running counters -- then Mask/Bitval by a bit-sliced comparison with T and N - T.
+//                            Groups with many rows are cut into slices (one warp each) whose accumulators are merged by
+//                            ibp_mask_merge_kernel; no atomics, results do not depend on the launch shape.
+//   ibp_pack_kernel     S0'  strict: a warp packs runs of rows of one group; per 32-bit word a 5-stage parallel-suffix bit
+//                            compress (Hacker's Delight 7-4) with move masks hoisted per group, OR-ed into a per-warp shared-
+//                            memory row image at the word's bit offset (exclusive scan of the kept-bit counts),
+//                            then written to the store (host memory, over PCIe) with wide stores.
+//   ibp_size_kernel     S0'  thresholded: participation of every 4-byte chunk, bitsSaved, size or raw (Fig. 3 lines 1-19)
+//   ibp_scan_*               exclusive scan of the row sizes -> row offsets (16-byte units)
+//   ibp_pack_t_kernel   S0'  thresholded: [participation bits][payloads] per row (Fig. 3 lines 21-33), raw rows copied
+// The result is bit-identical to ibp_build's (same Mask/Bitval/k, same packed bytes): both are checked against the oracle.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "ibp_devutil.cuh"
+
+namespace {
+
+__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE8;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
+// bit b of the result = 1 iff the bit-sliced counter b (planes pl[0..NP), LSB plane first) is >= T
+template <int NP>
+__device__ __forceinline__ uint32_t sliced_ge(const uint32_t* pl, uint64_t T) {
+    if (NP < 64 && (T >> NP)) return 0u;
+    uint32_t gt = 0, eq = 0xFFFFFFFFu;
+#pragma unroll
+    for (int j = NP - 1; j >= 0; --j) {
+        const uint32_t tj = ((T >> j) & 1ull) ? 0xFFFFFFFFu : 0u;
+        gt |= eq & pl[j] & ~tj;
+        eq &= ~(pl[j] ^ tj);
+    }
+    return gt | eq;
+}
+// ... is <= L
+template <int NP>
+__device__ __forceinline__ uint32_t sliced_le(const uint32_t* pl, uint64_t L) {
+    if (NP < 64 && (L >> NP)) return 0xFFFFFFFFu;
+    uint32_t lt = 0, eq = 0xFFFFFFFFu;
+#pragma unroll
+    for (int j = NP - 1; j >= 0; --j) {
+        const uint32_t tj = ((L >> j) & 1ull) ? 0xFFFFFFFFu : 0u;
+        lt |= eq & ~pl[j] & tj;
+        eq &= ~(pl[j] ^ tj);
+    }
+    return lt | eq;
+}
+
+struct BuildParams {
+    const uint32_t* rows;
+    uint64_t n_rows, n_groups;
+    uint32_t nw, n_pass;
+    uint32_t group_param, group_shift, strided;
+    uint32_t ns;                 // slices per group
+    uint64_t rows_per_slice;
+    uint32_t thr_num, thr_den;
+    uint32_t* meta;              // per group: Mask words, Bitval words
+    uint32_t* kbits;             // per group: popcount(~Mask)
+    uint32_t* scratch;           // ns > 1: per (group, slice) accumulators
+};
+
+__device__ __forceinline__ uint64_t group_count(const BuildParams& P, uint64_t g) {
+    if (P.strided) return (P.n_rows - g + P.group_param - 1) / P.group_param;
+    const uint64_t first = g * P.group_param;
+    return min((uint64_t)P.group_param, P.n_rows - first);
+}
+__device__ __forceinline__ uint64_t group_row(const BuildParams& P, uint64_t g, uint64_t j) {
+    return P.strided ? j * P.group_param + g : g * P.group_param + j;
+}
+__device__ __forceinline__ uint64_t threshold_of(uint64_t N, uint32_t num, uint32_t den) { return (N * num + den - 1) / den; }
+
+// ------------------------------------------------------------------------------------------------ S0: masks
+// One warp per (group, slice).  TM = thresholded (bit-sliced counters, NP planes: a slice has at most 2^NP - 1 rows).
+template <int W, bool TM, int NP>
+__global__ void __launch_bounds__(256) ibp_mask_kernel(const BuildParams P) {
+    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    const uint64_t n_units = P.n_groups * P.ns;
+    for (uint64_t u = (uint64_t)blockIdx.x * wpc + (threadIdx.x >> 5); u < n_units; u += (uint64_t)gridDim.x * wpc) {
+        const uint64_t g = u / P.ns;
+        const uint32_t s = (uint32_t)(u - g * P.ns);
+        const uint64_t N = group_count(P, g);
+        const uint64_t j0 = min(N, (uint64_t)s * P.rows_per_slice), j1 = min(N, j0 + P.rows_per_slice);
+        uint32_t k_total = 0;
+        for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+            const uint32_t w0 = (pass * 32u + lane) * W;
+            const bool active = w0 < P.nw;
+            uint32_t a[W], o[W], pl[TM ? NP : 1][W];
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                a[q] = 0xFFFFFFFFu; o[q] = 0;
+#pragma unroll
+                for (int j = 0; j < (TM ? NP : 1); ++j) pl[j][q] = 0;
+            }
+            if (active) {
+                const uint32_t* base = P.rows + w0;
+                uint64_t j = j0;
+                for (; j + 4 <= j1; j += 4) {
+                    uint32_t x0[W], x1[W], x2[W], x3[W];
+                    VecIO<W>::ld(base + group_row(P, g, j) * P.nw, x0);
+                    VecIO<W>::ld(base + group_row(P, g, j + 1) * P.nw, x1);
+                    VecIO<W>::ld(base + group_row(P, g, j + 2) * P.nw, x2);
+                    VecIO<W>::ld(base + group_row(P, g, j + 3) * P.nw, x3);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        if (!TM) {
+                            a[q] &= x0[q] & x1[q] & x2[q] & x3[q];
+                            o[q] |= x0[q] | x1[q] | x2[q] | x3[q];
+                        } else {
+                            // carry-save adders: four rows enter plane 0, two carries enter plane 1, one carry ripples on
+                            const uint32_t s1 = xor3(pl[0][q], x0[q], x1[q]), c1 = maj3(pl[0][q], x0[q], x1[q]);
+                            const uint32_t s2 = xor3(s1, x2[q], x3[q]), c2 = maj3(s1, x2[q], x3[q]);
+                            pl[0][q] = s2;
+                            uint32_t c = maj3(pl[1][q], c1, c2);
+                            pl[1][q] = xor3(pl[1][q], c1, c2);
+#pragma unroll
+                            for (int p = 2; p < NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
+                        }
+                    }
+                }
+                for (; j < j1; ++j) {
+                    uint32_t x[W];
+                    VecIO<W>::ld(base + group_row(P, g, j) * P.nw, x);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        if (!TM) { a[q] &= x[q]; o[q] |= x[q]; }
+                        else {
+                            uint32_t c = x[q];
+#pragma unroll
+                            for (int p = 0; p < NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
+                        }
+                    }
+                }
+            }
+            if (P.ns == 1) {
+                uint32_t mk[W], bv[W];
+                const uint64_t T = TM ? threshold_of(N, P.thr_num, P.thr_den) : 0;
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    if (!TM) {
+                        mk[q] = ~(a[q] ^ o[q]);
+                        bv[q] = a[q] & mk[q];
+                    } else {
+                        uint32_t col[NP];
+#pragma unroll
+                        for (int p = 0; p < NP; ++p) col[p] = pl[p][q];
+                        const uint32_t ge = sliced_ge<NP>(col, T), le = sliced_le<NP>(col, N - T);
+                        mk[q] = ge | le;
+                        bv[q] = ge;
+                    }
+                    if (active) k_total += __popc(~mk[q]);
+                }
+                if (active) {
+                    uint32_t* gm = P.meta + g * 2ull * P.nw;
+                    VecIO<W>::st_keep((uint8_t*)(gm + w0), mk);
+                    VecIO<W>::st_keep((uint8_t*)(gm + P.nw + w0), bv);
+                }
+            } else if (active) {
+                if (!TM) {
+                    VecIO<W>::st_keep((uint8_t*)(P.scratch + (u * 2ull) * P.nw + w0), a);
+                    VecIO<W>::st_keep((uint8_t*)(P.scratch + (u * 2ull + 1) * P.nw + w0), o);
+                } else {
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        uint32_t col[W];
+#pragma unroll
+                        for (int q = 0; q < W; ++q) col[q] = pl[p][q];
+                        VecIO<W>::st_keep((uint8_t*)(P.scratch + (u * (uint64_t)NP + p) * P.nw + w0), col);
+                    }
+                }
+            }
+        }
+        if (P.ns == 1) {
+#pragma unroll
+            for (int d = 16; d; d >>= 1) k_total += __shfl_xor_sync(0xFFFFFFFFu, k_total, d);
+            if (lane == 0) P.kbits[g] = k_total;
+        }
+    }
+}
+
+// Merge of the slices of a group: one thread per (group, word).  kbits must be zero on entry.
+template <bool TM, int NP>
+__global__ void ibp_mask_merge_kernel(const BuildParams P) {
+    const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+    if (i >= P.n_groups * P.nw) return;
+    const uint64_t g = i / P.nw;
+    const uint32_t w = (uint32_t)(i - g * P.nw);
+    const uint64_t N = group_count(P, g);
+    uint32_t mk, bv;
+    if (!TM) {
+        uint32_t a = 0xFFFFFFFFu, o = 0;
+        for (uint32_t s = 0; s < P.ns; ++s) {
+            const uint64_t u = g * P.ns + s;
+            a &= P.scratch[(u * 2ull) * P.nw + w];
+            o |= P.scratch[(u * 2ull + 1) * P.nw + w];
+        }
+        mk = ~(a ^ o);
+        bv = a & mk;
+    } else {
+        uint32_t acc[32];
+#pragma unroll
+        for (int p = 0; p < 32; ++p) acc[p] = 0;
+        for (uint32_t s = 0; s < P.ns; ++s) {
+            const uint64_t u = g * P.ns + s;
+            uint32_t c = 0;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const uint32_t q = P.scratch[(u * (uint64_t)NP + p) * P.nw + w];
+                const uint32_t t = acc[p];
+                acc[p] = xor3(t, q, c);
+                c = maj3(t, q, c);
+            }
+#pragma unroll
+            for (int p = NP; p < 32; ++p) { const uint32_t t = acc[p]; acc[p] = t ^ c; c &= t; }
+        }
+        const uint64_t T = threshold_of(N, P.thr_num, P.thr_den);
+        const uint32_t ge = sliced_ge<32>(acc, T), le = sliced_le<32>(acc, N - T);
+        mk = ge | le;
+        bv = ge;
+    }
+    P.meta[g * 2ull * P.nw + w] = mk;
+    P.meta[g * 2ull * P.nw + P.nw + w] = bv;
+    atomicAdd(&P.kbits[g], (uint32_t)__popc(~mk));
+}
+
+// ------------------------------------------------------------------------------------------------ S0': pack
+// the five move masks of the parallel-suffix compress/expand for the kept positions nv (Hacker's Delight 7-4)
+__device__ __forceinline__ void suffix_masks(uint32_t nv, uint32_t mv[5]) {
+    uint32_t m = nv, mk = ~nv << 1;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        uint32_t mp = mk ^ (mk << 1);
+        mp ^= mp << 2;
+        mp ^= mp << 4;
+        mp ^= mp << 8;
+        mp ^= mp << 16;
+        const uint32_t v = mp & m;
+        mv[i] = v;
+        m = (m ^ v) | (v >> (1 << i));
+        mk &= ~mp;
+    }
+}
+// the bits of x at the set positions of nv, moved to the low end in order ("the matching bits are removed")
+__device__ __forceinline__ uint32_t compress_bits(uint32_t x, uint32_t nv, const uint32_t mv[5]) {
+    x &= nv;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        const uint32_t t = x & mv[i];
+        x = (x ^ t) | (t >> (1 << i));
+    }
+    return x;
+}
+// OR the low k bits of c into the LSB-first bit image `img` (shared memory) at bit offset `bit` (P:292-295 insertBits)
+__device__ __forceinline__ void insert_bits(uint32_t* img, uint32_t bit, uint32_t c, uint32_t k) {
+    if (!k) return;
+    const uint32_t wq = bit >> 5, sh = bit & 31u;
+    atomicOr(img + wq, c << sh);
+    if (sh + k > 32u) atomicOr(img + wq + 1, c >> (32u - sh));
+}
+
+struct PackParams {
+    const uint32_t* rows;
+    const uint32_t* meta;
+    const IbpGroupEntry* gtab;
+    uint8_t* store;              // device-visible address of the packed store
+    uint64_t n_rows, n_units, row_stride_strided;
+    uint32_t nw, n_pass, group_param, group_shift, strided, align_bytes;
+    uint32_t slot_bytes;         // per-warp shared-memory row image
+    // thresholded
+    const uint32_t* row_off;     // 16-byte units
+    uint32_t* row_off_out;       // size kernel: units per row (scanned afterwards)
+    uint32_t* row_flag;
+    unsigned long long* sum_size;
+};
+
+// warp-cooperative copy of nbytes from the shared row image to the store; `align` = guaranteed alignment of dst and nbytes
+__device__ __forceinline__ void image_to_store(const uint8_t* img, uint8_t* dst, uint32_t nbytes, uint32_t align, int lane) {
+    if (align >= 16) {
+        for (uint32_t v = lane; v < nbytes / 16; v += 32) ((uint4*)dst)[v] = ((const uint4*)img)[v];
+    } else if (align >= 4) {
+        for (uint32_t v = lane; v < nbytes / 4; v += 32) ((uint32_t*)dst)[v] = ((const uint32_t*)img)[v];
+    } else {
+        for (uint32_t v = lane; v < nbytes; v += 32) dst[v] = img[v];
+    }
+}
+
+// Strict mode.  Unit = 16 consecutive rows (blocked) or 16 matrix rows of one column tile (strided): the metadata, the bit
+// offsets and the compress masks of the group stay in registers while consecutive rows share the group (single-pass rows).
+template <int W>
+__global__ void __launch_bounds__(256) ibp_pack_kernel(const PackParams P) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    uint32_t* img = (uint32_t*)(smem + (size_t)wib * P.slot_bytes);
+    const uint64_t S = P.group_param;
+    uint64_t prep_g = ~0ull;
+    uint32_t prep_pass = ~0u;
+    uint32_t m[W], ex[W], kq[W], mv[W][5], tot = 0;
+    IbpGroupEntry e{0, 0, 0};
+
+    auto prepare = [&](uint64_t g, uint32_t pass) {
+        const uint32_t w0 = (pass * 32u + lane) * W;
+        if (w0 < P.nw) VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
+        else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) m[q] = 0xFFFFFFFFu;
+        }
+        uint32_t t = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) { kq[q] = __popc(~m[q]); ex[q] = t; t += kq[q]; }
+        const uint32_t incl = warp_inclusive_scan(t, lane);
+#pragma unroll
+        for (int q = 0; q < W; ++q) {
+            ex[q] += incl - t;
+            if (q > 0 && m[q] == m[q - 1]) {
+#pragma unroll
+                for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+            } else {
+                suffix_masks(~m[q], mv[q]);
+            }
+        }
+        tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        if (g != prep_g) e = P.gtab[g];
+        prep_g = g; prep_pass = pass;
+    };
+
+    for (uint64_t u = (uint64_t)blockIdx.x * wpc + wib; u < P.n_units; u += (uint64_t)gridDim.x * wpc) {
+        uint64_t id0, id_step;
+        uint32_t nrows;
+        if (!P.strided) {
+            id0 = u * 16; id_step = 1;
+            nrows = (uint32_t)min((uint64_t)16, P.n_rows - id0);
+        } else {
+            const uint64_t rb = u / S, t = u - rb * S;
+            id0 = rb * 16 * S + t; id_step = S;
+            const uint64_t n_mrows_t = t < P.n_rows ? (P.n_rows - t + S - 1) / S : 0;   // rows of tile t
+            nrows = rb * 16 < n_mrows_t ? (uint32_t)min((uint64_t)16, n_mrows_t - rb * 16) : 0u;
+        }
+        for (uint32_t j = 0; j < nrows; ++j) {
+            const uint64_t id = id0 + j * id_step;
+            const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
+            // zero the row image (the previous row's copy-out is complete: __syncwarp below)
+            for (uint32_t v = lane; v < P.slot_bytes / 16; v += 32) ((uint4*)img)[v] = make_uint4(0, 0, 0, 0);
+            __syncwarp();
+            uint32_t carry = 0;
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                if (g != prep_g || pass != prep_pass) prepare(g, pass);
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                if (w0 < P.nw) {
+                    uint32_t x[W];
+                    VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) insert_bits(img, carry + ex[q], compress_bits(x[q], ~m[q], mv[q]), kq[q]);
+                }
+                carry += tot;
+            }
+            __syncwarp();
+            if (e.stride) {
+                const uint64_t off = P.strided ? (id / S) * P.row_stride_strided + e.base : e.base + (id - g * S) * (uint64_t)e.stride;
+                image_to_store((const uint8_t*)img, P.store + off, e.stride, P.align_bytes, lane);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// Thresholded mode, pass 1 (Fig. 3 lines 1-19 = P:244-271): unit = 32 consecutive rows (one word of the per-row bitmask).
+template <int W>
+__global__ void __launch_bounds__(256) ibp_size_kernel(const PackParams P) {
+    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    const uint64_t S = P.group_param;
+    unsigned long long local_sum = 0;
+    for (uint64_t u = (uint64_t)blockIdx.x * wpc + (threadIdx.x >> 5); u < P.n_units; u += (uint64_t)gridDim.x * wpc) {
+        const uint64_t id0 = u * 32;
+        const uint32_t nrows = (uint32_t)min((uint64_t)32, P.n_rows - id0);
+        uint32_t flags = 0;
+        for (uint32_t j = 0; j < nrows; ++j) {
+            const uint64_t id = id0 + j;
+            const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
+            uint32_t saved = 0;
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                if (w0 < P.nw) {
+                    uint32_t m[W], b[W], x[W];
+                    VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
+                    VecIO<W>::ld(P.meta + g * 2ull * P.nw + P.nw + w0, b);
+                    VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) saved += ((x[q] & m[q]) == b[q]) ? __popc(m[q]) : 0u;
+                }
+            }
+#pragma unroll
+            for (int d = 16; d; d >>= 1) saved += __shfl_xor_sync(0xFFFFFFFFu, saved, d);
+            const int64_t net = (int64_t)saved - (int64_t)P.nw;                                          // minus participation bits
+            const uint32_t bytes_saved = net >= 8 ? (uint32_t)(net / 8) : 0u;                            // floor
+            const uint32_t size = 4u * P.nw - bytes_saved;
+            if (bytes_saved) flags |= 1u << j;                                                           // else stored raw
+            if (lane == 0) {
+                P.row_off_out[id] = (size + P.align_bytes - 1) / P.align_bytes * (P.align_bytes / 16);
+                local_sum += size;
+            }
+        }
+        if (lane == 0) P.row_flag[u] = flags;
+    }
+    if (lane == 0 && local_sum) atomicAdd(P.sum_size, local_sum);
+}
+
+// Thresholded mode, pass 2 (Fig. 3 lines 21-33 = P:275-298): one row at a time per warp.
+template <int W>
+__global__ void __launch_bounds__(256) ibp_pack_t_kernel(const PackParams P) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    uint32_t* img = (uint32_t*)(smem + (size_t)wib * P.slot_bytes);
+    const uint64_t S = P.group_param;
+    for (uint64_t id = (uint64_t)blockIdx.x * wpc + wib; id < P.n_rows; id += (uint64_t)gridDim.x * wpc) {
+        const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
+        const uint32_t o0 = P.row_off[id], o1 = P.row_off[id + 1];
+        uint8_t* dst = P.store + 16ull * o0;
+        const bool compressed = (P.row_flag[id >> 5] >> (id & 31u)) & 1u;
+        if (!compressed) {                                               // kept raw
+            for (uint32_t w = lane; w < P.nw; w += 32) ((uint32_t*)dst)[w] = P.rows[id * P.nw + w];
+            for (uint32_t w = P.nw + lane; w < (o1 - o0) * 4u; w += 32) ((uint32_t*)dst)[w] = 0u;
+            continue;
+        }
+        for (uint32_t v = lane; v < P.slot_bytes / 16; v += 32) ((uint4*)img)[v] = make_uint4(0, 0, 0, 0);
+        __syncwarp();
+        uint32_t carry = P.nw;                                           // payloads follow the participation bits (R8)
+        for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+            const uint32_t w0 = (pass * 32u + lane) * W;
+            const bool active = w0 < P.nw;
+            uint32_t m[W], b[W], x[W], kq[W], part = 0, t = 0;
+            if (active) {
+                VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
+                VecIO<W>::ld(P.meta + g * 2ull * P.nw + P.nw + w0, b);
+                VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+            }
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                const bool p = active && (x[q] & m[q]) == b[q];
+                part |= (uint32_t)p << q;
+                kq[q] = active ? (p ? __popc(~m[q]) : 32u) : 0u;
+                t += kq[q];
+            }
+            const uint32_t incl = warp_inclusive_scan(t, lane);
+            uint32_t bit = carry + incl - t;
+            if (active) {
+                if (part) atomicOr(img + (w0 >> 5), part << (w0 & 31u));                     // W divides 32: one word
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    uint32_t c = x[q];
+                    if ((part >> q) & 1u) { uint32_t mv[5]; suffix_masks(~m[q], mv); c = compress_bits(x[q], ~m[q], mv); }
+                    if (kq[q] == 32u) {                                                       // two plain halves (no shift by 32)
+                        const uint32_t wq = bit >> 5, sh = bit & 31u;
+                        atomicOr(img + wq, c << sh);
+                        if (sh) atomicOr(img + wq + 1, c >> (32u - sh));
+                    } else {
+                        insert_bits(img, bit, c, kq[q]);
+                    }
+                    bit += kq[q];
+                }
+            }
+            carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
+        }
+        __syncwarp();
+        image_to_store((const uint8_t*)img, dst, (o1 - o0) * 16u, 16, lane);
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ exclusive scan (u32 -> u32)
+// 4096 items per block of 1024 threads; totals in 64 bits so that an overflow of the 32-bit offsets is detected.
+__global__ void __launch_bounds__(1024) ibp_scan_sums(const uint32_t* __restrict__ in, uint64_t n, unsigned long long* __restrict__ bsum) {
+    __shared__ unsigned long long ws[32];
+    const uint64_t i0 = (uint64_t)blockIdx.x * 4096 + threadIdx.x * 4ull;
+    unsigned long long s = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) if (i0 + k < n) s += in[i0 + k];
+#pragma unroll
+    for (int d = 16; d; d >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, d);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        s = ws[threadIdx.x];
+#pragma unroll
+        for (int d = 16; d; d >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, d);
+        if (threadIdx.x == 0) bsum[blockIdx.x] = s;
+    }
+}
+// exclusive scan of bsum[0..nblk) in place by one block; bsum[nblk] = total
+__global__ void __launch_bounds__(1024) ibp_scan_bsums(unsigned long long* bsum, uint64_t nblk) {
+    __shared__ unsigned long long ws[32];
+    __shared__ unsigned long long run_s;
+    if (threadIdx.x == 0) run_s = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (uint64_t base = 0; base < nblk; base += 1024) {
+        const uint64_t i = base + threadIdx.x;
+        const unsigned long long v = i < nblk ? bsum[i] : 0ull;
+        unsigned long long incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, incl, d); if (lane >= d) incl += t; }
+        if (lane == 31) ws[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned long long w = ws[lane], wi = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, wi, d); if (lane >= d) wi += t; }
+            ws[lane] = wi - w;
+        }
+        __syncthreads();
+        const unsigned long long run = run_s;
+        if (i < nblk) bsum[i] = run + ws[wid] + incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) run_s = run + ws[31] + incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) bsum[nblk] = run_s;
+}
+// in place: data[i] = exclusive prefix; data[n] = total (low 32 bits)
+__global__ void __launch_bounds__(1024) ibp_scan_apply(uint32_t* data, uint64_t n, const unsigned long long* __restrict__ bsum) {
+    __shared__ uint32_t ws[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const uint64_t i0 = (uint64_t)blockIdx.x * 4096 + threadIdx.x * 4ull;
+    uint32_t v[4], s = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { v[k] = i0 + k < n ? data[i0 + k] : 0u; s += v[k]; }
+    const uint32_t incl = warp_inclusive_scan(s, lane);
+    if (lane == 31) ws[wid] = incl;
+    __syncthreads();
+    if (wid == 0) { const uint32_t w = ws[lane]; ws[lane] = warp_inclusive_scan(w, lane) - w; }
+    __syncthreads();
+    uint32_t e = (uint32_t)bsum[blockIdx.x] + ws[wid] + incl - s;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { if (i0 + k < n) data[i0 + k] = e; e += v[k]; }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) data[n] = (uint32_t)bsum[gridDim.x];
+}
+
+int pick_W(uint32_t row_bytes) {
+    if (row_bytes % 16 == 0 && row_bytes >= 512) return 4;
+    if (row_bytes % 8 == 0 && row_bytes >= 256) return 2;
+    return 1;
+}
+
+template <int W>
+ibp_status launch_masks(const BuildParams& P, bool tm, int np, int grid, cudaStream_t st) {
+    if (!tm) ibp_mask_kernel<W, false, 1><<<grid, 256, 0, st>>>(P);
+    else if (np == 9) ibp_mask_kernel<W, true, 9><<<grid, 256, 0, st>>>(P);
+    else ibp_mask_kernel<W, true, 16><<<grid, 256, 0, st>>>(P);
+    IBP_CUDA(cudaGetLastError());
+    if (P.ns > 1) {
+        const uint64_t cells = P.n_groups * P.nw;
+        const unsigned blocks = (unsigned)((cells + 127) / 128);
+        if (!tm) ibp_mask_merge_kernel<false, 1><<<blocks, 128, 0, st>>>(P);
+        else if (np == 9) ibp_mask_merge_kernel<true, 9><<<blocks, 128, 0, st>>>(P);
+        else ibp_mask_merge_kernel<true, 16><<<blocks, 128, 0, st>>>(P);
+        IBP_CUDA(cudaGetLastError());
+    }
+    return IBP_OK;
+}
+
+struct DevBuf {                       // frees device scratch on every exit path
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+};
+
+}  // namespace
+
+extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_params* params, int device, void* cuda_stream,
+                                       ibp_handle** out_handle) {
+    if (!rows_dev || !params || !out_handle) { ibp_set_error("ibp_build_device: null argument"); return IBP_ERR_INVALID_ARG; }
+    if ((uintptr_t)rows_dev & 15u) { ibp_set_error("ibp_build_device: rows_dev must be 16-byte aligned"); return IBP_ERR_INVALID_ARG; }
+    if (params->struct_size == sizeof(ibp_build_params) && (params->flags & IBP_FLAG_PAGEABLE_STORE)) {
+        ibp_set_error("ibp_build_device: the GPU writes the packed store in place; a pageable store is not GPU-visible");
+        return IBP_ERR_INVALID_ARG;
+    }
+    int ndev = 0;
+    IBP_CUDA(cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) { ibp_set_error("ibp_build_device: no CUDA device %d", device); return IBP_ERR_CUDA; }
+    cudaDeviceProp prop;
+    IBP_CUDA(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) { ibp_set_error("ibp_build_device: device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor); return IBP_ERR_UNSUPPORTED; }
+    IBP_CUDA(cudaSetDevice(device));
+    ibp_handle* h = nullptr;
+    ibp_status rc = ibp_prepare_handle(params, "ibp_build_device", &h);
+    if (rc != IBP_OK) return rc;
+    struct Guard { ibp_handle* h; ~Guard() { if (h) ibp_destroy(h); } } guard{h};
+
+    const ibp_build_params& p = h->p;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint32_t nw = h->n_words;
+    const uint64_t ng = h->n_groups, n = p.n_rows;
+    const int W = pick_W(p.row_bytes);
+    const int sms = prop.multiProcessorCount;
+    const uint64_t Nmax = p.group_kind == IBP_GROUP_BLOCKED ? std::min<uint64_t>(p.group_param, n) : (n + p.group_param - 1) / p.group_param;
+    if (Nmax > 0xFFFFFFFFull) { ibp_set_error("ibp_build_device: groups of more than 2^32-1 rows are not supported"); return IBP_ERR_UNSUPPORTED; }
+
+    BuildParams B;
+    memset(&B, 0, sizeof B);
+    B.rows = (const uint32_t*)rows_dev;
+    B.n_rows = n; B.n_groups = ng; B.nw = nw;
+    B.n_pass = (nw + 32 * W - 1) / (32 * W);
+    B.group_param = p.group_param;
+    B.group_shift = 0xFFFFFFFFu;
+    if ((p.group_param & (p.group_param - 1)) == 0) { uint32_t s = 0; while ((1u << s) < p.group_param) ++s; B.group_shift = s; }
+    B.strided = p.group_kind == IBP_GROUP_STRIDED;
+    B.thr_num = p.threshold_num; B.thr_den = p.threshold_den;
+    // slices: enough warps to fill the GPU when there are few groups; a slice never exceeds 65535 rows (16 counter planes)
+    const uint64_t target_units = (uint64_t)sms * 32;
+    uint64_t ns = 1;
+    if (ng < target_units) ns = std::min<uint64_t>((target_units + ng - 1) / ng, (Nmax + 63) / 64);
+    ns = std::max<uint64_t>(ns, (Nmax + 65534) / 65535);
+    ns = std::max<uint64_t>(ns, 1);
+    B.rows_per_slice = (Nmax + ns - 1) / ns;
+    B.ns = (uint32_t)((Nmax + B.rows_per_slice - 1) / B.rows_per_slice);
+    const int np = B.rows_per_slice <= 511 ? 9 : 16;
+
+    IBP_CUDA(cudaMalloc((void**)&h->meta_dev, ng * 2ull * nw * 4));
+    DevBuf kbits, scratch;
+    IBP_CUDA(cudaMalloc(&kbits.p, ng * 4));
+    B.meta = h->meta_dev;
+    B.kbits = (uint32_t*)kbits.p;
+    if (B.ns > 1) {
+        const uint64_t per_unit = (uint64_t)(h->thresholded ? np : 2) * nw * 4;
+        if (cudaMalloc(&scratch.p, ng * B.ns * per_unit) != cudaSuccess) {
+            (void)cudaGetLastError();
+            ibp_set_error("ibp_build_device: out of device memory (slice accumulators, %llu bytes)", (unsigned long long)(ng * B.ns * per_unit));
+            return IBP_ERR_OUT_OF_MEMORY;
+        }
+        B.scratch = (uint32_t*)scratch.p;
+        IBP_CUDA(cudaMemsetAsync(kbits.p, 0, ng * 4, st));
+    }
+    const int grid_masks = (int)std::min<uint64_t>((ng * B.ns + 7) / 8, (uint64_t)sms * 8);
+    switch (W) {
+        case 4: rc = launch_masks<4>(B, h->thresholded, np, grid_masks, st); break;
+        case 2: rc = launch_masks<2>(B, h->thresholded, np, grid_masks, st); break;
+        default: rc = launch_masks<1>(B, h->thresholded, np, grid_masks, st); break;
+    }
+    if (rc != IBP_OK) return rc;
+
+    // host copies of the metadata (accessors, layout)
+    std::vector<uint32_t> kb;
+    try { kb.resize(ng); } catch (...) { ibp_set_error("ibp_build_device: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    IBP_CUDA(cudaMemcpyAsync(kb.data(), kbits.p, ng * 4, cudaMemcpyDeviceToHost, st));
+    IBP_CUDA(cudaMemcpyAsync(h->meta.data(), h->meta_dev, ng * 2ull * nw * 4, cudaMemcpyDeviceToHost, st));
+    IBP_CUDA(cudaStreamSynchronize(st));
+    for (uint64_t g = 0; g < ng; ++g) h->gtab[g].k_bits = kb[g];
+    const int nthreads = p.n_threads ? (int)p.n_threads : 0;
+
+    PackParams K;
+    memset(&K, 0, sizeof K);
+    K.rows = B.rows; K.meta = h->meta_dev;
+    K.n_rows = n; K.nw = nw; K.n_pass = B.n_pass;
+    K.group_param = p.group_param; K.group_shift = B.group_shift; K.strided = B.strided;
+    K.align_bytes = p.align_bytes;
+    const int wpc = 8;
+
+    if (!h->thresholded) {
+        ibp_layout_strict(h);
+        rc = ibp_alloc_store(h, nthreads);
+        if (rc != IBP_OK) return rc;
+        rc = ibp_attach_device(h, device, cuda_stream);
+        if (rc != IBP_OK) return rc;
+        if (!h->store_dev) { ibp_set_error("ibp_build_device: the packed store is not GPU-visible"); return IBP_ERR_BAD_STATE; }
+        K.gtab = h->gtab_dev;
+        K.store = h->store_dev;
+        K.row_stride_strided = h->row_stride_strided;
+        K.slot_bytes = (h->max_stride + 15u) / 16u * 16u + 16u;
+        K.n_units = B.strided ? ((((n + p.group_param - 1) / p.group_param) + 15) / 16) * (uint64_t)p.group_param : (n + 15) / 16;
+        const size_t smem = (size_t)wpc * K.slot_bytes;
+        if (smem > 200 * 1024) { ibp_set_error("ibp_build_device: packed rows of %u bytes do not fit the shared-memory row images", h->max_stride); return IBP_ERR_UNSUPPORTED; }
+        const int grid = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 8);
+#define IBP_PACK(W_)                                                                                                         \
+    do {                                                                                                                     \
+        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(ibp_pack_kernel<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        ibp_pack_kernel<W_><<<grid, wpc * 32, smem, st>>>(K);                                                                \
+    } while (0)
+        if (h->max_stride) {
+            switch (W) { case 4: IBP_PACK(4); break; case 2: IBP_PACK(2); break; default: IBP_PACK(1); break; }
+        }
+#undef IBP_PACK
+        IBP_CUDA(cudaGetLastError());
+        IBP_CUDA(cudaStreamSynchronize(st));
+    } else {
+        // pass 1: sizes and flags; scan -> row offsets
+        const uint64_t n_flag_words = (n + 31) / 32;
+        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, (n + 1) * 4));
+        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, n_flag_words * 4));
+        const uint64_t nblk = (n + 4095) / 4096;
+        DevBuf aux;
+        IBP_CUDA(cudaMalloc(&aux.p, (nblk + 2) * 8));
+        unsigned long long* bsum = (unsigned long long*)aux.p;
+        unsigned long long* sum_size = bsum + nblk + 1;
+        IBP_CUDA(cudaMemsetAsync(sum_size, 0, 8, st));
+        K.row_off_out = h->row_off_dev;
+        K.row_flag = h->row_flag_dev;
+        K.sum_size = sum_size;
+        K.n_units = n_flag_words;
+        const int grid1 = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 8);
+        switch (W) {
+            case 4: ibp_size_kernel<4><<<grid1, wpc * 32, 0, st>>>(K); break;
+            case 2: ibp_size_kernel<2><<<grid1, wpc * 32, 0, st>>>(K); break;
+            default: ibp_size_kernel<1><<<grid1, wpc * 32, 0, st>>>(K); break;
+        }
+        IBP_CUDA(cudaGetLastError());
+        ibp_scan_sums<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+        ibp_scan_bsums<<<1, 1024, 0, st>>>(bsum, nblk);
+        ibp_scan_apply<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+        IBP_CUDA(cudaGetLastError());
+        unsigned long long totals[2] = {0, 0};   // [0] = store size in 16-byte units, [1] = sum of the byte-aligned row sizes
+        IBP_CUDA(cudaMemcpyAsync(totals, bsum + nblk, 16, cudaMemcpyDeviceToHost, st));
+        try { h->row_off.resize(n + 1); h->row_flag.resize(n_flag_words); }
+        catch (...) { ibp_set_error("ibp_build_device: out of memory (row offsets)"); return IBP_ERR_OUT_OF_MEMORY; }
+        IBP_CUDA(cudaMemcpyAsync(h->row_flag.data(), h->row_flag_dev, n_flag_words * 4, cudaMemcpyDeviceToHost, st));
+        IBP_CUDA(cudaStreamSynchronize(st));
+        if (totals[0] > 0xFFFFFFFFull) { ibp_set_error("ibp_build_device: thresholded store exceeds 64 GiB (4-byte row offsets in 16-byte units)"); return IBP_ERR_UNSUPPORTED; }
+        IBP_CUDA(cudaMemcpyAsync(h->row_off.data(), h->row_off_dev, (n + 1) * 4, cudaMemcpyDeviceToHost, st));
+        uint64_t n_comp = 0;
+        for (uint64_t i = 0; i < n_flag_words; ++i) n_comp += (uint64_t)__builtin_popcount(h->row_flag[i]);
+        h->n_rows_raw = n - n_comp;
+        h->packed_bytes_bytealigned = totals[1];
+        h->packed_bytes_rows = totals[0] * 16;
+        h->store_used = totals[0] * 16;
+        h->store_bytes = (h->store_used + 64 + 4095) / 4096 * 4096;
+        h->max_stride = (p.row_bytes + p.align_bytes - 1) / p.align_bytes * p.align_bytes;
+        rc = ibp_alloc_store(h, nthreads);
+        if (rc != IBP_OK) return rc;
+        rc = ibp_attach_device(h, device, cuda_stream);
+        if (rc != IBP_OK) return rc;
+        if (!h->store_dev) { ibp_set_error("ibp_build_device: the packed store is not GPU-visible"); return IBP_ERR_BAD_STATE; }
+        K.store = h->store_dev;
+        K.row_off = h->row_off_dev;
+        K.slot_bytes = (h->max_stride + 15u) / 16u * 16u + 16u;
+        const size_t smem = (size_t)wpc * K.slot_bytes;
+        if (smem > 200 * 1024) { ibp_set_error("ibp_build_device: rows of %u bytes do not fit the shared-memory row images", p.row_bytes); return IBP_ERR_UNSUPPORTED; }
+        const int grid2 = (int)std::min<uint64_t>((n + wpc - 1) / wpc, (uint64_t)sms * 8);
+#define IBP_PACK_T(W_)                                                                                                         \
+    do {                                                                                                                       \
+        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(ibp_pack_t_kernel<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        ibp_pack_t_kernel<W_><<<grid2, wpc * 32, smem, st>>>(K);                                                               \
+    } while (0)
+        switch (W) { case 4: IBP_PACK_T(4); break; case 2: IBP_PACK_T(2); break; default: IBP_PACK_T(1); break; }
+#undef IBP_PACK_T
+        IBP_CUDA(cudaGetLastError());
+        IBP_CUDA(cudaStreamSynchronize(st));
+    }
+    guard.h = nullptr;
+    *out_handle = h;
+    return IBP_OK;
+}

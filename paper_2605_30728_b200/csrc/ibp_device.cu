@@ -24,15 +24,7 @@
 
 #include "ibp_internal.h"
 
-#define IBP_CUDA(call)                                                                              \
-    do {                                                                                            \
-        cudaError_t e_ = (call);                                                                    \
-        if (e_ != cudaSuccess) {                                                                    \
-            ibp_set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
-            (void)cudaGetLastError();                                                               \
-            return IBP_ERR_CUDA;                                                                    \
-        }                                                                                           \
-    } while (0)
+#include "ibp_devutil.cuh"
 
 enum { MODE_ROWS = 0, MODE_SPANS = 1, MODE_STRIDED = 2 };
 
@@ -68,15 +60,6 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        uint32_t t = __shfl_up_sync(0xFFFFFFFFu, v, d);
-        if (lane >= d) v += t;
-    }
-    return v;
-}
-
 // Deposit the low popc(nv) bits of x at the set positions of nv, lowest first, one run of contiguous positions per
 // iteration (float data has 1-3 runs per 32-bit word).  S5 "re-insert the removed bits" (P:211, P:319 step 5).
 __device__ __forceinline__ uint32_t deposit_runs(uint32_t x, uint32_t nv) {
@@ -91,23 +74,6 @@ __device__ __forceinline__ uint32_t deposit_runs(uint32_t x, uint32_t nv) {
     }
     return r;
 }
-
-template <int W> struct VecIO;
-template <> struct VecIO<1> {
-    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { v[0] = __ldg(p); }
-    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.b32 [%0], %1;" ::"l"(p), "r"(v[0]) : "memory"); }
-    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint32_t*)p = v[0]; }
-};
-template <> struct VecIO<2> {
-    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint2 t = __ldg((const uint2*)p); v[0] = t.x; v[1] = t.y; }
-    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v2.b32 [%0], {%1,%2};" ::"l"(p), "r"(v[0]), "r"(v[1]) : "memory"); }
-    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint2*)p = make_uint2(v[0], v[1]); }
-};
-template <> struct VecIO<4> {
-    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint4 t = __ldg((const uint4*)p); v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w; }
-    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory"); }
-    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint4*)p = make_uint4(v[0], v[1], v[2], v[3]); }
-};
 
 __device__ __forceinline__ uint64_t group_of(const DecodeParams& P, uint64_t id, bool strided) {
     if (strided) return id % P.group_param;
@@ -142,10 +108,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
-__device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t group_shift, uint64_t id) {
-    return group_shift != 0xFFFFFFFFu ? (id >> group_shift) : (id / group_param);
 }
 
 #include "ibp_stream.cuh"
@@ -790,9 +752,7 @@ static ibp_status check_ready(const ibp_handle* h, const char* who) {
 }
 
 // ------------------------------------------------------------------------------------------------ C ABI
-extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream) {
-    if (!h) { ibp_set_error("ibp_upload_metadata: null handle"); return IBP_ERR_INVALID_ARG; }
-    if (h->device >= 0 && h->device != device) { ibp_set_error("ibp_upload_metadata: handle already lives on device %d", h->device); return IBP_ERR_INVALID_ARG; }
+ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream) {
     int ndev = 0;
     IBP_CUDA(cudaGetDeviceCount(&ndev));
     if (device < 0 || device >= ndev) { ibp_set_error("ibp_upload_metadata: no CUDA device %d", device); return IBP_ERR_CUDA; }
@@ -802,18 +762,24 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
     IBP_CUDA(cudaSetDevice(device));
     if (h->device == device) return IBP_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    IBP_CUDA(cudaMalloc((void**)&h->meta_dev, h->meta.size() * 4));
-    IBP_CUDA(cudaMalloc((void**)&h->gtab_dev, h->gtab.size() * sizeof(IbpGroupEntry)));
-    IBP_CUDA(cudaMemcpyAsync(h->meta_dev, h->meta.data(), h->meta.size() * 4, cudaMemcpyHostToDevice, st));
-    IBP_CUDA(cudaMemcpyAsync(h->gtab_dev, h->gtab.data(), h->gtab.size() * sizeof(IbpGroupEntry), cudaMemcpyHostToDevice, st));
-    if (h->thresholded) {
+    if (!h->meta_dev) {
+        IBP_CUDA(cudaMalloc((void**)&h->meta_dev, h->meta.size() * 4));
+        IBP_CUDA(cudaMemcpyAsync(h->meta_dev, h->meta.data(), h->meta.size() * 4, cudaMemcpyHostToDevice, st));
+    }
+    if (!h->gtab_dev) {
+        IBP_CUDA(cudaMalloc((void**)&h->gtab_dev, h->gtab.size() * sizeof(IbpGroupEntry)));
+        IBP_CUDA(cudaMemcpyAsync(h->gtab_dev, h->gtab.data(), h->gtab.size() * sizeof(IbpGroupEntry), cudaMemcpyHostToDevice, st));
+    }
+    if (h->thresholded && !h->row_off_dev) {
         IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, h->row_off.size() * 4));
-        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, h->row_flag.size() * 4));
         IBP_CUDA(cudaMemcpyAsync(h->row_off_dev, h->row_off.data(), h->row_off.size() * 4, cudaMemcpyHostToDevice, st));
+    }
+    if (h->thresholded && !h->row_flag_dev) {
+        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, h->row_flag.size() * 4));
         IBP_CUDA(cudaMemcpyAsync(h->row_flag_dev, h->row_flag.data(), h->row_flag.size() * 4, cudaMemcpyHostToDevice, st));
     }
     // expand move masks per (group, word) when the table has few groups (strided column tiles, small tables): 20 B per word
-    if (!h->thresholded && h->n_groups * (uint64_t)h->n_words * 20ull <= (8ull << 20)) {
+    if (!h->thresholded && !h->mvtab_dev && h->n_groups * (uint64_t)h->n_words * 20ull <= (8ull << 20)) {
         const uint64_t cells = h->n_groups * (uint64_t)h->n_words;
         IBP_CUDA(cudaMalloc((void**)&h->mvtab_dev, cells * 20));
         ibp_build_mvtab<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(h->meta_dev, h->n_words, h->n_groups, h->mvtab_dev);
@@ -839,6 +805,12 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
     (void)cudaGetLastError();
     h->device = device;
     return IBP_OK;
+}
+
+extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream) {
+    if (!h) { ibp_set_error("ibp_upload_metadata: null handle"); return IBP_ERR_INVALID_ARG; }
+    if (h->device >= 0 && h->device != device) { ibp_set_error("ibp_upload_metadata: handle already lives on device %d", h->device); return IBP_ERR_INVALID_ARG; }
+    return ibp_attach_device(h, device, cuda_stream);
 }
 
 extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream) {

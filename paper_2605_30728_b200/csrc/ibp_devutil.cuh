@@ -1,0 +1,48 @@
+// ibp_devutil.cuh -- small device/host helpers shared by the CUDA translation units of libibp.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "ibp_internal.h"
+
+#define IBP_CUDA(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            ibp_set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            (void)cudaGetLastError();                                                               \
+            return IBP_ERR_CUDA;                                                                    \
+        }                                                                                           \
+    } while (0)
+
+__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xFFFFFFFFu, v, d);
+        if (lane >= d) v += t;
+    }
+    return v;
+}
+
+template <int W> struct VecIO;
+template <> struct VecIO<1> {
+    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { v[0] = __ldg(p); }
+    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.b32 [%0], %1;" ::"l"(p), "r"(v[0]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint32_t*)p = v[0]; }
+};
+template <> struct VecIO<2> {
+    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint2 t = __ldg((const uint2*)p); v[0] = t.x; v[1] = t.y; }
+    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v2.b32 [%0], {%1,%2};" ::"l"(p), "r"(v[0]), "r"(v[1]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint2*)p = make_uint2(v[0], v[1]); }
+};
+template <> struct VecIO<4> {
+    static __device__ __forceinline__ void ld(const uint32_t* p, uint32_t* v) { uint4 t = __ldg((const uint4*)p); v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w; }
+    static __device__ __forceinline__ void st(uint8_t* p, const uint32_t* v) { asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory"); }
+    static __device__ __forceinline__ void st_keep(uint8_t* p, const uint32_t* v) { *(uint4*)p = make_uint4(v[0], v[1], v[2], v[3]); }
+};
+
+__device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t group_shift, uint64_t id) {
+    return group_shift != 0xFFFFFFFFu ? (id >> group_shift) : (id / group_param);
+}
+

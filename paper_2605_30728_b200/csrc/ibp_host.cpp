@@ -86,7 +86,8 @@ static inline uint64_t round_up(uint64_t v, uint64_t a) { return (v + a - 1) / a
 
 // ------------------------------------------------------------------------------------------------ packed store
 // Allocates h->store (h->store_bytes bytes, already set) and zero-fills it.
-static ibp_status alloc_store(ibp_handle* h, int nthreads) {
+ibp_status ibp_alloc_store(ibp_handle* h, int nthreads) {
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
     // ---- packed store in host memory that the GPU can read in place (P:239 zero-copy).  Two kinds:
     //   managed-host: cudaMallocManaged + preferred location CPU; ibp_upload_metadata adds the direct GPU mapping
     //                 (accessed-by).  The pages stay in host memory, SM loads cross PCIe, and the GPU maps them
@@ -149,37 +150,87 @@ static ibp_status alloc_store(ibp_handle* h, int nthreads) {
 static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nthreads);
 
 // ------------------------------------------------------------------------------------------------ build
-extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle) {
-    if (!rows_host || !params || !out_handle) { ibp_set_error("ibp_build: null argument"); return IBP_ERR_INVALID_ARG; }
-    if (params->struct_size != sizeof(ibp_build_params)) { ibp_set_error("ibp_build: struct_size %u != %zu", params->struct_size, sizeof(ibp_build_params)); return IBP_ERR_INVALID_ARG; }
+// Validates the build parameters (shared by ibp_build and ibp_build_device), fills in the defaults and allocates the handle with
+// its host-side metadata arrays.
+ibp_status ibp_prepare_handle(const ibp_build_params* params, const char* who, ibp_handle** out) {
+    if (params->struct_size != sizeof(ibp_build_params)) { ibp_set_error("%s: struct_size %u != %zu", who, params->struct_size, sizeof(ibp_build_params)); return IBP_ERR_INVALID_ARG; }
     ibp_build_params p = *params;
-    if (p.row_bytes == 0 || p.row_bytes % 4 || p.row_bytes > 65536) { ibp_set_error("ibp_build: row_bytes %u must be a multiple of 4 in 4..65536", p.row_bytes); return IBP_ERR_INVALID_ARG; }
-    if (p.n_rows == 0 || p.group_param == 0 || p.group_kind > 1) { ibp_set_error("ibp_build: n_rows, group_param must be >= 1 and group_kind 0|1"); return IBP_ERR_INVALID_ARG; }
+    if (p.row_bytes == 0 || p.row_bytes % 4 || p.row_bytes > 65536) { ibp_set_error("%s: row_bytes %u must be a multiple of 4 in 4..65536", who, p.row_bytes); return IBP_ERR_INVALID_ARG; }
+    if (p.n_rows == 0 || p.group_param == 0 || p.group_kind > 1) { ibp_set_error("%s: n_rows, group_param must be >= 1 and group_kind 0|1", who); return IBP_ERR_INVALID_ARG; }
     if (p.threshold_num == 0 && p.threshold_den == 0) p.threshold_num = p.threshold_den = 1;
-    if (p.threshold_den == 0 || p.threshold_num > p.threshold_den) { ibp_set_error("ibp_build: bad threshold"); return IBP_ERR_INVALID_ARG; }
+    if (p.threshold_den == 0 || p.threshold_num > p.threshold_den) { ibp_set_error("%s: bad threshold", who); return IBP_ERR_INVALID_ARG; }
     const bool thresholded = p.threshold_num != p.threshold_den;
-    if (thresholded && 2ull * p.threshold_num <= p.threshold_den) { ibp_set_error("ibp_build: threshold must exceed 1/2 (a bit cannot be invariant-1 and invariant-0 at once)"); return IBP_ERR_INVALID_ARG; }
+    if (thresholded && 2ull * p.threshold_num <= p.threshold_den) { ibp_set_error("%s: threshold must exceed 1/2 (a bit cannot be invariant-1 and invariant-0 at once)", who); return IBP_ERR_INVALID_ARG; }
     if (p.align_bytes == 0) p.align_bytes = 32;
-    if (p.align_bytes > 128 || (p.align_bytes & (p.align_bytes - 1))) { ibp_set_error("ibp_build: align_bytes %u must be a power of two <= 128", p.align_bytes); return IBP_ERR_INVALID_ARG; }
-    if (thresholded && p.align_bytes < 16) { ibp_set_error("ibp_build: thresholded mode needs align_bytes >= 16 (row offsets are kept in 16-byte units)"); return IBP_ERR_INVALID_ARG; }
+    if (p.align_bytes > 128 || (p.align_bytes & (p.align_bytes - 1))) { ibp_set_error("%s: align_bytes %u must be a power of two <= 128", who, p.align_bytes); return IBP_ERR_INVALID_ARG; }
+    if (thresholded && p.align_bytes < 16) { ibp_set_error("%s: thresholded mode needs align_bytes >= 16 (row offsets are kept in 16-byte units)", who); return IBP_ERR_INVALID_ARG; }
     if (p.index_span == 0) p.index_span = 1;
-    if (p.n_rows % p.index_span) { ibp_set_error("ibp_build: n_rows must be a multiple of index_span"); return IBP_ERR_INVALID_ARG; }
-    if (p.index_span > 1 && p.group_kind != IBP_GROUP_BLOCKED) { ibp_set_error("ibp_build: index_span > 1 needs blocked groups"); return IBP_ERR_INVALID_ARG; }
+    if (p.n_rows % p.index_span) { ibp_set_error("%s: n_rows must be a multiple of index_span", who); return IBP_ERR_INVALID_ARG; }
+    if (p.index_span > 1 && p.group_kind != IBP_GROUP_BLOCKED) { ibp_set_error("%s: index_span > 1 needs blocked groups", who); return IBP_ERR_INVALID_ARG; }
 
     ibp_handle* h = new (std::nothrow) ibp_handle();
-    if (!h) { ibp_set_error("ibp_build: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    if (!h) { ibp_set_error("%s: out of memory", who); return IBP_ERR_OUT_OF_MEMORY; }
     h->p = p;
     h->n_words = p.row_bytes / 4;
     h->n_groups = p.group_kind == IBP_GROUP_BLOCKED ? (p.n_rows + p.group_param - 1) / p.group_param
                                                      : std::min<uint64_t>(p.group_param, p.n_rows);
+    h->thresholded = thresholded;
+    try {
+        h->meta.assign(h->n_groups * 2 * h->n_words, 0);
+        h->gtab.assign(h->n_groups, IbpGroupEntry{0, 0, 0});
+    } catch (...) { delete h; ibp_set_error("%s: out of memory (metadata)", who); return IBP_ERR_OUT_OF_MEMORY; }
+    *out = h;
+    return IBP_OK;
+}
+
+// Strict mode: from gtab[].k_bits to the store layout (strides, bases, totals); include/ibp.h "Store layout".
+void ibp_layout_strict(ibp_handle* h) {
+    const ibp_build_params& p = h->p;
+    const uint64_t ng = h->n_groups, G = p.group_param;
+    const uint64_t A = p.align_bytes, base_align = std::max<uint64_t>(A, 16);
+    uint64_t cursor = 0;
+    h->max_stride = 0;
+    h->packed_bytes_rows = h->packed_bytes_bytealigned = 0;
+    for (uint64_t g = 0; g < ng; ++g) {
+        IbpGroupEntry& e = h->gtab[g];
+        const uint64_t nbytes = (e.k_bits + 7) / 8;
+        e.stride = (uint32_t)round_up(nbytes, A);
+        h->max_stride = std::max(h->max_stride, e.stride);
+        uint64_t count;
+        if (p.group_kind == IBP_GROUP_BLOCKED) {
+            count = std::min<uint64_t>(G, p.n_rows - g * G);
+            cursor = round_up(cursor, base_align);
+            e.base = cursor;
+            cursor += count * e.stride;
+        } else {
+            count = (p.n_rows - g + G - 1) / G;
+            e.base = cursor;                 // prefix inside one packed matrix row
+            cursor += e.stride;
+        }
+        h->packed_bytes_rows += count * e.stride;
+        h->packed_bytes_bytealigned += count * nbytes;
+    }
+    if (p.group_kind == IBP_GROUP_STRIDED) {
+        h->row_stride_strided = round_up(cursor, base_align);
+        cursor = h->row_stride_strided * ((p.n_rows + G - 1) / G);
+    }
+    h->store_used = cursor;
+    h->store_bytes = round_up(cursor + 64, 4096);   // slack: 16-byte vector reads may run past the last row
+}
+
+extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_handle** out_handle) {
+    if (!rows_host || !params || !out_handle) { ibp_set_error("ibp_build: null argument"); return IBP_ERR_INVALID_ARG; }
+    ibp_handle* h = nullptr;
+    {
+        const ibp_status st = ibp_prepare_handle(params, "ibp_build", &h);
+        if (st != IBP_OK) return st;
+    }
+    const ibp_build_params& p = h->p;
+    const bool thresholded = h->thresholded;
     const uint32_t nw = h->n_words;
     const uint64_t ng = h->n_groups, G = p.group_param;
     const uint32_t* rows = (const uint32_t*)rows_host;
     const int nthreads = p.n_threads ? (int)p.n_threads : omp_get_max_threads();
-    try {
-        h->meta.assign(ng * 2 * nw, 0);
-        h->gtab.assign(ng, IbpGroupEntry{0, 0, 0});
-    } catch (...) { delete h; ibp_set_error("ibp_build: out of memory (metadata)"); return IBP_ERR_OUT_OF_MEMORY; }
 
     if (thresholded) {
         ibp_status st = IBP_OK;
@@ -244,38 +295,10 @@ extern "C" ibp_status ibp_build(const void* rows_host, const ibp_build_params* p
     }
 
     // ---- layout
-    const uint64_t A = p.align_bytes, base_align = std::max<uint64_t>(A, 16);
-    uint64_t cursor = 0;
-    h->max_stride = 0;
-    h->packed_bytes_rows = h->packed_bytes_bytealigned = 0;
-    for (uint64_t g = 0; g < ng; ++g) {
-        IbpGroupEntry& e = h->gtab[g];
-        const uint64_t nbytes = (e.k_bits + 7) / 8;
-        e.stride = (uint32_t)round_up(nbytes, A);
-        h->max_stride = std::max(h->max_stride, e.stride);
-        uint64_t count;
-        if (p.group_kind == IBP_GROUP_BLOCKED) {
-            count = std::min<uint64_t>(G, p.n_rows - g * G);
-            cursor = round_up(cursor, base_align);
-            e.base = cursor;
-            cursor += count * e.stride;
-        } else {
-            count = (p.n_rows - g + G - 1) / G;
-            e.base = cursor;                 // prefix inside one packed matrix row
-            cursor += e.stride;
-        }
-        h->packed_bytes_rows += count * e.stride;
-        h->packed_bytes_bytealigned += count * nbytes;
-    }
-    if (p.group_kind == IBP_GROUP_STRIDED) {
-        h->row_stride_strided = round_up(cursor, base_align);
-        cursor = h->row_stride_strided * ((p.n_rows + G - 1) / G);
-    }
-    h->store_used = cursor;
-    h->store_bytes = round_up(cursor + 64, 4096);   // slack: 16-byte vector reads may run past the last row
+    ibp_layout_strict(h);
 
     {
-        const ibp_status st = alloc_store(h, nthreads);
+        const ibp_status st = ibp_alloc_store(h, nthreads);
         if (st != IBP_OK) { delete h; return st; }
     }
     if (p.group_kind == IBP_GROUP_BLOCKED) {
@@ -391,7 +414,6 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
     const ibp_build_params& p = h->p;
     const uint32_t nw = h->n_words;
     const uint64_t ng = h->n_groups, G = p.group_param, n = p.n_rows;
-    h->thresholded = true;
     auto thr = [&](uint64_t N) { return (N * p.threshold_num + p.threshold_den - 1) / p.threshold_den; };
 
     // ---- S0: counters -> Mask/Bitval
@@ -480,7 +502,7 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
     h->max_stride = (uint32_t)round_up(p.row_bytes, A);
     for (uint64_t g = 0; g < ng; ++g) { h->gtab[g].base = 0; h->gtab[g].stride = 0; }    // unused in this mode
 
-    ibp_status st = alloc_store(h, nthreads);
+    ibp_status st = ibp_alloc_store(h, nthreads);
     if (st != IBP_OK) return st;
 
     // ---- S0' pass 2: the bit streams

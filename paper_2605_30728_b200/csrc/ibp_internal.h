@@ -59,6 +59,13 @@ struct ibp_handle {
 // error plumbing (thread local)
 void ibp_set_error(const char* fmt, ...);
 
+// shared by the host compressor (ibp_host.cpp) and the GPU compressor (ibp_build_device.cu)
+ibp_status ibp_prepare_handle(const ibp_build_params* params, const char* who, ibp_handle** out);   // validate + allocate
+void ibp_layout_strict(ibp_handle* h);                          // gtab[].k_bits -> strides, bases, totals
+ibp_status ibp_alloc_store(ibp_handle* h, int nthreads);         // host store of h->store_bytes bytes, zero-filled
+// ibp_device.cu: everything ibp_upload_metadata does; arrays that already exist on the device are kept as they are
+ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream);
+
 // byte offset of packed row `id` inside the store
 static inline uint64_t ibp_row_offset(const ibp_handle* h, uint64_t id) {
     if (h->thresholded) return 16ull * h->row_off[id];

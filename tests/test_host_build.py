@@ -11,10 +11,14 @@ from paper_2605_30728_b200 import binding as ibp
 from paper_2605_30728_b200 import datagen, workloads
 
 
-def _check_against_oracle(X, kind, param, align, span=1, rows_to_check=None):
+def _check_against_oracle(X, kind, param, align, span=1, rows_to_check=None, build=None):
+    """build: optional callable (Xb, rb, kind, param, align, span) -> Handle, for the GPU-side compressor's parity tests."""
     Xb = np.ascontiguousarray(X).view(np.uint8).reshape(X.shape[0], -1)
     n, rb = Xb.shape
-    h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, index_span=span, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    if build is None:
+        h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, index_span=span, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    else:
+        h = build(Xb, rb, kind, param, align, span)
     ds = oracle.Dataset(Xb, kind, param)
     info = h.info()
     assert info.n_groups == ds.n_groups
@@ -146,10 +150,13 @@ def test_batch_link_bytes():
 # ---------------------------------------------------------------------------------------------------------------------
 # thresholded mode (tau < 1; the paper's default codec): the library's compressor against oracle.DatasetT
 # ---------------------------------------------------------------------------------------------------------------------
-def _check_T_against_oracle(X, kind, param, thr, align=32, rows_to_check=None):
+def _check_T_against_oracle(X, kind, param, thr, align=32, rows_to_check=None, build=None):
     Xb = np.ascontiguousarray(X).view(np.uint8).reshape(X.shape[0], -1)
     n, rb = Xb.shape
-    h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, flags=ibp.IBP_FLAG_PAGEABLE_STORE, threshold=thr)
+    if build is None:
+        h = ibp.ibp_build(Xb, rb, kind, param, align_bytes=align, flags=ibp.IBP_FLAG_PAGEABLE_STORE, threshold=thr)
+    else:
+        h = build(Xb, rb, kind, param, align, thr)
     ds = oracle.DatasetT(Xb, kind, param, thr[0], thr[1])
     info = h.info()
     assert info.thresholded == 1 and (info.threshold_num, info.threshold_den) == thr
