@@ -558,6 +558,117 @@ def run_weights(args):
             m[0].destroy()
 
 
+# ------------------------------------------------------------------------------------------------- GPU-side compressor
+def run_build(args):
+    """ibp_build_device on the workload's table, rows resident in HBM, the
+    packed store written in place into host memory over PCIe.  One step = one whole build (mask kernel, [size kernel, scan,]
+    pack kernel).  Kernel times are CUDA events recorded inside the library around each kernel (ibp_get_build_stats)."""
+    import torch
+    from paper_2605_30728_b200 import binding as ibp
+    import oracle
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --phase build runs on one GPU")
+    torch.cuda.set_device(0)
+    w = make_workload(args.workload)
+    thr = parse_threshold(args.threshold)
+    align = args.align if args.align else w.align_bytes
+    X = w.table()
+    Xb = X.view(np.uint8).reshape(w.n_rows, -1)
+    xd = torch.from_numpy(Xb).cuda()
+    stream = torch.cuda.current_stream().cuda_stream
+    flags = ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0
+    W, K = min(max(1, args.warmup), 2), max(1, min(args.steps, 5))
+    d2h_ceiling = ibp.ibp_measure_d2h(0, 1 << 30, 8)
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_peak = 6650.0
+
+    def build():
+        return ibp.ibp_build_device(xd.data_ptr(), w.n_rows, w.row_bytes, w.group_kind, w.group_param, align_bytes=align,
+                                    index_span=w.index_span, flags=flags, threshold=thr, stream=stream)
+
+    # parity of a sample against the oracle (groups are independent: the oracle compresses the sampled groups alone)
+    h = build()
+    G = w.group_param
+    rng = np.random.default_rng(0)
+    for g in rng.choice(w.n_rows // G, 6, replace=False):
+        blk = Xb[g * G:(g + 1) * G]
+        m, b, k = h.metadata_host(int(g))
+        if thr[0] == thr[1]:
+            ds = oracle.Dataset(blk, 0, G)
+            ok = np.array_equal(m, ds.mask(0)) and np.array_equal(b, ds.bitval(0)) and k == ds.k_bits(0)
+            for r in range(0, G, 7):
+                data, _ = h.packed_row(int(g) * G + r)
+                want = ds.packed_row(r)
+                ok = ok and np.array_equal(data[:want.size], want) and not data[want.size:].any()
+        else:
+            ds = oracle.DatasetT(blk, 0, G, thr[0], thr[1])
+            ok = np.array_equal(m, ds.mask(0)) and np.array_equal(b, ds.bitval(0))
+            for r in range(0, G, 7):
+                data, stored, comp = h.row_info(int(g) * G + r)
+                want, want_comp = ds.row(r)
+                ok = ok and comp == want_comp and np.array_equal(data, want)
+        ds.close()
+        if not ok:
+            raise SystemExit("bench.py: the GPU-built store differs from the oracle; refusing to report a number")
+    info = h.info()
+    h.destroy()
+    for _ in range(W - 1):
+        build().destroy()
+    clocks = ClockSampler(0)
+    clocks.start()
+    stats = []
+    for _ in range(K):
+        h = build()
+        stats.append(h.build_stats())
+        h.destroy()
+    clk = clocks.stop()
+    mean = lambda f: float(np.mean([getattr(s_, f) for s_ in stats]))
+    raw = stats[0].raw_bytes
+    k_ms = mean("mask_ms") + mean("size_ms") + mean("scan_ms") + mean("pack_ms")
+    # host compressor (ibp_build, all cores) and the oracle's compressor (1 core, sample of groups) for comparison
+    t0 = time.perf_counter()
+    hh = ibp.ibp_build(Xb, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span, flags=flags, threshold=thr)
+    t_host = time.perf_counter() - t0
+    hh.destroy()
+    cpu = None
+    if not args.no_cpu:
+        ng_s = 1
+        t0 = time.perf_counter()
+        done = 0
+        while time.perf_counter() - t0 < 10.0:
+            blk = Xb[done * G:(done + ng_s) * G]
+            (oracle.Dataset(blk, 0, G) if thr[0] == thr[1] else oracle.DatasetT(blk, 0, G, thr[0], thr[1])).close()
+            done += ng_s
+            ng_s = min(ng_s * 2, 64)
+        dt = time.perf_counter() - t0
+        cpu = {"value": round(done * G * w.row_bytes / dt * 1e-9, 5), "unit": "GB/s", "cores": 1, "kind": "oracle",
+               "sample": f"oracle compressor (masks + pack) on the first {done} groups ({done * G} rows) of the {w.name} table, {dt:.1f} s"}
+    line = {
+        "metric": "compression throughput, raw GB/s (ibp_build_device kernels)", "value": round(raw / (k_ms * 1e-3) * 1e-9, 3), "unit": "GB/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": round(k_ms, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": describe(w) + " -- whole table compressed, rows resident in HBM, packed store written to host memory", "align_bytes": info.align_bytes,
+                   "codec": "group-strict (tau = 1)" if not info.thresholded else f"thresholded, tau = {thr[0]}/{thr[1]}",
+                   "store": {1: "pinned (cudaHostAlloc)", 2: "managed host-resident"}[info.store_kind], "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3),
+                   "slices_per_group": stats[0].slices_per_group},
+        "kernels_ms": {"mask": round(mean("mask_ms"), 4), "size": round(mean("size_ms"), 4), "scan": round(mean("scan_ms"), 4), "pack": round(mean("pack_ms"), 4)},
+        "roofline": {"bound": "pcie", "kernel": "ibp_pack_t_kernel" if info.thresholded else ("ibp_pack_bulk_kernel" if (w.group_kind == 0 and info.align_bytes >= 16) else "ibp_pack_kernel"), "achieved": round(stats[0].store_bytes / (mean("pack_ms") * 1e-3) * 1e-9, 3),
+                     "peak": round(d2h_ceiling, 3), "unit": "GB/s", "frac": round(stats[0].store_bytes / (mean("pack_ms") * 1e-3) * 1e-9 / d2h_ceiling, 4), "traffic": None,
+                     "peak_source": "cudaMemcpyAsync D2H of 1 GiB into pinned memory, best of 8, this run (ibp_measure_d2h)",
+                     "algorithmic_bytes_per_launch": int(stats[0].store_bytes)},
+        "roofline_mask_kernel": {"bound": "hbm", "kernel": "ibp_mask_kernel", "achieved": round(raw / (mean("mask_ms") * 1e-3) * 1e-9, 1), "peak": hbm_peak, "unit": "GB/s",
+                                 "frac": round(raw / (mean("mask_ms") * 1e-3) * 1e-9 / hbm_peak, 4), "algorithmic_bytes_per_launch": int(raw)},
+        "e2e": {"value": round(raw / (mean("total_ms") * 1e-3) * 1e-9, 3), "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": int(stats[0].store_bytes),
+                "note": "whole ibp_build_device call: kernels + host-side store allocation and zero fill + metadata copies to the host"},
+        "host_build": {"value": round(raw / t_host * 1e-9, 3), "unit": "GB/s", "what": f"ibp_build (host compressor, all {os.cpu_count()} cores), {t_host:.2f} s"},
+        "gpu_launches": K * (2 if not info.thresholded else 6), "clocks": clk, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -573,6 +684,7 @@ def main():
     ap.add_argument("--threshold", default="1/1", help="tau = T/N as a fraction: 1/1 = group-strict (BASELINE.json), 4/5 = the paper's thresholded codec")
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
+    ap.add_argument("--phase", default="gather", choices=["gather", "build"], help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device")
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
@@ -581,6 +693,8 @@ def main():
         if args.workload == "weights":
             args.workload = "kv"      # the oracle arm samples row decodes; bf16 256-byte rows either way
         run_reference(args)
+    elif args.phase == "build":
+        run_build(args)
     elif args.workload == "weights":
         run_weights(args)
     else:

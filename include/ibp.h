@@ -137,6 +137,20 @@ ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_
 ibp_status ibp_build_device(const void* rows_dev, const ibp_build_params* params, int device, void* cuda_stream,
                             ibp_handle** out_handle);
 
+/* Where the time of an ibp_build_device call went (CUDA events on the stream around each kernel; total = wall clock of the
+ * call including the host-side store allocation and copies).  BAD_STATE for a handle built by ibp_build.              */
+typedef struct {
+    double mask_ms;      /* ibp_mask_kernel (+ slice merge): reads every row once                                    */
+    double size_ms;      /* thresholded: ibp_size_kernel (reads every row once); 0 in strict mode                    */
+    double scan_ms;      /* thresholded: row-offset scan; 0 in strict mode                                            */
+    double pack_ms;      /* ibp_pack_kernel / ibp_pack_t_kernel: reads every row once, writes the packed store       */
+    double total_ms;
+    uint64_t raw_bytes;  /* n_rows * row_bytes                                                                        */
+    uint64_t store_bytes;/* packed bytes written to the store (rows incl. alignment padding)                          */
+    uint32_t slices_per_group, reserved;
+} ibp_build_stats;
+ibp_status ibp_get_build_stats(const ibp_handle* h, ibp_build_stats* out);
+
 /* -- S0'': copy Mask/Bitval and the group table to HBM on `device` ("stored in GPU memory").  Idempotent for the
  * same device; INVALID_ARG for a second device.  Synchronises the stream before returning.                         */
 ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream);
@@ -247,6 +261,9 @@ ibp_status ibp_host_free_managed(void* ptr);
  * ibp_measure_zero_copy_read: best of `reps` SM-issued contiguous 16-byte zero-copy reads of nbytes, in GB/s.       */
 ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, double* gbps);
 ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps);
+/* ibp_measure_d2h: best of `reps` cudaMemcpyAsync D2H copies of nbytes into pinned memory (the ceiling of the GPU-side
+ * compressor's store writes), in GB/s.                                                                              */
+ibp_status ibp_measure_d2h(int device, size_t nbytes, int reps, double* gbps);
 
 #ifdef __cplusplus
 }

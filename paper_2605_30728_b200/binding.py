@@ -46,11 +46,18 @@ class ibp_info(C.Structure):
                 ("rowflag_bytes", C.c_uint64), ("rowoffset_bytes", C.c_uint64)]
 
 
+class ibp_build_stats(C.Structure):
+    _fields_ = [("mask_ms", C.c_double), ("size_ms", C.c_double), ("scan_ms", C.c_double), ("pack_ms", C.c_double),
+                ("total_ms", C.c_double), ("raw_bytes", C.c_uint64), ("store_bytes", C.c_uint64),
+                ("slices_per_group", C.c_uint32), ("reserved", C.c_uint32)]
+
+
 # name -> (restype, argtypes); every symbol include/ibp.h declares (tests/test_abi.py checks the two lists agree)
 _vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int
 SIGNATURES = {
     "ibp_build": (_int, [_vp, C.POINTER(ibp_build_params), C.POINTER(_vp)]),
     "ibp_build_device": (_int, [_vp, C.POINTER(ibp_build_params), _int, _vp, C.POINTER(_vp)]),
+    "ibp_get_build_stats": (_int, [_vp, C.POINTER(ibp_build_stats)]),
     "ibp_upload_metadata": (_int, [_vp, _int, _vp]),
     "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
@@ -80,6 +87,7 @@ SIGNATURES = {
     "ibp_host_free_managed": (_int, [_vp]),
     "ibp_measure_h2d": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
     "ibp_measure_zero_copy_read": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
+    "ibp_measure_d2h": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
 }
 
 _lib = None
@@ -167,6 +175,11 @@ class Handle:
         out = ibp_info()
         _check(lib().ibp_get_info(self._h, C.byref(out)))
         return out
+
+    def build_stats(self):
+        st = ibp_build_stats()
+        _check(lib().ibp_get_build_stats(self._h, C.byref(st)))
+        return st
 
     def configure(self, max_ctas=0, warps_per_cta=0):
         _check(lib().ibp_configure(self._h, max_ctas, warps_per_cta))
@@ -283,6 +296,12 @@ def ibp_measure_h2d(device=0, nbytes=1 << 30, reps=10) -> float:
 def ibp_measure_zero_copy_read(device=0, nbytes=1 << 30, reps=5) -> float:
     g = C.c_double()
     _check(lib().ibp_measure_zero_copy_read(device, nbytes, reps, C.byref(g)))
+    return g.value
+
+
+def ibp_measure_d2h(device=0, nbytes=1 << 30, reps=10) -> float:
+    g = C.c_double()
+    _check(lib().ibp_measure_d2h(device, nbytes, reps, C.byref(g)))
     return g.value
 
 

@@ -17,7 +17,9 @@
 //   ibp_pack_t_kernel   S0'  thresholded: [participation bits][payloads] per row (Fig. 3 lines 21-33), raw rows copied
 // The result is bit-identical to ibp_build's (same Mask/Bitval/k, same packed bytes): both are checked against the oracle.
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -282,6 +284,7 @@ struct PackParams {
     uint64_t n_rows, n_units, row_stride_strided;
     uint32_t nw, n_pass, group_param, group_shift, strided, align_bytes;
     uint32_t slot_bytes;         // per-warp shared-memory row image
+    uint32_t rows_per_unit;      // bulk variant: consecutive rows packed into one image and stored with one bulk copy
     // thresholded
     const uint32_t* row_off;     // 16-byte units
     uint32_t* row_off_out;       // size kernel: units per row (scanned afterwards)
@@ -379,6 +382,96 @@ __global__ void __launch_bounds__(256) ibp_pack_kernel(const PackParams P) {
     }
 }
 
+// Strict mode, blocked groups, A >= 16: the packed rows of consecutive rows of one group are contiguous in the store, so a warp
+// packs a whole unit (rows_per_unit rows) into one shared-memory image and hands it to the bulk-copy engine as ONE
+// cp.async.bulk shared -> global store per run of rows of a group (PCIe sees long contiguous writes instead of one short
+// write per lane); two images per warp, so the store of unit i overlaps the packing of unit i+1.
+template <int W>
+__global__ void __launch_bounds__(256) ibp_pack_bulk_kernel(const PackParams P) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    uint8_t* img2 = smem + (size_t)wib * 2 * P.slot_bytes;
+    const uint64_t S = P.group_param;
+    uint64_t prep_g = ~0ull;
+    uint32_t prep_pass = ~0u;
+    uint32_t m[W], ex[W], kq[W], mv[W][5], tot = 0;
+    IbpGroupEntry e{0, 0, 0};
+
+    auto prepare = [&](uint64_t g, uint32_t pass) {
+        const uint32_t w0 = (pass * 32u + lane) * W;
+        if (w0 < P.nw) VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
+        else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) m[q] = 0xFFFFFFFFu;
+        }
+        uint32_t t = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) { kq[q] = __popc(~m[q]); ex[q] = t; t += kq[q]; }
+        const uint32_t incl = warp_inclusive_scan(t, lane);
+#pragma unroll
+        for (int q = 0; q < W; ++q) {
+            ex[q] += incl - t;
+            if (q > 0 && m[q] == m[q - 1]) {
+#pragma unroll
+                for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+            } else {
+                suffix_masks(~m[q], mv[q]);
+            }
+        }
+        tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        if (g != prep_g) e = P.gtab[g];
+        prep_g = g; prep_pass = pass;
+    };
+    // shared -> global bulk store of [src, src+bytes) (generic-proxy writes made visible to the async proxy first)
+    auto flush = [&](const uint8_t* src, uint64_t dst_off, uint32_t bytes) {
+        if (!bytes) return;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0)
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                         ::"l"(P.store + dst_off), "r"((uint32_t)__cvta_generic_to_shared(src)), "r"(bytes) : "memory");
+    };
+
+    uint32_t it = 0;
+    for (uint64_t u = (uint64_t)blockIdx.x * wpc + wib; u < P.n_units; u += (uint64_t)gridDim.x * wpc, ++it) {
+        const uint64_t id0 = u * P.rows_per_unit;
+        const uint32_t nrows = (uint32_t)min((uint64_t)P.rows_per_unit, P.n_rows - id0);
+        uint8_t* img = img2 + (size_t)(it & 1u) * P.slot_bytes;
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store that last used this image has read it
+        __syncwarp();
+        for (uint32_t v = lane; v < P.slot_bytes / 16; v += 32) ((uint4*)img)[v] = make_uint4(0, 0, 0, 0);
+        __syncwarp();
+        uint32_t pos = 0, run_start = 0;
+        uint64_t run_dst = 0, run_g = ~0ull;
+        for (uint32_t j = 0; j < nrows; ++j) {
+            const uint64_t id = id0 + j;
+            const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
+            uint32_t carry = 0;
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                if (g != prep_g || pass != prep_pass) prepare(g, pass);
+                if (pass == 0 && g != run_g) {                       // a new run of rows of one group starts here
+                    flush(img + run_start, run_dst, pos - run_start);
+                    run_start = pos; run_g = g;
+                    run_dst = e.base + (id - g * S) * (uint64_t)e.stride;
+                }
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                if (w0 < P.nw) {
+                    uint32_t x[W];
+                    VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) insert_bits((uint32_t*)(img + pos), carry + ex[q], compress_bits(x[q], ~m[q], mv[q]), kq[q]);
+                }
+                carry += tot;
+            }
+            pos += e.stride;
+        }
+        flush(img + run_start, run_dst, pos - run_start);
+        if (lane == 0) asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    __syncwarp();
+}
+
 // Thresholded mode, pass 1 (Fig. 3 lines 1-19 = P:244-271): unit = 32 consecutive rows (one word of the per-row bitmask).
 template <int W>
 __global__ void __launch_bounds__(256) ibp_size_kernel(const PackParams P) {
@@ -420,66 +513,84 @@ __global__ void __launch_bounds__(256) ibp_size_kernel(const PackParams P) {
     if (lane == 0 && local_sum) atomicAdd(P.sum_size, local_sum);
 }
 
-// Thresholded mode, pass 2 (Fig. 3 lines 21-33 = P:275-298): one row at a time per warp.
+// Thresholded mode, pass 2 (Fig. 3 lines 21-33 = P:275-298).  Rows lie in id order in the store, so a warp packs a unit of
+// rows_per_unit consecutive rows into one shared-memory image (row r at 16*(row_off[r] - row_off[first])) and stores the
+// whole unit with one cp.async.bulk shared -> global copy; two images per warp overlap the store with the next unit.
 template <int W>
 __global__ void __launch_bounds__(256) ibp_pack_t_kernel(const PackParams P) {
-    extern __shared__ __align__(16) uint8_t smem[];
+    extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
-    uint32_t* img = (uint32_t*)(smem + (size_t)wib * P.slot_bytes);
+    uint8_t* img2 = smem + (size_t)wib * 2 * P.slot_bytes;
     const uint64_t S = P.group_param;
-    for (uint64_t id = (uint64_t)blockIdx.x * wpc + wib; id < P.n_rows; id += (uint64_t)gridDim.x * wpc) {
-        const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
-        const uint32_t o0 = P.row_off[id], o1 = P.row_off[id + 1];
-        uint8_t* dst = P.store + 16ull * o0;
-        const bool compressed = (P.row_flag[id >> 5] >> (id & 31u)) & 1u;
-        if (!compressed) {                                               // kept raw
-            for (uint32_t w = lane; w < P.nw; w += 32) ((uint32_t*)dst)[w] = P.rows[id * P.nw + w];
-            for (uint32_t w = P.nw + lane; w < (o1 - o0) * 4u; w += 32) ((uint32_t*)dst)[w] = 0u;
-            continue;
-        }
-        for (uint32_t v = lane; v < P.slot_bytes / 16; v += 32) ((uint4*)img)[v] = make_uint4(0, 0, 0, 0);
+    uint32_t it = 0;
+    for (uint64_t u = (uint64_t)blockIdx.x * wpc + wib; u < P.n_units; u += (uint64_t)gridDim.x * wpc, ++it) {
+        const uint64_t id0 = u * P.rows_per_unit;
+        const uint32_t nrows = (uint32_t)min((uint64_t)P.rows_per_unit, P.n_rows - id0);
+        uint8_t* ubuf = img2 + (size_t)(it & 1u) * P.slot_bytes;
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
         __syncwarp();
-        uint32_t carry = P.nw;                                           // payloads follow the participation bits (R8)
-        for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
-            const uint32_t w0 = (pass * 32u + lane) * W;
-            const bool active = w0 < P.nw;
-            uint32_t m[W], b[W], x[W], kq[W], part = 0, t = 0;
-            if (active) {
-                VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
-                VecIO<W>::ld(P.meta + g * 2ull * P.nw + P.nw + w0, b);
-                VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+        const uint32_t off0 = P.row_off[id0], off_end = P.row_off[id0 + nrows];
+        const uint32_t unit_bytes = (off_end - off0) * 16u;
+        for (uint32_t v = lane; v < unit_bytes / 16 + 1; v += 32) ((uint4*)ubuf)[v] = make_uint4(0, 0, 0, 0);
+        __syncwarp();
+        for (uint32_t j = 0; j < nrows; ++j) {
+            const uint64_t id = id0 + j;
+            const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
+            uint32_t* img = (uint32_t*)(ubuf + 16ull * (P.row_off[id] - off0));
+            const bool compressed = (P.row_flag[id >> 5] >> (id & 31u)) & 1u;
+            if (!compressed) {                                           // kept raw
+                for (uint32_t w = lane; w < P.nw; w += 32) img[w] = P.rows[id * P.nw + w];
+                continue;
             }
-#pragma unroll
-            for (int q = 0; q < W; ++q) {
-                const bool p = active && (x[q] & m[q]) == b[q];
-                part |= (uint32_t)p << q;
-                kq[q] = active ? (p ? __popc(~m[q]) : 32u) : 0u;
-                t += kq[q];
-            }
-            const uint32_t incl = warp_inclusive_scan(t, lane);
-            uint32_t bit = carry + incl - t;
-            if (active) {
-                if (part) atomicOr(img + (w0 >> 5), part << (w0 & 31u));                     // W divides 32: one word
+            uint32_t carry = P.nw;                                       // payloads follow the participation bits (R8)
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                const bool active = w0 < P.nw;
+                uint32_t m[W], b[W], x[W], kq[W], part = 0, t = 0;
+                if (active) {
+                    VecIO<W>::ld(P.meta + g * 2ull * P.nw + w0, m);
+                    VecIO<W>::ld(P.meta + g * 2ull * P.nw + P.nw + w0, b);
+                    VecIO<W>::ld(P.rows + id * P.nw + w0, x);
+                }
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    uint32_t c = x[q];
-                    if ((part >> q) & 1u) { uint32_t mv[5]; suffix_masks(~m[q], mv); c = compress_bits(x[q], ~m[q], mv); }
-                    if (kq[q] == 32u) {                                                       // two plain halves (no shift by 32)
-                        const uint32_t wq = bit >> 5, sh = bit & 31u;
-                        atomicOr(img + wq, c << sh);
-                        if (sh) atomicOr(img + wq + 1, c >> (32u - sh));
-                    } else {
-                        insert_bits(img, bit, c, kq[q]);
-                    }
-                    bit += kq[q];
+                    const bool p = active && (x[q] & m[q]) == b[q];
+                    part |= (uint32_t)p << q;
+                    kq[q] = active ? (p ? __popc(~m[q]) : 32u) : 0u;
+                    t += kq[q];
                 }
+                const uint32_t incl = warp_inclusive_scan(t, lane);
+                uint32_t bit = carry + incl - t;
+                if (active) {
+                    if (part) atomicOr(img + (w0 >> 5), part << (w0 & 31u));                 // W divides 32: one word
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        uint32_t c = x[q];
+                        if ((part >> q) & 1u) { uint32_t mv[5]; suffix_masks(~m[q], mv); c = compress_bits(x[q], ~m[q], mv); }
+                        if (kq[q] == 32u) {                                                   // two plain halves (no shift by 32)
+                            const uint32_t wq = bit >> 5, sh = bit & 31u;
+                            atomicOr(img + wq, c << sh);
+                            if (sh) atomicOr(img + wq + 1, c >> (32u - sh));
+                        } else {
+                            insert_bits(img, bit, c, kq[q]);
+                        }
+                        bit += kq[q];
+                    }
+                }
+                carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
             }
-            carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
         }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
-        image_to_store((const uint8_t*)img, dst, (o1 - o0) * 16u, 16, lane);
-        __syncwarp();
+        if (lane == 0) {
+            if (unit_bytes)
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                             ::"l"(P.store + 16ull * off0), "r"((uint32_t)__cvta_generic_to_shared(ubuf)), "r"(unit_bytes) : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
     }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    __syncwarp();
 }
 
 // ------------------------------------------------------------------------------------------------ exclusive scan (u32 -> u32)
@@ -573,6 +684,16 @@ ibp_status launch_masks(const BuildParams& P, bool tm, int np, int grid, cudaStr
     return IBP_OK;
 }
 
+struct Timer {                        // CUDA events on the stream around a phase of the build
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaStream_t st;
+    explicit Timer(cudaStream_t s) : st(s) { cudaEventCreate(&a); cudaEventCreate(&b); }
+    ~Timer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    void start() { cudaEventRecord(a, st); }
+    void stop() { cudaEventRecord(b, st); }
+    double ms() { float t = 0; if (cudaEventSynchronize(b) != cudaSuccess || cudaEventElapsedTime(&t, a, b) != cudaSuccess) { (void)cudaGetLastError(); return 0; } return t; }
+};
+
 struct DevBuf {                       // frees device scratch on every exit path
     void* p = nullptr;
     ~DevBuf() { if (p) cudaFree(p); }
@@ -595,6 +716,7 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
     IBP_CUDA(cudaGetDeviceProperties(&prop, device));
     if (prop.major != 10) { ibp_set_error("ibp_build_device: device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor); return IBP_ERR_UNSUPPORTED; }
     IBP_CUDA(cudaSetDevice(device));
+    const auto t_begin = std::chrono::steady_clock::now();
     ibp_handle* h = nullptr;
     ibp_status rc = ibp_prepare_handle(params, "ibp_build_device", &h);
     if (rc != IBP_OK) return rc;
@@ -645,11 +767,14 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         IBP_CUDA(cudaMemsetAsync(kbits.p, 0, ng * 4, st));
     }
     const int grid_masks = (int)std::min<uint64_t>((ng * B.ns + 7) / 8, (uint64_t)sms * 8);
+    Timer t_mask(st), t_size(st), t_scan(st), t_pack(st);
+    t_mask.start();
     switch (W) {
         case 4: rc = launch_masks<4>(B, h->thresholded, np, grid_masks, st); break;
         case 2: rc = launch_masks<2>(B, h->thresholded, np, grid_masks, st); break;
         default: rc = launch_masks<1>(B, h->thresholded, np, grid_masks, st); break;
     }
+    t_mask.stop();
     if (rc != IBP_OK) return rc;
 
     // host copies of the metadata (accessors, layout)
@@ -667,7 +792,7 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
     K.n_rows = n; K.nw = nw; K.n_pass = B.n_pass;
     K.group_param = p.group_param; K.group_shift = B.group_shift; K.strided = B.strided;
     K.align_bytes = p.align_bytes;
-    const int wpc = 8;
+    int wpc = 8;
 
     if (!h->thresholded) {
         ibp_layout_strict(h);
@@ -679,20 +804,35 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         K.gtab = h->gtab_dev;
         K.store = h->store_dev;
         K.row_stride_strided = h->row_stride_strided;
-        K.slot_bytes = (h->max_stride + 15u) / 16u * 16u + 16u;
-        K.n_units = B.strided ? ((((n + p.group_param - 1) / p.group_param) + 15) / 16) * (uint64_t)p.group_param : (n + 15) / 16;
-        const size_t smem = (size_t)wpc * K.slot_bytes;
+        const bool bulk = !B.strided && p.align_bytes >= 16 && h->max_stride > 0 && h->max_stride <= 12288 && !getenv("IBP_PACK_NO_BULK");
+        size_t smem;
+        if (bulk) {
+            K.rows_per_unit = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(16, 12288 / h->max_stride));
+            K.slot_bytes = (K.rows_per_unit * h->max_stride + 16u + 127u) / 128u * 128u;
+            K.n_units = (n + K.rows_per_unit - 1) / K.rows_per_unit;
+            while (wpc > 1 && (size_t)wpc * 2 * K.slot_bytes > 200 * 1024) wpc >>= 1;
+            smem = (size_t)wpc * 2 * K.slot_bytes;
+        } else {
+            K.slot_bytes = (h->max_stride + 15u) / 16u * 16u + 16u;
+            K.n_units = B.strided ? ((((n + p.group_param - 1) / p.group_param) + 15) / 16) * (uint64_t)p.group_param : (n + 15) / 16;
+            while (wpc > 1 && (size_t)wpc * K.slot_bytes > 200 * 1024) wpc >>= 1;
+            smem = (size_t)wpc * K.slot_bytes;
+        }
         if (smem > 200 * 1024) { ibp_set_error("ibp_build_device: packed rows of %u bytes do not fit the shared-memory row images", h->max_stride); return IBP_ERR_UNSUPPORTED; }
-        const int grid = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 8);
-#define IBP_PACK(W_)                                                                                                         \
+        const int grid = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * (bulk ? 2 : 8));
+#define IBP_PACK(KERN_, W_)                                                                                                  \
     do {                                                                                                                     \
-        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(ibp_pack_kernel<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        ibp_pack_kernel<W_><<<grid, wpc * 32, smem, st>>>(K);                                                                \
+        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(KERN_<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        KERN_<W_><<<grid, wpc * 32, smem, st>>>(K);                                                                          \
     } while (0)
-        if (h->max_stride) {
-            switch (W) { case 4: IBP_PACK(4); break; case 2: IBP_PACK(2); break; default: IBP_PACK(1); break; }
+        t_pack.start();
+        if (h->max_stride && bulk) {
+            switch (W) { case 4: IBP_PACK(ibp_pack_bulk_kernel, 4); break; case 2: IBP_PACK(ibp_pack_bulk_kernel, 2); break; default: IBP_PACK(ibp_pack_bulk_kernel, 1); break; }
+        } else if (h->max_stride) {
+            switch (W) { case 4: IBP_PACK(ibp_pack_kernel, 4); break; case 2: IBP_PACK(ibp_pack_kernel, 2); break; default: IBP_PACK(ibp_pack_kernel, 1); break; }
         }
 #undef IBP_PACK
+        t_pack.stop();
         IBP_CUDA(cudaGetLastError());
         IBP_CUDA(cudaStreamSynchronize(st));
     } else {
@@ -711,15 +851,19 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         K.sum_size = sum_size;
         K.n_units = n_flag_words;
         const int grid1 = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 8);
+        t_size.start();
         switch (W) {
             case 4: ibp_size_kernel<4><<<grid1, wpc * 32, 0, st>>>(K); break;
             case 2: ibp_size_kernel<2><<<grid1, wpc * 32, 0, st>>>(K); break;
             default: ibp_size_kernel<1><<<grid1, wpc * 32, 0, st>>>(K); break;
         }
+        t_size.stop();
         IBP_CUDA(cudaGetLastError());
+        t_scan.start();
         ibp_scan_sums<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
         ibp_scan_bsums<<<1, 1024, 0, st>>>(bsum, nblk);
         ibp_scan_apply<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+        t_scan.stop();
         IBP_CUDA(cudaGetLastError());
         unsigned long long totals[2] = {0, 0};   // [0] = store size in 16-byte units, [1] = sum of the byte-aligned row sizes
         IBP_CUDA(cudaMemcpyAsync(totals, bsum + nblk, 16, cudaMemcpyDeviceToHost, st));
@@ -744,21 +888,42 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         if (!h->store_dev) { ibp_set_error("ibp_build_device: the packed store is not GPU-visible"); return IBP_ERR_BAD_STATE; }
         K.store = h->store_dev;
         K.row_off = h->row_off_dev;
-        K.slot_bytes = (h->max_stride + 15u) / 16u * 16u + 16u;
-        const size_t smem = (size_t)wpc * K.slot_bytes;
+        K.rows_per_unit = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(16, 12288 / h->max_stride));
+        K.slot_bytes = (K.rows_per_unit * h->max_stride + 16u + 127u) / 128u * 128u;
+        K.n_units = (n + K.rows_per_unit - 1) / K.rows_per_unit;
+        while (wpc > 1 && (size_t)wpc * 2 * K.slot_bytes > 200 * 1024) wpc >>= 1;
+        const size_t smem = (size_t)wpc * 2 * K.slot_bytes;
         if (smem > 200 * 1024) { ibp_set_error("ibp_build_device: rows of %u bytes do not fit the shared-memory row images", p.row_bytes); return IBP_ERR_UNSUPPORTED; }
-        const int grid2 = (int)std::min<uint64_t>((n + wpc - 1) / wpc, (uint64_t)sms * 8);
+        const int grid2 = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 2);
 #define IBP_PACK_T(W_)                                                                                                         \
     do {                                                                                                                       \
         if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(ibp_pack_t_kernel<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
         ibp_pack_t_kernel<W_><<<grid2, wpc * 32, smem, st>>>(K);                                                               \
     } while (0)
+        t_pack.start();
         switch (W) { case 4: IBP_PACK_T(4); break; case 2: IBP_PACK_T(2); break; default: IBP_PACK_T(1); break; }
 #undef IBP_PACK_T
+        t_pack.stop();
         IBP_CUDA(cudaGetLastError());
         IBP_CUDA(cudaStreamSynchronize(st));
     }
+    h->built_on_device = true;
+    ibp_build_stats& S = h->build_stats;
+    S.mask_ms = t_mask.ms();
+    S.pack_ms = t_pack.ms();
+    if (h->thresholded) { S.size_ms = t_size.ms(); S.scan_ms = t_scan.ms(); }
+    S.raw_bytes = n * (uint64_t)p.row_bytes;
+    S.store_bytes = h->packed_bytes_rows;
+    S.slices_per_group = B.ns;
+    S.total_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     guard.h = nullptr;
     *out_handle = h;
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_get_build_stats(const ibp_handle* h, ibp_build_stats* out) {
+    if (!h || !out) { ibp_set_error("ibp_get_build_stats: null argument"); return IBP_ERR_INVALID_ARG; }
+    if (!h->built_on_device) { ibp_set_error("ibp_get_build_stats: the handle was built by ibp_build (host)"); return IBP_ERR_BAD_STATE; }
+    *out = h->build_stats;
     return IBP_OK;
 }

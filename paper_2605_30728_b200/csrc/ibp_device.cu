@@ -1069,7 +1069,7 @@ __global__ void ibp_contig_read_kernel(const uint4* __restrict__ src, size_t n_v
     if (acc == 0x9E3779B9u) *sink = acc;   // keeps the loads alive; practically never true
 }
 
-static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps, bool zero_copy) {
+static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps, bool zero_copy, bool d2h = false) {
     if (!gbps || nbytes < (1u << 20) || reps < 1) { ibp_set_error("ibp_measure_*: bad argument"); return IBP_ERR_INVALID_ARG; }
     IBP_CUDA(cudaSetDevice(device));
     void *hp = nullptr, *dp = nullptr, *hd = nullptr;
@@ -1087,6 +1087,7 @@ static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps
         for (int it = 0; it < reps + 1; ++it) {   // first iteration is a warm-up
             cudaEventRecord(a, 0);
             if (zero_copy) ibp_contig_read_kernel<<<148 * 4, 512>>>((const uint4*)hd, nbytes / 16, sink);
+            else if (d2h) cudaMemcpyAsync(hp, dp, nbytes, cudaMemcpyDeviceToHost, 0);
             else cudaMemcpyAsync(dp, hp, nbytes, cudaMemcpyHostToDevice, 0);
             cudaEventRecord(b, 0);
             if (cudaEventSynchronize(b) != cudaSuccess) { ibp_set_error("ibp_measure_*: %s", cudaGetErrorString(cudaGetLastError())); rc = IBP_ERR_CUDA; break; }
@@ -1105,6 +1106,7 @@ static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps
 }
 extern "C" ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, false); }
 extern "C" ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, true); }
+extern "C" ibp_status ibp_measure_d2h(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, false, true); }
 
 // 1 = de-duplicate the ids of a random gather before fetching; 0 = fetch every id (the caller knows the ids are distinct);
 // -1 = automatic (default): on for batches of >= 16384 ids.

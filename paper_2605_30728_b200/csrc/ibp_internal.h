@@ -46,6 +46,10 @@ struct ibp_handle {
     IbpGroupEntry* gtab_dev = nullptr;
     uint32_t* mvtab_dev = nullptr;         // optional expand move masks, 5 per (group, word)
 
+    // ibp_build_device only
+    bool built_on_device = false;
+    ibp_build_stats build_stats{};
+
     // launch configuration
     uint32_t max_ctas = 0, warps_per_cta = 0;
     int sm_count = 0;

@@ -55,7 +55,7 @@ def test_tiny_blocked(align):
     (1, 5, 203, 32, 16), (1, 8, 64, 16, 1), (1, 3, 2, 4, 16), (0, 1, 9, 20, 8), (0, 33, 1000, 100, 32),
     (0, 128, 700, 256, 32), (0, 256, 1500, 512, 32), (0, 50, 333, 1024, 32), (0, 20, 77, 4096, 64), (1, 6, 600, 2048, 16),
     (0, 9, 100, 516, 4), (0, 9, 100, 264, 1), (0, 4, 30, 8192, 128), (0, 5000, 20000, 64, 32), (1, 3, 30000, 128, 16),
-    (0, 1 << 30, 70000, 32, 32),
+    (0, 1 << 30, 70000, 32, 32), (0, 4, 12, 65536, 32),
 ])
 def test_strict_shapes(kind, param, n, rb, align):
     """Odd row sizes (W = 1, 2, 4; 1..16 passes), ragged last groups, strided groups with a partial last matrix row, groups
@@ -127,7 +127,8 @@ def test_source_rows_in_mapped_host_memory():
 @pytest.mark.parametrize("kind,param,n,rb,thr", [(0, 64, 1000, 64, (4, 5)), (0, 7, 50, 12, (4, 5)), (0, 256, 700, 512, (7, 10)),
                                                  (1, 5, 203, 32, (4, 5)), (1, 6, 600, 256, (9, 10)), (0, 1 << 30, 900, 128, (4, 5)),
                                                  (0, 300, 1000, 8, (4, 5)), (0, 16, 100, 2048, (3, 4)), (0, 600, 3000, 64, (4, 5)),
-                                                 (0, 1 << 30, 70000, 32, (4, 5)), (1, 3, 30000, 128, (3, 4))])
+                                                 (0, 1 << 30, 70000, 32, (4, 5)), (1, 3, 30000, 128, (3, 4)),
+                                                 (0, 4, 12, 65536, (3, 4))])
 def test_T_shapes(kind, param, n, rb, thr):
     rng = np.random.default_rng(rb + n)
     X = _masked_rows(n, rb)
