@@ -212,6 +212,43 @@ ibp_status ibp_validate_ids(ibp_handle* h, const int64_t* row_ids_dev, int64_t n
 ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* row_ids_host, int64_t n, uint64_t* n_unique,
                                 uint64_t* stored, uint64_t* bytealigned);
 
+/* -- Compressed GPU software cache (Fig. 6a).  A static cache of packed rows in GPU memory:
+ * "data slabs" (one contiguous region each, up to 8: the 3-bit slab id) hold the rows exactly as they lie in the host store,
+ * and a hash map in GPU memory maps a row id to ONE 64-bit value (reading R22 for the bit positions):
+ *      bits  0..39  byte offset inside the slab (40 bits, 1 TB)
+ *      bits 40..42  slab id (3 bits)
+ *      bit  43      1 = the row is stored compressed, 0 = raw (thresholded mode keeps some rows raw; strict: always 1)
+ *      bits 44..63  spare, zero
+ * ibp_cache_gather_decompress is ibp_gather_decompress with one extra step in S1: the id is looked up in the map; a hit
+ * reads the packed row from its slab (HBM), a miss reads it from the host store over PCIe; S2-S6 are the same kernel code,
+ * so the output is identical.  index_span must be 1.  The cache borrows the handle, which must outlive it.             */
+typedef struct ibp_cache ibp_cache;
+#define IBP_CACHE_MISS 0xFFFFFFFFFFFFFFFFull
+typedef struct {
+    uint64_t capacity_bytes, used_bytes;   /* all slabs together                                                        */
+    uint64_t n_entries, max_entries;
+    uint64_t map_bytes;                    /* hash map in GPU memory: 16 bytes per slot, >= 2 slots per possible entry  */
+    uint32_t n_slabs, reserved;
+    uint64_t slab_bytes;                   /* capacity of one slab                                                      */
+} ibp_cache_info;
+/* capacity_bytes is split evenly over n_slabs (1..8) slabs on the handle's device; max_entries bounds the map (0 = n_rows).
+ * BAD_STATE before ibp_upload_metadata / with a pageable store; UNSUPPORTED when index_span != 1.                       */
+ibp_status ibp_cache_create(ibp_handle* h, uint64_t capacity_bytes, uint32_t n_slabs, uint64_t max_entries, void* cuda_stream,
+                            ibp_cache** out_cache);
+/* Static fill: for every id of row_ids_host (n int64 on the HOST, in priority order) that is not cached yet, copies its packed
+ * row from the host store into the current slab (a CUDA kernel reading zero-copy) and adds the map entry; stops at the first
+ * row that does not fit.  *n_inserted_host (optional) = rows added.  Synchronises the stream.  INVALID_ARG for ids out of
+ * range.                                                                                                               */
+ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host, int64_t n, void* cuda_stream, int64_t* n_inserted_host);
+/* S1-S6 with the cache in front of the host store (see above).  Arguments as ibp_gather_decompress.                    */
+ibp_status ibp_cache_gather_decompress(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);
+/* entries_dev[i] = the map value of row_ids_dev[i], or IBP_CACHE_MISS.  For tests and hit-rate accounting.  Asynchronous. */
+ibp_status ibp_cache_lookup(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, uint64_t* entries_dev, void* cuda_stream);
+/* Copies nbytes of slab memory addressed by a map value (slab id + offset) to the host.  For cross-checks.  Synchronous.   */
+ibp_status ibp_cache_read(const ibp_cache* c, uint64_t entry, uint32_t nbytes, void* out_host);
+ibp_status ibp_cache_get_info(const ibp_cache* c, ibp_cache_info* out);
+void ibp_cache_destroy(ibp_cache* c);
+
 void ibp_destroy(ibp_handle* h);
 const char* ibp_last_error(void);
 const char* ibp_version(void);

@@ -264,3 +264,23 @@ class DatasetT:
             self.close()
         except Exception:
             pass
+
+
+# ---------------------------------------------------------------------------------------------------- cache map value
+# "the hashmap now maps an ID to a 3-bit data slab ID, a 40-bit offset, and a bit indicating whether the tensor
+# is in compressed form or not ... We have 20 spare bits".  The paper gives the widths, not the positions; reading R22
+# (DESIGN.md): offset in bits 0..39, slab id in bits 40..42, compressed flag in bit 43, bits 44..63 zero.
+CACHE_OFFSET_BITS, CACHE_SLAB_BITS, CACHE_FLAG_BITS, CACHE_SPARE_BITS = 40, 3, 1, 20
+
+
+def cache_value(slab: int, offset: int, compressed: bool) -> int:
+    if not (0 <= slab < (1 << CACHE_SLAB_BITS)) or not (0 <= offset < (1 << CACHE_OFFSET_BITS)):
+        raise ValueError("slab id needs 3 bits, offset 40 bits (PAPER.md:353)")
+    return offset | (slab << CACHE_OFFSET_BITS) | (int(bool(compressed)) << (CACHE_OFFSET_BITS + CACHE_SLAB_BITS))
+
+
+def cache_value_fields(value: int):
+    """-> (slab, offset, compressed, spare)"""
+    value = int(value)
+    return ((value >> CACHE_OFFSET_BITS) & ((1 << CACHE_SLAB_BITS) - 1), value & ((1 << CACHE_OFFSET_BITS) - 1),
+            bool((value >> (CACHE_OFFSET_BITS + CACHE_SLAB_BITS)) & 1), value >> (CACHE_OFFSET_BITS + CACHE_SLAB_BITS + CACHE_FLAG_BITS))

@@ -52,6 +52,13 @@ class ibp_build_stats(C.Structure):
                 ("slices_per_group", C.c_uint32), ("reserved", C.c_uint32)]
 
 
+class ibp_cache_info(C.Structure):
+    _fields_ = [("capacity_bytes", C.c_uint64), ("used_bytes", C.c_uint64), ("n_entries", C.c_uint64), ("max_entries", C.c_uint64),
+                ("map_bytes", C.c_uint64), ("n_slabs", C.c_uint32), ("reserved", C.c_uint32), ("slab_bytes", C.c_uint64)]
+
+
+IBP_CACHE_MISS = 0xFFFFFFFFFFFFFFFF
+
 # name -> (restype, argtypes); every symbol include/ibp.h declares (tests/test_abi.py checks the two lists agree)
 _vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int
 SIGNATURES = {
@@ -71,6 +78,13 @@ SIGNATURES = {
     "ibp_configure": (_int, [_vp, _u32, _u32]),
     "ibp_validate_ids": (_int, [_vp, _vp, _i64, C.POINTER(_i64), _vp]),
     "ibp_batch_link_bytes": (_int, [_vp, _vp, _i64, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]),
+    "ibp_cache_create": (_int, [_vp, _u64, _u32, _u64, _vp, C.POINTER(_vp)]),
+    "ibp_cache_insert": (_int, [_vp, _vp, _i64, _vp, C.POINTER(_i64)]),
+    "ibp_cache_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
+    "ibp_cache_lookup": (_int, [_vp, _vp, _i64, _vp, _vp]),
+    "ibp_cache_read": (_int, [_vp, _u64, _u32, _vp]),
+    "ibp_cache_get_info": (_int, [_vp, C.POINTER(ibp_cache_info)]),
+    "ibp_cache_destroy": (None, [_vp]),
     "ibp_destroy": (None, [_vp]),
     "ibp_last_error": (C.c_char_p, []),
     "ibp_version": (C.c_char_p, []),
@@ -153,6 +167,12 @@ class Handle:
         data = np.ctypeslib.as_array(C.cast(p.value, C.POINTER(C.c_uint8)), (st.value,)).copy() if st.value else np.zeros(0, np.uint8)
         return data, k.value
 
+    def row_ptr(self, row) -> int:
+        """host address of the packed row inside the store"""
+        p = _vp()
+        _check(lib().ibp_row_info(self._h, row, C.byref(p), None, None, None))
+        return p.value or 0
+
     def row_info(self, row):
         """(the row's byte-aligned stored bytes, bytes occupied incl. padding, is_compressed)"""
         p, st, sz, fl = _vp(), _u32(), _u32(), _int()
@@ -220,6 +240,48 @@ class Handle:
         if self._h:
             lib().ibp_destroy(self._h)
             self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class Cache:
+    """Owns an ibp_cache* (compressed GPU software cache).  Keeps its Handle alive."""
+
+    def __init__(self, handle: Handle, capacity_bytes: int, n_slabs: int = 1, max_entries: int = 0, stream=None):
+        c = _vp()
+        _check(lib().ibp_cache_create(handle._h, capacity_bytes, n_slabs, max_entries, stream, C.byref(c)))
+        self._c, self.handle = c, handle
+
+    def insert(self, row_ids_host, stream=None) -> int:
+        ids = np.ascontiguousarray(row_ids_host, dtype=np.int64)
+        k = _i64()
+        _check(lib().ibp_cache_insert(self._c, ids.ctypes.data, ids.size, stream, C.byref(k)))
+        return k.value
+
+    def gather_decompress(self, row_ids_dev, n, out_dev, stream=None):
+        _check(lib().ibp_cache_gather_decompress(self._c, _ptr(row_ids_dev), n, _ptr(out_dev), stream))
+
+    def lookup(self, row_ids_dev, n, entries_dev, stream=None):
+        _check(lib().ibp_cache_lookup(self._c, _ptr(row_ids_dev), n, _ptr(entries_dev), stream))
+
+    def read(self, entry: int, nbytes: int) -> np.ndarray:
+        out = np.empty(nbytes, np.uint8)
+        _check(lib().ibp_cache_read(self._c, entry, nbytes, out.ctypes.data))
+        return out
+
+    def info(self):
+        ci = ibp_cache_info()
+        _check(lib().ibp_cache_get_info(self._c, C.byref(ci)))
+        return ci
+
+    def destroy(self):
+        if self._c:
+            lib().ibp_cache_destroy(self._c)
+            self._c = None
 
     def __del__(self):
         try:

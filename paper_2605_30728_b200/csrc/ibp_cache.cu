@@ -1,0 +1,176 @@
+// ibp_cache.cu -- compressed GPU software cache (Fig. 6a): data slabs + hash map; management side.
+// The lookup-and-decode path is ibp_cache_gather_decompress in ibp_device.cu (the decode kernel with a map probe in S1).
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "ibp_devutil.cuh"
+
+namespace {
+
+struct FillItem {          // one row to add: copy `bytes` from the host store at `src` to slab memory at `dst`, then map id -> entry
+    uint64_t id, entry, src;
+    uint32_t bytes, slab;
+};
+
+__global__ void ibp_cache_fill_kernel(const FillItem* __restrict__ items, int64_t n, const uint8_t* __restrict__ store,
+                                      uint8_t* const* __restrict__ slabs, uint64_t* __restrict__ map, uint32_t mask) {
+    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    for (int64_t i = (int64_t)blockIdx.x * wpc + (threadIdx.x >> 5); i < n; i += (int64_t)gridDim.x * wpc) {
+        const FillItem it = items[i];
+        const uint4* src = (const uint4*)(store + it.src);
+        uint4* dst = (uint4*)(slabs[it.slab] + (it.entry & ((1ull << 40) - 1)));
+        for (uint32_t v = lane; v < it.bytes / 16; v += 32) {
+            uint4 t;
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(t.x), "=r"(t.y), "=r"(t.z), "=r"(t.w) : "l"(src + v));
+            dst[v] = t;
+        }
+        if (lane == 0) {
+            uint32_t slot = ibp_cache_hash(it.id, mask);
+            for (;;) {
+                const unsigned long long prev = atomicCAS((unsigned long long*)&map[2ull * slot], 0ull, (unsigned long long)(it.id + 1));
+                if (prev == 0ull || prev == it.id + 1) { map[2ull * slot + 1] = it.entry; break; }
+                slot = (slot + 1) & mask;
+            }
+        }
+    }
+}
+
+__global__ void ibp_cache_lookup_kernel(const uint64_t* __restrict__ map, uint32_t mask, const int64_t* __restrict__ ids, int64_t n,
+                                        uint64_t* __restrict__ entries) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        entries[i] = ibp_cache_find(map, mask, (uint64_t)ids[i]);
+}
+
+}  // namespace
+
+extern "C" ibp_status ibp_cache_create(ibp_handle* h, uint64_t capacity_bytes, uint32_t n_slabs, uint64_t max_entries, void* cuda_stream,
+                                       ibp_cache** out_cache) {
+    if (!h || !out_cache || n_slabs < 1 || n_slabs > 8 || capacity_bytes == 0) { ibp_set_error("ibp_cache_create: bad argument (1..8 slabs, capacity > 0)"); return IBP_ERR_INVALID_ARG; }
+    if (h->device < 0 || !h->meta_dev) { ibp_set_error("ibp_cache_create: call ibp_upload_metadata first"); return IBP_ERR_BAD_STATE; }
+    if (!h->store_dev) { ibp_set_error("ibp_cache_create: the packed store is not GPU-mapped (pageable store)"); return IBP_ERR_BAD_STATE; }
+    if (h->p.index_span != 1) { ibp_set_error("ibp_cache_create: index_span must be 1"); return IBP_ERR_UNSUPPORTED; }
+    const uint64_t slab_bytes = capacity_bytes / n_slabs / 16 * 16;
+    if (slab_bytes == 0 || slab_bytes >= (1ull << 40)) { ibp_set_error("ibp_cache_create: a slab must hold 16 bytes .. 1 TB (40-bit offsets, P:353)"); return IBP_ERR_INVALID_ARG; }
+    ibp_cache* c = new (std::nothrow) ibp_cache();
+    if (!c) { ibp_set_error("ibp_cache_create: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    c->h = h;
+    c->n_slabs = n_slabs;
+    c->slab_bytes = slab_bytes;
+    c->max_entries = max_entries ? std::min<uint64_t>(max_entries, h->p.n_rows) : h->p.n_rows;
+    uint64_t cap = 1024;
+    while (cap < 2 * c->max_entries) cap <<= 1;
+    if (cap > (1ull << 31)) { delete c; ibp_set_error("ibp_cache_create: too many entries for the map"); return IBP_ERR_UNSUPPORTED; }
+    c->map_cap = (uint32_t)cap;
+    try { c->present.assign((h->p.n_rows + 63) / 64, 0ull); } catch (...) { delete c; ibp_set_error("ibp_cache_create: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSetDevice(h->device);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->map_dev, cap * 16);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->map_dev, 0, cap * 16, st);
+    for (uint32_t s = 0; s < n_slabs && e == cudaSuccess; ++s) e = cudaMalloc((void**)&c->slab_dev[s], slab_bytes + 64);   // slack: 16-byte covers
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        ibp_set_error("ibp_cache_create: %s", cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        ibp_cache_destroy(c);
+        return e == cudaErrorMemoryAllocation ? IBP_ERR_OUT_OF_MEMORY : IBP_ERR_CUDA;
+    }
+    *out_cache = c;
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host, int64_t n, void* cuda_stream, int64_t* n_inserted_host) {
+    if (!c || n < 0 || (!row_ids_host && n > 0)) { ibp_set_error("ibp_cache_insert: bad argument"); return IBP_ERR_INVALID_ARG; }
+    if (n_inserted_host) *n_inserted_host = 0;
+    const ibp_handle* h = c->h;
+    std::vector<FillItem> items;
+    try { items.reserve((size_t)std::min<int64_t>(n, 1 << 20)); } catch (...) {}
+    bool full = false;
+    for (int64_t i = 0; i < n && !full; ++i) {
+        const int64_t sid = row_ids_host[i];
+        if (sid < 0 || (uint64_t)sid >= h->p.n_rows) { ibp_set_error("ibp_cache_insert: id %lld out of range", (long long)sid); return IBP_ERR_INVALID_ARG; }
+        const uint64_t id = (uint64_t)sid;
+        if ((c->present[id >> 6] >> (id & 63)) & 1ull) continue;
+        if (c->n_entries + items.size() >= c->max_entries) break;
+        // the 16-byte-aligned cover of the packed row, exactly what the decode kernel fetches from the store
+        const uint64_t off = ibp_row_offset(h, id);
+        uint64_t bytes, flag = 1;
+        if (h->thresholded) {
+            bytes = 16ull * (h->row_off[id + 1] - h->row_off[id]);
+            flag = (h->row_flag[id >> 5] >> (id & 31)) & 1u;
+        } else {
+            bytes = h->gtab[ibp_group_of(h, id)].stride;
+        }
+        const uint64_t head = off & 15ull, cover = bytes ? (head + bytes + 15ull) & ~15ull : 0ull;
+        while (c->cur_slab < c->n_slabs && c->slab_used[c->cur_slab] + cover > c->slab_bytes) ++c->cur_slab;
+        if (c->cur_slab >= c->n_slabs) { full = true; c->cur_slab = c->n_slabs - 1; break; }
+        FillItem it;
+        it.id = id;
+        it.slab = c->cur_slab;
+        it.entry = c->slab_used[it.slab] | ((uint64_t)it.slab << 40) | (flag << 43);
+        it.src = off - head;
+        it.bytes = (uint32_t)cover;
+        c->slab_used[it.slab] += cover;
+        c->present[id >> 6] |= 1ull << (id & 63);
+        try { items.push_back(it); } catch (...) { ibp_set_error("ibp_cache_insert: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    }
+    if (items.empty()) return IBP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    IBP_CUDA(cudaSetDevice(h->device));
+    FillItem* items_dev = nullptr;
+    uint8_t** slabs_dev = nullptr;
+    IBP_CUDA(cudaMalloc((void**)&items_dev, items.size() * sizeof(FillItem)));
+    cudaError_t e = cudaMalloc((void**)&slabs_dev, 8 * sizeof(uint8_t*));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(items_dev, items.data(), items.size() * sizeof(FillItem), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(slabs_dev, c->slab_dev, 8 * sizeof(uint8_t*), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        const int blocks = (int)std::min<size_t>((items.size() + 7) / 8, 148 * 8);
+        ibp_cache_fill_kernel<<<blocks, 256, 0, st>>>(items_dev, (int64_t)items.size(), h->store_dev, slabs_dev, c->map_dev, c->map_cap - 1);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(items_dev);
+    if (slabs_dev) cudaFree(slabs_dev);
+    if (e != cudaSuccess) { ibp_set_error("ibp_cache_insert: %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return IBP_ERR_CUDA; }
+    c->n_entries += items.size();
+    if (n_inserted_host) *n_inserted_host = (int64_t)items.size();
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_cache_lookup(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, uint64_t* entries_dev, void* cuda_stream) {
+    if (!c || n < 0 || (n > 0 && (!row_ids_dev || !entries_dev))) { ibp_set_error("ibp_cache_lookup: bad argument"); return IBP_ERR_INVALID_ARG; }
+    if (n == 0) return IBP_OK;
+    ibp_cache_lookup_kernel<<<(int)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, (cudaStream_t)cuda_stream>>>(c->map_dev, c->map_cap - 1, row_ids_dev, n, entries_dev);
+    IBP_CUDA(cudaGetLastError());
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_cache_read(const ibp_cache* c, uint64_t entry, uint32_t nbytes, void* out_host) {
+    if (!c || !out_host || entry == IBP_CACHE_MISS) { ibp_set_error("ibp_cache_read: bad argument"); return IBP_ERR_INVALID_ARG; }
+    const uint64_t off = entry & ((1ull << 40) - 1), slab = (entry >> 40) & 7ull;
+    if (slab >= c->n_slabs || off + nbytes > c->slab_bytes + 64 || (entry >> 44)) { ibp_set_error("ibp_cache_read: not a valid map value"); return IBP_ERR_INVALID_ARG; }
+    IBP_CUDA(cudaMemcpy(out_host, c->slab_dev[slab] + off, nbytes, cudaMemcpyDeviceToHost));
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_cache_get_info(const ibp_cache* c, ibp_cache_info* out) {
+    if (!c || !out) { ibp_set_error("ibp_cache_get_info: null argument"); return IBP_ERR_INVALID_ARG; }
+    memset(out, 0, sizeof *out);
+    out->capacity_bytes = c->slab_bytes * c->n_slabs;
+    for (uint32_t s = 0; s < c->n_slabs; ++s) out->used_bytes += c->slab_used[s];
+    out->n_entries = c->n_entries;
+    out->max_entries = c->max_entries;
+    out->map_bytes = (uint64_t)c->map_cap * 16;
+    out->n_slabs = c->n_slabs;
+    out->slab_bytes = c->slab_bytes;
+    return IBP_OK;
+}
+
+extern "C" void ibp_cache_destroy(ibp_cache* c) {
+    if (!c) return;
+    if (c->map_dev) cudaFree(c->map_dev);
+    for (int s = 0; s < 8; ++s) if (c->slab_dev[s]) cudaFree(c->slab_dev[s]);
+    (void)cudaGetLastError();
+    delete c;
+}

@@ -50,6 +50,10 @@ struct DecodeParams {
     const uint32_t* row_off;       // thresholded mode: per-row offsets (16-byte units), n_rows + 1 entries
     const uint32_t* row_flag;      // thresholded mode: bit r = 1 iff row r is compressed
     uint32_t keep_l2;              // write the rows with the default cache policy (a later pass re-reads them) instead of streaming
+    // compressed GPU cache in front of the store (CACHE instantiations only)
+    const uint64_t* cmap;          // hash map slots {id + 1, value}; value = offset:40 | slab:3 | compressed:1
+    uint32_t cmap_mask;
+    const uint8_t* slab[8];
 };
 
 // ------------------------------------------------------------------------------------------------ device helpers
@@ -117,7 +121,9 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 // offset table, the per-row bitmask says whether it is stored raw, the first n_words bits of a compressed row are
 // the participation bits (one per 4-byte chunk), and a chunk contributes 32 - popc(Mask_i) bits if it participates, else 32
 // (reading R7) -- so the exclusive scan of step 3 runs per row instead of per group.
-template <int W, int NST, int MODE, int FETCH, bool TM>
+// CACHE = the compressed GPU cache sits in front of the store: S1 probes the hash map; a hit fetches the same
+// 16-byte-aligned cover from the row's slab in HBM instead of the host store, everything after the fetch is unchanged.
+template <int W, int NST, int MODE, int FETCH, bool TM, bool CACHE = false>
 __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
@@ -206,6 +212,10 @@ __global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) 
                 const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
                 a0 = src - head;                                              // 16-byte aligned cover
                 nvec = fe.stride ? (head + fe.stride + 15u) >> 4 : 0u;
+            }
+            if (CACHE) {
+                const uint64_t ent = ibp_cache_find(P.cmap, P.cmap_mask, id);
+                if (ent != IBP_CACHE_MISS_DEV) a0 = P.slab[(ent >> 40) & 7ull] + (ent & ((1ull << 40) - 1));
             }
             const uint32_t slot = seq_f % NST;
             const uint32_t dst = ring_s + slot * P.slot_bytes;
@@ -509,9 +519,9 @@ static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_s
 // ------------------------------------------------------------------------------------------------ launch
 // The grid is persistent: at most as many CTAs as are resident at once, so that the units in flight form one contiguous
 // window of the (locality-ordered) unit list; a larger grid with a grid-stride loop would interleave far-apart windows.
-template <int W, int NST, int MODE, int FETCH, bool TM = false>
+template <int W, int NST, int MODE, int FETCH, bool TM = false, bool CACHE = false>
 static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64_t max_ctas, int sm_count, int wpc, size_t smem, cudaStream_t st) {
-    auto kern = ibp_decode_kernel<W, NST, MODE, FETCH, TM>;
+    auto kern = ibp_decode_kernel<W, NST, MODE, FETCH, TM, CACHE>;
     static thread_local size_t attr_smem = 0;
     if (smem > 48 * 1024 && smem > attr_smem) {
         IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -549,6 +559,10 @@ static ibp_status launch_decode(ibp_handle* h, DecodeParams& P, int mode, cudaSt
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory ring", h->max_stride); return IBP_ERR_UNSUPPORTED; }
     const int64_t blocks = (P.n_units + wpc - 1) / wpc;
 #define IBP_LAUNCH(W_, NST_, MODE_)                                                                                   \
+    if (MODE_ == MODE_ROWS && P.cmap) {                                                                                \
+        if (h->thresholded) return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, true, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
+        return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, false, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
+    }                                                                                                                  \
     if (h->thresholded) return launch_one<W_, NST_, MODE_, FETCH_TMA, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
     return fetch == FETCH_TMA ? launch_one<W_, NST_, MODE_, FETCH_TMA>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st) \
                               : launch_one<W_, NST_, MODE_, FETCH_LSU>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st)
@@ -813,6 +827,62 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
     return ibp_attach_device(h, device, cuda_stream);
 }
 
+// Random row gather (index_span 1): pre-passes, decode kernel, replication of repeats.  `c` = optional compressed GPU cache.
+static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, cudaStream_t st) {
+    if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
+    DecodeParams P;
+    fill_common(h, P);
+    P.store = h->store_dev;
+    P.ids = row_ids_dev;
+    P.out = (uint8_t*)out_dev;
+    P.n = n;
+    P.span = 1;
+    P.n_units = n;
+    if (c) {
+        P.cmap = c->map_dev;
+        P.cmap_mask = c->map_cap - 1;
+        for (int s = 0; s < 8; ++s) P.slab[s] = c->slab_dev[s];
+    }
+    const bool dedup = (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
+    // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
+    // Essential for the 4 KB-page pinned store, a few percent for the managed-host store -- unless repeated ids are
+    // fetched one by one (dedup off on a batch with repeats), where neighbours in the order collide on the same lines.
+    const bool order = h->order_mode == 1 || (h->order_mode < 0 && h->store_used > (64ull << 20) && n >= 4096);
+    RowPrepass R;
+    ibp_status s = IBP_OK;
+    if (dedup || order) {
+        s = rows_prepass(row_ids_dev, n, dedup, order, h->p.n_rows, h->store_used, st, &R);
+        if (s != IBP_OK) return s;
+    }
+    P.order = R.list;
+    P.n_units_dev = R.n_list;
+    P.keep_l2 = dedup;                  // the replication pass re-reads the decoded rows: keep them in L2
+    s = launch_decode(h, P, MODE_ROWS, st);
+    if (s == IBP_OK && dedup) {
+        const uint32_t rb = h->p.row_bytes;
+        const int lpr = rb >= 512 ? 32 : rb >= 256 ? 16 : rb >= 128 ? 8 : 4, rpw = 32 / lpr;
+        const int blocks = (int)std::min<int64_t>((n + 8 * rpw - 1) / (8 * rpw), 148 * 8);
+        switch (lpr) {
+            case 32: ibp_dedup_copy<32><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+            case 16: ibp_dedup_copy<16><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+            case 8: ibp_dedup_copy<8><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+            default: ibp_dedup_copy<4><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
+        }
+        if (cudaGetLastError() != cudaSuccess) { ibp_set_error("ibp_dedup_copy launch failed"); s = IBP_ERR_CUDA; }
+    }
+    if (R.ws) IBP_CUDA(cudaFreeAsync(R.ws, st));
+    return s;
+}
+
+extern "C" ibp_status ibp_cache_gather_decompress(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream) {
+    if (!c) { ibp_set_error("ibp_cache_gather_decompress: null cache"); return IBP_ERR_INVALID_ARG; }
+    ibp_status s = check_ready(c->h, "ibp_cache_gather_decompress");
+    if (s != IBP_OK) return s;
+    if (n == 0) return IBP_OK;
+    if (n < 0 || !row_ids_dev || !out_dev || ((uintptr_t)out_dev & 15u)) { ibp_set_error("ibp_cache_gather_decompress: bad argument (null pointer, n<0, or out not 16-byte aligned)"); return IBP_ERR_INVALID_ARG; }
+    return gather_rows(c->h, c, row_ids_dev, n, out_dev, (cudaStream_t)cuda_stream);
+}
+
 extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream) {
     ibp_status s = check_ready(h, "ibp_gather_decompress");
     if (s != IBP_OK) return s;
@@ -820,6 +890,7 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     if (n < 0 || !row_ids_dev || !out_dev || ((uintptr_t)out_dev & 15u)) { ibp_set_error("ibp_gather_decompress: bad argument (null pointer, n<0, or out not 16-byte aligned)"); return IBP_ERR_INVALID_ARG; }
     if (!h->store_dev) { ibp_set_error("ibp_gather_decompress: the packed store is not GPU-mapped (pageable store)"); return IBP_ERR_BAD_STATE; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (h->p.index_span == 1) return gather_rows(h, nullptr, row_ids_dev, n, out_dev, st);
     DecodeParams P;
     fill_common(h, P);
     P.store = h->store_dev;
@@ -827,38 +898,6 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     P.out = (uint8_t*)out_dev;
     P.n = n;
     P.span = h->p.index_span;
-    if (h->p.index_span == 1) {
-        if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
-        P.n_units = n;
-        const bool dedup = (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
-        // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
-        // Essential for the 4 KB-page pinned store, a few percent for the managed-host store -- unless repeated ids are
-        // fetched one by one (dedup off on a batch with repeats), where neighbours in the order collide on the same lines.
-        const bool order = h->order_mode == 1 || (h->order_mode < 0 && h->store_used > (64ull << 20) && n >= 4096);
-        RowPrepass R;
-        if (dedup || order) {
-            s = rows_prepass(row_ids_dev, n, dedup, order, h->p.n_rows, h->store_used, st, &R);
-            if (s != IBP_OK) return s;
-        }
-        P.order = R.list;
-        P.n_units_dev = R.n_list;
-        P.keep_l2 = dedup;                  // the replication pass re-reads the decoded rows: keep them in L2
-        s = launch_decode(h, P, MODE_ROWS, st);
-        if (s == IBP_OK && dedup) {
-            const uint32_t rb = h->p.row_bytes;
-            const int lpr = rb >= 512 ? 32 : rb >= 256 ? 16 : rb >= 128 ? 8 : 4, rpw = 32 / lpr;
-            const int blocks = (int)std::min<int64_t>((n + 8 * rpw - 1) / (8 * rpw), 148 * 8);
-            switch (lpr) {
-                case 32: ibp_dedup_copy<32><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
-                case 16: ibp_dedup_copy<16><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
-                case 8: ibp_dedup_copy<8><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
-                default: ibp_dedup_copy<4><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
-            }
-            if (cudaGetLastError() != cudaSuccess) { ibp_set_error("ibp_dedup_copy launch failed"); s = IBP_ERR_CUDA; }
-        }
-        if (R.ws) IBP_CUDA(cudaFreeAsync(R.ws, st));
-        return s;
-    }
     if (h->stream_mode && h->thresholded && stream_t_fits(h))
         return launch_stream_t(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
     if (h->stream_mode && !h->thresholded)

@@ -46,3 +46,18 @@ __device__ __forceinline__ uint64_t group_of_u(uint32_t group_param, uint32_t gr
     return group_shift != 0xFFFFFFFFu ? (id >> group_shift) : (id / group_param);
 }
 
+
+// ---- compressed GPU cache map: open addressing, linear probing, slots of {key = id + 1, value}
+#define IBP_CACHE_MISS_DEV 0xFFFFFFFFFFFFFFFFull
+__device__ __forceinline__ uint32_t ibp_cache_hash(uint64_t id, uint32_t mask) {
+    return (uint32_t)((id * 0x9E3779B97F4A7C15ull) >> 32) & mask;
+}
+__device__ __forceinline__ uint64_t ibp_cache_find(const uint64_t* __restrict__ map, uint32_t mask, uint64_t id) {
+    uint32_t slot = ibp_cache_hash(id, mask);
+    for (;;) {
+        const ulonglong2 e = __ldg((const ulonglong2*)map + slot);
+        if (e.x == id + 1) return e.y;
+        if (e.x == 0ull) return IBP_CACHE_MISS_DEV;
+        slot = (slot + 1) & mask;
+    }
+}

@@ -60,6 +60,19 @@ struct ibp_handle {
     int fetch_mode = 1;                    // 0 = cp.async (LSU), 1 = cp.async.bulk (TMA)
 };
 
+// Compressed GPU cache: slabs of packed rows + a hash map id -> 64-bit value {offset:40, slab:3, compressed:1}.
+struct ibp_cache {
+    ibp_handle* h = nullptr;
+    uint32_t n_slabs = 0, cur_slab = 0;
+    uint64_t slab_bytes = 0;
+    uint8_t* slab_dev[8] = {};
+    uint64_t slab_used[8] = {};
+    uint64_t* map_dev = nullptr;           // map_cap slots of {key = id + 1 (0 = empty), value}
+    uint32_t map_cap = 0;                  // power of two
+    uint64_t n_entries = 0, max_entries = 0;
+    std::vector<uint64_t> present;         // host bitmap of the cached row ids
+};
+
 // error plumbing (thread local)
 void ibp_set_error(const char* fmt, ...);
 

@@ -126,6 +126,10 @@ class GNN(Workload):
             self._cache["perm"] = np.random.Generator(np.random.PCG64(self.seed)).permutation(self.n_rows)
         return self._cache["cdf"], self._cache["perm"]
 
+    def hot_ids(self, k):
+        """The k ids of highest sampling probability (Zipf rank order): what a static cache would hold."""
+        return self._sampler()[1][:k].astype(np.int64)
+
     def ids(self, iteration):
         cdf, perm = self._sampler()
         want = min(self.batch_ids, self.n_rows)
@@ -159,6 +163,14 @@ class DLRM(Workload):
             self._cache["cdf"] = _zipf_cdf(self.rows_per_table, 1.05)
             self._cache["perm"] = np.random.Generator(np.random.PCG64(self.seed)).permutation(self.rows_per_table)
         return self._cache["cdf"], self._cache["perm"]
+
+    def hot_ids(self, k):
+        """The k ids of highest sampling probability: rank-major over the tables (every table has the same rank law)."""
+        _, perm = self._sampler()
+        n, per = self.rows_per_table, -(-k // self.n_tables)
+        t = np.arange(self.n_tables, dtype=np.int64)[None, :]
+        row = (perm[:per, None] + t * 104729) % n
+        return (t * n + row).reshape(-1)[:k].astype(np.int64)
 
     def ids(self, iteration):
         cdf, perm = self._sampler()

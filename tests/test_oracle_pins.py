@@ -380,3 +380,24 @@ def test_datasetT_rejects_tau_at_most_half():
     rows = datagen.random_bytes(64, 1).reshape(8, 8)
     with pytest.raises(ValueError):
         oracle.DatasetT(rows, oracle.BLOCKED, 8, 1, 2)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# compressed GPU cache: the 64-bit map value
+# ---------------------------------------------------------------------------------------------------------------------
+def test_cache_value_widths_from_the_paper():
+    """3-bit slab id ("up to 8 GPU slabs"), 40-bit offset ("up to 1 TB"), 1 flag bit, "20 spare bits" of 64."""
+    assert oracle.CACHE_SLAB_BITS + oracle.CACHE_OFFSET_BITS + oracle.CACHE_FLAG_BITS + oracle.CACHE_SPARE_BITS == 64
+    assert 1 << oracle.CACHE_SLAB_BITS == 8 and 1 << oracle.CACHE_OFFSET_BITS == 1 << 40 == 1024 ** 4
+    top = oracle.cache_value(7, (1 << 40) - 1, True)
+    assert top == (1 << 44) - 1 and top >> 44 == 0                       # the 20 spare bits stay zero
+    for slab, off, comp in [(0, 0, False), (0, 0, True), (5, 123456789, True), (7, 1 << 39, False)]:
+        assert oracle.cache_value_fields(oracle.cache_value(slab, off, comp)) == (slab, off, comp, 0)
+    # the fields do not overlap: flipping one changes only that field
+    a = oracle.cache_value(1, 16, True)
+    assert oracle.cache_value_fields(a ^ (1 << 43)) == (1, 16, False, 0)
+    assert oracle.cache_value_fields(a ^ (1 << 40)) == (0, 16, True, 0)
+    with pytest.raises(ValueError):
+        oracle.cache_value(8, 0, True)
+    with pytest.raises(ValueError):
+        oracle.cache_value(0, 1 << 40, True)
