@@ -216,6 +216,13 @@ def run_cuda(args):
     dedup = args.dedup if args.dedup is not None else (0 if w.ids_unique else -1)
     h.set_dedup_mode(dedup)
     info = h.info()
+    cache = None
+    if args.cache_frac > 0:                                    # S8f NEXT #3: compressed GPU cache in front of the store
+        if w.index_span != 1 or not hasattr(w, "hot_ids"):
+            raise SystemExit("bench.py --cache-frac needs a row-gather workload with a hot set (gnn, dlrm)")
+        cache = ibp.Cache(h, int(info.packed_bytes_stored * args.cache_frac), 1, max_entries=max(1024, int(w.n_rows * min(1.0, 2 * args.cache_frac))))
+        cache.insert(w.hot_ids(int(w.n_rows * min(1.0, 2 * args.cache_frac))), stream)
+        cinfo = cache.info()
 
     # ---- ceilings measured on this box, this run
     h2d_ceiling = ibp.ibp_measure_h2d(local, 1 << 30, 8)
@@ -235,13 +242,28 @@ def run_cuda(args):
     ids_dev = [torch.from_numpy(b).cuda() for b in batches]
     out = torch.empty((n_rows_out, w.row_bytes), dtype=torch.uint8, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    link = [h.batch_link_bytes(b) for b in batches]            # (unique ids, stored bytes, byte-aligned bytes)
+    hit_rate = None
+    if cache is not None:                                      # only the misses cross PCIe: account the link bytes over them
+        ent = torch.empty(n, dtype=torch.int64, device="cuda")
+        link, hits = [], []
+        for b, bd in zip(batches, ids_dev):
+            cache.lookup(bd.data_ptr(), n, ent.data_ptr(), stream)
+            torch.cuda.synchronize()
+            miss = ent.cpu().numpy() == -1
+            hits.append(1.0 - miss.mean())
+            link.append(h.batch_link_bytes(b[miss]) if miss.any() else (1, 1, 1))
+        hit_rate = float(np.mean(hits[W:]))
+    else:
+        link = [h.batch_link_bytes(b) for b in batches]        # (unique ids, stored bytes, byte-aligned bytes)
     order_on = w.index_span == 1 and ((args.order == 1) or (args.order is None and info.packed_bytes_stored > (64 << 20) and n >= 4096))
     dedup_on = w.index_span == 1 and (dedup == 1 or (dedup < 0 and n >= 16384))
     launches_per_step = 1 + (3 if order_on else 0) + (2 if dedup_on else 0)
 
     def step(i):
-        h.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
+        if cache is not None:
+            cache.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
+        else:
+            h.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -297,6 +319,8 @@ def run_cuda(args):
     ratio_alg = w.n_rows * w.row_bytes / info.packed_bytes_bytealigned
     batch_ratio_stored = float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(stored_timed))
     eff_roof = min(h2d_ceiling * batch_ratio_stored * (n / np.mean(unique_timed)), hbm_peak)
+    if cache is not None:                                       # all n rows are delivered for the link bytes of the distinct misses
+        eff_roof = min(h2d_ceiling * n * w.row_bytes / float(np.mean(stored_timed)), hbm_peak)
 
     # ---- e2e: pinned host ids -> device -> gather -> pinned host rows, through the C ABI host entry point
     ids_pin = ibp.PinnedBuffer(n * 8)
@@ -304,9 +328,19 @@ def run_cuda(args):
     ids_pin_np = ids_pin.view(np.int64)
     out_pin_np = out_pin.view(np.uint8, (n_rows_out, w.row_bytes))
 
+    ids_stage = torch.empty(n, dtype=torch.int64, device="cuda")
+    ids_pin_t = torch.from_numpy(ids_pin_np)
+    out_pin_t = torch.from_numpy(out_pin_np)
+
     def step_e2e(i):
         ids_pin_np[:] = batches[i]
-        h.gather_decompress_host(ids_pin_np, n, out_pin_np, stream)
+        if cache is not None:                                   # no host entry point for the cache: the same copies through torch
+            ids_stage.copy_(ids_pin_t, non_blocking=True)
+            cache.gather_decompress(ids_stage.data_ptr(), n, out.data_ptr(), stream)
+            out_pin_t.copy_(out, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        else:
+            h.gather_decompress_host(ids_pin_np, n, out_pin_np, stream)
 
     for i in range(min(W, 3)):
         step_e2e(i)
@@ -383,6 +417,9 @@ def run_cuda(args):
                 "codec": "group-strict (tau = 1)" if not info.thresholded else f"thresholded, tau = {thr[0]}/{thr[1]} per group, 4-byte chunks, participation bits; {info.n_rows_raw} of {info.n_rows} rows kept raw",
                 "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
                 "locality_order": bool(order_on), "dedup": bool(dedup_on), "ids_unique_by_construction": bool(w.ids_unique), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
+                "cache": None if cache is None else {"what": "compressed GPU software cache (P:349-357) holding the hottest rows of the sampler, static fill", "capacity_frac_of_packed_store": args.cache_frac,
+                                                      "capacity_MB": round(cinfo.capacity_bytes * 1e-6, 1), "used_MB": round(cinfo.used_bytes * 1e-6, 1), "entries": cinfo.n_entries, "map_MB": round(cinfo.map_bytes * 1e-6, 1),
+                                                      "hit_rate": round(hit_rate, 4), "equivalent_uncompressed_cache_rows": int(cinfo.capacity_bytes // w.row_bytes)},
                 "ratio_stored": round(ratio_stored, 4), "ratio_bytealigned": round(ratio_alg, 4),
                 "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3), "metadata_MB": round(info.metadata_bytes * 1e-6, 2),
                 "build_s": round(t_build, 2), "datagen_s": round(t_gen, 2), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
@@ -408,6 +445,8 @@ def run_cuda(args):
             "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)
+    if cache is not None:
+        cache.destroy()
     h.destroy()
     if world > 1:
         dist.destroy_process_group()
@@ -685,6 +724,7 @@ def main():
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
     ap.add_argument("--phase", default="gather", choices=["gather", "build"], help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device")
+    ap.add_argument("--cache-frac", type=float, default=0.0, help="gnn/dlrm: put a compressed GPU cache of this fraction of the packed store in front of the host store")
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
