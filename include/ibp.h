@@ -183,6 +183,10 @@ ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t
 /* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
 ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
 
+/* Device-visible address of byte 0 of the packed store (what the decode kernels read; for mock-transfer baselines that move
+ * packed bytes without decoding).  BAD_STATE before ibp_upload_metadata or with a pageable store.               */
+ibp_status ibp_store_device_ptr(const ibp_handle* h, const void** dev_ptr);
+
 /* Location of one packed row inside the store (host pointer, stride bytes, variant bits k).  For cross-checks.
  * Thresholded mode: stride = stored bytes incl. padding, k_bits = 8 * the row's byte-aligned size.                 */
 ibp_status ibp_packed_row(const ibp_handle* h, int64_t row, const void** host_ptr, uint32_t* stride_bytes, uint32_t* k_bits);

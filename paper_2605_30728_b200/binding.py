@@ -71,6 +71,7 @@ SIGNATURES = {
     "ibp_decompress_resident": (_int, [_vp, _vp, _i64, _i64, _vp, _vp]),
     "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
+    "ibp_store_device_ptr": (_int, [_vp, C.POINTER(_vp)]),
     "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
     "ibp_row_info": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32), C.POINTER(_int)]),
     "ibp_get_metadata_host": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_u32)]),
@@ -166,6 +167,11 @@ class Handle:
         _check(lib().ibp_packed_row(self._h, row, C.byref(p), C.byref(st), C.byref(k)))
         data = np.ctypeslib.as_array(C.cast(p.value, C.POINTER(C.c_uint8)), (st.value,)).copy() if st.value else np.zeros(0, np.uint8)
         return data, k.value
+
+    def store_device_ptr(self) -> int:
+        p = _vp()
+        _check(lib().ibp_store_device_ptr(self._h, C.byref(p)))
+        return p.value
 
     def row_ptr(self, row) -> int:
         """host address of the packed row inside the store"""

@@ -970,24 +970,55 @@ extern "C" ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_r
     return decode_range(h, h->store_dev + ibp_row_offset(h, (uint64_t)first_row), first_row, n_rows, out_dev, (cudaStream_t)cuda_stream);
 }
 
+// Host-buffer entry point.  Large batches are cut into chunks so that the device->host copy of chunk c (copy engine, PCIe
+// writes) overlaps the gather of chunk c+1 (SM-issued PCIe reads): the two directions of the link work at the same time.
 extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host, int64_t n, void* out_host, void* cuda_stream) {
     ibp_status s = check_ready(h, "ibp_gather_decompress_host");
     if (s != IBP_OK) return s;
     if (n == 0) return IBP_OK;
     if (n < 0 || !row_ids_host || !out_host) { ibp_set_error("ibp_gather_decompress_host: bad argument"); return IBP_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t out_bytes = (size_t)n * h->p.index_span * h->p.row_bytes, id_bytes = ((size_t)n * 8 + 255) / 256 * 256;
+    const size_t id_bytes_row = (size_t)h->p.index_span * h->p.row_bytes;
+    const size_t out_bytes = (size_t)n * id_bytes_row, id_bytes = ((size_t)n * 8 + 255) / 256 * 256;
+    int n_chunks = out_bytes >= (32u << 20) ? 4 : out_bytes >= (8u << 20) ? 2 : 1;
+    if (n < n_chunks) n_chunks = 1;
     uint8_t* buf = nullptr;
     IBP_CUDA(cudaMallocAsync((void**)&buf, id_bytes + out_bytes, st));
     IBP_CUDA(cudaMemcpyAsync(buf, row_ids_host, (size_t)n * 8, cudaMemcpyHostToDevice, st));
-    s = ibp_gather_decompress(h, (const int64_t*)buf, n, buf + id_bytes, cuda_stream);
-    if (s == IBP_OK) {
-        cudaError_t e = cudaMemcpyAsync(out_host, buf + id_bytes, out_bytes, cudaMemcpyDeviceToHost, st);
-        if (e != cudaSuccess) { ibp_set_error("D2H copy failed: %s", cudaGetErrorString(e)); s = IBP_ERR_CUDA; }
+    cudaStream_t copy_st = nullptr;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaError_t e = cudaSuccess;
+    if (n_chunks > 1) {
+        e = cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking);
+        for (int c = 0; c <= n_chunks && e == cudaSuccess; ++c) e = cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming);
     }
+    for (int c = 0; c < n_chunks && s == IBP_OK && e == cudaSuccess; ++c) {
+        const int64_t i0 = n * c / n_chunks, i1 = n * (c + 1) / n_chunks;
+        uint8_t* dout = buf + id_bytes + (size_t)i0 * id_bytes_row;
+        s = ibp_gather_decompress(h, (const int64_t*)buf + i0, i1 - i0, dout, cuda_stream);
+        if (s != IBP_OK) break;
+        cudaStream_t cs = st;
+        if (n_chunks > 1) {
+            e = cudaEventRecord(ev[c], st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(copy_st, ev[c], 0);
+            cs = copy_st;
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync((uint8_t*)out_host + (size_t)i0 * id_bytes_row, dout, (size_t)(i1 - i0) * id_bytes_row, cudaMemcpyDeviceToHost, cs);
+    }
+    if (n_chunks > 1 && e == cudaSuccess && copy_st) {
+        e = cudaEventRecord(ev[n_chunks], copy_st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev[n_chunks], 0);
+    }
+    if (copy_st && (s != IBP_OK || e != cudaSuccess)) cudaStreamSynchronize(copy_st);   // nothing may still write out_host after an error return
     cudaFreeAsync(buf, st);
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (s == IBP_OK && e != cudaSuccess) { ibp_set_error("stream sync failed: %s", cudaGetErrorString(e)); (void)cudaGetLastError(); s = IBP_ERR_CUDA; }
+    const cudaError_t e2 = cudaStreamSynchronize(st);
+    for (int c = 0; c < 5; ++c) if (ev[c]) cudaEventDestroy(ev[c]);
+    if (copy_st) cudaStreamDestroy(copy_st);
+    if (s == IBP_OK && (e != cudaSuccess || e2 != cudaSuccess)) {
+        ibp_set_error("ibp_gather_decompress_host: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+        (void)cudaGetLastError();
+        s = IBP_ERR_CUDA;
+    }
     return s;
 }
 

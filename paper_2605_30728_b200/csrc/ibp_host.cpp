@@ -614,6 +614,13 @@ extern "C" ibp_status ibp_packed_row(const ibp_handle* h, int64_t row, const voi
     return IBP_OK;
 }
 
+extern "C" ibp_status ibp_store_device_ptr(const ibp_handle* h, const void** dev_ptr) {
+    if (!h || !dev_ptr) { ibp_set_error("ibp_store_device_ptr: null argument"); return IBP_ERR_INVALID_ARG; }
+    if (h->device < 0 || !h->store_dev) { ibp_set_error("ibp_store_device_ptr: the store is not attached to a device (upload first; pageable stores never are)"); return IBP_ERR_BAD_STATE; }
+    *dev_ptr = h->store_dev;
+    return IBP_OK;
+}
+
 extern "C" ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes) {
     if (!h || !host_ptr || !nbytes || first_row < 0 || n_rows < 0 || (uint64_t)(first_row + n_rows) > h->p.n_rows) {
         ibp_set_error("ibp_packed_range: bad range");

@@ -238,6 +238,19 @@ def test_uncompressed_baseline_and_host_api():
     out_h = np.zeros((len(ids), 512), np.uint8)
     h.gather_decompress_host(ids, len(ids), out_h, torch.cuda.current_stream().cuda_stream)
     assert np.array_equal(out_h, oracle.gather_plain(X, ids))
+    # large batches are cut into chunks (device->host copy of one overlaps the gather of the next): 2 and 4 chunks, pinned
+    # and pageable destinations, duplicates across chunk borders
+    for n_big in (20_000, 70_001):
+        big = np.random.default_rng(n_big).integers(0, w.n_rows, n_big).astype(np.int64)
+        want = oracle.gather_plain(X, big)
+        out_big = np.zeros((n_big, 512), np.uint8)
+        h.gather_decompress_host(big, n_big, out_big, torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(out_big, want)
+        pout = ibp.PinnedBuffer(n_big * 512)
+        side = torch.cuda.Stream()
+        h.gather_decompress_host(big, n_big, pout.view(np.uint8, (n_big, 512)), side.cuda_stream)
+        assert np.array_equal(pout.view(np.uint8, (n_big, 512)), want)
+        pout.free()
     h.destroy()
     pin.free()
 
