@@ -828,7 +828,8 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
 }
 
 // Random row gather (index_span 1): pre-passes, decode kernel, replication of repeats.  `c` = optional compressed GPU cache.
-static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, cudaStream_t st) {
+static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, cudaStream_t st,
+                              bool allow_dedup = true) {
     if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
     DecodeParams P;
     fill_common(h, P);
@@ -843,7 +844,7 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
         P.cmap_mask = c->map_cap - 1;
         for (int s = 0; s < 8; ++s) P.slab[s] = c->slab_dev[s];
     }
-    const bool dedup = (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
+    const bool dedup = allow_dedup && (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
     // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
     // Essential for the 4 KB-page pinned store, a few percent for the managed-host store -- unless repeated ids are
     // fetched one by one (dedup off on a batch with repeats), where neighbours in the order collide on the same lines.
@@ -980,7 +981,29 @@ extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* r
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t id_bytes_row = (size_t)h->p.index_span * h->p.row_bytes;
     const size_t out_bytes = (size_t)n * id_bytes_row, id_bytes = ((size_t)n * 8 + 255) / 256 * 256;
+    // Pinned, GPU-mapped destination (cudaHostAlloc / cudaHostRegister / ibp_host_alloc): the decode kernel stores the rows
+    // straight into host memory (zero-copy writes), so PCIe reads of packed rows and PCIe writes of decoded rows share one
+    // kernel and nothing is staged in HBM.  Every id is fetched (no de-duplication: its replication pass would read the
+    // output back over the link), which costs nothing because the writes, not the reads, bound this path.
+    {
+        cudaPointerAttributes attr;
+        void* out_dev_alias = nullptr;
+        if (!getenv("IBP_HOST_NO_DIRECT") && cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+            cudaHostGetDevicePointer(&out_dev_alias, out_host, 0) == cudaSuccess && out_dev_alias && !((uintptr_t)out_dev_alias & 15u) && h->store_dev) {
+            int64_t* ids_d = nullptr;
+            IBP_CUDA(cudaMallocAsync((void**)&ids_d, id_bytes, st));
+            IBP_CUDA(cudaMemcpyAsync(ids_d, row_ids_host, (size_t)n * 8, cudaMemcpyHostToDevice, st));
+            if (h->p.index_span == 1) s = gather_rows(h, nullptr, ids_d, n, out_dev_alias, st, false);
+            else s = ibp_gather_decompress(h, ids_d, n, out_dev_alias, cuda_stream);
+            cudaFreeAsync(ids_d, st);
+            const cudaError_t es = cudaStreamSynchronize(st);
+            if (s == IBP_OK && es != cudaSuccess) { ibp_set_error("ibp_gather_decompress_host: %s", cudaGetErrorString(es)); (void)cudaGetLastError(); s = IBP_ERR_CUDA; }
+            return s;
+        }
+        (void)cudaGetLastError();
+    }
     int n_chunks = out_bytes >= (32u << 20) ? 4 : out_bytes >= (8u << 20) ? 2 : 1;
+    if (const char* e = getenv("IBP_HOST_CHUNKS")) n_chunks = std::max(1, std::min(4, atoi(e)));   // tuning experiments only
     if (n < n_chunks) n_chunks = 1;
     uint8_t* buf = nullptr;
     IBP_CUDA(cudaMallocAsync((void**)&buf, id_bytes + out_bytes, st));
