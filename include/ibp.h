@@ -305,6 +305,73 @@ ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, doubl
 /* ibp_measure_d2h: best of `reps` cudaMemcpyAsync D2H copies of nbytes into pinned memory (the ceiling of the GPU-side
  * compressor's store writes), in GB/s.                                                                              */
 ibp_status ibp_measure_d2h(int device, size_t nbytes, int reps, double* gbps);
+/* ibp_measure_random_read: SM-issued zero-copy reads of `span_bytes`-byte spans (16..512, multiple of 16) at uniformly random
+ * span-aligned offsets inside a managed host-resident buffer of `footprint_bytes`; best of `reps`, in spans per second
+ * and GB/s.  This is the ceiling of a random gather of small packed rows: above a few hundred MB of footprint it is set
+ * by address translation on the host path, not by the link.                                   */
+ibp_status ibp_measure_random_read(int device, size_t footprint_bytes, uint32_t span_bytes, int reps, double* spans_per_s,
+                                   double* gbps);
+
+/* -- Mask-quality tools: the paper's preprocessing counters exposed, so that Mask/Bitval can be
+ * built for any threshold from one counting pass (tau sweep), from a sample of the rows, evaluated
+ * under any chunk size (Fig. 13), and per cluster of a bit-similarity k-means.  All arrays named
+ * *_dev live on the current device; calls are asynchronous on the stream unless stated.  Everything is integer work and
+ * agrees exactly with oracle/mask_tools.py.                                                                          */
+enum { IBP_GROUP_MAP = 2 }; /* group(id) = row_group_dev[id]: an explicit row -> group map (clusters)               */
+
+typedef struct {
+    uint32_t struct_size;          /* = sizeof(ibp_table_desc)                                                       */
+    uint32_t row_bytes;            /* multiple of 4                                                                  */
+    uint64_t n_rows;
+    uint32_t group_kind;           /* IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED or IBP_GROUP_MAP                          */
+    uint32_t group_param;          /* G or S; ignored for MAP                                                        */
+    uint64_t n_groups;             /* MAP: number of groups; BLOCKED/STRIDED: 0 or the derived count                 */
+    const uint32_t* row_group_dev; /* MAP: n_rows entries, each < n_groups; else NULL                                */
+} ibp_table_desc;
+
+/* Number of groups the descriptor implies (ceil(n_rows/G), min(S, n_rows), or n_groups).                            */
+ibp_status ibp_table_groups(const ibp_table_desc* t, uint64_t* n_groups);
+
+/* P:229 "for each set bit in each input tensor, we increment the corresponding counter".
+ * counts_dev[g*8*row_bytes + p] += number of listed rows of group g whose bit p is set; group_n_dev[g] += rows listed.
+ * Rows listed: sample_ids_dev[0..n_sample) (repeats count twice; consecutive ids of one group are cheapest), or every
+ * row when sample_ids_dev is NULL.  Both outputs are ACCUMULATED into: the caller zeroes them (cudaMemsetAsync) first. */
+ibp_status ibp_bit_counts_device(const void* rows_dev, const ibp_table_desc* t, const int64_t* sample_ids_dev,
+                                 int64_t n_sample, uint32_t* counts_dev, uint32_t* group_n_dev, void* cuda_stream);
+
+/* P:231 with reading R2: T = ceil(tau N_g); Mask bit = 1 and Bitval bit = 1 where count >= T; Mask = 1, Bitval = 0 where
+ * count <= N_g - T; else both 0.  A group with N_g = 0 gets Mask = 0.  mask_dev / bitval_dev: n_groups x row_bytes each;
+ * kbits_dev (may be NULL): popcount(~Mask) per group.  INVALID_ARG unless 1/2 < tau <= 1.                           */
+ibp_status ibp_masks_from_counts_device(const uint32_t* counts_dev, const uint32_t* group_n_dev, uint64_t n_groups,
+                                        uint32_t row_bytes, uint32_t tau_num, uint32_t tau_den, void* mask_dev,
+                                        void* bitval_dev, uint32_t* kbits_dev, void* cuda_stream);
+
+/* getCompressSize (Fig. 3 lines 1-19 = P:243-271) of every row under its group's Mask/Bitval with chunks of chunk_bytes
+ * in {1, 2, 4, 8} (row_bytes must be a multiple): a chunk participates iff (chunk AND Mask) == Bitval; bitsSaved = sum of
+ * popcount(Mask) over participating chunks; bytesSaved = floor((bitsSaved - row_bytes/chunk_bytes)/8); <= 0 -> the row
+ * stays raw.  sizes_dev (may be NULL): stored bytes per row.  totals_dev[0] += sum of the sizes, totals_dev[1] +=
+ * rows kept raw (caller zeroes).                                                                                    */
+ibp_status ibp_compressed_size_device(const void* rows_dev, const ibp_table_desc* t, const void* mask_dev,
+                                      const void* bitval_dev, uint32_t chunk_bytes, uint32_t* sizes_dev,
+                                      uint64_t* totals_dev, void* cuda_stream);
+
+/* One counting pass, then every (tau, chunk size) pair: total_bytes_host[i*n_cs + j] and raw_rows_host[i*n_cs + j] for
+ * taus_host[2i] / taus_host[2i+1] and chunk_bytes_host[j].  Masks come from the listed sample (NULL = all rows), sizes are
+ * evaluated on ALL rows.  Synchronous.                                                                  */
+ibp_status ibp_mask_sweep_device(const void* rows_dev, const ibp_table_desc* t, const int64_t* sample_ids_dev,
+                                 int64_t n_sample, const uint32_t* taus_host, uint32_t n_tau,
+                                 const uint32_t* chunk_bytes_host, uint32_t n_cs, uint64_t* total_bytes_host,
+                                 uint64_t* raw_rows_host, void* cuda_stream);
+
+/* Bit-similarity k-means (reading R25 in DESIGN.md): Lloyd iterations with the Hamming distance between a row and
+ * a centroid bit vector; a centroid bit is the strict majority of its cluster's rows (tie -> 0); assignment ties go to
+ * the lowest cluster index; an empty cluster keeps its centroid.  Initial centroids = rows init_ids_dev[0..k).
+ * assign_dev: n_rows entries, the assignment of the LAST iteration; centroids_dev: k x row_bytes, after the last update;
+ * cost_dev (may be NULL): iters entries, summed distance of every row to its assigned centroid in that iteration.
+ * row_bytes <= 4096.  Allocates workspaces on the stream (stream-ordered).                                          */
+ibp_status ibp_kmeans_bits_device(const void* rows_dev, uint64_t n_rows, uint32_t row_bytes, uint32_t k,
+                                  const int64_t* init_ids_dev, uint32_t iters, uint32_t* assign_dev, void* centroids_dev,
+                                  uint64_t* cost_dev, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -16,7 +16,7 @@ from ._build import build_library
 IBP_OK = 0
 STATUS = {0: "IBP_OK", 1: "IBP_ERR_INVALID_ARG", 2: "IBP_ERR_OUT_OF_MEMORY", 3: "IBP_ERR_CUDA", 4: "IBP_ERR_BAD_STATE",
           5: "IBP_ERR_UNSUPPORTED"}
-IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED = 0, 1
+IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED, IBP_GROUP_MAP = 0, 1, 2
 IBP_FLAG_PAGEABLE_STORE = 1
 IBP_FLAG_HOSTALLOC_STORE = 2
 IBP_STORE_PAGEABLE, IBP_STORE_PINNED, IBP_STORE_MANAGED_HOST = 0, 1, 2
@@ -55,6 +55,11 @@ class ibp_build_stats(C.Structure):
 class ibp_cache_info(C.Structure):
     _fields_ = [("capacity_bytes", C.c_uint64), ("used_bytes", C.c_uint64), ("n_entries", C.c_uint64), ("max_entries", C.c_uint64),
                 ("map_bytes", C.c_uint64), ("n_slabs", C.c_uint32), ("reserved", C.c_uint32), ("slab_bytes", C.c_uint64)]
+
+
+class ibp_table_desc(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("row_bytes", C.c_uint32), ("n_rows", C.c_uint64), ("group_kind", C.c_uint32),
+                ("group_param", C.c_uint32), ("n_groups", C.c_uint64), ("row_group_dev", C.c_void_p)]
 
 
 IBP_CACHE_MISS = 0xFFFFFFFFFFFFFFFF
@@ -103,6 +108,13 @@ SIGNATURES = {
     "ibp_measure_h2d": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
     "ibp_measure_zero_copy_read": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
     "ibp_measure_d2h": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
+    "ibp_measure_random_read": (_int, [_int, C.c_size_t, _u32, _int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "ibp_table_groups": (_int, [C.POINTER(ibp_table_desc), C.POINTER(_u64)]),
+    "ibp_bit_counts_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _i64, _vp, _vp, _vp]),
+    "ibp_masks_from_counts_device": (_int, [_vp, _vp, _u64, _u32, _u32, _u32, _vp, _vp, _vp, _vp]),
+    "ibp_compressed_size_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _vp, _u32, _vp, _vp, _vp]),
+    "ibp_mask_sweep_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _i64, _vp, _u32, _vp, _u32, _vp, _vp, _vp]),
+    "ibp_kmeans_bits_device": (_int, [_vp, _u64, _u32, _u32, _vp, _u32, _vp, _vp, _vp, _vp]),
 }
 
 _lib = None
@@ -371,6 +383,55 @@ def ibp_measure_d2h(device=0, nbytes=1 << 30, reps=10) -> float:
     g = C.c_double()
     _check(lib().ibp_measure_d2h(device, nbytes, reps, C.byref(g)))
     return g.value
+
+
+def ibp_measure_random_read(device=0, footprint_bytes=4 << 30, span_bytes=128, reps=3):
+    """(spans per second, GB/s) of random span-aligned zero-copy reads from managed host-resident memory."""
+    r, g = C.c_double(), C.c_double()
+    _check(lib().ibp_measure_random_read(device, footprint_bytes, span_bytes, reps, C.byref(r), C.byref(g)))
+    return r.value, g.value
+
+
+# ---- mask-quality tools (SURVEY 8(f) NEXT #4): marshalling only, the work is in csrc/ibp_analysis.cu
+def table_desc(n_rows, row_bytes, group_kind, group_param=0, n_groups=0, row_group_dev=None) -> ibp_table_desc:
+    return ibp_table_desc(C.sizeof(ibp_table_desc), row_bytes, n_rows, group_kind, group_param, n_groups, _ptr(row_group_dev))
+
+
+def ibp_table_groups(t: ibp_table_desc) -> int:
+    n = _u64()
+    _check(lib().ibp_table_groups(C.byref(t), C.byref(n)))
+    return n.value
+
+
+def ibp_bit_counts_device(rows_dev, t, sample_ids_dev, n_sample, counts_dev, group_n_dev, stream=None):
+    _check(lib().ibp_bit_counts_device(_ptr(rows_dev), C.byref(t), _ptr(sample_ids_dev), n_sample, _ptr(counts_dev), _ptr(group_n_dev), stream))
+
+
+def ibp_masks_from_counts_device(counts_dev, group_n_dev, n_groups, row_bytes, tau_num, tau_den, mask_dev, bitval_dev, kbits_dev=None,
+                                 stream=None):
+    _check(lib().ibp_masks_from_counts_device(_ptr(counts_dev), _ptr(group_n_dev), n_groups, row_bytes, tau_num, tau_den, _ptr(mask_dev),
+                                              _ptr(bitval_dev), _ptr(kbits_dev), stream))
+
+
+def ibp_compressed_size_device(rows_dev, t, mask_dev, bitval_dev, chunk_bytes, sizes_dev, totals_dev, stream=None):
+    _check(lib().ibp_compressed_size_device(_ptr(rows_dev), C.byref(t), _ptr(mask_dev), _ptr(bitval_dev), chunk_bytes, _ptr(sizes_dev),
+                                            _ptr(totals_dev), stream))
+
+
+def ibp_mask_sweep_device(rows_dev, t, sample_ids_dev, n_sample, taus, chunk_bytes, stream=None):
+    """taus: [(num, den), ...]; chunk_bytes: [1|2|4|8, ...] -> (total_bytes[n_tau][n_cs], raw_rows[n_tau][n_cs]) as numpy uint64."""
+    ta = np.ascontiguousarray(np.asarray(taus, dtype=np.uint32).reshape(-1, 2))
+    cs = np.ascontiguousarray(np.asarray(chunk_bytes, dtype=np.uint32))
+    tot = np.zeros((len(ta), len(cs)), np.uint64)
+    raw = np.zeros((len(ta), len(cs)), np.uint64)
+    _check(lib().ibp_mask_sweep_device(_ptr(rows_dev), C.byref(t), _ptr(sample_ids_dev), n_sample, ta.ctypes.data, len(ta), cs.ctypes.data,
+                                       len(cs), tot.ctypes.data, raw.ctypes.data, stream))
+    return tot, raw
+
+
+def ibp_kmeans_bits_device(rows_dev, n_rows, row_bytes, k, init_ids_dev, iters, assign_dev, centroids_dev, cost_dev=None, stream=None):
+    _check(lib().ibp_kmeans_bits_device(_ptr(rows_dev), n_rows, row_bytes, k, _ptr(init_ids_dev), iters, _ptr(assign_dev),
+                                        _ptr(centroids_dev), _ptr(cost_dev), stream))
 
 
 def ibp_version() -> str:

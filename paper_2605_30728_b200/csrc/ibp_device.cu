@@ -1201,6 +1201,64 @@ extern "C" ibp_status ibp_measure_h2d(int device, size_t nbytes, int reps, doubl
 extern "C" ibp_status ibp_measure_zero_copy_read(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, true); }
 extern "C" ibp_status ibp_measure_d2h(int device, size_t nbytes, int reps, double* gbps) { return measure_link(device, nbytes, reps, gbps, false, true); }
 
+// Random span reads: `lanes` = span_bytes/16 consecutive lanes read one span at a hashed, span-aligned offset.
+__global__ void ibp_random_read_kernel(const uint4* __restrict__ src, uint64_t n_spans_buf, uint32_t reads_per_group, uint32_t lanes, uint64_t seed,
+                                       unsigned* sink) {
+    const uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x, grp = t / lanes;
+    const uint32_t sub = (uint32_t)(t % lanes);
+    unsigned acc = 0;
+    for (uint32_t i = 0; i < reads_per_group; ++i) {
+        uint64_t z = (grp * 0x100000001B3ull + i) ^ seed;
+        z += 0x9E3779B97F4A7C15ull; z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+        const uint64_t s = z % n_spans_buf;
+        uint4 v;
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(src + s * lanes + sub));
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    if (acc == 0x9E3779B9u) *sink = acc;
+}
+
+extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes, uint32_t span_bytes, int reps, double* spans_per_s, double* gbps) {
+    if (!spans_per_s || !gbps || footprint_bytes < (1u << 20) || reps < 1 || span_bytes < 16 || span_bytes > 512 || span_bytes % 16) {
+        ibp_set_error("ibp_measure_random_read: bad argument"); return IBP_ERR_INVALID_ARG;
+    }
+    IBP_CUDA(cudaSetDevice(device));
+    void* p = nullptr;
+    ibp_status rc = ibp_host_alloc_managed(footprint_bytes, device, &p);
+    if (rc != IBP_OK) return rc;
+    {   // first touch on the host, in parallel
+        const int64_t nchunk = (int64_t)((footprint_bytes + (1u << 22) - 1) >> 22);
+#pragma omp parallel for schedule(static)
+        for (int64_t c = 0; c < nchunk; ++c) memset((char*)p + ((size_t)c << 22), 0x5A, std::min<size_t>(1u << 22, footprint_bytes - ((size_t)c << 22)));
+    }
+    unsigned* sink = nullptr;
+    cudaEvent_t a, b;
+    float best = 1e30f;
+    const uint32_t lanes = span_bytes / 16, rpg = 64;
+    const int grid = 148 * 8, block = 256;
+    const double n_reads = (double)((uint64_t)grid * block / lanes) * rpg;
+    if (cudaMalloc((void**)&sink, 4) != cudaSuccess || cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+        ibp_set_error("ibp_measure_random_read: allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        rc = IBP_ERR_CUDA;
+    } else {
+        for (int it = 0; it < reps + 1; ++it) {
+            cudaEventRecord(a, 0);
+            ibp_random_read_kernel<<<grid, block>>>((const uint4*)p, footprint_bytes / span_bytes, rpg, lanes, 0x1234u + it, sink);
+            cudaEventRecord(b, 0);
+            if (cudaEventSynchronize(b) != cudaSuccess) { ibp_set_error("ibp_measure_random_read: %s", cudaGetErrorString(cudaGetLastError())); rc = IBP_ERR_CUDA; break; }
+            float ms = 0;
+            cudaEventElapsedTime(&ms, a, b);
+            if (it) best = std::min(best, ms);
+        }
+        cudaEventDestroy(a);
+        cudaEventDestroy(b);
+    }
+    if (sink) cudaFree(sink);
+    ibp_host_free_managed(p);
+    if (rc == IBP_OK) { *spans_per_s = n_reads / (best * 1e-3); *gbps = *spans_per_s * span_bytes * 1e-9; }
+    return rc;
+}
+
 // 1 = de-duplicate the ids of a random gather before fetching; 0 = fetch every id (the caller knows the ids are distinct);
 // -1 = automatic (default): on for batches of >= 16384 ids.
 extern "C" ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode) {
