@@ -1,10 +1,11 @@
 // ibp_analysis.cu -- mask-quality tools of libibp.so (sm_100a): SURVEY 8(f) NEXT #4.
 //
-//   ibp_count_kernel      P:229  per-bit counters of the listed rows.  A warp takes a run of list positions; lane l owns the
-//                                words l, l+32, ... of the row; the 32 counters of a word are BIT-SLICED over NP planes held
-//                                in registers (plane j = bit j of the 32 running counts), a row enters by a ripple add of
-//                                2 logic ops per plane; planes are unpacked and added to the global counters with atomicAdd
-//                                only when the run's group changes or the run ends.
+//   ibp_count_kernel      P:229  per-bit counters of the listed rows.  A warp takes a run of up to 4092 list positions; lane l
+//                                owns W consecutive words of the row (one vector load per row); the 32 counters of a word are
+//                                BIT-SLICED over 12 planes held in registers (plane j = bit j of the 32 running counts); four
+//                                rows enter at a time through two carry-save adders (lop3 xor3 / maj3) and a carry ripple;
+//                                planes are unpacked and added to the global counters with atomicAdd only when the run's
+//                                group changes or the run ends.
 //   ibp_masks_kernel      P:231  Mask/Bitval from the counters for T = ceil(tau N_g): re-run per tau of the sweep.
 //   ibp_csize_kernel      Fig. 3 lines 1-19  getCompressSize per row for chunk sizes 1/2/4/8 bytes: warp per row,
 //                                lane per 8-byte unit, byte-wise match flags by SIMD-in-register tests, warp sum.
@@ -15,6 +16,7 @@
 // Integer arithmetic only; results do not depend on the launch shape (sums of integers).  Checked against
 // oracle/mask_tools.py in tests/test_gpu_mask_tools.py.
 #include <algorithm>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <vector>
@@ -47,8 +49,20 @@ __device__ __forceinline__ uint64_t table_item(const TableDev& T, uint64_t pos) 
     return pos;
 }
 
-constexpr int COUNT_RUN = 96;   // list positions per warp run
-constexpr int COUNT_NP = 7;     // planes: a run adds at most 96 < 2^7 rows to a counter before it is flushed
+constexpr int COUNT_NP = 12;               // planes: a run adds at most 2^12 - 1 rows to a counter before it is flushed
+constexpr uint32_t COUNT_RUN_MAX = 4092;   // multiple of 4 below 2^12
+constexpr uint32_t COUNT_RUN_MIN = 96;
+
+__device__ __forceinline__ uint32_t axor3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t amaj3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE8;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
 
 template <int NP>
 __device__ __forceinline__ void flush_planes(uint32_t* pl, uint32_t* dst /* 32 counters of this word */) {
@@ -67,43 +81,119 @@ __device__ __forceinline__ void flush_planes(uint32_t* pl, uint32_t* dst /* 32 c
     for (int p = 0; p < NP; ++p) pl[p] = 0;
 }
 
-__global__ void __launch_bounds__(256) ibp_count_kernel(const TableDev T, uint32_t* __restrict__ counts, uint32_t* __restrict__ group_n) {
+// A warp takes a run of `run_len` list positions; lane l owns W consecutive words of each 32*W-word pass (one vector load per
+// row).  Positions are taken four at a time: when the four rows belong to the run's current group (the common case: sorted
+// lists, blocked groups, one global group) they enter through two carry-save adders; otherwise one by one with a flush at
+// every group change.
+template <int W>
+__global__ void __launch_bounds__(256) ibp_count_kernel(const TableDev T, uint32_t run_len, uint32_t* __restrict__ counts, uint32_t* __restrict__ group_n) {
     const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
-    const uint64_t n_runs = (T.n_list + COUNT_RUN - 1) / COUNT_RUN;
-    const uint32_t n_pass = (T.nw + 31) / 32;
+    const uint64_t n_runs = (T.n_list + run_len - 1) / run_len;
+    const uint32_t n_pass = (T.nw + 32 * W - 1) / (32 * W);
     const uint64_t nbits = 32ull * T.nw;
     for (uint64_t run = (uint64_t)blockIdx.x * wpc + (threadIdx.x >> 5); run < n_runs; run += (uint64_t)gridDim.x * wpc) {
-        const uint64_t p0 = run * COUNT_RUN, p1 = min(T.n_list, p0 + COUNT_RUN);
+        const uint64_t p0 = run * run_len, p1 = min(T.n_list, p0 + run_len);
         for (uint32_t pass = 0; pass < n_pass; ++pass) {
-            const uint32_t w = pass * 32u + lane;
-            const bool active = w < T.nw;
-            uint32_t pl[COUNT_NP];
+            const uint32_t w0 = (pass * 32u + lane) * W;
+            const bool active = w0 < T.nw;
+            uint32_t pl[COUNT_NP][W];
 #pragma unroll
-            for (int p = 0; p < COUNT_NP; ++p) pl[p] = 0;
+            for (int p = 0; p < COUNT_NP; ++p)
+#pragma unroll
+                for (int q = 0; q < W; ++q) pl[p][q] = 0;
             uint64_t cur_g = ~0ull;
             uint32_t cur_n = 0;
-            for (uint64_t pos = p0; pos < p1; ++pos) {
-                const uint64_t row = table_item(T, pos);
-                if (row == ~0ull) continue;
-                const uint64_t g = table_group(T, row);
-                if (g != cur_g) {
-                    if (cur_g != ~0ull) {
-                        if (active) flush_planes<COUNT_NP>(pl, counts + cur_g * nbits + 32ull * w);
-                        if (pass == 0 && lane == 0) atomicAdd(group_n + cur_g, cur_n);
-                    }
-                    cur_g = g; cur_n = 0;
-                }
-                cur_n += 1;
+            auto flush = [&]() {
+                if (cur_g == ~0ull) return;
                 if (active) {
-                    uint32_t c = __ldg(T.rows + row * T.nw + w);
 #pragma unroll
-                    for (int p = 0; p < COUNT_NP; ++p) { const uint32_t t = pl[p]; pl[p] = t ^ c; c &= t; }
+                    for (int q = 0; q < W; ++q) {
+                        uint32_t col[COUNT_NP];
+#pragma unroll
+                        for (int p = 0; p < COUNT_NP; ++p) col[p] = pl[p][q];
+                        flush_planes<COUNT_NP>(col, counts + cur_g * nbits + 32ull * (w0 + q));
+#pragma unroll
+                        for (int p = 0; p < COUNT_NP; ++p) pl[p][q] = 0;
+                    }
+                }
+                if (pass == 0 && lane == 0) atomicAdd(group_n + cur_g, cur_n);
+            };
+            auto add4 = [&](uint64_t r0, uint64_t r1, uint64_t r2, uint64_t r3) {
+                uint32_t x0[W], x1[W], x2[W], x3[W];
+                VecIO<W>::ld(T.rows + r0 * T.nw + w0, x0);
+                VecIO<W>::ld(T.rows + r1 * T.nw + w0, x1);
+                VecIO<W>::ld(T.rows + r2 * T.nw + w0, x2);
+                VecIO<W>::ld(T.rows + r3 * T.nw + w0, x3);
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    const uint32_t s1 = axor3(pl[0][q], x0[q], x1[q]), c1 = amaj3(pl[0][q], x0[q], x1[q]);
+                    const uint32_t s2 = axor3(s1, x2[q], x3[q]), c2 = amaj3(s1, x2[q], x3[q]);
+                    pl[0][q] = s2;
+                    uint32_t c = amaj3(pl[1][q], c1, c2);
+                    pl[1][q] = axor3(pl[1][q], c1, c2);
+#pragma unroll
+                    for (int p = 2; p < COUNT_NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
+                }
+            };
+            auto add1 = [&](uint64_t r0) {
+                uint32_t x[W];
+                VecIO<W>::ld(T.rows + r0 * T.nw + w0, x);
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    uint32_t c = x[q];
+#pragma unroll
+                    for (int p = 0; p < COUNT_NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
+                }
+            };
+            uint64_t pos = p0;
+            if (!T.list && T.kind != IBP_GROUP_MAP) {
+                // every row, blocked or strided groups: segments of one group with row ids in arithmetic progression
+                while (pos < p1) {
+                    uint64_t g, seg_end, row, step;
+                    if (T.kind == IBP_GROUP_BLOCKED) {
+                        g = pos / T.param; seg_end = min(p1, (g + 1) * (uint64_t)T.param); row = pos; step = 1;
+                    } else {
+                        g = pos / T.q_strided;
+                        const uint64_t j = pos - g * T.q_strided, cnt = (T.n_rows - g + T.param - 1) / T.param;
+                        if (j >= cnt) { pos = (g + 1) * T.q_strided; continue; }
+                        seg_end = min(p1, g * T.q_strided + cnt); row = j * T.param + g; step = T.param;
+                    }
+                    const uint64_t n_seg = seg_end - pos;
+                    cur_g = g; cur_n = (uint32_t)n_seg;
+                    if (active) {
+                        uint64_t i = 0;
+                        for (; i + 4 <= n_seg; i += 4, row += 4 * step) add4(row, row + step, row + 2 * step, row + 3 * step);
+                        for (; i < n_seg; ++i, row += step) add1(row);
+                    }
+                    flush();
+                    cur_g = ~0ull;
+                    pos = seg_end;
+                }
+            } else {
+                while (pos < p1) {
+                    uint64_t r[4], g[4];
+                    const int m = (int)min((uint64_t)4, p1 - pos);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        r[i] = i < m ? table_item(T, pos + i) : ~0ull;
+                        g[i] = r[i] != ~0ull ? table_group(T, r[i]) : ~0ull;
+                    }
+                    if (cur_g == ~0ull && g[0] != ~0ull) { cur_g = g[0]; cur_n = 0; }
+                    if (m == 4 && g[0] == cur_g && g[1] == cur_g && g[2] == cur_g && g[3] == cur_g) {
+                        cur_n += 4;
+                        if (active) add4(r[0], r[1], r[2], r[3]);
+                    } else {
+                        for (int i = 0; i < m; ++i) {
+                            if (r[i] == ~0ull) continue;
+                            if (g[i] != cur_g) { flush(); cur_g = g[i]; cur_n = 0; }
+                            cur_n += 1;
+                            if (active) add1(r[i]);
+                        }
+                    }
+                    pos += m;
                 }
             }
-            if (cur_g != ~0ull) {
-                if (active) flush_planes<COUNT_NP>(pl, counts + cur_g * nbits + 32ull * w);
-                if (pass == 0 && lane == 0) atomicAdd(group_n + cur_g, cur_n);
-            }
+            flush();
         }
     }
 }
@@ -190,6 +280,74 @@ __global__ void __launch_bounds__(256) ibp_csize_kernel(const TableDev T, const 
             sum_sizes += size;
             sum_raw += bytes_saved ? 0 : 1;
         }
+    }
+    if (lane == 0 && (sum_sizes | sum_raw)) {
+        atomicAdd(totals, sum_sizes);
+        atomicAdd(totals + 1, sum_raw);
+    }
+}
+
+// Fast variant for rows that are a multiple of 8 bytes (8-byte aligned base): a warp takes FOUR consecutive rows per step, all
+// their loads are issued before the first use, Mask/Bitval are loaded once when the four rows share a group, and the four
+// sums are reduced together.
+template <int CS>
+__global__ void __launch_bounds__(256) ibp_csize4_kernel(const TableDev T, const uint32_t* __restrict__ mask, const uint32_t* __restrict__ bitval,
+                                                         uint32_t* __restrict__ sizes, unsigned long long* __restrict__ totals) {
+    const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    const uint32_t row_bytes = 4u * T.nw, n_units = T.nw / 2, n_chunks = row_bytes / CS;
+    const uint64_t n_batches = (T.n_rows + 3) / 4;
+    unsigned long long sum_sizes = 0, sum_raw = 0;
+    for (uint64_t bt = (uint64_t)blockIdx.x * wpc + (threadIdx.x >> 5); bt < n_batches; bt += (uint64_t)gridDim.x * wpc) {
+        const uint64_t row0 = bt * 4;
+        const int m = (int)min((uint64_t)4, T.n_rows - row0);
+        uint64_t g[4];
+        bool same;
+        if (T.kind == IBP_GROUP_BLOCKED) {      // one division per step: the four rows usually lie in one group
+            g[0] = row0 / T.param;
+            same = row0 + 3 < (g[0] + 1) * (uint64_t)T.param;
+#pragma unroll
+            for (int i = 1; i < 4; ++i) g[i] = same ? g[0] : (row0 + (i < m ? i : 0)) / T.param;
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) g[i] = table_group(T, row0 + (i < m ? i : 0));
+            same = g[0] == g[1] && g[0] == g[2] && g[0] == g[3];
+        }
+        uint32_t saved[4] = {0, 0, 0, 0};
+        for (uint32_t u = lane; u < n_units; u += 32) {
+            uint2 x[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) x[i] = __ldg((const uint2*)(T.rows + (row0 + (i < m ? i : 0)) * T.nw) + u);
+            if (same) {
+                const uint2 mm = __ldg((const uint2*)(mask + g[0] * T.nw) + u), bb = __ldg((const uint2*)(bitval + g[0] * T.nw) + u);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) saved[i] += saved_bits_unit<CS>((x[i].x & mm.x) ^ bb.x, mm.x, (x[i].y & mm.y) ^ bb.y, mm.y);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const uint2 mm = __ldg((const uint2*)(mask + g[i] * T.nw) + u), bb = __ldg((const uint2*)(bitval + g[i] * T.nw) + u);
+                    saved[i] += saved_bits_unit<CS>((x[i].x & mm.x) ^ bb.x, mm.x, (x[i].y & mm.y) ^ bb.y, mm.y);
+                }
+            }
+        }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) saved[i] += __shfl_xor_sync(0xFFFFFFFFu, saved[i], d);
+        }
+        if (lane < m) {
+            const uint32_t sv = lane == 0 ? saved[0] : lane == 1 ? saved[1] : lane == 2 ? saved[2] : saved[3];
+            const int diff = (int)sv - (int)n_chunks;
+            const uint32_t bytes_saved = diff > 0 ? (uint32_t)diff / 8u : 0u;
+            const uint32_t size = bytes_saved ? row_bytes - bytes_saved : row_bytes;
+            if (sizes) sizes[row0 + lane] = size;
+            sum_sizes += size;
+            sum_raw += bytes_saved ? 0 : 1;
+        }
+    }
+#pragma unroll
+    for (int d = 2; d; d >>= 1) {     // lanes 0..3 hold the partial sums
+        sum_sizes += __shfl_xor_sync(0xFFFFFFFFu, sum_sizes, d);
+        sum_raw += __shfl_xor_sync(0xFFFFFFFFu, sum_raw, d);
     }
     if (lane == 0 && (sum_sizes | sum_raw)) {
         atomicAdd(totals, sum_sizes);
@@ -334,8 +492,17 @@ static ibp_status launch_counts(TableDev T, const int64_t* sample_ids_dev, int64
     if (sample_ids_dev) { T.list = sample_ids_dev; T.n_list = (uint64_t)n_sample; }
     else if (T.kind == IBP_GROUP_STRIDED) { T.q_strided = (T.n_rows + T.param - 1) / T.param; T.n_list = T.q_strided * std::min<uint64_t>(T.param, T.n_rows); }
     if (T.n_list == 0) return IBP_OK;
-    const uint64_t n_runs = (T.n_list + COUNT_RUN - 1) / COUNT_RUN;
-    ibp_count_kernel<<<analysis_grid(n_runs), 256, 0, st>>>(T, counts_dev, group_n_dev);
+    // run length: enough runs to fill the machine (8 warps x 8 CTAs per SM), each as long as the planes allow, so that the
+    // atomic flushes (32 per word per run and group) stay rare
+    const int grid_full = analysis_grid(~0ull >> 8);
+    uint64_t run = ((T.n_list + (uint64_t)grid_full * 8 - 1) / ((uint64_t)grid_full * 8) + 3) / 4 * 4;   // ceil: no second, partial round of runs
+    run = std::max<uint64_t>(COUNT_RUN_MIN, std::min<uint64_t>(COUNT_RUN_MAX, run));
+    const uint64_t n_runs = (T.n_list + run - 1) / run;
+    const int grid = analysis_grid(n_runs);
+    const bool a16 = (uintptr_t)T.rows % 16 == 0, a8 = (uintptr_t)T.rows % 8 == 0;
+    if (T.nw % 4 == 0 && a16) ibp_count_kernel<4><<<grid, 256, 0, st>>>(T, (uint32_t)run, counts_dev, group_n_dev);
+    else if (T.nw % 2 == 0 && a8) ibp_count_kernel<2><<<grid, 256, 0, st>>>(T, (uint32_t)run, counts_dev, group_n_dev);
+    else ibp_count_kernel<1><<<grid, 256, 0, st>>>(T, (uint32_t)run, counts_dev, group_n_dev);
     IBP_CUDA(cudaGetLastError());
     return IBP_OK;
 }
@@ -375,15 +542,19 @@ extern "C" ibp_status ibp_masks_from_counts_device(const uint32_t* counts_dev, c
 
 static ibp_status launch_csize(const TableDev& T, const void* mask_dev, const void* bitval_dev, uint32_t cs, uint32_t* sizes_dev, uint64_t* totals_dev,
                                cudaStream_t st) {
-    const int grid = analysis_grid(T.n_rows);
     const uint32_t* m = (const uint32_t*)mask_dev; const uint32_t* b = (const uint32_t*)bitval_dev;
     unsigned long long* tot = (unsigned long long*)totals_dev;
+    const bool fast = T.nw % 2 == 0 && ((uintptr_t)T.rows | (uintptr_t)m | (uintptr_t)b) % 8 == 0;
+    const int grid = analysis_grid(fast ? (T.n_rows + 3) / 4 : T.n_rows);
+#define IBP_CSIZE(CS_) \
+    do { if (fast) ibp_csize4_kernel<CS_><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); else ibp_csize_kernel<CS_><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); } while (0)
     switch (cs) {
-        case 1: ibp_csize_kernel<1><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); break;
-        case 2: ibp_csize_kernel<2><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); break;
-        case 4: ibp_csize_kernel<4><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); break;
-        default: ibp_csize_kernel<8><<<grid, 256, 0, st>>>(T, m, b, sizes_dev, tot); break;
+        case 1: IBP_CSIZE(1); break;
+        case 2: IBP_CSIZE(2); break;
+        case 4: IBP_CSIZE(4); break;
+        default: IBP_CSIZE(8); break;
     }
+#undef IBP_CSIZE
     IBP_CUDA(cudaGetLastError());
     return IBP_OK;
 }
