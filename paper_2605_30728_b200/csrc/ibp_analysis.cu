@@ -1,9 +1,10 @@
 // ibp_analysis.cu -- mask-quality tools of libibp.so (sm_100a): SURVEY 8(f) NEXT #4.
 //
-//   ibp_count_kernel      P:229  per-bit counters of the listed rows.  A warp takes a run of up to 4092 list positions; lane l
+//   ibp_count_kernel      P:229  per-bit counters of the listed rows.  A warp takes a run of up to 1016 list positions; lane l
 //                                owns W consecutive words of the row (one vector load per row); the 32 counters of a word are
-//                                BIT-SLICED over 12 planes held in registers (plane j = bit j of the 32 running counts); four
-//                                rows enter at a time through two carry-save adders (lop3 xor3 / maj3) and a carry ripple;
+//                                BIT-SLICED over 10 planes held in registers (plane j = bit j of the 32 running counts); eight
+//                                rows are loaded at a time and enter four by four through two carry-save adders (lop3 xor3 /
+//                                maj3) and a carry ripple;
 //                                planes are unpacked and added to the global counters with atomicAdd only when the run's
 //                                group changes or the run ends.
 //   ibp_masks_kernel      P:231  Mask/Bitval from the counters for T = ceil(tau N_g): re-run per tau of the sweep.
@@ -49,8 +50,8 @@ __device__ __forceinline__ uint64_t table_item(const TableDev& T, uint64_t pos) 
     return pos;
 }
 
-constexpr int COUNT_NP = 12;               // planes: a run adds at most 2^12 - 1 rows to a counter before it is flushed
-constexpr uint32_t COUNT_RUN_MAX = 4092;   // multiple of 4 below 2^12
+constexpr int COUNT_NP = 10;               // planes: a run adds at most 2^10 - 1 rows to a counter before it is flushed
+constexpr uint32_t COUNT_RUN_MAX = 1016;   // multiple of 8 below 2^10
 constexpr uint32_t COUNT_RUN_MIN = 96;
 
 __device__ __forceinline__ uint32_t axor3(uint32_t a, uint32_t b, uint32_t c) {
@@ -135,6 +136,25 @@ __global__ void __launch_bounds__(256) ibp_count_kernel(const TableDev T, uint32
                     for (int p = 2; p < COUNT_NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
                 }
             };
+            // eight rows in flight (the kernel is latency-bound at the occupancy its plane registers allow)
+            auto add8 = [&](uint64_t r0, uint64_t step) {
+                uint32_t x[8][W];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) VecIO<W>::ld(T.rows + (r0 + i * step) * T.nw + w0, x[i]);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        const uint32_t s1 = axor3(pl[0][q], x[4 * h][q], x[4 * h + 1][q]), c1 = amaj3(pl[0][q], x[4 * h][q], x[4 * h + 1][q]);
+                        const uint32_t s2 = axor3(s1, x[4 * h + 2][q], x[4 * h + 3][q]), c2 = amaj3(s1, x[4 * h + 2][q], x[4 * h + 3][q]);
+                        pl[0][q] = s2;
+                        uint32_t c = amaj3(pl[1][q], c1, c2);
+                        pl[1][q] = axor3(pl[1][q], c1, c2);
+#pragma unroll
+                        for (int p = 2; p < COUNT_NP; ++p) { const uint32_t t = pl[p][q]; pl[p][q] = t ^ c; c &= t; }
+                    }
+                }
+            };
             auto add1 = [&](uint64_t r0) {
                 uint32_t x[W];
                 VecIO<W>::ld(T.rows + r0 * T.nw + w0, x);
@@ -162,6 +182,7 @@ __global__ void __launch_bounds__(256) ibp_count_kernel(const TableDev T, uint32
                     cur_g = g; cur_n = (uint32_t)n_seg;
                     if (active) {
                         uint64_t i = 0;
+                        for (; i + 8 <= n_seg; i += 8, row += 8 * step) add8(row, step);
                         for (; i + 4 <= n_seg; i += 4, row += 4 * step) add4(row, row + step, row + 2 * step, row + 3 * step);
                         for (; i < n_seg; ++i, row += step) add1(row);
                     }
@@ -495,7 +516,7 @@ static ibp_status launch_counts(TableDev T, const int64_t* sample_ids_dev, int64
     // run length: enough runs to fill the machine (8 warps x 8 CTAs per SM), each as long as the planes allow, so that the
     // atomic flushes (32 per word per run and group) stay rare
     const int grid_full = analysis_grid(~0ull >> 8);
-    uint64_t run = ((T.n_list + (uint64_t)grid_full * 8 - 1) / ((uint64_t)grid_full * 8) + 3) / 4 * 4;   // ceil: no second, partial round of runs
+    uint64_t run = ((T.n_list + (uint64_t)grid_full * 8 - 1) / ((uint64_t)grid_full * 8) + 7) / 8 * 8;   // ceil: no second, partial round of runs
     run = std::max<uint64_t>(COUNT_RUN_MIN, std::min<uint64_t>(COUNT_RUN_MAX, run));
     const uint64_t n_runs = (T.n_list + run - 1) / run;
     const int grid = analysis_grid(n_runs);
