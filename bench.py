@@ -227,6 +227,17 @@ def run_cuda(args):
     # ---- ceilings measured on this box, this run
     h2d_ceiling = ibp.ibp_measure_h2d(local, 1 << 30, 8)
     zc_ceiling = ibp.ibp_measure_zero_copy_read(local, 1 << 30, 3)
+    # random-row gathers: the same link read as random, span-aligned spans of about one packed row, over a managed host
+    # buffer as large as the packed store (beyond a few hundred MB address translation, not the link,
+    # sets this rate) -- the measured ceiling of any random gather of rows this small on this box
+    rand_ceiling = None
+    if w.index_span == 1 and rank == 0 and info.packed_bytes_stored >= (64 << 20):
+        mean_row = info.packed_bytes_rows / w.n_rows
+        span = 128 if mean_row <= 128 else 256 if mean_row <= 256 else 512
+        sps, gbs = ibp.ibp_measure_random_read(local, int(min(info.packed_bytes_stored, 8 << 30)), span, 3)
+        rand_ceiling = {"span_bytes": span, "footprint_GB": round(min(info.packed_bytes_stored, 8 << 30) * 1e-9, 2),
+                        "spans_per_s": round(sps), "GBps": round(gbs, 2),
+                        "what": "ibp_measure_random_read: LSU 16-byte loads of span-aligned random spans, managed host-resident buffer"}
     hbm_peak = None
     try:
         hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
@@ -431,6 +442,8 @@ def run_cuda(args):
                 "kernel": "ibp_stream_kernel" if (w.index_span > 1 and not info.thresholded) else "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
                 "algorithmic_bytes_per_launch": int(np.mean(stored_timed)),
                 "zero_copy_read_ceiling": round(zc_ceiling, 3), "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
+                "random_span_ceiling": rand_ceiling,
+                "distinct_rows_per_s": round(float(np.sum(unique_timed)) / (float(np.sum(kernel_ms)) * 1e-3)),
                 "effective_roofline_GBps": round(float(eff_roof), 2), "frac_of_effective_roofline": round(value / world / float(eff_roof), 4),
                 "effective_roofline_def": "min(H2D ceiling x raw bytes / stored packed bytes of the batch, HBM peak)",
                 "frac_vs_bytealigned_ratio": round(value / world / min(h2d_ceiling * float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(alg_timed)) * (n / np.mean(unique_timed)), hbm_peak), 4),
