@@ -53,9 +53,12 @@ __device__ __forceinline__ uint32_t bitselect(uint32_t a, uint32_t b, uint32_t c
     asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
+// NSTG = number of low stages that can move a bit: a group whose words never move a bit by 8 or 16 positions (bf16 pairs
+// with a few invariant exponent bits per half) needs 3 stages instead of 5.
+template <int NSTG = 5>
 __device__ __forceinline__ uint32_t expand_bits(uint32_t x, const uint32_t mv[5]) {
 #pragma unroll
-    for (int i = 4; i >= 0; --i) x = bitselect(x << (1 << i), x, mv[i]);
+    for (int i = NSTG - 1; i >= 0; --i) x = bitselect(x << (1 << i), x, mv[i]);
     return x;
 }
 
@@ -86,7 +89,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
 
     // chunk c -> first row id, rows (blocked) or matrix rows (strided), first output row, packed byte range
     auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0, uint64_t& b0, uint64_t& b1) {
-        const int64_t si = c / P.chunks_per_span;
+        const int64_t si = !P.ids ? 0 : (P.n_chunks <= 0x7FFFFFFFll ? (int64_t)((uint32_t)c / P.chunks_per_span) : c / P.chunks_per_span);
         const int64_t cc = c - si * P.chunks_per_span;
         const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
         if (!P.strided) {
@@ -137,6 +140,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     // words inside a packed row, the five expand masks -- and the row loop is: 2 ld.shared + 1 funnel shift + 11 logic
     // ops per word, one vector store, two pointer bumps.
     uint32_t m[W], b[W], ex[W], mv[W][5];
+    uint32_t n_stages = 5;             // expand stages the prepared group needs (warp-uniform)
     uint64_t prep_g = ~0ull;
     const uint32_t w0_fast = lane * W;
     const bool fast = P.n_pass == 1 && P.fast_rows;
@@ -172,11 +176,16 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 }
             }
         }
+        uint32_t hi8 = 0, hi16 = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) { hi8 |= mv[q][3]; hi16 |= mv[q][4]; }
+        n_stages = __any_sync(0xFFFFFFFFu, hi16 != 0) ? 5u : __any_sync(0xFFFFFFFFu, hi8 != 0) ? 4u : 3u;
         prep_g = g;
     };
 
     // `count` rows of the prepared group: packed row r at shared address saddr + r*sstride, output row at optr + r*ostride
-    auto decode_run = [&](uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
+    auto decode_run_n = [&](auto nstg, uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
+        constexpr int NSTG = decltype(nstg)::value;
         uint32_t wa[W], sh[W];
 #pragma unroll
         for (int q = 0; q < W; ++q) { wa[q] = saddr + (ex[q] >> 5) * 4u; sh[q] = ex[q] & 31u; }
@@ -188,12 +197,17 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 uint32_t lo, hi;
                 asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wa[q]));
                 const uint32_t x = __funnelshift_r(lo, hi, sh[q]);
-                o[q] = bitselect(b[q], expand_bits(x, mv[q]), m[q]);   // Bitval where Mask is 1, expanded bits elsewhere
+                o[q] = bitselect(b[q], expand_bits<NSTG>(x, mv[q]), m[q]);   // Bitval where Mask is 1, expanded bits elsewhere
                 wa[q] += sstride;
             }
             if (active_fast) VecIO<W>::st(optr, o);
             optr += ostride;
         }
+    };
+    auto decode_run = [&](uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
+        if (n_stages == 3) decode_run_n(std::integral_constant<int, 3>{}, saddr, sstride, optr, ostride, count);
+        else if (n_stages == 4) decode_run_n(std::integral_constant<int, 4>{}, saddr, sstride, optr, ostride, count);
+        else decode_run_n(std::integral_constant<int, 5>{}, saddr, sstride, optr, ostride, count);
     };
 
     uint32_t k = 0;

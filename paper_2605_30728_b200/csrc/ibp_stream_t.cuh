@@ -44,7 +44,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
 
     // chunk c -> first row id, number of rows (consecutive ids), first output row
     auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0) {
-        const int64_t si = c / P.chunks_per_span;
+        const int64_t si = !P.ids ? 0 : (P.n_chunks <= 0x7FFFFFFFll ? (int64_t)((uint32_t)c / P.chunks_per_span) : c / P.chunks_per_span);
         const int64_t cc = c - si * P.chunks_per_span;
         const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
         const int64_t per = P.strided ? (int64_t)P.rows_per_chunk * (int64_t)S : (int64_t)P.rows_per_chunk;
