@@ -389,7 +389,7 @@ def run_cuda(args):
         resident = {"rows": nr, "ms": round(t_r, 4), "out_GBps": round(nr * w.row_bytes / (t_r * 1e-3) * 1e-9, 1),
                     "in_plus_out_GBps": round((nb + nr * w.row_bytes) / (t_r * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": hbm_peak,
                     "frac": round((nb + nr * w.row_bytes + meta_bytes) / (t_r * 1e-3) * 1e-9 / hbm_peak, 4),
-                    "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes), "kernel": ("ibp_decode_kernel" if info.thresholded else "ibp_stream_kernel") + " (ibp_decompress_resident)",
+                    "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes), "kernel": ("ibp_stream_t_kernel" if info.thresholded else "ibp_stream_kernel") + " (ibp_decompress_resident)",
                     "what": "packed bytes of the first rows of the table staged in HBM, decoded to HBM; L2 flushed between launches"}
         del staged, outr
 
