@@ -615,13 +615,14 @@ static ibp_status launch_stream_one(const StreamParams& P, int64_t max_ctas, int
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
     int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
     if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
+    if (P.n_tile_blocks) blocks = std::max<int64_t>(P.n_tile_blocks, blocks / P.n_tile_blocks * P.n_tile_blocks);   // one tile block per CTA
     kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(P);
     IBP_CUDA(cudaGetLastError());
     return IBP_OK;
 }
 
 static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
-                                int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st) {
+                                int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st, bool resident = false) {
     if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
     const int W = pick_W(h->p.row_bytes);
     const uint32_t NW = 8;
@@ -660,6 +661,28 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
         P.piece_rows = U;
         need = rc * h->max_stride + (rc / G + 2) * 128 + 64;
         P.chunks_per_span = (uint32_t)((span_rows + (int64_t)rc - 1) / (int64_t)rc);
+    } else if (resident && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1 && (!h->max_ctas || h->max_ctas >= (G + NW - 1) / NW)) {
+        // resident decode of a strided table: tile-block chunks (ibp_stream.cuh).  A whole-row chunk holds only 2-7 matrix rows
+        // of the 7B shapes, so every warp would re-prepare a tile (Mask/Bitval, offsets, expand masks) for a handful of rows;
+        // here a CTA keeps one block of NW tiles for all its chunks and prepares once.  The source is HBM, so the shorter
+        // contiguous reads (one block of one matrix row per bulk copy) cost nothing; the host-store path keeps whole rows.
+        const uint32_t n_tb = (uint32_t)((G + NW - 1) / NW);
+        uint64_t max_len = 0;
+        for (uint32_t tb = 0; tb < n_tb; ++tb) {
+            const IbpGroupEntry& e0 = h->gtab[(uint64_t)tb * NW];
+            const IbpGroupEntry& e1 = h->gtab[std::min<uint64_t>(G, (uint64_t)tb * NW + NW) - 1];
+            max_len = std::max<uint64_t>(max_len, e1.base + e1.stride - e0.base);
+        }
+        const uint64_t pitch = (max_len + 31 + 15) / 16 * 16;
+        const int64_t n_mrows = (span_rows + (int64_t)G - 1) / (int64_t)G;
+        uint64_t rc = std::max<uint64_t>(1, std::min<uint64_t>(32, (48ull * 1024) / pitch));
+        rc = (uint64_t)std::min<int64_t>((int64_t)rc, n_mrows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = (uint32_t)rc;
+        P.n_tile_blocks = n_tb;
+        P.tb_pitch = (uint32_t)pitch;
+        need = rc * pitch + 64;
+        P.chunks_per_span = (uint32_t)(((n_mrows + (int64_t)rc - 1) / (int64_t)rc) * n_tb);
     } else {
         const uint64_t rs = h->row_stride_strided;
         const uint64_t cap = rs > 8192 ? 64ull * 1024 : 48ull * 1024;
@@ -733,9 +756,10 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     const uint64_t stride = h->max_stride;                                             // a raw row: the largest stored row
     uint64_t per;                                                                      // consecutive rows per chunk
     if (!P.strided) {
-        const uint32_t U = 16;
+        uint32_t U = 16;
         uint64_t rc = std::min<uint64_t>((uint64_t)NW * U, (48ull * 1024) / stride);
         rc = std::max<uint64_t>(rc, 1);
+        if (rc < (uint64_t)NW * U) U = (uint32_t)std::max<uint64_t>(1, rc / NW);   // one piece per consumer warp (GNN: 96 rows = 8 x 12, not 6 x 16)
         if (rc >= U) rc = rc / U * U;
         rc = (uint64_t)std::min<int64_t>((int64_t)rc, span_rows);
         P.rows_per_chunk = (uint32_t)rc;
@@ -922,11 +946,11 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
 
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
 // byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
-static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st) {
+static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st, bool resident = false) {
     if (h->stream_mode && h->thresholded && stream_t_fits(h))
         return launch_stream_t(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     if (h->stream_mode && !h->thresholded)
-        return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
+        return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st, resident);
     DecodeParams P;
     fill_common(h, P);
     P.store = packed;
@@ -966,7 +990,7 @@ extern "C" ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_
     if (!packed_dev || ((uintptr_t)packed_dev & 15u)) { ibp_set_error("ibp_decompress_resident: packed_dev must be a 16-byte aligned device pointer"); return IBP_ERR_INVALID_ARG; }
     s = check_range(h, "ibp_decompress_resident", first_row, n_rows, out_dev);
     if (s != IBP_OK) return s;
-    return decode_range(h, (const uint8_t*)packed_dev, first_row, n_rows, out_dev, (cudaStream_t)cuda_stream);
+    return decode_range(h, (const uint8_t*)packed_dev, first_row, n_rows, out_dev, (cudaStream_t)cuda_stream, true);
 }
 
 extern "C" ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream) {

@@ -29,6 +29,11 @@ struct StreamParams {
     uint32_t group_param, group_shift, strided;
     uint32_t stage_bytes;
     uint32_t fast_rows;            // packed rows start on 4-byte boundaries (A >= 4): the hoisted single-pass path applies
+    // strided tables, tile-block mode (resident decode): a chunk is `rows_per_chunk` matrix rows x one block of NW column
+    // tiles, and chunk c belongs to block c % n_tile_blocks -- with a grid that is a multiple of n_tile_blocks every CTA
+    // keeps ONE block, so consumer warp w decodes the same tile in every chunk and prepares it once.  0 = off.
+    uint32_t n_tile_blocks;
+    uint32_t tb_pitch;             // bytes between the block's images of consecutive matrix rows inside a stage
 };
 
 // The five move masks of the parallel-suffix expand for deposit positions nv (set bits = positions to fill, lowest first).
@@ -118,6 +123,27 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         // ------------------------------------------------------------------ producer
         if (lane != 0) return;
         uint32_t k = 0;
+        if (P.n_tile_blocks) {
+            for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+                const uint32_t s = k % NS;
+                mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
+                const uint32_t tb = (uint32_t)c % P.n_tile_blocks, rbk = (uint32_t)c / P.n_tile_blocks;
+                const uint32_t t0 = tb * NW, t1 = min((uint32_t)S, t0 + NW);
+                const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
+                const int64_t mr0 = (int64_t)rbk * P.rows_per_chunk;
+                const uint32_t nrows = (uint32_t)min((int64_t)P.rows_per_chunk, n_mrows - mr0);
+                const IbpGroupEntry e0 = P.gtab[t0], e1 = P.gtab[t1 - 1];
+                const uint64_t lo = e0.base, len = e1.base + e1.stride - lo;
+                const uint8_t* src = P.store + (((uint64_t)P.first_row / S + (uint64_t)mr0) * P.row_stride_strided + lo - P.bias);
+                const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
+                const uint32_t bytes = (uint32_t)((head + len + 15u) & ~15ull);
+                mbar_expect_tx(full_s + s * 8, bytes * nrows);
+                const uint32_t dst = smem_s + s * P.stage_bytes;
+                for (uint32_t i = 0; i < nrows; ++i)
+                    bulk_g2s(dst + i * P.tb_pitch, src - head + (uint64_t)i * P.row_stride_strided, bytes, full_s + s * 8);
+            }
+            return;
+        }
         for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
             const uint32_t s = k % NS;
             mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
@@ -211,6 +237,31 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     };
 
     uint32_t k = 0;
+    if (P.n_tile_blocks) {
+        // tile-block mode: this CTA's chunks all carry tile block blockIdx.x % n_tile_blocks; warp wib owns one tile of it
+        const uint32_t tb = blockIdx.x % P.n_tile_blocks, t = tb * NW + wib;
+        const bool has_tile = t < (uint32_t)S;
+        uint32_t toff = 0;
+        if (has_tile) {
+            const IbpGroupEntry e0 = P.gtab[tb * NW], e = P.gtab[t];
+            const uint8_t* src = P.store + (((uint64_t)P.first_row / S) * P.row_stride_strided + e0.base - P.bias);
+            toff = (uint32_t)((uintptr_t)src & 15u) + (uint32_t)(e.base - e0.base);   // row_stride_strided is a multiple of 16
+            prepare(t);
+        }
+        const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
+        const int64_t tile_rows = has_tile ? (P.span_rows - (int64_t)t + (int64_t)S - 1) / (int64_t)S : 0;   // rows of tile t in range
+        for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+            const uint32_t s = k % NS;
+            const int64_t mr0 = (int64_t)((uint32_t)c / P.n_tile_blocks) * P.rows_per_chunk;
+            const int64_t cnt = min(min((int64_t)P.rows_per_chunk, n_mrows - mr0), tile_rows - mr0);
+            mbar_wait(full_s + s * 8, (k / NS) & 1u);
+            if (cnt > 0)
+                decode_run(smem_s + s * P.stage_bytes + toff, P.tb_pitch, P.out + ((uint64_t)mr0 * S + t) * P.row_bytes, S * P.row_bytes, (uint32_t)cnt);
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+        }
+        return;
+    }
     for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
         const uint32_t s = k % NS;
         int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;

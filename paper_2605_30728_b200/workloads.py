@@ -107,13 +107,20 @@ class GNN(Workload):
     """configs[1]: 10M x 128 fp32; ids < 70%: N(0,1) in 2^-8 steps; the rest sparse 0.0/1.0 with 2% density (R15:
     contiguous by type); groups of 256; 250k UNIQUE ids per batch, Zipf(0.9) through a seeded permutation (R16, R21)."""
 
-    def __init__(self, n_rows=10_000_000, batch=250_000):
+    def __init__(self, n_rows=10_000_000, batch=250_000, interleaved=False):
         super().__init__("gnn", 1, n_rows, 512, "f32", BLOCKED, 256, 1, 32, batch, ids_unique=True)
         self.n_dense = (n_rows * 7) // 10
+        self.interleaved = interleaved       # R15's secondary variant: row type drawn per row (70/30), every group mixes both
 
     def fill_rows(self, first, count, out):
         e = self.row_elems
         flat = out.reshape(-1)
+        if self.interleaved:
+            sparse = (datagen.u64(count, self.seed + 4242, first) % np.uint64(10)) >= np.uint64(7)
+            datagen.normal_f32(count * e, self.seed, first * e, 1.0, 2.0 ** -8, 0.0, out=flat)
+            sp = datagen.bernoulli_f32(count * e, self.seed + 7777, first * e, 0.02).reshape(count, e)
+            out.reshape(count, e)[sparse] = sp[sparse]
+            return
         nd = max(0, min(first + count, self.n_dense) - first)          # dense rows in this range
         if nd:
             datagen.normal_f32(nd * e, self.seed, first * e, 1.0, 2.0 ** -8, 0.0, out=flat[: nd * e])

@@ -106,6 +106,29 @@ def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
     h.destroy()
 
 
+@pytest.mark.parametrize("S,n,rb,align", [(86, 86 * 40 + 13, 256, 16), (32, 32 * 70, 256, 16), (9, 9 * 33 + 4, 512, 32), (16, 16 * 5, 64, 4),
+                                           (17, 17 * 100 + 16, 128, 16), (8, 8 * 3 + 1, 256, 32), (3, 50, 512, 16), (40, 40 * 64 + 39, 128, 4)])
+def test_strided_resident_tile_blocks(S, n, rb, align):
+    """Resident decode of strided tables takes tile-block chunks (a CTA keeps one block of 8 column tiles, a warp one tile):
+    tile counts that are not a multiple of 8, fewer tiles than consumer warps, a partial last matrix row, ranges that start
+    inside the table, a tile whose rows are all identical (k = 0) and one with no invariant bit."""
+    X = (datagen.random_bytes(n * rb, 11 + S).reshape(n, rb) & datagen.random_bytes(rb, 19)[None, :]) | 0x01
+    X[1 % S::S] = X[1 % S]                                              # tile 1: every row the same -> nothing stored
+    X[2 % S::S] = datagen.random_bytes(len(X[2 % S::S]) * rb, 23).reshape(-1, rb)   # tile 2: (almost surely) nothing invariant
+    h = ibp.ibp_build(X, rb, 1, S, align_bytes=align).upload_metadata(0)
+    ds = oracle.Dataset(X, 1, S)
+    assert np.array_equal(_resident(h, 0, n), X)
+    assert np.array_equal(ds.gather_decompress(np.arange(n)), X)
+    for first, cnt in [(0, S), (0, 2 * S + 1), (S * ((n // S) // 2), n - S * ((n // S) // 2)), (S, min(n - S, 3 * S - 1))]:
+        if cnt > 0 and first + cnt <= n:
+            assert np.array_equal(_resident(h, first, cnt), X[first:first + cnt]), (first, cnt)
+            assert np.array_equal(_range(h, first, cnt), X[first:first + cnt]), (first, cnt)
+    h.configure(4, 0)                                                   # fewer CTAs than tile blocks: whole-row chunks again
+    assert np.array_equal(_resident(h, 0, n), X)
+    h.destroy()
+    ds.close()
+
+
 def test_edge_cases():
     rb = 256
     r = datagen.random_bytes(rb, 3)

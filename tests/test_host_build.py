@@ -219,3 +219,21 @@ def test_T_workload_shapes():
     _check_T_against_oracle(X, 0, 1 << 20, (4, 5), rows_to_check=range(0, 2048, 7))   # one global Mask/Bitval
     t = workloads.Tiny(n_rows=512).table()
     _check_T_against_oracle(t, 0, 64, (4, 5), align=16)
+
+
+def test_gnn_interleaved_variant_recipe_and_ratio():
+    """Reading R15's secondary workload: row types drawn per row (about 70/30), any row range regenerates alone, and the host
+    build of a table whose groups all mix both types keeps almost none of the sparse rows' compressibility (SURVEY 8(d):
+    "the sparse rows lose their 4.6x")."""
+    w = workloads.GNN(n_rows=8192, batch=64, interleaved=True)
+    X = w.table()
+    assert np.array_equal(w.rows(3000, 77).view(np.uint32), X[3000:3077].view(np.uint32))
+    sparse = ((X == 0) | (X == 1)).all(axis=1)
+    assert 0.25 < sparse.mean() < 0.35
+    mixed = ibp.ibp_build(X, 512, 0, 256, align_bytes=1, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    typed = ibp.ibp_build(workloads.GNN(n_rows=8192, batch=64).table(), 512, 0, 256, align_bytes=1, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    r_mixed = X.nbytes / mixed.info().packed_bytes_bytealigned
+    r_typed = X.nbytes / typed.info().packed_bytes_bytealigned
+    assert r_mixed < r_typed and r_mixed < 1.9
+    mixed.destroy()
+    typed.destroy()
