@@ -918,6 +918,119 @@ def run_masks(args):
     print(json.dumps(line), flush=True)
 
 
+def run_resident(args):
+    """SURVEY 8(a) S8 alone: ibp_decompress_resident of a contiguous range whose packed bytes were staged in HBM beforehand
+    (what a compressed GPU cache or a DMA-staged block decodes).  One step = one launch over the range: the first
+    2^20 rows of the workload's table, or one 4096 x 11008 bf16 matrix for `weights`.  HBM-bound: algorithmic bytes = packed
+    in + rows out + Mask/Bitval of the groups touched."""
+    import torch
+    from paper_2605_30728_b200 import binding as ibp, workloads
+    import oracle
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --phase resident runs on one GPU")
+    torch.cuda.set_device(0)
+    thr = parse_threshold(args.threshold)
+    if args.workload == "weights":
+        w = workloads.WeightMatrix(rows=4096, cols=11008)
+        nr = w.n_rows
+        label = "configs[4] one 4096 x 11008 bf16 matrix N(0,0.02), 128-column tiles as strided groups (86 tiles)"
+    else:
+        w = make_workload(args.workload)
+        nr = min(w.n_rows, 1 << 20)
+        label = describe(w) + f" -- the first {nr} rows"
+    align = args.align if args.align else w.align_bytes
+    X = w.rows(0, nr)
+    Xb = X.view(np.uint8).reshape(nr, -1)
+    h = ibp.ibp_build(Xb, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, threshold=thr, flags=ibp.IBP_FLAG_PAGEABLE_STORE).upload_metadata(0)
+    info = h.info()
+    stream = torch.cuda.current_stream().cuda_stream
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_peak = 6650.0
+    ptr, nb = h.packed_range(0, nr)
+    staged = torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda()
+    out = torch.empty((nr, w.row_bytes), dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    W, K = max(3, args.warmup), max(1, args.steps)
+    for _ in range(W):
+        h.decompress_resident(staged.data_ptr(), 0, nr, out.data_ptr(), stream)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    if not np.array_equal(got, Xb):                                            # (c1): the original rows, every byte
+        raise SystemExit("bench.py: resident decode differs from the original rows; refusing to report a number")
+    ids = np.random.default_rng(0).choice(nr, 256, replace=False)
+    ds = (oracle.Dataset(Xb, w.group_kind, w.group_param) if thr[0] == thr[1] else oracle.DatasetT(Xb, w.group_kind, w.group_param, thr[0], thr[1])) if nr * w.row_bytes <= (64 << 20) else None
+    if ds is not None:
+        if not np.array_equal(got[ids], ds.gather_decompress(ids)):
+            raise SystemExit("bench.py: resident decode differs from the oracle codec")
+        ds.close()
+    clocks = ClockSampler(0)
+    clocks.start()
+    ms = []
+    for _ in range(K):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        h.decompress_resident(staged.data_ptr(), 0, nr, out.data_ptr(), stream)
+        b.record()
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+    clk = clocks.stop()
+    t = float(np.mean(ms))
+    meta_bytes = info.n_groups * 2 * w.row_bytes
+    alg = nb + nr * w.row_bytes + meta_bytes
+    # e2e: the packed bytes come from pinned host memory (DMA staging, P:357 cache fill path) and the rows go back to the host
+    pk_pin = ibp.PinnedBuffer(nb)
+    pk_pin.view(np.uint8)[:] = h.packed_view(ptr, nb)
+    out_pin = ibp.PinnedBuffer(nr * w.row_bytes)
+    pin_t = torch.from_numpy(pk_pin.view(np.uint8))
+    out_t = torch.from_numpy(out_pin.view(np.uint8, (nr, w.row_bytes)))
+    te = []
+    for i in range(5):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        staged.copy_(pin_t, non_blocking=True)
+        h.decompress_resident(staged.data_ptr(), 0, nr, out.data_ptr(), stream)
+        out_t.copy_(out, non_blocking=True)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= 2:
+            te.append(a.elapsed_time(b))
+    cpu = None
+    if not args.no_cpu:
+        sample = Xb[: 96 * w.group_param] if w.group_kind == 0 else Xb
+        dsb = oracle.Dataset(sample, w.group_kind, w.group_param) if thr[0] == thr[1] else oracle.DatasetT(sample, w.group_kind, w.group_param, thr[0], thr[1])
+        t0 = time.perf_counter()
+        done = 0
+        sid = np.arange(min(len(sample), 20000), dtype=np.int64)
+        while time.perf_counter() - t0 < 10.0:
+            dsb.gather_decompress(sid)
+            done += len(sid)
+        dt = time.perf_counter() - t0
+        dsb.close()
+        cpu = {"value": round(done * w.row_bytes / dt * 1e-9, 5), "unit": "GB/s", "cores": 1, "kind": "oracle",
+               "sample": f"{done} row decodes of the first {len(sid)} rows by the oracle codec, {dt:.1f} s"}
+    kernel = "ibp_stream_t_kernel" if info.thresholded else "ibp_stream_kernel"
+    line = {
+        "metric": "resident decode, decompressed GB/s (ibp_decompress_resident)", "value": round(nr * w.row_bytes / (t * 1e-3) * 1e-9, 1), "unit": "GB/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": round(t, 5), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic", "rows_per_s": round(nr / (t * 1e-3)),
+        "config": {"workload": label + "; packed bytes staged in HBM, decoded to HBM", "rows": nr, "row_bytes": w.row_bytes, "align_bytes": info.align_bytes,
+                   "codec": "group-strict (tau = 1)" if not info.thresholded else f"thresholded, tau = {thr[0]}/{thr[1]}",
+                   "packed_MB": round(nb * 1e-6, 2), "ratio_stored": round(nr * w.row_bytes / nb, 4),
+                   "l2": "flushed with a 256 MiB write between steps (outside the events)"},
+        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": round(alg / (t * 1e-3) * 1e-9, 1), "peak": hbm_peak, "unit": "GB/s",
+                     "frac": round(alg / (t * 1e-3) * 1e-9 / hbm_peak, 4), "traffic": None, "algorithmic_bytes_per_launch": int(alg),
+                     "algorithmic_bytes_def": "packed bytes in + rows out + 2*row_bytes of Mask/Bitval per group", "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy; read+write bytes)"},
+        "e2e": {"value": round(nr * w.row_bytes / (float(np.mean(te)) * 1e-3) * 1e-9, 2), "unit": "GB/s", "h2d_bytes_per_step": int(nb), "d2h_bytes_per_step": int(nr * w.row_bytes),
+                "api": "cudaMemcpyAsync of the packed range from pinned memory, ibp_decompress_resident, cudaMemcpyAsync of the rows to pinned memory"},
+        "gpu_launches": K, "clocks": clk, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -933,8 +1046,8 @@ def main():
     ap.add_argument("--threshold", default="1/1", help="tau = T/N as a fraction: 1/1 = group-strict (BASELINE.json), 4/5 = the paper's thresholded codec")
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
-    ap.add_argument("--phase", default="gather", choices=["gather", "build", "masks"],
-                    help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device; masks = the mask-quality tools (tau / chunk-size sweep, sampled masks, k-means)")
+    ap.add_argument("--phase", default="gather", choices=["gather", "build", "masks", "resident"],
+                    help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device; masks = the mask-quality tools (tau / chunk-size sweep, sampled masks, k-means); resident = ibp_decompress_resident alone (S8)")
     ap.add_argument("--cache-frac", type=float, default=0.0, help="gnn/dlrm: put a compressed GPU cache of this fraction of the packed store in front of the host store")
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -950,6 +1063,8 @@ def main():
         run_build(args)
     elif args.phase == "masks":
         run_masks(args)
+    elif args.phase == "resident":
+        run_resident(args)
     elif args.workload == "weights":
         run_weights(args)
     else:
