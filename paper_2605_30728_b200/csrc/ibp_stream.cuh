@@ -58,6 +58,12 @@ __device__ __forceinline__ uint32_t bitselect(uint32_t a, uint32_t b, uint32_t c
     asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
+// (a & b) | c in one logic op
+__device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
 // NSTG = number of low stages that can move a bit: a group whose words never move a bit by 8 or 16 positions (bf16 pairs
 // with a few invariant exponent bits per half) needs 3 stages instead of 5.
 template <int NSTG = 5>
@@ -165,8 +171,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     // only on the group is hoisted out of the row loop -- Mask/Bitval, the word offset and shift of each of the lane's W
     // words inside a packed row, the five expand masks -- and the row loop is: 2 ld.shared + 1 funnel shift + 11 logic
     // ops per word, one vector store, two pointer bumps.
-    uint32_t m[W], b[W], ex[W], mv[W][5];
-    uint32_t n_stages = 5;             // expand stages the prepared group needs (warp-uniform)
+    // Per-group decode state of the lane's W words.  Two forms, chosen per group (warp-uniform `mode`):
+    //   runs (mode 1..3): every word of the group has at most 3 runs of variant bits (float data: a mantissa run, an exponent run,
+    //     the sign).  Run j takes bits [c_j, c_j+len_j) of the extracted word to positions [p_j, p_j+len_j): one multiply by
+    //     2^(p_j-c_j) and one lop3 (and-or) per run -- mv[q][j] = the multiplier, mv[q][3+j] = the run's mask;
+    //   expand (mode 13..15): the general 5-stage parallel-suffix expand, mv[q][0..4] = its move masks, 3/4/5 stages as needed.
+    uint32_t m[W], b[W], ex[W], mv[W][6];
+    uint32_t mode = 15;
     uint64_t prep_g = ~0ull;
     const uint32_t w0_fast = lane * W;
     const bool fast = P.n_pass == 1 && P.fast_rows;
@@ -185,6 +196,28 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         const uint32_t incl = warp_inclusive_scan(t, lane);
 #pragma unroll
         for (int q = 0; q < W; ++q) ex[q] += incl - t;
+        // runs of variant bits, lowest first (3 at most; `more` = a word has a fourth)
+        bool more = false;
+        uint32_t n_runs = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) {
+            uint32_t nv = ~m[q], c = 0;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const uint32_t low = nv & (0u - nv), run = nv & ~(nv + low);     // nv == 0 -> low = run = 0
+                mv[q][j] = run ? 1u << ((__ffs(low) - 1) - c) : 0u;
+                mv[q][3 + j] = run;
+                c += __popc(run);
+                nv &= ~run;
+                n_runs = max(n_runs, run ? (uint32_t)j + 1u : 0u);
+            }
+            more = more || nv != 0;
+        }
+        if (!__any_sync(0xFFFFFFFFu, more)) {
+            mode = __any_sync(0xFFFFFFFFu, n_runs == 3) ? 3u : __any_sync(0xFFFFFFFFu, n_runs == 2) ? 2u : 1u;
+            prep_g = g;
+            return;
+        }
         if (P.mvtab && active_fast) {
             const uint32_t* tv = P.mvtab + (g * P.n_words + w0_fast) * 5ull;
 #pragma unroll
@@ -205,13 +238,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         uint32_t hi8 = 0, hi16 = 0;
 #pragma unroll
         for (int q = 0; q < W; ++q) { hi8 |= mv[q][3]; hi16 |= mv[q][4]; }
-        n_stages = __any_sync(0xFFFFFFFFu, hi16 != 0) ? 5u : __any_sync(0xFFFFFFFFu, hi8 != 0) ? 4u : 3u;
+        mode = __any_sync(0xFFFFFFFFu, hi16 != 0) ? 15u : __any_sync(0xFFFFFFFFu, hi8 != 0) ? 14u : 13u;
         prep_g = g;
     };
 
     // `count` rows of the prepared group: packed row r at shared address saddr + r*sstride, output row at optr + r*ostride
-    auto decode_run_n = [&](auto nstg, uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
-        constexpr int NSTG = decltype(nstg)::value;
+    auto decode_run_n = [&](auto nstg, auto runs, uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
+        constexpr int NSTG = decltype(nstg)::value;         // expand stages, or runs per word
+        constexpr bool RUNS = decltype(runs)::value;
         uint32_t wa[W], sh[W];
 #pragma unroll
         for (int q = 0; q < W; ++q) { wa[q] = saddr + (ex[q] >> 5) * 4u; sh[q] = ex[q] & 31u; }
@@ -223,7 +257,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 uint32_t lo, hi;
                 asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wa[q]));
                 const uint32_t x = __funnelshift_r(lo, hi, sh[q]);
-                o[q] = bitselect(b[q], expand_bits<NSTG>(x, mv[q]), m[q]);   // Bitval where Mask is 1, expanded bits elsewhere
+                if (NSTG <= 3 && RUNS) {
+                    uint32_t acc = b[q];                                        // Bitval, then each run of variant bits or-ed in
+#pragma unroll
+                    for (int j = 0; j < NSTG; ++j) acc = and_or(x * mv[q][j], mv[q][3 + j], acc);
+                    o[q] = acc;
+                } else {
+                    o[q] = bitselect(b[q], expand_bits<NSTG>(x, mv[q]), m[q]);   // Bitval where Mask is 1, expanded bits elsewhere
+                }
                 wa[q] += sstride;
             }
             if (active_fast) VecIO<W>::st(optr, o);
@@ -231,9 +272,17 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         }
     };
     auto decode_run = [&](uint32_t saddr, uint32_t sstride, uint8_t* optr, uint64_t ostride, uint32_t count) {
-        if (n_stages == 3) decode_run_n(std::integral_constant<int, 3>{}, saddr, sstride, optr, ostride, count);
-        else if (n_stages == 4) decode_run_n(std::integral_constant<int, 4>{}, saddr, sstride, optr, ostride, count);
-        else decode_run_n(std::integral_constant<int, 5>{}, saddr, sstride, optr, ostride, count);
+        using std::integral_constant;
+        using std::true_type;
+        using std::false_type;
+        switch (mode) {
+            case 1: decode_run_n(integral_constant<int, 1>{}, true_type{}, saddr, sstride, optr, ostride, count); break;
+            case 2: decode_run_n(integral_constant<int, 2>{}, true_type{}, saddr, sstride, optr, ostride, count); break;
+            case 3: decode_run_n(integral_constant<int, 3>{}, true_type{}, saddr, sstride, optr, ostride, count); break;
+            case 13: decode_run_n(integral_constant<int, 3>{}, false_type{}, saddr, sstride, optr, ostride, count); break;
+            case 14: decode_run_n(integral_constant<int, 4>{}, false_type{}, saddr, sstride, optr, ostride, count); break;
+            default: decode_run_n(integral_constant<int, 5>{}, false_type{}, saddr, sstride, optr, ostride, count); break;
+        }
     };
 
     uint32_t k = 0;
