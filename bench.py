@@ -894,8 +894,16 @@ def run_masks(args):
         tk, _ = ibp.ibp_mask_sweep_device(xs.data_ptr(), ibp.table_desc(nk, rb, ibp.IBP_GROUP_MAP, 0, k, assign.data_ptr()), None, 0, [(4, 5)], [4], st)
         fig15[str(k)] = {"net_space_saved_pct": round(100.0 * (1 - (int(tk[0, 0]) + 2 * rb * used) / (nk * rb)), 2), "clusters_used": used,
                          "ms_4_iterations": round(e0.elapsed_time(e1), 2), "cost": [int(c) for c in cost.cpu().tolist()]}
-    cpu = None if args.no_cpu else {"value": round(len(sample) * rb / t_or * 1e-9, 6), "unit": "GB/s", "cores": 1, "kind": "oracle",
-                                    "sample": f"oracle/mask_tools.bit_counters on {len(sample)} sampled rows of the {w.name} table, {t_or:.1f} s"}
+    cpu = None
+    if not args.no_cpu:                                                # the oracle's counting pass on successive slices, about 12 s
+        t0 = time.perf_counter()
+        done = 0
+        while time.perf_counter() - t0 < 12.0 and done + 20000 <= n:
+            mt.bit_counters(Xb[done:done + 20000], np.zeros(20000, np.int64), 1)
+            done += 20000
+        dt = time.perf_counter() - t0
+        cpu = {"value": round(done * rb / dt * 1e-9, 6), "unit": "GB/s", "cores": 1, "kind": "oracle",
+               "sample": f"oracle/mask_tools.bit_counters (P:229, one row at a time) on the first {done} rows of the {w.name} table, {dt:.1f} s"}
     line = {
         "metric": "preprocessing throughput, raw GB/s (per-bit counters + compressed sizes of the whole table)", "value": round(raw / ((ms_cnt + ms_sz) * 1e-3) * 1e-9, 1),
         "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": round(ms_cnt + ms_sz, 4), "higher_is_better": True, "scaling": "weak",
