@@ -661,16 +661,18 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
         P.piece_rows = U;
         need = rc * h->max_stride + (rc / G + 2) * 128 + 64;
         P.chunks_per_span = (uint32_t)((span_rows + (int64_t)rc - 1) / (int64_t)rc);
-    } else if (resident && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1 && (!h->max_ctas || h->max_ctas >= (G + NW - 1) / NW)) {
+    } else if (resident && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1 && (!h->max_ctas || h->max_ctas >= (h->n_groups + NW - 1) / NW)) {
         // resident decode of a strided table: tile-block chunks (ibp_stream.cuh).  A whole-row chunk holds only 2-7 matrix rows
         // of the 7B shapes, so every warp would re-prepare a tile (Mask/Bitval, offsets, expand masks) for a handful of rows;
         // here a CTA keeps one block of NW tiles for all its chunks and prepares once.  The source is HBM, so the shorter
         // contiguous reads (one block of one matrix row per bulk copy) cost nothing; the host-store path keeps whole rows.
-        const uint32_t n_tb = (uint32_t)((G + NW - 1) / NW);
+        const uint64_t n_tiles = h->n_groups;                      // min(S, rows): the group table ends there
+        const uint32_t n_tb = (uint32_t)((n_tiles + NW - 1) / NW);
+        P.n_tiles = (uint32_t)n_tiles;
         uint64_t max_len = 0;
         for (uint32_t tb = 0; tb < n_tb; ++tb) {
             const IbpGroupEntry& e0 = h->gtab[(uint64_t)tb * NW];
-            const IbpGroupEntry& e1 = h->gtab[std::min<uint64_t>(G, (uint64_t)tb * NW + NW) - 1];
+            const IbpGroupEntry& e1 = h->gtab[std::min<uint64_t>(n_tiles, (uint64_t)tb * NW + NW) - 1];
             max_len = std::max<uint64_t>(max_len, e1.base + e1.stride - e0.base);
         }
         const uint64_t pitch = (max_len + 31 + 15) / 16 * 16;
@@ -712,10 +714,10 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
 
 // Thresholded-mode contiguous runs through ibp_stream_t_kernel.  Returns IBP_ERR_UNSUPPORTED (without setting an error
 // the caller would report) when the shape does not fit: the caller then uses the per-row kernel.
-template <int W, int NS>
+template <int W, int NS, bool RUNS>
 static ibp_status launch_stream_t_one(const StreamTParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
     constexpr int NW = 8;
-    auto kern = ibp_stream_t_kernel<W, NS, NW>;
+    auto kern = ibp_stream_t_kernel<W, NS, NW, RUNS>;
     static thread_local size_t attr_smem = 0;
     if (smem > 48 * 1024 && smem > attr_smem) {
         IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -780,9 +782,12 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
     const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
     if (smem > 220 * 1024) { ibp_set_error("thresholded rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
-#define IBP_STREAM_T(W_)                                                                          \
-    return ns == 2 ? launch_stream_t_one<W_, 2>(P, h->max_ctas, h->sm_count, smem, st)            \
-                   : launch_stream_t_one<W_, 3>(P, h->max_ctas, h->sm_count, smem, st)
+    const bool runs = h->max_runs >= 0 && h->max_runs <= 3;
+#define IBP_STREAM_T(W_)                                                                                         \
+    if (runs) return ns == 2 ? launch_stream_t_one<W_, 2, true>(P, h->max_ctas, h->sm_count, smem, st)           \
+                             : launch_stream_t_one<W_, 3, true>(P, h->max_ctas, h->sm_count, smem, st);          \
+    return ns == 2 ? launch_stream_t_one<W_, 2, false>(P, h->max_ctas, h->sm_count, smem, st)                    \
+                   : launch_stream_t_one<W_, 3, false>(P, h->max_ctas, h->sm_count, smem, st)
     switch (W) {
         case 4: IBP_STREAM_T(4);
         case 2: IBP_STREAM_T(2);
@@ -832,6 +837,22 @@ ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream) {
         IBP_CUDA(cudaGetLastError());
     }
     IBP_CUDA(cudaStreamSynchronize(st));
+    if (h->max_runs < 0) {
+        // most runs of variant bits in any Mask word: at most three everywhere lets the thresholded stream kernel re-insert bits
+        // run by run (2 operations per run) instead of through the five-stage expand
+        int mr = 0;
+        const int64_t ng = (int64_t)h->n_groups;
+        const uint32_t nw = h->n_words;
+#pragma omp parallel for reduction(max : mr) schedule(static)
+        for (int64_t g = 0; g < ng; ++g) {
+            const uint32_t* mk = &h->meta[(uint64_t)g * 2 * nw];
+            for (uint32_t w = 0; w < nw; ++w) {
+                const uint32_t nv = ~mk[w];
+                mr = std::max(mr, __builtin_popcount(nv & ~(nv << 1)));
+            }
+        }
+        h->max_runs = mr;
+    }
     h->sm_count = prop.multiProcessorCount;
     if (h->store_kind == IBP_STORE_PINNED && !h->store_dev) {
         void* dptr = nullptr;

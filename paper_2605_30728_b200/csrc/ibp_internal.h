@@ -45,6 +45,7 @@ struct ibp_handle {
     uint32_t* meta_dev = nullptr;
     IbpGroupEntry* gtab_dev = nullptr;
     uint32_t* mvtab_dev = nullptr;         // optional expand move masks, 5 per (group, word)
+    int max_runs = -1;                     // most runs of variant bits in any Mask word of the table (set by ibp_attach_device)
 
     // ibp_build_device only
     bool built_on_device = false;

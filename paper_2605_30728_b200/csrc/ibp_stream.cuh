@@ -33,6 +33,7 @@ struct StreamParams {
     // tiles, and chunk c belongs to block c % n_tile_blocks -- with a grid that is a multiple of n_tile_blocks every CTA
     // keeps ONE block, so consumer warp w decodes the same tile in every chunk and prepares it once.  0 = off.
     uint32_t n_tile_blocks;
+    uint32_t n_tiles;              // groups that exist: min(S, rows of the table) -- the group table has no entry beyond them
     uint32_t tb_pitch;             // bytes between the block's images of consecutive matrix rows inside a stage
 };
 
@@ -134,7 +135,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 const uint32_t s = k % NS;
                 mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
                 const uint32_t tb = (uint32_t)c % P.n_tile_blocks, rbk = (uint32_t)c / P.n_tile_blocks;
-                const uint32_t t0 = tb * NW, t1 = min((uint32_t)S, t0 + NW);
+                const uint32_t t0 = tb * NW, t1 = min(P.n_tiles, t0 + NW);
                 const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
                 const int64_t mr0 = (int64_t)rbk * P.rows_per_chunk;
                 const uint32_t nrows = (uint32_t)min((int64_t)P.rows_per_chunk, n_mrows - mr0);
@@ -289,7 +290,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     if (P.n_tile_blocks) {
         // tile-block mode: this CTA's chunks all carry tile block blockIdx.x % n_tile_blocks; warp wib owns one tile of it
         const uint32_t tb = blockIdx.x % P.n_tile_blocks, t = tb * NW + wib;
-        const bool has_tile = t < (uint32_t)S;
+        const bool has_tile = t < P.n_tiles;
         uint32_t toff = 0;
         if (has_tile) {
             const IbpGroupEntry e0 = P.gtab[tb * NW], e = P.gtab[t];

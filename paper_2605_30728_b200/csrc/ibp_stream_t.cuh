@@ -28,7 +28,9 @@ struct StreamTParams {
     uint32_t stage_bytes;
 };
 
-template <int W, int NS, int NW>
+// RUNS: every word of every group of the table has at most three runs of variant bits (decided once per handle on the host):
+// bits are re-inserted run by run (ibp_stream.cuh) instead of through the five-stage expand.
+template <int W, int NS, int NW, bool RUNS>
 __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const StreamTParams P) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -75,7 +77,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
     }
 
     // ---------------------------------------------------------------------- consumers
-    uint32_t m[W], b[W], kq[W], ex[W], mv[W][5];
+    // mv: the group's bit re-insertion state per word: RUNS -- mv[q][j] = multiplier 2^(p_j - c_j), mv[q][3+j] = mask of run j
+    // (j < 3); else the five expand move masks.
+    uint32_t m[W], b[W], kq[W], ex[W], mv[W][RUNS ? 6 : 5];
     uint64_t prep_g = ~0ull;
     const uint32_t w0 = lane * W;
     const bool active = w0 < P.n_words;
@@ -94,16 +98,42 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
         const uint32_t incl = warp_inclusive_scan(t, lane);
 #pragma unroll
         for (int q = 0; q < W; ++q) ex[q] += P.n_words + incl - t;            // payloads follow the participation bits
+        if constexpr (RUNS) {
 #pragma unroll
-        for (int q = 0; q < W; ++q) {
-            if (q > 0 && m[q] == m[q - 1]) {
+            for (int q = 0; q < W; ++q) {
+                uint32_t nv = ~m[q], c = 0;
 #pragma unroll
-                for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
-            } else {
-                expand_masks(~m[q], mv[q]);
+                for (int j = 0; j < 3; ++j) {
+                    const uint32_t low = nv & (0u - nv), run = nv & ~(nv + low);     // nv == 0 -> low = run = 0
+                    mv[q][j] = run ? 1u << ((__ffs(low) - 1) - c) : 0u;
+                    mv[q][3 + j] = run;
+                    c += __popc(run);
+                    nv &= ~run;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                if (q > 0 && m[q] == m[q - 1]) {
+#pragma unroll
+                    for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+                } else {
+                    expand_masks(~m[q], mv[q]);
+                }
             }
         }
         prep_g = g;
+    };
+    // the chunk's bits x (variant bits at bit 0 upwards) back at the Mask = 0 positions, Bitval elsewhere
+    auto reinsert = [&](uint32_t x, int q) -> uint32_t {
+        if constexpr (RUNS) {
+            uint32_t acc = b[q];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) acc = and_or(x * mv[q][j], mv[q][RUNS ? 3 + j : 0], acc);
+            return acc;
+        } else {
+            return bitselect(b[q], expand_bits(x, mv[q]), m[q]);
+        }
     };
 
     // one row of the prepared group: packed bytes at shared address saddr, `comp` = the row's bit of the bitmask
@@ -135,13 +165,55 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
                 uint32_t lo, hi;
                 asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(saddr + (bit[q] >> 5) * 4u));
                 const uint32_t x = __funnelshift_r(lo, hi, bit[q] & 31u);
-                const uint32_t e = bitselect(b[q], expand_bits(x, mv[q]), m[q]);
+                const uint32_t e = reinsert(x, q);
                 o[q] = ((part >> q) & 1u) ? e : x;                             // non-participating chunk: all 32 bits
             }
         }
         if (active) VecIO<W>::st(orow + (size_t)w0 * 4, o);
     };
 
+    // RB compressed rows of the prepared group at once.  One row is a chain of dependent steps -- participation read, kept-bit
+    // counts, the 5-step shuffle scan of P:319 step 3, the extraction loads, the expand -- of about 1,200 cycles, and with two
+    // warps per scheduler nothing hides it (measured: the same 7.6 us per 96-row chunk whether the SM runs one CTA or two).
+    // Written out for RB rows side by side, the chains are independent and the scheduler interleaves them.
+    constexpr int RB = 4;
+    auto decode_rows = [&](const uint32_t* saddr, uint8_t* orow) {
+        uint32_t part[RB], tl[RB], incl[RB], bit[RB][W];
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            part[i] = pmask;
+            if (active) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(part[i]) : "r"(saddr[i] + (w0 >> 5) * 4u)); part[i] = (part[i] >> (w0 & 31u)) & pmask; }
+        }
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            uint32_t t = 0;
+#pragma unroll
+            for (int q = 0; q < W; ++q) { bit[i][q] = t; t += active ? (((part[i] >> q) & 1u) ? kq[q] : 32u) : 0u; }
+            tl[i] = t; incl[i] = t;
+        }
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+#pragma unroll
+            for (int i = 0; i < RB; ++i) {
+                const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl[i], d);
+                if (lane >= d) incl[i] += v;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            uint32_t o[W];
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                const uint32_t bq = bit[i][q] + P.n_words + incl[i] - tl[i];
+                uint32_t lo, hi;
+                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(saddr[i] + (bq >> 5) * 4u));
+                const uint32_t x = __funnelshift_r(lo, hi, bq & 31u);
+                const uint32_t e = reinsert(x, q);
+                o[q] = ((part[i] >> q) & 1u) ? e : x;
+            }
+            if (active) VecIO<W>::st(orow + (size_t)i * P.row_bytes + (size_t)w0 * 4, o);
+        }
+    };
     // Row offsets and raw flags of a piece (lane r <-> row id0 + r): one coalesced load each.  The loads for a warp's FIRST
     // piece of its next chunk are issued before the current chunk is decoded, so their latency (an HBM/L2 round trip in
     // front of every piece otherwise: ncu showed long-scoreboard as the top stall) overlaps the decode.
@@ -188,12 +260,23 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
                 if (p != (uint32_t)wib) load_piece(id0, cnt, my_off, my_flag);   // later pieces of the chunk: on demand
                 const uint32_t flags = __ballot_sync(0xFFFFFFFFu, my_flag);
                 uint8_t* orow = P.out + (uint64_t)(out0 + j0) * P.row_bytes;
-                for (uint32_t r = 0; r < cnt; ++r, orow += P.row_bytes) {
+                uint32_t r = 0;
+                while (r < cnt) {
                     const uint64_t g = group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + r));
                     if (g != prep_g) prepare(g);
                     if (!waited) { mbar_wait(full_s + s * 8, (k / NS) & 1u); waited = true; }
-                    const uint32_t roff = (__shfl_sync(0xFFFFFFFFu, my_off, r) - base_off) * 16u;
-                    decode_row(stage_s + roff, (flags >> r) & 1u, orow);
+                    if (r + RB <= cnt && ((flags >> r) & ((1u << RB) - 1u)) == ((1u << RB) - 1u) &&
+                        group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + r + RB - 1)) == g) {
+                        uint32_t sa[RB];                                   // RB compressed rows of one group
+#pragma unroll
+                        for (int i = 0; i < RB; ++i) sa[i] = stage_s + (__shfl_sync(0xFFFFFFFFu, my_off, r + i) - base_off) * 16u;
+                        decode_rows(sa, orow);
+                        r += RB; orow += (size_t)RB * P.row_bytes;
+                    } else {
+                        const uint32_t roff = (__shfl_sync(0xFFFFFFFFu, my_off, r) - base_off) * 16u;
+                        decode_row(stage_s + roff, (flags >> r) & 1u, orow);
+                        r += 1; orow += P.row_bytes;
+                    }
                 }
             }
         } else {
