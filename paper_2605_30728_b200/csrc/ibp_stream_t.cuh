@@ -176,7 +176,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
     // counts, the 5-step shuffle scan of P:319 step 3, the extraction loads, the expand -- of about 1,200 cycles, and with two
     // warps per scheduler nothing hides it (measured: the same 7.6 us per 96-row chunk whether the SM runs one CTA or two).
     // Written out for RB rows side by side, the chains are independent and the scheduler interleaves them.
-    constexpr int RB = 4;
+    constexpr int RB = W == 4 ? 2 : 4;   // W = 4: four rows side by side spill under the two-CTAs-per-SM register budget
     auto decode_rows = [&](const uint32_t* saddr, uint8_t* orow) {
         uint32_t part[RB], tl[RB], incl[RB], bit[RB][W];
 #pragma unroll
