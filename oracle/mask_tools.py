@@ -19,6 +19,10 @@ What the paper defines (PAPER.md line numbers):
   net_space_saved       "space savings due to compression minus metadata overhead for additional Mask and Bitval" (P:544):
                          1 - (sum of compressed row sizes + 2 * row_bytes * clusters) / (n_rows * row_bytes).
 
+Parity unpinned: the READING R25 of "bit-similarity k-means" (P:542 is one sentence, the paper prints no worked example): the
+pins below check this implementation of the reading, not that the authors' code takes the same distance and tie rules; and every
+number of Fig. 13 / Table 5 / Fig. 15, which needs the paper's datasets.
+
 Pins (tests/test_oracle_mask_tools.py): brute force with Python integers on tiny inputs; the closed form of the counters
 of a full enumeration (2^(k-1)); tau = 1 == the AND/OR form; the participation overheads the paper prints (12.5 % at
 CS = 1 B, 1.6 % at CS = 8 B); Lloyd monotonicity; exact recovery of planted clusters.
