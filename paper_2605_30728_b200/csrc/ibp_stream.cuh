@@ -7,9 +7,14 @@
 //             Host store: the link sees long contiguous reads instead of one short read per row.  HBM source: same code.
 //   consumers NW warps wait on the full mbarrier, decode "pieces" of the chunk (rows of one group: Mask/Bitval, bit
 //             offsets and the five bit-expand move masks live in registers for the whole piece), then release the stage.
-// Bit re-insertion (S5) is the branch-free 5-stage expand of Hacker's Delight 7-5 (x = (x & ~mv_i) | ((x << 2^i) & mv_i)):
-// 11 integer ops per 32-bit word whatever the mask looks like, with the move masks computed once per piece, or loaded
-// from a per-group table built at upload time when the table has few groups (strided column-tile tables).
+// Bit re-insertion (S5), chosen per group from its masks (warp-uniform):
+//   - at most three runs of variant bits in every word (float data: mantissa run, exponent run, sign): run-wise deposit, one
+//     multiply by 2^(p_j - c_j) and one lop3 and-or with the run's mask per run, starting from Bitval (2-6 ops per word);
+//   - otherwise the branch-free parallel-suffix expand of Hacker's Delight 7-5 (x = (x & ~mv_i) | ((x << 2^i) & mv_i)) with 3, 4
+//     or 5 stages depending on the largest move, the move masks computed once per piece or loaded from a per-group table built
+//     at upload time when the table has few groups (strided column-tile tables).
+// Strided tables decoded from HBM use tile-block chunks (StreamParams::n_tile_blocks): a CTA keeps one block of NW column tiles
+// for all its chunks, so a consumer warp prepares its tile once.
 #pragma once
 
 struct StreamParams {
@@ -170,8 +175,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     // ---------------------------------------------------------------------- consumers
     // Fast path (single-pass rows whose packed bytes start on a 4-byte boundary, i.e. A >= 4): everything that depends
     // only on the group is hoisted out of the row loop -- Mask/Bitval, the word offset and shift of each of the lane's W
-    // words inside a packed row, the five expand masks -- and the row loop is: 2 ld.shared + 1 funnel shift + 11 logic
-    // ops per word, one vector store, two pointer bumps.
+    // words inside a packed row, the run multipliers and masks or the expand masks -- and the row loop is: 2 ld.shared + 1
+    // funnel shift + 2-12 integer ops per word, one vector store, two pointer bumps.
     // Per-group decode state of the lane's W words.  Two forms, chosen per group (warp-uniform `mode`):
     //   runs (mode 1..3): every word of the group has at most 3 runs of variant bits (float data: a mantissa run, an exponent run,
     //     the sign).  Run j takes bits [c_j, c_j+len_j) of the extracted word to positions [p_j, p_j+len_j): one multiply by
