@@ -397,3 +397,14 @@ def test_T_edge_cases_and_spans():
         hk.set_stream_mode(sm)
         assert np.array_equal(_gather(hk, ids, span=w.index_span), oracle.gather_plain(Xk, ids, w.index_span))
     hk.destroy()
+
+
+def test_link_probes():
+    """The ceilings bench.py reports are measured by the library itself: sane values and argument checks."""
+    sps, gbs = ibp.ibp_measure_random_read(0, 64 << 20, 128, 1)
+    assert sps > 1e7 and abs(gbs - sps * 128e-9) < 1e-6 * gbs + 1e-9
+    assert 5 < ibp.ibp_measure_zero_copy_read(0, 64 << 20, 1) < 200
+    for bad in [(64 << 20, 100), (64 << 20, 1024), (1 << 10, 128)]:
+        with pytest.raises(ibp.IbpError) as e:
+            ibp.ibp_measure_random_read(0, bad[0], bad[1], 1)
+        assert e.value.status == 1
