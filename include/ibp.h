@@ -373,6 +373,14 @@ ibp_status ibp_kmeans_bits_device(const void* rows_dev, uint64_t n_rows, uint32_
                                   const int64_t* init_ids_dev, uint32_t iters, uint32_t* assign_dev, void* centroids_dev,
                                   uint64_t* cost_dev, void* cuda_stream);
 
+/* Rows ordered by group: a counting sort of the row ids by row_group_dev (each < n_groups).  order_dev[0..n_rows) becomes a
+ * permutation of the row ids in which the rows of group 0 come first, then group 1, ...; the order inside a group is
+ * unspecified.  group_start_dev (may be NULL): n_groups + 1 offsets into order_dev.  Use: reorder a table so that the clusters
+ * of ibp_kmeans_bits_device become runs of consecutive rows, then build it with blocked groups -- clustered compression
+ * with this library's positional groups; ids are mapped through the inverse permutation by the caller.        */
+ibp_status ibp_order_by_group_device(const uint32_t* row_group_dev, uint64_t n_rows, uint32_t n_groups, int64_t* order_dev,
+                                     uint32_t* group_start_dev, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -115,6 +115,7 @@ SIGNATURES = {
     "ibp_compressed_size_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _vp, _u32, _vp, _vp, _vp]),
     "ibp_mask_sweep_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _i64, _vp, _u32, _vp, _u32, _vp, _vp, _vp]),
     "ibp_kmeans_bits_device": (_int, [_vp, _u64, _u32, _u32, _vp, _u32, _vp, _vp, _vp, _vp]),
+    "ibp_order_by_group_device": (_int, [_vp, _u64, _u32, _vp, _vp, _vp]),
 }
 
 _lib = None
@@ -432,6 +433,10 @@ def ibp_mask_sweep_device(rows_dev, t, sample_ids_dev, n_sample, taus, chunk_byt
 def ibp_kmeans_bits_device(rows_dev, n_rows, row_bytes, k, init_ids_dev, iters, assign_dev, centroids_dev, cost_dev=None, stream=None):
     _check(lib().ibp_kmeans_bits_device(_ptr(rows_dev), n_rows, row_bytes, k, _ptr(init_ids_dev), iters, _ptr(assign_dev),
                                         _ptr(centroids_dev), _ptr(cost_dev), stream))
+
+
+def ibp_order_by_group_device(row_group_dev, n_rows, n_groups, order_dev, group_start_dev=None, stream=None):
+    _check(lib().ibp_order_by_group_device(_ptr(row_group_dev), n_rows, n_groups, _ptr(order_dev), _ptr(group_start_dev), stream))
 
 
 def ibp_version() -> str:

@@ -682,3 +682,29 @@ extern "C" ibp_status ibp_kmeans_bits_device(const void* rows_dev, uint64_t n_ro
     cudaFreeAsync(counts, st); cudaFreeAsync(gn, st); cudaFreeAsync(hist, st); cudaFreeAsync(cursor, st); cudaFreeAsync(order, st);
     return s;
 }
+
+extern "C" ibp_status ibp_order_by_group_device(const uint32_t* row_group_dev, uint64_t n_rows, uint32_t n_groups, int64_t* order_dev,
+                                                uint32_t* group_start_dev, void* cuda_stream) {
+    if (!row_group_dev || !order_dev || n_rows == 0 || n_groups == 0 || n_rows > 0xFFFFFFFFull) {
+        ibp_set_error("ibp_order_by_group_device: null or empty argument (at most 2^32 - 1 rows)"); return IBP_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint32_t *hist = nullptr, *cursor = nullptr;
+    IBP_CUDA(cudaMallocAsync((void**)&hist, (uint64_t)n_groups * 4, st));
+    IBP_CUDA(cudaMallocAsync((void**)&cursor, (uint64_t)n_groups * 4, st));
+    IBP_CUDA(cudaMemsetAsync(hist, 0, (uint64_t)n_groups * 4, st));
+    const int grid = analysis_grid((n_rows + 31) / 32);
+    ibp_cluster_hist<<<grid, 256, 0, st>>>(row_group_dev, n_rows, hist);
+    ibp_cluster_scan<<<1, 1024, 0, st>>>(hist, n_groups, cursor);
+    IBP_CUDA(cudaGetLastError());
+    if (group_start_dev) {
+        const uint32_t last = (uint32_t)n_rows;
+        IBP_CUDA(cudaMemcpyAsync(group_start_dev, cursor, (uint64_t)n_groups * 4, cudaMemcpyDeviceToDevice, st));
+        IBP_CUDA(cudaMemcpyAsync(group_start_dev + n_groups, &last, 4, cudaMemcpyHostToDevice, st));
+        IBP_CUDA(cudaStreamSynchronize(st));      // `last` lives on this stack frame
+    }
+    ibp_cluster_scatter<<<grid, 256, 0, st>>>(row_group_dev, n_rows, cursor, order_dev);
+    IBP_CUDA(cudaGetLastError());
+    cudaFreeAsync(hist, st); cudaFreeAsync(cursor, st);
+    return IBP_OK;
+}

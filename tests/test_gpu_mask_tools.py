@@ -212,3 +212,58 @@ def test_bad_arguments():
         ibp.ibp_mask_sweep_device(X.data_ptr(), ibp.table_desc(8, 18, 0, 4), None, 0, [(4, 5)], [4], _st())
     with pytest.raises(ibp.IbpError):
         ibp.ibp_table_groups(ibp.table_desc(8, 16, ibp.IBP_GROUP_MAP, 0, 0, None))
+
+
+def test_order_by_group_is_a_grouped_permutation():
+    """Several correct answers exist (the order inside a group is unspecified): check what is unique -- a permutation, groups in
+    ascending order, the group offsets -- incl. empty groups."""
+    n, k = 50_000, 37
+    grp = np.random.default_rng(2).integers(0, k, n).astype(np.uint32)
+    grp[grp == 5] = 6                                          # an empty group
+    gd = torch.from_numpy(grp).cuda()
+    order = torch.zeros(n, dtype=torch.int64, device="cuda")
+    start = torch.zeros(k + 1, dtype=torch.int32, device="cuda")
+    ibp.ibp_order_by_group_device(gd.data_ptr(), n, k, order.data_ptr(), start.data_ptr(), _st())
+    torch.cuda.synchronize()
+    o = order.cpu().numpy()
+    assert np.array_equal(np.sort(o), np.arange(n))
+    assert np.all(np.diff(grp[o].astype(np.int64)) >= 0)
+    assert np.array_equal(start.cpu().numpy().astype(np.int64), np.concatenate([[0], np.cumsum(np.bincount(grp, minlength=k))]))
+
+
+def test_clustered_store_through_reordering():
+    """Clustered compression end to end with positional groups: k-means on the interleaved GNN variant (reading R15),
+    rows reordered so that clusters are runs of consecutive rows, blocked groups of 256 over the reordered table, ids mapped
+    through the inverse permutation.  The gather returns the original rows (plain definition), and the reordered table
+    compresses better than the table in its original order."""
+    w = workloads.GNN(n_rows=32_768, batch=4096, interleaved=True)
+    X = w.table()
+    Xb = np.ascontiguousarray(X).view(np.uint8).reshape(w.n_rows, -1)
+    n, rb = Xb.shape
+    sparse = ((X == 0) | (X == 1)).all(axis=1)
+    init = np.array([int(np.flatnonzero(~sparse)[0]), int(np.flatnonzero(sparse)[0])], np.int64)
+    xd = torch.from_numpy(Xb).cuda()
+    idd = torch.from_numpy(init).cuda()
+    assign = torch.zeros(n, dtype=torch.int32, device="cuda")
+    cent = torch.zeros((2, rb), dtype=torch.uint8, device="cuda")
+    ibp.ibp_kmeans_bits_device(xd.data_ptr(), n, rb, 2, idd.data_ptr(), 3, assign.data_ptr(), cent.data_ptr(), None, _st())
+    order = torch.zeros(n, dtype=torch.int64, device="cuda")
+    ibp.ibp_order_by_group_device(assign.data_ptr(), n, 2, order.data_ptr(), None, _st())
+    torch.cuda.synchronize()
+    assert np.array_equal(assign.cpu().numpy().astype(bool), sparse)             # the two row types are the two clusters
+    o = order.cpu().numpy()
+    inv = np.empty(n, np.int64)
+    inv[o] = np.arange(n)
+    h0 = ibp.ibp_build(Xb, rb, 0, 256, align_bytes=32, flags=ibp.IBP_FLAG_PAGEABLE_STORE)
+    h1 = ibp.ibp_build(np.ascontiguousarray(Xb[o]), rb, 0, 256, align_bytes=32).upload_metadata(0)
+    r0 = Xb.nbytes / h0.info().packed_bytes_rows
+    r1 = Xb.nbytes / h1.info().packed_bytes_rows
+    assert r1 > 1.1 * r0, (r0, r1)
+    ids = w.ids(0)
+    ids_d = torch.from_numpy(inv[ids]).cuda()
+    out = torch.zeros((len(ids), rb), dtype=torch.uint8, device="cuda")
+    h1.gather_decompress(ids_d.data_ptr(), len(ids), out.data_ptr(), _st())
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle.gather_plain(Xb, ids))
+    h0.destroy()
+    h1.destroy()
