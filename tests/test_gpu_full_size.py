@@ -160,3 +160,48 @@ def test_full_dlrm_thresholded():
     touched = np.unique(ids // 128)
     _check_T_codec_on_groups(h, X, list(touched[:5]) + list(touched[-5:]), 128, (4, 5))
     h.destroy()
+
+
+def test_kv_thresholded_spans_and_resident():
+    """configs[3]'s shape (8 of the 32 layers: 4.3 GB) under the paper's default codec: page spans through the thresholded
+    stream kernel (expand form: 16-row groups of bf16 pairs have words with four runs of variant bits; four rows decoded side by
+    side), a staged page range from HBM, sampled groups against the oracle codec."""
+    w = workloads.KV(layers=8)
+    X = w.table()
+    h = ibp.ibp_build(X, 256, 0, 16, align_bytes=16, index_span=512, threshold=(4, 5)).upload_metadata(0)
+    assert h.info().thresholded == 1
+    ids = w.ids(0)
+    got = _gather(h, ids, len(ids) * 512, 256)
+    assert np.array_equal(got, oracle.gather_plain(X, ids, 512))
+    first_rows = ids[:4] * 512
+    _check_T_codec_on_groups(h, X, [int(r // 16) + j for r in first_rows for j in (0, 31)], 16, (4, 5))
+    st = torch.cuda.current_stream().cuda_stream
+    first, n = int(ids[5]) * 512, 6 * 512
+    ptr, nbytes = h.packed_range(first, n)
+    packed = torch.from_numpy(h.packed_view(ptr, nbytes).copy()).cuda()
+    out = torch.empty((n, 256), dtype=torch.uint8, device="cuda")
+    h.decompress_resident(packed.data_ptr(), first, n, out.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), _u8(X)[first:first + n])
+    h.destroy()
+
+
+def test_weight_matrix_thresholded_stream_and_resident():
+    """One 4096 x 11008 bf16 matrix of configs[4] (86 column tiles as strided groups) under tau = 0.8: whole-matrix range gather
+    from the host store and resident decode, both through the thresholded stream kernel's strided branch."""
+    w = workloads.WeightMatrix(rows=4096, cols=11008)
+    X = w.table()
+    n = w.n_rows
+    h = ibp.ibp_build(X, 256, 1, w.group_param, align_bytes=16, threshold=(4, 5)).upload_metadata(0)
+    st = torch.cuda.current_stream().cuda_stream
+    out = torch.empty((n, 256), dtype=torch.uint8, device="cuda")
+    h.gather_decompress_range(0, n, out.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), _u8(X))
+    ptr, nbytes = h.packed_range(0, n)
+    packed = torch.from_numpy(h.packed_view(ptr, nbytes).copy()).cuda()
+    out.zero_()
+    h.decompress_resident(packed.data_ptr(), 0, n, out.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), _u8(X))
+    h.destroy()
