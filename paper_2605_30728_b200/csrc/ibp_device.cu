@@ -48,6 +48,7 @@ struct DecodeParams {
     uint32_t rows_per_unit, units_per_span;
     uint32_t slot_bytes;
     uint32_t strided;              // group kind of the handle (MODE_ROWS serves both kinds)
+    uint32_t occ_cap;              // host side only: CTAs per SM for random-row gathers (0 = 2)
     const uint32_t* row_off;       // thresholded mode: per-row offsets (16-byte units), n_rows + 1 entries
     const uint32_t* row_flag;      // thresholded mode: bit r = 1 iff row r is compressed
     uint32_t keep_l2;              // write the rows with the default cache policy (a later pass re-reads them) instead of streaming
@@ -532,7 +533,7 @@ static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
     // random rows: 2 CTAs per SM keep enough reads in flight for the link; more only widens the window of store pages touched
     // at once (measured: DLRM 0.716 -> 0.685 ms, GNN 1.388 -> 1.375 ms per batch)
-    if (MODE == MODE_ROWS) occ = std::min(occ, 2);
+    if (MODE == MODE_ROWS) occ = std::min(occ, P.occ_cap ? (int)P.occ_cap : 2);
     int64_t blocks = std::min<int64_t>(blocks_needed, (int64_t)std::max(occ, 1) * sm_count);
     if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
     kern<<<(int)blocks, wpc * 32, smem, st>>>(P);
@@ -896,6 +897,11 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
         P.cmap = c->map_dev;
         P.cmap_mask = c->map_cap - 1;
         for (int s = 0; s < 8; ++s) P.slab[s] = c->slab_dev[s];
+        // A cache that holds a sizeable share of the table serves most rows from HBM slabs: those are latency-bound (map probe,
+        // then the bulk copy), so every resident CTA helps (DLRM, 10 % of the rows cached: 357 -> 414 GB/s; 60 %: 361 -> 520).
+        // A small cache leaves the misses in charge, and for them a wider window of store pages in flight costs more than it
+        // gains (DLRM, 2 %: 314 -> 280 GB/s with 4 CTAs per SM), so the cap of the uncached gather stays.
+        if (c->n_entries * 12 >= h->p.n_rows) P.occ_cap = 4;
     }
     const bool dedup = allow_dedup && (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
     // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
