@@ -415,24 +415,38 @@ static void bucket_shape(uint64_t n_rows, uint64_t store_bytes, uint64_t target,
 __global__ void ibp_dedup_insert(const int64_t* __restrict__ ids, int64_t n, unsigned long long* __restrict__ table, uint32_t mask,
                                  int32_t* __restrict__ rep, int32_t* __restrict__ uniq, uint32_t* __restrict__ n_uniq,
                                  uint32_t* __restrict__ cnt, uint32_t shift, uint32_t nb) {
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const uint64_t key = (uint64_t)ids[i];
-        uint32_t slot = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 32) & mask;
-        const unsigned long long mine = ((key + 1) << 32) | (uint32_t)i;     // 0 = empty slot
-        int32_t r;
-        for (;;) {
-            unsigned long long cur = table[slot];
-            if (cur == 0ull) cur = atomicCAS(&table[slot], 0ull, mine);
-            if (cur == 0ull) {
-                r = (int32_t)i;
-                uniq[atomicAdd(n_uniq, 1u)] = (int32_t)i;
-                if (cnt) { const uint64_t bk = key >> shift; atomicAdd(&cnt[bk < nb ? bk : nb - 1], 1u); }   // locality histogram
-                break;
+    const int lane = threadIdx.x & 31;
+    // warp-uniform trip count, so that the winners of a warp can claim their work-list slots with ONE atomicAdd on the shared
+    // counter (a batch has ~10^5 winners: one same-address atomic each was the longest chain of this kernel)
+    for (int64_t base = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) - lane; base < n; base += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = base + lane;
+        bool won = false;
+        if (i < n) {
+            const uint64_t key = (uint64_t)ids[i];
+            uint32_t slot = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 32) & mask;
+            const unsigned long long mine = ((key + 1) << 32) | (uint32_t)i;     // 0 = empty slot
+            int32_t r;
+            for (;;) {
+                unsigned long long cur = table[slot];
+                if (cur == 0ull) cur = atomicCAS(&table[slot], 0ull, mine);
+                if (cur == 0ull) {
+                    r = (int32_t)i;
+                    won = true;
+                    if (cnt) { const uint64_t bk = key >> shift; atomicAdd(&cnt[bk < nb ? bk : nb - 1], 1u); }   // locality histogram
+                    break;
+                }
+                if ((cur >> 32) == key + 1) { r = (int32_t)(uint32_t)cur; break; }
+                slot = (slot + 1) & mask;
             }
-            if ((cur >> 32) == key + 1) { r = (int32_t)(uint32_t)cur; break; }
-            slot = (slot + 1) & mask;
+            rep[i] = r;
         }
-        rep[i] = r;
+        const uint32_t winners = __ballot_sync(0xFFFFFFFFu, won);
+        if (winners) {
+            uint32_t first = 0;
+            if (lane == __ffs(winners) - 1) first = atomicAdd(n_uniq, (uint32_t)__popc(winners));
+            first = __shfl_sync(0xFFFFFFFFu, first, __ffs(winners) - 1);
+            if (won) uniq[first + __popc(winners & ((1u << lane) - 1u))] = (int32_t)i;
+        }
     }
 }
 // LPR lanes per row (a power of two, 16 bytes per lane and trip): a 256-byte row keeps half a warp busy, so a warp copies two.
