@@ -164,7 +164,12 @@ ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_ids_dev, int6
 
 /* Same result with HOST buffers: row_ids_host (n int64) is copied to the device, the gather runs, and the rows are
  * copied back into out_host, all on the stream, which is synchronised before returning.  The end-to-end entry point
- * bench.py times.  The buffers should be pinned for full copy speed; pageable memory works.                        */
+ * bench.py times.  The buffers should be pinned for full copy speed; pageable memory works.
+ * Paths: a batch the library would de-duplicate (ibp_set_dedup_mode: mode 1, or automatic and n >= 16384) is gathered into a
+ * device staging buffer -- every distinct row crosses PCIe once -- and copied out in chunks; any other batch whose out_host is
+ * pinned and GPU-mapped is decoded straight into out_host by the kernel (nothing staged; every id is fetched, which is what
+ * the handle's de-duplication setting asks for in that case).  There is no host entry point for the compressed GPU cache:
+ * a cached gather is ibp_cache_gather_decompress with device buffers.                                              */
 ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host, int64_t n, void* out_host, void* cuda_stream);
 
 /* -- S8: decode rows [first_row, first_row+n_rows) whose packed bytes the caller already staged in device memory
@@ -241,8 +246,11 @@ ibp_status ibp_cache_create(ibp_handle* h, uint64_t capacity_bytes, uint32_t n_s
                             ibp_cache** out_cache);
 /* Static fill: for every id of row_ids_host (n int64 on the HOST, in priority order) that is not cached yet, copies its packed
  * row from the host store into the current slab (a CUDA kernel reading zero-copy) and adds the map entry; stops at the first
- * row that does not fit.  *n_inserted_host (optional) = rows added.  Synchronises the stream.  INVALID_ARG for ids out of
- * range.                                                                                                               */
+ * row that does not fit.  *n_inserted_host (optional) = rows added.  Synchronises the stream.  All ids are validated before
+ * anything changes: INVALID_ARG for an id out of range, OUT_OF_MEMORY and CUDA errors leave the cache exactly as it was.
+ * An insert may run while gathers on other streams use the cache: the slab bytes are written first and a map slot {key, value}
+ * is published with one 16-byte compare-and-swap, so a concurrent gather sees a row either as cached or as not cached (then
+ * it reads the host store) -- the output is the same.  Two inserts on one cache must not overlap.                        */
 ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host, int64_t n, void* cuda_stream, int64_t* n_inserted_host);
 /* S1-S6 with the cache in front of the host store (see above).  Arguments as ibp_gather_decompress.                    */
 ibp_status ibp_cache_gather_decompress(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);

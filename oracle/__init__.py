@@ -24,7 +24,7 @@ _lib = None
 
 def build(force: bool = False) -> Path:
     if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
-        tmp = _SO.with_suffix(".so.tmp")
+        tmp = _SO.with_suffix(f".so.tmp{os.getpid()}")      # per process: concurrent first-time builds (spawned test workers) do not collide
         r = subprocess.run(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", str(_SRC), "-o", str(tmp)],
                            capture_output=True, text=True)
         if r.returncode != 0:

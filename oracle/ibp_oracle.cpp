@@ -11,13 +11,17 @@
 //
 // Parity pins (tests/test_oracle_pins.py, all -m "not gpu"):
 //   ibp_oracle_group_masks   : brute force over all rows in Python; closed form AND/OR; invariants P:231, P:237;
-//                              hand-worked fixtures tests/golden/strict_group_*.txt
+//                              hand-worked fixture tests/golden/worked_example_strict.txt
 //   ibp_oracle_pack_row      : canonical-order construction (row j of the 2^k-row group packs to integer j);
 //                              all-variant group == memcpy; sizes == ceil(k/8)
 //   ibp_oracle_unpack_row    : round trip on random bit patterns for masks of every popcount; k=0 == Bitval broadcast
-//   ibp_oracle_build/gather  : equals the plain gather out[i] = X[ids[i]] byte for byte (losslessness)
+//   ibp_oracle_build/gather  : equals the plain gather out[i] = X[ids[i]] byte for byte (losslessness);
+//                              the group partition (blocked with a ragged last group, strided with n % S != 0 and n < S):
+//                              every group's Mask/Bitval equal those computed from exactly X[gG:(g+1)G] / X[g::S] by
+//                              Python-integer brute force and by the AND/OR closed form (test_dataset_group_partition)
 //   thresholded mode (T<N)   : round trip; compressed <= raw; participation overhead row_bytes/CS bits
-//                              (P:527 prints 12.5% and 1.6%); at T=N payload == strict payload; hand-worked fixture
+//                              (P:527 prints 12.5% and 1.6%); at T=N payload == strict payload; hand-worked fixtures
+//                              tests/golden/worked_example_thresholded.txt, worked_example_mixed_chunks.txt
 //   ibp_oracle_build_T/gather: equals the plain gather byte for byte; bitmask bytes = ceil(n_rows/8); at tau=1
 //                              Mask/Bitval equal the strict dataset's; T = ceil(tau N_g) against Fig. 2's T=4, N=5;
 //                              hand-worked 5-row dataset fixture (sizes, flags, stored bytes)

@@ -53,7 +53,7 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
     src = sorted((PKG / "csrc").glob("*.cu")) + sorted((PKG / "csrc").glob("*.cpp"))
     deps = src + sorted((PKG / "csrc").glob("*.h")) + sorted((PKG / "csrc").glob("*.cuh")) + sorted((ROOT / "include").glob("*.h"))
     if force or _stale(LIB, deps):
-        tmp = LIB.with_suffix(".so.tmp")
+        tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")       # per process: concurrent builds (torchrun ranks, test workers) do not collide
         _run([nvcc_path(), *NVCC_FLAGS, *extra_flags, "-I", ROOT / "include", "-I", PKG / "csrc", "-x", "cu", *src,
               "-o", tmp, "-lgomp"], verbose)
         os.replace(tmp, LIB)
@@ -63,7 +63,7 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
 def build_datagen(force: bool = False, verbose: bool = False) -> Path:
     src = PKG / "datagen" / "ibp_datagen.c"
     if force or _stale(DATAGEN_LIB, [src]):
-        tmp = DATAGEN_LIB.with_suffix(".so.tmp")
+        tmp = DATAGEN_LIB.with_suffix(f".so.tmp{os.getpid()}")
         _run(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", src, "-o", tmp, "-lm"], verbose)
         os.replace(tmp, DATAGEN_LIB)
     return DATAGEN_LIB

@@ -493,9 +493,7 @@ static ibp_status check_table(const ibp_table_desc* t, const void* rows_dev, con
 }
 
 static int analysis_grid(uint64_t work_warps) {
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    (void)cudaGetLastError();
+    const int sms = ibp_sm_count_current();
     const uint64_t ctas = (work_warps + 7) / 8;
     return (int)std::max<uint64_t>(1, std::min<uint64_t>(ctas, (uint64_t)sms * 8));
 }
@@ -649,7 +647,8 @@ extern "C" ibp_status ibp_kmeans_bits_device(const void* rows_dev, uint64_t n_ro
     uint32_t nt = std::min<uint32_t>(256, (160u * 1024u / row_bytes) / 32u * 32u);
     if (nt < 32) nt = 32;
     const size_t smem = (size_t)nt * row_bytes;
-    IBP_CUDA(cudaFuncSetAttribute(ibp_assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static unsigned long long optin_done = 0;
+    if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(ibp_assign_kernel, &optin_done));
     uint32_t *counts = nullptr, *gn = nullptr, *hist = nullptr, *cursor = nullptr; int64_t* order = nullptr;
     IBP_CUDA(cudaMallocAsync((void**)&counts, (uint64_t)k * 32ull * nw * 4, st));
     IBP_CUDA(cudaMallocAsync((void**)&gn, (uint64_t)k * 4, st));

@@ -804,7 +804,7 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         K.gtab = h->gtab_dev;
         K.store = h->store_dev;
         K.row_stride_strided = h->row_stride_strided;
-        const bool bulk = !B.strided && p.align_bytes >= 16 && h->max_stride > 0 && h->max_stride <= 12288 && !getenv("IBP_PACK_NO_BULK");
+        const bool bulk = !B.strided && p.align_bytes >= 16 && h->max_stride > 0 && h->max_stride <= 12288;
         size_t smem;
         if (bulk) {
             K.rows_per_unit = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(16, 12288 / h->max_stride));
@@ -822,7 +822,8 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         const int grid = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * (bulk ? 2 : 8));
 #define IBP_PACK(KERN_, W_)                                                                                                  \
     do {                                                                                                                     \
-        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(KERN_<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        static unsigned long long optin_done = 0;                                                                            \
+        if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(KERN_<W_>, &optin_done));                                          \
         KERN_<W_><<<grid, wpc * 32, smem, st>>>(K);                                                                          \
     } while (0)
         t_pack.start();
@@ -897,7 +898,8 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         const int grid2 = (int)std::min<uint64_t>((K.n_units + wpc - 1) / wpc, (uint64_t)sms * 2);
 #define IBP_PACK_T(W_)                                                                                                         \
     do {                                                                                                                       \
-        if (smem > 48 * 1024) IBP_CUDA(cudaFuncSetAttribute(ibp_pack_t_kernel<W_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        static unsigned long long optin_done = 0;                                                                              \
+        if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(ibp_pack_t_kernel<W_>, &optin_done));                                \
         ibp_pack_t_kernel<W_><<<grid2, wpc * 32, smem, st>>>(K);                                                               \
     } while (0)
         t_pack.start();

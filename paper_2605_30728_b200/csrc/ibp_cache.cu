@@ -14,6 +14,16 @@ struct FillItem {          // one row to add: copy `bytes` from the host store a
     uint32_t bytes, slab;
 };
 
+// {key, value} of a map slot published with ONE 16-byte compare-and-swap: a concurrent probe (16-byte load) sees the slot either
+// empty or complete, never a key without its value.
+__device__ __forceinline__ ulonglong2 cas128(void* addr, ulonglong2 cmp, ulonglong2 val) {
+    ulonglong2 old;
+    asm volatile("{\n\t.reg .b128 c, n, o;\n\tmov.b128 c, {%2, %3};\n\tmov.b128 n, {%4, %5};\n\t"
+                 "atom.global.acq_rel.gpu.cas.b128 o, [%6], c, n;\n\tmov.b128 {%0, %1}, o;\n\t}"
+                 : "=l"(old.x), "=l"(old.y) : "l"(cmp.x), "l"(cmp.y), "l"(val.x), "l"(val.y), "l"(addr) : "memory");
+    return old;
+}
+
 __global__ void ibp_cache_fill_kernel(const FillItem* __restrict__ items, int64_t n, const uint8_t* __restrict__ store,
                                       uint8_t* const* __restrict__ slabs, uint64_t* __restrict__ map, uint32_t mask) {
     const int lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
@@ -26,11 +36,13 @@ __global__ void ibp_cache_fill_kernel(const FillItem* __restrict__ items, int64_
             asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(t.x), "=r"(t.y), "=r"(t.z), "=r"(t.w) : "l"(src + v));
             dst[v] = t;
         }
+        __threadfence();    // the slab bytes (possibly in a peer GPU's memory) are visible before the entry that points at them
+        __syncwarp();
         if (lane == 0) {
             uint32_t slot = ibp_cache_hash(it.id, mask);
             for (;;) {
-                const unsigned long long prev = atomicCAS((unsigned long long*)&map[2ull * slot], 0ull, (unsigned long long)(it.id + 1));
-                if (prev == 0ull || prev == it.id + 1) { map[2ull * slot + 1] = it.entry; break; }
+                const ulonglong2 prev = cas128(&map[2ull * slot], make_ulonglong2(0ull, 0ull), make_ulonglong2(it.id + 1, it.entry));
+                if (prev.x == 0ull || prev.x == it.id + 1) break;
                 slot = (slot + 1) & mask;
             }
         }
@@ -84,55 +96,78 @@ extern "C" ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host
     if (!c || n < 0 || (!row_ids_host && n > 0)) { ibp_set_error("ibp_cache_insert: bad argument"); return IBP_ERR_INVALID_ARG; }
     if (n_inserted_host) *n_inserted_host = 0;
     const ibp_handle* h = c->h;
-    std::vector<FillItem> items;
-    try { items.reserve((size_t)std::min<int64_t>(n, 1 << 20)); } catch (...) {}
-    bool full = false;
-    for (int64_t i = 0; i < n && !full; ++i) {
+    // every id is validated before any state changes: an error return leaves the cache exactly as it was
+    for (int64_t i = 0; i < n; ++i) {
         const int64_t sid = row_ids_host[i];
         if (sid < 0 || (uint64_t)sid >= h->p.n_rows) { ibp_set_error("ibp_cache_insert: id %lld out of range", (long long)sid); return IBP_ERR_INVALID_ARG; }
-        const uint64_t id = (uint64_t)sid;
-        if ((c->present[id >> 6] >> (id & 63)) & 1ull) continue;
-        if (c->n_entries + items.size() >= c->max_entries) break;
-        // the 16-byte-aligned cover of the packed row, exactly what the decode kernel fetches from the store
-        const uint64_t off = ibp_row_offset(h, id);
-        uint64_t bytes, flag = 1;
-        if (h->thresholded) {
-            bytes = 16ull * (h->row_off[id + 1] - h->row_off[id]);
-            flag = (h->row_flag[id >> 5] >> (id & 31)) & 1u;
-        } else {
-            bytes = h->gtab[ibp_group_of(h, id)].stride;
+    }
+    std::vector<FillItem> items;
+    // bookkeeping is staged in copies and committed only after the fill kernel has succeeded; `present` is marked while the list
+    // is built (it also de-duplicates ids repeated inside this call) and unmarked again on any failure
+    uint64_t slab_used[8];
+    memcpy(slab_used, c->slab_used, sizeof slab_used);
+    uint32_t cur_slab = c->cur_slab;
+    auto rollback = [&]() { for (const FillItem& it : items) c->present[it.id >> 6] &= ~(1ull << (it.id & 63)); };
+    try {
+        items.reserve((size_t)std::min<int64_t>(n, 1 << 20));
+        for (int64_t i = 0; i < n; ++i) {
+            const uint64_t id = (uint64_t)row_ids_host[i];
+            if ((c->present[id >> 6] >> (id & 63)) & 1ull) continue;
+            if (c->n_entries + items.size() >= c->max_entries) break;
+            // the 16-byte-aligned cover of the packed row, exactly what the decode kernel fetches from the store
+            const uint64_t off = ibp_row_offset(h, id);
+            uint64_t bytes, flag = 1;
+            if (h->thresholded) {
+                bytes = 16ull * (h->row_off[id + 1] - h->row_off[id]);
+                flag = (h->row_flag[id >> 5] >> (id & 31)) & 1u;
+            } else {
+                bytes = h->gtab[ibp_group_of(h, id)].stride;
+            }
+            const uint64_t head = off & 15ull, cover = bytes ? (head + bytes + 15ull) & ~15ull : 0ull;
+            while (cur_slab < c->n_slabs && slab_used[cur_slab] + cover > c->slab_bytes) ++cur_slab;
+            if (cur_slab >= c->n_slabs) { cur_slab = c->n_slabs - 1; break; }      // full: stop at the first row that does not fit
+            FillItem it;
+            it.id = id;
+            it.slab = cur_slab;
+            it.entry = slab_used[it.slab] | ((uint64_t)it.slab << 40) | (flag << 43);
+            it.src = off - head;
+            it.bytes = (uint32_t)cover;
+            items.push_back(it);
+            slab_used[it.slab] += cover;
+            c->present[id >> 6] |= 1ull << (id & 63);
         }
-        const uint64_t head = off & 15ull, cover = bytes ? (head + bytes + 15ull) & ~15ull : 0ull;
-        while (c->cur_slab < c->n_slabs && c->slab_used[c->cur_slab] + cover > c->slab_bytes) ++c->cur_slab;
-        if (c->cur_slab >= c->n_slabs) { full = true; c->cur_slab = c->n_slabs - 1; break; }
-        FillItem it;
-        it.id = id;
-        it.slab = c->cur_slab;
-        it.entry = c->slab_used[it.slab] | ((uint64_t)it.slab << 40) | (flag << 43);
-        it.src = off - head;
-        it.bytes = (uint32_t)cover;
-        c->slab_used[it.slab] += cover;
-        c->present[id >> 6] |= 1ull << (id & 63);
-        try { items.push_back(it); } catch (...) { ibp_set_error("ibp_cache_insert: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    } catch (...) {
+        rollback();
+        ibp_set_error("ibp_cache_insert: out of memory");
+        return IBP_ERR_OUT_OF_MEMORY;
     }
     if (items.empty()) return IBP_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    IBP_CUDA(cudaSetDevice(h->device));
     FillItem* items_dev = nullptr;
     uint8_t** slabs_dev = nullptr;
-    IBP_CUDA(cudaMalloc((void**)&items_dev, items.size() * sizeof(FillItem)));
-    cudaError_t e = cudaMalloc((void**)&slabs_dev, 8 * sizeof(uint8_t*));
+    cudaError_t e = cudaSetDevice(h->device);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&items_dev, items.size() * sizeof(FillItem));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&slabs_dev, 8 * sizeof(uint8_t*));
     if (e == cudaSuccess) e = cudaMemcpyAsync(items_dev, items.data(), items.size() * sizeof(FillItem), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(slabs_dev, c->slab_dev, 8 * sizeof(uint8_t*), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) {
-        const int blocks = (int)std::min<size_t>((items.size() + 7) / 8, 148 * 8);
+        const int blocks = (int)std::min<size_t>((items.size() + 7) / 8, (size_t)h->sm_count * 8);
         ibp_cache_fill_kernel<<<blocks, 256, 0, st>>>(items_dev, (int64_t)items.size(), h->store_dev, slabs_dev, c->map_dev, c->map_cap - 1);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(items_dev);
+    if (items_dev) cudaFree(items_dev);
     if (slabs_dev) cudaFree(slabs_dev);
-    if (e != cudaSuccess) { ibp_set_error("ibp_cache_insert: %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return IBP_ERR_CUDA; }
+    if (e != cudaSuccess) {
+        // a failure before the launch (allocation, copies) has touched neither the slabs nor the map; a failure of the kernel itself
+        // is a sticky context error after which no call on this device works anyway.  Either way nothing is committed.
+        rollback();
+        ibp_set_error("ibp_cache_insert: %s (the cache keeps its previous contents)", cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? IBP_ERR_OUT_OF_MEMORY : IBP_ERR_CUDA;
+    }
+    memcpy(c->slab_used, slab_used, sizeof slab_used);
+    c->cur_slab = cur_slab;
     c->n_entries += items.size();
     if (n_inserted_host) *n_inserted_host = (int64_t)items.size();
     return IBP_OK;
@@ -141,7 +176,7 @@ extern "C" ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host
 extern "C" ibp_status ibp_cache_lookup(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, uint64_t* entries_dev, void* cuda_stream) {
     if (!c || n < 0 || (n > 0 && (!row_ids_dev || !entries_dev))) { ibp_set_error("ibp_cache_lookup: bad argument"); return IBP_ERR_INVALID_ARG; }
     if (n == 0) return IBP_OK;
-    ibp_cache_lookup_kernel<<<(int)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, (cudaStream_t)cuda_stream>>>(c->map_dev, c->map_cap - 1, row_ids_dev, n, entries_dev);
+    ibp_cache_lookup_kernel<<<(int)std::min<int64_t>((n + 255) / 256, (int64_t)c->h->sm_count * 8), 256, 0, (cudaStream_t)cuda_stream>>>(c->map_dev, c->map_cap - 1, row_ids_dev, n, entries_dev);
     IBP_CUDA(cudaGetLastError());
     return IBP_OK;
 }

@@ -126,7 +126,7 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 // CACHE = the compressed GPU cache sits in front of the store: S1 probes the hash map; a hit fetches the same
 // 16-byte-aligned cover from the row's slab in HBM instead of the host store, everything after the fetch is unchanged.
 template <int W, int NST, int MODE, int FETCH, bool TM, bool CACHE = false>
-__global__ void __launch_bounds__(1024) ibp_decode_kernel(const DecodeParams P) {
+__global__ void __launch_bounds__(256) ibp_decode_kernel(const DecodeParams P) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
     uint8_t* ring = smem + (size_t)wib * NST * P.slot_bytes;
@@ -481,12 +481,10 @@ struct RowPrepass {
 };
 
 static ibp_status rows_prepass(const int64_t* ids_dev, int64_t n, bool dedup, bool order, uint64_t n_ids_space, uint64_t store_bytes,
-                               cudaStream_t st, RowPrepass* R) {
+                               int sm_count, cudaStream_t st, RowPrepass* R) {
     uint32_t shift = 0, nb = 0, nb_pad = 0, cap = 0;
     if (order) {
-        uint64_t target = 256ull << 10;
-        if (const char* e = getenv("IBP_BUCKET_BYTES")) target = strtoull(e, nullptr, 10);   // tuning experiments only
-        bucket_shape(n_ids_space, store_bytes, target, &shift, &nb);
+        bucket_shape(n_ids_space, store_bytes, 256ull << 10, &shift, &nb);   // about 256 KB of the store per bucket
         nb_pad = (nb + 4095u) / 4096u * 4096u;
     }
     if (dedup) { cap = 1024; while ((uint64_t)cap < 2ull * (uint64_t)n) cap <<= 1; }
@@ -500,7 +498,7 @@ static ibp_status rows_prepass(const int64_t* ids_dev, int64_t n, bool dedup, bo
     uint32_t* cnt = order ? (uint32_t*)(ws + 256) : nullptr;
     unsigned long long* table = (unsigned long long*)(ws + 256 + cnt_bytes);
     uint8_t* idx = ws + zero_bytes;
-    const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, 148 * 8);
+    const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, (int64_t)sm_count * 8);
     const int32_t* list = nullptr;
     const uint32_t* n_list = nullptr;
     if (dedup) {
@@ -526,7 +524,7 @@ static ibp_status rows_prepass(const int64_t* ids_dev, int64_t n, bool dedup, bo
 static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_space, uint64_t store_bytes, cudaStream_t st,
                              int32_t** order_out, void** ws_out) {
     RowPrepass R;
-    ibp_status s = rows_prepass(ids_dev, n, false, true, n_ids_space, store_bytes, st, &R);
+    ibp_status s = rows_prepass(ids_dev, n, false, true, n_ids_space, store_bytes, ibp_sm_count_current(), st, &R);
     *order_out = (int32_t*)R.list;
     *ws_out = R.ws;
     return s;
@@ -538,11 +536,8 @@ static ibp_status make_order(const int64_t* ids_dev, int64_t n, uint64_t n_ids_s
 template <int W, int NST, int MODE, int FETCH, bool TM = false, bool CACHE = false>
 static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64_t max_ctas, int sm_count, int wpc, size_t smem, cudaStream_t st) {
     auto kern = ibp_decode_kernel<W, NST, MODE, FETCH, TM, CACHE>;
-    static thread_local size_t attr_smem = 0;
-    if (smem > 48 * 1024 && smem > attr_smem) {
-        IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+    static unsigned long long smem_optin_done = 0;
+    if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
     // random rows: 2 CTAs per SM keep enough reads in flight for the link; more only widens the window of store pages touched
@@ -621,11 +616,8 @@ template <int W, int NS>
 static ibp_status launch_stream_one(const StreamParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
     constexpr int NW = 8;
     auto kern = ibp_stream_kernel<W, NS, NW>;
-    static thread_local size_t attr_smem = 0;
-    if (smem > 48 * 1024 && smem > attr_smem) {
-        IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+    static unsigned long long smem_optin_done = 0;
+    if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
     int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
@@ -733,11 +725,8 @@ template <int W, int NS, bool RUNS>
 static ibp_status launch_stream_t_one(const StreamTParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
     constexpr int NW = 8;
     auto kern = ibp_stream_t_kernel<W, NS, NW, RUNS>;
-    static thread_local size_t attr_smem = 0;
-    if (smem > 48 * 1024 && smem > attr_smem) {
-        IBP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+    static unsigned long long smem_optin_done = 0;
+    if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
     int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
@@ -925,7 +914,7 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
     RowPrepass R;
     ibp_status s = IBP_OK;
     if (dedup || order) {
-        s = rows_prepass(row_ids_dev, n, dedup, order, h->p.n_rows, h->store_used, st, &R);
+        s = rows_prepass(row_ids_dev, n, dedup, order, h->p.n_rows, h->store_used, h->sm_count, st, &R);
         if (s != IBP_OK) return s;
     }
     P.order = R.list;
@@ -935,7 +924,7 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
     if (s == IBP_OK && dedup) {
         const uint32_t rb = h->p.row_bytes;
         const int lpr = rb >= 512 ? 32 : rb >= 256 ? 16 : rb >= 128 ? 8 : 4, rpw = 32 / lpr;
-        const int blocks = (int)std::min<int64_t>((n + 8 * rpw - 1) / (8 * rpw), 148 * 8);
+        const int blocks = (int)std::min<int64_t>((n + 8 * rpw - 1) / (8 * rpw), (int64_t)h->sm_count * 8);
         switch (lpr) {
             case 32: ibp_dedup_copy<32><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
             case 16: ibp_dedup_copy<16><<<blocks, 256, 0, st>>>(R.rep, n, rb, (uint8_t*)out_dev); break;
@@ -1065,7 +1054,7 @@ extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* r
     if (!would_dedup) {
         cudaPointerAttributes attr;
         void* out_dev_alias = nullptr;
-        if (!getenv("IBP_HOST_NO_DIRECT") && cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+        if (cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
             cudaHostGetDevicePointer(&out_dev_alias, out_host, 0) == cudaSuccess && out_dev_alias && !((uintptr_t)out_dev_alias & 15u) && h->store_dev) {
             int64_t* ids_d = nullptr;
             IBP_CUDA(cudaMallocAsync((void**)&ids_d, id_bytes, st));
@@ -1080,7 +1069,6 @@ extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* r
         (void)cudaGetLastError();
     }
     int n_chunks = out_bytes >= (32u << 20) ? 4 : out_bytes >= (8u << 20) ? 2 : 1;
-    if (const char* e = getenv("IBP_HOST_CHUNKS")) n_chunks = std::max(1, std::min(4, atoi(e)));   // tuning experiments only
     if (n < n_chunks) n_chunks = 1;
     uint8_t* buf = nullptr;
     IBP_CUDA(cudaMallocAsync((void**)&buf, id_bytes + out_bytes, st));
@@ -1092,8 +1080,14 @@ extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* r
         e = cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking);
         for (int c = 0; c <= n_chunks && e == cudaSuccess; ++c) e = cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming);
     }
+    // chunk boundaries on multiples of `q` rows, so that every chunk's output starts 16-byte aligned inside the staging buffer
+    // whatever row_bytes is (any multiple of 4 is allowed: 12, 100, 516, ...)
+    int64_t q = 1;
+    while ((q * (int64_t)id_bytes_row) % 16) q <<= 1;
+    auto cut = [&](int c) { return c >= n_chunks ? n : (n * c / n_chunks) / q * q; };
     for (int c = 0; c < n_chunks && s == IBP_OK && e == cudaSuccess; ++c) {
-        const int64_t i0 = n * c / n_chunks, i1 = n * (c + 1) / n_chunks;
+        const int64_t i0 = cut(c), i1 = cut(c + 1);
+        if (i1 <= i0) continue;
         uint8_t* dout = buf + id_bytes + (size_t)i0 * id_bytes_row;
         s = ibp_gather_decompress(h, (const int64_t*)buf + i0, i1 - i0, dout, cuda_stream);
         if (s != IBP_OK) break;
@@ -1137,7 +1131,7 @@ extern "C" ibp_status ibp_validate_ids(ibp_handle* h, const int64_t* row_ids_dev
     unsigned long long* bad = nullptr;
     IBP_CUDA(cudaMallocAsync((void**)&bad, 8, st));
     IBP_CUDA(cudaMemsetAsync(bad, 0, 8, st));
-    if (n > 0) ibp_count_bad_ids<<<(int)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, st>>>(row_ids_dev, n, (int64_t)(h->p.n_rows / h->p.index_span), bad);
+    if (n > 0) ibp_count_bad_ids<<<(int)std::min<int64_t>((n + 255) / 256, (int64_t)h->sm_count * 8), 256, 0, st>>>(row_ids_dev, n, (int64_t)(h->p.n_rows / h->p.index_span), bad);
     unsigned long long hb = 0;
     IBP_CUDA(cudaMemcpyAsync(&hb, bad, 8, cudaMemcpyDeviceToHost, st));
     IBP_CUDA(cudaFreeAsync(bad, st));
@@ -1181,7 +1175,7 @@ extern "C" ibp_status ibp_gather_uncompressed_ex(const void* rows_mapped, uint32
     const int wpc = 8;
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ibp_gather_rows_kernel, wpc * 32, 0));
-    const int blocks = (int)std::min<int64_t>((n + wpc - 1) / wpc, 148 * (int64_t)std::max(occ, 1));
+    const int blocks = (int)std::min<int64_t>((n + wpc - 1) / wpc, ibp_sm_count_current() * (int64_t)std::max(occ, 1));
     ibp_gather_rows_kernel<<<blocks, wpc * 32, 0, st>>>((const uint8_t*)rows_mapped, row_bytes, row_ids_dev, ord, n, (uint8_t*)out_dev);
     IBP_CUDA(cudaGetLastError());
     if (ws) IBP_CUDA(cudaFreeAsync(ws, st));
@@ -1256,7 +1250,7 @@ static ibp_status measure_link(int device, size_t nbytes, int reps, double* gbps
     } else {
         for (int it = 0; it < reps + 1; ++it) {   // first iteration is a warm-up
             cudaEventRecord(a, 0);
-            if (zero_copy) ibp_contig_read_kernel<<<148 * 4, 512>>>((const uint4*)hd, nbytes / 16, sink);
+            if (zero_copy) ibp_contig_read_kernel<<<ibp_sm_count_current() * 4, 512>>>((const uint4*)hd, nbytes / 16, sink);
             else if (d2h) cudaMemcpyAsync(hp, dp, nbytes, cudaMemcpyDeviceToHost, 0);
             else cudaMemcpyAsync(dp, hp, nbytes, cudaMemcpyHostToDevice, 0);
             cudaEventRecord(b, 0);
@@ -1312,7 +1306,7 @@ extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes
     cudaEvent_t a, b;
     float best = 1e30f;
     const uint32_t lanes = span_bytes / 16, rpg = 64;
-    const int grid = 148 * 8, block = 256;
+    const int grid = ibp_sm_count_current() * 8, block = 256;
     const double n_reads = (double)((uint64_t)grid * block / lanes) * rpg;
     if (cudaMalloc((void**)&sink, 4) != cudaSuccess || cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
         ibp_set_error("ibp_measure_random_read: allocation failed: %s", cudaGetErrorString(cudaGetLastError()));

@@ -16,6 +16,42 @@
         }                                                                                           \
     } while (0)
 
+// SMs of the current device (grids are sized from this, never from a literal).  Cached per device.
+static inline int ibp_sm_count_current() {
+    static int cached[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return 148; }
+    int n = cached[dev];
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { (void)cudaGetLastError(); return 148; }
+        cached[dev] = n;   // benign race: every thread writes the same value
+    }
+    return n;
+}
+
+// Opt a kernel in to the device's largest dynamic shared-memory size ONCE per (kernel, device).  The attribute is per function
+// and per device for the whole process, so a per-thread "largest size seen" cache would let a second host thread lower it under
+// the first one's feet; raising it to the device maximum once is order-independent.  `done` is the caller's per-kernel bitmask
+// (one static per template instantiation), bit d = device d is set up.
+template <typename Kern>
+static inline cudaError_t ibp_optin_max_smem(Kern kern, unsigned long long* done) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (__atomic_load_n(done, __ATOMIC_ACQUIRE) & bit) return cudaSuccess;
+    int optin = 0;
+    e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+    if (e != cudaSuccess) return e;
+    __atomic_fetch_or(done, bit, __ATOMIC_RELEASE);
+    return cudaSuccess;
+}
+
 __device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {

@@ -278,6 +278,23 @@ def test_uncompressed_baseline_and_host_api():
     pin.free()
 
 
+@pytest.mark.parametrize("rb,n_big", [(100, 90_001), (12, 700_003), (516, 70_001)])
+def test_host_entry_chunks_with_odd_row_sizes(rb, n_big):
+    """ibp_gather_decompress_host cuts outputs of >= 8 MB (2 chunks) / >= 32 MB (4 chunks) into chunks; with row_bytes not a
+    multiple of 16 the chunk borders must fall on rows whose output offset is 16-byte aligned (a border at an arbitrary row
+    made ibp_gather_decompress reject the chunk with INVALID_ARG).  Pageable destination = the staged path; ids repeat."""
+    n = 5000
+    X = (datagen.random_bytes(n * rb, 31 + rb).reshape(n, rb) & datagen.random_bytes(rb, 32)[None, :]) | 0x02
+    h = ibp.ibp_build(X, rb, 0, 50, align_bytes=16).upload_metadata(0)
+    big = np.random.default_rng(rb).integers(0, n, n_big).astype(np.int64)
+    for mode in (-1, 0, 1):
+        h.set_dedup_mode(mode)
+        out = np.zeros((n_big, rb), np.uint8)
+        h.gather_decompress_host(big, n_big, out, torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(out, oracle.gather_plain(X, big))
+    h.destroy()
+
+
 def test_configure_limits_grid_and_streams():
     """SM-limited launch and a non-default stream give the same bytes."""
     w = workloads.Tiny()

@@ -225,6 +225,58 @@ def test_dataset_equals_plain_gather(kind, param, n_rows, rb):
         ds.gather_decompress(np.array([n_rows], np.int64))
 
 
+def _brute_masks(rows_u8, T=None):
+    """Mask/Bitval of exactly these rows from Python integers: per bit position, count the rows with the bit set
+     and compare with T and N - T (reading R2); nothing of oracle/ is called."""
+    n, rb = rows_u8.shape
+    T = n if T is None else T
+    ints = [int.from_bytes(r.tobytes(), "little") for r in rows_u8]
+    mask = bitval = 0
+    for p in range(8 * rb):
+        c1 = sum((v >> p) & 1 for v in ints)
+        if c1 >= T:
+            mask |= 1 << p
+            bitval |= 1 << p
+        elif c1 <= n - T:
+            mask |= 1 << p
+    to = lambda v: np.frombuffer(v.to_bytes(rb, "little"), np.uint8)
+    return to(mask), to(bitval)
+
+
+@pytest.mark.parametrize("kind,param,n_rows,rb", [(1, 5, 203, 8), (1, 8, 64, 4), (1, 3, 2, 4), (1, 86, 615, 8), (0, 7, 50, 8),
+                                                   (0, 256, 700, 4), (0, 64, 64, 8), (0, 1000, 10, 8)])
+def test_dataset_group_partition(kind, param, n_rows, rb):
+    """SURVEY 8(c) strict step 1 / PAPER.md:542 (one Mask/Bitval per cluster): group g of a Dataset holds EXACTLY the rows
+    X[g*G:(g+1)*G] (blocked; ragged last group) or X[g::S] (strided; n % S != 0, n < S).  A partition that takes a
+    superset (or a subset) of a group's rows stays lossless and keeps n_groups, so only a direct comparison of every
+    group's Mask/Bitval with masks computed from exactly those rows catches it: brute force over Python integers and the
+    AND/OR closed form  Bitval = AND rows, Mask = ~(AND ^ OR)."""
+    X = (datagen.random_bytes(n_rows * rb, 4242 + rb + param).reshape(n_rows, rb) & datagen.random_bytes(rb, 11)[None, :]) | 0x10
+    X[:: 3] ^= (datagen.random_bytes(rb, 12) & 0x0F)[None, :]           # bits shared by SOME rows only: a wrong partition changes the masks
+    ds = oracle.Dataset(X, kind, param)
+    dt1 = oracle.DatasetT(X, kind, param, 1, 1)
+    dt = oracle.DatasetT(X, kind, param, 4, 5)
+    n_groups = -(-n_rows // param) if kind == 0 else min(param, n_rows)
+    assert ds.n_groups == dt.n_groups == n_groups
+    seen = np.zeros(n_rows, np.int64)
+    for g in range(n_groups):
+        members = np.arange(g * param, min((g + 1) * param, n_rows)) if kind == 0 else np.arange(g, n_rows, param)
+        seen[members] += 1
+        rows = X[members]
+        a, o = np.bitwise_and.reduce(rows, axis=0), np.bitwise_or.reduce(rows, axis=0)
+        want_mask, want_bitval = _brute_masks(rows)
+        assert np.array_equal(want_mask, ~(a ^ o)) and np.array_equal(want_bitval, a)      # the two independent forms agree
+        assert np.array_equal(ds.mask(g), want_mask), f"group {g}: Mask is not that of its own rows"
+        assert np.array_equal(ds.bitval(g), want_bitval)
+        assert ds.k_bits(g) == 8 * rb - int(np.unpackbits(want_mask).sum())
+        assert np.array_equal(dt1.mask(g), want_mask) and np.array_equal(dt1.bitval(g), want_bitval)
+        T = -(-len(members) * 4 // 5)
+        assert dt.threshold(g) == T
+        tm, tb = _brute_masks(rows, T)
+        assert np.array_equal(dt.mask(g), tm) and np.array_equal(dt.bitval(g), tb)
+    assert np.all(seen == 1)                                             # the groups partition the rows
+
+
 def test_dataset_index_span():
     X = workloads.KV(layers=1, pages=4, heads=2).table()
     ds = oracle.Dataset(X, 0, 16)
