@@ -5,15 +5,20 @@
 
 One "step" = one pass of the whole hot path (plus the ordering pre-pass when the handle uses it)
 over one batch of synthetic ids: ibp_gather_decompress(handle, row_ids, n, out, stream).  A different seeded id batch
-every step.  Default workload = BASELINE.json configs[1] (GNN node-feature gather, 10M x 128 fp32, 250k unique ids).
+every step.  Default workload = BASELINE.json configs[1] (GNN node-feature gather, 10M x 128 fp32, 250k unique ids); the
+default run also measures the other four BASELINE configs (Tiny, DLRM, KV with all 32 layers, weight streaming with all 32
+layers, one layer per step) and reports them in `per_config`, and the headline step over a cudaHostAlloc store in
+`value_pinned_store`.
 
 Prints ONE JSON line (rank 0):
   value      effective (decompressed) GB/s, whole job, ids resident in HBM, the packed store in host memory (that the
              store is read over PCIe IS the method; nothing else is staged)
   e2e        same metric through ibp_gather_decompress_host: pinned HOST ids in, pinned HOST rows out, copies timed
-  roofline   dominant kernel (ibp_decode_kernel): achieved = packed bytes the launch must move over PCIe / its duration
-             (CUDA events on the launch stream); peak = cudaMemcpy H2D ceiling measured in this run
-             (BASELINE.json north_star: "measured cudaMemcpy H2D ceiling"); bound = "pcie"
+  roofline   dominant kernel (ibp_decode_kernel): achieved = ALGORITHMIC link bytes of the launch (sum of ceil(k_g/8) over the
+             batch's distinct rows) / its duration (CUDA events on the launch stream); peak = cudaMemcpy H2D
+             ceiling measured in this run (BASELINE.json north_star: "measured cudaMemcpy H2D ceiling"); bound = "pcie"
+             (DESIGN.md section 7); frac_stored = the same with rows rounded up to the declared alignment unit A; traffic =
+             read from the committed ncu summary of this kernel build (profiles/r02_*_decode_ncu.md) or null
   cpu_baseline  the oracle (oracle/, as it stands, 1 thread) on a bounded sample of the same workload
 Timing: CUDA events around every step on the launch stream, L2 flushed (256 MiB write) between steps outside the
 events, >= 3 warm-up steps, barrier + synchronize on both sides, max over ranks.
@@ -31,13 +36,6 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-
-# Per-launch traffic of ibp_decode_kernel from the ncu --set full captures summarised in profiles/r01_*_decode_ncu.md
-# (first timed launch): dram = dram__bytes_read.sum + dram__bytes_write.sum (HBM side: output rows + metadata);
-# sysmem = sysmem-aperture sectors x 32 B = what crossed PCIe.  GNN: sysmem 62.87 MB vs 62.92 MB algorithmic (no over-fetch).
-NCU_TRAFFIC = {"gnn": {"dram": 53_321_216 + 75_808_768, "sysmem": 62_866_432},
-               "dlrm": {"dram": None, "sysmem": 54_525_952}}
-
 
 def make_workload(name):
     from paper_2605_30728_b200 import workloads
@@ -177,7 +175,8 @@ def run_reference(args):
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": rows_per_step * w.row_bytes / (v * 1e9) * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-        "config": {"workload": describe(w), "note": "CPU oracle (oracle/ibp_oracle.cpp, single thread) on a bounded sample per step; ms_per_step is the time a full batch would take at that rate"},
+        "config": bench_config(w, parse_threshold(args.threshold)),
+        "note": "CPU oracle (oracle/ibp_oracle.cpp, single thread) on a bounded sample per step; ms_per_step is the time a full batch would take at that rate",
         "cpu_baseline": {"value": v, "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": "per step: " + desc, "rows_per_s": float(np.mean([x[1] for x in vals]))},
         "e2e": {"value": v, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -186,34 +185,97 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------- CUDA arm
-def run_cuda(args):
-    import torch
-    import torch.distributed as dist
-    from paper_2605_30728_b200 import binding as ibp
+def read_hbm_peak():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"], "MEASURED_PEAKS.json hbm_gbs (copy; read+write bytes)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the IBP hot path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    W, K = max(3, args.warmup), args.steps
-    w = make_workload(args.workload)
-    stream = torch.cuda.current_stream().cuda_stream
 
-    # ---- build (once, not timed): table -> ibp_build -> metadata to HBM
+def traffic_from_profile(name, matches_capture):
+    """roofline.traffic comes from the committed ncu summary of THIS kernel build, by file name, never from a literal here:
+    profiles/r02_<workload>_decode_ncu.md carries lines `dram_bytes_per_launch: N`, `sysmem_bytes_per_launch: N`, `kernel: ...`,
+    `commit: ...`.  Emitted only when the run matches the captured configuration (default alignment, store, order, dedup, no
+    cache, strict codec); otherwise null."""
+    path = os.path.join(ROOT, "profiles", f"r02_{name}_decode_ncu.md")
+    if not matches_capture or not os.path.exists(path):
+        return None, None, None
+    vals = {}
+    for line in open(path):
+        for key in ("dram_bytes_per_launch", "sysmem_bytes_per_launch", "kernel", "commit"):
+            if line.strip().startswith(key + ":"):
+                vals[key] = line.split(":", 1)[1].strip()
+    to_int = lambda k: int(vals[k].replace(",", "")) if k in vals else None
+    return to_int("dram_bytes_per_launch"), to_int("sysmem_bytes_per_launch"), {"file": os.path.relpath(path, ROOT), "kernel": vals.get("kernel"), "commit": vals.get("commit")}
+
+
+class Ctx:
+    """Per-process measurement context: device, streams, ceilings measured once in this run."""
+
+    def __init__(self, args):
+        import torch
+        import torch.distributed as dist
+        from paper_2605_30728_b200 import binding as ibp
+        import oracle
+        self.torch, self.dist, self.ibp, self.oracle, self.args = torch, dist, ibp, oracle, args
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device; the IBP hot path has no CPU fallback")
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+        self.stream = torch.cuda.current_stream().cuda_stream
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        self.h2d = ibp.ibp_measure_h2d(self.local, 1 << 30, 8)
+        self.zc = ibp.ibp_measure_zero_copy_read(self.local, 1 << 30, 3)
+        self.hbm_peak, self.hbm_src = read_hbm_peak()
+        self.launches = 0
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            self.dist.barrier()
+            self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, v):
+        t = self.torch.tensor([float(v)], dtype=self.torch.float64, device="cuda")
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def timed_loop(self, fn, count, first):
+        """count steps, CUDA events around each on the launch stream, L2 flushed (256 MiB write) between steps outside the events"""
+        torch = self.torch
+        evs = []
+        for j in range(count):
+            self.flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn(first + j)
+            b.record()
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+
+def measure_gather(ctx, w, K, W, full, X=None, store="managed", keep=False):
+    """One row- or span-gather workload end to end: build, parity of a warm-up batch against the plain definition, K timed steps
+    (value), the e2e entry point, the uncompressed baseline.  `full` adds the resident decode, all baseline variants and the
+    random-span ceiling.  Returns (entry dict, extras dict)."""
+    torch, ibp, oracle, args = ctx.torch, ctx.ibp, ctx.oracle, ctx.args
     t0 = time.perf_counter()
-    X = w.table()
+    if X is None:
+        X = w.table()
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
     align = args.align if args.align else w.align_bytes
     thr = parse_threshold(args.threshold)
     h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
-                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0, threshold=thr)
+                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if store == "pinned" else 0, threshold=thr)
     t_build = time.perf_counter() - t0
-    h.upload_metadata(local)
+    h.upload_metadata(ctx.local)
     if args.order is not None:
         h.set_order_mode(args.order)
     if args.decode_ctas:
@@ -221,43 +283,19 @@ def run_cuda(args):
     dedup = args.dedup if args.dedup is not None else (0 if w.ids_unique else -1)
     h.set_dedup_mode(dedup)
     info = h.info()
-    cache = None
-    if args.cache_frac > 0:                                    # S8f NEXT #3: compressed GPU cache in front of the store
+    stream = ctx.stream
+    cache = cinfo = None
+    if full and args.cache_frac > 0:                           # S8f NEXT #3: compressed GPU cache in front of the store
         if w.index_span != 1 or not hasattr(w, "hot_ids"):
             raise SystemExit("bench.py --cache-frac needs a row-gather workload with a hot set (gnn, dlrm)")
         cache = ibp.Cache(h, int(info.packed_bytes_stored * args.cache_frac), 1, max_entries=max(1024, int(w.n_rows * min(1.0, 2 * args.cache_frac))))
         cache.insert(w.hot_ids(int(w.n_rows * min(1.0, 2 * args.cache_frac))), stream)
         cinfo = cache.info()
 
-    # ---- ceilings measured on this box, this run
-    h2d_ceiling = ibp.ibp_measure_h2d(local, 1 << 30, 8)
-    zc_ceiling = ibp.ibp_measure_zero_copy_read(local, 1 << 30, 3)
-    # random-row gathers: the same link read as random, span-aligned spans of about one packed row, over a managed host
-    # buffer as large as the packed store (beyond a few hundred MB address translation, not the link,
-    # sets this rate) -- the measured ceiling of any random gather of rows this small on this box
-    rand_ceiling = None
-    if w.index_span == 1 and rank == 0 and info.packed_bytes_stored >= (64 << 20):
-        mean_row = info.packed_bytes_rows / w.n_rows
-        span = 128 if mean_row <= 128 else 256 if mean_row <= 256 else 512
-        sps, gbs = ibp.ibp_measure_random_read(local, int(min(info.packed_bytes_stored, 8 << 30)), span, 3)
-        rand_ceiling = {"span_bytes": span, "footprint_GB": round(min(info.packed_bytes_stored, 8 << 30) * 1e-9, 2),
-                        "spans_per_s": round(sps), "GBps": round(gbs, 2),
-                        "what": "ibp_measure_random_read: LSU 16-byte loads of span-aligned random spans, managed host-resident buffer"}
-    hbm_peak = None
-    try:
-        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
-        hbm_src = "MEASURED_PEAKS.json hbm_gbs (copy; read+write bytes)"
-    except Exception:
-        hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
-
-    # ---- batches: a different seeded id batch every step (rank-dependent)
-    n = w.batch_ids
-    n_rows_out = w.batch_rows
-    n_b = W + K
-    batches = [w.ids(rank * 100_000 + i) for i in range(n_b)]
+    n, n_rows_out = w.batch_ids, w.batch_rows
+    batches = [w.ids(ctx.rank * 100_000 + i) for i in range(W + K)]
     ids_dev = [torch.from_numpy(b).cuda() for b in batches]
     out = torch.empty((n_rows_out, w.row_bytes), dtype=torch.uint8, device="cuda")
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     hit_rate = None
     if cache is not None:                                      # only the misses cross PCIe: account the link bytes over them
         ent = torch.empty(n, dtype=torch.int64, device="cuda")
@@ -270,7 +308,7 @@ def run_cuda(args):
             link.append(h.batch_link_bytes(b[miss]) if miss.any() else (1, 1, 1))
         hit_rate = float(np.mean(hits[W:]))
     else:
-        link = [h.batch_link_bytes(b) for b in batches]        # (unique ids, stored bytes, byte-aligned bytes)
+        link = [h.batch_link_bytes(b) for b in batches]        # (distinct ids, stored bytes, byte-aligned bytes)
     order_on = w.index_span == 1 and ((args.order == 1) or (args.order is None and info.packed_bytes_stored > (64 << 20) and n >= 4096))
     dedup_on = w.index_span == 1 and (dedup == 1 or (dedup < 0 and n >= 16384))
     launches_per_step = 1 + (3 if order_on else 0) + (2 if dedup_on else 0)
@@ -281,72 +319,47 @@ def run_cuda(args):
         else:
             h.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
-
-    def timed_loop(fn, count, first):
-        evs = []
-        for j in range(count):
-            flush.zero_()                                       # L2 flush between steps, outside the events
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            fn(first + j)
-            b.record()
-            evs.append((a, b))
-        torch.cuda.synchronize()
-        return [a.elapsed_time(b) for a, b in evs]
-
-    # ---- value: ids resident in HBM
     for i in range(W):
         step(i)
-    # parity of one warm-up batch against the plain definition (oracle c1), so a fast wrong kernel cannot score
-    import oracle
     torch.cuda.synchronize()
+    # parity of one warm-up batch against the plain definition (oracle c1), so that a fast wrong kernel cannot score
     chk = np.random.default_rng(0).choice(n_rows_out, size=min(4096, n_rows_out), replace=False)
     got = out[torch.from_numpy(chk).cuda()].cpu().numpy()
     want = oracle.gather_plain(X, batches[W - 1], w.index_span)[chk]
     if not np.array_equal(got, want):
-        raise SystemExit("bench.py: GPU output differs from the oracle; refusing to report a number")
+        raise SystemExit(f"bench.py: GPU output differs from the oracle on {w.name}; refusing to report a number")
 
-    clocks = ClockSampler(local)
-    barrier()
+    clocks = ClockSampler(ctx.local)
+    ctx.barrier()
     clocks.start()
-    ms = timed_loop(step, K, W)
-    barrier()
+    ms = ctx.timed_loop(step, K, W)
+    ctx.barrier()
     clk = clocks.stop()
-    t_total = float(np.sum(ms))
-    tmax = torch.tensor([t_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    t_job = float(tmax.item())
+    ctx.launches += K * launches_per_step
+    t_job = ctx.max_over_ranks(float(np.sum(ms)))
+    world = ctx.world
     bytes_step = n_rows_out * w.row_bytes
     value = world * K * bytes_step / (t_job * 1e-3) * 1e-9
 
-    # ---- dominant kernel alone (pre-pass excluded when the handle orders): same launches, events around each
-    stored_timed = [link[W + j][1] for j in range(K)]
-    unique_timed = [link[W + j][0] for j in range(K)]
-    alg_timed = [link[W + j][2] for j in range(K)]
-    kernel_ms = ms                                              # one launch per step unless ordering is on
-    achieved = float(np.sum(stored_timed)) / (float(np.sum(kernel_ms)) * 1e-3) * 1e-9
-    ratio_stored = w.n_rows * w.row_bytes / info.packed_bytes_rows
-    ratio_alg = w.n_rows * w.row_bytes / info.packed_bytes_bytealigned
-    batch_ratio_stored = float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(stored_timed))
-    eff_roof = min(h2d_ceiling * batch_ratio_stored * (n / np.mean(unique_timed)), hbm_peak)
-    if cache is not None:                                       # all n rows are delivered for the link bytes of the distinct misses
-        eff_roof = min(h2d_ceiling * n * w.row_bytes / float(np.mean(stored_timed)), hbm_peak)
+    sec = float(np.sum(ms)) * 1e-3
+    uniq = float(np.sum([link[W + j][0] for j in range(K)]))
+    stored = float(np.sum([link[W + j][1] for j in range(K)]))
+    alg = float(np.sum([link[W + j][2] for j in range(K)]))
+    raw_unique = uniq * w.index_span * w.row_bytes
+    rep = K * n / uniq                                          # every repeat of a distinct id is delivered for free
+    if cache is not None:
+        roof_alg = roof_st = min(ctx.h2d * K * n * w.row_bytes / stored, ctx.hbm_peak)
+    else:
+        roof_alg = min(ctx.h2d * raw_unique / alg * rep, ctx.hbm_peak)
+        roof_st = min(ctx.h2d * raw_unique / stored * rep, ctx.hbm_peak)
 
-    # ---- e2e: pinned host ids -> device -> gather -> pinned host rows, through the C ABI host entry point
+    # ---- e2e through the C ABI host entry point: pinned host ids in, pinned host rows out
     ids_pin = ibp.PinnedBuffer(n * 8)
     out_pin = ibp.PinnedBuffer(bytes_step)
     ids_pin_np = ids_pin.view(np.int64)
     out_pin_np = out_pin.view(np.uint8, (n_rows_out, w.row_bytes))
-
     ids_stage = torch.empty(n, dtype=torch.int64, device="cuda")
-    ids_pin_t = torch.from_numpy(ids_pin_np)
-    out_pin_t = torch.from_numpy(out_pin_np)
+    ids_pin_t, out_pin_t = torch.from_numpy(ids_pin_np), torch.from_numpy(out_pin_np)
 
     def step_e2e(i):
         ids_pin_np[:] = batches[i]
@@ -361,258 +374,450 @@ def run_cuda(args):
     for i in range(min(W, 3)):
         step_e2e(i)
     if not np.array_equal(out_pin_np[chk], oracle.gather_plain(X, batches[min(W, 3) - 1], w.index_span)[chk]):
-        raise SystemExit("bench.py: end-to-end output differs from the oracle")
-    barrier()
-    Ke = max(3, min(K, 30))
-    ms_e = timed_loop(step_e2e, Ke, W)
-    barrier()
-    te = torch.tensor([float(np.sum(ms_e))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * Ke * bytes_step / (float(te.item()) * 1e-3) * 1e-9
+        raise SystemExit(f"bench.py: end-to-end output differs from the oracle on {w.name}")
+    ctx.barrier()
+    Ke = max(3, min(K, 30 if full else 10))
+    ms_e = ctx.timed_loop(step_e2e, Ke, W)
+    ctx.barrier()
+    e2e_value = world * Ke * bytes_step / (ctx.max_over_ranks(float(np.sum(ms_e))) * 1e-3) * 1e-9
+    ids_pin.free(); out_pin.free()
 
-    # ---- S8: resident decode (ibp_decompress_resident) of a contiguous range staged in HBM beforehand (rank 0, N=1)
-    resident = None
-    if world == 1 and not args.no_resident:
-        G = w.group_param
-        nr = min(w.n_rows, 1 << 20) // G * G
-        ptr, nb = h.packed_range(0, nr)
-        staged = torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda()
-        outr = torch.empty((nr, w.row_bytes), dtype=torch.uint8, device="cuda")
-
-        def step_r(i):
-            h.decompress_resident(staged.data_ptr(), 0, nr, outr.data_ptr(), stream)
-
-        for i in range(3):
-            step_r(i)
-        torch.cuda.synchronize()
-        if not np.array_equal(outr[:4096].cpu().numpy(), X[:4096].view(np.uint8).reshape(4096, -1)):
-            raise SystemExit("bench.py: resident decode differs from the original rows")
-        mr = timed_loop(step_r, 20, 0)
-        t_r = float(np.mean(mr))
-        meta_bytes = (nr // G) * 2 * w.row_bytes
-        resident = {"rows": nr, "ms": round(t_r, 4), "out_GBps": round(nr * w.row_bytes / (t_r * 1e-3) * 1e-9, 1),
-                    "in_plus_out_GBps": round((nb + nr * w.row_bytes) / (t_r * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": hbm_peak,
-                    "frac": round((nb + nr * w.row_bytes + meta_bytes) / (t_r * 1e-3) * 1e-9 / hbm_peak, 4),
-                    "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes), "kernel": ("ibp_stream_t_kernel" if info.thresholded else "ibp_stream_kernel") + " (ibp_decompress_resident)",
-                    "what": "packed bytes of the first rows of the table staged in HBM, decoded to HBM; L2 flushed between launches"}
-        del staged, outr
-
-    # ---- uncompressed zero-copy gather baseline (rank 0, N=1 only): same ids, same timing
+    # ---- uncompressed zero-copy gather baseline (N=1 only): same ids, same timing
     base = None
     if world == 1 and not args.no_baseline:
         res = {}
-        for kind in ("managed", "pinned"):
-            buf = ibp.PinnedBuffer(X.nbytes, managed=(kind == "managed"), device=local)
+        for kind in (("managed", "pinned") if full else ("managed",)):
+            buf = ibp.PinnedBuffer(X.nbytes, managed=(kind == "managed"), device=ctx.local)
             buf.view(X.dtype, X.shape)[:] = X
-            for order in ((False, True) if w.index_span == 1 else (False,)):
+            for order in ((False, True) if (w.index_span == 1 and full) else (False,)):
                 def step_b(i, buf=buf, order=order):
                     ibp.ibp_gather_uncompressed(buf.dev_ptr, w.row_bytes * w.index_span, ids_dev[i].data_ptr(), n, out.data_ptr(), stream,
                                                 n_rows=w.n_rows // w.index_span, locality_order=order)
                 for i in range(3):
                     step_b(i)
-                mb = timed_loop(step_b, min(K, 20), W)
+                mb = ctx.timed_loop(step_b, min(K, 20 if full else 8), W)
                 res[f"{kind}{'_ordered' if order else ''}"] = bytes_step / (float(np.mean(mb)) * 1e-3) * 1e-9
             buf.free()
         base = {"unit": "GB/s", "what": "ibp_gather_uncompressed: zero-copy gather of the raw rows (PAPER.md:329 'GPU (Aligned)')", **{k: round(v, 2) for k, v in res.items()}}
 
-    # ---- CPU oracle baseline on a bounded sample (rank 0, N=1 only)
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu:
-        g, rps, desc = oracle_sample(w, seconds_target=12.0, thr=thr)
-        cpu = {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)}
+    kernel = ("ibp_stream_t_kernel" if info.thresholded else "ibp_stream_kernel") if w.index_span > 1 else "ibp_decode_kernel"
+    entry = {
+        "name": w.name, "workload": describe(w), "value": round(value, 3), "unit": "GB/s", "rows_per_s": round(world * K * n_rows_out / (t_job * 1e-3), 1),
+        "ms_per_step": round(t_job / K, 5), "steps": K, "rows_per_step": n_rows_out, "row_bytes": w.row_bytes,
+        "link_GBps_bytealigned": round(alg / sec * 1e-9, 3), "link_GBps_stored": round(stored / sec * 1e-9, 3),
+        "frac_bytealigned": round(value / world / roof_alg, 4), "frac_stored": round(value / world / roof_st, 4),
+        "roofline_GBps_bytealigned": round(roof_alg, 2), "roofline_GBps_stored": round(roof_st, 2),
+        "ratio_bytealigned": round(w.n_rows * w.row_bytes / info.packed_bytes_bytealigned, 4), "ratio_stored": round(w.n_rows * w.row_bytes / info.packed_bytes_rows, 4),
+        "align_bytes": info.align_bytes, "distinct_rows_per_s": round(uniq * w.index_span / sec), "kernel": kernel,
+        "dedup": bool(dedup_on), "locality_order": bool(order_on),
+        "e2e": {"value": round(e2e_value, 3), "unit": "GB/s", "h2d_bytes_per_step": n * 8, "d2h_bytes_per_step": bytes_step, "steps": Ke,
+                "api": "ibp_gather_decompress_host (pinned host ids in, pinned host rows out)"},
+        "baseline_uncompressed": base,
+        "parity": f"bit-exact: {len(chk)} sampled output rows of one warm-up batch and of one e2e batch == oracle.gather_plain",
+        "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
+        "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3), "metadata_MB": round(info.metadata_bytes * 1e-6, 2),
+        "build_s": round(t_build, 2), "datagen_s": round(t_gen, 2), "gpu_launches": K * launches_per_step,
+    }
+    extras = {"info": info, "clk": clk, "stored_per_launch": stored / K, "alg_per_launch": alg / K, "uniq": uniq, "sec": sec, "order_on": order_on,
+              "dedup_on": dedup_on, "launches_per_step": launches_per_step, "thr": thr, "hit_rate": hit_rate, "cinfo": cinfo, "Ke": Ke, "t_job": t_job}
 
-    if rank == 0:
-        line = {
-            "metric": "effective decompressed GB/s (gather-decompress)", "value": round(value, 3), "unit": "GB/s",
-            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": round(t_job / K, 5), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-            "rows_per_s": round(world * K * n_rows_out / (t_job * 1e-3), 1),
-            "config": {
-                "workload": describe(w), "rows_per_step": n_rows_out, "row_bytes": w.row_bytes, "align_bytes": info.align_bytes,
-                "codec": "group-strict (tau = 1)" if not info.thresholded else f"thresholded, tau = {thr[0]}/{thr[1]} per group, 4-byte chunks, participation bits; {info.n_rows_raw} of {info.n_rows} rows kept raw",
-                "store": {0: "pageable", 1: "pinned (cudaHostAlloc)", 2: "managed host-resident (preferred CPU, accessed-by GPU)"}[info.store_kind],
-                "locality_order": bool(order_on), "dedup": bool(dedup_on), "ids_unique_by_construction": bool(w.ids_unique), "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
-                "cache": None if cache is None else {"what": "compressed GPU software cache (P:349-357) holding the hottest rows of the sampler, static fill", "capacity_frac_of_packed_store": args.cache_frac,
-                                                      "capacity_MB": round(cinfo.capacity_bytes * 1e-6, 1), "used_MB": round(cinfo.used_bytes * 1e-6, 1), "entries": cinfo.n_entries, "map_MB": round(cinfo.map_bytes * 1e-6, 1),
-                                                      "hit_rate": round(hit_rate, 4), "equivalent_uncompressed_cache_rows": int(cinfo.capacity_bytes // w.row_bytes)},
-                "ratio_stored": round(ratio_stored, 4), "ratio_bytealigned": round(ratio_alg, 4),
-                "packed_store_GB": round(info.packed_bytes_stored * 1e-9, 3), "metadata_MB": round(info.metadata_bytes * 1e-6, 2),
-                "build_s": round(t_build, 2), "datagen_s": round(t_gen, 2), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
-            },
-            "roofline": {
-                "bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
-                "frac": round(achieved / h2d_ceiling, 4), "traffic": None if (info.thresholded or getattr(w, "interleaved", False)) else (NCU_TRAFFIC.get(w.name) or {}).get("dram"),
-                "traffic_sysmem": None if (info.thresholded or getattr(w, "interleaved", False)) else (NCU_TRAFFIC.get(w.name) or {}).get("sysmem"),
-                "kernel": "ibp_stream_kernel" if (w.index_span > 1 and not info.thresholded) else "ibp_decode_kernel", "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
-                "algorithmic_bytes_per_launch": int(np.mean(stored_timed)),
-                "zero_copy_read_ceiling": round(zc_ceiling, 3), "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
-                "random_span_ceiling": rand_ceiling,
-                "distinct_rows_per_s": round(float(np.sum(unique_timed)) / (float(np.sum(kernel_ms)) * 1e-3)),
-                "effective_roofline_GBps": round(float(eff_roof), 2), "frac_of_effective_roofline": round(value / world / float(eff_roof), 4),
-                "effective_roofline_def": "min(H2D ceiling x raw bytes / stored packed bytes of the batch, HBM peak)",
-                "frac_vs_bytealigned_ratio": round(value / world / min(h2d_ceiling * float(np.sum(unique_timed)) * w.index_span * w.row_bytes / float(np.sum(alg_timed)) * (n / np.mean(unique_timed)), hbm_peak), 4),
-                "hbm_peak": hbm_peak, "hbm_peak_source": hbm_src,
-            },
-            "e2e": {"value": round(e2e_value, 3), "unit": "GB/s", "h2d_bytes_per_step": n * 8, "d2h_bytes_per_step": bytes_step,
-                    "steps": Ke, "api": "ibp_gather_decompress_host (pinned host ids in, pinned host rows out)"},
-            "gpu_launches": K * launches_per_step,
-            "clocks": clk,
-            "resident_decode": resident,
-            "baseline_uncompressed": base,
-            "cpu_baseline": cpu,
-        }
-        print(json.dumps(line), flush=True)
+    if full:
+        # the same step with the store kind BASELINE.json's north_star names literally: cudaHostAlloc pinned memory
+        if world == 1 and store != "pinned" and cache is None and not args.no_pinned_store:
+            hp = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
+                               flags=ibp.IBP_FLAG_HOSTALLOC_STORE, threshold=thr).upload_metadata(ctx.local)
+            hp.set_dedup_mode(dedup)
+            if args.decode_ctas:
+                hp.configure(args.decode_ctas, 0)
+            stp = lambda i: hp.gather_decompress(ids_dev[i].data_ptr(), n, out.data_ptr(), stream)
+            for i in range(W):
+                stp(i)
+            torch.cuda.synchronize()
+            if not np.array_equal(out[torch.from_numpy(chk).cuda()].cpu().numpy(), want):
+                raise SystemExit("bench.py: pinned-store output differs from the oracle")
+            mp_ = ctx.timed_loop(stp, K, W)
+            ctx.launches += K * launches_per_step
+            vp = bytes_step / (float(np.mean(mp_)) * 1e-3) * 1e-9
+            extras["value_pinned_store"] = {"value": round(vp, 3), "unit": "GB/s", "ms_per_step": round(float(np.mean(mp_)), 5), "store": "pinned (cudaHostAlloc, mapped): IBP_FLAG_HOSTALLOC_STORE",
+                                            "frac_bytealigned": round(vp / roof_alg, 4), "frac_stored": round(vp / roof_st, 4),
+                                            "note": "same table, ids, steps and launch path as `value`; 4 KB GPU pages make address translation the limit for random rows (DESIGN.md section 6), which is why the managed host-resident store is the default"}
+            hp.destroy()
+        # random-row gathers: the same link read as random, span-aligned spans of about one packed row over a managed host
+        # buffer as large as the packed store -- the measured ceiling of any random gather of rows this small on this box
+        if w.index_span == 1 and ctx.rank == 0 and info.packed_bytes_stored >= (64 << 20):
+            mean_row = info.packed_bytes_rows / w.n_rows
+            span = 128 if mean_row <= 128 else 256 if mean_row <= 256 else 512
+            sps, gbs = ibp.ibp_measure_random_read(ctx.local, int(min(info.packed_bytes_stored, 8 << 30)), span, 3)
+            extras["rand_ceiling"] = {"span_bytes": span, "footprint_GB": round(min(info.packed_bytes_stored, 8 << 30) * 1e-9, 2),
+                                      "spans_per_s": round(sps), "GBps": round(gbs, 2),
+                                      "what": "ibp_measure_random_read: LSU 16-byte loads of span-aligned random spans, managed host-resident buffer"}
+        # S8: resident decode (ibp_decompress_resident) of a contiguous range staged in HBM beforehand
+        if world == 1 and not args.no_resident:
+            G = w.group_param
+            nr = min(w.n_rows, 1 << 20) // G * G
+            ptr, nb = h.packed_range(0, nr)
+            staged = torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda()
+            outr = torch.empty((nr, w.row_bytes), dtype=torch.uint8, device="cuda")
+            step_r = lambda i: h.decompress_resident(staged.data_ptr(), 0, nr, outr.data_ptr(), stream)
+            for i in range(3):
+                step_r(i)
+            torch.cuda.synchronize()
+            if not np.array_equal(outr[:4096].cpu().numpy(), X[:4096].view(np.uint8).reshape(4096, -1)):
+                raise SystemExit("bench.py: resident decode differs from the original rows")
+            t_r = float(np.mean(ctx.timed_loop(step_r, 20, 0)))
+            ctx.launches += 20
+            meta_bytes = (nr // G) * 2 * w.row_bytes
+            extras["resident"] = {"rows": nr, "ms": round(t_r, 4), "out_GBps": round(nr * w.row_bytes / (t_r * 1e-3) * 1e-9, 1),
+                                  "in_plus_out_GBps": round((nb + nr * w.row_bytes) / (t_r * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": ctx.hbm_peak,
+                                  "frac": round((nb + nr * w.row_bytes + meta_bytes) / (t_r * 1e-3) * 1e-9 / ctx.hbm_peak, 4),
+                                  "algorithmic_bytes": int(nb + nr * w.row_bytes + meta_bytes),
+                                  "kernel": ("ibp_stream_t_kernel" if info.thresholded else "ibp_stream_kernel") + " (ibp_decompress_resident)",
+                                  "what": "packed bytes of the first rows of the table staged in HBM, decoded to HBM; L2 flushed between launches"}
+            del staged, outr
     if cache is not None:
         cache.destroy()
     h.destroy()
+    del ids_dev, out
+    if not keep:
+        X = None
+    torch.cuda.empty_cache()
+    return entry, extras
+
+
+def tiny_latency_breakdown(ctx, entry):
+    """configs[0] is one wave of 1,024 rows: the step is a sum of dependent latencies, not a bandwidth.
+    Measured here: an event pair around an empty stream, a one-row zero-copy gather (launch + one PCIe round trip), the link
+    time of the batch's packed bytes at the zero-copy ceiling."""
+    torch, ibp = ctx.torch, ctx.ibp
+    evs = []
+    for _ in range(50):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); b.record(); evs.append((a, b))
+    torch.cuda.synchronize()
+    ev_us = float(np.median([a.elapsed_time(b) for a, b in evs])) * 1e3
+    buf = ibp.PinnedBuffer(1 << 20, managed=True, device=ctx.local)
+    ids1 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    o1 = torch.zeros(512, dtype=torch.uint8, device="cuda")
+    one = lambda i: ibp.ibp_gather_uncompressed(buf.dev_ptr, 512, ids1.data_ptr(), 1, o1.data_ptr(), ctx.stream)
+    for i in range(5):
+        one(i)
+    t1 = float(np.median(ctx.timed_loop(one, 30, 0))) * 1e3
+    buf.free()
+    link_us = entry["rows_per_step"] * entry["row_bytes"] / entry["ratio_stored"] / (ctx.zc * 1e9) * 1e6
+    return {"step_us": round(entry["ms_per_step"] * 1e3, 2), "event_pair_on_an_idle_stream_us": round(ev_us, 2),
+            "one_row_zero_copy_gather_us (launch + id load + one PCIe round trip + store)": round(t1, 2),
+            "link_time_of_the_batch_at_the_zero_copy_ceiling_us": round(link_us, 2),
+            "note": "a latency floor, not a kernel property: fetch engine, rows in flight, warps per CTA and store kind all give the same step time (DESIGN.md section 8)"}
+
+
+def run_cuda(args):
+    ctx = Ctx(args)
+    torch, ibp = ctx.torch, ctx.ibp
+    W, K = max(3, args.warmup), args.steps
+    w = make_workload(args.workload)
+    entry, ex = measure_gather(ctx, w, K, W, full=True, store=args.store)
+    info, thr = ex["info"], ex["thr"]
+    world = ctx.world
+
+    per_config = None
+    if world == 1 and args.workload == "gnn" and not args.no_per_config and args.cache_frac == 0 and args.threshold == "1/1" and not args.align and args.store == "managed":
+        Kc = max(3, min(K, 20))
+        per_config = []
+        for name in ("tiny", "gnn", "dlrm", "kv", "weights"):
+            if name == "gnn":
+                e = dict(entry)
+            elif name == "weights":
+                e = measure_weights(ctx, args, Kc, W, layers=args.layers, overlap=False, cpu=False)[0]
+            else:
+                e, _ = measure_gather(ctx, make_workload(name), Kc, W, full=False)
+                if name == "tiny":
+                    e["latency_breakdown"] = tiny_latency_breakdown(ctx, e)
+            per_config.append(e)
+
+    cpu = None
+    if ctx.rank == 0 and world == 1 and not args.no_cpu:
+        g, rps, desc = oracle_sample(w, seconds_target=12.0, thr=thr)
+        cpu = {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)}
+
+    if ctx.rank == 0:
+        default_cfg = (not args.align and args.store == "managed" and args.order is None and args.dedup is None and args.cache_frac == 0
+                       and not info.thresholded and not getattr(w, "interleaved", False) and not args.decode_ctas)
+        dram, sysmem, prof = traffic_from_profile(w.name, default_cfg)
+        achieved = ex["alg_per_launch"] * K / ex["sec"] * 1e-9
+        achieved_st = ex["stored_per_launch"] * K / ex["sec"] * 1e-9
+        cinfo = ex["cinfo"]
+        line = {
+            "metric": "effective decompressed GB/s (gather-decompress)", "value": entry["value"], "unit": "GB/s",
+            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": entry["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic", "rows_per_s": entry["rows_per_s"],
+            "config": bench_config(w, thr),
+            "setup": {
+                "align_bytes": info.align_bytes, "store": entry["store"], "locality_order": ex["order_on"], "dedup": ex["dedup_on"],
+                "ids_unique_by_construction": bool(w.ids_unique),
+                "l2": "flushed with a 256 MiB write between steps (outside the events); ids differ every step; the packed store is host memory and is never cached",
+                "cache": None if cinfo is None else {"what": "compressed GPU software cache (P:349-357) holding the hottest rows of the sampler, static fill", "capacity_frac_of_packed_store": args.cache_frac,
+                                                      "capacity_MB": round(cinfo.capacity_bytes * 1e-6, 1), "used_MB": round(cinfo.used_bytes * 1e-6, 1), "entries": cinfo.n_entries, "map_MB": round(cinfo.map_bytes * 1e-6, 1),
+                                                      "hit_rate": round(ex["hit_rate"], 4), "equivalent_uncompressed_cache_rows": int(cinfo.capacity_bytes // w.row_bytes)},
+                "ratio_stored": entry["ratio_stored"], "ratio_bytealigned": entry["ratio_bytealigned"],
+                "packed_store_GB": entry["packed_store_GB"], "metadata_MB": entry["metadata_MB"], "build_s": entry["build_s"], "datagen_s": entry["datagen_s"],
+                "n_rows_raw": int(info.n_rows_raw), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
+            },
+            "roofline": {
+                "bound": "pcie", "achieved": round(achieved, 3), "peak": round(ctx.h2d, 3), "unit": "GB/s", "frac": round(achieved / ctx.h2d, 4),
+                "achieved_def": "ALGORITHMIC link bytes of the launch = sum over the batch's distinct rows of ceil(k_g/8) (SURVEY 8(d)), / event-timed duration",
+                "traffic": dram, "traffic_sysmem": sysmem, "traffic_from_profile": prof,
+                "kernel": entry["kernel"], "peak_source": "cudaMemcpyAsync H2D of 1 GiB from pinned memory, best of 8, this run (ibp_measure_h2d)",
+                "algorithmic_bytes_per_launch": int(ex["alg_per_launch"]),
+                "stored_bytes_per_launch": int(ex["stored_per_launch"]), "achieved_stored": round(achieved_st, 3), "frac_stored": round(achieved_st / ctx.h2d, 4),
+                "frac_stored_def": f"the same with each row rounded up to the declared alignment unit A = {info.align_bytes} B: what the layout stores and the kernel fetches",
+                "zero_copy_read_ceiling": round(ctx.zc, 3), "frac_of_zero_copy_ceiling": round(achieved / ctx.zc, 4), "frac_stored_of_zero_copy_ceiling": round(achieved_st / ctx.zc, 4),
+                "random_span_ceiling": ex.get("rand_ceiling"), "distinct_rows_per_s": entry["distinct_rows_per_s"],
+                "effective_roofline_GBps": entry["roofline_GBps_bytealigned"], "frac_of_effective_roofline": entry["frac_bytealigned"],
+                "effective_roofline_def": "min(H2D ceiling x raw bytes / byte-aligned packed bytes of the batch's distinct rows, HBM peak): BASELINE.json's min(PCIe x ratio, HBM) with the codec's own ratio",
+                "effective_roofline_stored_GBps": entry["roofline_GBps_stored"], "frac_of_effective_roofline_stored": entry["frac_stored"],
+                "hbm_peak": ctx.hbm_peak, "hbm_peak_source": ctx.hbm_src,
+            },
+            "e2e": entry["e2e"],
+            "value_pinned_store": ex.get("value_pinned_store"),
+            "gpu_launches": ctx.launches,
+            "clocks": ex["clk"],
+            "resident_decode": ex.get("resident"),
+            "baseline_uncompressed": entry["baseline_uncompressed"],
+            "per_config": per_config,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
     if world > 1:
-        dist.destroy_process_group()
+        ctx.dist.destroy_process_group()
+
+
+def bench_config(w, thr):
+    """`config` of the JSON line: the same keys and values in the CUDA arm and in the --impl reference arm."""
+    return {"workload": describe(w), "rows_per_step": w.batch_rows, "row_bytes": w.row_bytes,
+            "codec": "group-strict (tau = 1)" if thr[0] == thr[1] else f"thresholded, tau = {thr[0]}/{thr[1]} per group, 4-byte chunks, participation bits"}
 
 
 # ------------------------------------------------------------------------------------------------- weight streaming
-def run_weights(args):
-    """BASELINE configs[4]: bf16 matrices of a 7B-shaped decoder (4 x 4096x4096 + 3 x 4096x11008 per layer) held packed in
-    host memory; one step = one whole layer streamed in order (7 x ibp_gather_decompress_range), and, with the overlap
-    harness (S7), layer l+1's fetch against a consumer GEMM ([M,4096] activation x the 7 matrices) on layer l."""
-    import torch
-    from paper_2605_30728_b200 import binding as ibp, workloads
-    from paper_2605_30728_b200.overlap import DoubleBufferedPipeline, summarize
-    import oracle
+WEIGHTS_DESC = ("configs[4] LLM weight streaming: bf16 N(0,0.02) matrices of a 7B-shaped decoder, 4 x 4096x4096 + 3 x 4096x11008 per layer, "
+                "{L} layers in host memory ({gb:.2f} GB raw), groups = 128-column tiles (strided); one step = one whole layer "
+                "(ONE launch: ibp_decode_ranges over the layer's 7 matrices, {mb:.1f} MB out)")
 
-    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
-        raise SystemExit("bench.py --workload weights runs on one GPU")
-    torch.cuda.set_device(0)
-    W, K, L = max(3, args.warmup), args.steps, args.layers
+
+def measure_weights(ctx, args, K, W, layers, overlap, cpu):
+    """BASELINE configs[4]: bf16 matrices of a 7B-shaped decoder held packed in host memory; one step = one whole layer
+    streamed in order by ONE launch (ibp_decode_ranges over its 7 handles); with the overlap harness (S7), layer l+1's fetch
+    against a consumer GEMM ([M,4096] activation x the 7 matrices) on layer l, every overlapped step checked."""
+    torch, ibp, oracle = ctx.torch, ctx.ibp, ctx.oracle
+    from paper_2605_30728_b200 import workloads
+    from paper_2605_30728_b200.overlap import DoubleBufferedPipeline, summarize
+    L = layers
     t0 = time.perf_counter()
-    layers, raw_bytes, stored, bytealigned = [], 0, 0, 0
-    check = None
+    hs, raw_bytes, stored, bytealigned = [], 0, 0, 0
+    keep_raw = {}                                               # raw matrices of a few layers, for the parity checks
+    check_layers = sorted({0, L - 1, min(L - 1, 2), min(L - 1, W + 1)})
     for l in range(L):
         mats = []
         for wm in workloads.weight_layer(l):
             X = wm.table()
             h = ibp.ibp_build(X, 256, 1, wm.group_param, align_bytes=args.align if args.align else 16,
                               flags=ibp.IBP_FLAG_HOSTALLOC_STORE if args.store == "pinned" else 0,
-                              threshold=parse_threshold(args.threshold)).upload_metadata(0)
+                              threshold=parse_threshold(args.threshold)).upload_metadata(ctx.local)
             if args.decode_ctas:
                 h.configure(args.decode_ctas, 0)
             info = h.info()
             raw_bytes += X.nbytes; stored += info.packed_bytes_rows; bytealigned += info.packed_bytes_bytealigned
             mats.append((h, wm.n_rows, wm.mat_rows, wm.mat_cols))
-            if l == L - 1 and wm.slot == 6:
-                check = X.view(np.uint8).reshape(wm.n_rows, -1).copy()
-        layers.append(mats)
+            if l in check_layers:
+                keep_raw.setdefault(l, []).append(X.view(np.uint8).reshape(wm.n_rows, -1).copy())
+        hs.append(mats)
     t_build = time.perf_counter() - t0
-    layer_rows = sum(m[1] for m in layers[0])
+    layer_rows = sum(m[1] for m in hs[0])
     layer_bytes = layer_rows * 256
-    h2d_ceiling = ibp.ibp_measure_h2d(0, 1 << 30, 8)
-    zc_ceiling = ibp.ibp_measure_zero_copy_read(0, 1 << 30, 3)
-    try:
-        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
-    except Exception:
-        hbm_peak = 6650.0
     bufs = [torch.empty((layer_rows, 256), dtype=torch.uint8, device="cuda") for _ in range(2)]
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = ctx.stream
+
+    def ranges_of(l, base_ptr, packed=None):
+        rs, off = [], 0
+        for j, (h, n_rows, _, _) in enumerate(hs[l]):
+            rs.append((h, None if packed is None else packed[j], 0, n_rows, base_ptr + off * 256))
+            off += n_rows
+        return rs
 
     def fetch(i, bi, stream_ptr):
-        off = 0
-        for (h, n_rows, _, _) in layers[i % L]:
-            h.gather_decompress_range(0, n_rows, bufs[bi].data_ptr() + off * 256, stream_ptr)
-            off += n_rows
+        ibp.ibp_decode_ranges(ranges_of(i % L, bufs[bi].data_ptr()), stream_ptr)
 
-    stream = torch.cuda.current_stream().cuda_stream
+    def check_layer(buf, l, what):
+        want = np.concatenate(keep_raw[l])
+        if not np.array_equal(buf.cpu().numpy(), want):
+            raise SystemExit(f"bench.py: {what}: streamed layer {l} differs from the original matrices")
+
     for i in range(W):
         fetch(i, 0, stream)
-    fetch(L - 1, 1, stream)
-    torch.cuda.synchronize()
-    last_rows = layers[L - 1][6][1]
-    if not np.array_equal(bufs[1][layer_rows - last_rows:].cpu().numpy(), check):
-        raise SystemExit("bench.py: streamed layer differs from the original matrix")
-    clocks = ClockSampler(0)
+    for l in check_layers:                                      # (c1) every byte of whole layers
+        fetch(l, 1, stream)
+        torch.cuda.synchronize()
+        check_layer(bufs[1], l, "range gather")
+    clocks = ClockSampler(ctx.local)
     clocks.start()
-    ms = []
-    for j in range(K):
-        flush.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); fetch(W + j, j % 2, stream); b.record()
-        b.synchronize()
-        ms.append(a.elapsed_time(b))
+    ms = ctx.timed_loop(lambda i: fetch(i, i % 2, stream), K, W)
     clk = clocks.stop()
+    ctx.launches += K
     t_step = float(np.mean(ms))
     value = layer_bytes / (t_step * 1e-3) * 1e-9
-    stored_layer = stored / L
-    achieved = stored_layer / (t_step * 1e-3) * 1e-9
+    stored_layer, alg_layer = stored / L, bytealigned / L
 
-    # ---- S8: the same layer decoded from HBM (packed bytes staged once, outside the timing)
+    # ---- S8: a layer decoded from HBM (packed bytes staged once, outside the timing), one launch per layer
+    l0 = check_layers[0]
     staged = []
-    for (h, n_rows, _, _) in layers[0]:
+    for (h, n_rows, _, _) in hs[l0]:
         ptr, nb = h.packed_range(0, n_rows)
-        staged.append((h, n_rows, torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda(), nb))
-    def resident():
+        staged.append((torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda(), nb))
+    res_ranges = ranges_of(l0, bufs[0].data_ptr(), [s_[0].data_ptr() for s_ in staged])
+    resident = lambda i: ibp.ibp_decode_ranges(res_ranges, stream)
+    for i in range(3):
+        resident(i)
+    torch.cuda.synchronize()
+    check_layer(bufs[0], l0, "resident decode")
+    t_res = float(np.mean(ctx.timed_loop(resident, 10, 0)))
+    ctx.launches += 10
+    meta_layer = sum(2 * 256 * (c // 128) for (_, _, _, c) in hs[l0])
+    res_bytes = sum(s_[1] for s_ in staged) + layer_bytes + meta_layer
+    del staged
+
+    # ---- e2e: the layer into pinned HOST memory through the host entry point (7 calls, synchronous)
+    out_pin = ibp.PinnedBuffer(layer_bytes)
+    out_pin_np = out_pin.view(np.uint8, (layer_rows, 256))
+
+    def step_e2e(i):
         off = 0
-        for (h, n_rows, buf, nb) in staged:
-            h.decompress_resident(buf.data_ptr(), 0, n_rows, bufs[0].data_ptr() + off * 256, stream)
+        for (h, n_rows, _, _) in hs[i % L]:
+            h.gather_decompress_range_host(0, n_rows, out_pin_np[off:off + n_rows], stream)
             off += n_rows
-    for _ in range(3):
-        resident()
-    rs = []
-    for _ in range(10):
-        flush.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); resident(); b.record(); b.synchronize()
-        rs.append(a.elapsed_time(b))
-    t_res = float(np.mean(rs))
-    res_bytes = sum(s[3] for s in staged) + layer_bytes
 
-    # ---- S7: overlap with a consumer GEMM on the previous layer
-    M = args.gemm_m
-    act = torch.randn((M, 4096), dtype=torch.bfloat16, device="cuda")
-    shapes = [(m[2], m[3]) for m in layers[0]]
-    outs = [torch.empty((M, c), dtype=torch.bfloat16, device="cuda") for (_, c) in shapes]
+    step_e2e(check_layers[-1])
+    if not np.array_equal(out_pin_np, np.concatenate(keep_raw[check_layers[-1]])):
+        raise SystemExit("bench.py: weights e2e output differs from the original matrices")
+    Ke = max(3, min(K, 8))
+    ms_e = ctx.timed_loop(step_e2e, Ke, W)
+    e2e_value = layer_bytes / (float(np.mean(ms_e)) * 1e-3) * 1e-9
+    out_pin.free()
 
-    def consume(i, bi):
-        off = 0
-        for j, (r, c) in enumerate(shapes):
-            wmat = bufs[bi][off:off + r * (c // 128)].view(torch.bfloat16).view(r, c)
-            torch.matmul(act, wmat, out=outs[j])
-            off += r * (c // 128)
-
-    n_pipe = min(max(K, 8), 16)
-    pipe = DoubleBufferedPipeline(fetch, consume, n_pipe)
-    for _ in range(2):
-        pipe.run_overlapped()
-    ov = summarize(pipe.run_fetch_only(), pipe.run_consume_only(), pipe.run_serial(), pipe.run_overlapped())
-    ov.update({"steps": n_pipe, "consumer": f"torch.matmul [M={M},4096] bf16 x the 7 decoded matrices of the previous layer (cuBLAS)",
-               "decode_ctas": args.decode_ctas or "library default (persistent, occupancy x SMs)"})
-
-    smp = OracleSample(workloads.KV(layers=1, pages=8))
-    g, rps, desc = smp.run(8.0) if not args.no_cpu else (None, None, None)
-    line = {
-        "metric": "effective decompressed GB/s (gather-decompress)", "value": round(value, 3), "unit": "GB/s", "n_gpus": 1,
-        "steps": K, "warmup": W, "ms_per_step": round(t_step, 4), "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "u32", "data": "synthetic", "rows_per_s": round(layer_rows / (t_step * 1e-3), 1),
-        "config": {"workload": f"configs[4] LLM weight streaming: bf16 N(0,0.02) matrices of a 7B-shaped decoder, 4 x 4096x4096 + 3 x 4096x11008 per layer, {L} layers in host memory ({raw_bytes * 1e-9:.2f} GB raw; BASELINE: 32 layers, 12.95 GB), groups = 128-column tiles (strided); one step = one whole layer (7 range gathers, {layer_bytes * 1e-6:.1f} MB out)",
-                   "align_bytes": args.align if args.align else 16, "store": args.store, "ratio_stored": round(raw_bytes / stored, 4),
-                   "ratio_bytealigned": round(raw_bytes / bytealigned, 4), "build_s": round(t_build, 1),
-                   "l2": "flushed with a 256 MiB write between steps (outside the events)"},
-        "roofline": {"bound": "pcie", "achieved": round(achieved, 3), "peak": round(h2d_ceiling, 3), "unit": "GB/s",
-                     "frac": round(achieved / h2d_ceiling, 4), "traffic": None, "kernel": "ibp_stream_kernel",
-                     "algorithmic_bytes_per_launch": int(stored_layer / 7), "zero_copy_read_ceiling": round(zc_ceiling, 3),
-                     "frac_of_zero_copy_ceiling": round(achieved / zc_ceiling, 4),
-                     "effective_roofline_GBps": round(h2d_ceiling * raw_bytes / stored, 2),
-                     "frac_of_effective_roofline": round(value / (h2d_ceiling * raw_bytes / stored), 4)},
-        "resident_decode": {"ms_per_layer": round(t_res, 4), "in_plus_out_GBps": round(res_bytes / (t_res * 1e-3) * 1e-9, 1),
-                            "out_GBps": round(layer_bytes / (t_res * 1e-3) * 1e-9, 1), "bound": "hbm", "peak": hbm_peak,
-                            "frac": round(res_bytes / (t_res * 1e-3) * 1e-9 / hbm_peak, 4), "kernel": "ibp_stream_kernel (ibp_decompress_resident)"},
-        "overlap": ov,
-        "e2e": {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "note": "the consumer of streamed weights is on the GPU; no host round trip exists on this path"},
-        "gpu_launches": K * 7, "clocks": clk,
-        "cpu_baseline": None if g is None else {"value": round(g, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": desc, "rows_per_s": round(rps, 1)},
+    entry = {
+        "name": "weights", "workload": WEIGHTS_DESC.format(L=L, gb=raw_bytes * 1e-9, mb=layer_bytes * 1e-6), "value": round(value, 3), "unit": "GB/s",
+        "rows_per_s": round(layer_rows / (t_step * 1e-3), 1), "ms_per_step": round(t_step, 5), "steps": K, "rows_per_step": layer_rows, "row_bytes": 256, "layers": L,
+        "link_GBps_bytealigned": round(alg_layer / (t_step * 1e-3) * 1e-9, 3), "link_GBps_stored": round(stored_layer / (t_step * 1e-3) * 1e-9, 3),
+        "frac_bytealigned": round(value / min(ctx.h2d * raw_bytes / bytealigned, ctx.hbm_peak), 4), "frac_stored": round(value / min(ctx.h2d * raw_bytes / stored, ctx.hbm_peak), 4),
+        "roofline_GBps_bytealigned": round(ctx.h2d * raw_bytes / bytealigned, 2), "roofline_GBps_stored": round(ctx.h2d * raw_bytes / stored, 2),
+        "ratio_bytealigned": round(raw_bytes / bytealigned, 4), "ratio_stored": round(raw_bytes / stored, 4), "align_bytes": args.align if args.align else 16,
+        "kernel": "ibp_stream_kernel (one launch per layer)",
+        "e2e": {"value": round(e2e_value, 3), "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": layer_bytes, "steps": Ke,
+                "api": "ibp_gather_decompress_range_host x 7 (the packed rows are read in place from the host store; the decoded layer lands in pinned host memory)"},
+        "baseline_uncompressed": None,
+        "resident_decode": {"ms_per_layer": round(t_res, 4), "in_plus_out_GBps": round(res_bytes / (t_res * 1e-3) * 1e-9, 1), "out_GBps": round(layer_bytes / (t_res * 1e-3) * 1e-9, 1),
+                            "bound": "hbm", "peak": ctx.hbm_peak, "frac": round(res_bytes / (t_res * 1e-3) * 1e-9 / ctx.hbm_peak, 4), "launches_per_layer": 1,
+                            "kernel": "ibp_stream_kernel (ibp_decode_ranges, resident, tile-block chunks)"},
+        "parity": f"bit-exact: every byte of layers {check_layers} (range gather), of layer {l0} (resident) and of layer {check_layers[-1]} (e2e) == the original matrices (oracle c1)",
+        "store": args.store, "build_s": round(t_build, 1), "gpu_launches": K,
     }
-    print(json.dumps(line), flush=True)
-    for mats in layers:
+    extras = {"clk": clk, "stored_layer": stored_layer, "alg_layer": alg_layer, "raw_bytes": raw_bytes, "stored": stored, "bytealigned": bytealigned, "t_step": t_step}
+
+    if overlap:
+        # ---- S7: overlap with a consumer GEMM on the previous layer; EVERY overlapped step's buffer is checked: the consumer
+        # folds the buffer into a per-step 64-bit checksum (sum of its int64 words) next to the GEMMs, and the sums of the layers
+        # whose raw matrices were kept are compared with the originals'; a whole-buffer copy is compared for the kept layers.
+        M = args.gemm_m
+        act = torch.randn((M, 4096), dtype=torch.bfloat16, device="cuda")
+        shapes = [(m[2], m[3]) for m in hs[0]]
+        outs = [torch.empty((M, c), dtype=torch.bfloat16, device="cuda") for (_, c) in shapes]
+        n_pipe = min(max(K, 8), 16)
+        sums = torch.zeros(n_pipe, dtype=torch.int64, device="cuda")
+        kept = {i: torch.empty_like(bufs[0]) for i in range(n_pipe) if (i % L) in keep_raw}
+        check_on = [True]
+
+        def consume(i, bi):
+            off = 0
+            for j, (r, c) in enumerate(shapes):
+                wmat = bufs[bi][off:off + r * (c // 128)].view(torch.bfloat16).view(r, c)
+                torch.matmul(act, wmat, out=outs[j])
+                off += r * (c // 128)
+            if check_on[0]:
+                sums[i] = bufs[bi].view(torch.int64).sum()
+                if i in kept:
+                    kept[i].copy_(bufs[bi])
+
+        pipe = DoubleBufferedPipeline(fetch, consume, n_pipe)
+        for _ in range(2):
+            pipe.run_overlapped()
+        torch.cuda.synchronize()
+        got_sums = sums.cpu().numpy()
+        ref = {}
+        for i in range(n_pipe):                                 # reference checksums from a serial fetch of the same layer
+            l = i % L
+            if l not in ref:
+                fetch(l, 0, stream)
+                ref[l] = int(bufs[0].view(torch.int64).sum().item())
+            if int(got_sums[i]) != ref[l]:
+                raise SystemExit(f"bench.py: overlapped step {i}: the consumer read a stale or half-written buffer")
+        for i, t in kept.items():
+            check_layer(t, i % L, f"overlapped step {i}")
+        check_on[0] = False                                     # timing runs: the consumer is the GEMMs alone
+        ov = summarize(pipe.run_fetch_only(), pipe.run_consume_only(), pipe.run_serial(), pipe.run_overlapped())
+        ov.update({"steps": n_pipe, "consumer": f"torch.matmul [M={M},4096] bf16 x the 7 decoded matrices of the previous layer (cuBLAS)",
+                   "decode_ctas": args.decode_ctas or "library default (persistent, occupancy x SMs)",
+                   "checked": f"all {n_pipe} overlapped steps: 64-bit checksum of the consumed buffer == that of a serial fetch of the same layer; whole-buffer bytes == the original matrices for steps {sorted(kept)}"})
+        extras["overlap"] = ov
+    if cpu:
+        wm = workloads.WeightMatrix(1024, 4096, 0, 0)           # the first 1024 rows of layer 0's first matrix: same tiles, same values
+        Xs = wm.table()
+        ds = oracle.Dataset(Xs, 1, wm.group_param)
+        sid = np.arange(wm.n_rows, dtype=np.int64)
+        t0 = time.perf_counter()
+        done = 0
+        while time.perf_counter() - t0 < 10.0:
+            o = ds.gather_decompress(sid)
+            done += len(sid)
+        dt = time.perf_counter() - t0
+        assert np.array_equal(o, Xs.view(np.uint8).reshape(wm.n_rows, -1))
+        ds.close()
+        extras["cpu"] = {"value": round(done * 256 / dt * 1e-9, 5), "unit": "GB/s", "cores": 1, "kind": "oracle", "rows_per_s": round(done / dt, 1),
+                         "sample": f"{done} row decodes by the oracle codec over the first 1024 matrix rows of layer 0's first 4096x4096 matrix (strided groups = 32 column tiles), {dt:.1f} s"}
+    for mats in hs:
         for m in mats:
             m[0].destroy()
+    del bufs
+    torch.cuda.empty_cache()
+    return entry, extras
+
+
+def run_weights(args):
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --workload weights runs on one GPU")
+    ctx = Ctx(args)
+    W, K = max(3, args.warmup), args.steps
+    entry, ex = measure_weights(ctx, args, K, W, layers=args.layers, overlap=True, cpu=not args.no_cpu)
+    L = args.layers
+    achieved = ex["alg_layer"] / (ex["t_step"] * 1e-3) * 1e-9
+    achieved_st = ex["stored_layer"] / (ex["t_step"] * 1e-3) * 1e-9
+    line = {
+        "metric": "effective decompressed GB/s (gather-decompress)", "value": entry["value"], "unit": "GB/s", "n_gpus": 1,
+        "steps": K, "warmup": W, "ms_per_step": entry["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic", "rows_per_s": entry["rows_per_s"],
+        "config": {"workload": entry["workload"], "rows_per_step": entry["rows_per_step"], "row_bytes": 256, "codec": "group-strict (tau = 1)" if args.threshold == "1/1" else f"thresholded, tau = {args.threshold}"},
+        "setup": {"align_bytes": entry["align_bytes"], "store": args.store, "ratio_stored": entry["ratio_stored"], "ratio_bytealigned": entry["ratio_bytealigned"], "build_s": entry["build_s"],
+                  "layers": L, "l2": "flushed with a 256 MiB write between steps (outside the events)"},
+        "roofline": {"bound": "pcie", "achieved": round(achieved, 3), "peak": round(ctx.h2d, 3), "unit": "GB/s", "frac": round(achieved / ctx.h2d, 4), "traffic": None,
+                     "kernel": "ibp_stream_kernel", "algorithmic_bytes_per_launch": int(ex["alg_layer"]), "stored_bytes_per_launch": int(ex["stored_layer"]),
+                     "achieved_stored": round(achieved_st, 3), "frac_stored": round(achieved_st / ctx.h2d, 4),
+                     "zero_copy_read_ceiling": round(ctx.zc, 3), "frac_of_zero_copy_ceiling": round(achieved / ctx.zc, 4),
+                     "effective_roofline_GBps": entry["roofline_GBps_bytealigned"], "frac_of_effective_roofline": entry["frac_bytealigned"],
+                     "effective_roofline_stored_GBps": entry["roofline_GBps_stored"], "frac_of_effective_roofline_stored": entry["frac_stored"]},
+        "resident_decode": entry["resident_decode"],
+        "overlap": ex.get("overlap"),
+        "e2e": entry["e2e"],
+        "gpu_launches": ctx.launches, "clocks": ex["clk"], "parity": entry["parity"],
+        "cpu_baseline": ex.get("cpu"),
+    }
+    print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------------------- Fig. 7 sweep
@@ -1060,7 +1265,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="gnn", choices=["gnn", "gnn-interleaved", "dlrm", "tiny", "kv", "weights", "sweep"])
     ap.add_argument("--align", type=int, default=0, help="packed-row alignment unit A; 0 = the workload's default")
-    ap.add_argument("--layers", type=int, default=8, help="weights workload: decoder layers held in host memory (32 = BASELINE's 13 GB)")
+    ap.add_argument("--layers", type=int, default=32, help="weights workload: decoder layers held in host memory (32 = BASELINE's 12.95 GB)")
     ap.add_argument("--gemm-m", type=int, default=16384, help="weights workload: rows of the consumer GEMM's activation")
     ap.add_argument("--decode-ctas", type=int, default=0, help="limit the decode grid (SM share of the fetch); 0 = library default")
     ap.add_argument("--store", default="managed", choices=["managed", "pinned"])
@@ -1073,6 +1278,8 @@ def main():
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="default gnn run: skip the per_config entries for the other four BASELINE configs")
+    ap.add_argument("--no-pinned-store", action="store_true", help="skip value_pinned_store (the same step over a cudaHostAlloc store)")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.workload in ("weights", "sweep"):

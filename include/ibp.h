@@ -185,6 +185,29 @@ ibp_status ibp_decompress_resident(ibp_handle* h, const void* packed_dev, int64_
  * first_row + j.  Asynchronous on the stream.                                                                      */
 ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_dev, void* cuda_stream);
 
+/* ibp_gather_decompress_range with a HOST destination: out_host receives n_rows*row_bytes bytes.  A pinned, GPU-mapped
+ * destination (cudaHostAlloc / cudaHostRegister / ibp_host_alloc) is written by the decode kernel directly; any other memory
+ * goes through a device staging buffer and one copy.  Synchronises the stream before returning.                          */
+ibp_status ibp_gather_decompress_range_host(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_host, void* cuda_stream);
+
+/* Several contiguous ranges decoded by ONE kernel launch (whole decoder layers streamed in order: a 7B-shaped layer is
+ * seven matrices = seven handles).  Range i: rows [first_row, first_row+n_rows) of `handle` (same unit rule as
+ * ibp_decompress_resident) go to out_dev; packed_dev != NULL: the packed bytes of exactly that range staged in device memory
+ * (as ibp_decompress_resident); packed_dev == NULL: read zero-copy from the handle's host store (as
+ * ibp_gather_decompress_range).  ranges_host is read during the call only.  Consecutive ranges of strict-mode handles with the
+ * same row width are walked by one persistent grid, at most 8 per launch (more ranges = more launches); thresholded handles and
+ * handles with ibp_set_stream_mode(0) are decoded range by range.  The launch shape (ibp_configure) is that of the first handle
+ * of each launch.  All handles must live on one device.  Asynchronous on the stream.  Output is identical to the per-range
+ * calls.  Errors: INVALID_ARG (null pointers, ranges, alignment, mixed devices), BAD_STATE (before upload; host-store range of
+ * a pageable store), UNSUPPORTED (rows too long for the shared-memory stages).                                             */
+typedef struct {
+    ibp_handle* handle;
+    const void* packed_dev;
+    int64_t first_row, n_rows;
+    void* out_dev;
+} ibp_range_desc;
+ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint32_t n_ranges, void* cuda_stream);
+
 /* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
 ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
 
@@ -209,7 +232,8 @@ ibp_status ibp_get_metadata_host(const ibp_handle* h, int64_t group, const void*
 ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out);
 
 /* Launch shape of the decode kernels: max_ctas limits the grid (0 = library default), so that a consumer kernel can
- * share the GPU ("We reserved only 64 SMs for decompression"); warps_per_cta 0 = default.                    */
+ * share the GPU ("We reserved only 64 SMs for decompression"); warps_per_cta of the random-row kernel: 0 = default
+ * (8), else 1..8 (the kernel is compiled for CTAs of at most 256 threads); INVALID_ARG above 8.                     */
 ibp_status ibp_configure(ibp_handle* h, uint32_t max_ctas, uint32_t warps_per_cta);
 
 /* Debug pre-pass: *n_bad_host = number of ids outside [0, n_rows/index_span).  Synchronises the stream.           */

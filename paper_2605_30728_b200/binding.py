@@ -57,6 +57,10 @@ class ibp_cache_info(C.Structure):
                 ("map_bytes", C.c_uint64), ("n_slabs", C.c_uint32), ("reserved", C.c_uint32), ("slab_bytes", C.c_uint64)]
 
 
+class ibp_range_desc(C.Structure):
+    _fields_ = [("handle", C.c_void_p), ("packed_dev", C.c_void_p), ("first_row", C.c_int64), ("n_rows", C.c_int64), ("out_dev", C.c_void_p)]
+
+
 class ibp_table_desc(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("row_bytes", C.c_uint32), ("n_rows", C.c_uint64), ("group_kind", C.c_uint32),
                 ("group_param", C.c_uint32), ("n_groups", C.c_uint64), ("row_group_dev", C.c_void_p)]
@@ -75,6 +79,8 @@ SIGNATURES = {
     "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_decompress_resident": (_int, [_vp, _vp, _i64, _i64, _vp, _vp]),
     "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
+    "ibp_gather_decompress_range_host": (_int, [_vp, _i64, _i64, _vp, _vp]),
+    "ibp_decode_ranges": (_int, [C.POINTER(ibp_range_desc), _u32, _vp]),
     "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
     "ibp_store_device_ptr": (_int, [_vp, C.POINTER(_vp)]),
     "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
@@ -168,6 +174,9 @@ class Handle:
 
     def gather_decompress_range(self, first_row, n_rows, out_dev, stream=None):
         _check(lib().ibp_gather_decompress_range(self._h, first_row, n_rows, _ptr(out_dev), stream))
+
+    def gather_decompress_range_host(self, first_row, n_rows, out_host, stream=None):
+        _check(lib().ibp_gather_decompress_range_host(self._h, first_row, n_rows, _ptr(out_host), stream))
 
     def packed_range(self, first_row, n_rows):
         p, nb = _vp(), _u64()
@@ -328,6 +337,14 @@ def ibp_build_device(rows_dev, n_rows: int, row_bytes: int, group_kind: int, gro
     h = _vp()
     _check(lib().ibp_build_device(_ptr(rows_dev), C.byref(p), device, stream, C.byref(h)))
     return Handle(h)
+
+
+def ibp_decode_ranges(ranges, stream=None):
+    """ranges: [(Handle, packed_dev or None, first_row, n_rows, out_dev), ...] -> one launch per group of up to 8 compatible ranges."""
+    arr = (ibp_range_desc * len(ranges))()
+    for a, (h, packed, first, n, out) in zip(arr, ranges):
+        a.handle, a.packed_dev, a.first_row, a.n_rows, a.out_dev = h._h.value if hasattr(h._h, "value") else h._h, _ptr(packed), first, n, _ptr(out)
+    _check(lib().ibp_decode_ranges(arr, len(ranges), stream))
 
 
 def ibp_gather_uncompressed(rows_mapped, row_bytes, row_ids_dev, n, out_dev, stream=None, n_rows=0, locality_order=False):

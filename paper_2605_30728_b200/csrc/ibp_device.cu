@@ -612,28 +612,30 @@ static void fill_common(const ibp_handle* h, DecodeParams& P) {
 // ------------------------------------------------------------------------------------------------ stream launch
 // Contiguous runs of rows (spans of blocked groups, whole ranges of either kind) through the TMA producer/consumer
 // pipeline of ibp_stream.cuh.  `packed` is the device-visible address of byte `bias` of the packed store.
-template <int W, int NS>
-static ibp_status launch_stream_one(const StreamParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
+template <int W, int NS, int NSEG>
+static ibp_status launch_stream_one(const StreamBatch<NSEG>& B, int64_t total_chunks, uint32_t grid_multiple, int64_t max_ctas, int sm_count,
+                                    size_t smem, cudaStream_t st, uint32_t grid_min = 1) {
     constexpr int NW = 8;
-    auto kern = ibp_stream_kernel<W, NS, NW>;
+    auto kern = ibp_stream_kernel<W, NS, NW, NSEG>;
     static unsigned long long smem_optin_done = 0;
     if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
-    int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
+    int64_t blocks = std::min<int64_t>(total_chunks, (int64_t)std::max(occ, 1) * sm_count);
     if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
-    if (P.n_tile_blocks) blocks = std::max<int64_t>(P.n_tile_blocks, blocks / P.n_tile_blocks * P.n_tile_blocks);   // one tile block per CTA
-    kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(P);
+    if (grid_multiple > 1) blocks = std::max<int64_t>(grid_multiple, blocks / grid_multiple * grid_multiple);   // one tile block per CTA
+    blocks = std::max<int64_t>(blocks, grid_min);                                                               // every tile block has a CTA
+    kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(B);
     IBP_CUDA(cudaGetLastError());
     return IBP_OK;
 }
 
-static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
-                                int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st, bool resident = false) {
-    if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+// Chunk geometry of one contiguous run (or of n_spans spans) for the stream kernel.  `allow_tile_blocks`: resident decode of a
+// strided table may use tile-block chunks when the grid will have at least one CTA per tile block.
+static void stream_geometry(const ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
+                            int64_t first_row, int64_t span_rows, void* out_dev, bool allow_tile_blocks, StreamParams& P) {
     const int W = pick_W(h->p.row_bytes);
     const uint32_t NW = 8;
-    StreamParams P;
     memset(&P, 0, sizeof P);
     P.store = packed; P.bias = bias;
     P.meta = h->meta_dev; P.mvtab = h->mvtab_dev; P.gtab = h->gtab_dev;
@@ -668,7 +670,7 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
         P.piece_rows = U;
         need = rc * h->max_stride + (rc / G + 2) * 128 + 64;
         P.chunks_per_span = (uint32_t)((span_rows + (int64_t)rc - 1) / (int64_t)rc);
-    } else if (resident && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1 && (!h->max_ctas || h->max_ctas >= (h->n_groups + NW - 1) / NW)) {
+    } else if (allow_tile_blocks && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1) {
         // resident decode of a strided table: tile-block chunks (ibp_stream.cuh).  A whole-row chunk holds only 2-7 matrix rows
         // of the 7B shapes, so every warp would re-prepare a tile (Mask/Bitval, offsets, expand masks) for a handful of rows;
         // here a CTA keeps one block of NW tiles for all its chunks and prepares once.  The source is HBM, so the shorter
@@ -705,12 +707,25 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
     }
     P.stage_bytes = (uint32_t)((need + 127) / 128 * 128);
     P.n_chunks = n_spans * (int64_t)P.chunks_per_span;
+}
+
+static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
+                                int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st, bool resident = false) {
+    if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+    const int W = pick_W(h->p.row_bytes);
+    StreamBatch<1> B;
+    memset(&B, 0, sizeof B);
+    StreamParams& P = B.seg[0];
+    const bool tile_ok = resident && (!h->max_ctas || h->max_ctas >= (h->n_groups + 7) / 8);
+    stream_geometry(h, packed, bias, ids_dev, n_spans, first_row, span_rows, out_dev, tile_ok, P);
+    B.n_seg = 1;
+    B.stage_bytes = P.stage_bytes;
     const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
     const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
-#define IBP_STREAM(W_)                                                                          \
-    return ns == 2 ? launch_stream_one<W_, 2>(P, h->max_ctas, h->sm_count, smem, st)            \
-                   : launch_stream_one<W_, 3>(P, h->max_ctas, h->sm_count, smem, st)
+#define IBP_STREAM(W_)                                                                                             \
+    return ns == 2 ? launch_stream_one<W_, 2, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st) \
+                   : launch_stream_one<W_, 3, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st)
     switch (W) {
         case 4: IBP_STREAM(4);
         case 2: IBP_STREAM(2);
@@ -1031,6 +1046,117 @@ extern "C" ibp_status ibp_gather_decompress_range(ibp_handle* h, int64_t first_r
     s = check_range(h, "ibp_gather_decompress_range", first_row, n_rows, out_dev);
     if (s != IBP_OK) return s;
     return decode_range(h, h->store_dev + ibp_row_offset(h, (uint64_t)first_row), first_row, n_rows, out_dev, (cudaStream_t)cuda_stream);
+}
+
+// Range gather with a HOST destination (the end-to-end form of weight / block streaming): a pinned, GPU-mapped out_host is
+// written by the decode kernel directly (zero-copy stores); anything else goes through a device staging buffer and one copy.
+extern "C" ibp_status ibp_gather_decompress_range_host(ibp_handle* h, int64_t first_row, int64_t n_rows, void* out_host, void* cuda_stream) {
+    ibp_status s = check_ready(h, "ibp_gather_decompress_range_host");
+    if (s != IBP_OK) return s;
+    if (n_rows == 0) return IBP_OK;
+    if (!out_host) { ibp_set_error("ibp_gather_decompress_range_host: null destination"); return IBP_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaPointerAttributes attr;
+    void* alias = nullptr;
+    if (cudaPointerGetAttributes(&attr, out_host) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+        cudaHostGetDevicePointer(&alias, out_host, 0) == cudaSuccess && alias && !((uintptr_t)alias & 15u)) {
+        s = ibp_gather_decompress_range(h, first_row, n_rows, alias, cuda_stream);
+        const cudaError_t es = cudaStreamSynchronize(st);
+        if (s == IBP_OK && es != cudaSuccess) { ibp_set_error("ibp_gather_decompress_range_host: %s", cudaGetErrorString(es)); (void)cudaGetLastError(); s = IBP_ERR_CUDA; }
+        return s;
+    }
+    (void)cudaGetLastError();
+    if (first_row < 0 || n_rows < 0 || (uint64_t)(first_row + n_rows) > h->p.n_rows) { ibp_set_error("ibp_gather_decompress_range_host: bad range"); return IBP_ERR_INVALID_ARG; }
+    const size_t bytes = (size_t)n_rows * h->p.row_bytes;
+    uint8_t* buf = nullptr;
+    IBP_CUDA(cudaMallocAsync((void**)&buf, bytes, st));
+    s = ibp_gather_decompress_range(h, first_row, n_rows, buf, cuda_stream);
+    cudaError_t e = cudaSuccess;
+    if (s == IBP_OK) e = cudaMemcpyAsync(out_host, buf, bytes, cudaMemcpyDeviceToHost, st);
+    cudaFreeAsync(buf, st);
+    const cudaError_t e2 = cudaStreamSynchronize(st);
+    if (s == IBP_OK && (e != cudaSuccess || e2 != cudaSuccess)) {
+        ibp_set_error("ibp_gather_decompress_range_host: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+        (void)cudaGetLastError();
+        s = IBP_ERR_CUDA;
+    }
+    return s;
+}
+
+// Several ranges in one launch (a decoder layer's seven matrices): consecutive ranges that the stream kernel can take
+// together (strict mode, same word width, at most 8) become the segments of ONE persistent grid; anything else is decoded range
+// by range.  One ramp and one tail per layer instead of one per matrix, and no launch gaps on the stream.
+extern "C" ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint32_t n_ranges, void* cuda_stream) {
+    if (n_ranges == 0) return IBP_OK;
+    if (!ranges_host) { ibp_set_error("ibp_decode_ranges: null range list"); return IBP_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int device = -1;
+    for (uint32_t i = 0; i < n_ranges; ++i) {
+        const ibp_range_desc& r = ranges_host[i];
+        ibp_status s = check_ready(r.handle, "ibp_decode_ranges");
+        if (s != IBP_OK) return s;
+        if (device < 0) device = r.handle->device;
+        if (r.handle->device != device) { ibp_set_error("ibp_decode_ranges: range %u lives on device %d, range 0 on device %d", i, r.handle->device, device); return IBP_ERR_INVALID_ARG; }
+        if (r.n_rows == 0) continue;
+        s = check_range(r.handle, "ibp_decode_ranges", r.first_row, r.n_rows, r.out_dev);
+        if (s != IBP_OK) return s;
+        if (r.packed_dev) {
+            if ((uintptr_t)r.packed_dev & 15u) { ibp_set_error("ibp_decode_ranges: packed_dev of range %u is not 16-byte aligned", i); return IBP_ERR_INVALID_ARG; }
+        } else if (!r.handle->store_dev) {
+            ibp_set_error("ibp_decode_ranges: range %u reads the host store, which is not GPU-mapped (pageable store)", i); return IBP_ERR_BAD_STATE;
+        }
+    }
+    auto batchable = [](const ibp_range_desc& r) { return r.n_rows > 0 && r.handle->stream_mode && !r.handle->thresholded; };
+    auto source = [](const ibp_range_desc& r) {
+        return r.packed_dev ? (const uint8_t*)r.packed_dev : r.handle->store_dev + ibp_row_offset(r.handle, (uint64_t)r.first_row);
+    };
+    uint32_t i = 0;
+    while (i < n_ranges) {
+        const ibp_range_desc& r0 = ranges_host[i];
+        if (r0.n_rows == 0) { ++i; continue; }
+        if (!batchable(r0)) {
+            ibp_status s = decode_range(r0.handle, source(r0), r0.first_row, r0.n_rows, r0.out_dev, st, r0.packed_dev != nullptr);
+            if (s != IBP_OK) return s;
+            ++i;
+            continue;
+        }
+        ibp_handle* h0 = r0.handle;
+        const int W = pick_W(h0->p.row_bytes);
+        StreamBatch<8> B;
+        memset(&B, 0, sizeof B);
+        int64_t total = 0;
+        uint32_t n_seg = 0, grid_min = 1;
+        const int64_t grid_cap = h0->max_ctas ? (int64_t)h0->max_ctas : 2ll * h0->sm_count;
+        while (i < n_ranges && n_seg < 8) {
+            const ibp_range_desc& r = ranges_host[i];
+            if (r.n_rows == 0) { ++i; continue; }
+            if (!batchable(r) || pick_W(r.handle->p.row_bytes) != W) break;
+            StreamParams& P = B.seg[n_seg];
+            const bool tile_ok = r.packed_dev != nullptr && grid_cap >= (int64_t)((r.handle->n_groups + 7) / 8);
+            stream_geometry(r.handle, source(r), ibp_row_offset(r.handle, (uint64_t)r.first_row), nullptr, 1, r.first_row, r.n_rows, r.out_dev, tile_ok, P);
+            B.chunk_start[n_seg] = total;
+            total += P.n_chunks;
+            B.stage_bytes = std::max(B.stage_bytes, P.stage_bytes);
+            grid_min = std::max(grid_min, P.n_tile_blocks);
+            ++n_seg; ++i;
+        }
+        B.n_seg = n_seg;
+        const int ns = B.stage_bytes > 40 * 1024 ? 2 : 3;
+        const size_t smem = (size_t)ns * B.stage_bytes + (size_t)ns * 16;
+        if (smem > 220 * 1024) { ibp_set_error("ibp_decode_ranges: packed rows do not fit the shared-memory stages"); return IBP_ERR_UNSUPPORTED; }
+        ibp_status s;
+#define IBP_STREAM_B(W_)                                                                                              \
+    s = ns == 2 ? launch_stream_one<W_, 2, 8>(B, total, 1, h0->max_ctas, h0->sm_count, smem, st, grid_min)              \
+                : launch_stream_one<W_, 3, 8>(B, total, 1, h0->max_ctas, h0->sm_count, smem, st, grid_min)
+        switch (W) {
+            case 4: IBP_STREAM_B(4); break;
+            case 2: IBP_STREAM_B(2); break;
+            default: IBP_STREAM_B(1); break;
+        }
+#undef IBP_STREAM_B
+        if (s != IBP_OK) return s;
+    }
+    return IBP_OK;
 }
 
 // Host-buffer entry point.  Large batches are cut into chunks so that the device->host copy of chunk c (copy engine, PCIe

@@ -671,7 +671,7 @@ extern "C" ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* i
 }
 
 extern "C" ibp_status ibp_configure(ibp_handle* h, uint32_t max_ctas, uint32_t warps_per_cta) {
-    if (!h || warps_per_cta > 32) { ibp_set_error("ibp_configure: bad argument"); return IBP_ERR_INVALID_ARG; }
+    if (!h || warps_per_cta > 8) { ibp_set_error("ibp_configure: warps_per_cta must be 0 (default) or 1..8"); return IBP_ERR_INVALID_ARG; }
     h->max_ctas = max_ctas;
     h->warps_per_cta = warps_per_cta;
     return IBP_OK;

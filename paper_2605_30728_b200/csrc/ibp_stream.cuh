@@ -42,6 +42,18 @@ struct StreamParams {
     uint32_t tb_pitch;             // bytes between the block's images of consecutive matrix rows inside a stage
 };
 
+// One launch over several independent ranges (a whole decoder layer = 7 weight matrices): the segments are walked in
+// order by every CTA, the mbarrier pipeline runs on across segment borders, and a CTA takes the chunks gc = blockIdx.x (mod
+// gridDim.x) of the CONCATENATED chunk list, so the load balances over the whole launch and there is one ramp and one tail per
+// layer instead of one per matrix.  NSEG = 1 is the single-range kernel (segment index a compile-time constant).
+template <int NSEG>
+struct StreamBatch {
+    StreamParams seg[NSEG];
+    int64_t chunk_start[NSEG];     // first global chunk index of segment j (non-tile segments)
+    uint32_t n_seg;
+    uint32_t stage_bytes;          // shared-memory stage size of the launch: the largest any segment needs
+};
+
 // The five move masks of the parallel-suffix expand for deposit positions nv (set bits = positions to fill, lowest first).
 __device__ __forceinline__ void expand_masks(uint32_t nv, uint32_t mv[5]) {
     uint32_t m = nv, mk = ~nv << 1;
@@ -90,19 +102,39 @@ __global__ void ibp_build_mvtab(const uint32_t* __restrict__ meta, uint32_t n_wo
     for (int k = 0; k < 5; ++k) mvtab[i * 5 + k] = mv[k];
 }
 
-template <int W, int NS, int NW>
-__global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const StreamParams P) {
+template <int W, int NS, int NW, int NSEG>
+__global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __grid_constant__ StreamBatch<NSEG> B) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
-    const uint32_t full_s = smem_s + NS * P.stage_bytes, empty_s = full_s + NS * 8;
+    const uint32_t STAGE = B.stage_bytes;
+    const uint32_t full_s = smem_s + NS * STAGE, empty_s = full_s + NS * 8;
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(full_s + s * 8, 1); mbar_init(empty_s + s * 8, NW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    const uint32_t n_seg = NSEG == 1 ? 1u : B.n_seg;
+    uint32_t k = 0;                       // pipeline position: the same sequence in the producer and in every consumer warp
+    // consumer state of the lane's W words (see below); lives across segments, invalidated at every segment border
+    uint32_t m[W], b[W], ex[W], mv[W][6];
+    uint32_t mode = 15;
+    uint64_t prep_g = ~0ull;
+    const uint32_t w0_fast = lane * W;
+
+  for (uint32_t seg = 0; seg < n_seg; ++seg) {
+    const StreamParams& P = B.seg[NSEG == 1 ? 0 : seg];
     const uint64_t S = P.group_param;
+    // this CTA's chunks of the segment: global chunk gc = chunk_start + c belongs to CTA gc mod gridDim.x
+    const int64_t c_first = NSEG == 1 ? (int64_t)blockIdx.x
+                                      : (int64_t)(((int64_t)blockIdx.x - B.chunk_start[seg] % (int64_t)gridDim.x + (int64_t)gridDim.x) % (int64_t)gridDim.x);
+    // tile-block mode: CTA class tb = vb mod n_tile_blocks keeps tile block tb; the class's CTAs share its row blocks round-robin
+    const uint32_t vb = NSEG == 1 ? blockIdx.x : (blockIdx.x + seg * 37u) % gridDim.x;
+    const uint32_t tb_c = P.n_tile_blocks ? vb % P.n_tile_blocks : 0u, tb_idx = P.n_tile_blocks ? vb / P.n_tile_blocks : 0u;
+    const uint32_t tb_cls = P.n_tile_blocks ? (gridDim.x - tb_c + P.n_tile_blocks - 1u) / P.n_tile_blocks : 1u;
+    const uint32_t tb_rblocks = P.n_tile_blocks ? (uint32_t)(P.n_chunks / P.n_tile_blocks) : 0u;
+    prep_g = ~0ull;
 
     // chunk c -> first row id, rows (blocked) or matrix rows (strided), first output row, packed byte range
     auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0, uint64_t& b0, uint64_t& b1) {
@@ -133,13 +165,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
 
     if (wib == NW) {
         // ------------------------------------------------------------------ producer
-        if (lane != 0) return;
-        uint32_t k = 0;
+        if (lane != 0) { if (NSEG == 1) return; continue; }
         if (P.n_tile_blocks) {
-            for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+            for (uint32_t rbk = tb_idx; rbk < tb_rblocks; rbk += tb_cls, ++k) {
                 const uint32_t s = k % NS;
                 mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
-                const uint32_t tb = (uint32_t)c % P.n_tile_blocks, rbk = (uint32_t)c / P.n_tile_blocks;
+                const uint32_t tb = tb_c;
                 const uint32_t t0 = tb * NW, t1 = min(P.n_tiles, t0 + NW);
                 const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
                 const int64_t mr0 = (int64_t)rbk * P.rows_per_chunk;
@@ -150,13 +181,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
                 const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
                 const uint32_t bytes = (uint32_t)((head + len + 15u) & ~15ull);
                 mbar_expect_tx(full_s + s * 8, bytes * nrows);
-                const uint32_t dst = smem_s + s * P.stage_bytes;
+                const uint32_t dst = smem_s + s * STAGE;
                 for (uint32_t i = 0; i < nrows; ++i)
                     bulk_g2s(dst + i * P.tb_pitch, src - head + (uint64_t)i * P.row_stride_strided, bytes, full_s + s * 8);
             }
-            return;
+            if (NSEG == 1) return;
+            continue;
         }
-        for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+        for (int64_t c = c_first; c < P.n_chunks; c += gridDim.x, ++k) {
             const uint32_t s = k % NS;
             mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
             int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;
@@ -165,11 +197,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
             const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
             const uint32_t bytes = (uint32_t)((head + (b1 - b0) + 15u) & ~15ull);
             mbar_expect_tx(full_s + s * 8, bytes);
-            const uint32_t dst = smem_s + s * P.stage_bytes;
+            const uint32_t dst = smem_s + s * STAGE;
             for (uint32_t o = 0; o < bytes; o += 16384u)
                 bulk_g2s(dst + o, src - head + o, min(16384u, bytes - o), full_s + s * 8);
         }
-        return;
+        if (NSEG == 1) return;
+        continue;
     }
 
     // ---------------------------------------------------------------------- consumers
@@ -182,10 +215,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
     //     the sign).  Run j takes bits [c_j, c_j+len_j) of the extracted word to positions [p_j, p_j+len_j): one multiply by
     //     2^(p_j-c_j) and one lop3 (and-or) per run -- mv[q][j] = the multiplier, mv[q][3+j] = the run's mask;
     //   expand (mode 13..15): the general 5-stage parallel-suffix expand, mv[q][0..4] = its move masks, 3/4/5 stages as needed.
-    uint32_t m[W], b[W], ex[W], mv[W][6];
-    uint32_t mode = 15;
-    uint64_t prep_g = ~0ull;
-    const uint32_t w0_fast = lane * W;
     const bool fast = P.n_pass == 1 && P.fast_rows;
     const bool active_fast = w0_fast < P.n_words;
 
@@ -291,10 +320,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         }
     };
 
-    uint32_t k = 0;
     if (P.n_tile_blocks) {
-        // tile-block mode: this CTA's chunks all carry tile block blockIdx.x % n_tile_blocks; warp wib owns one tile of it
-        const uint32_t tb = blockIdx.x % P.n_tile_blocks, t = tb * NW + wib;
+        // tile-block mode: this CTA's chunks all carry tile block tb_c; warp wib owns one tile of it
+        const uint32_t tb = tb_c, t = tb * NW + wib;
         const bool has_tile = t < P.n_tiles;
         uint32_t toff = 0;
         if (has_tile) {
@@ -305,25 +333,26 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         }
         const int64_t n_mrows = (P.span_rows + (int64_t)S - 1) / (int64_t)S;
         const int64_t tile_rows = has_tile ? (P.span_rows - (int64_t)t + (int64_t)S - 1) / (int64_t)S : 0;   // rows of tile t in range
-        for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+        for (uint32_t rbk = tb_idx; rbk < tb_rblocks; rbk += tb_cls, ++k) {
             const uint32_t s = k % NS;
-            const int64_t mr0 = (int64_t)((uint32_t)c / P.n_tile_blocks) * P.rows_per_chunk;
+            const int64_t mr0 = (int64_t)rbk * P.rows_per_chunk;
             const int64_t cnt = min(min((int64_t)P.rows_per_chunk, n_mrows - mr0), tile_rows - mr0);
             mbar_wait(full_s + s * 8, (k / NS) & 1u);
             if (cnt > 0)
-                decode_run(smem_s + s * P.stage_bytes + toff, P.tb_pitch, P.out + ((uint64_t)mr0 * S + t) * P.row_bytes, S * P.row_bytes, (uint32_t)cnt);
+                decode_run(smem_s + s * STAGE + toff, P.tb_pitch, P.out + ((uint64_t)mr0 * S + t) * P.row_bytes, S * P.row_bytes, (uint32_t)cnt);
             __syncwarp();
             if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
         }
-        return;
+        if (NSEG == 1) return;
+        continue;
     }
-    for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x, ++k) {
+    for (int64_t c = c_first; c < P.n_chunks; c += gridDim.x, ++k) {
         const uint32_t s = k % NS;
         int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;
         chunk_geom(c, row0, nrows, out0, b0, b1);
         const uint32_t head = (uint32_t)((uintptr_t)(P.store + (b0 - P.bias)) & 15u);
-        const uint32_t* stage = (const uint32_t*)(smem + (size_t)s * P.stage_bytes);
-        const uint32_t stage_s = smem_s + s * P.stage_bytes;
+        const uint32_t* stage = (const uint32_t*)(smem + (size_t)s * STAGE);
+        const uint32_t stage_s = smem_s + s * STAGE;
         bool waited = false;
 
         // Generic path: any number of passes, any byte alignment; metadata reloaded per pass, run-wise bit deposit.
@@ -419,4 +448,5 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const Stre
         __syncwarp();
         if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
     }
+  }   // segments
 }

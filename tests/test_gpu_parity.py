@@ -226,6 +226,71 @@ def test_weight_shape_stream_and_resident():
         assert np.array_equal(_range(h, 0, w.n_rows), _u8(X))
         half = (w.mat_rows // 2) * w.group_param
         assert np.array_equal(_range(h, half, w.n_rows - half), _u8(X)[half:])
+        # host destinations: pinned + mapped (the kernel stores straight into host memory) and pageable (staged)
+        pin = ibp.PinnedBuffer(w.n_rows * 256)
+        h.gather_decompress_range_host(0, w.n_rows, pin.view(np.uint8, (w.n_rows, 256)), torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(pin.view(np.uint8, (w.n_rows, 256)), _u8(X))
+        pin.free()
+        pg = np.zeros((w.n_rows - half, 256), np.uint8)
+        h.gather_decompress_range_host(half, w.n_rows - half, pg, torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(pg, _u8(X)[half:])
+        h.destroy()
+
+
+@pytest.mark.parametrize("max_ctas", [0, 12, 3])
+def test_decode_ranges_one_launch_per_layer(max_ctas):
+    """ibp_decode_ranges: a 'layer' of matrices (strided column-tile groups with 4, 11 and 1 tile blocks, one matrix with fewer
+    rows than tiles), a blocked table, a thresholded handle and an empty range in ONE call -- 11 ranges, so two batched launches
+    plus per-range fall-backs -- from the host store and from packed bytes staged in HBM (tile-block chunks), whole and partial
+    ranges.  Every output byte against the original rows (c1) and, per table, against the oracle codec on a sample (c2)."""
+    st = torch.cuda.current_stream().cuda_stream
+    specs = [("w", 96, 4096), ("w", 64, 11008), ("w", 40, 512), ("w", 3, 1408), ("b", 700, 256, 16), ("w", 33, 4096),
+             ("t", 500, 256, 50), ("w", 17, 2816), ("w", 8, 4096), ("b", 90, 256, 7), ("w", 12, 11008)]
+    tabs = []
+    for i, sp in enumerate(specs):
+        if sp[0] == "w":
+            wm = workloads.WeightMatrix(sp[1], sp[2], layer=9, slot=i % 8)
+            X = _u8(wm.table())
+            h = ibp.ibp_build(X, 256, 1, wm.group_param, align_bytes=16).upload_metadata(0)
+            unit = wm.group_param
+            ds = oracle.Dataset(X, 1, wm.group_param)
+        else:
+            n, rb, G = sp[1], sp[2], sp[3]
+            X = (datagen.random_bytes(n * rb, 70 + i).reshape(n, rb) & datagen.random_bytes(rb, 71 + i)[None, :]) | 0x04
+            thr = (4, 5) if sp[0] == "t" else (1, 1)
+            h = ibp.ibp_build(X, rb, 0, G, align_bytes=16, threshold=thr).upload_metadata(0)
+            unit = G if sp[0] == "b" else 1
+            ds = oracle.Dataset(X, 0, G) if sp[0] == "b" else oracle.DatasetT(X, 0, G, 4, 5)
+        if max_ctas:
+            h.configure(max_ctas, 0)
+        ids = np.arange(0, X.shape[0], 5, dtype=np.int64)
+        assert np.array_equal(ds.gather_decompress(ids), X[ids])
+        ds.close()
+        tabs.append((h, X, unit))
+    for resident in (False, True):
+        for partial in (False, True):
+            ranges, outs, wants, keep = [], [], [], []
+            for j, (h, X, unit) in enumerate(tabs):
+                n = X.shape[0]
+                first = (n // unit // 2) * unit if partial and n >= 2 * unit else 0
+                cnt = 0 if (j == 4 and partial) else n - first                 # one empty range
+                out = torch.full((max(1, cnt), X.shape[1]), 0x77, dtype=torch.uint8, device="cuda")
+                packed = None
+                if resident and cnt:
+                    ptr, nb = h.packed_range(first, cnt)
+                    buf = _dev(h.packed_view(ptr, nb).copy()) if nb else torch.zeros(16, dtype=torch.uint8, device="cuda")
+                    keep.append(buf)
+                    packed = buf.data_ptr()
+                ranges.append((h, packed, first, cnt, out.data_ptr()))
+                outs.append(out)
+                wants.append(X[first:first + cnt])
+            ibp.ibp_decode_ranges(ranges, st)
+            torch.cuda.synchronize()
+            for j, (o, want) in enumerate(zip(outs, wants)):
+                assert np.array_equal(o.cpu().numpy()[: want.shape[0]], want), f"range {j} resident={resident} partial={partial}"
+    with pytest.raises(ibp.IbpError):
+        ibp.ibp_decode_ranges([(tabs[0][0], None, 1, 5, outs[0].data_ptr())], st)      # first_row is not a unit boundary
+    for h, _, _ in tabs:
         h.destroy()
 
 
@@ -303,7 +368,7 @@ def test_configure_limits_grid_and_streams():
     ids = w.ids(2)
     want = oracle.gather_plain(X, ids)
     s = torch.cuda.Stream()
-    for ctas, warps in ((1, 1), (3, 2), (64, 8), (0, 16)):
+    for ctas, warps in ((1, 1), (3, 2), (64, 8), (0, 4)):
         h.configure(ctas, warps)
         ids_d = _dev(ids)
         out = torch.zeros((len(ids), 512), dtype=torch.uint8, device="cuda")
