@@ -45,6 +45,8 @@ def make_workload(name):
         return workloads.GNN(interleaved=True)
     if name == "dlrm":
         return workloads.DLRM()
+    if name == "dlrm-hot":
+        return workloads.DLRM(hot_order=True)
     if name == "tiny":
         return workloads.Tiny()
     if name == "kv":
@@ -53,6 +55,9 @@ def make_workload(name):
 
 
 def describe(w):
+    if getattr(w, "hot_order", False):
+        return ("configs[2] DLRM embedding lookup with the store laid out by sampling rank (slot = rank x 26 + table; the entries are i.i.d., so "
+                "ratio and content are unchanged): 26 x 2M x 64 fp32 (13.3 GB), groups of 128, 16384 x 26 Zipf(1.05) ids per step (repeats kept)")
     if getattr(w, "interleaved", False):
         return ("configs[1] GNN node-feature gather, SECONDARY variant (reading R15): the 70% N(0,1)-in-2^-8-steps rows and the 30% sparse 0/1 rows are "
                 "interleaved at random, so every group of 256 mixes both types; 10M x 128 fp32, 250k unique Zipf(0.9) ids per step")
@@ -1169,6 +1174,8 @@ def run_resident(args):
     X = w.rows(0, nr)
     Xb = X.view(np.uint8).reshape(nr, -1)
     h = ibp.ibp_build(Xb, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, threshold=thr, flags=ibp.IBP_FLAG_PAGEABLE_STORE).upload_metadata(0)
+    if args.stream_mode is not None:
+        h.set_stream_mode(args.stream_mode)
     info = h.info()
     stream = torch.cuda.current_stream().cuda_stream
     try:
@@ -1263,7 +1270,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="gnn", choices=["gnn", "gnn-interleaved", "dlrm", "tiny", "kv", "weights", "sweep"])
+    ap.add_argument("--workload", default="gnn", choices=["gnn", "gnn-interleaved", "dlrm", "dlrm-hot", "tiny", "kv", "weights", "sweep"])
     ap.add_argument("--align", type=int, default=0, help="packed-row alignment unit A; 0 = the workload's default")
     ap.add_argument("--layers", type=int, default=32, help="weights workload: decoder layers held in host memory (32 = BASELINE's 12.95 GB)")
     ap.add_argument("--gemm-m", type=int, default=16384, help="weights workload: rows of the consumer GEMM's activation")
@@ -1275,6 +1282,7 @@ def main():
     ap.add_argument("--phase", default="gather", choices=["gather", "build", "masks", "resident"],
                     help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device; masks = the mask-quality tools (tau / chunk-size sweep, sampled masks, k-means); resident = ibp_decompress_resident alone (S8)")
     ap.add_argument("--cache-frac", type=float, default=0.0, help="gnn/dlrm: put a compressed GPU cache of this fraction of the packed store in front of the host store")
+    ap.add_argument("--stream-mode", type=int, default=None, choices=[0, 1, 2], help="--phase resident: ibp_set_stream_mode (test/compare hook)")
     ap.add_argument("--no-baseline", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-resident", action="store_true")

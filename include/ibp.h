@@ -314,8 +314,9 @@ ibp_status ibp_set_fetch_mode(ibp_handle* h, int mode);
  * batches of >= 16384 ids.  Output is identical either way.  Needs n_rows < 2^32 - 1, else it is ignored.          */
 ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode);
 
-/* Tuning/test hook: contiguous runs (spans, ranges, resident decode): 1 = TMA producer/consumer stream kernel (default),
- * 0 = per-row fetch kernel.  Results are identical either way.                                                       */
+/* Tuning/test hook: contiguous runs (spans, ranges, resident decode): 1 = TMA producer/consumer stream kernels (default),
+ * 0 = per-row fetch kernel, 2 = stream kernels with the row-per-warp form of the thresholded decode instead of the sub-warp
+ * form used for 128/256/512-byte rows.  Results are identical in every mode.                                         */
 ibp_status ibp_set_stream_mode(ibp_handle* h, int mode);
 
 /* Tuning/test hook: rows each warp keeps in flight in random gathers (ring depth): 1, 2 or 4.                       */

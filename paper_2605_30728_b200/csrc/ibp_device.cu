@@ -751,6 +751,21 @@ static ibp_status launch_stream_t_one(const StreamTParams& P, int64_t max_ctas, 
     return IBP_OK;
 }
 
+template <int LPR, int NS, int NR>
+static ibp_status launch_stream_t2_one(const StreamTParams& P, int64_t max_ctas, int sm_count, size_t smem, cudaStream_t st) {
+    constexpr int NW = 8;
+    auto kern = ibp_stream_t2_kernel<LPR, NS, NW, NR>;
+    static unsigned long long smem_optin_done = 0;
+    if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
+    int occ = 0;
+    IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (NW + 1) * 32, smem));
+    int64_t blocks = std::min<int64_t>(P.n_chunks, (int64_t)std::max(occ, 1) * sm_count);
+    if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
+    kern<<<(int)blocks, (NW + 1) * 32, smem, st>>>(P);
+    IBP_CUDA(cudaGetLastError());
+    return IBP_OK;
+}
+
 static bool stream_t_fits(const ibp_handle* h) {
     const int W = pick_W(h->p.row_bytes);
     if ((h->n_words + 32 * W - 1) / (32 * W) != 1) return false;                       // single-pass rows only
@@ -776,7 +791,33 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     P.strided = h->p.group_kind == IBP_GROUP_STRIDED;
     const uint64_t stride = h->max_stride;                                             // a raw row: the largest stored row
     uint64_t per;                                                                      // consecutive rows per chunk
-    if (!P.strided) {
+    // rows of 128 / 256 / 512 bytes (every BASELINE workload): the sub-warp kernel (ibp_stream_t.cuh, ibp_stream_t2_kernel)
+    const uint32_t lpr = h->p.row_bytes % 16 == 0 ? h->p.row_bytes / 16 : 0;
+    bool t2 = (lpr == 8 || lpr == 16 || lpr == 32) && h->t2_mode && !P.strided;
+    if (t2) {
+        // pieces of 32 rows (16 for 512-byte rows), NW pieces per chunk.  Stages are sized for the typical chunk (56 KB); a chunk
+        // whose stored bytes exceed a stage -- only with many raw rows -- is loaded as sub-loads of split_rows rows.
+        const uint32_t U = lpr == 32 ? 16u : 32u;
+        const uint64_t STAGE = 36ull * 1024;
+        uint64_t rc = (uint64_t)std::min<int64_t>((int64_t)NW * U, span_rows);
+        P.rows_per_chunk = (uint32_t)rc;
+        P.piece_rows = U;
+        per = rc;
+        if (rc * stride + 64 <= STAGE) {
+            P.nsplit = 1;
+            P.stage_bytes = (uint32_t)((rc * stride + 64 + 127) / 128 * 128);
+        } else {
+            const uint64_t split_rows = ((STAGE - 64) / stride) / U * U;
+            if (split_rows == 0) t2 = false;
+            else {
+                P.split_rows = (uint32_t)split_rows;
+                P.nsplit = (uint32_t)((rc + split_rows - 1) / split_rows);
+                P.stage_bytes = (uint32_t)STAGE;
+            }
+        }
+    }
+    if (t2) {
+    } else if (!P.strided) {
         uint32_t U = 16;
         uint64_t rc = std::min<uint64_t>((uint64_t)NW * U, (48ull * 1024) / stride);
         rc = std::max<uint64_t>(rc, 1);
@@ -795,12 +836,28 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
         P.piece_rows = (uint32_t)rc;
         per = rc * S;
     }
-    P.stage_bytes = (uint32_t)((per * stride + 64 + 127) / 128 * 128);
+    if (!t2) P.stage_bytes = (uint32_t)((per * stride + 64 + 127) / 128 * 128);
     P.chunks_per_span = (uint32_t)((span_rows + (int64_t)per - 1) / (int64_t)per);
     P.n_chunks = n_spans * (int64_t)P.chunks_per_span;
-    const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
+    const int ns = (P.stage_bytes > 40 * 1024 || t2) ? 2 : 3;
     const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
     if (smem > 220 * 1024) { ibp_set_error("thresholded rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
+    if (t2) {
+        const int nr = (h->max_runs >= 1 && h->max_runs <= 3) ? h->max_runs : 0;
+#define IBP_T2_NR(LPR_, NS_)                                                                              \
+        switch (nr) {                                                                                     \
+            case 1: return launch_stream_t2_one<LPR_, NS_, 1>(P, h->max_ctas, h->sm_count, smem, st);     \
+            case 2: return launch_stream_t2_one<LPR_, NS_, 2>(P, h->max_ctas, h->sm_count, smem, st);     \
+            case 3: return launch_stream_t2_one<LPR_, NS_, 3>(P, h->max_ctas, h->sm_count, smem, st);     \
+            default: return launch_stream_t2_one<LPR_, NS_, 0>(P, h->max_ctas, h->sm_count, smem, st);    \
+        }
+#define IBP_T2(LPR_) if (ns == 2) { IBP_T2_NR(LPR_, 2) } else { IBP_T2_NR(LPR_, 3) }
+        if (lpr == 32) { IBP_T2(32) }
+        if (lpr == 16) { IBP_T2(16) }
+        IBP_T2(8)
+#undef IBP_T2
+#undef IBP_T2_NR
+    }
     const bool runs = h->max_runs >= 0 && h->max_runs <= 3;
 #define IBP_STREAM_T(W_)                                                                                         \
     if (runs) return ns == 2 ? launch_stream_t_one<W_, 2, true>(P, h->max_ctas, h->sm_count, smem, st)           \
@@ -1466,8 +1523,9 @@ extern "C" ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode) {
 
 // Test/tuning hook: 1 = contiguous runs through the TMA producer/consumer stream kernel (default), 0 = per-row fetch.
 extern "C" ibp_status ibp_set_stream_mode(ibp_handle* h, int mode) {
-    if (!h || mode < 0 || mode > 1) { ibp_set_error("ibp_set_stream_mode: bad argument"); return IBP_ERR_INVALID_ARG; }
-    h->stream_mode = mode;
+    if (!h || mode < 0 || mode > 2) { ibp_set_error("ibp_set_stream_mode: bad argument"); return IBP_ERR_INVALID_ARG; }
+    h->stream_mode = mode ? 1 : 0;
+    h->t2_mode = mode == 2 ? 0 : 1;
     return IBP_OK;
 }
 

@@ -59,6 +59,7 @@ struct ibp_handle {
     int dedup_mode = -1;                   // random gathers: 1 = fetch each distinct id once, replicate in HBM; -1 auto
     int stream_mode = 1;                   // contiguous runs: 1 = TMA pipeline stream kernel, 0 = per-row fetch
     int fetch_mode = 1;                    // 0 = cp.async (LSU), 1 = cp.async.bulk (TMA)
+    int t2_mode = 1;                       // thresholded contiguous runs: 1 = sub-warp kernel (ibp_stream_t2_kernel), 0 = row-per-warp kernel
 };
 
 // Compressed GPU cache: slabs of packed rows + a hash map id -> 64-bit value {offset:40, slab:3, compressed:1}.

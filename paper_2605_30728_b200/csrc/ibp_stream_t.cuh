@@ -26,6 +26,7 @@ struct StreamTParams {
     uint32_t row_bytes, n_words;
     uint32_t group_param, group_shift, strided;
     uint32_t stage_bytes;
+    uint32_t nsplit, split_rows;   // ibp_stream_t2_kernel: a chunk above one stage is loaded as nsplit sub-loads of split_rows rows (0/1 = never)
 };
 
 // RUNS: every word of every group of the table has at most three runs of variant bits (decided once per handle on the host):
@@ -301,5 +302,308 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
         if (!waited) mbar_wait(full_s + s * 8, (k / NS) & 1u);   // a warp without a piece still has to follow the phases
         __syncwarp();
         if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------------
+// ibp_stream_t2_kernel -- the thresholded stream decode for rows of 16*LPR bytes (LPR = 8, 16 or 32 lanes per row; W = 4
+// words per lane: 128 / 256 / 512-byte rows, i.e. every BASELINE workload).  Same producer/consumer pipeline as above; the
+// consumer side is rebuilt around the instruction count per row, which is what bounded the kernel above (ncu: 177 warp
+// instructions per 512-byte row at 60 % issue utilisation against 68 for the strict kernel):
+// Blocked groups only (strided tables keep the kernel above).
+//   - a warp decodes 32/LPR rows per pass, one row per group of LPR lanes (256-byte rows: two at a time), so the per-row fixed
+//     work (participation read, counts, scan, address set-up, store) is shared by twice or four times the data;
+//   - the lane groups of a pass take rows of DIFFERENT parts of the piece (group of lanes s: rows [s*Q, (s+1)*Q)), so with small
+//     groups (KV: 16 rows) one set-up -- Mask/Bitval loads, run masks or expand masks -- prepares two or four groups at once;
+//   - pieces are 32 rows (16 for 512-byte rows), chunks NW pieces; a chunk whose stored bytes exceed a stage (many raw rows) is
+//     loaded as NSPLIT sub-loads into consecutive stages -- both sides decide that from the same two row offsets;
+//   - raw rows take the SAME code with an empty header and no participating chunk (every chunk then contributes its 32
+//     bits at offset 32*c), so a pass never diverges on the row kind;
+//   - bits removed in front of each of the lane's 4 chunks come from ONE packed computation: popc(Mask) of the 4 chunks sit in
+//     the bytes of one register, the 4 participation bits are spread to byte masks by a multiply, and a multiply by 0x01010101
+//     gives the four running sums (P:319 step 2 for four chunks at once);
+//   - the exclusive scan over the lanes of a row (P:319 step 3) runs on two rows packed into one register (16 bits each: a row
+//     removes at most 4,096 bits), and RB = 2 passes are written out side by side, branch-free (the store is predicated), so
+//     that their dependency chains interleave;
+//   - NR (handle level: the most runs of variant bits in any Mask word of the table): bits go back run by run with exactly NR
+//     multiply + and-or pairs; NR = 0 selects the five-stage expand.
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
+    // consumer-side wait with a suspend-time hint: a waiting warp stays off the issue port instead of polling
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+    }
+}
+
+template <int LPR, int NS, int NW, int NR>
+__global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const StreamTParams P) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t full_s = smem_s + NS * P.stage_bytes, empty_s = full_s + NS * 8;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) { mbar_init(full_s + s * 8, 1); mbar_init(empty_s + s * 8, NW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint64_t S = P.group_param;
+    const uint32_t cap16 = (P.stage_bytes - 64u) / 16u;          // what one stage holds, in 16-byte units
+    const uint32_t nsplit = P.nsplit, sub_rows = P.split_rows;   // nsplit > 1: a chunk above cap16 is loaded as nsplit sub-loads of sub_rows rows
+
+    auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0) {
+        const int64_t si = !P.ids ? 0 : (P.n_chunks <= 0x7FFFFFFFll ? (int64_t)((uint32_t)c / P.chunks_per_span) : c / P.chunks_per_span);
+        const int64_t cc = c - si * P.chunks_per_span;
+        const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
+        const int64_t per = (int64_t)P.rows_per_chunk;                          // blocked groups only (strided tables: the kernel above)
+        const int64_t r = cc * per;
+        row0 = span_first + r;
+        nrows = (uint32_t)min(per, P.span_rows - r);
+        out0 = si * P.span_rows + r;
+    };
+
+    if (wib == NW) {
+        if (lane != 0) return;
+        uint32_t k = 0;
+        for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x) {
+            int64_t row0, out0; uint32_t nrows;
+            chunk_geom(c, row0, nrows, out0);
+            const uint32_t o0 = __ldg(P.row_off + row0), o1 = __ldg(P.row_off + row0 + nrows);
+            const uint32_t parts = (nsplit > 1 && o1 - o0 > cap16) ? nsplit : 1u;
+            for (uint32_t j = 0; j < parts; ++j, ++k) {
+                const uint32_t s = k % NS;
+                uint32_t a0 = o0, a1 = o1;
+                if (parts > 1) {
+                    const uint32_t r0 = min(nrows, j * sub_rows), r1 = min(nrows, r0 + sub_rows);
+                    a0 = __ldg(P.row_off + row0 + r0);
+                    a1 = __ldg(P.row_off + row0 + r1);
+                }
+                mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
+                const uint8_t* src = P.store + (16ull * a0 - P.bias);
+                const uint32_t bytes = (a1 - a0) * 16u;
+                mbar_expect_tx(full_s + s * 8, bytes);
+                const uint32_t dst = smem_s + s * P.stage_bytes;
+                for (uint32_t o = 0; o < bytes; o += 16384u)
+                    bulk_g2s(dst + o, src + o, min(16384u, bytes - o), full_s + s * 8);
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumers
+    constexpr int W = 4, RPP = 32 / LPR, RB = 2;
+    constexpr int NMV = NR ? 2 * NR : 5;
+    const uint32_t sub = (uint32_t)lane / LPR, sl = (uint32_t)lane % LPR;      // lane group (row of a pass), lane inside the row
+    const uint32_t w0 = sl * W;                                                // first chunk (32-bit word) of this lane
+    const uint32_t hdr_off = (w0 >> 5) * 4u, hdr_sh = w0 & 31u;                // where the lane's 4 participation bits sit
+    uint32_t m[W], b[W], mv[W][NMV], pm4 = 0;                                  // pm4: popc(Mask) of the 4 chunks, one per byte
+    uint64_t prep_g = ~0ull;                                                   // per lane: lane groups may hold different groups
+
+    auto prepare = [&](uint64_t g) {
+        const uint32_t* gm = P.meta + g * 2ull * P.n_words;
+        VecIO<W>::ld(gm + w0, m);
+        VecIO<W>::ld(gm + P.n_words + w0, b);
+        pm4 = 0;
+#pragma unroll
+        for (int q = 0; q < W; ++q) pm4 |= (uint32_t)__popc(m[q]) << (8 * q);   // <= 32 each
+        if constexpr (NR > 0) {
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                uint32_t nv = ~m[q], c = 0;
+#pragma unroll
+                for (int j = 0; j < NR; ++j) {
+                    const uint32_t low = nv & (0u - nv), run = nv & ~(nv + low);     // nv == 0 -> low = run = 0
+                    mv[q][j] = run ? 1u << ((__ffs(low) - 1) - c) : 0u;
+                    mv[q][NR + j] = run;
+                    c += __popc(run);
+                    nv &= ~run;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                if (q > 0 && m[q] == m[q - 1]) {
+#pragma unroll
+                    for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+                } else {
+                    expand_masks(~m[q], mv[q]);
+                }
+            }
+        }
+        prep_g = g;
+    };
+    auto reinsert = [&](auto nstg_c, uint32_t x, int q) -> uint32_t {
+        if constexpr (NR > 0) {
+            uint32_t acc = b[q];
+#pragma unroll
+            for (int j = 0; j < NR; ++j) acc = and_or(x * mv[q][j], mv[q][NR + j], acc);
+            return acc;
+        } else {
+            return bitselect(b[q], expand_bits<decltype(nstg_c)::value>(x, mv[q]), m[q]);
+        }
+    };
+
+    // RB passes side by side: lane group `sub` decodes row rr[i] of the piece in pass i (valid[i] = 0: the row is a repeat whose
+    // result is not stored).  my_off / flags: offsets (lane i <-> row i of the piece) and compressed-bits of the piece.
+    auto decode_rows_n = [&](auto nstg_c, const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
+                             uint32_t stage_s, uint8_t* orow0, uint32_t ostride) {
+        uint32_t bitbase[RB], part[RB], s[RB], d4[RB];
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            const uint32_t sa = stage_s + (__shfl_sync(0xFFFFFFFFu, my_off, rr[i]) - base_off) * 16u;
+            const bool comp = (flags >> rr[i]) & 1u;
+            uint32_t h;
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(h) : "r"(sa + hdr_off));
+            part[i] = comp ? (h >> hdr_sh) & 0xFu : 0u;                        // raw row: no chunk participates ...
+            const uint32_t sel = ((part[i] * 0x00204081u) & 0x01010101u) * 0xFFu;   // participation bit q -> byte q = 0xFF
+            const uint32_t in4 = (pm4 & sel) * 0x01010101u;                    // byte q = bits removed in chunks 0..q of this lane
+            s[i] = in4 >> 24;
+            d4[i] = 0x60402000u - (in4 << 8);                                  // byte q = 32*q - bits removed in front of chunk q (>= 0)
+            bitbase[i] = sa * 8u + (comp ? P.n_words : 0u) + 32u * w0;         // ... and there is no header; a BIT address
+        }
+        static_assert(RB == 2, "the packed scan holds two passes");
+        uint32_t inc = s[0] | (s[1] << 16);                                    // exclusive scan over the lanes of a row (P:319 step 3)
+#pragma unroll
+        for (int d = 1; d < LPR; d <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, d, LPR);
+            if (sl >= (uint32_t)d) inc += v;
+        }
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+            const uint32_t bb = bitbase[i] + s[i] - (i == 0 ? (inc & 0xFFFFu) : (inc >> 16));   // minus the bits removed in the lanes in front
+            uint32_t o[W];
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                const uint32_t ba = bb + __byte_perm(d4[i], 0, 0x4440 + q);
+                uint32_t lo, hi;
+                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"((ba >> 3) & ~3u));
+                const uint32_t x = __funnelshift_r(lo, hi, ba);                // shift = ba mod 32
+                const uint32_t e = reinsert(nstg_c, x, q);
+                o[q] = ((part[i] >> q) & 1u) ? e : x;                          // non-participating chunk: all 32 bits
+            }
+            uint8_t* dst = orow0 + rr[i] * ostride;
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};\n\t}"
+                         ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]), "r"(valid[i]) : "memory");
+        }
+    };
+
+    auto decode_rows = [&](const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
+                           uint32_t stage_s, uint8_t* orow0, uint32_t ostride) {
+        using std::integral_constant;
+        // (specialising the expand to 3 / 4 stages per group, as the strict kernel does, was measured slower here: three copies of
+        // the pass body under the 72-register budget cost more than the two stages they save -- KV 0.54 -> 0.52)
+        decode_rows_n(integral_constant<int, 5>{}, rr, valid, my_off, flags, base_off, stage_s, orow0, ostride);
+    };
+
+    // One piece: rows id0, id0 + id_step, ... (cnt <= 32), all inside one stage.  orow = output address of row 0 of the piece.
+    const uint32_t Q = (P.piece_rows + RPP - 1) / RPP;                         // rows of a piece per lane group
+    auto decode_piece = [&](int64_t id0, int64_t id_step, uint32_t cnt, uint32_t my_off, uint32_t flags, uint32_t base_off,
+                            uint32_t stage_s, uint8_t* orow, uint32_t ostride, bool& waited, uint32_t bar, uint32_t parity) {
+        orow += (size_t)w0 * 4;
+        const uint32_t qs = min(cnt, sub * Q), qe = min(cnt, qs + Q);
+        const bool have = qs < qe;
+        uint64_t glo = 0, ghi = 0;
+        if (have) {
+            glo = group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + qs));
+            ghi = group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + qe - 1));
+        }
+        if (__all_sync(0xFFFFFFFFu, !have || glo == ghi)) {
+            // every lane group's rows lie in one group of the table: one set-up per piece, possibly of several groups at once
+            const uint64_t g = have ? glo : group_of_u(P.group_param, P.group_shift, (uint64_t)id0);
+            if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g);
+            if (!waited) { mbar_wait_relaxed(bar, parity); waited = true; }
+            const uint32_t n_it = min(Q, cnt);
+            for (uint32_t i = 0; i < n_it; i += RB) {
+                uint32_t rr[RB], valid[RB];
+#pragma unroll
+                for (int j = 0; j < RB; ++j) {
+                    const uint32_t r = qs + i + j;
+                    valid[j] = r < qe;
+                    rr[j] = valid[j] ? r : (have ? qs : 0u);
+                }
+                decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow, ostride);
+            }
+        } else {
+            // a table group ends inside a lane group's rows (a range that starts off a group boundary): run by run of one group
+            uint32_t r = 0;
+            while (r < cnt) {
+                const uint64_t id = (uint64_t)(id0 + r);
+                const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
+                const uint32_t r_end = (uint32_t)min((uint64_t)cnt, (uint64_t)r + ((g + 1) * S - id));
+                if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g);
+                if (!waited) { mbar_wait_relaxed(bar, parity); waited = true; }
+                for (; r < r_end; r += RB * RPP) {
+                    uint32_t rr[RB], valid[RB];
+#pragma unroll
+                    for (int j = 0; j < RB; ++j) {
+                        const uint32_t x = r + (uint32_t)j * RPP + sub;
+                        valid[j] = x < r_end;
+                        rr[j] = valid[j] ? x : r;
+                    }
+                    decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow, ostride);
+                }
+                r = r_end;
+            }
+        }
+    };
+
+    auto load_piece = [&](int64_t id0, int64_t id_step, uint32_t cnt, uint32_t& off_abs, uint32_t& flag) {
+        const int64_t id = id0 + (int64_t)lane * id_step;
+        off_abs = (uint32_t)lane < cnt ? __ldg(P.row_off + id) : 0u;
+        flag = (uint32_t)lane < cnt ? (__ldg(P.row_flag + (id >> 5)) >> (id & 31)) & 1u : 0u;
+    };
+    const uint32_t U = P.piece_rows;
+    int64_t n_row0 = 0, n_out0 = 0;
+    uint32_t n_nrows = 0, n_base = 0, n_end = 0, n_off = 0, n_flag = 0;
+    if ((int64_t)blockIdx.x < P.n_chunks) {
+        chunk_geom(blockIdx.x, n_row0, n_nrows, n_out0);
+        n_base = __ldg(P.row_off + n_row0);
+        n_end = __ldg(P.row_off + n_row0 + n_nrows);
+        if (wib * U < n_nrows) load_piece(n_row0 + wib * U, 1, min(U, n_nrows - wib * U), n_off, n_flag);
+    }
+
+    uint32_t k = 0;
+    for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x) {
+        const int64_t row0 = n_row0, out0 = n_out0;
+        const uint32_t nrows = n_nrows, base_off = n_base;
+        const uint32_t parts = (nsplit > 1 && n_end - n_base > cap16) ? nsplit : 1u;
+        uint32_t my_off = n_off, my_flag = n_flag;
+        if (c + gridDim.x < P.n_chunks) {
+            chunk_geom(c + gridDim.x, n_row0, n_nrows, n_out0);
+            n_base = __ldg(P.row_off + n_row0);
+            n_end = __ldg(P.row_off + n_row0 + n_nrows);
+            if (wib * U < n_nrows) {
+                load_piece(n_row0 + wib * U, 1, min(U, n_nrows - wib * U), n_off, n_flag);
+                const uint64_t ng = group_of_u(P.group_param, P.group_shift, (uint64_t)n_row0 + wib * U + min(sub * Q, U - 1));   // warm L1 with its Mask/Bitval
+                const uint32_t* ngm = P.meta + ng * 2ull * P.n_words + w0;
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm + P.n_words));
+            }
+        }
+        {
+            const uint32_t n_pieces = (nrows + U - 1) / U;
+            for (uint32_t j = 0; j < parts; ++j, ++k) {                        // one pass unless the chunk was split
+                const uint32_t s = k % NS, stage_s = smem_s + s * P.stage_bytes;
+                const uint32_t bar = full_s + s * 8, parity = (k / NS) & 1u;
+                const uint32_t r_lo = parts > 1 ? min(nrows, j * sub_rows) : 0u, r_hi = parts > 1 ? min(nrows, r_lo + sub_rows) : nrows;
+                const uint32_t sub_base = parts > 1 ? __ldg(P.row_off + row0 + r_lo) : base_off;
+                bool waited = false;
+                for (uint32_t p = wib; p < n_pieces; p += NW) {
+                    const uint32_t j0 = p * U, cnt = min(U, nrows - j0);
+                    if (j0 < r_lo || j0 >= r_hi) continue;                     // sub_rows is a multiple of the piece size
+                    const int64_t id0 = row0 + j0;
+                    if (p != (uint32_t)wib) load_piece(id0, 1, cnt, my_off, my_flag);   // later pieces of the chunk: on demand
+                    const uint32_t flags = __ballot_sync(0xFFFFFFFFu, my_flag);
+                    decode_piece(id0, 1, cnt, my_off, flags, sub_base, stage_s, P.out + (uint64_t)(out0 + j0) * P.row_bytes, P.row_bytes, waited, bar, parity);
+                }
+                if (!waited) mbar_wait_relaxed(bar, parity);                   // a warp without a piece still has to follow the phases
+                __syncwarp();
+                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+            }
+        }
     }
 }

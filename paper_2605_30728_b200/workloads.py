@@ -157,9 +157,13 @@ class DLRM(Workload):
     """configs[2]: 26 tables x 2M x 64 fp32 (global id = table*rows_per_table + row), U(-0.05,0.05) snapped to 2^-12;
     groups of 128; batch = 16,384 samples x 26 lookups, Zipf(1.05) per table, repeats kept, sample-major order."""
 
-    def __init__(self, rows_per_table=2_000_000, n_tables=26, samples=16_384):
+    def __init__(self, rows_per_table=2_000_000, n_tables=26, samples=16_384, hot_order=False):
         super().__init__("dlrm", 2, rows_per_table * n_tables, 256, "f32", BLOCKED, 128, 1, 32, samples * n_tables)
         self.rows_per_table, self.n_tables, self.samples = rows_per_table, n_tables, samples
+        # hot_order: the store is laid out by sampling rank (what a frequency-ordered build gives, e.g. through
+        # ibp_build_params.row_slot_host): slot = rank * n_tables + table, so the rows a Zipf batch touches most lie in
+        # one small region of the store.  The entries are i.i.d., so the table content is the same generator either way.
+        self.hot_order = hot_order
 
     def fill_rows(self, first, count, out):
         e = self.row_elems
@@ -185,6 +189,8 @@ class DLRM(Workload):
         u = _uniform01(self.samples * self.n_tables, self.batch_seed(iteration)).reshape(self.samples, self.n_tables)
         rank = np.searchsorted(cdf, u, side="left").clip(0, n - 1)
         t = np.arange(self.n_tables, dtype=np.int64)[None, :]
+        if self.hot_order:
+            return (rank.astype(np.int64) * self.n_tables + t).reshape(-1).astype(np.int64)
         row = (perm[rank] + t * 104729) % n                                # a different hot set per table
         return (t * n + row).reshape(-1).astype(np.int64)
 

@@ -420,6 +420,8 @@ def test_T_tiny_config_gather(align, thr):
     (1, 5, 203, 32, 16, (4, 5)), (1, 8, 64, 16, 32, (4, 5)), (0, 33, 1000, 100, 32, (7, 10)), (0, 128, 700, 256, 32, (4, 5)),
     (0, 256, 1500, 512, 32, (4, 5)), (0, 50, 333, 1024, 64, (4, 5)), (0, 20, 77, 4096, 64, (4, 5)), (1, 6, 600, 2048, 16, (9, 10)),
     (0, 9, 100, 516, 16, (4, 5)), (0, 1 << 30, 2000, 128, 32, (4, 5)), (0, 4, 30, 8192, 128, (4, 5)),
+    (0, 16, 1000, 256, 16, (4, 5)), (0, 5, 333, 128, 16, (3, 4)), (0, 3, 700, 512, 16, (4, 5)), (1, 32, 2100, 256, 16, (4, 5)),
+    (1, 86, 1000, 256, 16, (4, 5)), (1, 7, 500, 512, 32, (7, 10)), (1, 3, 100, 128, 16, (4, 5)), (0, 1 << 30, 3000, 512, 16, (9, 10)),
 ])
 def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
     """W=1,2,4 and 1..16 passes, ragged last groups, strided groups, one global group; rows with non-participating chunks
@@ -438,7 +440,7 @@ def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
         for dd in (0, 1):
             h.set_dedup_mode(dd)
             assert np.array_equal(_gather(h, ids), want)
-    for sm in (0, 1):                                                       # per-row fetch kernel / TMA stream kernel
+    for sm in (0, 1, 2):                                                    # per-row fetch kernel / TMA stream kernels (sub-warp, row-per-warp)
         h.set_stream_mode(sm)
         assert np.array_equal(_resident(h, 0, n), X)
         assert np.array_equal(_range(h, 0, n), X)
@@ -449,6 +451,38 @@ def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
         if kind == 0 and n > 5:
             assert np.array_equal(_resident(h, 3, n - 5), X[3:n - 2])       # per-row offsets: any row starts a unit
     h.destroy()
+
+
+@pytest.mark.parametrize("rb,G,n,raw_frac", [(512, 64, 1500, 1.0), (256, 16, 3000, 1.0), (512, 256, 2000, 0.6), (256, 128, 2500, 0.5), (128, 8, 900, 1.0)])
+def test_T_chunks_larger_than_a_stage(rb, G, n, raw_frac):
+    """Thresholded stream decode when most rows are kept raw: a chunk of NW pieces then exceeds one shared-memory stage
+    and is loaded as sub-loads into consecutive stages; the producer and every consumer warp take that decision from the same
+    two row offsets.  Contiguous ranges from the host store, resident decode, ranges starting off a group boundary, spans."""
+    rng = np.random.default_rng(rb + n)
+    X = _perturbed(n, rb, 3 * rb + n)
+    raw = rng.random(n) < raw_frac
+    X[raw] = rng.integers(0, 256, size=(int(raw.sum()), rb), dtype=np.uint8)
+    h = ibp.ibp_build(X, rb, 0, G, align_bytes=16, threshold=(4, 5)).upload_metadata(0)
+    ds = oracle.DatasetT(X, 0, G, 4, 5)
+    assert h.info().n_rows_raw == ds.n_raw
+    if G >= 64:
+        assert ds.n_raw >= int(0.9 * raw.sum())                                 # random rows in a large group: nothing to gain, kept raw
+    ids = np.arange(0, n, 3, dtype=np.int64)
+    assert np.array_equal(ds.gather_decompress(ids), X[ids])
+    ds.close()
+    for sm in (1, 2):
+        h.set_stream_mode(sm)
+        assert np.array_equal(_resident(h, 0, n), X)
+        assert np.array_equal(_range(h, 0, n), X)
+        assert np.array_equal(_resident(h, 5, n - 9), X[5:n - 4])
+        assert np.array_equal(_range(h, G + 3, n - G - 3), X[G + 3:])
+    h.destroy()
+    span = 4 * G
+    hs = ibp.ibp_build(X[: n // span * span], rb, 0, G, align_bytes=16, index_span=span, threshold=(4, 5)).upload_metadata(0)
+    ns = n // span
+    sids = np.array([ns // 2, 0, ns - 1, ns // 2], np.int64)
+    assert np.array_equal(_gather(hs, sids, span=span), oracle.gather_plain(X, sids, span))
+    hs.destroy()
 
 
 def test_T_edge_cases_and_spans():
@@ -475,7 +509,7 @@ def test_T_edge_cases_and_spans():
     Xk = w.table()
     hk = ibp.ibp_build(Xk, w.row_bytes, w.group_kind, w.group_param, align_bytes=16, index_span=w.index_span, threshold=(4, 5)).upload_metadata(0)
     ids = np.array([3, 0, 5, 5, 1], np.int64)
-    for sm in (0, 1):
+    for sm in (0, 1, 2):
         hk.set_stream_mode(sm)
         assert np.array_equal(_gather(hk, ids, span=w.index_span), oracle.gather_plain(Xk, ids, w.index_span))
     hk.destroy()
