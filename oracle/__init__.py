@@ -84,6 +84,10 @@ def lib():
         L.ibp_oracle_T_bitval.restype = vp
         L.ibp_oracle_T_row.argtypes = [vp, u64, C.POINTER(u64), C.POINTER(C.c_int)]
         L.ibp_oracle_T_row.restype = vp
+        L.ibp_oracle_T_append.argtypes = [vp, vp, u64]
+        L.ibp_oracle_T_append.restype = C.c_int
+        L.ibp_oracle_T_n_rows.argtypes = [vp]
+        L.ibp_oracle_T_n_rows.restype = u64
         L.ibp_oracle_gather_decompress_T.argtypes = [vp, vp, i64, u32, vp]
         L.ibp_oracle_gather_decompress_T.restype = C.c_int
         _lib = L
@@ -246,6 +250,28 @@ class DatasetT:
         p = lib().ibp_oracle_T_row(self._h, row_id, C.byref(n), C.byref(f))
         data = np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_uint8)), (n.value,)).copy() if n.value else np.zeros(0, np.uint8)
         return data, bool(f.value)
+
+    def append(self, rows):
+        """rows produced after the build are compressed under the existing Mask/Bitval of their group."""
+        R = _u8(np.asarray(rows).reshape(-1, self.row_bytes) if np.asarray(rows).ndim < 2 else rows)
+        if R.shape[1] != self.row_bytes:
+            raise ValueError("row size mismatch")
+        if lib().ibp_oracle_T_append(self._h, R.ctypes.data, R.shape[0]):
+            raise ValueError("an appended row falls in a group that has no Mask/Bitval")
+        self.n_rows = int(lib().ibp_oracle_T_n_rows(self._h))
+        self.n_raw = int(lib().ibp_oracle_T_n_raw(self._h))
+        self.stored_bytes = int(lib().ibp_oracle_T_stored_bytes(self._h))
+        self.rowflag_bytes = int(lib().ibp_oracle_T_rowflag_bytes(self._h))
+
+    def slot_image(self, capacity_rows: int, slot_bytes: int = 0):
+        """PAPER.md:361 in-place storage: "each tensor occupies its original slot and only the first compressed_size bytes are
+        read": row r at r*slot_bytes (slot_bytes = row_bytes unless an alignment unit rounds it up), zero beyond its size."""
+        slot = slot_bytes or self.row_bytes
+        img = np.zeros((capacity_rows, slot), np.uint8)
+        for r in range(self.n_rows):
+            data, _ = self.row(r)
+            img[r, : data.size] = data
+        return img
 
     def gather_decompress(self, ids, index_span: int = 1):
         ids = np.ascontiguousarray(ids, dtype=np.int64)

@@ -25,6 +25,10 @@
 //   ibp_oracle_build_T/gather: equals the plain gather byte for byte; bitmask bytes = ceil(n_rows/8); at tau=1
 //                              Mask/Bitval equal the strict dataset's; T = ceil(tau N_g) against Fig. 2's T=4, N=5;
 //                              hand-worked 5-row dataset fixture (sizes, flags, stored bytes)
+//   ibp_oracle_T_append      : append then gather == plain gather of the concatenated table; Mask/Bitval unchanged by an append;
+//                              an appended row's stored bytes == ibp_oracle_compress_row_T under the group's existing masks (the
+//                              row-level function is pinned above); the in-place slot image (row r in its original slot,
+//                              the first `size` bytes meaningful) has capacity x row_bytes bytes: the closed form of P:361
 //   Ratios on the paper's real datasets (Tables 2, 4, 5): parity unpinned -- the datasets are not available.
 //
 // Build: g++ -O1 -shared -fPIC oracle/ibp_oracle.cpp -o oracle/libibp_oracle.so
@@ -315,6 +319,32 @@ const uint8_t* ibp_oracle_T_row(const ibp_oracle_ds_T* d, uint64_t id, uint64_t*
     *is_compressed = get_bit(d->rowflag.data(), id);
     return d->stored.data() + d->row_offset[id];
 }
+
+// Online append ("During the prefill phase, we sample ... to create the Mask and Bitval.  This metadata is used to
+// compress the KV cache generated in the decode phase"): rows that arrive after the build are compressed under the EXISTING
+// Mask/Bitval of their group -- nothing is re-counted, the metadata does not change -- and stored after the rows already there.
+// A new row belongs to group id div G (blocked) or id mod S (strided) like any other; its group must already have metadata.
+// Returns 0, or 1 (nothing appended) when a new row's group does not exist.
+int ibp_oracle_T_append(ibp_oracle_ds_T* d, const uint8_t* rows, uint64_t n_new) {
+    for (uint64_t j = 0; j < n_new; ++j)
+        if (group_of_T(d, d->n_rows + j) >= d->n_groups) return 1;
+    std::vector<uint8_t> tmp(d->row_bytes);
+    for (uint64_t j = 0; j < n_new; ++j) {
+        const uint64_t id = d->n_rows;
+        const uint64_t g = group_of_T(d, id);
+        int comp = 0;
+        const uint32_t size = ibp_oracle_compress_row_T(rows + j * d->row_bytes, &d->mask[g * d->row_bytes], &d->bitval[g * d->row_bytes],
+                                                        d->row_bytes, d->CS, tmp.data(), &comp);
+        if (d->rowflag.size() * 8 < id + 1) d->rowflag.push_back(0);
+        put_bit(d->rowflag.data(), id, comp);
+        if (!comp) d->n_raw += 1;
+        d->row_offset.push_back(d->row_offset[id] + size);
+        d->stored.insert(d->stored.end(), tmp.begin(), tmp.begin() + size);
+        d->n_rows += 1;
+    }
+    return 0;
+}
+uint64_t ibp_oracle_T_n_rows(const ibp_oracle_ds_T* d) { return d->n_rows; }
 
 // Gather-decompress in thresholded mode (S8c thresholded step 7): check the per-row bit, copy or decode.
 int ibp_oracle_gather_decompress_T(const ibp_oracle_ds_T* d, const int64_t* ids, int64_t n, uint32_t index_span, uint8_t* out) {

@@ -453,3 +453,51 @@ def test_cache_value_widths_from_the_paper():
         oracle.cache_value(8, 0, True)
     with pytest.raises(ValueError):
         oracle.cache_value(0, 1 << 40, True)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# online append and the in-place slot layout
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,param,n0,n_new,rb", [(1, 6, 60, 45, 32), (0, 1 << 20, 200, 77, 64), (0, 16, 40, 8, 16), (0, 16, 40, 30, 16), (1, 4, 4, 9, 8)])
+def test_append_under_existing_masks(kind, param, n0, n_new, rb):
+    """Appended rows are compressed under the Mask/Bitval built from the first n0 rows: the metadata does not change, an
+    appended row's stored bytes are exactly compress_row_T(row, mask_g, bitval_g) (itself pinned by the hand-worked fixtures),
+    and gathering from the grown dataset equals the plain gather of the concatenated table (losslessness).  A mistake in
+    the group of an appended row (id taken relative to the batch instead of the table) fails the stored-bytes check."""
+    n = n0 + n_new
+    X = (datagen.random_bytes(n * rb, 900 + rb).reshape(n, rb) & datagen.random_bytes(rb, 901)[None, :]) | 0x20
+    X[n0 + 3] = datagen.random_bytes(rb, 902)                               # an appended row that does not match: kept raw or mostly non-participating
+    X[::5, 0] ^= 0x0F
+    gp = min(param, n0) if kind == 0 and param < (1 << 20) else param
+    ds = oracle.DatasetT(X[:n0], kind, gp, 4, 5)
+    masks = [(ds.mask(g).copy(), ds.bitval(g).copy()) for g in range(ds.n_groups)]
+    n_groups = ds.n_groups
+    fit = (-n0) % gp if (kind == 0 and gp < (1 << 20)) else n_new           # blocked groups: room left in the last built group
+    if n_new > fit:
+        with pytest.raises(ValueError):                                     # rows beyond the last built group have no metadata
+            ds.append(X[n0:])
+        assert ds.n_rows == n0                                              # ... and nothing was appended
+    ds.append(X[n0:n0 + min(fit, n_new)])
+    n = n0 + min(fit, n_new)
+    assert ds.n_rows == n and ds.n_groups == n_groups
+    for g, (m, b) in enumerate(masks):
+        assert np.array_equal(ds.mask(g), m) and np.array_equal(ds.bitval(g), b)
+    total = 0
+    for r in range(n):
+        g = r // gp if kind == 0 else r % gp
+        want, want_comp = oracle.compress_row_T(X[r], masks[g][0], masks[g][1])
+        got, comp = ds.row(r)
+        assert comp == want_comp and np.array_equal(got, want), f"row {r}"
+        total += want.size
+    assert ds.stored_bytes == total
+    ids = np.concatenate([np.arange(n, dtype=np.int64), (datagen.u64(300, 5) % np.uint64(n)).astype(np.int64)])
+    assert np.array_equal(ds.gather_decompress(ids), oracle.gather_plain(X[:n], ids))
+    # P:361: the in-place image keeps every row in its original slot: capacity x row_bytes bytes whatever the ratio, the first
+    # `size` bytes of a slot are the compressed row, the rest is zero
+    cap = n + 10
+    img = ds.slot_image(cap)
+    assert img.shape == (cap, rb) and img.nbytes == cap * rb
+    for r in (0, n0 - 1, n - 1):
+        data, _ = ds.row(r)
+        assert np.array_equal(img[r, : data.size], data) and not img[r, data.size:].any()
+    assert not img[n:].any()
