@@ -28,7 +28,8 @@
  *   - Thresholded mode: a compressed row is [participation bits, one per 4-byte chunk, chunk order][per chunk: its bits
  *     at the Mask=0 positions if it participates, else all 32 bits], LSB-first, zero padded to
  *     row_bytes - floor((bitsSaved - chunks)/8) bytes (Fig. 3 = P:243-299) and then to A; a raw row is the row.
- *     Rows lie in id order, each starting on a multiple of A (A >= 16 in this mode).
+ *     Rows lie in id order, each starting on a multiple of A (A >= 16 in this mode); with IBP_FLAG_SLOT_LAYOUT row r starts
+ *     at r * roundup(row_bytes, A) instead (the paper's in-place slots).
  *   - Store layout.  Blocked groups: groups in order, each group's base aligned to max(A,16); rows of a group at
  *     base + j*stride_g.  Strided groups: matrix row r (= id div S) at r*rowstride, tile t at prefix_t inside it.
  *   - Pointers are named *_host (CPU addressable), *_dev (GPU addressable on the handle's device).
@@ -71,7 +72,12 @@ typedef enum {
 
 enum {
     IBP_FLAG_PAGEABLE_STORE = 1u,  /* keep the packed store in ordinary memory: no zero-copy gather (CPU-only tests)  */
-    IBP_FLAG_HOSTALLOC_STORE = 2u  /* use cudaHostAlloc pinned memory instead of the default managed-host allocation  */
+    IBP_FLAG_HOSTALLOC_STORE = 2u, /* use cudaHostAlloc pinned memory instead of the default managed-host allocation  */
+    IBP_FLAG_SLOT_LAYOUT = 4u      /* thresholded mode only: the paper's in-place storage -- row r keeps a fixed slot of
+                                      roundup(row_bytes, A) bytes at r * slot, only its first `size` bytes are meaningful and
+                                      read; one byte per row in GPU memory holds the size (16-byte units) instead of a 4-byte
+                                      offset.  Host memory is not saved (the paper accepts that); in exchange a row can be
+                                      (re)written in place, so the store is APPENDABLE: ibp_append_rows_device            */
 };
 
 typedef enum {
@@ -93,6 +99,9 @@ typedef struct {
     uint32_t index_span;    /* consecutive rows selected by one id in ibp_gather_decompress; 0 = 1               */
     uint32_t flags;         /* IBP_FLAG_*                                                                        */
     uint32_t n_threads;     /* host threads for the build; 0 = all                                               */
+    uint64_t capacity_rows; /* IBP_FLAG_SLOT_LAYOUT: rows the store has slots for (>= n_rows; 0 = n_rows): the room
+                               ibp_append_rows_device can fill.  Ignored otherwise.  (struct_size without this field -- the
+                               layout of version 0.3 -- is accepted and means 0.)                                        */
 } ibp_build_params;
 
 typedef struct {
@@ -111,7 +120,11 @@ typedef struct {
     uint32_t reserved0;
     uint64_t n_rows_raw;               /* thresholded: rows kept uncompressed                            */
     uint64_t rowflag_bytes;            /* thresholded: per-row bitmask, 4*ceil(n_rows/32) bytes          */
-    uint64_t rowoffset_bytes;          /* thresholded: per-row offsets, 4*(n_rows+1) bytes                       */
+    uint64_t rowoffset_bytes;          /* thresholded: per-row offsets, 4*(n_rows+1) bytes (0 with the slot layout) */
+    uint64_t capacity_rows;            /* slot layout: rows the store has slots for; else n_rows                 */
+    uint64_t rowsize_bytes;            /* slot layout: per-row sizes, 1 byte per slot; else 0                    */
+    uint32_t slot_bytes;               /* slot layout: bytes per slot = roundup(row_bytes, A); else 0            */
+    uint32_t reserved1;
 } ibp_info;
 
 /* -- S0, S0': host-side compressor (P:229-231 masks with T=N per group; P:237-241, P:275-298 packing). ---------------
@@ -136,6 +149,19 @@ ibp_status ibp_build(const void* rows_host, const ibp_build_params* params, ibp_
  * missing or non-sm_100 device, UNSUPPORTED for groups of more than 2^32-1 rows.                                    */
 ibp_status ibp_build_device(const void* rows_dev, const ibp_build_params* params, int device, void* cuda_stream,
                             ibp_handle** out_handle);
+
+/* -- Online append ("we sample the KV cache generated from the prompt tokens to create the Mask
+ * and Bitval.  This metadata is used to compress the KV cache generated in the decode phase").  The handle must use the slot
+ * layout (IBP_FLAG_SLOT_LAYOUT) and have room: n_rows + n_new <= capacity_rows.  rows_dev: n_new x row_bytes on the handle's
+ * device (HBM or mapped host memory), 16-byte aligned.  New row j gets id n_rows + j and is compressed by a CUDA kernel under the
+ * EXISTING Mask/Bitval of its group (id div G, or id mod S) -- the metadata never changes -- and written into its slot of the host
+ * store over PCIe; its size byte and its bit of the per-row bitmask are set in GPU memory.  The group must already have metadata:
+ * strided groups need n_rows >= S at build time, blocked groups can only fill their last group (one group spanning all rows,
+ * group_param >= capacity_rows, is the paper's single global Mask/Bitval and takes any number of rows).  Synchronises the stream;
+ * the host mirrors (ibp_row_info, ibp_get_info) are updated.  Not concurrent with gathers that touch the new rows or with
+ * another append.  index_span must be 1 or divide n_new.  Errors: BAD_STATE (no slot layout, before upload), INVALID_ARG,
+ * UNSUPPORTED (no room, a group without metadata).                                                                     */
+ibp_status ibp_append_rows_device(ibp_handle* h, const void* rows_dev, int64_t n_new, void* cuda_stream);
 
 /* Where the time of an ibp_build_device call went (CUDA events on the stream around each kernel; total = wall clock of the
  * call including the host-side store allocation and copies).  BAD_STATE for a handle built by ibp_build.              */

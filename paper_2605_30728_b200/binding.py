@@ -19,6 +19,7 @@ STATUS = {0: "IBP_OK", 1: "IBP_ERR_INVALID_ARG", 2: "IBP_ERR_OUT_OF_MEMORY", 3: 
 IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED, IBP_GROUP_MAP = 0, 1, 2
 IBP_FLAG_PAGEABLE_STORE = 1
 IBP_FLAG_HOSTALLOC_STORE = 2
+IBP_FLAG_SLOT_LAYOUT = 4
 IBP_STORE_PAGEABLE, IBP_STORE_PINNED, IBP_STORE_MANAGED_HOST = 0, 1, 2
 
 
@@ -32,7 +33,7 @@ class ibp_build_params(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("row_bytes", C.c_uint32), ("n_rows", C.c_uint64),
                 ("group_kind", C.c_uint32), ("group_param", C.c_uint32), ("threshold_num", C.c_uint32),
                 ("threshold_den", C.c_uint32), ("align_bytes", C.c_uint32), ("index_span", C.c_uint32),
-                ("flags", C.c_uint32), ("n_threads", C.c_uint32)]
+                ("flags", C.c_uint32), ("n_threads", C.c_uint32), ("capacity_rows", C.c_uint64)]
 
 
 class ibp_info(C.Structure):
@@ -43,7 +44,8 @@ class ibp_info(C.Structure):
                 ("group_param", C.c_uint32), ("max_row_stride", C.c_uint32), ("device", C.c_int32),
                 ("store_kind", C.c_uint32), ("thresholded", C.c_uint32), ("threshold_num", C.c_uint32),
                 ("threshold_den", C.c_uint32), ("reserved0", C.c_uint32), ("n_rows_raw", C.c_uint64),
-                ("rowflag_bytes", C.c_uint64), ("rowoffset_bytes", C.c_uint64)]
+                ("rowflag_bytes", C.c_uint64), ("rowoffset_bytes", C.c_uint64), ("capacity_rows", C.c_uint64),
+                ("rowsize_bytes", C.c_uint64), ("slot_bytes", C.c_uint32), ("reserved1", C.c_uint32)]
 
 
 class ibp_build_stats(C.Structure):
@@ -73,6 +75,7 @@ _vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c
 SIGNATURES = {
     "ibp_build": (_int, [_vp, C.POINTER(ibp_build_params), C.POINTER(_vp)]),
     "ibp_build_device": (_int, [_vp, C.POINTER(ibp_build_params), _int, _vp, C.POINTER(_vp)]),
+    "ibp_append_rows_device": (_int, [_vp, _vp, _i64, _vp]),
     "ibp_get_build_stats": (_int, [_vp, C.POINTER(ibp_build_stats)]),
     "ibp_upload_metadata": (_int, [_vp, _int, _vp]),
     "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
@@ -177,6 +180,10 @@ class Handle:
 
     def gather_decompress_range_host(self, first_row, n_rows, out_host, stream=None):
         _check(lib().ibp_gather_decompress_range_host(self._h, first_row, n_rows, _ptr(out_host), stream))
+
+    def append_rows_device(self, rows_dev, n_new, stream=None):
+        _check(lib().ibp_append_rows_device(self._h, _ptr(rows_dev), n_new, stream))
+        return self
 
     def packed_range(self, first_row, n_rows):
         p, nb = _vp(), _u64()
@@ -319,21 +326,21 @@ class Cache:
 
 
 def ibp_build(rows_host: np.ndarray, row_bytes: int, group_kind: int, group_param: int, align_bytes: int = 0,
-              index_span: int = 1, flags: int = 0, n_threads: int = 0, threshold=(1, 1)) -> Handle:
+              index_span: int = 1, flags: int = 0, n_threads: int = 0, threshold=(1, 1), capacity_rows: int = 0) -> Handle:
     rows = np.ascontiguousarray(rows_host)
     assert rows.nbytes % row_bytes == 0
     p = ibp_build_params(C.sizeof(ibp_build_params), row_bytes, rows.nbytes // row_bytes, group_kind, group_param,
-                         threshold[0], threshold[1], align_bytes, index_span, flags, n_threads)
+                         threshold[0], threshold[1], align_bytes, index_span, flags, n_threads, capacity_rows)
     h = _vp()
     _check(lib().ibp_build(rows.ctypes.data, C.byref(p), C.byref(h)))
     return Handle(h)
 
 
 def ibp_build_device(rows_dev, n_rows: int, row_bytes: int, group_kind: int, group_param: int, align_bytes: int = 0,
-                     index_span: int = 1, flags: int = 0, threshold=(1, 1), device: int = 0, stream=None) -> Handle:
+                     index_span: int = 1, flags: int = 0, threshold=(1, 1), device: int = 0, stream=None, capacity_rows: int = 0) -> Handle:
     """rows_dev: address of n_rows x row_bytes bytes the device can read (HBM or mapped host memory)."""
     p = ibp_build_params(C.sizeof(ibp_build_params), row_bytes, n_rows, group_kind, group_param,
-                         threshold[0], threshold[1], align_bytes, index_span, flags, 0)
+                         threshold[0], threshold[1], align_bytes, index_span, flags, 0, capacity_rows)
     h = _vp()
     _check(lib().ibp_build_device(_ptr(rows_dev), C.byref(p), device, stream, C.byref(h)))
     return Handle(h)

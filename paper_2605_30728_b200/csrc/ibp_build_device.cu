@@ -593,6 +593,126 @@ __global__ void __launch_bounds__(256) ibp_pack_t_kernel(const PackParams P) {
     __syncwarp();
 }
 
+// Online append, slot layout: one warp per NEW row.  The row is compressed under the existing Mask/Bitval of
+// its group -- getCompressSize (Fig. 3 lines 1-19) and compress (lines 21-33) in one visit -- into a shared-memory image and
+// written to its own slot of the host store; the size byte and the bit of the per-row bitmask are set in GPU memory.
+struct AppendParams {
+    const uint32_t* rows;        // n_new rows
+    const uint32_t* meta;
+    uint8_t* store;
+    uint8_t* row_size;
+    uint32_t* row_flag;
+    unsigned long long* sums;    // [0] += byte-aligned sizes, [1] += stored bytes incl. padding, [2] += rows kept raw
+    uint64_t first_id, n_new;
+    uint32_t nw, n_pass, group_param, group_shift, strided, align_bytes, slot_bytes, img_bytes;
+};
+
+template <int W>
+__global__ void __launch_bounds__(256) ibp_append_kernel(const AppendParams P) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    uint32_t* img = (uint32_t*)(smem + (size_t)wib * P.img_bytes);
+    const uint64_t S = P.group_param;
+    for (uint64_t j = (uint64_t)blockIdx.x * wpc + wib; j < P.n_new; j += (uint64_t)gridDim.x * wpc) {
+        const uint64_t id = P.first_id + j;
+        const uint64_t g = P.strided ? id % S : group_of_u(P.group_param, P.group_shift, id);
+        const uint32_t* x_row = P.rows + j * P.nw;
+        const uint32_t* gm = P.meta + g * 2ull * P.nw;
+        // ---- size
+        uint32_t saved = 0;
+        for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+            const uint32_t w0 = (pass * 32u + lane) * W;
+            if (w0 < P.nw) {
+                uint32_t m[W], b[W], x[W];
+                VecIO<W>::ld(gm + w0, m);
+                VecIO<W>::ld(gm + P.nw + w0, b);
+                VecIO<W>::ld(x_row + w0, x);
+#pragma unroll
+                for (int q = 0; q < W; ++q) saved += ((x[q] & m[q]) == b[q]) ? __popc(m[q]) : 0u;
+            }
+        }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) saved += __shfl_xor_sync(0xFFFFFFFFu, saved, d);
+        const int64_t net = (int64_t)saved - (int64_t)P.nw;                       // minus the participation bits
+        const uint32_t bytes_saved = net >= 8 ? (uint32_t)(net / 8) : 0u;         // floor
+        const uint32_t size = 4u * P.nw - bytes_saved;
+        const bool compressed = bytes_saved != 0;                                  // else stored raw
+        const uint32_t stored = (size + P.align_bytes - 1) / P.align_bytes * P.align_bytes;
+        // ---- image
+        for (uint32_t v = lane; v < stored / 16 + 1; v += 32) ((uint4*)img)[v] = make_uint4(0, 0, 0, 0);
+        __syncwarp();
+        if (!compressed) {
+            for (uint32_t w = lane; w < P.nw; w += 32) img[w] = x_row[w];
+        } else {
+            uint32_t carry = P.nw;                                                // payloads follow the participation bits (R8)
+            for (uint32_t pass = 0; pass < P.n_pass; ++pass) {
+                const uint32_t w0 = (pass * 32u + lane) * W;
+                const bool active = w0 < P.nw;
+                uint32_t m[W], b[W], x[W], kq[W], part = 0, t = 0;
+                if (active) {
+                    VecIO<W>::ld(gm + w0, m);
+                    VecIO<W>::ld(gm + P.nw + w0, b);
+                    VecIO<W>::ld(x_row + w0, x);
+                }
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    const bool pq = active && (x[q] & m[q]) == b[q];
+                    part |= (uint32_t)pq << q;
+                    kq[q] = active ? (pq ? __popc(~m[q]) : 32u) : 0u;
+                    t += kq[q];
+                }
+                const uint32_t incl = warp_inclusive_scan(t, lane);
+                uint32_t bit = carry + incl - t;
+                if (active) {
+                    if (part) atomicOr(img + (w0 >> 5), part << (w0 & 31u));       // W divides 32: one word
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        uint32_t c = x[q];
+                        if ((part >> q) & 1u) { uint32_t mv[5]; suffix_masks(~m[q], mv); c = compress_bits(x[q], ~m[q], mv); }
+                        if (kq[q] == 32u) {
+                            const uint32_t wq = bit >> 5, sh = bit & 31u;
+                            atomicOr(img + wq, c << sh);
+                            if (sh) atomicOr(img + wq + 1, c >> (32u - sh));
+                        } else {
+                            insert_bits(img, bit, c, kq[q]);
+                        }
+                        bit += kq[q];
+                    }
+                }
+                carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
+            }
+        }
+        __syncwarp();
+        // the whole slot is rewritten (zeros beyond the row), so a slot can be reused
+        uint8_t* dst = P.store + id * (uint64_t)P.slot_bytes;
+        for (uint32_t v = lane; v < P.slot_bytes / 16; v += 32) {
+            const uint4 t4 = v < stored / 16 ? ((const uint4*)img)[v] : make_uint4(0, 0, 0, 0);
+            ((uint4*)dst)[v] = t4;
+        }
+        if (lane == 0) {
+            P.row_size[id] = (uint8_t)(stored / 16);
+            if (compressed) atomicOr(P.row_flag + (id >> 5), 1u << (id & 31u));
+            else atomicAnd(P.row_flag + (id >> 5), ~(1u << (id & 31u)));
+            atomicAdd(P.sums + 0, (unsigned long long)size);
+            atomicAdd(P.sums + 1, (unsigned long long)stored);
+            if (!compressed) atomicAdd(P.sums + 2, 1ull);
+        }
+        __syncwarp();
+    }
+}
+
+// Slot layout in ibp_build_device: the size kernel's per-row units become the size bytes, and the offsets the pack kernel
+// walks are the fixed shifts r * slot16 (a temporary array: the handle keeps no offsets in this layout).
+__global__ void ibp_slot_layout_kernel(uint32_t* __restrict__ units_to_off, uint64_t n, uint32_t slot16, uint8_t* __restrict__ row_size,
+                                       unsigned long long* __restrict__ stored_units) {
+    unsigned long long local = 0;
+    for (uint64_t r = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; r <= n; r += (uint64_t)gridDim.x * blockDim.x) {
+        if (r < n) { const uint32_t u = units_to_off[r]; row_size[r] = (uint8_t)u; local += u; }
+        units_to_off[r] = (uint32_t)(r * slot16);
+    }
+    if (local) atomicAdd(stored_units, local);
+}
+
 // ------------------------------------------------------------------------------------------------ exclusive scan (u32 -> u32)
 // 4096 items per block of 1024 threads; totals in 64 bits so that an overflow of the 32-bit offsets is detected.
 __global__ void __launch_bounds__(1024) ibp_scan_sums(const uint32_t* __restrict__ in, uint64_t n, unsigned long long* __restrict__ bsum) {
@@ -840,7 +960,11 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         // pass 1: sizes and flags; scan -> row offsets
         const uint64_t n_flag_words = (n + 31) / 32;
         IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, (n + 1) * 4));
-        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, n_flag_words * 4));
+        {
+            const uint64_t words = h->slot_layout ? (h->capacity_rows + 31) / 32 : n_flag_words;
+            IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, words * 4));
+            IBP_CUDA(cudaMemsetAsync(h->row_flag_dev, 0, words * 4, st));
+        }
         const uint64_t nblk = (n + 4095) / 4096;
         DevBuf aux;
         IBP_CUDA(cudaMalloc(&aux.p, (nblk + 2) * 8));
@@ -860,26 +984,39 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         }
         t_size.stop();
         IBP_CUDA(cudaGetLastError());
+        unsigned long long totals[2] = {0, 0};   // [0] = stored bytes of the rows in 16-byte units, [1] = sum of the byte-aligned row sizes
         t_scan.start();
-        ibp_scan_sums<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
-        ibp_scan_bsums<<<1, 1024, 0, st>>>(bsum, nblk);
-        ibp_scan_apply<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+        if (h->slot_layout) {
+            const uint64_t cap = h->capacity_rows;
+            if (h->slot_bytes / 16 > 255) { ibp_set_error("ibp_build_device: slot layout needs row_bytes <= 4080"); return IBP_ERR_UNSUPPORTED; }
+            IBP_CUDA(cudaMalloc((void**)&h->row_size_dev, std::max<uint64_t>(cap, 16)));
+            IBP_CUDA(cudaMemsetAsync(h->row_size_dev, 0, std::max<uint64_t>(cap, 16), st));
+            IBP_CUDA(cudaMemsetAsync(bsum + nblk, 0, 8, st));
+            ibp_slot_layout_kernel<<<(unsigned)std::min<uint64_t>((n + 256) / 256, (uint64_t)sms * 8), 256, 0, st>>>(h->row_off_dev, n, h->slot_bytes / 16, h->row_size_dev, bsum + nblk);
+        } else {
+            ibp_scan_sums<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+            ibp_scan_bsums<<<1, 1024, 0, st>>>(bsum, nblk);
+            ibp_scan_apply<<<(unsigned)nblk, 1024, 0, st>>>(h->row_off_dev, n, bsum);
+        }
         t_scan.stop();
         IBP_CUDA(cudaGetLastError());
-        unsigned long long totals[2] = {0, 0};   // [0] = store size in 16-byte units, [1] = sum of the byte-aligned row sizes
         IBP_CUDA(cudaMemcpyAsync(totals, bsum + nblk, 16, cudaMemcpyDeviceToHost, st));
-        try { h->row_off.resize(n + 1); h->row_flag.resize(n_flag_words); }
-        catch (...) { ibp_set_error("ibp_build_device: out of memory (row offsets)"); return IBP_ERR_OUT_OF_MEMORY; }
+        const uint64_t n_flag_alloc = h->slot_layout ? (h->capacity_rows + 31) / 32 : n_flag_words;
+        try {
+            if (h->slot_layout) h->row_size.assign(h->capacity_rows, 0); else h->row_off.resize(n + 1);
+            h->row_flag.assign(n_flag_alloc, 0u);
+        } catch (...) { ibp_set_error("ibp_build_device: out of memory (row offsets)"); return IBP_ERR_OUT_OF_MEMORY; }
         IBP_CUDA(cudaMemcpyAsync(h->row_flag.data(), h->row_flag_dev, n_flag_words * 4, cudaMemcpyDeviceToHost, st));
         IBP_CUDA(cudaStreamSynchronize(st));
-        if (totals[0] > 0xFFFFFFFFull) { ibp_set_error("ibp_build_device: thresholded store exceeds 64 GiB (4-byte row offsets in 16-byte units)"); return IBP_ERR_UNSUPPORTED; }
-        IBP_CUDA(cudaMemcpyAsync(h->row_off.data(), h->row_off_dev, (n + 1) * 4, cudaMemcpyDeviceToHost, st));
+        if (!h->slot_layout && totals[0] > 0xFFFFFFFFull) { ibp_set_error("ibp_build_device: thresholded store exceeds 64 GiB (4-byte row offsets in 16-byte units)"); return IBP_ERR_UNSUPPORTED; }
+        if (h->slot_layout) IBP_CUDA(cudaMemcpyAsync(h->row_size.data(), h->row_size_dev, n, cudaMemcpyDeviceToHost, st));
+        else IBP_CUDA(cudaMemcpyAsync(h->row_off.data(), h->row_off_dev, (n + 1) * 4, cudaMemcpyDeviceToHost, st));
         uint64_t n_comp = 0;
         for (uint64_t i = 0; i < n_flag_words; ++i) n_comp += (uint64_t)__builtin_popcount(h->row_flag[i]);
         h->n_rows_raw = n - n_comp;
         h->packed_bytes_bytealigned = totals[1];
         h->packed_bytes_rows = totals[0] * 16;
-        h->store_used = totals[0] * 16;
+        h->store_used = h->slot_layout ? h->capacity_rows * (uint64_t)h->slot_bytes : totals[0] * 16;
         h->store_bytes = (h->store_used + 64 + 4095) / 4096 * 4096;
         h->max_stride = (p.row_bytes + p.align_bytes - 1) / p.align_bytes * p.align_bytes;
         rc = ibp_alloc_store(h, nthreads);
@@ -908,6 +1045,7 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
         t_pack.stop();
         IBP_CUDA(cudaGetLastError());
         IBP_CUDA(cudaStreamSynchronize(st));
+        if (h->slot_layout) { cudaFree(h->row_off_dev); h->row_off_dev = nullptr; }   // the fixed shift needs no table
     }
     h->built_on_device = true;
     ibp_build_stats& S = h->build_stats;
@@ -920,6 +1058,67 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
     S.total_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     guard.h = nullptr;
     *out_handle = h;
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_append_rows_device(ibp_handle* h, const void* rows_dev, int64_t n_new, void* cuda_stream) {
+    if (!h) { ibp_set_error("ibp_append_rows_device: null handle"); return IBP_ERR_INVALID_ARG; }
+    if (!h->slot_layout) { ibp_set_error("ibp_append_rows_device: the handle was not built with IBP_FLAG_SLOT_LAYOUT (a dense store cannot grow in place)"); return IBP_ERR_BAD_STATE; }
+    if (h->device < 0 || !h->meta_dev || !h->store_dev) { ibp_set_error("ibp_append_rows_device: call ibp_upload_metadata first (GPU-visible store)"); return IBP_ERR_BAD_STATE; }
+    if (n_new == 0) return IBP_OK;
+    if (n_new < 0 || !rows_dev || ((uintptr_t)rows_dev & 15u)) { ibp_set_error("ibp_append_rows_device: bad argument (n_new < 0, null or unaligned rows_dev)"); return IBP_ERR_INVALID_ARG; }
+    ibp_build_params& p = h->p;
+    const uint64_t first = p.n_rows, last = first + (uint64_t)n_new - 1;
+    if (last >= h->capacity_rows) { ibp_set_error("ibp_append_rows_device: %lld rows do not fit (%llu of %llu slots used)", (long long)n_new, (unsigned long long)first, (unsigned long long)h->capacity_rows); return IBP_ERR_UNSUPPORTED; }
+    if ((uint64_t)n_new % p.index_span) { ibp_set_error("ibp_append_rows_device: n_new must be a multiple of index_span"); return IBP_ERR_INVALID_ARG; }
+    const uint64_t g_last = p.group_kind == IBP_GROUP_BLOCKED ? last / p.group_param : std::min<uint64_t>(last, (uint64_t)p.group_param - 1);
+    const uint64_t g_need = p.group_kind == IBP_GROUP_BLOCKED ? g_last : (first + (uint64_t)n_new >= p.group_param ? (uint64_t)p.group_param - 1 : last);
+    if (std::max(g_last, g_need) >= h->n_groups) {
+        ibp_set_error("ibp_append_rows_device: a new row falls in group %llu, which has no Mask/Bitval (%llu groups were built)", (unsigned long long)std::max(g_last, g_need), (unsigned long long)h->n_groups);
+        return IBP_ERR_UNSUPPORTED;
+    }
+    IBP_CUDA(cudaSetDevice(h->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int W = pick_W(p.row_bytes);
+    AppendParams A;
+    memset(&A, 0, sizeof A);
+    A.rows = (const uint32_t*)rows_dev; A.meta = h->meta_dev; A.store = h->store_dev;
+    A.row_size = h->row_size_dev; A.row_flag = h->row_flag_dev;
+    A.first_id = first; A.n_new = (uint64_t)n_new;
+    A.nw = h->n_words; A.n_pass = (h->n_words + 32 * W - 1) / (32 * W);
+    A.group_param = p.group_param; A.group_shift = 0xFFFFFFFFu;
+    if ((p.group_param & (p.group_param - 1)) == 0) { uint32_t sft = 0; while ((1u << sft) < p.group_param) ++sft; A.group_shift = sft; }
+    A.strided = p.group_kind == IBP_GROUP_STRIDED;
+    A.align_bytes = p.align_bytes; A.slot_bytes = h->slot_bytes;
+    A.img_bytes = (h->slot_bytes + 32u + 127u) / 128u * 128u;
+    int wpc = 8;
+    while (wpc > 1 && (size_t)wpc * A.img_bytes > 200 * 1024) wpc >>= 1;
+    const size_t smem = (size_t)wpc * A.img_bytes;
+    DevBuf sums;
+    IBP_CUDA(cudaMalloc(&sums.p, 24));
+    IBP_CUDA(cudaMemsetAsync(sums.p, 0, 24, st));
+    A.sums = (unsigned long long*)sums.p;
+    const int grid = (int)std::min<uint64_t>(((uint64_t)n_new + wpc - 1) / wpc, (uint64_t)h->sm_count * 4);
+#define IBP_APPEND(W_)                                                                              \
+    do {                                                                                            \
+        static unsigned long long optin_done = 0;                                                   \
+        if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(ibp_append_kernel<W_>, &optin_done));     \
+        ibp_append_kernel<W_><<<grid, wpc * 32, smem, st>>>(A);                                     \
+    } while (0)
+    switch (W) { case 4: IBP_APPEND(4); break; case 2: IBP_APPEND(2); break; default: IBP_APPEND(1); break; }
+#undef IBP_APPEND
+    IBP_CUDA(cudaGetLastError());
+    // host mirrors: sizes and flag words of the new rows, totals
+    unsigned long long tot[3] = {0, 0, 0};
+    const uint64_t w_lo = first >> 5, w_hi = last >> 5;
+    IBP_CUDA(cudaMemcpyAsync(tot, sums.p, 24, cudaMemcpyDeviceToHost, st));
+    IBP_CUDA(cudaMemcpyAsync(h->row_size.data() + first, h->row_size_dev + first, (size_t)n_new, cudaMemcpyDeviceToHost, st));
+    IBP_CUDA(cudaMemcpyAsync(h->row_flag.data() + w_lo, h->row_flag_dev + w_lo, (size_t)(w_hi - w_lo + 1) * 4, cudaMemcpyDeviceToHost, st));
+    IBP_CUDA(cudaStreamSynchronize(st));
+    p.n_rows += (uint64_t)n_new;
+    h->packed_bytes_bytealigned += tot[0];
+    h->packed_bytes_rows += tot[1];
+    h->n_rows_raw += tot[2];
     return IBP_OK;
 }
 

@@ -118,7 +118,7 @@ extern "C" ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host
             const uint64_t off = ibp_row_offset(h, id);
             uint64_t bytes, flag = 1;
             if (h->thresholded) {
-                bytes = 16ull * (h->row_off[id + 1] - h->row_off[id]);
+                bytes = ibp_row_stored_T(h, id);
                 flag = (h->row_flag[id >> 5] >> (id & 31)) & 1u;
             } else {
                 bytes = h->gtab[ibp_group_of(h, id)].stride;

@@ -51,6 +51,8 @@ struct DecodeParams {
     uint32_t occ_cap;              // host side only: CTAs per SM for random-row gathers (0 = 2)
     const uint32_t* row_off;       // thresholded mode: per-row offsets (16-byte units), n_rows + 1 entries
     const uint32_t* row_flag;      // thresholded mode: bit r = 1 iff row r is compressed
+    const uint8_t* row_size;       // slot layout: stored size of row r in 16-byte units; the row lies at r * slot16 * 16
+    uint32_t slot16;               // slot layout: slot size in 16-byte units; 0 = dense rows addressed through row_off
     uint32_t keep_l2;              // write the rows with the default cache policy (a later pass re-reads them) instead of streaming
     // compressed GPU cache in front of the store (CACHE instantiations only)
     const uint64_t* cmap;          // hash map slots {id + 1, value}; value = offset:40 | slab:3 | compressed:1
@@ -202,9 +204,14 @@ __global__ void __launch_bounds__(256) ibp_decode_kernel(const DecodeParams P) {
             const uint8_t* a0;
             uint32_t nvec;
             if (TM) {
-                const uint32_t o0 = __ldg(P.row_off + id), o1 = __ldg(P.row_off + id + 1);
-                a0 = P.store + (16ull * o0 - P.bias);                         // rows start on 16-byte boundaries
-                nvec = o1 - o0;
+                if (P.slot16) {                                               // in-place slots: a fixed shift, only the first `size` bytes are read
+                    a0 = P.store + (16ull * P.slot16 * id - P.bias);
+                    nvec = P.row_size[id];
+                } else {
+                    const uint32_t o0 = __ldg(P.row_off + id), o1 = __ldg(P.row_off + id + 1);
+                    a0 = P.store + (16ull * o0 - P.bias);                     // rows start on 16-byte boundaries
+                    nvec = o1 - o0;
+                }
             } else {
                 const uint64_t g = group_of(P, id, STRIDED);
                 if (g != fg) { fg = g; fe = P.gtab[g]; }
@@ -607,6 +614,8 @@ static void fill_common(const ibp_handle* h, DecodeParams& P) {
     if ((h->p.group_param & (h->p.group_param - 1)) == 0) { uint32_t s = 0; while ((1u << s) < h->p.group_param) ++s; P.group_shift = s; }
     P.row_off = h->row_off_dev;
     P.row_flag = h->row_flag_dev;
+    P.row_size = h->row_size_dev;
+    P.slot16 = h->slot_layout ? h->slot_bytes / 16 : 0;
 }
 
 // ------------------------------------------------------------------------------------------------ stream launch
@@ -897,7 +906,11 @@ ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream) {
         IBP_CUDA(cudaMalloc((void**)&h->gtab_dev, h->gtab.size() * sizeof(IbpGroupEntry)));
         IBP_CUDA(cudaMemcpyAsync(h->gtab_dev, h->gtab.data(), h->gtab.size() * sizeof(IbpGroupEntry), cudaMemcpyHostToDevice, st));
     }
-    if (h->thresholded && !h->row_off_dev) {
+    if (h->slot_layout && !h->row_size_dev) {
+        IBP_CUDA(cudaMalloc((void**)&h->row_size_dev, std::max<size_t>(h->row_size.size(), 16)));
+        IBP_CUDA(cudaMemcpyAsync(h->row_size_dev, h->row_size.data(), h->row_size.size(), cudaMemcpyHostToDevice, st));
+    }
+    if (h->thresholded && !h->slot_layout && !h->row_off_dev) {
         IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, h->row_off.size() * 4));
         IBP_CUDA(cudaMemcpyAsync(h->row_off_dev, h->row_off.data(), h->row_off.size() * 4, cudaMemcpyHostToDevice, st));
     }
@@ -1033,7 +1046,7 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     P.out = (uint8_t*)out_dev;
     P.n = n;
     P.span = h->p.index_span;
-    if (h->stream_mode && h->thresholded && stream_t_fits(h))
+    if (h->stream_mode && h->thresholded && !h->slot_layout && stream_t_fits(h))
         return launch_stream_t(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
     if (h->stream_mode && !h->thresholded)
         return launch_stream(h, h->store_dev, 0, row_ids_dev, n, 0, (int64_t)h->p.index_span, out_dev, st);
@@ -1049,7 +1062,9 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
 // byte of first_row.  Shared by the resident decode (packed bytes staged in HBM) and the zero-copy range gather.
 static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t first_row, int64_t n_rows, void* out_dev, cudaStream_t st, bool resident = false) {
-    if (h->stream_mode && h->thresholded && stream_t_fits(h))
+    // (slot layout: consecutive rows are not contiguous in the store -- only the head of every slot is meaningful -- so runs
+    // take the per-row kernel, which fetches exactly each row's bytes)
+    if (h->stream_mode && h->thresholded && !h->slot_layout && stream_t_fits(h))
         return launch_stream_t(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
     if (h->stream_mode && !h->thresholded)
         return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st, resident);

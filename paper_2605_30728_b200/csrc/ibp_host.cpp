@@ -10,6 +10,7 @@
 
 #include <algorithm>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -153,8 +154,15 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
 // Validates the build parameters (shared by ibp_build and ibp_build_device), fills in the defaults and allocates the handle with
 // its host-side metadata arrays.
 ibp_status ibp_prepare_handle(const ibp_build_params* params, const char* who, ibp_handle** out) {
-    if (params->struct_size != sizeof(ibp_build_params)) { ibp_set_error("%s: struct_size %u != %zu", who, params->struct_size, sizeof(ibp_build_params)); return IBP_ERR_INVALID_ARG; }
-    ibp_build_params p = *params;
+    const size_t size_v03 = offsetof(ibp_build_params, capacity_rows);        // the struct before capacity_rows was added
+    if (params->struct_size != sizeof(ibp_build_params) && params->struct_size != size_v03) {
+        ibp_set_error("%s: struct_size %u is neither %zu nor %zu", who, params->struct_size, sizeof(ibp_build_params), size_v03);
+        return IBP_ERR_INVALID_ARG;
+    }
+    ibp_build_params p;
+    memset(&p, 0, sizeof p);
+    memcpy(&p, params, params->struct_size);
+    p.struct_size = sizeof(ibp_build_params);
     if (p.row_bytes == 0 || p.row_bytes % 4 || p.row_bytes > 65536) { ibp_set_error("%s: row_bytes %u must be a multiple of 4 in 4..65536", who, p.row_bytes); return IBP_ERR_INVALID_ARG; }
     if (p.n_rows == 0 || p.group_param == 0 || p.group_kind > 1) { ibp_set_error("%s: n_rows, group_param must be >= 1 and group_kind 0|1", who); return IBP_ERR_INVALID_ARG; }
     if (p.threshold_num == 0 && p.threshold_den == 0) p.threshold_num = p.threshold_den = 1;
@@ -167,6 +175,13 @@ ibp_status ibp_prepare_handle(const ibp_build_params* params, const char* who, i
     if (p.index_span == 0) p.index_span = 1;
     if (p.n_rows % p.index_span) { ibp_set_error("%s: n_rows must be a multiple of index_span", who); return IBP_ERR_INVALID_ARG; }
     if (p.index_span > 1 && p.group_kind != IBP_GROUP_BLOCKED) { ibp_set_error("%s: index_span > 1 needs blocked groups", who); return IBP_ERR_INVALID_ARG; }
+    if (p.flags & IBP_FLAG_SLOT_LAYOUT) {
+        if (!thresholded) { ibp_set_error("%s: IBP_FLAG_SLOT_LAYOUT is a thresholded-mode layout (strict rows of a group all have one size: a dense store is already indexable)", who); return IBP_ERR_INVALID_ARG; }
+        if (p.capacity_rows == 0) p.capacity_rows = p.n_rows;
+        if (p.capacity_rows < p.n_rows) { ibp_set_error("%s: capacity_rows < n_rows", who); return IBP_ERR_INVALID_ARG; }
+    } else {
+        p.capacity_rows = 0;
+    }
 
     ibp_handle* h = new (std::nothrow) ibp_handle();
     if (!h) { ibp_set_error("%s: out of memory", who); return IBP_ERR_OUT_OF_MEMORY; }
@@ -175,6 +190,11 @@ ibp_status ibp_prepare_handle(const ibp_build_params* params, const char* who, i
     h->n_groups = p.group_kind == IBP_GROUP_BLOCKED ? (p.n_rows + p.group_param - 1) / p.group_param
                                                      : std::min<uint64_t>(p.group_param, p.n_rows);
     h->thresholded = thresholded;
+    if (p.flags & IBP_FLAG_SLOT_LAYOUT) {
+        h->slot_layout = true;
+        h->slot_bytes = (uint32_t)((p.row_bytes + p.align_bytes - 1) / p.align_bytes * p.align_bytes);
+        h->capacity_rows = p.capacity_rows;
+    }
     try {
         h->meta.assign(h->n_groups * 2 * h->n_words, 0);
         h->gtab.assign(h->n_groups, IbpGroupEntry{0, 0, 0});
@@ -488,6 +508,18 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
     }
     h->n_rows_raw = n_raw;
     h->packed_bytes_bytealigned = bytes_aligned;
+    if (h->slot_layout) {
+        // P:361 in-place storage: row r keeps the slot [r*slot, (r+1)*slot); one size byte per slot (16-byte units) replaces the offsets
+        const uint64_t cap = h->capacity_rows;
+        if (h->slot_bytes / 16 > 255) { ibp_set_error("ibp_build: slot layout needs row_bytes <= 4080 (one size byte per row, 16-byte units)"); return IBP_ERR_UNSUPPORTED; }
+        h->row_size.assign(cap, 0);
+        h->row_flag.resize((cap + 31) / 32, 0u);
+        uint64_t stored = 0;
+        for (uint64_t r = 0; r < n; ++r) { h->row_size[r] = (uint8_t)(round_up(size[r], A) / 16); stored += 16ull * h->row_size[r]; }
+        h->packed_bytes_rows = stored;
+        h->store_used = cap * (uint64_t)h->slot_bytes;
+        h->store_bytes = round_up(h->store_used + 64, 4096);
+    } else {
     h->row_off.assign(n + 1, 0u);
     uint64_t cursor = 0;                                                    // in 16-byte units
     for (uint64_t r = 0; r < n; ++r) {
@@ -499,6 +531,7 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
     h->packed_bytes_rows = cursor * 16;
     h->store_used = cursor * 16;
     h->store_bytes = round_up(h->store_used + 64, 4096);
+    }
     h->max_stride = (uint32_t)round_up(p.row_bytes, A);
     for (uint64_t g = 0; g < ng; ++g) { h->gtab[g].base = 0; h->gtab[g].stride = 0; }    // unused in this mode
 
@@ -509,7 +542,7 @@ static ibp_status build_thresholded(ibp_handle* h, const uint32_t* rows, int nth
 #pragma omp parallel for schedule(dynamic, 1024) num_threads(nthreads)
     for (int64_t r = 0; r < (int64_t)n; ++r) {
         const uint32_t* x = rows + (uint64_t)r * nw;
-        uint8_t* dst = h->store + 16ull * h->row_off[r];
+        uint8_t* dst = h->store + ibp_row_offset(h, (uint64_t)r);
         if (!((h->row_flag[r >> 5] >> (r & 31)) & 1u)) { memcpy(dst, x, 4ull * nw); continue; }
         const uint32_t* m = &h->meta[ibp_group_of(h, (uint64_t)r) * 2 * nw];
         const uint32_t* b = m + nw;
@@ -559,6 +592,9 @@ extern "C" ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out) {
     out->n_rows_raw = h->n_rows_raw;
     out->rowflag_bytes = h->row_flag.size() * 4ull;
     out->rowoffset_bytes = h->row_off.size() * 4ull;
+    out->capacity_rows = h->slot_layout ? h->capacity_rows : h->p.n_rows;
+    out->rowsize_bytes = h->row_size.size();
+    out->slot_bytes = h->slot_layout ? h->slot_bytes : 0;
     if (h->thresholded) out->aux_bytes = out->rowflag_bytes + out->rowoffset_bytes;
     return IBP_OK;
 }
@@ -577,7 +613,7 @@ static uint32_t row_size_from_store(const ibp_handle* h, uint64_t row) {
     if (!((h->row_flag[row >> 5] >> (row & 31)) & 1u)) return h->p.row_bytes;
     const uint32_t nw = h->n_words;
     const uint32_t* m = &h->meta[ibp_group_of(h, row) * 2 * nw];
-    const uint8_t* src = h->store + 16ull * h->row_off[row];
+    const uint8_t* src = h->store + ibp_row_offset(h, (uint64_t)row);
     uint64_t bits = nw;
     for (uint32_t w = 0; w < nw; ++w) bits += ((src[w >> 3] >> (w & 7)) & 1u) ? (uint32_t)__builtin_popcount(~m[w]) : 32u;
     return (uint32_t)((bits + 7) / 8);
@@ -587,7 +623,7 @@ extern "C" ibp_status ibp_row_info(const ibp_handle* h, int64_t row, const void*
     if (!h || row < 0 || (uint64_t)row >= h->p.n_rows) { ibp_set_error("ibp_row_info: bad row"); return IBP_ERR_INVALID_ARG; }
     if (host_ptr) *host_ptr = h->store + ibp_row_offset(h, (uint64_t)row);
     if (h->thresholded) {
-        if (stored_bytes) *stored_bytes = 16u * (h->row_off[row + 1] - h->row_off[row]);
+        if (stored_bytes) *stored_bytes = (uint32_t)ibp_row_stored_T(h, (uint64_t)row);
         if (size_bytes) *size_bytes = row_size_from_store(h, (uint64_t)row);
         if (is_compressed) *is_compressed = (int)((h->row_flag[row >> 5] >> (row & 31)) & 1u);
     } else {
@@ -630,7 +666,7 @@ extern "C" ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, i
     const uint64_t begin = (uint64_t)first_row < h->p.n_rows ? ibp_row_offset(h, (uint64_t)first_row) : h->store_used;
     uint64_t end = begin;
     if (h->thresholded) {
-        end = 16ull * h->row_off[first_row + n_rows];
+        end = h->slot_layout ? (uint64_t)(first_row + n_rows) * h->slot_bytes : 16ull * h->row_off[first_row + n_rows];
     } else if (n_rows > 0) {
         const uint64_t last = (uint64_t)(first_row + n_rows - 1);
         const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? last / h->p.group_param : last % h->p.group_param;
@@ -652,7 +688,7 @@ extern "C" ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* i
         if (id < 0 || (uint64_t)id * span >= h->p.n_rows) { ibp_set_error("ibp_batch_link_bytes: id out of range"); return IBP_ERR_INVALID_ARG; }
         for (uint64_t j = 0; j < span; ++j) {
             const uint64_t r = (uint64_t)id * span + j;
-            if (h->thresholded) { s += 16ull * (h->row_off[r + 1] - h->row_off[r]); b += row_size_from_store(h, r); continue; }
+            if (h->thresholded) { s += ibp_row_stored_T(h, r); b += row_size_from_store(h, r); continue; }
             const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? r / h->p.group_param : r % h->p.group_param;
             s += h->gtab[g].stride;
             b += (h->gtab[g].k_bits + 7) / 8;
@@ -683,6 +719,7 @@ extern "C" void ibp_destroy(ibp_handle* h) {
     if (h->gtab_dev) cudaFree(h->gtab_dev);
     if (h->mvtab_dev) cudaFree(h->mvtab_dev);
     if (h->row_off_dev) cudaFree(h->row_off_dev);
+    if (h->row_size_dev) cudaFree(h->row_size_dev);
     if (h->row_flag_dev) cudaFree(h->row_flag_dev);
     if (h->store) {
         if (h->store_kind == IBP_STORE_PINNED) cudaFreeHost(h->store);

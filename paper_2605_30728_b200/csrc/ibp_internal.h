@@ -39,6 +39,12 @@ struct ibp_handle {
     uint64_t n_rows_raw = 0;
     uint32_t* row_off_dev = nullptr;
     uint32_t* row_flag_dev = nullptr;
+    // slot layout (IBP_FLAG_SLOT_LAYOUT): row r at r * slot_bytes, its stored size in row_size[r] (16-byte units); no row_off
+    bool slot_layout = false;
+    uint32_t slot_bytes = 0;
+    uint64_t capacity_rows = 0;
+    std::vector<uint8_t> row_size;         // capacity_rows entries
+    uint8_t* row_size_dev = nullptr;
 
     // device copies
     int device = -1;
@@ -87,12 +93,18 @@ ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream);
 
 // byte offset of packed row `id` inside the store
 static inline uint64_t ibp_row_offset(const ibp_handle* h, uint64_t id) {
+    if (h->slot_layout) return id * (uint64_t)h->slot_bytes;
     if (h->thresholded) return 16ull * h->row_off[id];
     if (h->p.group_kind == IBP_GROUP_BLOCKED) {
         const uint64_t g = id / h->p.group_param;
         return h->gtab[g].base + (id - g * h->p.group_param) * (uint64_t)h->gtab[g].stride;
     }
     return (id / h->p.group_param) * h->row_stride_strided + h->gtab[id % h->p.group_param].base;
+}
+
+// thresholded mode: bytes row `id` occupies in the store incl. alignment padding (what a gather moves over the link)
+static inline uint64_t ibp_row_stored_T(const ibp_handle* h, uint64_t id) {
+    return h->slot_layout ? 16ull * h->row_size[id] : 16ull * (h->row_off[id + 1] - h->row_off[id]);
 }
 
 // group of a row id

@@ -237,3 +237,61 @@ def test_gnn_interleaved_variant_recipe_and_ratio():
     assert r_mixed < r_typed and r_mixed < 1.9
     mixed.destroy()
     typed.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# slot layout (PAPER.md:361 in-place storage) built by the host compressor
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,param,n,rb,align,cap", [(0, 1 << 20, 300, 64, 16, 400), (1, 6, 90, 32, 16, 0), (0, 16, 100, 256, 32, 112), (1, 4, 40, 516, 16, 64)])
+def test_slot_layout_host_build(kind, param, n, rb, align, cap):
+    """IBP_FLAG_SLOT_LAYOUT: row r lies at r * roundup(row_bytes, A); its first `size` bytes are the oracle's stored bytes of
+    that row, the rest of the slot and every unused slot are zero; one size byte per slot, no offsets."""
+    X = (datagen.random_bytes(n * rb, 400 + rb).reshape(n, rb) & datagen.random_bytes(rb, 401)[None, :]) | 0x08
+    X[::7, 1] ^= 0x33
+    X[5] = datagen.random_bytes(rb, 402)
+    gp = min(param, max(cap, n)) if kind == 0 and param >= (1 << 20) else param
+    h = ibp.ibp_build(X, rb, kind, gp, align_bytes=align, threshold=(4, 5), capacity_rows=cap,
+                      flags=ibp.IBP_FLAG_PAGEABLE_STORE | ibp.IBP_FLAG_SLOT_LAYOUT)
+    ds = oracle.DatasetT(X, kind, gp, 4, 5)
+    info = h.info()
+    slot = -(-rb // align) * align
+    capacity = cap or n
+    assert info.slot_bytes == slot and info.capacity_rows == capacity and info.rowsize_bytes == capacity and info.rowoffset_bytes == 0
+    assert info.packed_bytes_stored >= capacity * slot and info.packed_bytes_bytealigned == ds.stored_bytes
+    assert info.n_rows_raw == ds.n_raw
+    base = h.row_ptr(0)
+    img = ds.slot_image(capacity, slot)
+    ptr, nb = h.packed_range(0, n)
+    assert ptr == base and nb == n * slot
+    got = h.packed_view(base, capacity * slot).reshape(capacity, slot)
+    assert np.array_equal(got, img)                                             # every slot byte, used or not
+    for r in (0, 5, n - 1):
+        data, stored, comp = h.row_info(r)
+        want, want_comp = ds.row(r)
+        assert comp == want_comp and np.array_equal(data, want)
+        assert stored == -(-want.size // align) * align and h.row_ptr(r) == base + r * slot
+    h.destroy()
+    ds.close()
+
+
+def test_slot_layout_argument_checks():
+    X = datagen.random_bytes(64 * 32, 1).reshape(64, 32)
+    with pytest.raises(ibp.IbpError) as e:                                      # strict rows of a group all have one size: no slots
+        ibp.ibp_build(X, 32, 0, 16, flags=ibp.IBP_FLAG_PAGEABLE_STORE | ibp.IBP_FLAG_SLOT_LAYOUT)
+    assert e.value.status == 1
+    with pytest.raises(ibp.IbpError) as e:
+        ibp.ibp_build(X, 32, 0, 16, threshold=(4, 5), capacity_rows=10, flags=ibp.IBP_FLAG_PAGEABLE_STORE | ibp.IBP_FLAG_SLOT_LAYOUT)
+    assert e.value.status == 1
+    # the parameter struct of version 0.3 (no capacity_rows) is still accepted
+    import ctypes as C
+    p = ibp.ibp_build_params(C.sizeof(ibp.ibp_build_params) - 8, 32, 64, 0, 16, 1, 1, 16, 1, ibp.IBP_FLAG_PAGEABLE_STORE, 0, 0)
+    hp = C.c_void_p()
+    assert ibp.lib().ibp_build(X.ctypes.data, C.byref(p), C.byref(hp)) == 0
+    h = ibp.Handle(hp)
+    assert h.info().n_rows == 64
+    h.destroy()
+    h = ibp.ibp_build(X, 32, 0, 1 << 20, threshold=(4, 5), capacity_rows=100, flags=ibp.IBP_FLAG_PAGEABLE_STORE | ibp.IBP_FLAG_SLOT_LAYOUT)
+    with pytest.raises(ibp.IbpError) as e:                                      # append needs the GPU (no CPU fallback)
+        h.append_rows_device(X.ctypes.data, 4)
+    assert e.value.status == 4
+    h.destroy()
