@@ -270,15 +270,31 @@ def measure_gather(ctx, w, K, W, full, X=None, store="managed", keep=False):
     (value), the e2e entry point, the uncompressed baseline.  `full` adds the resident decode, all baseline variants and the
     random-span ceiling.  Returns (entry dict, extras dict)."""
     torch, ibp, oracle, args = ctx.torch, ctx.ibp, ctx.oracle, ctx.args
+    align = args.align if args.align else w.align_bytes
+    thr = parse_threshold(args.threshold)
+    shared = ctx.world > 1
     t0 = time.perf_counter()
-    if X is None:
+    if X is None and (not shared or ctx.rank == 0):
         X = w.table()
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
-    align = args.align if args.align else w.align_bytes
-    thr = parse_threshold(args.threshold)
-    h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
-                      flags=ibp.IBP_FLAG_HOSTALLOC_STORE if store == "pinned" else 0, threshold=thr)
+    if not shared:
+        h = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
+                          flags=ibp.IBP_FLAG_HOSTALLOC_STORE if store == "pinned" else 0, threshold=thr)
+    else:
+        # N > 1: ONE store in host memory for all ranks (SURVEY 8(e)): rank 0 builds and exports it into a shared-memory segment
+        # (pages interleaved over the NUMA nodes), every rank opens that segment and maps it for its own GPU
+        name = f"/ibp_bench_{os.environ.get('MASTER_PORT', '0')}_{w.name}"
+        if ctx.rank == 0:
+            h0 = ibp.ibp_build(X, w.row_bytes, w.group_kind, w.group_param, align_bytes=align, index_span=w.index_span,
+                               flags=ibp.IBP_FLAG_PAGEABLE_STORE, threshold=thr)
+            h0.export_shared(name, numa_policy=1)
+            h0.destroy()
+        ctx.barrier()
+        h = ibp.ibp_open_shared(name)
+        ctx.barrier()
+        if ctx.rank == 0:
+            ibp.ibp_unlink_shared(name)
     t_build = time.perf_counter() - t0
     h.upload_metadata(ctx.local)
     if args.order is not None:
@@ -330,9 +346,11 @@ def measure_gather(ctx, w, K, W, full, X=None, store="managed", keep=False):
     # parity of one warm-up batch against the plain definition (oracle c1), so that a fast wrong kernel cannot score
     chk = np.random.default_rng(0).choice(n_rows_out, size=min(4096, n_rows_out), replace=False)
     got = out[torch.from_numpy(chk).cuda()].cpu().numpy()
-    want = oracle.gather_plain(X, batches[W - 1], w.index_span)[chk]
-    if not np.array_equal(got, want):
-        raise SystemExit(f"bench.py: GPU output differs from the oracle on {w.name}; refusing to report a number")
+    want = None
+    if X is not None:                                           # N > 1: rank 0 holds the table (the others read the shared store only)
+        want = oracle.gather_plain(X, batches[W - 1], w.index_span)[chk]
+        if not np.array_equal(got, want):
+            raise SystemExit(f"bench.py: GPU output differs from the oracle on {w.name}; refusing to report a number")
 
     clocks = ClockSampler(ctx.local)
     ctx.barrier()
@@ -378,7 +396,7 @@ def measure_gather(ctx, w, K, W, full, X=None, store="managed", keep=False):
 
     for i in range(min(W, 3)):
         step_e2e(i)
-    if not np.array_equal(out_pin_np[chk], oracle.gather_plain(X, batches[min(W, 3) - 1], w.index_span)[chk]):
+    if X is not None and not np.array_equal(out_pin_np[chk], oracle.gather_plain(X, batches[min(W, 3) - 1], w.index_span)[chk]):
         raise SystemExit(f"bench.py: end-to-end output differs from the oracle on {w.name}")
     ctx.barrier()
     Ke = max(3, min(K, 30 if full else 10))
@@ -565,7 +583,8 @@ def run_cuda(args):
                                                       "hit_rate": round(ex["hit_rate"], 4), "equivalent_uncompressed_cache_rows": int(cinfo.capacity_bytes // w.row_bytes)},
                 "ratio_stored": entry["ratio_stored"], "ratio_bytealigned": entry["ratio_bytealigned"],
                 "packed_store_GB": entry["packed_store_GB"], "metadata_MB": entry["metadata_MB"], "build_s": entry["build_s"], "datagen_s": entry["datagen_s"],
-                "n_rows_raw": int(info.n_rows_raw), "sharding": "ids sharded over ranks, no collective" if world > 1 else "single GPU",
+                "n_rows_raw": int(info.n_rows_raw),
+                "sharding": "ids sharded over ranks, no collective; ONE store in host memory (POSIX shared memory, pages interleaved over the NUMA nodes) read by every rank's GPU over its own PCIe link" if world > 1 else "single GPU",
             },
             "roofline": {
                 "bound": "pcie", "achieved": round(achieved, 3), "peak": round(ctx.h2d, 3), "unit": "GB/s", "frac": round(achieved / ctx.h2d, 4),

@@ -83,8 +83,11 @@ enum {
 typedef enum {
     IBP_STORE_PAGEABLE = 0,     /* ordinary host memory; the GPU cannot read it in place                              */
     IBP_STORE_PINNED = 1,       /* cudaHostAlloc(mapped|portable): page-locked, 4 KB GPU pages                        */
-    IBP_STORE_MANAGED_HOST = 2  /* cudaMallocManaged, preferred location CPU, accessed-by GPU: host-resident, read in
+    IBP_STORE_MANAGED_HOST = 2, /* cudaMallocManaged, preferred location CPU, accessed-by GPU: host-resident, read in
                                    place over PCIe, mapped by the GPU with large pages        */
+    IBP_STORE_SHARED = 3        /* a POSIX shared-memory segment (ibp_export_shared / ibp_open_shared), page-locked and
+                                   GPU-mapped by every process that uploads it: ONE copy of the store in host RAM for all
+                                   the ranks of a one-process-per-GPU job                                            */
 } ibp_store_kind;
 
 typedef struct {
@@ -310,6 +313,25 @@ ibp_status ibp_cache_lookup(ibp_cache* c, const int64_t* row_ids_dev, int64_t n,
 ibp_status ibp_cache_read(const ibp_cache* c, uint64_t entry, uint32_t nbytes, void* out_host);
 ibp_status ibp_cache_get_info(const ibp_cache* c, ibp_cache_info* out);
 void ibp_cache_destroy(ibp_cache* c);
+
+/* -- One store for all ranks of a one-process-per-GPU job ("each GPU reads the shared pinned store over its own
+ * PCIe link").  ibp_export_shared writes a complete image of a built handle -- parameters, Mask/Bitval, group table, row
+ * offsets / sizes / flags, the packed store -- into the POSIX shared-memory segment `shm_name` (created; an existing one is
+ * replaced).  numa_policy places the segment's pages before they are first touched: 0 = the kernel's default (first touch:
+ * the exporting thread's node), 1 = interleaved over all NUMA nodes (ranks on both sockets see the same average distance),
+ * 2 + k = bound to NUMA node k (e.g. the node of the GPU that reads it; ibp_device_numa_node).  Placement is best effort: on a
+ * machine without NUMA support the call still succeeds.  ibp_open_shared maps the segment in another (or the same) process and
+ * returns a handle that BORROWS everything from it: no per-process copy of the store or of the host metadata mirrors.
+ * ibp_upload_metadata on such a handle page-locks and GPU-maps the store for this process (cudaHostRegister) and replicates the
+ * metadata on its device, after which every gather / decode entry point works as on the original.  The handle is read-only
+ * (ibp_append_rows_device: BAD_STATE).  ibp_destroy unmaps; ibp_unlink_shared removes the name (the memory lives on until the
+ * last process unmaps it).  Errors: INVALID_ARG (names, a segment that is not an IBP image or not complete), OUT_OF_MEMORY
+ * (shm_open / ftruncate / mmap failed), CUDA (registration).                                                          */
+ibp_status ibp_export_shared(const ibp_handle* h, const char* shm_name, int numa_policy);
+ibp_status ibp_open_shared(const char* shm_name, ibp_handle** out_handle);
+ibp_status ibp_unlink_shared(const char* shm_name);
+/* NUMA node of a CUDA device's PCIe slot (sysfs), -1 if unknown.                                                       */
+ibp_status ibp_device_numa_node(int device, int* node);
 
 void ibp_destroy(ibp_handle* h);
 const char* ibp_last_error(void);

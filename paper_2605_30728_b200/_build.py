@@ -55,7 +55,7 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
     if force or _stale(LIB, deps):
         tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")       # per process: concurrent builds (torchrun ranks, test workers) do not collide
         _run([nvcc_path(), *NVCC_FLAGS, *extra_flags, "-I", ROOT / "include", "-I", PKG / "csrc", "-x", "cu", *src,
-              "-o", tmp, "-lgomp"], verbose)
+              "-o", tmp, "-lgomp", "-lrt"], verbose)
         os.replace(tmp, LIB)
     return LIB
 

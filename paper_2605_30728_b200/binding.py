@@ -20,7 +20,7 @@ IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED, IBP_GROUP_MAP = 0, 1, 2
 IBP_FLAG_PAGEABLE_STORE = 1
 IBP_FLAG_HOSTALLOC_STORE = 2
 IBP_FLAG_SLOT_LAYOUT = 4
-IBP_STORE_PAGEABLE, IBP_STORE_PINNED, IBP_STORE_MANAGED_HOST = 0, 1, 2
+IBP_STORE_PAGEABLE, IBP_STORE_PINNED, IBP_STORE_MANAGED_HOST, IBP_STORE_SHARED = 0, 1, 2, 3
 
 
 class IbpError(RuntimeError):
@@ -100,6 +100,10 @@ SIGNATURES = {
     "ibp_cache_read": (_int, [_vp, _u64, _u32, _vp]),
     "ibp_cache_get_info": (_int, [_vp, C.POINTER(ibp_cache_info)]),
     "ibp_cache_destroy": (None, [_vp]),
+    "ibp_export_shared": (_int, [_vp, C.c_char_p, _int]),
+    "ibp_open_shared": (_int, [C.c_char_p, C.POINTER(_vp)]),
+    "ibp_unlink_shared": (_int, [C.c_char_p]),
+    "ibp_device_numa_node": (_int, [_int, C.POINTER(_int)]),
     "ibp_destroy": (None, [_vp]),
     "ibp_last_error": (C.c_char_p, []),
     "ibp_version": (C.c_char_p, []),
@@ -271,6 +275,10 @@ class Handle:
         _check(lib().ibp_batch_link_bytes(self._h, ids.ctypes.data, ids.size, C.byref(nu), C.byref(st), C.byref(ba)))
         return nu.value, st.value, ba.value
 
+    def export_shared(self, shm_name: str, numa_policy: int = 0):
+        _check(lib().ibp_export_shared(self._h, shm_name.encode(), numa_policy))
+        return self
+
     def destroy(self):
         if self._h:
             lib().ibp_destroy(self._h)
@@ -281,6 +289,22 @@ class Handle:
             self.destroy()
         except Exception:
             pass
+
+
+def ibp_open_shared(shm_name: str) -> Handle:
+    h = _vp()
+    _check(lib().ibp_open_shared(shm_name.encode(), C.byref(h)))
+    return Handle(h)
+
+
+def ibp_unlink_shared(shm_name: str):
+    _check(lib().ibp_unlink_shared(shm_name.encode()))
+
+
+def ibp_device_numa_node(device: int = 0) -> int:
+    n = _int(-1)
+    _check(lib().ibp_device_numa_node(device, C.byref(n)))
+    return n.value
 
 
 class Cache:

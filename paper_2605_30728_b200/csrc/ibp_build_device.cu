@@ -1064,6 +1064,7 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
 extern "C" ibp_status ibp_append_rows_device(ibp_handle* h, const void* rows_dev, int64_t n_new, void* cuda_stream) {
     if (!h) { ibp_set_error("ibp_append_rows_device: null handle"); return IBP_ERR_INVALID_ARG; }
     if (!h->slot_layout) { ibp_set_error("ibp_append_rows_device: the handle was not built with IBP_FLAG_SLOT_LAYOUT (a dense store cannot grow in place)"); return IBP_ERR_BAD_STATE; }
+    if (h->store_kind == IBP_STORE_SHARED) { ibp_set_error("ibp_append_rows_device: a shared store (ibp_open_shared) is read-only"); return IBP_ERR_BAD_STATE; }
     if (h->device < 0 || !h->meta_dev || !h->store_dev) { ibp_set_error("ibp_append_rows_device: call ibp_upload_metadata first (GPU-visible store)"); return IBP_ERR_BAD_STATE; }
     if (n_new == 0) return IBP_OK;
     if (n_new < 0 || !rows_dev || ((uintptr_t)rows_dev & 15u)) { ibp_set_error("ibp_append_rows_device: bad argument (n_new < 0, null or unaligned rows_dev)"); return IBP_ERR_INVALID_ARG; }

@@ -948,6 +948,16 @@ ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream) {
         IBP_CUDA(cudaHostGetDevicePointer(&dptr, h->store, 0));
         h->store_dev = (uint8_t*)dptr;
     }
+    if (h->store_kind == IBP_STORE_SHARED && !h->store_dev) {
+        // the shared segment: page-lock and map it for THIS process; every rank does the same with the same physical pages
+        if (!h->shm_registered) {
+            IBP_CUDA(cudaHostRegister(h->store, h->store_bytes, cudaHostRegisterMapped | cudaHostRegisterPortable));
+            h->shm_registered = true;
+        }
+        void* dptr = nullptr;
+        IBP_CUDA(cudaHostGetDevicePointer(&dptr, h->store, 0));
+        h->store_dev = (uint8_t*)dptr;
+    }
     if (h->store_kind == IBP_STORE_MANAGED_HOST) {
         // direct mapping of the host-resident pages into this GPU's page tables: accesses go over PCIe, nothing migrates
         IBP_CUDA(cudaMemAdvise(h->store, h->store_bytes, cudaMemAdviseSetAccessedBy, device));

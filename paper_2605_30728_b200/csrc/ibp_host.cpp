@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include <immintrin.h>
 #include <omp.h>
+#include <sys/mman.h>
 
 #include <algorithm>
 #include <cstdarg>
@@ -721,6 +722,11 @@ extern "C" void ibp_destroy(ibp_handle* h) {
     if (h->row_off_dev) cudaFree(h->row_off_dev);
     if (h->row_size_dev) cudaFree(h->row_size_dev);
     if (h->row_flag_dev) cudaFree(h->row_flag_dev);
+    if (h->store_kind == IBP_STORE_SHARED) {
+        if (h->shm_registered) cudaHostUnregister(h->store);
+        if (h->shm_base) munmap(h->shm_base, h->shm_bytes);
+        h->store = nullptr;
+    }
     if (h->store) {
         if (h->store_kind == IBP_STORE_PINNED) cudaFreeHost(h->store);
         else if (h->store_kind == IBP_STORE_MANAGED_HOST) cudaFree(h->store);

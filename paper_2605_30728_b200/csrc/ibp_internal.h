@@ -6,6 +6,26 @@
 
 #include "ibp.h"
 
+// Host array that either owns its elements or borrows them from a mapping (a shared store segment, ibp_shared.cpp): the host
+// mirrors of the metadata need not be copied into every process that opens the same store.
+template <typename T>
+struct HostArray {
+    std::vector<T> own;
+    T* ptr = nullptr;
+    size_t n = 0;
+    void assign(size_t count, const T& v) { own.assign(count, v); ptr = own.data(); n = count; }
+    void resize(size_t count, const T& v = T()) {
+        if (ptr != own.data() && n) own.assign(ptr, ptr + n);     // was borrowed: take a private copy first
+        own.resize(count, v); ptr = own.data(); n = count;
+    }
+    void borrow(T* p, size_t count) { std::vector<T>().swap(own); ptr = p; n = count; }
+    T* data() { return ptr; }
+    const T* data() const { return ptr; }
+    size_t size() const { return n; }
+    T& operator[](size_t i) { return ptr[i]; }
+    const T& operator[](size_t i) const { return ptr[i]; }
+};
+
 // One entry per group, 16 bytes, mirrored in HBM.
 //   blocked: packed row j of the group lies at store + base + j*stride
 //   strided: tile t of matrix row r lies at store + r*row_stride_strided + base   (base = prefix_t)
@@ -23,19 +43,23 @@ struct ibp_handle {
     uint32_t max_stride = 0;
 
     // host copies
-    std::vector<uint32_t> meta;            // per group: Mask words then Bitval words (2*n_words)
-    std::vector<IbpGroupEntry> gtab;
+    HostArray<uint32_t> meta;              // per group: Mask words then Bitval words (2*n_words)
+    HostArray<IbpGroupEntry> gtab;
     uint8_t* store = nullptr;              // packed store (pinned+mapped, or malloc)
     uint8_t* store_dev = nullptr;          // device-visible address of the store (nullptr if pageable)
     uint64_t store_bytes = 0;              // incl. slack
     uint64_t store_used = 0;
     int store_kind = IBP_STORE_PAGEABLE;   // ibp_store_kind
+    // IBP_STORE_SHARED: the store and the host mirrors live in a POSIX shared-memory segment opened by ibp_open_shared
+    void* shm_base = nullptr;
+    uint64_t shm_bytes = 0;
+    bool shm_registered = false;           // cudaHostRegister'ed by this process (ibp_attach_device)
     uint64_t packed_bytes_rows = 0, packed_bytes_bytealigned = 0;
 
     // thresholded mode (tau < 1): data-dependent row sizes
     bool thresholded = false;
-    std::vector<uint32_t> row_off;         // n_rows + 1 offsets into the store, in 16-byte units
-    std::vector<uint32_t> row_flag;        // bit r (word r/32, bit r%32) = 1 iff row r is compressed
+    HostArray<uint32_t> row_off;           // n_rows + 1 offsets into the store, in 16-byte units
+    HostArray<uint32_t> row_flag;          // bit r (word r/32, bit r%32) = 1 iff row r is compressed
     uint64_t n_rows_raw = 0;
     uint32_t* row_off_dev = nullptr;
     uint32_t* row_flag_dev = nullptr;
@@ -43,7 +67,7 @@ struct ibp_handle {
     bool slot_layout = false;
     uint32_t slot_bytes = 0;
     uint64_t capacity_rows = 0;
-    std::vector<uint8_t> row_size;         // capacity_rows entries
+    HostArray<uint8_t> row_size;           // capacity_rows entries
     uint8_t* row_size_dev = nullptr;
 
     // device copies

@@ -515,6 +515,33 @@ def test_T_edge_cases_and_spans():
     hk.destroy()
 
 
+@pytest.mark.parametrize("thr,flags,cap", [((1, 1), 0, 0), ((4, 5), 0, 0), ((4, 5), ibp.IBP_FLAG_SLOT_LAYOUT, 0)])
+def test_shared_store_gather(thr, flags, cap):
+    """One store for all ranks: a handle exported into a POSIX shared-memory segment and opened again -- here twice
+    in one process, standing in for two ranks -- is page-locked and GPU-mapped by ibp_upload_metadata and decodes the same bytes
+    as the original: random gather, range, resident."""
+    import os
+    name = f"/ibp_gputest_{os.getpid()}"
+    w = workloads.GNN(n_rows=30_000, batch=4000)
+    X = _u8(w.table())
+    h0 = ibp.ibp_build(X, 512, 0, 256, align_bytes=32 if not flags else 16, threshold=thr, flags=flags | ibp.IBP_FLAG_PAGEABLE_STORE, capacity_rows=cap)
+    h0.export_shared(name, numa_policy=1)
+    h0.destroy()                                                            # only the segment is left
+    ha = ibp.ibp_open_shared(name).upload_metadata(0)
+    hb = ibp.ibp_open_shared(name).upload_metadata(0)
+    ibp.ibp_unlink_shared(name)                                             # the mappings keep the memory alive
+    assert ha.info().store_kind == ibp.IBP_STORE_SHARED and ha.info().device == 0
+    ids = w.ids(0)
+    for h in (ha, hb):
+        assert np.array_equal(_gather(h, ids), X[ids])
+        assert np.array_equal(_range(h, 256 * 3, 5000), X[768:5768])
+        assert np.array_equal(_resident(h, 0, 2048), X[:2048])
+    ha.destroy()
+    assert np.array_equal(_gather(hb, ids[:100]), X[ids[:100]])             # one rank leaving does not disturb the other
+    hb.destroy()
+    assert ibp.ibp_device_numa_node(0) >= -1
+
+
 def test_link_probes():
     """The ceilings bench.py reports are measured by the library itself: sane values and argument checks."""
     sps, gbs = ibp.ibp_measure_random_read(0, 64 << 20, 128, 1)
