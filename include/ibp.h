@@ -303,8 +303,38 @@ ibp_status ibp_cache_create(ibp_handle* h, uint64_t capacity_bytes, uint32_t n_s
  * anything changes: INVALID_ARG for an id out of range, OUT_OF_MEMORY and CUDA errors leave the cache exactly as it was.
  * An insert may run while gathers on other streams use the cache: the slab bytes are written first and a map slot {key, value}
  * is published with one 16-byte compare-and-swap, so a concurrent gather sees a row either as cached or as not cached (then
- * it reads the host store) -- the output is the same.  Two inserts on one cache must not overlap.                        */
+ * it reads the host store) -- the output is the same.  Two inserts on one cache must not overlap.  Only slabs this cache
+ * allocated are filled (a peer process's slab is filled by its owner: ibp_cache_insert_slab below).                        */
 ibp_status ibp_cache_insert(ibp_cache* c, const int64_t* row_ids_host, int64_t n, void* cuda_stream, int64_t* n_inserted_host);
+
+/* -- Slabs on several GPUs ("we allocate a contiguous memory region per interconnected GPU, which we call a data slab; e.g.,
+ * an 8-GPU system would have 8 separate data slabs.  Together, these slabs make up the data store"; "using the data slab ID,
+ * we identify which GPU slab the required tensor is on").  The slab id of a map value names the GPU whose memory holds the row; the
+ * decode kernel of the handle's device reads a hit from that slab -- its own HBM, or a peer GPU's memory over NVLink -- with the same
+ * bulk copy, so S2-S6 and the output do not change.
+ *
+ * One process driving several GPUs: ibp_cache_create_multi is ibp_cache_create with slab s allocated on CUDA device
+ * slab_devices[s] (-1 = the handle's device); peer access from the handle's device is enabled (UNSUPPORTED when the two devices
+ * cannot reach each other, INVALID_ARG for a device this process does not have).  ibp_cache_insert then fills the slabs in order,
+ * writing peer slabs over the interconnect.
+ *
+ * One process per GPU (the layout of this library's multi-GPU runs): every rank creates its cache with its own slab
+ * local and the others marked IBP_SLAB_REMOTE, publishes its slab with ibp_cache_slab_export (a CUDA IPC memory handle,
+ * IBP_IPC_HANDLE_BYTES bytes, sent to the peers by any host channel), and maps the peers' slabs with ibp_cache_slab_attach.  Rows
+ * are then placed slab by slab with ibp_cache_insert_slab: EVERY rank calls it for EVERY slab with the same id list -- the placement
+ * (offsets in insertion order, 16-byte covers) is a function of the list alone, so all ranks build identical map entries -- and
+ * passes fill = 1 only for the slab it owns (it copies the packed rows from the host store into it); fill = 0 adds the entries
+ * without touching the slab.  After all ranks have returned (the call synchronises the stream; the ranks then meet at a host
+ * barrier) every rank's gathers hit any slab.  Errors: BAD_STATE (exporting a slab this cache did not allocate, attaching over a
+ * slab that has memory, inserting into a slab with no memory, fill = 1 on a peer's slab), INVALID_ARG, CUDA.                   */
+#define IBP_SLAB_REMOTE (-2)
+#define IBP_IPC_HANDLE_BYTES 64
+ibp_status ibp_cache_create_multi(ibp_handle* h, uint64_t capacity_bytes, uint32_t n_slabs, const int32_t* slab_devices,
+                                  uint64_t max_entries, void* cuda_stream, ibp_cache** out_cache);
+ibp_status ibp_cache_slab_export(const ibp_cache* c, uint32_t slab, void* ipc_handle_out);
+ibp_status ibp_cache_slab_attach(ibp_cache* c, uint32_t slab, const void* ipc_handle);
+ibp_status ibp_cache_insert_slab(ibp_cache* c, uint32_t slab, const int64_t* row_ids_host, int64_t n, int fill, void* cuda_stream,
+                                 int64_t* n_inserted_host);
 /* S1-S6 with the cache in front of the host store (see above).  Arguments as ibp_gather_decompress.                    */
 ibp_status ibp_cache_gather_decompress(ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);
 /* entries_dev[i] = the map value of row_ids_dev[i], or IBP_CACHE_MISS.  For tests and hit-rate accounting.  Asynchronous. */

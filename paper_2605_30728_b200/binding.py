@@ -69,6 +69,8 @@ class ibp_table_desc(C.Structure):
 
 
 IBP_CACHE_MISS = 0xFFFFFFFFFFFFFFFF
+IBP_SLAB_REMOTE = -2
+IBP_IPC_HANDLE_BYTES = 64
 
 # name -> (restype, argtypes); every symbol include/ibp.h declares (tests/test_abi.py checks the two lists agree)
 _vp, _i64, _u64, _u32, _int = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int
@@ -95,6 +97,10 @@ SIGNATURES = {
     "ibp_batch_link_bytes": (_int, [_vp, _vp, _i64, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]),
     "ibp_cache_create": (_int, [_vp, _u64, _u32, _u64, _vp, C.POINTER(_vp)]),
     "ibp_cache_insert": (_int, [_vp, _vp, _i64, _vp, C.POINTER(_i64)]),
+    "ibp_cache_create_multi": (_int, [_vp, _u64, _u32, _vp, _u64, _vp, C.POINTER(_vp)]),
+    "ibp_cache_slab_export": (_int, [_vp, _u32, _vp]),
+    "ibp_cache_slab_attach": (_int, [_vp, _u32, _vp]),
+    "ibp_cache_insert_slab": (_int, [_vp, _u32, _vp, _i64, _int, _vp, C.POINTER(_i64)]),
     "ibp_cache_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_cache_lookup": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_cache_read": (_int, [_vp, _u64, _u32, _vp]),
@@ -310,10 +316,31 @@ def ibp_device_numa_node(device: int = 0) -> int:
 class Cache:
     """Owns an ibp_cache* (compressed GPU software cache).  Keeps its Handle alive."""
 
-    def __init__(self, handle: Handle, capacity_bytes: int, n_slabs: int = 1, max_entries: int = 0, stream=None):
+    def __init__(self, handle: Handle, capacity_bytes: int, n_slabs: int = 1, max_entries: int = 0, stream=None, slab_devices=None):
+        """slab_devices (ibp_cache_create_multi): per slab a CUDA device, -1 = the handle's, IBP_SLAB_REMOTE = a peer process's."""
         c = _vp()
-        _check(lib().ibp_cache_create(handle._h, capacity_bytes, n_slabs, max_entries, stream, C.byref(c)))
+        if slab_devices is None:
+            _check(lib().ibp_cache_create(handle._h, capacity_bytes, n_slabs, max_entries, stream, C.byref(c)))
+        else:
+            devs = np.ascontiguousarray(slab_devices, dtype=np.int32)
+            assert devs.size == n_slabs
+            _check(lib().ibp_cache_create_multi(handle._h, capacity_bytes, n_slabs, devs.ctypes.data, max_entries, stream, C.byref(c)))
         self._c, self.handle = c, handle
+
+    def slab_export(self, slab: int) -> bytes:
+        buf = C.create_string_buffer(IBP_IPC_HANDLE_BYTES)
+        _check(lib().ibp_cache_slab_export(self._c, slab, buf))
+        return buf.raw
+
+    def slab_attach(self, slab: int, ipc_handle: bytes):
+        assert len(ipc_handle) == IBP_IPC_HANDLE_BYTES
+        _check(lib().ibp_cache_slab_attach(self._c, slab, C.create_string_buffer(ipc_handle, IBP_IPC_HANDLE_BYTES)))
+
+    def insert_slab(self, slab: int, row_ids_host, fill: bool, stream=None) -> int:
+        ids = np.ascontiguousarray(row_ids_host, dtype=np.int64)
+        k = _i64()
+        _check(lib().ibp_cache_insert_slab(self._c, slab, ids.ctypes.data, ids.size, 1 if fill else 0, stream, C.byref(k)))
+        return k.value
 
     def insert(self, row_ids_host, stream=None) -> int:
         ids = np.ascontiguousarray(row_ids_host, dtype=np.int64)

@@ -99,6 +99,9 @@ struct ibp_cache {
     uint64_t slab_bytes = 0;
     uint8_t* slab_dev[8] = {};
     uint64_t slab_used[8] = {};
+    int slab_device[8] = {-1, -1, -1, -1, -1, -1, -1, -1};   // CUDA device whose memory holds the slab; -1: none yet (a peer process's slab, not attached)
+    bool slab_owned[8] = {};               // allocated by this cache (it fills it and frees it); false: a peer process's slab or nothing
+    bool slab_imported[8] = {};            // opened from a CUDA IPC handle (ibp_cache_slab_attach)
     uint64_t* map_dev = nullptr;           // map_cap slots of {key = id + 1 (0 = empty), value}
     uint32_t map_cap = 0;                  // power of two
     uint64_t n_entries = 0, max_entries = 0;

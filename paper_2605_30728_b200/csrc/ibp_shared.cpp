@@ -125,11 +125,12 @@ extern "C" ibp_status ibp_export_shared(const ibp_handle* h, const char* shm_nam
     if (base == MAP_FAILED) { ibp_set_error("ibp_export_shared: mmap failed: %s", strerror(errno)); shm_unlink(shm_name); return IBP_ERR_OUT_OF_MEMORY; }
     place_pages(base, H.total_bytes, numa_policy);           // before the first touch
     uint8_t* b = (uint8_t*)base;
-    memcpy(b + H.off_meta, h->meta.data(), H.n_meta * 4);
-    memcpy(b + H.off_gtab, h->gtab.data(), H.n_gtab * sizeof(IbpGroupEntry));
-    memcpy(b + H.off_row_off, h->row_off.data(), H.n_row_off * 4);
-    memcpy(b + H.off_row_flag, h->row_flag.data(), H.n_row_flag * 4);
-    memcpy(b + H.off_row_size, h->row_size.data(), H.n_row_size);
+    auto put = [&](uint64_t off, const void* src, uint64_t nbytes) { if (nbytes) memcpy(b + off, src, nbytes); };   // an empty vector's data() may be null
+    put(H.off_meta, h->meta.data(), H.n_meta * 4);
+    put(H.off_gtab, h->gtab.data(), H.n_gtab * sizeof(IbpGroupEntry));
+    put(H.off_row_off, h->row_off.data(), H.n_row_off * 4);
+    put(H.off_row_flag, h->row_flag.data(), H.n_row_flag * 4);
+    put(H.off_row_size, h->row_size.data(), H.n_row_size);
     {
         const int64_t nchunk = (int64_t)((h->store_bytes + (1u << 22) - 1) >> 22);
 #pragma omp parallel for schedule(static)

@@ -177,3 +177,118 @@ def test_argument_errors():
         ibp.Cache(h, 1024)
     assert e.value.status == 5
     h.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# slabs on several GPUs (one data slab per interconnected GPU, the slab id of a map value names the GPU)
+# ---------------------------------------------------------------------------------------------------------------------
+def test_create_multi_on_this_process_devices():
+    """ibp_cache_create_multi: slabs placed device by device.  One GPU here, so every slab names device 0 (explicitly or as -1):
+    the layout, the map values and the output must equal ibp_cache_create's; a device this process does not have is refused."""
+    w = workloads.Tiny()
+    X = w.table()
+    h = ibp.ibp_build(X, 512, 0, 64, align_bytes=32).upload_metadata(0)
+    info = h.info()
+    hot = np.random.default_rng(11).permutation(w.n_rows)[:1500].astype(np.int64)
+    ref = ibp.Cache(h, info.packed_bytes_stored // 2, 3)
+    multi = ibp.Cache(h, info.packed_bytes_stored // 2, 3, slab_devices=[0, -1, 0])
+    assert ref.insert(hot) == multi.insert(hot) > 0
+    assert np.array_equal(_lookup(ref, hot), _lookup(multi, hot))          # same placement -> same 64-bit values (P:353)
+    ids = np.random.default_rng(12).integers(0, w.n_rows, 2000)
+    assert np.array_equal(_cache_gather(multi, ids, 512), oracle.gather_plain(X, ids))
+    n_dev = torch.cuda.device_count()
+    with pytest.raises(ibp.IbpError):
+        ibp.Cache(h, 1 << 20, 2, slab_devices=[0, n_dev])                   # no such device
+    with pytest.raises(ibp.IbpError):
+        ibp.Cache(h, 1 << 20, 2, slab_devices=[0, -3])
+    if n_dev > 1:                                                           # a real peer slab when the box has a second GPU
+        peer = ibp.Cache(h, info.packed_bytes_stored // 2, 2, slab_devices=[0, 1])
+        assert peer.insert(hot) > 0
+        assert np.array_equal(_cache_gather(peer, ids, 512), oracle.gather_plain(X, ids))
+        peer.destroy()
+    # a remote slab that was never attached holds nothing: inserts skip it, exporting it or inserting into it is a state error
+    part = ibp.Cache(h, info.packed_bytes_stored // 2, 2, slab_devices=[-1, ibp.IBP_SLAB_REMOTE])
+    k = part.insert(hot)
+    ent = _lookup(part, hot[:k])
+    assert k > 0 and all(oracle.cache_value_fields(int(e))[0] == 0 for e in ent)
+    with pytest.raises(ibp.IbpError):
+        part.slab_export(1)
+    with pytest.raises(ibp.IbpError):
+        part.insert_slab(1, hot[:4], False)
+    with pytest.raises(ibp.IbpError):
+        part.slab_attach(0, b"\0" * ibp.IBP_IPC_HANDLE_BYTES)               # slab 0 already has memory
+    assert np.array_equal(_cache_gather(part, ids, 512), oracle.gather_plain(X, ids))
+    for c in (ref, multi, part):
+        c.destroy()
+    h.destroy()
+
+
+def _peer_slab_worker(rank, world, port, thr, q):
+    """One process per GPU (both on device 0 here: the box has one): rank r owns slab r; the other slab is the peer's memory,
+    mapped through a CUDA IPC handle.  Every rank inserts every slab's id list; only the owner copies bytes."""
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        w = workloads.Tiny()
+        X = w.table()
+        h = ibp.ibp_build(X, 512, 0, 64, align_bytes=32, threshold=thr).upload_metadata(0)
+        ds = oracle.Dataset(X, 0, 64) if thr[0] == thr[1] else oracle.DatasetT(X, 0, 64, thr[0], thr[1])
+        info = h.info()
+        devs = [ibp.IBP_SLAB_REMOTE] * world
+        devs[rank] = -1
+        c = ibp.Cache(h, info.packed_bytes_stored // 2, world, slab_devices=devs)
+        handles = [None] * world
+        dist.all_gather_object(handles, c.slab_export(rank))
+        for s in range(world):
+            if s != rank:
+                c.slab_attach(s, handles[s])
+        hot = np.random.default_rng(21).permutation(w.n_rows)[:1600].astype(np.int64)
+        lists = [hot[s::world] for s in range(world)]                       # slab s caches every world-th hot row
+        counts = [c.insert_slab(s, lists[s], fill=(s == rank)) for s in range(world)]
+        dist.barrier()                                                      # every slab is filled by its owner before anyone reads it
+        ok = all(k == len(l) for k, l in zip(counts, lists))
+        # map values: slab id = the owner's rank, on every rank (P:353, P:357)
+        for s in range(world):
+            ent = _lookup(c, lists[s])
+            ok = ok and all(oracle.cache_value_fields(int(e))[0] == s and oracle.cache_value_fields(int(e))[3] == 0 for e in ent)
+            # the bytes behind a value, read from the OWNER's or the PEER's memory alike, are the oracle's packed row
+            for rid, e in list(zip(lists[s], ent))[:24]:
+                pr = ds.packed_row(int(rid)) if thr[0] == thr[1] else ds.row(int(rid))[0]
+                head = h.row_ptr(int(rid)) % 16                            # the slab stores the row's 16-byte cover
+                ok = ok and np.array_equal(c.read(int(e), head + len(pr))[head:], pr)
+        ids = np.random.default_rng(22 + rank).integers(0, w.n_rows, 3000)   # hits in both slabs and misses
+        ok = ok and np.array_equal(_cache_gather(c, ids, 512), oracle.gather_plain(X, ids))
+        ok = ok and np.array_equal(_cache_gather(c, ids, 512), ds.gather_decompress(ids))
+        dist.barrier()                                                      # nobody unmaps a slab a peer is still reading
+        c.destroy()
+        h.destroy()
+        ds.close()
+        q.put((rank, bool(ok)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("thr", [(1, 1), (4, 5)])
+def test_peer_slabs_two_processes_one_gpu(thr):
+    """P:351-357 in the one-process-per-GPU layout: two processes, each owning one slab, reading the other's through CUDA IPC."""
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_peer_slab_worker, args=(r, 2, port, thr, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=300) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1] and all(r[1] for r in res)
