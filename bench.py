@@ -1283,6 +1283,39 @@ def run_resident(args):
     print(json.dumps(line), flush=True)
 
 
+def run_probes(args):
+    """The link ceilings every roofline in this file is read against, and the levers that were tried on the random-row path
+    (DESIGN.md section 6): copy-engine H2D / D2H, SM-issued contiguous zero-copy reads, and random span reads over host memory of
+    every kind the library can map -- the span rate of a large footprint follows the GPU-side page size of the mapping."""
+    import torch
+    from paper_2605_30728_b200 import binding as ibp
+    torch.cuda.set_device(0)
+    fp = 6 << 30
+    kinds = [("managed host-resident (default store)", ibp.IBP_MEM_MANAGED_HOST), ("cudaHostAlloc", ibp.IBP_MEM_HOSTALLOC),
+             ("mmap 4 KB pages + cudaHostRegister", ibp.IBP_MEM_MALLOC_REGISTERED), ("mmap + MADV_HUGEPAGE + cudaHostRegister", ibp.IBP_MEM_THP_REGISTERED),
+             ("hugetlbfs 2 MB pages + cudaHostRegister", ibp.IBP_MEM_HUGETLB_2M_REGISTERED)]
+    table = []
+    for name, k in kinds:
+        row = {"memory": name}
+        for span in (128, 256):
+            try:
+                sps, gbs = ibp.ibp_measure_random_read_kind(0, fp, span, k, 3)
+                row[f"span_{span}B"] = {"M_spans_per_s": round(sps * 1e-6, 1), "GBps": round(gbs, 2)}
+            except ibp.IbpError as e:
+                row[f"span_{span}B"] = {"unavailable": str(e)[:160]}
+        table.append(row)
+    scan = []
+    for mb in (32, 256, 1024, 2048, 6144):
+        sps, gbs = ibp.ibp_measure_random_read_kind(0, mb << 20, 128, ibp.IBP_MEM_MANAGED_HOST, 3)
+        scan.append({"footprint_MiB": mb, "M_spans_per_s": round(sps * 1e-6, 1), "GBps": round(gbs, 2)})
+    line = {"metric": "link probes", "unit": "GB/s", "n_gpus": 1,
+            "h2d_memcpy_GBps": round(ibp.ibp_measure_h2d(0, 1 << 30, 8), 2), "d2h_memcpy_GBps": round(ibp.ibp_measure_d2h(0, 1 << 30, 8), 2),
+            "zero_copy_contiguous_read_GBps": round(ibp.ibp_measure_zero_copy_read(0, 1 << 30, 3), 2),
+            "random_span_reads_6GiB_footprint": table, "random_128B_spans_managed_by_footprint": scan,
+            "hugepages": {k: open(f).read().strip() for k, f in (("nr_hugepages", "/proc/sys/vm/nr_hugepages"), ("thp", "/sys/kernel/mm/transparent_hugepage/enabled")) if os.path.exists(f)}}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -1298,7 +1331,7 @@ def main():
     ap.add_argument("--threshold", default="1/1", help="tau = T/N as a fraction: 1/1 = group-strict (BASELINE.json), 4/5 = the paper's thresholded codec")
     ap.add_argument("--order", type=int, default=None, choices=[0, 1])
     ap.add_argument("--dedup", type=int, default=None, choices=[0, 1], help="default: off when the workload's sampler guarantees distinct ids, else the library's automatic mode")
-    ap.add_argument("--phase", default="gather", choices=["gather", "build", "masks", "resident"],
+    ap.add_argument("--phase", default="gather", choices=["gather", "build", "masks", "resident", "probes"],
                     help="gather = the hot path (default); build = the GPU-side compressor ibp_build_device; masks = the mask-quality tools (tau / chunk-size sweep, sampled masks, k-means); resident = ibp_decompress_resident alone (S8)")
     ap.add_argument("--cache-frac", type=float, default=0.0, help="gnn/dlrm: put a compressed GPU cache of this fraction of the packed store in front of the host store")
     ap.add_argument("--stream-mode", type=int, default=None, choices=[0, 1, 2], help="--phase resident: ibp_set_stream_mode (test/compare hook)")
@@ -1320,6 +1353,8 @@ def main():
         run_masks(args)
     elif args.phase == "resident":
         run_resident(args)
+    elif args.phase == "probes":
+        run_probes(args)
     elif args.workload == "weights":
         run_weights(args)
     else:

@@ -422,6 +422,18 @@ ibp_status ibp_measure_d2h(int device, size_t nbytes, int reps, double* gbps);
  * by address translation on the host path, not by the link.                                   */
 ibp_status ibp_measure_random_read(int device, size_t footprint_bytes, uint32_t span_bytes, int reps, double* spans_per_s,
                                    double* gbps);
+/* The same probe over host memory obtained in other ways, to show what the store kind costs on a machine: the span rate of a large
+ * footprint follows the GPU-side page size of the mapping (managed host-resident memory is mapped with large GPU pages; page-locked
+ * memory with 4 KB ones, whatever the host page size).  UNSUPPORTED: no huge pages are reserved on this machine (HUGETLB).       */
+enum {
+    IBP_MEM_MANAGED_HOST = 0,          /* cudaMallocManaged, preferred location CPU, accessed-by GPU (the default store kind)      */
+    IBP_MEM_HOSTALLOC = 1,             /* cudaHostAlloc mapped (IBP_FLAG_HOSTALLOC_STORE)                                          */
+    IBP_MEM_MALLOC_REGISTERED = 2,     /* anonymous mmap, 4 KB pages, cudaHostRegister (what IBP_STORE_SHARED segments get)        */
+    IBP_MEM_THP_REGISTERED = 3,        /* the same with madvise(MADV_HUGEPAGE) before the first touch                              */
+    IBP_MEM_HUGETLB_2M_REGISTERED = 4  /* mmap(MAP_HUGETLB, 2 MB pages), cudaHostRegister                                          */
+};
+ibp_status ibp_measure_random_read_kind(int device, size_t footprint_bytes, uint32_t span_bytes, int memory_kind, int reps,
+                                        double* spans_per_s, double* gbps);
 
 /* -- Mask-quality tools: the paper's preprocessing counters exposed, so that Mask/Bitval can be
  * built for any threshold from one counting pass (tau sweep), from a sample of the rows, evaluated

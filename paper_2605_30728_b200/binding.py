@@ -69,6 +69,7 @@ class ibp_table_desc(C.Structure):
 
 
 IBP_CACHE_MISS = 0xFFFFFFFFFFFFFFFF
+IBP_MEM_MANAGED_HOST, IBP_MEM_HOSTALLOC, IBP_MEM_MALLOC_REGISTERED, IBP_MEM_THP_REGISTERED, IBP_MEM_HUGETLB_2M_REGISTERED = range(5)
 IBP_SLAB_REMOTE = -2
 IBP_IPC_HANDLE_BYTES = 64
 
@@ -128,6 +129,7 @@ SIGNATURES = {
     "ibp_measure_zero_copy_read": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
     "ibp_measure_d2h": (_int, [_int, C.c_size_t, _int, C.POINTER(C.c_double)]),
     "ibp_measure_random_read": (_int, [_int, C.c_size_t, _u32, _int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "ibp_measure_random_read_kind": (_int, [_int, C.c_size_t, _u32, _int, _int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "ibp_table_groups": (_int, [C.POINTER(ibp_table_desc), C.POINTER(_u64)]),
     "ibp_bit_counts_device": (_int, [_vp, C.POINTER(ibp_table_desc), _vp, _i64, _vp, _vp, _vp]),
     "ibp_masks_from_counts_device": (_int, [_vp, _vp, _u64, _u32, _u32, _u32, _vp, _vp, _vp, _vp]),
@@ -466,6 +468,13 @@ def ibp_measure_random_read(device=0, footprint_bytes=4 << 30, span_bytes=128, r
     r, g = C.c_double(), C.c_double()
     _check(lib().ibp_measure_random_read(device, footprint_bytes, span_bytes, reps, C.byref(r), C.byref(g)))
     return r.value, g.value
+
+
+def ibp_measure_random_read_kind(device: int, footprint_bytes: int, span_bytes: int, memory_kind: int, reps: int = 3):
+    """(spans per second, GB/s) of random span reads over host memory of the given IBP_MEM_* kind"""
+    a, b = C.c_double(), C.c_double()
+    _check(lib().ibp_measure_random_read_kind(device, footprint_bytes, span_bytes, memory_kind, reps, C.byref(a), C.byref(b)))
+    return a.value, b.value
 
 
 # ---- mask-quality tools (SURVEY 8(f) NEXT #4): marshalling only, the work is in csrc/ibp_analysis.cu

@@ -15,6 +15,9 @@
 //   S5 expand   funnel-shift the k_i bits out of shared memory, deposit them at the Mask=0 positions, OR Bitval
 //   S6 store    one 16/8/4-byte streaming store per lane: 512/256/128 contiguous bytes per warp instruction
 #include <cuda_runtime.h>
+#include <sys/mman.h>
+
+#include <cerrno>
 
 #include <algorithm>
 #include <cstdio>
@@ -1497,18 +1500,63 @@ __global__ void ibp_random_read_kernel(const uint4* __restrict__ src, uint64_t n
     if (acc == 0x9E3779B9u) *sink = acc;
 }
 
-extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes, uint32_t span_bytes, int reps, double* spans_per_s, double* gbps) {
-    if (!spans_per_s || !gbps || footprint_bytes < (1u << 20) || reps < 1 || span_bytes < 16 || span_bytes > 512 || span_bytes % 16) {
+// memory_kind: how the host buffer is obtained and mapped for the GPU (ibp.h: IBP_MEM_*).  The span rate of a large footprint is set
+// by the GPU-side page size of the mapping, not by the host page size.
+extern "C" ibp_status ibp_measure_random_read_kind(int device, size_t footprint_bytes, uint32_t span_bytes, int memory_kind, int reps,
+                                                   double* spans_per_s, double* gbps) {
+    if (!spans_per_s || !gbps || footprint_bytes < (1u << 20) || reps < 1 || span_bytes < 16 || span_bytes > 512 || span_bytes % 16 ||
+        memory_kind < IBP_MEM_MANAGED_HOST || memory_kind > IBP_MEM_HUGETLB_2M_REGISTERED) {
         ibp_set_error("ibp_measure_random_read: bad argument"); return IBP_ERR_INVALID_ARG;
     }
     IBP_CUDA(cudaSetDevice(device));
-    void* p = nullptr;
-    ibp_status rc = ibp_host_alloc_managed(footprint_bytes, device, &p);
-    if (rc != IBP_OK) return rc;
-    {   // first touch on the host, in parallel
+    void *p = nullptr, *dptr = nullptr;
+    ibp_status rc = IBP_OK;
+    size_t map_bytes = 0;
+    bool registered = false;
+    auto release = [&]() {
+        if (registered) cudaHostUnregister(p);
+        if (memory_kind == IBP_MEM_MANAGED_HOST && p) ibp_host_free_managed(p);
+        else if (memory_kind == IBP_MEM_HOSTALLOC && p) cudaFreeHost(p);
+        else if (p && map_bytes) munmap(p, map_bytes);
+        (void)cudaGetLastError();
+    };
+    if (memory_kind == IBP_MEM_MANAGED_HOST) {
+        rc = ibp_host_alloc_managed(footprint_bytes, device, &p);
+        if (rc != IBP_OK) return rc;
+        dptr = p;
+    } else if (memory_kind == IBP_MEM_HOSTALLOC) {
+        if (cudaHostAlloc(&p, footprint_bytes, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) {
+            ibp_set_error("ibp_measure_random_read: cudaHostAlloc: %s", cudaGetErrorString(cudaGetLastError())); return IBP_ERR_OUT_OF_MEMORY;
+        }
+    } else {
+        map_bytes = (footprint_bytes + (2u << 20) - 1) & ~(size_t)((2u << 20) - 1);
+        int flags = MAP_PRIVATE | MAP_ANONYMOUS;
+        if (memory_kind == IBP_MEM_HUGETLB_2M_REGISTERED) flags |= MAP_HUGETLB | (21 << 26 /* MAP_HUGE_SHIFT */);
+        p = mmap(nullptr, map_bytes, PROT_READ | PROT_WRITE, flags, -1, 0);
+        if (p == MAP_FAILED) {
+            p = nullptr;
+            ibp_set_error("ibp_measure_random_read: mmap of %zu bytes (kind %d) failed: %s", map_bytes, memory_kind, strerror(errno));
+            return memory_kind == IBP_MEM_HUGETLB_2M_REGISTERED ? IBP_ERR_UNSUPPORTED : IBP_ERR_OUT_OF_MEMORY;   // no huge pages reserved on this machine
+        }
+        if (memory_kind == IBP_MEM_THP_REGISTERED) (void)madvise(p, map_bytes, MADV_HUGEPAGE);
+    }
+    {   // first touch on the host, in parallel (before page-locking: the pages exist when they are registered)
         const int64_t nchunk = (int64_t)((footprint_bytes + (1u << 22) - 1) >> 22);
 #pragma omp parallel for schedule(static)
         for (int64_t c = 0; c < nchunk; ++c) memset((char*)p + ((size_t)c << 22), 0x5A, std::min<size_t>(1u << 22, footprint_bytes - ((size_t)c << 22)));
+    }
+    if (memory_kind >= IBP_MEM_MALLOC_REGISTERED) {
+        if (cudaHostRegister(p, map_bytes, cudaHostRegisterMapped | cudaHostRegisterPortable) != cudaSuccess) {
+            ibp_set_error("ibp_measure_random_read: cudaHostRegister: %s", cudaGetErrorString(cudaGetLastError()));
+            release();
+            return IBP_ERR_CUDA;
+        }
+        registered = true;
+    }
+    if (!dptr && cudaHostGetDevicePointer(&dptr, p, 0) != cudaSuccess) {
+        ibp_set_error("ibp_measure_random_read: cudaHostGetDevicePointer: %s", cudaGetErrorString(cudaGetLastError()));
+        release();
+        return IBP_ERR_CUDA;
     }
     unsigned* sink = nullptr;
     cudaEvent_t a, b;
@@ -1522,7 +1570,7 @@ extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes
     } else {
         for (int it = 0; it < reps + 1; ++it) {
             cudaEventRecord(a, 0);
-            ibp_random_read_kernel<<<grid, block>>>((const uint4*)p, footprint_bytes / span_bytes, rpg, lanes, 0x1234u + it, sink);
+            ibp_random_read_kernel<<<grid, block>>>((const uint4*)dptr, footprint_bytes / span_bytes, rpg, lanes, 0x1234u + it, sink);
             cudaEventRecord(b, 0);
             if (cudaEventSynchronize(b) != cudaSuccess) { ibp_set_error("ibp_measure_random_read: %s", cudaGetErrorString(cudaGetLastError())); rc = IBP_ERR_CUDA; break; }
             float ms = 0;
@@ -1533,9 +1581,13 @@ extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes
         cudaEventDestroy(b);
     }
     if (sink) cudaFree(sink);
-    ibp_host_free_managed(p);
+    release();
     if (rc == IBP_OK) { *spans_per_s = n_reads / (best * 1e-3); *gbps = *spans_per_s * span_bytes * 1e-9; }
     return rc;
+}
+
+extern "C" ibp_status ibp_measure_random_read(int device, size_t footprint_bytes, uint32_t span_bytes, int reps, double* spans_per_s, double* gbps) {
+    return ibp_measure_random_read_kind(device, footprint_bytes, span_bytes, IBP_MEM_MANAGED_HOST, reps, spans_per_s, gbps);
 }
 
 // 1 = de-duplicate the ids of a random gather before fetching; 0 = fetch every id (the caller knows the ids are distinct);
