@@ -959,10 +959,10 @@ extern "C" ibp_status ibp_build_device(const void* rows_dev, const ibp_build_par
     } else {
         // pass 1: sizes and flags; scan -> row offsets
         const uint64_t n_flag_words = (n + 31) / 32;
-        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, (n + 1) * 4));
+        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, (n + 1) * 4 + 64));   // slack: the stream kernels copy 16-byte covers
         {
             const uint64_t words = h->slot_layout ? (h->capacity_rows + 31) / 32 : n_flag_words;
-            IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, words * 4));
+            IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, words * 4 + 64));
             IBP_CUDA(cudaMemsetAsync(h->row_flag_dev, 0, words * 4, st));
         }
         const uint64_t nblk = (n + 4095) / 4096;

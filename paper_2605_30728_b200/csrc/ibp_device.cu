@@ -807,24 +807,39 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     const uint32_t lpr = h->p.row_bytes % 16 == 0 ? h->p.row_bytes / 16 : 0;
     bool t2 = (lpr == 8 || lpr == 16 || lpr == 32) && h->t2_mode && !P.strided;
     if (t2) {
-        // pieces of 32 rows (16 for 512-byte rows), NW pieces per chunk.  Stages are sized for the typical chunk (56 KB); a chunk
-        // whose stored bytes exceed a stage -- only with many raw rows -- is loaded as sub-loads of split_rows rows.
-        const uint32_t U = lpr == 32 ? 16u : 32u;
-        const uint64_t STAGE = 36ull * 1024;
-        uint64_t rc = (uint64_t)std::min<int64_t>((int64_t)NW * U, span_rows);
+        // A unit (= chunk, = stage) is NW pieces, one per consumer warp; a stage holds the unit's packed bytes plus an aux region:
+        // descriptor, row-offset cover, row-flag cover, Mask/Bitval of the groups the unit touches (ibp_stream_t.cuh).  Two stages
+        // per CTA, three CTAs per SM: 38,144 bytes per stage.  The piece is the largest of 32 / 16 / 8 rows whose unit fits a stage
+        // even when every row is stored raw, so that no chunk is ever split (256-byte rows: 16, 512-byte rows: 8); only if even
+        // 8-row pieces do not fit is a chunk above a stage loaded as sub-units of split_rows rows.
+        const uint64_t STAGE = 38144;
+        const uint64_t G = h->p.group_param;
+        uint32_t U = lpr == 32 ? 16u : 32u;
+        uint64_t rc = 0, data_cap = 0;
+        for (;; U >>= 1) {
+            rc = (uint64_t)std::min<int64_t>((int64_t)NW * U, span_rows);
+            const uint64_t off_max = ((rc + 1 + 3 + 3 + 3) & ~3ull) * 4, flag_max = ((rc / 32 + 2 + 3 + 3) & ~3ull) * 4 + 16;
+            const uint64_t groups_max = rc < 2 ? 1 : (rc - 2) / G + 2, meta_max = groups_max * 2 * h->p.row_bytes;
+            P.aux_flag_off = (uint32_t)(32 + off_max);                        // [descriptor 32 B][row offsets][row flags][Mask/Bitval]
+            const uint64_t meta_off = (P.aux_flag_off + flag_max + 127) / 128 * 128;
+            const bool stage_meta = meta_max <= 8192;                        // small groups (a Mask/Bitval pair per row or two) stay in global memory
+            P.aux_meta_off = stage_meta ? (uint32_t)meta_off : 0u;
+            P.aux_bytes = (uint32_t)(stage_meta ? meta_off + meta_max : meta_off);
+            data_cap = STAGE - P.aux_bytes;
+            if (rc * stride + 64 <= data_cap || U <= 8) break;
+        }
         P.rows_per_chunk = (uint32_t)rc;
         P.piece_rows = U;
+        P.stage_bytes = (uint32_t)STAGE;
         per = rc;
-        if (rc * stride + 64 <= STAGE) {
+        if (rc * stride + 64 <= data_cap) {
             P.nsplit = 1;
-            P.stage_bytes = (uint32_t)((rc * stride + 64 + 127) / 128 * 128);
         } else {
-            const uint64_t split_rows = ((STAGE - 64) / stride) / U * U;
+            const uint64_t split_rows = ((data_cap - 64) / stride) / U * U;
             if (split_rows == 0) t2 = false;
             else {
                 P.split_rows = (uint32_t)split_rows;
                 P.nsplit = (uint32_t)((rc + split_rows - 1) / split_rows);
-                P.stage_bytes = (uint32_t)STAGE;
             }
         }
     }
@@ -855,15 +870,16 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
     if (smem > 220 * 1024) { ibp_set_error("thresholded rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
     if (t2) {
-        const int nr = (h->max_runs >= 1 && h->max_runs <= 3) ? h->max_runs : 0;
+        const int nr = (h->max_runs >= 1 && h->max_runs <= 4) ? h->max_runs : 0;      // bf16 pairs: mantissa + sign per half = 4 runs
 #define IBP_T2_NR(LPR_, NS_)                                                                              \
         switch (nr) {                                                                                     \
             case 1: return launch_stream_t2_one<LPR_, NS_, 1>(P, h->max_ctas, h->sm_count, smem, st);     \
             case 2: return launch_stream_t2_one<LPR_, NS_, 2>(P, h->max_ctas, h->sm_count, smem, st);     \
             case 3: return launch_stream_t2_one<LPR_, NS_, 3>(P, h->max_ctas, h->sm_count, smem, st);     \
+            case 4: return launch_stream_t2_one<LPR_, NS_, 4>(P, h->max_ctas, h->sm_count, smem, st);     \
             default: return launch_stream_t2_one<LPR_, NS_, 0>(P, h->max_ctas, h->sm_count, smem, st);    \
         }
-#define IBP_T2(LPR_) if (ns == 2) { IBP_T2_NR(LPR_, 2) } else { IBP_T2_NR(LPR_, 3) }
+#define IBP_T2(LPR_) { IBP_T2_NR(LPR_, 2) }                                                            /* t2: always two stages */
         if (lpr == 32) { IBP_T2(32) }
         if (lpr == 16) { IBP_T2(16) }
         IBP_T2(8)
@@ -914,11 +930,11 @@ ibp_status ibp_attach_device(ibp_handle* h, int device, void* cuda_stream) {
         IBP_CUDA(cudaMemcpyAsync(h->row_size_dev, h->row_size.data(), h->row_size.size(), cudaMemcpyHostToDevice, st));
     }
     if (h->thresholded && !h->slot_layout && !h->row_off_dev) {
-        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, h->row_off.size() * 4));
+        IBP_CUDA(cudaMalloc((void**)&h->row_off_dev, h->row_off.size() * 4 + 64));   // slack: the stream kernels copy 16-byte covers
         IBP_CUDA(cudaMemcpyAsync(h->row_off_dev, h->row_off.data(), h->row_off.size() * 4, cudaMemcpyHostToDevice, st));
     }
     if (h->thresholded && !h->row_flag_dev) {
-        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, h->row_flag.size() * 4));
+        IBP_CUDA(cudaMalloc((void**)&h->row_flag_dev, h->row_flag.size() * 4 + 64));
         IBP_CUDA(cudaMemcpyAsync(h->row_flag_dev, h->row_flag.data(), h->row_flag.size() * 4, cudaMemcpyHostToDevice, st));
     }
     // expand move masks per (group, word) when the table has few groups (strided column tiles, small tables): 20 B per word

@@ -70,6 +70,26 @@ __device__ __forceinline__ void expand_masks(uint32_t nv, uint32_t mv[5]) {
         mk &= ~mp;
     }
 }
+// The same with only the first nstg stages computed (nstg warp-uniform): stage i moves bits by 2^i, and a bit moves by the number of
+// invariant bits below it, so a word with fewer than 2^i invariant bits has mv[i] = 0 -- exactly, not approximately.
+__device__ __forceinline__ void expand_masks_n(uint32_t nv, uint32_t mv[5], int nstg) {
+    uint32_t m = nv, mk = ~nv << 1;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        mv[i] = 0;
+        if (i < nstg) {
+            uint32_t mp = mk ^ (mk << 1);
+            mp ^= mp << 2;
+            mp ^= mp << 4;
+            mp ^= mp << 8;
+            mp ^= mp << 16;
+            const uint32_t v = mp & m;
+            mv[i] = v;
+            m = (m ^ v) | (v >> (1 << i));
+            mk &= ~mp;
+        }
+    }
+}
 // bit-select in ONE logic op: (c & a) | (~c & b)  (lop3 truth table 0xE4 for inputs a, b, c)
 __device__ __forceinline__ uint32_t bitselect(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t d;

@@ -27,6 +27,8 @@ struct StreamTParams {
     uint32_t group_param, group_shift, strided;
     uint32_t stage_bytes;
     uint32_t nsplit, split_rows;   // ibp_stream_t2_kernel: a chunk above one stage is loaded as nsplit sub-loads of split_rows rows (0/1 = never)
+    // ibp_stream_t2_kernel: a stage = [packed bytes: stage_bytes - aux_bytes][aux: descriptor (32 B), row offsets, row flags, Mask/Bitval]
+    uint32_t aux_bytes, aux_flag_off, aux_meta_off;   // offsets inside the aux region; aux_meta_off = 0: Mask/Bitval are not staged
 };
 
 // RUNS: every word of every group of the table has at most three runs of variant bits (decided once per handle on the host):
@@ -307,16 +309,26 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
 
 // ------------------------------------------------------------------------------------------------------------------------
 // ibp_stream_t2_kernel -- the thresholded stream decode for rows of 16*LPR bytes (LPR = 8, 16 or 32 lanes per row; W = 4
-// words per lane: 128 / 256 / 512-byte rows, i.e. every BASELINE workload).  Same producer/consumer pipeline as above; the
-// consumer side is rebuilt around the instruction count per row, which is what bounded the kernel above (ncu: 177 warp
-// instructions per 512-byte row at 60 % issue utilisation against 68 for the strict kernel):
-// Blocked groups only (strided tables keep the kernel above).
+// words per lane: 128 / 256 / 512-byte rows, i.e. every BASELINE workload).  Blocked groups only (strided tables keep the
+// kernel above).  Built around two measurements of the kernel above (ncu, profiles/r01_resident_ncu.md, r02_resident_ncu.md):
+// the instruction count per row, and the long-scoreboard stalls of the consumer warps' own global loads.
+//
+// EVERYTHING a consumer warp reads comes out of shared memory.  The producer lane walks the chunks (the only place that reads
+// ids and row offsets from global memory) and loads UNITS: a unit is a chunk, or -- when the chunk's stored bytes exceed a stage,
+// which only happens with many raw rows -- one of its sub-ranges of split_rows rows.  For every unit it writes a 32-byte
+// descriptor {first row id, first output row, rows, offset of the first row, last-unit-of-the-chunk flag} into the stage and
+// issues bulk copies of (1) the unit's packed bytes (contiguous: rows lie back to back), (2) the 16-byte cover of the unit's row
+// offsets, (3) the cover of its row-flag words and (4) Mask/Bitval of the table groups it touches (consecutive groups
+// are contiguous in GPU memory: "shared-memory staging of the metadata") -- all completing on the stage's full barrier.  The
+// consumers wait for the barrier, read the descriptor and never touch global memory except to store rows: no prefetch state in
+// registers, no long-scoreboard stalls, and the same code for span gathers, ranges and resident decode.
+//
+// Consumer side:
 //   - a warp decodes 32/LPR rows per pass, one row per group of LPR lanes (256-byte rows: two at a time), so the per-row fixed
 //     work (participation read, counts, scan, address set-up, store) is shared by twice or four times the data;
 //   - the lane groups of a pass take rows of DIFFERENT parts of the piece (group of lanes s: rows [s*Q, (s+1)*Q)), so with small
 //     groups (KV: 16 rows) one set-up -- Mask/Bitval loads, run masks or expand masks -- prepares two or four groups at once;
-//   - pieces are 32 rows (16 for 512-byte rows), chunks NW pieces; a chunk whose stored bytes exceed a stage (many raw rows) is
-//     loaded as NSPLIT sub-loads into consecutive stages -- both sides decide that from the same two row offsets;
+//   - a unit is NW pieces, one per consumer warp, so every warp works on every stage and the stages double-buffer;
 //   - raw rows take the SAME code with an empty header and no participating chunk (every chunk then contributes its 32
 //     bits at offset 32*c), so a pass never diverges on the row kind;
 //   - bits removed in front of each of the lane's 4 chunks come from ONE packed computation: popc(Mask) of the 4 chunks sit in
@@ -328,7 +340,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
 //   - NR (handle level: the most runs of variant bits in any Mask word of the table): bits go back run by run with exactly NR
 //     multiply + and-or pairs; NR = 0 selects the five-stage expand.
 __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
-    // consumer-side wait with a suspend-time hint: a waiting warp stays off the issue port instead of polling
+    // wait with a suspend-time hint: a waiting warp stays off the issue port instead of polling
     uint32_t ok = 0;
     while (!ok) {
         asm volatile(
@@ -337,6 +349,14 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity)
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
     }
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void lds128(uint32_t a, uint32_t (&v)[4]) {
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(a));
 }
 
 template <int LPR, int NS, int NW, int NR>
@@ -352,43 +372,50 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     }
     __syncthreads();
     const uint64_t S = P.group_param;
-    const uint32_t cap16 = (P.stage_bytes - 64u) / 16u;          // what one stage holds, in 16-byte units
-    const uint32_t nsplit = P.nsplit, sub_rows = P.split_rows;   // nsplit > 1: a chunk above cap16 is loaded as nsplit sub-loads of sub_rows rows
-
-    auto chunk_geom = [&](int64_t c, int64_t& row0, uint32_t& nrows, int64_t& out0) {
-        const int64_t si = !P.ids ? 0 : (P.n_chunks <= 0x7FFFFFFFll ? (int64_t)((uint32_t)c / P.chunks_per_span) : c / P.chunks_per_span);
-        const int64_t cc = c - si * P.chunks_per_span;
-        const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
-        const int64_t per = (int64_t)P.rows_per_chunk;                          // blocked groups only (strided tables: the kernel above)
-        const int64_t r = cc * per;
-        row0 = span_first + r;
-        nrows = (uint32_t)min(per, P.span_rows - r);
-        out0 = si * P.span_rows + r;
-    };
+    const uint32_t data_cap = P.stage_bytes - P.aux_bytes;       // stage = [packed bytes][aux]
+    const uint32_t cap16 = (data_cap - 64u) / 16u;               // what one stage holds, in 16-byte units
+    const uint32_t row_bytes2 = 2u * P.row_bytes;
 
     if (wib == NW) {
+        // ------------------------------------------------------------------ producer: one lane walks the chunks
         if (lane != 0) return;
         uint32_t k = 0;
         for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x) {
-            int64_t row0, out0; uint32_t nrows;
-            chunk_geom(c, row0, nrows, out0);
+            const int64_t si = !P.ids ? 0 : (P.n_chunks <= 0x7FFFFFFFll ? (int64_t)((uint32_t)c / P.chunks_per_span) : c / P.chunks_per_span);
+            const int64_t cc = c - si * P.chunks_per_span;
+            const int64_t span_first = P.ids ? P.ids[si] * P.span_rows : P.first_row;
+            const int64_t r = cc * (int64_t)P.rows_per_chunk;
+            const int64_t row0 = span_first + r, out0 = si * P.span_rows + r;
+            const uint32_t nrows = (uint32_t)min((int64_t)P.rows_per_chunk, P.span_rows - r);
             const uint32_t o0 = __ldg(P.row_off + row0), o1 = __ldg(P.row_off + row0 + nrows);
-            const uint32_t parts = (nsplit > 1 && o1 - o0 > cap16) ? nsplit : 1u;
-            for (uint32_t j = 0; j < parts; ++j, ++k) {
-                const uint32_t s = k % NS;
-                uint32_t a0 = o0, a1 = o1;
-                if (parts > 1) {
-                    const uint32_t r0 = min(nrows, j * sub_rows), r1 = min(nrows, r0 + sub_rows);
-                    a0 = __ldg(P.row_off + row0 + r0);
-                    a1 = __ldg(P.row_off + row0 + r1);
-                }
-                mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
-                const uint8_t* src = P.store + (16ull * a0 - P.bias);
+            const bool split = P.nsplit > 1 && o1 - o0 > cap16;
+            const uint32_t step = split ? P.split_rows : nrows;
+            for (uint32_t r0 = 0; r0 < nrows; r0 += step, ++k) {
+                const uint32_t s = k % NS, r1 = min(nrows, r0 + step), n = r1 - r0;
+                const uint32_t a0 = split ? __ldg(P.row_off + row0 + r0) : o0, a1 = split ? __ldg(P.row_off + row0 + r1) : o1;
+                const int64_t first = row0 + r0;
+                // covers, all 16-byte aligned at both ends: row offsets [first, first + n] from index first & ~3, flag words from
+                // word (first >> 5) & ~3, Mask/Bitval of groups g0 .. g1
+                const int64_t oi = first & ~3ll;
+                const uint32_t off_bytes = (uint32_t)(((first + n + 1 - oi) + 3) & ~3ll) * 4u;
+                const int64_t fw = (first >> 5) & ~3ll;
+                const uint32_t flag_bytes = (uint32_t)(((((first + n - 1) >> 5) + 1 - fw) + 3) & ~3ll) * 4u;
+                const uint64_t g0 = group_of_u(P.group_param, P.group_shift, (uint64_t)first);
+                const uint64_t g1 = group_of_u(P.group_param, P.group_shift, (uint64_t)first + n - 1);
+                const uint32_t meta_bytes = P.aux_meta_off ? (uint32_t)(g1 - g0 + 1) * row_bytes2 : 0u;
                 const uint32_t bytes = (a1 - a0) * 16u;
-                mbar_expect_tx(full_s + s * 8, bytes);
-                const uint32_t dst = smem_s + s * P.stage_bytes;
+                const uint32_t stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap, bar = full_s + s * 8;
+                mbar_wait_relaxed(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s), "r"((uint32_t)first), "r"((uint32_t)((uint64_t)first >> 32)),
+                             "r"((uint32_t)(out0 + r0)), "r"((uint32_t)((uint64_t)(out0 + r0) >> 32)) : "memory");
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s + 16u), "r"(n), "r"(a0), "r"(r1 == nrows ? 1u : 0u), "r"(0u) : "memory");
+                mbar_expect_tx(bar, bytes + off_bytes + flag_bytes + meta_bytes);     // release: the descriptor is visible to whoever sees the phase complete
+                bulk_g2s(aux_s + 32u, P.row_off + oi, off_bytes, bar);
+                bulk_g2s(aux_s + P.aux_flag_off, P.row_flag + fw, flag_bytes, bar);
+                if (meta_bytes) bulk_g2s(aux_s + P.aux_meta_off, P.meta + g0 * 2ull * P.n_words, meta_bytes, bar);
+                const uint8_t* src = P.store + (16ull * a0 - P.bias);
                 for (uint32_t o = 0; o < bytes; o += 16384u)
-                    bulk_g2s(dst + o, src + o, min(16384u, bytes - o), full_s + s * 8);
+                    bulk_g2s(stage_s + o, src + o, min(16384u, bytes - o), bar);
             }
         }
         return;
@@ -402,11 +429,19 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     const uint32_t hdr_off = (w0 >> 5) * 4u, hdr_sh = w0 & 31u;                // where the lane's 4 participation bits sit
     uint32_t m[W], b[W], mv[W][NMV], pm4 = 0;                                  // pm4: popc(Mask) of the 4 chunks, one per byte
     uint64_t prep_g = ~0ull;                                                   // per lane: lane groups may hold different groups
+    bool five = true;                                                          // NR = 0: some bit of the prepared groups moves by >= 16 (warp-uniform)
 
-    auto prepare = [&](uint64_t g) {
-        const uint32_t* gm = P.meta + g * 2ull * P.n_words;
-        VecIO<W>::ld(gm + w0, m);
-        VecIO<W>::ld(gm + P.n_words + w0, b);
+    // S2 for group g: Mask/Bitval from the stage's aux region (meta_s = shared address of group g0's record), else from global memory
+    auto prepare = [&](uint64_t g, uint64_t g0, uint32_t meta_s) {
+        if (P.aux_meta_off) {
+            const uint32_t a = meta_s + (uint32_t)(g - g0) * row_bytes2 + w0 * 4u;
+            lds128(a, m);
+            lds128(a + P.row_bytes, b);
+        } else {
+            const uint32_t* gm = P.meta + g * 2ull * P.n_words;
+            VecIO<W>::ld(gm + w0, m);
+            VecIO<W>::ld(gm + P.n_words + w0, b);
+        }
         pm4 = 0;
 #pragma unroll
         for (int q = 0; q < W; ++q) pm4 |= (uint32_t)__popc(m[q]) << (8 * q);   // <= 32 each
@@ -416,21 +451,44 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 uint32_t nv = ~m[q], c = 0;
 #pragma unroll
                 for (int j = 0; j < NR; ++j) {
-                    const uint32_t low = nv & (0u - nv), run = nv & ~(nv + low);     // nv == 0 -> low = run = 0
-                    mv[q][j] = run ? 1u << ((__ffs(low) - 1) - c) : 0u;
+                    const uint32_t low = nv & (0u - nv), t = nv + low, run = nv & ~t;   // nv == 0 -> low = run = 0
+                    mv[q][j] = low >> c;                                         // 2^(p_j - c_j): run j moves up by (its position - bits below it)
                     mv[q][NR + j] = run;
                     c += __popc(run);
-                    nv &= ~run;
+                    nv &= t;
                 }
             }
         } else {
+            // five-stage expand: only the stages that can move a bit are computed (a bit moves by the number of invariant bits below
+            // it, at most popc(Mask word)); warp-uniform, so the branches do not diverge
+            const uint32_t pmax = __reduce_max_sync(0xFFFFFFFFu, max(max(pm4 & 0xFFu, (pm4 >> 8) & 0xFFu), max((pm4 >> 16) & 0xFFu, pm4 >> 24)));
+            const int nstg = pmax >= 16u ? 5 : pmax >= 8u ? 4 : pmax >= 4u ? 3 : pmax >= 2u ? 2 : pmax >= 1u ? 1 : 0;
+            five = nstg == 5;
+            bool shared = false;
+            if constexpr (RPP == 2) shared = __all_sync(0xFFFFFFFFu, g == __shfl_xor_sync(0xFFFFFFFFu, g, 16));
+            if (shared) {
+                // both half-warps hold the SAME group (pieces of one 16-row group, KV): each half derives the masks of two of the
+                // lane's four words and the halves swap results -- 10 shuffles instead of two more mask derivations
+                if constexpr (RPP == 2) {
+                    uint32_t t0[5], t1[5];
+                    expand_masks_n(~(sub ? m[2] : m[0]), t0, nstg);
+                    expand_masks_n(~(sub ? m[3] : m[1]), t1, nstg);
 #pragma unroll
-            for (int q = 0; q < W; ++q) {
-                if (q > 0 && m[q] == m[q - 1]) {
+                    for (int i = 0; i < 5; ++i) {
+                        const uint32_t o0 = __shfl_xor_sync(0xFFFFFFFFu, t0[i], 16), o1 = __shfl_xor_sync(0xFFFFFFFFu, t1[i], 16);
+                        mv[0][i] = sub ? o0 : t0[i]; mv[1][i] = sub ? o1 : t1[i];
+                        mv[2][i] = sub ? t0[i] : o0; mv[3][i] = sub ? t1[i] : o1;
+                    }
+                }
+            } else {
 #pragma unroll
-                    for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
-                } else {
-                    expand_masks(~m[q], mv[q]);
+                for (int q = 0; q < W; ++q) {
+                    if (q > 0 && m[q] == m[q - 1]) {
+#pragma unroll
+                        for (int i = 0; i < 5; ++i) mv[q][i] = mv[q - 1][i];
+                    } else {
+                        expand_masks_n(~m[q], mv[q], nstg);
+                    }
                 }
             }
         }
@@ -450,14 +508,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     // RB passes side by side: lane group `sub` decodes row rr[i] of the piece in pass i (valid[i] = 0: the row is a repeat whose
     // result is not stored).  my_off / flags: offsets (lane i <-> row i of the piece) and compressed-bits of the piece.
     auto decode_rows_n = [&](auto nstg_c, const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
-                             uint32_t stage_s, uint8_t* orow0, uint32_t ostride) {
+                             uint32_t stage_s, uint8_t* orow0) {
         uint32_t bitbase[RB], part[RB], s[RB], d4[RB];
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
             const uint32_t sa = stage_s + (__shfl_sync(0xFFFFFFFFu, my_off, rr[i]) - base_off) * 16u;
             const bool comp = (flags >> rr[i]) & 1u;
-            uint32_t h;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(h) : "r"(sa + hdr_off));
+            const uint32_t h = lds32(sa + hdr_off);
             part[i] = comp ? (h >> hdr_sh) & 0xFu : 0u;                        // raw row: no chunk participates ...
             const uint32_t sel = ((part[i] * 0x00204081u) & 0x01010101u) * 0xFFu;   // participation bit q -> byte q = 0xFF
             const uint32_t in4 = (pm4 & sel) * 0x01010101u;                    // byte q = bits removed in chunks 0..q of this lane
@@ -485,24 +542,25 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 const uint32_t e = reinsert(nstg_c, x, q);
                 o[q] = ((part[i] >> q) & 1u) ? e : x;                          // non-participating chunk: all 32 bits
             }
-            uint8_t* dst = orow0 + rr[i] * ostride;
+            uint8_t* dst = orow0 + (size_t)rr[i] * P.row_bytes;
             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};\n\t}"
                          ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]), "r"(valid[i]) : "memory");
         }
     };
-
+    // NR = 0: two copies of the pass body, with and without the stage that moves bits by 16 (bf16 pairs with a few invariant
+    // exponent bits per half never need it); the choice is per prepared group and warp-uniform
     auto decode_rows = [&](const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
-                           uint32_t stage_s, uint8_t* orow0, uint32_t ostride) {
+                           uint32_t stage_s, uint8_t* orow0) {
         using std::integral_constant;
-        // (specialising the expand to 3 / 4 stages per group, as the strict kernel does, was measured slower here: three copies of
-        // the pass body under the 72-register budget cost more than the two stages they save -- KV 0.54 -> 0.52)
-        decode_rows_n(integral_constant<int, 5>{}, rr, valid, my_off, flags, base_off, stage_s, orow0, ostride);
+        if (NR > 0 || five) decode_rows_n(integral_constant<int, 5>{}, rr, valid, my_off, flags, base_off, stage_s, orow0);
+        else decode_rows_n(integral_constant<int, 4>{}, rr, valid, my_off, flags, base_off, stage_s, orow0);
     };
 
-    // One piece: rows id0, id0 + id_step, ... (cnt <= 32), all inside one stage.  orow = output address of row 0 of the piece.
-    const uint32_t Q = (P.piece_rows + RPP - 1) / RPP;                         // rows of a piece per lane group
-    auto decode_piece = [&](int64_t id0, int64_t id_step, uint32_t cnt, uint32_t my_off, uint32_t flags, uint32_t base_off,
-                            uint32_t stage_s, uint8_t* orow, uint32_t ostride, bool& waited, uint32_t bar, uint32_t parity) {
+    // One piece: rows id0 .. id0 + cnt - 1 (cnt <= 32), all inside the stage.  orow = output address of row 0 of the piece.
+    const uint32_t U = P.piece_rows;
+    const uint32_t Q = (U + RPP - 1) / RPP;                                    // rows of a piece per lane group
+    auto decode_piece = [&](int64_t id0, uint32_t cnt, uint32_t my_off, uint32_t flags, uint32_t base_off, uint32_t stage_s, uint8_t* orow,
+                            uint64_t g0, uint32_t meta_s) {
         orow += (size_t)w0 * 4;
         const uint32_t qs = min(cnt, sub * Q), qe = min(cnt, qs + Q);
         const bool have = qs < qe;
@@ -514,8 +572,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
         if (__all_sync(0xFFFFFFFFu, !have || glo == ghi)) {
             // every lane group's rows lie in one group of the table: one set-up per piece, possibly of several groups at once
             const uint64_t g = have ? glo : group_of_u(P.group_param, P.group_shift, (uint64_t)id0);
-            if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g);
-            if (!waited) { mbar_wait_relaxed(bar, parity); waited = true; }
+            if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
             const uint32_t n_it = min(Q, cnt);
             for (uint32_t i = 0; i < n_it; i += RB) {
                 uint32_t rr[RB], valid[RB];
@@ -525,7 +582,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                     valid[j] = r < qe;
                     rr[j] = valid[j] ? r : (have ? qs : 0u);
                 }
-                decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow, ostride);
+                decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow);
             }
         } else {
             // a table group ends inside a lane group's rows (a range that starts off a group boundary): run by run of one group
@@ -534,8 +591,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 const uint64_t id = (uint64_t)(id0 + r);
                 const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
                 const uint32_t r_end = (uint32_t)min((uint64_t)cnt, (uint64_t)r + ((g + 1) * S - id));
-                if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g);
-                if (!waited) { mbar_wait_relaxed(bar, parity); waited = true; }
+                if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
                 for (; r < r_end; r += RB * RPP) {
                     uint32_t rr[RB], valid[RB];
 #pragma unroll
@@ -544,66 +600,40 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                         valid[j] = x < r_end;
                         rr[j] = valid[j] ? x : r;
                     }
-                    decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow, ostride);
+                    decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow);
                 }
                 r = r_end;
             }
         }
     };
 
-    auto load_piece = [&](int64_t id0, int64_t id_step, uint32_t cnt, uint32_t& off_abs, uint32_t& flag) {
-        const int64_t id = id0 + (int64_t)lane * id_step;
-        off_abs = (uint32_t)lane < cnt ? __ldg(P.row_off + id) : 0u;
-        flag = (uint32_t)lane < cnt ? (__ldg(P.row_flag + (id >> 5)) >> (id & 31)) & 1u : 0u;
-    };
-    const uint32_t U = P.piece_rows;
-    int64_t n_row0 = 0, n_out0 = 0;
-    uint32_t n_nrows = 0, n_base = 0, n_end = 0, n_off = 0, n_flag = 0;
-    if ((int64_t)blockIdx.x < P.n_chunks) {
-        chunk_geom(blockIdx.x, n_row0, n_nrows, n_out0);
-        n_base = __ldg(P.row_off + n_row0);
-        n_end = __ldg(P.row_off + n_row0 + n_nrows);
-        if (wib * U < n_nrows) load_piece(n_row0 + wib * U, 1, min(U, n_nrows - wib * U), n_off, n_flag);
-    }
-
     uint32_t k = 0;
     for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x) {
-        const int64_t row0 = n_row0, out0 = n_out0;
-        const uint32_t nrows = n_nrows, base_off = n_base;
-        const uint32_t parts = (nsplit > 1 && n_end - n_base > cap16) ? nsplit : 1u;
-        uint32_t my_off = n_off, my_flag = n_flag;
-        if (c + gridDim.x < P.n_chunks) {
-            chunk_geom(c + gridDim.x, n_row0, n_nrows, n_out0);
-            n_base = __ldg(P.row_off + n_row0);
-            n_end = __ldg(P.row_off + n_row0 + n_nrows);
-            if (wib * U < n_nrows) {
-                load_piece(n_row0 + wib * U, 1, min(U, n_nrows - wib * U), n_off, n_flag);
-                const uint64_t ng = group_of_u(P.group_param, P.group_shift, (uint64_t)n_row0 + wib * U + min(sub * Q, U - 1));   // warm L1 with its Mask/Bitval
-                const uint32_t* ngm = P.meta + ng * 2ull * P.n_words + w0;
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm));
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm + P.n_words));
+        uint32_t last;
+        do {                                                                   // the units of chunk c, in the producer's order
+            const uint32_t s = k % NS, stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap;
+            mbar_wait_relaxed(full_s + s * 8, (k / NS) & 1u);
+            uint32_t d0[4], d1[4];
+            lds128(aux_s, d0);
+            lds128(aux_s + 16u, d1);
+            const int64_t first = (int64_t)(((uint64_t)d0[1] << 32) | d0[0]), out0 = (int64_t)(((uint64_t)d0[3] << 32) | d0[2]);
+            const uint32_t n = d1[0], base_off = d1[1];
+            last = d1[2];
+            const uint32_t off_s = aux_s + 32u - (uint32_t)(first & ~3ll) * 4u;          // shared address of row_off[0] (wraps mod 2^32: only differences matter)
+            const int64_t fw = (first >> 5) & ~3ll;
+            const uint64_t g0 = group_of_u(P.group_param, P.group_shift, (uint64_t)first);
+            for (uint32_t j0 = wib * U; j0 < n; j0 += NW * U) {
+                const uint32_t cnt = min(U, n - j0);
+                const int64_t id0 = first + j0;
+                const uint32_t my_off = (uint32_t)lane < cnt ? lds32(off_s + ((uint32_t)id0 + (uint32_t)lane) * 4u) : 0u;
+                const uint32_t fa = aux_s + P.aux_flag_off + (uint32_t)((id0 >> 5) - fw) * 4u;
+                uint32_t flags = __funnelshift_r(lds32(fa), lds32(fa + 4u), (uint32_t)id0 & 31u);   // bit r = flag of row id0 + r
+                if (cnt < 32u) flags &= (1u << cnt) - 1u;
+                decode_piece(id0, cnt, my_off, flags, base_off, stage_s, P.out + (uint64_t)(out0 + j0) * P.row_bytes, g0, aux_s + P.aux_meta_off);
             }
-        }
-        {
-            const uint32_t n_pieces = (nrows + U - 1) / U;
-            for (uint32_t j = 0; j < parts; ++j, ++k) {                        // one pass unless the chunk was split
-                const uint32_t s = k % NS, stage_s = smem_s + s * P.stage_bytes;
-                const uint32_t bar = full_s + s * 8, parity = (k / NS) & 1u;
-                const uint32_t r_lo = parts > 1 ? min(nrows, j * sub_rows) : 0u, r_hi = parts > 1 ? min(nrows, r_lo + sub_rows) : nrows;
-                const uint32_t sub_base = parts > 1 ? __ldg(P.row_off + row0 + r_lo) : base_off;
-                bool waited = false;
-                for (uint32_t p = wib; p < n_pieces; p += NW) {
-                    const uint32_t j0 = p * U, cnt = min(U, nrows - j0);
-                    if (j0 < r_lo || j0 >= r_hi) continue;                     // sub_rows is a multiple of the piece size
-                    const int64_t id0 = row0 + j0;
-                    if (p != (uint32_t)wib) load_piece(id0, 1, cnt, my_off, my_flag);   // later pieces of the chunk: on demand
-                    const uint32_t flags = __ballot_sync(0xFFFFFFFFu, my_flag);
-                    decode_piece(id0, 1, cnt, my_off, flags, sub_base, stage_s, P.out + (uint64_t)(out0 + j0) * P.row_bytes, P.row_bytes, waited, bar, parity);
-                }
-                if (!waited) mbar_wait_relaxed(bar, parity);                   // a warp without a piece still has to follow the phases
-                __syncwarp();
-                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
-            }
-        }
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+            ++k;
+        } while (!last);
     }
 }
