@@ -269,8 +269,9 @@ ibp_status ibp_configure(ibp_handle* h, uint32_t max_ctas, uint32_t warps_per_ct
 ibp_status ibp_validate_ids(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, int64_t* n_bad_host, void* cuda_stream);
 
 /* Sum over the DISTINCT ids of a batch of the packed bytes one id moves over PCIe (index_span rows each): the
- * algorithmic link traffic of one ibp_gather_decompress call.  stored = with alignment padding, bytealigned =
- * ceil(k/8) per row.  Host-side helper for roofline accounting; ids on the host.                                   */
+ * algorithmic link traffic of one ibp_gather_decompress call.  stored = what the kernels fetch: each row with its alignment
+ * padding (a single row: up to whole 32-byte sectors, at most its stride; rows of a span: the whole contiguous run),
+ * bytealigned = ceil(k/8) per row.  Host-side helper for roofline accounting; ids on the host.                      */
 ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* row_ids_host, int64_t n, uint64_t* n_unique,
                                 uint64_t* stored, uint64_t* bytealigned);
 

@@ -223,7 +223,10 @@ __global__ void __launch_bounds__(256) ibp_decode_kernel(const DecodeParams P) {
                 const uint8_t* src = P.store + (off - P.bias);
                 const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
                 a0 = src - head;                                              // 16-byte aligned cover
-                nvec = fe.stride ? (head + fe.stride + 15u) >> 4 : 0u;
+                // what is fetched: the row's bytes rounded up to whole 32-byte sectors, never more than its stride (A >= 64 pads rows to
+                // lines for alignment, and that padding need not cross the link)
+                const uint32_t fb = min(fe.stride, (((fe.k_bits + 7u) >> 3) + 31u) & ~31u);
+                nvec = fb ? (head + fb + 15u) >> 4 : 0u;
             }
             if (CACHE) {
                 const uint64_t ent = ibp_cache_find(P.cmap, P.cmap_mask, id);

@@ -691,8 +691,11 @@ extern "C" ibp_status ibp_batch_link_bytes(const ibp_handle* h, const int64_t* i
             const uint64_t r = (uint64_t)id * span + j;
             if (h->thresholded) { s += ibp_row_stored_T(h, r); b += row_size_from_store(h, r); continue; }
             const uint64_t g = h->p.group_kind == IBP_GROUP_BLOCKED ? r / h->p.group_param : r % h->p.group_param;
-            s += h->gtab[g].stride;
-            b += (h->gtab[g].k_bits + 7) / 8;
+            const uint64_t ba = (h->gtab[g].k_bits + 7) / 8;
+            // a single row is fetched up to whole 32-byte sectors, never beyond its stride (padding to A >= 64 stays in host memory);
+            // rows of a span are read as one contiguous run, padding included
+            s += span == 1 ? std::min<uint64_t>(h->gtab[g].stride, (ba + 31) & ~31ull) : h->gtab[g].stride;
+            b += ba;
             if (h->p.group_kind == IBP_GROUP_BLOCKED && span > 1) {       // whole groups inside a span: skip ahead
                 const uint64_t left = std::min<uint64_t>(h->p.group_param - (r % h->p.group_param), span - j) - 1;
                 s += left * h->gtab[g].stride;
