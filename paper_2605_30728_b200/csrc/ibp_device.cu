@@ -627,11 +627,11 @@ static void fill_common(const ibp_handle* h, DecodeParams& P) {
 // ------------------------------------------------------------------------------------------------ stream launch
 // Contiguous runs of rows (spans of blocked groups, whole ranges of either kind) through the TMA producer/consumer
 // pipeline of ibp_stream.cuh.  `packed` is the device-visible address of byte `bias` of the packed store.
-template <int W, int NS, int NSEG>
+template <int W, int NS, int NSEG, bool STAGED = false>
 static ibp_status launch_stream_one(const StreamBatch<NSEG>& B, int64_t total_chunks, uint32_t grid_multiple, int64_t max_ctas, int sm_count,
                                     size_t smem, cudaStream_t st, uint32_t grid_min = 1) {
     constexpr int NW = 8;
-    auto kern = ibp_stream_kernel<W, NS, NW, NSEG>;
+    auto kern = ibp_stream_kernel<W, NS, NW, NSEG, STAGED>;
     static unsigned long long smem_optin_done = 0;
     if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
@@ -648,7 +648,7 @@ static ibp_status launch_stream_one(const StreamBatch<NSEG>& B, int64_t total_ch
 // Chunk geometry of one contiguous run (or of n_spans spans) for the stream kernel.  `allow_tile_blocks`: resident decode of a
 // strided table may use tile-block chunks when the grid will have at least one CTA per tile block.
 static void stream_geometry(const ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
-                            int64_t first_row, int64_t span_rows, void* out_dev, bool allow_tile_blocks, StreamParams& P) {
+                            int64_t first_row, int64_t span_rows, void* out_dev, bool allow_tile_blocks, StreamParams& P, bool allow_staged = false) {
     const int W = pick_W(h->p.row_bytes);
     const uint32_t NW = 8;
     memset(&P, 0, sizeof P);
@@ -685,6 +685,18 @@ static void stream_geometry(const ibp_handle* h, const uint8_t* packed, uint64_t
         P.piece_rows = U;
         need = rc * h->max_stride + (rc / G + 2) * 128 + 64;
         P.chunks_per_span = (uint32_t)((span_rows + (int64_t)rc - 1) / (int64_t)rc);
+        // staged metadata (ibp_stream.cuh): [descriptor 32 B][group entries][Mask/Bitval of the chunk's groups] in front of the bytes
+        const uint64_t groups_max = rc < 2 ? 1 : (rc - 2) / G + 2;
+        const uint64_t meta_off = (32 + groups_max * 16 + 127) / 128 * 128, aux = meta_off + groups_max * 2 * h->p.row_bytes;
+        // Only for small groups (at least eight per chunk: KV pages of 16 rows), where every piece needs a fresh Mask/Bitval and the
+        // consumers' dependent global loads were the top stall (resident KV 0.80 -> 0.83 of the HBM peak); with groups of 128 / 256
+        // rows a warp keeps its prepared group across pieces and the extra stage traffic costs more than it saves (measured: GNN
+        // 0.87 -> 0.84, DLRM 0.84 -> 0.81), so those keep the consumer-side loads.
+        if (P.n_pass == 1 && P.fast_rows && h->p.row_bytes % 16 == 0 && aux <= 12ull * 1024 && G * 8 <= rc && allow_staged) {
+            P.aux_bytes = (uint32_t)((aux + 127) / 128 * 128);
+            P.aux_meta_off = (uint32_t)meta_off;
+            need += P.aux_bytes;
+        }
     } else if (allow_tile_blocks && P.n_pass == 1 && P.fast_rows && !ids_dev && n_spans == 1) {
         // resident decode of a strided table: tile-block chunks (ibp_stream.cuh).  A whole-row chunk holds only 2-7 matrix rows
         // of the 7B shapes, so every warp would re-prepare a tile (Mask/Bitval, offsets, expand masks) for a handful of rows;
@@ -732,13 +744,16 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
     memset(&B, 0, sizeof B);
     StreamParams& P = B.seg[0];
     const bool tile_ok = resident && (!h->max_ctas || h->max_ctas >= (h->n_groups + 7) / 8);
-    stream_geometry(h, packed, bias, ids_dev, n_spans, first_row, span_rows, out_dev, tile_ok, P);
+    stream_geometry(h, packed, bias, ids_dev, n_spans, first_row, span_rows, out_dev, tile_ok, P, true);
     B.n_seg = 1;
     B.stage_bytes = P.stage_bytes;
     const int ns = P.stage_bytes > 40 * 1024 ? 2 : 3;
     const size_t smem = (size_t)ns * P.stage_bytes + (size_t)ns * 16;
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
 #define IBP_STREAM(W_)                                                                                             \
+    if (P.aux_bytes)                                                                                               \
+        return ns == 2 ? launch_stream_one<W_, 2, 1, true>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st) \
+                       : launch_stream_one<W_, 3, 1, true>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st); \
     return ns == 2 ? launch_stream_one<W_, 2, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st) \
                    : launch_stream_one<W_, 3, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st)
     switch (W) {

@@ -38,6 +38,11 @@ struct StreamParams {
     // tiles, and chunk c belongs to block c % n_tile_blocks -- with a grid that is a multiple of n_tile_blocks every CTA
     // keeps ONE block, so consumer warp w decodes the same tile in every chunk and prepares it once.  0 = off.
     uint32_t n_tile_blocks;
+    // blocked groups, single-pass rows (round 2): the stage carries an aux region IN FRONT of the packed bytes -- a 32-byte chunk
+    // descriptor written by the producer, the group-table entries and Mask/Bitval of the groups the chunk touches (bulk copies) --
+    // so consumer warps read nothing from global memory.  aux_bytes = 0: off (consumers compute the geometry and load metadata
+    // themselves: strided tables, multi-pass rows, chunks that touch too many groups to stage).
+    uint32_t aux_bytes, aux_meta_off;
     uint32_t n_tiles;              // groups that exist: min(S, rows of the table) -- the group table has no entry beyond them
     uint32_t tb_pitch;             // bytes between the block's images of consecutive matrix rows inside a stage
 };
@@ -122,7 +127,31 @@ __global__ void ibp_build_mvtab(const uint32_t* __restrict__ meta, uint32_t n_wo
     for (int k = 0; k < 5; ++k) mvtab[i * 5 + k] = mv[k];
 }
 
-template <int W, int NS, int NW, int NSEG>
+template <int W> __device__ __forceinline__ void lds_words(uint32_t a, uint32_t (&v)[W]);
+template <> __device__ __forceinline__ void lds_words<1>(uint32_t a, uint32_t (&v)[1]) {
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[0]) : "r"(a));
+}
+template <> __device__ __forceinline__ void lds_words<2>(uint32_t a, uint32_t (&v)[2]) {
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(a));
+}
+template <> __device__ __forceinline__ void lds_words<4>(uint32_t a, uint32_t (&v)[4]) {
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(a));
+}
+// consumer-side wait with a suspend-time hint: a waiting warp stays off the issue port instead of polling
+__device__ __forceinline__ void mbar_wait_hint(uint32_t bar, uint32_t parity) {
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+    }
+}
+
+// STAGED: the aux region of StreamParams::aux_bytes is in use (single-segment launches of blocked tables with small groups); a
+// separate instantiation, so that the other launches keep exactly the code they had.
+template <int W, int NS, int NW, int NSEG, bool STAGED = false>
 __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __grid_constant__ StreamBatch<NSEG> B) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -210,16 +239,31 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __gr
         }
         for (int64_t c = c_first; c < P.n_chunks; c += gridDim.x, ++k) {
             const uint32_t s = k % NS;
-            mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
             int64_t row0, out0; uint32_t nrows; uint64_t b0, b1;
+            if constexpr (!STAGED) mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
             chunk_geom(c, row0, nrows, out0, b0, b1);
             const uint8_t* src = P.store + (b0 - P.bias);
             const uint32_t head = (uint32_t)((uintptr_t)src & 15u);
             const uint32_t bytes = (uint32_t)((head + (b1 - b0) + 15u) & ~15ull);
-            mbar_expect_tx(full_s + s * 8, bytes);
-            const uint32_t dst = smem_s + s * STAGE;
+            if constexpr (STAGED) mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);   // after the geometry: its loads overlap the consumers' work
+            const uint32_t dst = smem_s + s * STAGE, bar = full_s + s * 8;
+            if constexpr (STAGED) {
+                // staged metadata: descriptor by plain stores (made visible by the release of the arrive below), group-table entries
+                // and Mask/Bitval of groups g0 .. g1 by bulk copies (consecutive groups are contiguous in GPU memory)
+                const uint64_t g0 = group_of_u(P.group_param, P.group_shift, (uint64_t)row0);
+                const uint64_t g1 = group_of_u(P.group_param, P.group_shift, (uint64_t)row0 + nrows - 1);
+                const uint32_t ng = (uint32_t)(g1 - g0 + 1);
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(dst), "r"((uint32_t)row0), "r"((uint32_t)((uint64_t)row0 >> 32)),
+                             "r"((uint32_t)out0), "r"((uint32_t)((uint64_t)out0 >> 32)) : "memory");
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(dst + 16u), "r"(nrows), "r"(head), "r"((uint32_t)b0), "r"((uint32_t)(b0 >> 32)) : "memory");
+                mbar_expect_tx(bar, bytes + ng * 16u + ng * 2u * P.row_bytes);
+                bulk_g2s(dst + 32u, P.gtab + g0, ng * 16u, bar);
+                bulk_g2s(dst + P.aux_meta_off, P.meta + g0 * 2ull * P.n_words, ng * 2u * P.row_bytes, bar);
+            } else {
+                mbar_expect_tx(bar, bytes);
+            }
             for (uint32_t o = 0; o < bytes; o += 16384u)
-                bulk_g2s(dst + o, src - head + o, min(16384u, bytes - o), full_s + s * 8);
+                bulk_g2s(dst + (STAGED ? P.aux_bytes : 0u) + o, src - head + o, min(16384u, bytes - o), bar);
         }
         if (NSEG == 1) return;
         continue;
@@ -238,9 +282,11 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __gr
     const bool fast = P.n_pass == 1 && P.fast_rows;
     const bool active_fast = w0_fast < P.n_words;
 
-    auto prepare = [&](uint64_t g) {   // S2 + S4 for a single-pass row of group g
+    // meta_s != 0: shared address of the group's staged [Mask][Bitval] record
+    auto prepare = [&](uint64_t g, uint32_t meta_s = 0u) {   // S2 + S4 for a single-pass row of group g
         const uint32_t* gm = P.meta + g * 2ull * P.n_words;
-        if (active_fast) { VecIO<W>::ld(gm + w0_fast, m); VecIO<W>::ld(gm + P.n_words + w0_fast, b); }
+        if (STAGED && active_fast && meta_s) { lds_words<W>(meta_s + w0_fast * 4u, m); lds_words<W>(meta_s + P.row_bytes + w0_fast * 4u, b); }
+        else if (active_fast) { VecIO<W>::ld(gm + w0_fast, m); VecIO<W>::ld(gm + P.n_words + w0_fast, b); }
         else {
 #pragma unroll
             for (int q = 0; q < W; ++q) { m[q] = 0xFFFFFFFFu; b[q] = 0; }
@@ -360,6 +406,42 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __gr
             mbar_wait(full_s + s * 8, (k / NS) & 1u);
             if (cnt > 0)
                 decode_run(smem_s + s * STAGE + toff, P.tb_pitch, P.out + ((uint64_t)mr0 * S + t) * P.row_bytes, S * P.row_bytes, (uint32_t)cnt);
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
+        }
+        if (NSEG == 1) return;
+        continue;
+    }
+    if constexpr (STAGED) {
+        // staged chunks (blocked groups, single-pass rows): descriptor, group entries and Mask/Bitval come out of the stage
+        const uint32_t U = P.piece_rows;
+        for (int64_t c = c_first; c < P.n_chunks; c += gridDim.x, ++k) {
+            const uint32_t s = k % NS, stage_s = smem_s + s * STAGE;
+            mbar_wait_hint(full_s + s * 8, (k / NS) & 1u);
+            uint32_t d0[4], d1[4];
+            lds_words<4>(stage_s, d0);
+            lds_words<4>(stage_s + 16u, d1);
+            const uint64_t row0 = ((uint64_t)d0[1] << 32) | d0[0], out0 = ((uint64_t)d0[3] << 32) | d0[2];
+            const uint32_t nrows = d1[0], head = d1[1];
+            const uint64_t b0 = ((uint64_t)d1[3] << 32) | d1[2];
+            const uint64_t g0 = group_of_u(P.group_param, P.group_shift, row0);
+            const uint32_t n_pieces = (nrows + U - 1) / U;
+            for (uint32_t p = wib; p < n_pieces; p += NW) {
+                uint32_t j = p * U;
+                const uint32_t j1 = min(nrows, j + U);
+                while (j < j1) {                                   // runs of rows of one group inside the piece
+                    const uint64_t id = row0 + j;
+                    const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
+                    const uint32_t run = (uint32_t)min((uint64_t)(j1 - j), (g + 1) * S - id);
+                    uint32_t e[4];                                 // IbpGroupEntry {base lo, base hi, stride, k_bits}
+                    lds_words<4>(stage_s + 32u + (uint32_t)(g - g0) * 16u, e);
+                    const uint64_t base = ((uint64_t)e[1] << 32) | e[0];
+                    const uint32_t roff = head + (uint32_t)(base + (id - g * S) * e[2] - b0);
+                    if (g != prep_g) prepare(g, stage_s + P.aux_meta_off + (uint32_t)(g - g0) * 2u * P.row_bytes);
+                    decode_run(stage_s + P.aux_bytes + roff, e[2], P.out + (out0 + j) * P.row_bytes, P.row_bytes, run);
+                    j += run;
+                }
+            }
             __syncwarp();
             if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
         }

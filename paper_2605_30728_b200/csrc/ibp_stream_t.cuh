@@ -405,7 +405,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 const uint32_t meta_bytes = P.aux_meta_off ? (uint32_t)(g1 - g0 + 1) * row_bytes2 : 0u;
                 const uint32_t bytes = (a1 - a0) * 16u;
                 const uint32_t stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap, bar = full_s + s * 8;
-                mbar_wait_relaxed(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);
+                mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);      // the producer polls: a suspended wait reacts later and the refill starts late
                 asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s), "r"((uint32_t)first), "r"((uint32_t)((uint64_t)first >> 32)),
                              "r"((uint32_t)(out0 + r0)), "r"((uint32_t)((uint64_t)(out0 + r0) >> 32)) : "memory");
                 asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s + 16u), "r"(n), "r"(a0), "r"(r1 == nrows ? 1u : 0u), "r"(0u) : "memory");
