@@ -28,7 +28,7 @@ void ibp_set_error(const char* fmt, ...) {
     va_end(ap);
 }
 extern "C" const char* ibp_last_error(void) { return g_err; }
-extern "C" const char* ibp_version(void) { return "ibp-b200 0.3 (sm_100a; group-strict and thresholded IBP, GPU build, compressed cache, mask tools)"; }
+extern "C" const char* ibp_version(void) { return "ibp-b200 0.4 (sm_100a; group-strict and thresholded IBP, GPU build and append, compressed multi-GPU cache, shared store, mask tools)"; }
 
 // ------------------------------------------------------------------------------------------------ bit helpers
 static inline uint64_t pext64_soft(uint64_t v, uint64_t m) {
