@@ -832,19 +832,39 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
         // 8-row pieces do not fit is a chunk above a stage loaded as sub-units of split_rows rows.
         const uint64_t STAGE = 38144;
         const uint64_t G = h->p.group_param;
-        uint32_t U = lpr == 32 ? 16u : 32u;
-        uint64_t rc = 0, data_cap = 0;
-        for (;; U >>= 1) {
-            rc = (uint64_t)std::min<int64_t>((int64_t)NW * U, span_rows);
-            const uint64_t off_max = ((rc + 1 + 3 + 3 + 3) & ~3ull) * 4, flag_max = ((rc / 32 + 2 + 3 + 3) & ~3ull) * 4 + 16;
-            const uint64_t groups_max = rc < 2 ? 1 : (rc - 2) / G + 2, meta_max = groups_max * 2 * h->p.row_bytes;
+        auto layout = [&](uint32_t U_, uint64_t& rc_, uint64_t& cap_) {     // aux layout and data capacity of a unit of NW pieces of U_ rows
+            rc_ = (uint64_t)std::min<int64_t>((int64_t)NW * U_, span_rows);
+            const uint64_t off_max = ((rc_ + 1 + 3 + 3 + 3) & ~3ull) * 4, flag_max = ((rc_ / 32 + 2 + 3 + 3) & ~3ull) * 4 + 16;
+            const uint64_t groups_max = rc_ < 2 ? 1 : (rc_ - 2) / G + 2, meta_max = groups_max * 2 * h->p.row_bytes;
             P.aux_flag_off = (uint32_t)(32 + off_max);                        // [descriptor 32 B][row offsets][row flags][Mask/Bitval]
             const uint64_t meta_off = (P.aux_flag_off + flag_max + 127) / 128 * 128;
             const bool stage_meta = meta_max <= 8192;                        // small groups (a Mask/Bitval pair per row or two) stay in global memory
             P.aux_meta_off = stage_meta ? (uint32_t)meta_off : 0u;
             P.aux_bytes = (uint32_t)(stage_meta ? meta_off + meta_max : meta_off);
-            data_cap = STAGE - P.aux_bytes;
+            cap_ = STAGE - P.aux_bytes;
+        };
+        uint32_t U = lpr == 32 ? 16u : 32u;
+        uint64_t rc = 0, data_cap = 0;
+        for (;; U >>= 1) {                                                   // worst case: every row raw
+            layout(U, rc, data_cap);
             if (rc * stride + 64 <= data_cap || U <= 8) break;
+        }
+        // Larger pieces when the rows the table actually stores are well below the raw size (GNN: 289 of 512 bytes): a unit sized
+        // for the table's AVERAGE stored row with 10 % to spare amortises the per-piece work over more rows; the rare unit that
+        // exceeds a stage is split.  Only when groups are long against the piece (a piece that straddles a group boundary takes the
+        // slower run-by-run path) or the piece divides / is a multiple of the group.
+        {
+            const uint64_t avg = std::max<uint64_t>(16, (h->packed_bytes_rows + h->p.n_rows - 1) / std::max<uint64_t>(1, h->p.n_rows));
+            const uint32_t gran = 2u * (32u / lpr);                          // two passes of 32/LPR rows
+            for (uint32_t Ut = 32u / gran * gran; Ut > U; Ut -= gran) {
+                if (!(G >= 8ull * Ut || G % Ut == 0 || Ut % G == 0)) continue;
+                uint64_t rct, capt;
+                layout(Ut, rct, capt);
+                if (rct < (uint64_t)NW * Ut) continue;                       // short spans: keep the worst-case size
+                const uint64_t split_rows = ((capt - 64) / stride) / Ut * Ut;
+                if (rct * avg * 11 / 10 + 64 <= capt && split_rows >= Ut) { U = Ut; break; }
+            }
+            layout(U, rc, data_cap);
         }
         P.rows_per_chunk = (uint32_t)rc;
         P.piece_rows = U;
