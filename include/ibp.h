@@ -237,6 +237,13 @@ typedef struct {
 } ibp_range_desc;
 ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint32_t n_ranges, void* cuda_stream);
 
+/* The same with HOST destinations: the out_dev field of every range holds a HOST pointer that receives n_rows*row_bytes bytes.
+ * When all destinations are pinned, GPU-mapped memory (cudaHostAlloc / cudaHostRegister / ibp_host_alloc) the decode kernels store
+ * into them directly, with the batching of ibp_decode_ranges (a 7-matrix layer: one launch); otherwise every range goes through
+ * ibp_gather_decompress_range_host (device staging buffer + copy; packed_dev ranges then are UNSUPPORTED).  Synchronises the
+ * stream before returning.  Errors as ibp_decode_ranges.                                                                     */
+ibp_status ibp_decode_ranges_host(const ibp_range_desc* ranges_host, uint32_t n_ranges, void* cuda_stream);
+
 /* Byte range of the packed store that holds rows [first_row, first_row+n_rows) (same unit rule as above).         */
 ibp_status ibp_packed_range(const ibp_handle* h, int64_t first_row, int64_t n_rows, const void** host_ptr, uint64_t* nbytes);
 

@@ -87,6 +87,7 @@ SIGNATURES = {
     "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_gather_decompress_range_host": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_decode_ranges": (_int, [C.POINTER(ibp_range_desc), _u32, _vp]),
+    "ibp_decode_ranges_host": (_int, [C.POINTER(ibp_range_desc), _u32, _vp]),
     "ibp_packed_range": (_int, [_vp, _i64, _i64, C.POINTER(_vp), C.POINTER(_u64)]),
     "ibp_store_device_ptr": (_int, [_vp, C.POINTER(_vp)]),
     "ibp_packed_row": (_int, [_vp, _i64, C.POINTER(_vp), C.POINTER(_u32), C.POINTER(_u32)]),
@@ -405,6 +406,14 @@ def ibp_decode_ranges(ranges, stream=None):
     for a, (h, packed, first, n, out) in zip(arr, ranges):
         a.handle, a.packed_dev, a.first_row, a.n_rows, a.out_dev = h._h.value if hasattr(h._h, "value") else h._h, _ptr(packed), first, n, _ptr(out)
     _check(lib().ibp_decode_ranges(arr, len(ranges), stream))
+
+
+def ibp_decode_ranges_host(ranges, stream=None):
+    """ranges: [(Handle, packed_dev or None, first_row, n_rows, out_host: numpy array or address), ...]; synchronises the stream."""
+    arr = (ibp_range_desc * len(ranges))()
+    for a, (h, packed, first, n, out) in zip(arr, ranges):
+        a.handle, a.packed_dev, a.first_row, a.n_rows, a.out_dev = h._h.value if hasattr(h._h, "value") else h._h, _ptr(packed), first, n, _ptr(out)
+    _check(lib().ibp_decode_ranges_host(arr, len(ranges), stream))
 
 
 def ibp_gather_uncompressed(rows_mapped, row_bytes, row_ids_dev, n, out_dev, stream=None, n_rows=0, locality_order=False):

@@ -1298,6 +1298,41 @@ extern "C" ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint3
     return IBP_OK;
 }
 
+// ibp_decode_ranges with HOST destinations.  When every destination is pinned, GPU-mapped memory the ranges are decoded by the
+// batched launches of ibp_decode_ranges, the kernels storing straight into host memory (one launch and one synchronisation per
+// layer instead of seven); otherwise range by range through ibp_gather_decompress_range_host (staging buffer + copy).
+extern "C" ibp_status ibp_decode_ranges_host(const ibp_range_desc* ranges_host, uint32_t n_ranges, void* cuda_stream) {
+    if (n_ranges == 0) return IBP_OK;
+    if (!ranges_host) { ibp_set_error("ibp_decode_ranges_host: null range list"); return IBP_ERR_INVALID_ARG; }
+    std::vector<ibp_range_desc> dev;
+    try { dev.assign(ranges_host, ranges_host + n_ranges); } catch (...) { ibp_set_error("ibp_decode_ranges_host: out of memory"); return IBP_ERR_OUT_OF_MEMORY; }
+    bool direct = true;
+    for (uint32_t i = 0; i < n_ranges && direct; ++i) {
+        if (dev[i].n_rows == 0) continue;
+        if (!dev[i].out_dev) { ibp_set_error("ibp_decode_ranges_host: null destination in range %u", i); return IBP_ERR_INVALID_ARG; }
+        cudaPointerAttributes attr;
+        void* alias = nullptr;
+        if (cudaPointerGetAttributes(&attr, dev[i].out_dev) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+            cudaHostGetDevicePointer(&alias, dev[i].out_dev, 0) == cudaSuccess && alias && !((uintptr_t)alias & 15u)) dev[i].out_dev = alias;
+        else direct = false;
+    }
+    (void)cudaGetLastError();
+    if (direct) {
+        ibp_status s = ibp_decode_ranges(dev.data(), n_ranges, cuda_stream);
+        const cudaError_t es = cudaStreamSynchronize((cudaStream_t)cuda_stream);
+        if (s == IBP_OK && es != cudaSuccess) { ibp_set_error("ibp_decode_ranges_host: %s", cudaGetErrorString(es)); (void)cudaGetLastError(); s = IBP_ERR_CUDA; }
+        return s;
+    }
+    for (uint32_t i = 0; i < n_ranges; ++i) {
+        const ibp_range_desc& r = ranges_host[i];
+        if (r.n_rows == 0) continue;
+        if (r.packed_dev) { ibp_set_error("ibp_decode_ranges_host: a range with packed_dev needs a pinned, GPU-mapped destination"); return IBP_ERR_UNSUPPORTED; }
+        ibp_status s = ibp_gather_decompress_range_host(r.handle, r.first_row, r.n_rows, r.out_dev, cuda_stream);
+        if (s != IBP_OK) return s;
+    }
+    return IBP_OK;
+}
+
 // Host-buffer entry point.  Large batches are cut into chunks so that the device->host copy of chunk c (copy engine, PCIe
 // writes) overlaps the gather of chunk c+1 (SM-issued PCIe reads): the two directions of the link work at the same time.
 extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* row_ids_host, int64_t n, void* out_host, void* cuda_stream) {

@@ -106,6 +106,31 @@ def test_ragged_shapes_gather_and_resident(kind, param, n, rb, align):
     h.destroy()
 
 
+def test_decode_ranges_host_destinations():
+    """ibp_decode_ranges_host: several ranges of several handles into HOST buffers -- pinned and GPU-mapped (the kernels store
+    straight into them, batched launches) and ordinary pageable memory (range by range through a staging buffer)."""
+    mats = []
+    for j, (S, n, rb) in enumerate([(8, 8 * 50, 256), (8, 8 * 31 + 3, 256), (5, 203, 256), (16, 16 * 20, 256)]):
+        X = (datagen.random_bytes(n * rb, 40 + j).reshape(n, rb) & datagen.random_bytes(rb, 60 + j)[None, :]) | 0x01
+        mats.append((ibp.ibp_build(X, rb, 1, S, align_bytes=16).upload_metadata(0), X))
+    Xb = (datagen.random_bytes(300 * 256, 7).reshape(300, 256) & 0x3F) | 0x40
+    mats.append((ibp.ibp_build(Xb, 256, 0, 64, align_bytes=16, threshold=(4, 5)).upload_metadata(0), Xb))   # a thresholded handle in the list
+    total = sum(len(X) for _, X in mats)
+    st = torch.cuda.current_stream().cuda_stream
+    pin = ibp.PinnedBuffer(total * 256)
+    for name, dest in (("pinned", pin.view(np.uint8, (total, 256))), ("pageable", np.zeros((total, 256), np.uint8))):
+        dest[:] = 0xEE
+        rs, off = [], 0
+        for h, X in mats:
+            rs.append((h, None, 0, len(X), dest[off:off + len(X)]))
+            off += len(X)
+        ibp.ibp_decode_ranges_host(rs, st)
+        assert np.array_equal(dest, np.concatenate([X for _, X in mats])), name
+    pin.free()
+    for h, _ in mats:
+        h.destroy()
+
+
 @pytest.mark.parametrize("S,n,rb,align", [(86, 86 * 40 + 13, 256, 16), (32, 32 * 70, 256, 16), (9, 9 * 33 + 4, 512, 32), (16, 16 * 5, 64, 4),
                                            (17, 17 * 100 + 16, 128, 16), (8, 8 * 3 + 1, 256, 32), (3, 50, 512, 16), (40, 40 * 64 + 39, 128, 4)])
 def test_strided_resident_tile_blocks(S, n, rb, align):
