@@ -478,14 +478,17 @@ def test_T_ragged_shapes_gather_and_resident(kind, param, n, rb, align, thr):
     h.destroy()
 
 
-@pytest.mark.parametrize("rb,G,n,raw_frac", [(512, 64, 1500, 1.0), (256, 16, 3000, 1.0), (512, 256, 2000, 0.6), (256, 128, 2500, 0.5), (128, 8, 900, 1.0)])
+@pytest.mark.parametrize("rb,G,n,raw_frac", [(512, 64, 1500, 1.0), (256, 16, 3000, 1.0), (512, 256, 2000, 0.6), (256, 128, 2500, 0.5), (128, 8, 900, 1.0),
+                                             (512, 256, 3000, -0.7), (256, 512, 4000, -0.8)])
 def test_T_chunks_larger_than_a_stage(rb, G, n, raw_frac):
     """Thresholded stream decode when most rows are kept raw: a chunk of NW pieces then exceeds one shared-memory stage
     and is loaded as sub-loads into consecutive stages; the producer and every consumer warp take that decision from the same
     two row offsets.  Contiguous ranges from the host store, resident decode, ranges starting off a group boundary, spans."""
     rng = np.random.default_rng(rb + n)
     X = _perturbed(n, rb, 3 * rb + n)
-    raw = rng.random(n) < raw_frac
+    # raw_frac < 0: the raw rows are the TAIL of the table (from |raw_frac| * n on), so the table's average stored row is small -- units
+    # are sized for it -- while every unit of the tail exceeds a stage and is split
+    raw = rng.random(n) < raw_frac if raw_frac >= 0 else np.arange(n) >= int(-raw_frac * n)
     X[raw] = rng.integers(0, 256, size=(int(raw.sum()), rb), dtype=np.uint8)
     h = ibp.ibp_build(X, rb, 0, G, align_bytes=16, threshold=(4, 5)).upload_metadata(0)
     ds = oracle.DatasetT(X, 0, G, 4, 5)
