@@ -505,6 +505,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_kernel(const __gr
                     const uint32_t* ngm = P.meta + ng * 2ull * P.n_words + w0_fast;
                     asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm));
                     asm volatile("prefetch.global.L1 [%0];" ::"l"(ngm + P.n_words));
+                    // ... and with the group-table entries its geometry starts from (two dependent loads at the head of the chunk)
+                    if (lane == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.gtab + group_of_u(P.group_param, P.group_shift, (uint64_t)nrow0)));
+                    if (lane == 1) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.gtab + ng));
                 }
             }
             for (uint32_t p = wib; p < n_pieces; p += NW) {
