@@ -788,7 +788,7 @@ def measure_weights(ctx, args, K, W, layers, overlap, cpu):
         check_on[0] = False                                     # timing runs: the consumer is the GEMMs alone
         ov = summarize(pipe.run_fetch_only(), pipe.run_consume_only(), pipe.run_serial(), pipe.run_overlapped())
         ov.update({"steps": n_pipe, "consumer": f"torch.matmul [M={M},4096] bf16 x the 7 decoded matrices of the previous layer (cuBLAS)",
-                   "decode_ctas": args.decode_ctas or "library default (persistent, occupancy x SMs)",
+                   "decode_ctas": args.decode_ctas or "library default (host-store streams: 48 CTAs)",
                    "checked": f"all {n_pipe} overlapped steps: 64-bit checksum of the consumed buffer == that of a serial fetch of the same layer; whole-buffer bytes == the original matrices for steps {sorted(kept)}"})
         extras["overlap"] = ov
     if cpu:

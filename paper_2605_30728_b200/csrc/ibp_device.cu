@@ -736,9 +736,19 @@ static void stream_geometry(const ibp_handle* h, const uint8_t* packed, uint64_t
     P.n_chunks = n_spans * (int64_t)P.chunks_per_span;
 }
 
+// Grid limit of a contiguous-run launch.  A stream that reads the HOST store is bound by the link, which 24 CTAs already saturate
+// (measured: a weight layer 62.77 GB/s with 24, 48, 64, 96 CTAs or the full persistent grid; KV spans 63.2 with 32, 64 or all), so
+// unless ibp_configure says otherwise it takes 48 CTAs and leaves the other SMs to whoever consumes the rows ("We reserved
+// only 64 SMs for decompression"): overlapped with a GEMM on the previous layer, 8 layers take 68.6 ms instead of 102.5 ms with the
+// full grid (ideal 64.5).  Resident decode (HBM source) is bound by HBM and the integer pipe and keeps the whole GPU.
+static inline int64_t stream_ctas(const ibp_handle* h, bool hbm_source) {
+    return h->max_ctas ? (int64_t)h->max_ctas : (hbm_source ? 0 : 48);
+}
+
 static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
                                 int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st, bool resident = false) {
     if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+    const int64_t max_ctas = stream_ctas(h, resident);
     const int W = pick_W(h->p.row_bytes);
     StreamBatch<1> B;
     memset(&B, 0, sizeof B);
@@ -752,10 +762,10 @@ static ibp_status launch_stream(ibp_handle* h, const uint8_t* packed, uint64_t b
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory stages", h->max_stride); return IBP_ERR_UNSUPPORTED; }
 #define IBP_STREAM(W_)                                                                                             \
     if (P.aux_bytes)                                                                                               \
-        return ns == 2 ? launch_stream_one<W_, 2, 1, true>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st) \
-                       : launch_stream_one<W_, 3, 1, true>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st); \
-    return ns == 2 ? launch_stream_one<W_, 2, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st) \
-                   : launch_stream_one<W_, 3, 1>(B, P.n_chunks, P.n_tile_blocks, h->max_ctas, h->sm_count, smem, st)
+        return ns == 2 ? launch_stream_one<W_, 2, 1, true>(B, P.n_chunks, P.n_tile_blocks, max_ctas, h->sm_count, smem, st) \
+                       : launch_stream_one<W_, 3, 1, true>(B, P.n_chunks, P.n_tile_blocks, max_ctas, h->sm_count, smem, st); \
+    return ns == 2 ? launch_stream_one<W_, 2, 1>(B, P.n_chunks, P.n_tile_blocks, max_ctas, h->sm_count, smem, st) \
+                   : launch_stream_one<W_, 3, 1>(B, P.n_chunks, P.n_tile_blocks, max_ctas, h->sm_count, smem, st)
     switch (W) {
         case 4: IBP_STREAM(4);
         case 2: IBP_STREAM(2);
@@ -804,8 +814,9 @@ static bool stream_t_fits(const ibp_handle* h) {
 }
 
 static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t bias, const int64_t* ids_dev, int64_t n_spans,
-                                  int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st) {
+                                  int64_t first_row, int64_t span_rows, void* out_dev, cudaStream_t st, bool resident = false) {
     if (n_spans <= 0 || span_rows <= 0) return IBP_OK;
+    const int64_t max_ctas = stream_ctas(h, resident);
     const int W = pick_W(h->p.row_bytes);
     const uint32_t NW = 8;
     StreamTParams P;
@@ -911,11 +922,11 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
         const int nr = (h->max_runs >= 1 && h->max_runs <= 4) ? h->max_runs : 0;      // bf16 pairs: mantissa + sign per half = 4 runs
 #define IBP_T2_NR(LPR_, NS_)                                                                              \
         switch (nr) {                                                                                     \
-            case 1: return launch_stream_t2_one<LPR_, NS_, 1>(P, h->max_ctas, h->sm_count, smem, st);     \
-            case 2: return launch_stream_t2_one<LPR_, NS_, 2>(P, h->max_ctas, h->sm_count, smem, st);     \
-            case 3: return launch_stream_t2_one<LPR_, NS_, 3>(P, h->max_ctas, h->sm_count, smem, st);     \
-            case 4: return launch_stream_t2_one<LPR_, NS_, 4>(P, h->max_ctas, h->sm_count, smem, st);     \
-            default: return launch_stream_t2_one<LPR_, NS_, 0>(P, h->max_ctas, h->sm_count, smem, st);    \
+            case 1: return launch_stream_t2_one<LPR_, NS_, 1>(P, max_ctas, h->sm_count, smem, st);     \
+            case 2: return launch_stream_t2_one<LPR_, NS_, 2>(P, max_ctas, h->sm_count, smem, st);     \
+            case 3: return launch_stream_t2_one<LPR_, NS_, 3>(P, max_ctas, h->sm_count, smem, st);     \
+            case 4: return launch_stream_t2_one<LPR_, NS_, 4>(P, max_ctas, h->sm_count, smem, st);     \
+            default: return launch_stream_t2_one<LPR_, NS_, 0>(P, max_ctas, h->sm_count, smem, st);    \
         }
 #define IBP_T2(LPR_) { IBP_T2_NR(LPR_, 2) }                                                            /* t2: always two stages */
         if (lpr == 32) { IBP_T2(32) }
@@ -926,10 +937,10 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     }
     const bool runs = h->max_runs >= 0 && h->max_runs <= 3;
 #define IBP_STREAM_T(W_)                                                                                         \
-    if (runs) return ns == 2 ? launch_stream_t_one<W_, 2, true>(P, h->max_ctas, h->sm_count, smem, st)           \
-                             : launch_stream_t_one<W_, 3, true>(P, h->max_ctas, h->sm_count, smem, st);          \
-    return ns == 2 ? launch_stream_t_one<W_, 2, false>(P, h->max_ctas, h->sm_count, smem, st)                    \
-                   : launch_stream_t_one<W_, 3, false>(P, h->max_ctas, h->sm_count, smem, st)
+    if (runs) return ns == 2 ? launch_stream_t_one<W_, 2, true>(P, max_ctas, h->sm_count, smem, st)           \
+                             : launch_stream_t_one<W_, 3, true>(P, max_ctas, h->sm_count, smem, st);          \
+    return ns == 2 ? launch_stream_t_one<W_, 2, false>(P, max_ctas, h->sm_count, smem, st)                    \
+                   : launch_stream_t_one<W_, 3, false>(P, max_ctas, h->sm_count, smem, st)
     switch (W) {
         case 4: IBP_STREAM_T(4);
         case 2: IBP_STREAM_T(2);
@@ -1132,7 +1143,7 @@ static ibp_status decode_range(ibp_handle* h, const uint8_t* packed, int64_t fir
     // (slot layout: consecutive rows are not contiguous in the store -- only the head of every slot is meaningful -- so runs
     // take the per-row kernel, which fetches exactly each row's bytes)
     if (h->stream_mode && h->thresholded && !h->slot_layout && stream_t_fits(h))
-        return launch_stream_t(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st);
+        return launch_stream_t(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st, resident);
     if (h->stream_mode && !h->thresholded)
         return launch_stream(h, packed, ibp_row_offset(h, (uint64_t)first_row), nullptr, 1, first_row, n_rows, out_dev, st, resident);
     DecodeParams P;
@@ -1266,6 +1277,7 @@ extern "C" ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint3
         int64_t total = 0;
         uint32_t n_seg = 0, grid_min = 1;
         const int64_t grid_cap = h0->max_ctas ? (int64_t)h0->max_ctas : 2ll * h0->sm_count;
+        bool all_host = true;
         while (i < n_ranges && n_seg < 8) {
             const ibp_range_desc& r = ranges_host[i];
             if (r.n_rows == 0) { ++i; continue; }
@@ -1274,6 +1286,7 @@ extern "C" ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint3
             const bool tile_ok = r.packed_dev != nullptr && grid_cap >= (int64_t)((r.handle->n_groups + 7) / 8);
             stream_geometry(r.handle, source(r), ibp_row_offset(r.handle, (uint64_t)r.first_row), nullptr, 1, r.first_row, r.n_rows, r.out_dev, tile_ok, P);
             B.chunk_start[n_seg] = total;
+            all_host = all_host && r.packed_dev == nullptr;
             total += P.n_chunks;
             B.stage_bytes = std::max(B.stage_bytes, P.stage_bytes);
             grid_min = std::max(grid_min, P.n_tile_blocks);
@@ -1285,8 +1298,8 @@ extern "C" ibp_status ibp_decode_ranges(const ibp_range_desc* ranges_host, uint3
         if (smem > 220 * 1024) { ibp_set_error("ibp_decode_ranges: packed rows do not fit the shared-memory stages"); return IBP_ERR_UNSUPPORTED; }
         ibp_status s;
 #define IBP_STREAM_B(W_)                                                                                              \
-    s = ns == 2 ? launch_stream_one<W_, 2, 8>(B, total, 1, h0->max_ctas, h0->sm_count, smem, st, grid_min)              \
-                : launch_stream_one<W_, 3, 8>(B, total, 1, h0->max_ctas, h0->sm_count, smem, st, grid_min)
+    s = ns == 2 ? launch_stream_one<W_, 2, 8>(B, total, 1, stream_ctas(h0, !all_host), h0->sm_count, smem, st, grid_min)   \
+                : launch_stream_one<W_, 3, 8>(B, total, 1, stream_ctas(h0, !all_host), h0->sm_count, smem, st, grid_min)
         switch (W) {
             case 4: IBP_STREAM_B(4); break;
             case 2: IBP_STREAM_B(2); break;
