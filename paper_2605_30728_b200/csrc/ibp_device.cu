@@ -553,8 +553,8 @@ static ibp_status launch_one(const DecodeParams& P, int64_t blocks_needed, int64
     if (smem > 48 * 1024) IBP_CUDA(ibp_optin_max_smem(kern, &smem_optin_done));
     int occ = 0;
     IBP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
-    // random rows: 2 CTAs per SM keep enough reads in flight for the link; more only widens the window of store pages touched
-    // at once (measured: DLRM 0.716 -> 0.685 ms, GNN 1.388 -> 1.375 ms per batch)
+    // random rows: at most 2 CTAs per SM (1 for rows of a line or more, see gather_rows) keep enough reads in flight for the link;
+    // more only widens the window of store pages touched at once (measured: DLRM 0.716 -> 0.685 ms, GNN 1.388 -> 1.375 ms per batch)
     if (MODE == MODE_ROWS) occ = std::min(occ, P.occ_cap ? (int)P.occ_cap : 2);
     int64_t blocks = std::min<int64_t>(blocks_needed, (int64_t)std::max(occ, 1) * sm_count);
     if (max_ctas) blocks = std::min<int64_t>(blocks, max_ctas);
@@ -1068,6 +1068,12 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
         // A small cache leaves the misses in charge, and for them a wider window of store pages in flight costs more than it
         // gains (DLRM, 2 %: 314 -> 280 GB/s with 4 CTAs per SM), so the cap of the uncached gather stays.
         if (c->n_entries * 12 >= h->p.n_rows) P.occ_cap = 4;
+    } else if (h->p.n_rows && h->packed_bytes_rows / h->p.n_rows >= 96 && h->p.row_bytes <= 512) {
+        // Rows of about a line or more are bound by link bytes, and ONE CTA per SM (8 warps x 2 rows in flight) already keeps the
+        // link busy: measured three times each, alternating, GNN 1.371 ms with 148 CTAs against 1.383 with 296, DLRM 0.6347 against
+        // 0.6378 -- and half the registers and warp slots of every SM stay free for whatever runs beside the gather.  Smaller packed
+        // rows are bound by rows per second, and rows of several passes (4 KB: 2-5 % slower with one CTA) by decode latency: both keep two.
+        P.occ_cap = 1;
     }
     const bool dedup = allow_dedup && (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
     // automatic: large batches over large stores are processed in store-address order (address translation, DESIGN 6).
