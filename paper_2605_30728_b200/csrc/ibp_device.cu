@@ -572,7 +572,14 @@ static int pick_W(uint32_t row_bytes) {
 static ibp_status launch_decode(ibp_handle* h, DecodeParams& P, int mode, cudaStream_t st) {
     if (P.n_units <= 0) return IBP_OK;
     const int W = pick_W(h->p.row_bytes);
-    const int nst = mode == MODE_ROWS ? h->rows_in_flight : 4;
+    // rows each warp keeps in flight.  Automatic: about 300 KB of packed bytes in flight over the whole GPU was the optimum of both
+    // locality-ordered gathers measured (GNN, 252-byte rows on average: 1,184 rows = one per warp, 1.351 ms against 1.370 with two
+    // and 1.41 with four; DLRM, 128-byte rows: 2,368 rows = two per warp, 0.633 ms against 0.663 with one; thresholded GNN, 213
+    // bytes: two, 1.308 against 1.318), so an ORDERED gather with one CTA per SM keeps one row per warp in flight when the average
+    // stored row is 240 bytes or more, and two otherwise (unordered gathers over small stores: two was better, 50.0 against 46.9 GB/s).
+    int nst = 4;
+    if (mode == MODE_ROWS) nst = h->rows_in_flight ? h->rows_in_flight
+                                 : (P.occ_cap == 1 && P.order && h->packed_bytes_rows / std::max<uint64_t>(1, h->p.n_rows) >= 240 ? 1 : 2);
     P.n_pass = (h->n_words + 32 * W - 1) / (32 * W);
     P.slot_bytes = ((h->max_stride + 15u) / 16u) * 16u + 48u;   // 16-byte head + tail cover + one spare word
     P.slot_bytes = (P.slot_bytes + 127u) / 128u * 128u;
@@ -1716,7 +1723,7 @@ extern "C" ibp_status ibp_set_stream_mode(ibp_handle* h, int mode) {
 
 // Test/tuning hook: engine for the packed-row fetch: 0 = cp.async through the LSU, 1 = cp.async.bulk (TMA) + mbarrier.
 extern "C" ibp_status ibp_set_rows_in_flight(ibp_handle* h, int nst) {
-    if (!h || (nst != 1 && nst != 2 && nst != 4)) { ibp_set_error("ibp_set_rows_in_flight: 1, 2 or 4"); return IBP_ERR_INVALID_ARG; }
+    if (!h || (nst != 0 && nst != 1 && nst != 2 && nst != 4)) { ibp_set_error("ibp_set_rows_in_flight: 0 (automatic), 1, 2 or 4"); return IBP_ERR_INVALID_ARG; }
     h->rows_in_flight = nst;
     return IBP_OK;
 }

@@ -85,7 +85,7 @@ struct ibp_handle {
     uint32_t max_ctas = 0, warps_per_cta = 0;
     int sm_count = 0;
     int order_mode = -1;                   // -1 auto, 0 off, 1 on (locality-ordered gather)
-    int rows_in_flight = 2;                // random gathers: rows each warp keeps in flight (1, 2 or 4)
+    int rows_in_flight = 0;                // random gathers: rows each warp keeps in flight (1, 2 or 4); 0 = automatic
     int dedup_mode = -1;                   // random gathers: 1 = fetch each distinct id once, replicate in HBM; -1 auto
     int stream_mode = 1;                   // contiguous runs: 1 = TMA pipeline stream kernel, 0 = per-row fetch
     int fetch_mode = 1;                    // 0 = cp.async (LSU), 1 = cp.async.bulk (TMA)
