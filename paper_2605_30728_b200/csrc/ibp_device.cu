@@ -1056,7 +1056,7 @@ extern "C" ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_
 
 // Random row gather (index_span 1): pre-passes, decode kernel, replication of repeats.  `c` = optional compressed GPU cache.
 static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* row_ids_dev, int64_t n, void* out_dev, cudaStream_t st,
-                              bool allow_dedup = true) {
+                              bool allow_dedup = true, bool host_out = false) {
     if (n > 0x7FFFFFFF) { ibp_set_error("ibp_gather_decompress: n too large"); return IBP_ERR_INVALID_ARG; }
     DecodeParams P;
     fill_common(h, P);
@@ -1075,11 +1075,13 @@ static ibp_status gather_rows(ibp_handle* h, const ibp_cache* c, const int64_t* 
         // A small cache leaves the misses in charge, and for them a wider window of store pages in flight costs more than it
         // gains (DLRM, 2 %: 314 -> 280 GB/s with 4 CTAs per SM), so the cap of the uncached gather stays.
         if (c->n_entries * 12 >= h->p.n_rows) P.occ_cap = 4;
-    } else if (h->p.n_rows && h->packed_bytes_rows / h->p.n_rows >= 96 && h->p.row_bytes <= 512) {
+    } else if (!host_out && h->p.n_rows && h->packed_bytes_rows / h->p.n_rows >= 96 && h->p.row_bytes <= 512) {
         // Rows of about a line or more are bound by link bytes, and ONE CTA per SM (8 warps x 2 rows in flight) already keeps the
         // link busy: measured three times each, alternating, GNN 1.371 ms with 148 CTAs against 1.383 with 296, DLRM 0.6347 against
         // 0.6378 -- and half the registers and warp slots of every SM stay free for whatever runs beside the gather.  Smaller packed
         // rows are bound by rows per second, and rows of several passes (4 KB: 2-5 % slower with one CTA) by decode latency: both keep two.
+        // So does a gather whose OUTPUT is host memory (the direct path of ibp_gather_decompress_host): its warps also wait on their
+        // zero-copy stores, and with fewer rows in flight the end-to-end rate drops (GNN 40 -> 33 GB/s).
         P.occ_cap = 1;
     }
     const bool dedup = allow_dedup && (h->dedup_mode == 1 || (h->dedup_mode < 0 && n >= 16384)) && n >= 2 && h->p.n_rows <= 0xFFFFFFFEull;
@@ -1385,7 +1387,7 @@ extern "C" ibp_status ibp_gather_decompress_host(ibp_handle* h, const int64_t* r
             int64_t* ids_d = nullptr;
             IBP_CUDA(cudaMallocAsync((void**)&ids_d, id_bytes, st));
             IBP_CUDA(cudaMemcpyAsync(ids_d, row_ids_host, (size_t)n * 8, cudaMemcpyHostToDevice, st));
-            if (h->p.index_span == 1) s = gather_rows(h, nullptr, ids_d, n, out_dev_alias, st, false);
+            if (h->p.index_span == 1) s = gather_rows(h, nullptr, ids_d, n, out_dev_alias, st, false, true);
             else s = ibp_gather_decompress(h, ids_d, n, out_dev_alias, cuda_stream);
             cudaFreeAsync(ids_d, st);
             const cudaError_t es = cudaStreamSynchronize(st);
