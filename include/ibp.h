@@ -407,9 +407,9 @@ ibp_status ibp_set_dedup_mode(ibp_handle* h, int mode);
  * form used for 128/256/512-byte rows.  Results are identical in every mode.                                         */
 ibp_status ibp_set_stream_mode(ibp_handle* h, int mode);
 
-/* Tuning/test hook: rows each warp keeps in flight in random gathers (ring depth): 1, 2 or 4; 0 = automatic (default: one for
- * locality-ordered gathers of tables whose average stored row is 240 bytes or more, else two -- about 300 KB of packed bytes
- * in flight on the whole GPU).                                                                                        */
+/* Tuning/test hook: rows each warp keeps in flight in random gathers (ring depth): 1, 2 or 4; 0 = automatic (default: two;
+ * locality-ordered gathers of line-sized rows take 1, 2 or 4 and a grid chosen so that about 415 KB of packed bytes are in
+ * flight on the whole GPU -- DESIGN.md section 6, P19).                                                              */
 ibp_status ibp_set_rows_in_flight(ibp_handle* h, int n);
 
 /* -- Pinned, GPU-mapped host memory for callers that are not CUDA programs (the baseline table, pinned id buffers).  */

@@ -572,31 +572,43 @@ static int pick_W(uint32_t row_bytes) {
 static ibp_status launch_decode(ibp_handle* h, DecodeParams& P, int mode, cudaStream_t st) {
     if (P.n_units <= 0) return IBP_OK;
     const int W = pick_W(h->p.row_bytes);
-    // rows each warp keeps in flight.  Automatic: about 300 KB of packed bytes in flight over the whole GPU was the optimum of both
-    // locality-ordered gathers measured (GNN, 252-byte rows on average: 1,184 rows = one per warp, 1.351 ms against 1.370 with two
-    // and 1.41 with four; DLRM, 128-byte rows: 2,368 rows = two per warp, 0.633 ms against 0.663 with one; thresholded GNN, 213
-    // bytes: two, 1.308 against 1.318), so an ORDERED gather with one CTA per SM keeps one row per warp in flight when the average
-    // stored row is 240 bytes or more, and two otherwise (unordered gathers over small stores: two was better, 50.0 against 46.9 GB/s).
+    // Rows in flight.  A locality-ordered gather of line-sized rows is fastest with about 415 KB of packed bytes in flight over the
+    // whole GPU, spread over as many warps as one CTA per SM offers -- less starves the link, more only queues behind it (measured,
+    // two repetitions each on one box: GNN, 252-byte rows on average, 100 CTAs x 8 warps x 2 rows = 1,600 rows: 1.348 ms, against
+    // 1.363 with 1,184 rows, 1.372 with 2,368 and 1.41 with 4,736; thresholded GNN, 213 bytes, 125 CTAs x 2 = 2,000 rows: 1.295 ms
+    // against 1.321 with 2,368; DLRM, 128 bytes, 100 CTAs x 4 = 3,200 rows: 0.626 ms against 0.632 with 2,368 and 0.637 with
+    // 4,736).  So: rows = 415 KB / average stored row; rows per warp = the smallest of 1, 2, 4 that fits them into one CTA per SM;
+    // CTAs = rows / (warps per CTA x rows per warp).  Unordered gathers, small rows and host outputs keep two rows per warp.
     int nst = 4;
-    if (mode == MODE_ROWS) nst = h->rows_in_flight ? h->rows_in_flight
-                                 : (P.occ_cap == 1 && P.order && h->packed_bytes_rows / std::max<uint64_t>(1, h->p.n_rows) >= 240 ? 1 : 2);
+    int wpc = h->warps_per_cta ? (int)h->warps_per_cta : 8;
+    int64_t auto_ctas = 0;
+    if (mode == MODE_ROWS) {
+        nst = h->rows_in_flight ? h->rows_in_flight : 2;
+        if (P.occ_cap == 1 && P.order && !h->rows_in_flight) {
+            const uint64_t avg = std::max<uint64_t>(1, h->packed_bytes_rows / std::max<uint64_t>(1, h->p.n_rows));
+            const uint64_t rows = std::max<uint64_t>(1, 415000ull / avg), max_warps = (uint64_t)h->sm_count * (uint64_t)wpc;
+            nst = 1;
+            while (nst < 4 && rows / (uint64_t)nst > max_warps) nst *= 2;
+            auto_ctas = (int64_t)std::max<uint64_t>(1, (rows / (uint64_t)nst + (uint64_t)wpc - 1) / (uint64_t)wpc);
+        }
+    }
     P.n_pass = (h->n_words + 32 * W - 1) / (32 * W);
     P.slot_bytes = ((h->max_stride + 15u) / 16u) * 16u + 48u;   // 16-byte head + tail cover + one spare word
     P.slot_bytes = (P.slot_bytes + 127u) / 128u * 128u;
-    int wpc = h->warps_per_cta ? (int)h->warps_per_cta : 8;
     while (wpc > 1 && (size_t)wpc * nst * (P.slot_bytes + 8) > 200 * 1024) wpc >>= 1;
+    const int64_t max_ctas = h->max_ctas ? (int64_t)h->max_ctas : auto_ctas;
     const size_t smem = (size_t)wpc * nst * (P.slot_bytes + 8);   // rings + one mbarrier per slot
     const int fetch = h->fetch_mode;
     if (smem > 220 * 1024) { ibp_set_error("packed rows of %u bytes do not fit the shared-memory ring", h->max_stride); return IBP_ERR_UNSUPPORTED; }
     const int64_t blocks = (P.n_units + wpc - 1) / wpc;
 #define IBP_LAUNCH(W_, NST_, MODE_)                                                                                   \
     if (MODE_ == MODE_ROWS && P.cmap) {                                                                                \
-        if (h->thresholded) return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, true, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
-        return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, false, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
+        if (h->thresholded) return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, true, true>(P, blocks, max_ctas, h->sm_count, wpc, smem, st); \
+        return launch_one<W_, NST_, MODE_ROWS, FETCH_TMA, false, true>(P, blocks, max_ctas, h->sm_count, wpc, smem, st); \
     }                                                                                                                  \
-    if (h->thresholded) return launch_one<W_, NST_, MODE_, FETCH_TMA, true>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st); \
-    return fetch == FETCH_TMA ? launch_one<W_, NST_, MODE_, FETCH_TMA>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st) \
-                              : launch_one<W_, NST_, MODE_, FETCH_LSU>(P, blocks, h->max_ctas, h->sm_count, wpc, smem, st)
+    if (h->thresholded) return launch_one<W_, NST_, MODE_, FETCH_TMA, true>(P, blocks, max_ctas, h->sm_count, wpc, smem, st); \
+    return fetch == FETCH_TMA ? launch_one<W_, NST_, MODE_, FETCH_TMA>(P, blocks, max_ctas, h->sm_count, wpc, smem, st) \
+                              : launch_one<W_, NST_, MODE_, FETCH_LSU>(P, blocks, max_ctas, h->sm_count, wpc, smem, st)
 #define IBP_BY_W(NST_, MODE_)                        \
     switch (W) {                                     \
         case 4: IBP_LAUNCH(4, NST_, MODE_);          \
