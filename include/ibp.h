@@ -268,9 +268,10 @@ ibp_status ibp_get_metadata_host(const ibp_handle* h, int64_t group, const void*
 ibp_status ibp_get_info(const ibp_handle* h, ibp_info* out);
 
 /* Launch shape of the decode kernels: max_ctas limits the grid, so that a consumer kernel can share the GPU ("We
- * reserved only 64 SMs for decompression"); 0 = library default: the persistent grid that fills the GPU, except for contiguous
- * runs read from the HOST store (span gathers, ibp_gather_decompress_range, host ranges of ibp_decode_ranges), which are bound
- * by the link and take 48 CTAs -- the same throughput, and the other SMs stay free for the consumer of the rows; warps_per_cta of the random-row kernel: 0 = default
+ * reserved only 64 SMs for decompression"); 0 = library default: resident decode fills the GPU; contiguous runs read from the
+ * HOST store (span gathers, ibp_gather_decompress_range, host ranges of ibp_decode_ranges) are bound by the link and take 48
+ * CTAs; locality-ordered random gathers of line-sized rows take the grid that keeps about 415 KB of packed bytes in flight
+ * (about 100 CTAs) -- the same or better throughput, and the other SMs stay free for the consumer of the rows; warps_per_cta of the random-row kernel: 0 = default
  * (8), else 1..8 (the kernel is compiled for CTAs of at most 256 threads); INVALID_ARG above 8.                     */
 ibp_status ibp_configure(ibp_handle* h, uint32_t max_ctas, uint32_t warps_per_cta);
 
