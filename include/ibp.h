@@ -191,6 +191,24 @@ ibp_status ibp_upload_metadata(ibp_handle* h, int device, void* cuda_stream);
  * undefined behaviour), see ibp_validate_ids.  BAD_STATE before upload or with a pageable store.                   */
 ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);
 
+/* The same gather of random rows (index_span 1) for callers that may not allocate: code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc.  ibp_gather_decompress takes the workspace of its locality-order pre-pass (bucket
+ * counters + the processing order of the batch) from cudaMallocAsync; this entry point keeps that scratch in a file-scope
+ * device array of the library instead and calls no cudaMalloc / cudaMallocAsync / cudaFree nor any allocating routine.
+ *   - Limit: n <= IBP_NOALLOC_MAX_IDS ids per call; a larger n is rejected with IBP_ERR_INVALID_ARG and a message (split the
+ *     batch).  The array is 256 B + 1 MiB of counters + 4 B per id = 5.25 MB, and every GPU that loads the library holds it
+ *     until the process exits.
+ *   - Same arguments, layout and result as ibp_gather_decompress, bit for bit (the pre-pass only changes the order in which rows
+ *     are fetched; repeated ids are each fetched, there is no de-duplication and no compressed cache on this path).
+ *   - The handle's device must be the CURRENT device of the calling thread (BAD_STATE otherwise).  The array's device address is
+ *     looked up once per device on the first call there (cudaGetSymbolAddress): make that first call outside stream capture.
+ *   - Every call on a device shares the one array, which keeps the last call's contents; the call clears its counters on the
+ *     stream first.  Two calls that OVERLAP on the GPU (different streams, or threads, without an ordering between them) race on
+ *     the array and give undefined output: keep calls on one stream or order them with events.
+ * Asynchronous on the stream.  UNSUPPORTED with index_span > 1; BAD_STATE before upload or with a pageable store.        */
+#define IBP_NOALLOC_MAX_IDS (1 << 20)
+ibp_status ibp_gather_decompress_noalloc(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream);
+
 /* Same result with HOST buffers: row_ids_host (n int64) is copied to the device, the gather runs, and the rows are
  * copied back into out_host, all on the stream, which is synchronised before returning.  The end-to-end entry point
  * bench.py times.  The buffers should be pinned for full copy speed; pageable memory works.

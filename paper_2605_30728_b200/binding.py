@@ -14,6 +14,7 @@ import numpy as np
 from ._build import build_library
 
 IBP_OK = 0
+IBP_ERR_INVALID_ARG, IBP_ERR_OUT_OF_MEMORY, IBP_ERR_CUDA, IBP_ERR_BAD_STATE, IBP_ERR_UNSUPPORTED = 1, 2, 3, 4, 5
 STATUS = {0: "IBP_OK", 1: "IBP_ERR_INVALID_ARG", 2: "IBP_ERR_OUT_OF_MEMORY", 3: "IBP_ERR_CUDA", 4: "IBP_ERR_BAD_STATE",
           5: "IBP_ERR_UNSUPPORTED"}
 IBP_GROUP_BLOCKED, IBP_GROUP_STRIDED, IBP_GROUP_MAP = 0, 1, 2
@@ -69,6 +70,7 @@ class ibp_table_desc(C.Structure):
 
 
 IBP_CACHE_MISS = 0xFFFFFFFFFFFFFFFF
+IBP_NOALLOC_MAX_IDS = 1 << 20
 IBP_MEM_MANAGED_HOST, IBP_MEM_HOSTALLOC, IBP_MEM_MALLOC_REGISTERED, IBP_MEM_THP_REGISTERED, IBP_MEM_HUGETLB_2M_REGISTERED = range(5)
 IBP_SLAB_REMOTE = -2
 IBP_IPC_HANDLE_BYTES = 64
@@ -83,6 +85,7 @@ SIGNATURES = {
     "ibp_upload_metadata": (_int, [_vp, _int, _vp]),
     "ibp_gather_decompress": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_gather_decompress_host": (_int, [_vp, _vp, _i64, _vp, _vp]),
+    "ibp_gather_decompress_noalloc": (_int, [_vp, _vp, _i64, _vp, _vp]),
     "ibp_decompress_resident": (_int, [_vp, _vp, _i64, _i64, _vp, _vp]),
     "ibp_gather_decompress_range": (_int, [_vp, _i64, _i64, _vp, _vp]),
     "ibp_gather_decompress_range_host": (_int, [_vp, _i64, _i64, _vp, _vp]),
@@ -181,6 +184,9 @@ class Handle:
 
     def gather_decompress(self, row_ids_dev, n, out_dev, stream=None):
         _check(lib().ibp_gather_decompress(self._h, _ptr(row_ids_dev), n, _ptr(out_dev), stream))
+
+    def gather_decompress_noalloc(self, row_ids_dev, n, out_dev, stream=None):
+        _check(lib().ibp_gather_decompress_noalloc(self._h, _ptr(row_ids_dev), n, _ptr(out_dev), stream))
 
     def gather_decompress_host(self, row_ids_host, n, out_host, stream=None):
         _check(lib().ibp_gather_decompress_host(self._h, _ptr(row_ids_host), n, _ptr(out_host), stream))

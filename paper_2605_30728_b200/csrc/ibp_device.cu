@@ -23,6 +23,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 #include <vector>
 
@@ -1162,6 +1163,84 @@ extern "C" ibp_status ibp_gather_decompress(ibp_handle* h, const int64_t* row_id
     P.units_per_span = (h->p.index_span + P.rows_per_unit - 1) / P.rows_per_unit;
     P.n_units = n * (int64_t)P.units_per_span;
     return launch_decode(h, P, MODE_SPANS, st);
+}
+
+// ------------------------------------------------------------------------------------------------ gather without allocation
+// ibp_gather_decompress_noalloc: the random-row gather for callers that may not allocate (CUDA graph capture, serving loops).
+// The locality-order pre-pass (bucket histogram, scan, scatter: the scratch-memory kernels of gather_rows) runs in a FIXED
+// device array instead of a cudaMallocAsync workspace: [n counter, 256 B][bucket counters, <= 2^18 x 4 B][order, n x 4 B].
+// The array lives in every GPU context that loads the library (5.25 MB per GPU until exit).  In host code its NAME is a
+// host-side stand-in, not a device address, so the address is taken with cudaGetSymbolAddress once per device, with that
+// device current, and passed to the kernels like any workspace pointer.
+constexpr size_t NOALLOC_CNT_BYTES = (size_t)(1u << 18) * 4;                                    // bucket_shape: at most 2^18 buckets
+constexpr size_t NOALLOC_ZERO_BYTES = 256 + NOALLOC_CNT_BYTES;
+constexpr size_t NOALLOC_SCRATCH_BYTES = NOALLOC_ZERO_BYTES + (size_t)IBP_NOALLOC_MAX_IDS * 4;
+static __device__ __align__(256) uint8_t ibp_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::mutex g_noalloc_mu;
+static uint8_t* g_noalloc_ptr[NOALLOC_MAX_DEVICES];                                             // device address of the array, per device
+
+static ibp_status noalloc_scratch_ptr(int device, uint8_t** out) {
+    int cur = -1;
+    IBP_CUDA(cudaGetDevice(&cur));
+    if (cur != device || device < 0 || device >= NOALLOC_MAX_DEVICES) {
+        ibp_set_error("ibp_gather_decompress_noalloc: the handle's device %d must be the current device (current: %d)", device, cur);
+        return IBP_ERR_BAD_STATE;
+    }
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, ibp_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            ibp_set_error("ibp_gather_decompress_noalloc: cudaGetSymbolAddress failed: %s", cudaGetErrorString(e));
+            (void)cudaGetLastError();
+            return IBP_ERR_CUDA;
+        }
+        g_noalloc_ptr[device] = (uint8_t*)p;
+    }
+    *out = g_noalloc_ptr[device];
+    return IBP_OK;
+}
+
+extern "C" ibp_status ibp_gather_decompress_noalloc(ibp_handle* h, const int64_t* row_ids_dev, int64_t n, void* out_dev, void* cuda_stream) {
+    ibp_status s = check_ready(h, "ibp_gather_decompress_noalloc");
+    if (s != IBP_OK) return s;
+    if (n == 0) return IBP_OK;
+    if (n < 0 || !row_ids_dev || !out_dev || ((uintptr_t)out_dev & 15u)) { ibp_set_error("ibp_gather_decompress_noalloc: bad argument (null pointer, n<0, or out not 16-byte aligned)"); return IBP_ERR_INVALID_ARG; }
+    if (n > (int64_t)IBP_NOALLOC_MAX_IDS) {
+        ibp_set_error("ibp_gather_decompress_noalloc: n = %lld exceeds IBP_NOALLOC_MAX_IDS = %d ids per call (the fixed scratch array); split the batch or use ibp_gather_decompress",
+                      (long long)n, (int)IBP_NOALLOC_MAX_IDS);
+        return IBP_ERR_INVALID_ARG;
+    }
+    if (h->p.index_span != 1 || h->p.n_rows == 0) { ibp_set_error("ibp_gather_decompress_noalloc: random rows only (index_span must be 1)"); return IBP_ERR_UNSUPPORTED; }
+    if (!h->store_dev) { ibp_set_error("ibp_gather_decompress_noalloc: the packed store is not GPU-mapped (pageable store)"); return IBP_ERR_BAD_STATE; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint8_t* ws = nullptr;
+    s = noalloc_scratch_ptr(h->device, &ws);
+    if (s != IBP_OK) return s;
+    uint32_t shift = 0, nb = 0;
+    bucket_shape(h->p.n_rows, h->store_used, 256ull << 10, &shift, &nb);
+    const uint32_t nb_pad = (nb + 4095u) / 4096u * 4096u;                                    // <= 2^18: fits NOALLOC_CNT_BYTES
+    // the array keeps the last call's contents: the counters must start at zero (the order list is fully rewritten)
+    IBP_CUDA(cudaMemsetAsync(ws, 0, 256 + (size_t)nb_pad * 4, st));
+    uint32_t* cnt = (uint32_t*)(ws + 256);
+    int32_t* ord = (int32_t*)(ws + NOALLOC_ZERO_BYTES);
+    const int thr = 256, blocks = (int)std::min<int64_t>((n + thr - 1) / thr, (int64_t)h->sm_count * 8);
+    ibp_bucket_hist<<<blocks, thr, 0, st>>>(row_ids_dev, nullptr, nullptr, n, shift, nb, cnt);
+    ibp_bucket_scan<<<1, 1024, 0, st>>>(cnt, nb_pad);
+    ibp_bucket_scatter<<<blocks, thr, 0, st>>>(row_ids_dev, nullptr, nullptr, n, shift, nb, cnt, ord);
+    IBP_CUDA(cudaGetLastError());
+    DecodeParams P;
+    fill_common(h, P);
+    P.store = h->store_dev;
+    P.ids = row_ids_dev;
+    P.out = (uint8_t*)out_dev;
+    P.n = n;
+    P.span = 1;
+    P.n_units = n;
+    P.order = ord;
+    if (h->packed_bytes_rows / h->p.n_rows >= 96 && h->p.row_bytes <= 512) P.occ_cap = 1;    // the launch shape gather_rows picks for line-sized rows
+    return launch_decode(h, P, MODE_ROWS, st);
 }
 
 // Rows [first_row, first_row+n_rows) in order, packed bytes at `packed` (device-visible), whose first byte is the packed
