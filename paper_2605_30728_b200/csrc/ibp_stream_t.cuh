@@ -350,6 +350,21 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity)
             : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
     }
 }
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+    // the producer lane's wait for a free stage: a plain try_wait loop comes back every ~25 cycles and its three instructions per
+    // round were 9-18 % of everything the kernel issued (ncu source counters); sleeping ~100 ns between tries costs 1 % of a unit's
+    // decode time in reaction at worst, and the refill has a whole stage of decode to hide behind
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) break;
+        __nanosleep(100);
+    }
+}
 __device__ __forceinline__ uint32_t lds32(uint32_t a) {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
@@ -405,7 +420,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 const uint32_t meta_bytes = P.aux_meta_off ? (uint32_t)(g1 - g0 + 1) * row_bytes2 : 0u;
                 const uint32_t bytes = (a1 - a0) * 16u;
                 const uint32_t stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap, bar = full_s + s * 8;
-                mbar_wait(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);      // the producer polls: a suspended wait reacts later and the refill starts late
+                mbar_wait_backoff(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);   // (a wait with a 20 us suspend hint reacts late and the refill starts late)
                 asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s), "r"((uint32_t)first), "r"((uint32_t)((uint64_t)first >> 32)),
                              "r"((uint32_t)(out0 + r0)), "r"((uint32_t)((uint64_t)(out0 + r0) >> 32)) : "memory");
                 asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s + 16u), "r"(n), "r"(a0), "r"(r1 == nrows ? 1u : 0u), "r"(0u) : "memory");
@@ -427,7 +442,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     const uint32_t sub = (uint32_t)lane / LPR, sl = (uint32_t)lane % LPR;      // lane group (row of a pass), lane inside the row
     const uint32_t w0 = sl * W;                                                // first chunk (32-bit word) of this lane
     const uint32_t hdr_off = (w0 >> 5) * 4u, hdr_sh = w0 & 31u;                // where the lane's 4 participation bits sit
-    uint32_t m[W], b[W], mv[W][NMV], pm4 = 0;                                  // pm4: popc(Mask) of the 4 chunks, one per byte
+    uint32_t m[W], b[W], mv[W][NMV], kq[W], pm4 = 0, npm4 = 0;                 // kq: bits a participating chunk stores (32 - popc(Mask)); pm4: popc(Mask) of the 4 chunks, one per byte; npm4: minus that, as signed bytes
     uint64_t prep_g = ~0ull;                                                   // per lane: lane groups may hold different groups
     bool five = true;                                                          // NR = 0: some bit of the prepared groups moves by >= 16 (warp-uniform)
 
@@ -444,7 +459,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
         }
         pm4 = 0;
 #pragma unroll
-        for (int q = 0; q < W; ++q) pm4 |= (uint32_t)__popc(m[q]) << (8 * q);   // <= 32 each
+        for (int q = 0; q < W; ++q) { const uint32_t pc = (uint32_t)__popc(m[q]); kq[q] = 32u - pc; pm4 |= pc << (8 * q); }   // <= 32 each
+        npm4 = (0x80808080u - pm4) ^ 0x80808080u;                                // per byte: -popc (no borrow crosses a byte: 0x80 - pc > 0)
         if constexpr (NR > 0) {
 #pragma unroll
             for (int q = 0; q < W; ++q) {
@@ -507,53 +523,67 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
 
     // RB passes side by side: lane group `sub` decodes row rr[i] of the piece in pass i (valid[i] = 0: the row is a repeat whose
     // result is not stored).  my_off / flags: offsets (lane i <-> row i of the piece) and compressed-bits of the piece.
-    auto decode_rows_n = [&](auto nstg_c, const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
+    auto decode_rows_n = [&](auto nstg_c, auto full_c, const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
                              uint32_t stage_s, uint8_t* orow0) {
-        uint32_t bitbase[RB], part[RB], s[RB], d4[RB];
+        // Per pass: the bits this lane's four chunks store (kept: kq[q] if the chunk participates, else all 32) as running sums
+        // rel[q] (bits in front of chunk q inside the lane) and tot; the exclusive scan of tot over the lanes of the row (P:319 step
+        // 3) gives the lane's first bit.  The integer (ALU) pipe is what binds this kernel (ncu: 70 % busy at half rate, the FMA pipe
+        // 19 %), so the arithmetic is arranged for the FMA pipe: sums are predicated adds, the compressed-row flag enters as a
+        // multiplier, shared-memory words are addressed by WORD index (the scaled address mode takes the shift).
+        uint32_t bw[RB], part[RB], tot[RB];
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
             const uint32_t sa = stage_s + (__shfl_sync(0xFFFFFFFFu, my_off, rr[i]) - base_off) * 16u;
-            const bool comp = (flags >> rr[i]) & 1u;
+            const uint32_t comp = (flags >> rr[i]) & 1u;
             const uint32_t h = lds32(sa + hdr_off);
-            part[i] = comp ? (h >> hdr_sh) & 0xFu : 0u;                        // raw row: no chunk participates ...
-            const uint32_t sel = ((part[i] * 0x00204081u) & 0x01010101u) * 0xFFu;   // participation bit q -> byte q = 0xFF
-            const uint32_t in4 = (pm4 & sel) * 0x01010101u;                    // byte q = bits removed in chunks 0..q of this lane
-            s[i] = in4 >> 24;
-            d4[i] = 0x60402000u - (in4 << 8);                                  // byte q = 32*q - bits removed in front of chunk q (>= 0)
-            bitbase[i] = sa * 8u + (comp ? P.n_words : 0u) + 32u * w0;         // ... and there is no header; a BIT address
+            part[i] = (h >> hdr_sh) & (comp * 0xFu);                           // raw row: no chunk participates ...
+            const uint32_t sel = (part[i] * 0x00204081u) & 0x01010101u;        // participation bit q -> byte q = 1
+            tot[i] = (uint32_t)__dp4a((int)npm4, (int)sel, 128);               // bits this lane's four chunks store: 128 - sum of popc(Mask) over its participating chunks (P:319 step 2)
+            bw[i] = sa * 8u + comp * P.n_words;                                 // ... and there is no header; a BIT address
         }
         static_assert(RB == 2, "the packed scan holds two passes");
-        uint32_t inc = s[0] | (s[1] << 16);                                    // exclusive scan over the lanes of a row (P:319 step 3)
+        uint32_t inc = tot[0] | (tot[1] << 16);                                // inclusive scan over the lanes of a row: <= 4,096 per row
 #pragma unroll
-        for (int d = 1; d < LPR; d <<= 1) {
-            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, d, LPR);
-            if (sl >= (uint32_t)d) inc += v;
-        }
+        for (int d = 1; d < LPR; d <<= 1)
+            asm volatile("{\n\t.reg .pred p;\n\t.reg .u32 v;\n\t"
+                "shfl.sync.up.b32 v|p, %0, %1, %2, 0xffffffff;\n\t@p add.u32 %0, %0, v;\n\t}"
+                : "+r"(inc) : "r"(d), "r"((32 - LPR) << 8));
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
-            const uint32_t bb = bitbase[i] + s[i] - (i == 0 ? (inc & 0xFFFFu) : (inc >> 16));   // minus the bits removed in the lanes in front
+            uint32_t ba = bw[i] + (i == 0 ? (inc & 0xFFFFu) : (inc >> 16)) - tot[i];   // plus the bits stored by the lanes in front
             uint32_t o[W];
 #pragma unroll
             for (int q = 0; q < W; ++q) {
-                const uint32_t ba = bb + __byte_perm(d4[i], 0, 0x4440 + q);
+                const bool in = (part[i] >> q) & 1u;
                 uint32_t lo, hi;
-                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"((ba >> 3) & ~3u));
+                uint32_t wi;
+                asm("shr.u32 %0, %1, 5;" : "=r"(wi) : "r"(ba));                  // word index (kept apart from the *4: one shift on the ALU pipe, the scaling elsewhere)
+                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wi * 4u));
                 const uint32_t x = __funnelshift_r(lo, hi, ba);                // shift = ba mod 32
                 const uint32_t e = reinsert(nstg_c, x, q);
-                o[q] = ((part[i] >> q) & 1u) ? e : x;                          // non-participating chunk: all 32 bits
+                o[q] = in ? e : x;                                             // non-participating chunk: all 32 bits
+                if (q + 1 < W) {                                               // the next chunk starts kq[q] bits on, or 32: an add and a predicated add
+                    uint32_t nx;
+                    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\tadd.u32 %0, %2, 32;\n\t@p add.u32 %0, %2, %3;\n\t}"
+                        : "=r"(nx) : "r"((uint32_t)in), "r"(ba), "r"(kq[q]));
+                    ba = nx;
+                }
             }
             uint8_t* dst = orow0 + (size_t)rr[i] * P.row_bytes;
-            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};\n\t}"
-                         ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]), "r"(valid[i]) : "memory");
+            if constexpr (decltype(full_c)::value)                                 // a whole piece: every pass stores
+                asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+            else
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};\n\t}"
+                             ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]), "r"(valid[i]) : "memory");
         }
     };
     // NR = 0: two copies of the pass body, with and without the stage that moves bits by 16 (bf16 pairs with a few invariant
     // exponent bits per half never need it); the choice is per prepared group and warp-uniform
-    auto decode_rows = [&](const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
+    auto decode_rows = [&](auto full_c, const uint32_t (&rr)[RB], const uint32_t (&valid)[RB], uint32_t my_off, uint32_t flags, uint32_t base_off,
                            uint32_t stage_s, uint8_t* orow0) {
         using std::integral_constant;
-        if (NR > 0 || five) decode_rows_n(integral_constant<int, 5>{}, rr, valid, my_off, flags, base_off, stage_s, orow0);
-        else decode_rows_n(integral_constant<int, 4>{}, rr, valid, my_off, flags, base_off, stage_s, orow0);
+        if (NR > 0 || five) decode_rows_n(integral_constant<int, 5>{}, full_c, rr, valid, my_off, flags, base_off, stage_s, orow0);
+        else decode_rows_n(integral_constant<int, 4>{}, full_c, rr, valid, my_off, flags, base_off, stage_s, orow0);
     };
 
     // One piece: rows id0 .. id0 + cnt - 1 (cnt <= 32), all inside the stage.  orow = output address of row 0 of the piece.
@@ -573,16 +603,26 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
             // every lane group's rows lie in one group of the table: one set-up per piece, possibly of several groups at once
             const uint64_t g = have ? glo : group_of_u(P.group_param, P.group_shift, (uint64_t)id0);
             if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
-            const uint32_t n_it = min(Q, cnt);
-            for (uint32_t i = 0; i < n_it; i += RB) {
-                uint32_t rr[RB], valid[RB];
+            if (cnt == RPP * Q && Q % RB == 0) {
+                // a whole piece (all but the tail of a span or range): every lane group has Q rows, no pass is a repeat
+                for (uint32_t i = 0; i < Q; i += RB) {
+                    uint32_t rr[RB], valid[RB];
 #pragma unroll
-                for (int j = 0; j < RB; ++j) {
-                    const uint32_t r = qs + i + j;
-                    valid[j] = r < qe;
-                    rr[j] = valid[j] ? r : (have ? qs : 0u);
+                    for (int j = 0; j < RB; ++j) { rr[j] = qs + i + j; valid[j] = 1u; }
+                    decode_rows(std::true_type{}, rr, valid, my_off, flags, base_off, stage_s, orow);
                 }
-                decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow);
+            } else {
+                const uint32_t n_it = min(Q, cnt);
+                for (uint32_t i = 0; i < n_it; i += RB) {
+                    uint32_t rr[RB], valid[RB];
+#pragma unroll
+                    for (int j = 0; j < RB; ++j) {
+                        const uint32_t r = qs + i + j;
+                        valid[j] = r < qe;
+                        rr[j] = valid[j] ? r : (have ? qs : 0u);
+                    }
+                    decode_rows(std::false_type{}, rr, valid, my_off, flags, base_off, stage_s, orow);
+                }
             }
         } else {
             // a table group ends inside a lane group's rows (a range that starts off a group boundary): run by run of one group
@@ -600,7 +640,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                         valid[j] = x < r_end;
                         rr[j] = valid[j] ? x : r;
                     }
-                    decode_rows(rr, valid, my_off, flags, base_off, stage_s, orow);
+                    decode_rows(std::false_type{}, rr, valid, my_off, flags, base_off, stage_s, orow);
                 }
                 r = r_end;
             }
