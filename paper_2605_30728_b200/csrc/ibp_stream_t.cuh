@@ -442,7 +442,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     const uint32_t sub = (uint32_t)lane / LPR, sl = (uint32_t)lane % LPR;      // lane group (row of a pass), lane inside the row
     const uint32_t w0 = sl * W;                                                // first chunk (32-bit word) of this lane
     const uint32_t hdr_off = (w0 >> 5) * 4u, hdr_sh = w0 & 31u;                // where the lane's 4 participation bits sit
-    uint32_t m[W], b[W], mv[W][NMV], kq[W], pm4 = 0, npm4 = 0;                 // kq: bits a participating chunk stores (32 - popc(Mask)); pm4: popc(Mask) of the 4 chunks, one per byte; npm4: minus that, as signed bytes
+    uint32_t m[W], b[W], mv[W][NMV], kq[W], pm4 = 0, npm4 = 0;                 // kq: bits a participating chunk leaves out (popc(Mask)); pm4: popc(Mask) of the 4 chunks, one per byte; npm4: minus that, as signed bytes
     uint64_t prep_g = ~0ull;                                                   // per lane: lane groups may hold different groups
     bool five = true;                                                          // NR = 0: some bit of the prepared groups moves by >= 16 (warp-uniform)
 
@@ -459,7 +459,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
         }
         pm4 = 0;
 #pragma unroll
-        for (int q = 0; q < W; ++q) { const uint32_t pc = (uint32_t)__popc(m[q]); kq[q] = 32u - pc; pm4 |= pc << (8 * q); }   // <= 32 each
+        for (int q = 0; q < W; ++q) { const uint32_t pc = (uint32_t)__popc(m[q]); kq[q] = pc; pm4 |= pc << (8 * q); }   // <= 32 each
         npm4 = (0x80808080u - pm4) ^ 0x80808080u;                                // per byte: -popc (no borrow crosses a byte: 0x80 - pc > 0)
         if constexpr (NR > 0) {
 #pragma unroll
@@ -550,27 +550,25 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 : "+r"(inc) : "r"(d), "r"((32 - LPR) << 8));
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
-            uint32_t ba = bw[i] + (i == 0 ? (inc & 0xFFFFu) : (inc >> 16)) - tot[i];   // plus the bits stored by the lanes in front
+            // t = the lane's first bit minus the bits removed in front of chunk q: chunk q sits at bit t + 32 q, i.e. q words further
+            // on (an immediate in the load) with the same shift; each participating chunk takes popc(Mask) off t (a predicated add)
+            uint32_t t = bw[i] + (i == 0 ? (inc & 0xFFFFu) : (inc >> 16)) - tot[i];   // plus the bits stored by the lanes in front
             uint32_t o[W];
 #pragma unroll
             for (int q = 0; q < W; ++q) {
-                const bool in = (part[i] >> q) & 1u;
-                uint32_t lo, hi;
-                uint32_t wi;
-                asm("shr.u32 %0, %1, 5;" : "=r"(wi) : "r"(ba));                  // word index (kept apart from the *4: one shift on the ALU pipe, the scaling elsewhere)
-                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wi * 4u));
-                const uint32_t x = __funnelshift_r(lo, hi, ba);                // shift = ba mod 32
+                const bool in = (part[i] & (1u << q)) != 0u;
+                uint32_t lo, hi, wi;
+                asm("shr.u32 %0, %1, 5;" : "=r"(wi) : "r"(t));                   // word index (kept apart from the *4: one shift on the ALU pipe, the scaling elsewhere)
+                asm volatile("ld.shared.u32 %0, [%2];\n\tld.shared.u32 %1, [%2+4];" : "=r"(lo), "=r"(hi) : "r"(wi * 4u + 4u * q));
+                const uint32_t x = __funnelshift_r(lo, hi, t);                 // shift = t mod 32
                 const uint32_t e = reinsert(nstg_c, x, q);
                 o[q] = in ? e : x;                                             // non-participating chunk: all 32 bits
-                if (q + 1 < W) {                                               // the next chunk starts kq[q] bits on, or 32: an add and a predicated add
-                    uint32_t nx;
-                    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\tadd.u32 %0, %2, 32;\n\t@p add.u32 %0, %2, %3;\n\t}"
-                        : "=r"(nx) : "r"((uint32_t)in), "r"(ba), "r"(kq[q]));
-                    ba = nx;
-                }
+                if (q + 1 < W)
+                    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p sub.u32 %0, %0, %2;\n\t}" : "+r"(t) : "r"((uint32_t)in), "r"(kq[q]));
             }
-            uint8_t* dst = orow0 + (size_t)rr[i] * P.row_bytes;
-            if constexpr (decltype(full_c)::value)                                 // a whole piece: every pass stores
+            constexpr uint32_t ROWB = 16u * LPR;                                   // = P.row_bytes (the launcher picks LPR from it)
+            uint8_t* dst = decltype(full_c)::value ? orow0 + (size_t)i * ROWB : orow0 + (size_t)rr[i] * ROWB;   // whole piece: orow0 is pass 0's row, rows are consecutive
+            if constexpr (decltype(full_c)::value)                                 // ... and every pass stores
                 asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
             else
                 asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};\n\t}"
@@ -605,11 +603,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
             if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
             if (cnt == RPP * Q && Q % RB == 0) {
                 // a whole piece (all but the tail of a span or range): every lane group has Q rows, no pass is a repeat
-                for (uint32_t i = 0; i < Q; i += RB) {
+                uint8_t* po = orow + (size_t)qs * (16u * LPR);
+                for (uint32_t i = 0; i < Q; i += RB, po += (size_t)RB * (16u * LPR)) {
                     uint32_t rr[RB], valid[RB];
 #pragma unroll
                     for (int j = 0; j < RB; ++j) { rr[j] = qs + i + j; valid[j] = 1u; }
-                    decode_rows(std::true_type{}, rr, valid, my_off, flags, base_off, stage_s, orow);
+                    decode_rows(std::true_type{}, rr, valid, my_off, flags, base_off, stage_s, po);
                 }
             } else {
                 const uint32_t n_it = min(Q, cnt);
