@@ -854,7 +854,7 @@ static ibp_status launch_stream_t(ibp_handle* h, const uint8_t* packed, uint64_t
     uint64_t per;                                                                      // consecutive rows per chunk
     // rows of 128 / 256 / 512 bytes (every BASELINE workload): the sub-warp kernel (ibp_stream_t.cuh, ibp_stream_t2_kernel)
     const uint32_t lpr = h->p.row_bytes % 16 == 0 ? h->p.row_bytes / 16 : 0;
-    bool t2 = (lpr == 8 || lpr == 16 || lpr == 32) && h->t2_mode && !P.strided;
+    bool t2 = (lpr == 8 || lpr == 16 || lpr == 32) && h->t2_mode && !P.strided && h->p.n_rows <= 0xFFFFFFFFull;   // (32-bit row ids on its consumer side)
     if (t2) {
         // A unit (= chunk, = stage) is NW pieces, one per consumer warp; a stage holds the unit's packed bytes plus an aux region:
         // descriptor, row-offset cover, row-flag cover, Mask/Bitval of the groups the unit touches (ibp_stream_t.cuh).  Two stages

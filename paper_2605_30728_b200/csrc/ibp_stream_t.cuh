@@ -443,17 +443,20 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     const uint32_t w0 = sl * W;                                                // first chunk (32-bit word) of this lane
     const uint32_t hdr_off = (w0 >> 5) * 4u, hdr_sh = w0 & 31u;                // where the lane's 4 participation bits sit
     uint32_t m[W], b[W], mv[W][NMV], kq[W], pm4 = 0, npm4 = 0;                 // kq: bits a participating chunk leaves out (popc(Mask)); pm4: popc(Mask) of the 4 chunks, one per byte; npm4: minus that, as signed bytes
-    uint64_t prep_g = ~0ull;                                                   // per lane: lane groups may hold different groups
+    // Row ids and group numbers are 32-bit on the consumer side (the launcher takes this kernel only for tables below 2^32 rows):
+    // half the registers and instructions of the per-piece bookkeeping.
+    auto group_of = [&](uint32_t id) -> uint32_t { return P.group_shift != 0xFFFFFFFFu ? id >> P.group_shift : id / P.group_param; };
+    uint32_t prep_g = ~0u;                                                     // per lane: lane groups may hold different groups
     bool five = true;                                                          // NR = 0: some bit of the prepared groups moves by >= 16 (warp-uniform)
 
     // S2 for group g: Mask/Bitval from the stage's aux region (meta_s = shared address of group g0's record), else from global memory
-    auto prepare = [&](uint64_t g, uint64_t g0, uint32_t meta_s) {
+    auto prepare = [&](uint32_t g, uint32_t g0, uint32_t meta_s) {
         if (P.aux_meta_off) {
             const uint32_t a = meta_s + (uint32_t)(g - g0) * row_bytes2 + w0 * 4u;
             lds128(a, m);
             lds128(a + P.row_bytes, b);
         } else {
-            const uint32_t* gm = P.meta + g * 2ull * P.n_words;
+            const uint32_t* gm = P.meta + (uint64_t)g * 2ull * P.n_words;
             VecIO<W>::ld(gm + w0, m);
             VecIO<W>::ld(gm + P.n_words + w0, b);
         }
@@ -587,19 +590,19 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
     // One piece: rows id0 .. id0 + cnt - 1 (cnt <= 32), all inside the stage.  orow = output address of row 0 of the piece.
     const uint32_t U = P.piece_rows;
     const uint32_t Q = (U + RPP - 1) / RPP;                                    // rows of a piece per lane group
-    auto decode_piece = [&](int64_t id0, uint32_t cnt, uint32_t my_off, uint32_t flags, uint32_t base_off, uint32_t stage_s, uint8_t* orow,
-                            uint64_t g0, uint32_t meta_s) {
+    auto decode_piece = [&](uint32_t id0, uint32_t cnt, uint32_t my_off, uint32_t flags, uint32_t base_off, uint32_t stage_s, uint8_t* orow,
+                            uint32_t g0, uint32_t meta_s) {
         orow += (size_t)w0 * 4;
         const uint32_t qs = min(cnt, sub * Q), qe = min(cnt, qs + Q);
         const bool have = qs < qe;
-        uint64_t glo = 0, ghi = 0;
+        uint32_t glo = 0, ghi = 0;
         if (have) {
-            glo = group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + qs));
-            ghi = group_of_u(P.group_param, P.group_shift, (uint64_t)(id0 + qe - 1));
+            glo = group_of(id0 + qs);
+            ghi = group_of(id0 + qe - 1);
         }
         if (__all_sync(0xFFFFFFFFu, !have || glo == ghi)) {
             // every lane group's rows lie in one group of the table: one set-up per piece, possibly of several groups at once
-            const uint64_t g = have ? glo : group_of_u(P.group_param, P.group_shift, (uint64_t)id0);
+            const uint32_t g = have ? glo : group_of(id0);
             if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
             if (cnt == RPP * Q && Q % RB == 0) {
                 // a whole piece (all but the tail of a span or range): every lane group has Q rows, no pass is a repeat
@@ -627,9 +630,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
             // a table group ends inside a lane group's rows (a range that starts off a group boundary): run by run of one group
             uint32_t r = 0;
             while (r < cnt) {
-                const uint64_t id = (uint64_t)(id0 + r);
-                const uint64_t g = group_of_u(P.group_param, P.group_shift, id);
-                const uint32_t r_end = (uint32_t)min((uint64_t)cnt, (uint64_t)r + ((g + 1) * S - id));
+                const uint32_t id = id0 + r;
+                const uint32_t g = group_of(id);
+                const uint32_t r_end = (uint32_t)min((uint64_t)cnt, (uint64_t)r + (((uint64_t)g + 1) * S - id));
                 if (__any_sync(0xFFFFFFFFu, g != prep_g)) prepare(g, g0, meta_s);
                 for (; r < r_end; r += RB * RPP) {
                     uint32_t rr[RB], valid[RB];
@@ -646,27 +649,31 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
         }
     };
 
+    // this CTA's chunks blockIdx.x, blockIdx.x + gridDim.x, ...: only their number matters here (the descriptor names the rows); a
+    // 32-bit down-counter, because the 64-bit chunk index was spilled and its reload stalled every unit (ncu: 7 % of the samples)
     uint32_t k = 0;
-    for (int64_t c = blockIdx.x; c < P.n_chunks; c += gridDim.x) {
+    uint32_t left = (int64_t)blockIdx.x < P.n_chunks ? (uint32_t)((P.n_chunks - 1 - (int64_t)blockIdx.x) / (int64_t)gridDim.x) + 1u : 0u;
+    for (; left; --left) {
         uint32_t last;
-        do {                                                                   // the units of chunk c, in the producer's order
+        do {                                                                   // the units of the chunk, in the producer's order
             const uint32_t s = k % NS, stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap;
             mbar_wait_relaxed(full_s + s * 8, (k / NS) & 1u);
             uint32_t d0[4], d1[4];
             lds128(aux_s, d0);
             lds128(aux_s + 16u, d1);
-            const int64_t first = (int64_t)(((uint64_t)d0[1] << 32) | d0[0]), out0 = (int64_t)(((uint64_t)d0[3] << 32) | d0[2]);
+            const uint32_t first = d0[0];                                    // (d0[1] = 0: below 2^32 rows)
+            const int64_t out0 = (int64_t)(((uint64_t)d0[3] << 32) | d0[2]);
             const uint32_t n = d1[0], base_off = d1[1];
             last = d1[2];
-            const uint32_t off_s = aux_s + 32u - (uint32_t)(first & ~3ll) * 4u;          // shared address of row_off[0] (wraps mod 2^32: only differences matter)
-            const int64_t fw = (first >> 5) & ~3ll;
-            const uint64_t g0 = group_of_u(P.group_param, P.group_shift, (uint64_t)first);
+            const uint32_t off_s = aux_s + 32u - (first & ~3u) * 4u;                    // shared address of row_off[0] (wraps mod 2^32: only differences matter)
+            const uint32_t fw = (first >> 5) & ~3u;
+            const uint32_t g0 = group_of(first);
             for (uint32_t j0 = wib * U; j0 < n; j0 += NW * U) {
                 const uint32_t cnt = min(U, n - j0);
-                const int64_t id0 = first + j0;
-                const uint32_t my_off = (uint32_t)lane < cnt ? lds32(off_s + ((uint32_t)id0 + (uint32_t)lane) * 4u) : 0u;
-                const uint32_t fa = aux_s + P.aux_flag_off + (uint32_t)((id0 >> 5) - fw) * 4u;
-                uint32_t flags = __funnelshift_r(lds32(fa), lds32(fa + 4u), (uint32_t)id0 & 31u);   // bit r = flag of row id0 + r
+                const uint32_t id0 = first + j0;
+                const uint32_t my_off = (uint32_t)lane < cnt ? lds32(off_s + (id0 + (uint32_t)lane) * 4u) : 0u;
+                const uint32_t fa = aux_s + P.aux_flag_off + ((id0 >> 5) - fw) * 4u;
+                uint32_t flags = __funnelshift_r(lds32(fa), lds32(fa + 4u), id0 & 31u);   // bit r = flag of row id0 + r
                 if (cnt < 32u) flags &= (1u << cnt) - 1u;
                 decode_piece(id0, cnt, my_off, flags, base_off, stage_s, P.out + (uint64_t)(out0 + j0) * P.row_bytes, g0, aux_s + P.aux_meta_off);
             }
