@@ -316,7 +316,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
 // EVERYTHING a consumer warp reads comes out of shared memory.  The producer lane walks the chunks (the only place that reads
 // ids and row offsets from global memory) and loads UNITS: a unit is a chunk, or -- when the chunk's stored bytes exceed a stage,
 // which only happens with many raw rows -- one of its sub-ranges of split_rows rows.  For every unit it writes a 32-byte
-// descriptor {first row id, first output row, rows, offset of the first row, last-unit-of-the-chunk flag} into the stage and
+// descriptor {first row id, first output row, rows, offset of the first row, last-unit-of-the-chunk flag, last-unit-of-the-CTA flag} into the stage and
 // issues bulk copies of (1) the unit's packed bytes (contiguous: rows lie back to back), (2) the 16-byte cover of the unit's row
 // offsets, (3) the cover of its row-flag words and (4) Mask/Bitval of the table groups it touches (consecutive groups
 // are contiguous in GPU memory: "shared-memory staging of the metadata") -- all completing on the stage's full barrier.  The
@@ -423,7 +423,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
                 mbar_wait_backoff(empty_s + s * 8, ((k / NS) & 1u) ^ 1u);   // (a wait with a 20 us suspend hint reacts late and the refill starts late)
                 asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s), "r"((uint32_t)first), "r"((uint32_t)((uint64_t)first >> 32)),
                              "r"((uint32_t)(out0 + r0)), "r"((uint32_t)((uint64_t)(out0 + r0) >> 32)) : "memory");
-                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s + 16u), "r"(n), "r"(a0), "r"(r1 == nrows ? 1u : 0u), "r"(0u) : "memory");
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(aux_s + 16u), "r"(n), "r"(a0), "r"(r1 == nrows ? 1u : 0u),
+                             "r"(r1 == nrows && c + (int64_t)gridDim.x >= P.n_chunks ? 1u : 0u) : "memory");   // .w: the CTA's last unit
                 mbar_expect_tx(bar, bytes + off_bytes + flag_bytes + meta_bytes);     // release: the descriptor is visible to whoever sees the phase complete
                 bulk_g2s(aux_s + 32u, P.row_off + oi, off_bytes, bar);
                 bulk_g2s(aux_s + P.aux_flag_off, P.row_flag + fw, flag_bytes, bar);
@@ -649,13 +650,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
         }
     };
 
-    // this CTA's chunks blockIdx.x, blockIdx.x + gridDim.x, ...: only their number matters here (the descriptor names the rows); a
-    // 32-bit down-counter, because the 64-bit chunk index was spilled and its reload stalled every unit (ncu: 7 % of the samples)
-    uint32_t k = 0;
-    uint32_t left = (int64_t)blockIdx.x < P.n_chunks ? (uint32_t)((P.n_chunks - 1 - (int64_t)blockIdx.x) / (int64_t)gridDim.x) + 1u : 0u;
-    for (; left; --left) {
-        uint32_t last;
-        do {                                                                   // the units of the chunk, in the producer's order
+    // The consumers follow the producer's units until the descriptor says "last unit of this CTA": no chunk counter on this side
+    // (a 64-bit chunk index, then a 32-bit down-counter, were spilled under the 72-register budget, and the reload at the end of
+    // every unit was 4-7 % of the stall samples).
+    if ((int64_t)blockIdx.x >= P.n_chunks) return;
+    uint32_t k = 0, fin;
+    {
+        do {                                                                   // the CTA's units, in the producer's order
             const uint32_t s = k % NS, stage_s = smem_s + s * P.stage_bytes, aux_s = stage_s + data_cap;
             mbar_wait_relaxed(full_s + s * 8, (k / NS) & 1u);
             uint32_t d0[4], d1[4];
@@ -664,7 +665,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
             const uint32_t first = d0[0];                                    // (d0[1] = 0: below 2^32 rows)
             const int64_t out0 = (int64_t)(((uint64_t)d0[3] << 32) | d0[2]);
             const uint32_t n = d1[0], base_off = d1[1];
-            last = d1[2];
+            fin = d1[3];
             const uint32_t off_s = aux_s + 32u - (first & ~3u) * 4u;                    // shared address of row_off[0] (wraps mod 2^32: only differences matter)
             const uint32_t fw = (first >> 5) & ~3u;
             const uint32_t g0 = group_of(first);
@@ -680,6 +681,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 3) ibp_stream_t2_kernel(const S
             __syncwarp();
             if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_s + s * 8) : "memory");
             ++k;
-        } while (!last);
+        } while (!fin);
     }
 }
