@@ -533,6 +533,47 @@ def tiny_latency_breakdown(ctx, entry):
             "note": "a latency floor, not a kernel property: fetch engine, rows in flight, warps per CTA and store kind all give the same step time (DESIGN.md section 8)"}
 
 
+def resident_thresholded(ctx, name, thr, steps=20):
+    """ibp_decompress_resident of the first 2^20 rows of a workload's table built with tau = thr (the paper's codec): packed
+    bytes staged in HBM, every decoded byte checked against the original rows, L2 flushed between the timed launches."""
+    import oracle
+    torch = ctx.torch
+    ibp = ctx.ibp
+    w = make_workload(name)
+    nr = min(w.n_rows, 1 << 20) // w.group_param * w.group_param
+    Xb = w.rows(0, nr).view(np.uint8).reshape(nr, -1)
+    h = ibp.ibp_build(Xb, w.row_bytes, w.group_kind, w.group_param, align_bytes=w.align_bytes, threshold=thr, flags=ibp.IBP_FLAG_PAGEABLE_STORE).upload_metadata(ctx.local)
+    info = h.info()
+    stream = torch.cuda.current_stream().cuda_stream
+    ptr, nb = h.packed_range(0, nr)
+    staged = torch.from_numpy(h.packed_view(ptr, nb).copy()).cuda()
+    out = torch.empty((nr, w.row_bytes), dtype=torch.uint8, device="cuda")
+    step = lambda i: h.decompress_resident(staged.data_ptr(), 0, nr, out.data_ptr(), stream)
+    for i in range(3):
+        step(i)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    if not np.array_equal(got, Xb):
+        raise SystemExit(f"bench.py: thresholded resident decode of {name} differs from the original rows")
+    n_or = min(nr, 1 << 16) // w.group_param * w.group_param                            # the oracle's codec on the first 65,536 rows
+    ids = np.random.default_rng(0).choice(n_or, 64, replace=False)
+    ds = oracle.DatasetT(Xb[:n_or], w.group_kind, w.group_param, thr[0], thr[1])
+    ok = np.array_equal(got[ids], ds.gather_decompress(ids))
+    ds.close()
+    if not ok:
+        raise SystemExit(f"bench.py: thresholded resident decode of {name} differs from the oracle codec")
+    t = float(np.mean(ctx.timed_loop(step, steps, 0)))
+    ctx.launches += steps
+    alg = nb + nr * w.row_bytes + info.n_groups * 2 * w.row_bytes
+    e = {"workload": name, "rows": nr, "threshold": f"{thr[0]}/{thr[1]}", "ms": round(t, 4), "in_plus_out_GBps": round((nb + nr * w.row_bytes) / (t * 1e-3) * 1e-9, 1),
+         "bound": "hbm", "peak": ctx.hbm_peak, "frac": round(alg / (t * 1e-3) * 1e-9 / ctx.hbm_peak, 4), "algorithmic_bytes": int(alg),
+         "ratio_stored": round(nr * w.row_bytes / nb, 3), "rows_kept_raw": int(info.n_rows_raw), "kernel": "ibp_stream_t2_kernel (ibp_decompress_resident)",
+         "parity": "every byte == the original rows; 64 sampled rows == the oracle's thresholded codec"}
+    h.destroy()
+    del staged, out
+    return e
+
+
 def run_cuda(args):
     ctx = Ctx(args)
     torch, ibp = ctx.torch, ctx.ibp
@@ -556,6 +597,11 @@ def run_cuda(args):
                 if name == "tiny":
                     e["latency_breakdown"] = tiny_latency_breakdown(ctx, e)
             per_config.append(e)
+
+    # S8 under the paper's own codec (tau = 4/5): resident decode of the first 2^20 rows of the three row-shaped configs
+    resident_t = None
+    if per_config is not None and not args.no_resident:
+        resident_t = [resident_thresholded(ctx, name, (4, 5)) for name in ("gnn", "dlrm", "kv")]
 
     cpu = None
     if ctx.rank == 0 and world == 1 and not args.no_cpu:
@@ -606,6 +652,7 @@ def run_cuda(args):
             "gpu_launches": ctx.launches,
             "clocks": ex["clk"],
             "resident_decode": ex.get("resident"),
+            "resident_decode_thresholded": resident_t,
             "baseline_uncompressed": entry["baseline_uncompressed"],
             "per_config": per_config,
             "cpu_baseline": cpu,
