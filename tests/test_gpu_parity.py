@@ -513,6 +513,32 @@ def test_T_chunks_larger_than_a_stage(rb, G, n, raw_frac):
     hs.destroy()
 
 
+@pytest.mark.parametrize("rb,G,n", [(256, 16, 5000), (256, 128, 7001), (512, 256, 4099), (128, 64, 9000)])
+def test_T_stream_grid_limits(rb, G, n):
+    """The thresholded stream kernel's consumers follow the producer's units until the descriptor marks the CTA's last one:
+    one CTA walking every chunk, a few CTAs (more chunks than CTAs, uneven shares), the default grid; split units (raw rows) and a
+    ragged last piece included.  Ranges from the host store, resident decode, page spans."""
+    rng = np.random.default_rng(7 * rb + n)
+    X = _perturbed(n, rb, rb + n)
+    raw = (np.arange(n) >= n - n // 5) | (rng.random(n) < 0.05)               # a raw tail (its units are split) and scattered raw rows
+    X[raw] = rng.integers(0, 256, size=(int(raw.sum()), rb), dtype=np.uint8)
+    h = ibp.ibp_build(X, rb, 0, G, align_bytes=16, threshold=(4, 5)).upload_metadata(0)
+    for max_ctas in (1, 3, 0):
+        h.configure(max_ctas, 0)
+        assert np.array_equal(_resident(h, 0, n), X), f"resident, max_ctas={max_ctas}"
+        assert np.array_equal(_range(h, 0, n), X), f"range, max_ctas={max_ctas}"
+        assert np.array_equal(_resident(h, G, n - G - 1), X[G:n - 1]), f"resident off the end, max_ctas={max_ctas}"
+    h.destroy()
+    span = 2 * G
+    ns = n // span
+    hs = ibp.ibp_build(X[: ns * span], rb, 0, G, align_bytes=16, index_span=span, threshold=(4, 5)).upload_metadata(0)
+    sids = rng.integers(0, ns, 37)
+    for max_ctas in (1, 5, 0):
+        hs.configure(max_ctas, 0)
+        assert np.array_equal(_gather(hs, sids, span=span), oracle.gather_plain(X, sids, span)), f"spans, max_ctas={max_ctas}"
+    hs.destroy()
+
+
 def test_T_edge_cases_and_spans():
     rb = 256
     r = datagen.random_bytes(rb, 3)
