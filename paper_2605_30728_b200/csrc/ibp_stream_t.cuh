@@ -331,12 +331,17 @@ __global__ void __launch_bounds__((NW + 1) * 32, 2) ibp_stream_t_kernel(const St
 //   - a unit is NW pieces, one per consumer warp, so every warp works on every stage and the stages double-buffer;
 //   - raw rows take the SAME code with an empty header and no participating chunk (every chunk then contributes its 32
 //     bits at offset 32*c), so a pass never diverges on the row kind;
-//   - bits removed in front of each of the lane's 4 chunks come from ONE packed computation: popc(Mask) of the 4 chunks sit in
-//     the bytes of one register, the 4 participation bits are spread to byte masks by a multiply, and a multiply by 0x01010101
-//     gives the four running sums (P:319 step 2 for four chunks at once);
-//   - the exclusive scan over the lanes of a row (P:319 step 3) runs on two rows packed into one register (16 bits each: a row
-//     removes at most 4,096 bits), and RB = 2 passes are written out side by side, branch-free (the store is predicated), so
-//     that their dependency chains interleave;
+//   - the bits a lane's 4 chunks store (P:319 step 2) come from ONE dp4a: -popc(Mask) of the 4 chunks sit as signed bytes in one
+//     register, the 4 participation bits are spread to bytes by a multiply, and the dot product + 128 is the lane's total;
+//   - the inclusive scan over the lanes of a row (P:319 step 3) runs on two rows packed into one register (16 bits each: a row
+//     stores at most 4,096 bits), each step a shuffle whose in-range predicate guards the add, and RB = 2 passes are written out
+//     side by side, branch-free, so that their dependency chains interleave;
+//   - chunk q of a lane is read q words past (the lane's first bit - the bits removed in front of q): one predicated subtraction
+//     per chunk, the word offset an immediate of the shared-memory load;
+//   - the integer ALU pipe was the binding unit (ncu: 70 % busy at half rate with the FMA pipe at 19 %), so sums, scalings and
+//     flags are written as (predicated) IMAD work wherever arithmetic allows, and whole pieces take a pass body without the
+//     repeat / valid handling; row ids and group numbers are 32-bit here (the launcher takes this kernel below 2^32 rows), and
+//     the consumers carry no chunk counter: they follow the producer's units until the descriptor marks the CTA's last one;
 //   - NR (handle level: the most runs of variant bits in any Mask word of the table): bits go back run by run with exactly NR
 //     multiply + and-or pairs; NR = 0 selects the five-stage expand.
 __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
